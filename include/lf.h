@@ -1,0 +1,180 @@
+/*
+ * lf.h -- C ABI of the B200-native Looking Forward hot path (arxiv 2402.14670, section VI).
+ *
+ * One library, three calls on the hot path: lf_create / lf_run / lf_destroy (BASELINE.json
+ * north_star (a)).  For every upstream (VELO-UT) seed of every event in a
+ * batch the library follows the track through the magnet into the 12 SciFi layers:
+ *
+ *   a1 extrapolation with the pT-kick
+ *   a2 search windows per layer and zone          PAPER.md:165, 181-204 (Eq. 3, n_window cap)
+ *   a3 x-layer triplet seeding
+ *   a4 extension to the other three x layers      PAPER.md:227-232 (Eq. 4)
+ *   a5 u/v stereo matching + hit-count rule
+ *   a6 fit, quality factor Q, best per seed, q/p  PAPER.md:238-279 (Eq. 5, 6), 327-338 (Eq. 9)
+ *   a7 stream compaction into dense track lists   north_star (c)
+ *
+ * All of it runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.  The readings of
+ * the points the paper leaves open are listed in DESIGN.md ("Readings", C1..C22).
+ *
+ * Conventions
+ *   - Plain C99 types only.  No exceptions cross the ABI; every call returns an lf_status.
+ *   - Unless a function says HOST, every data pointer is a DEVICE pointer (cudaMalloc'd or a
+ *     torch CUDA tensor's data_ptr) owned by the caller; the library never frees or reallocates
+ *     caller memory.  The library owns only its workspace (allocated in lf_create, never on the
+ *     hot path) and its constant tables.
+ *   - Lengths in mm, momenta in GeV, q/p in 1/GeV.
+ *   - Layout (north_star (b)): hits are event-major, then layer 0..11, then zone 0 (y < 0) /
+ *     zone 1 (y >= 0); the 24 segments of one event are contiguous; inside each segment the stored
+ *     coordinate s = x + y*tan_alpha is ASCENDING (precondition, not checked).  Offsets are
+ *     monotone.  q/p is finite.
+ *   - Output order contract: tracks are ordered by (event, seed index); at most one per seed.
+ */
+#ifndef LF_H
+#define LF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LF_ABI_VERSION 1u
+#define LF_N_LAYERS 12   /* three T-stations, x-u-v-x each */
+#define LF_N_ZONES 2     /* lower / upper half */
+#define LF_MAX_WINDOW 32   /* largest params.n_window this build supports (one warp lane per hit) */
+#define LF_MAX_TRIPLETS 16 /* largest params.n_triplets this build supports */
+
+typedef struct lf_handle lf_handle; /* opaque; owned by the library */
+
+typedef enum {
+  LF_OK = 0,
+  LF_ERR_INVALID_ARG = 1, /* NULL pointer, inconsistent size, value out of the documented range */
+  LF_ERR_CUDA = 2,        /* a CUDA runtime call failed (no device, out of memory, launch error) */
+  LF_ERR_CAPACITY = 3,    /* batch larger than lf_create's maxima, or out->capacity < n_seeds */
+  LF_ERR_UNSUPPORTED = 4  /* valid request this build does not implement */
+} lf_status;
+
+/* Detector + field model (section V).  HOST struct, copied at lf_create. */
+typedef struct {
+  int32_t n_layers;              /* must be LF_N_LAYERS */
+  float z[LF_N_LAYERS];          /* layer z positions */
+  float tan_alpha[LF_N_LAYERS];  /* stereo: stored s = x + y*tan_alpha; must be 0 for layers 0,3 (mod 4),
+                                    non-zero for layers 1,2 (mod 4) */
+  float z_seed, z_mag, kick;     /* z of the seed state; magnet centre; delta tx = kick * q/p (Eq. 2) */
+  float z_ref, d_ratio;          /* Eq. (1)/(4): dz = z - z_ref (8520 mm); dRatio per mm */
+  float k_first, k_last;         /* sagitta factors K_x1 of the two layer sets */
+  float qop_poly[5];             /* Eq. (9): q/p = dSlope / sum_i qop_poly[i] * dSlope^i */
+  float x_half, y_half;          /* acceptance; used by generators only, ignored by the library */
+  float z_state;                 /* z at which the output state is evaluated */
+  int32_t polarity;              /* +1 = MU, -1 = MD; selects the asymmetric window edge (Eq. 3) */
+} lf_geometry;
+
+/* Tunables: Table 3 "Forward" column, Table 4 and the DESIGN.md readings.
+ * HOST struct, copied at lf_create. */
+typedef struct {
+  float T_triplet, T_x, T_uv_slope, T_uv_min, T_ty, T_y, T_Q; /* 8, 2, 50, 0.5, 0.02, 800, 0.5 */
+  float C_nhits[4];                                           /* C(n) for n = 9..12: 5, 1, 0.8, 0.5 */
+  int32_t n_window, n_triplets, min_hits;                     /* 32, 12, 9;  2 <= n_window <= LF_MAX_WINDOW,
+                                                                 1 <= n_triplets <= LF_MAX_TRIPLETS */
+  float xtol_base, xtol_inv_p, x_asym, uv_half_width;         /* 150, 2000, 100, 800 */
+  float p_same_bend, mag_tol_base, mag_tol_inv_p, mag_tol_tx, mag_tol_max; /* 5, 8, 60, 20, 40 */
+  int32_t hit_storage;                                        /* 0 = fp32; 1 = fp16 copy of the hits for windows +
+                                                                 seeding, fp32 extension and fit */
+} lf_params;
+
+/* Input seeds: upstream track states at z_seed, SoA, all events back to back. */
+typedef struct {
+  const float *x, *y, *tx, *ty, *qop; /* n_seeds each */
+  const uint32_t* event_offsets;      /* n_events + 1; seeds of event e are [off[e], off[e+1]) */
+  size_t n_seeds;                     /* == event_offsets[n_events] (caller's knowledge; no device read-back) */
+} lf_seeds;
+
+/* Input hits. */
+typedef struct {
+  const float* x;              /* n_hits stored coordinates */
+  const uint32_t* seg_offsets; /* n_events*24 + 1; segment index = event*24 + layer*2 + zone */
+  size_t n_hits;               /* == seg_offsets[n_events*24] */
+} lf_hits;
+
+/* Output tracks (dense, (event, seed) order).  Arrays must hold `capacity` rows;
+ * capacity >= seeds->n_seeds is required (at most one track per seed), so no
+ * overflow is possible and no host synchronisation is needed to size anything. */
+typedef struct {
+  int32_t* hit_idx;        /* capacity*12: global hit index used on each layer, or -1 */
+  int32_t* seed_idx;       /* capacity: global index of the seed the track extends */
+  int32_t* n_hits;         /* capacity: number of hits (>= params.min_hits) */
+  float* state;            /* capacity*5: x, y, tx, ty, q/p at geometry.z_state */
+  float* quality;          /* capacity: Q of Eq. (6) */
+  uint32_t* event_offsets; /* n_events + 1: tracks of event e are [off[e], off[e+1]) */
+  uint32_t* n_tracks;      /* 1: total number of tracks written */
+  size_t capacity;
+} lf_tracks;
+
+/* Optional stage-boundary outputs for parity tests (device pointers; any may be NULL).
+ * NT = params.n_triplets.  Indices are global hit indices; -1 = none. */
+typedef struct {
+  int32_t* win_first;   /* n_seeds*12: first hit of the (capped) search window (undefined if empty) */
+  int32_t* win_count;   /* n_seeds*12: hits in the window (<= n_window) */
+  int32_t* n_triplets;  /* n_seeds: triplets kept, ordered by (chi2, set, h0, h2) */
+  int32_t* trip_hits;   /* n_seeds*NT*3: h0, h1, h2 */
+  int32_t* trip_set;    /* n_seeds*NT: 0 = first x layers {0,4,8}, 1 = last x layers {3,7,11} */
+  float* trip_chi2;     /* n_seeds*NT */
+  int32_t* cand_hits;   /* n_seeds*NT*12: hit per layer after extension */
+  float* cand_quality;  /* n_seeds*NT: Q; -1 = failed the hit-count rule; -2 = failed the t_y cut */
+} lf_debug;
+
+/* What the library launches, for benchmarks and occupancy reports (HOST struct, filled by lf_get_info). */
+typedef struct {
+  int32_t kernels_per_run;       /* kernel launches one lf_run enqueues */
+  int32_t track_regs, track_block, track_grid, track_ctas_per_sm;
+  int32_t track_smem_bytes;      /* dynamic shared memory of the track kernel */
+  int32_t staged_hits_per_event; /* events with more hits than this read hits from global memory */
+  int32_t sm_count;
+  size_t workspace_bytes;
+} lf_info;
+
+/* Creates a context for batches of at most max_events / max_seeds / max_hits.  Validates geometry
+ * and params, uploads constants, allocates the workspace (max_seeds*88 + max_events*4 bytes on the
+ * current CUDA device).  *out is set only on LF_OK.  HOST pointers. */
+lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t max_events,
+                    size_t max_seeds, size_t max_hits, lf_handle** out);
+
+/* Enqueues the whole hot path (a1..a7) for n_events events on `cuda_stream` (a cudaStream_t; NULL =
+ * the legacy default stream).  Asynchronous: performs no host synchronisation and returns after the
+ * launches; results are valid once the caller has synchronised the stream.  `seeds`, `hits`, `out`
+ * are HOST structs holding DEVICE pointers.  Safe to call repeatedly; calls on one handle must not
+ * overlap in time (they share the workspace).  n_events == 0 is valid (writes n_tracks = 0).
+ * Errors are detected before any launch: LF_ERR_INVALID_ARG (NULL pointer), LF_ERR_CAPACITY. */
+lf_status lf_run(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events,
+                 lf_tracks* out, void* cuda_stream);
+
+/* lf_run that also writes the stage-boundary tables of `debug` (slower; for tests). */
+lf_status lf_run_debug(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events,
+                       lf_tracks* out, const lf_debug* debug, void* cuda_stream);
+
+/* End-to-end variant: every pointer inside `seeds`, `hits`, `out` is a HOST pointer (pinned memory
+ * makes the copies asynchronous).  Copies the inputs to library-owned device buffers (allocated on
+ * first use, sized by lf_create's maxima), runs lf_run, copies the tracks back, and returns after
+ * synchronising `cuda_stream`: on LF_OK the host arrays hold the results. */
+lf_status lf_run_host(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events,
+                      lf_tracks* out, void* cuda_stream);
+
+/* Frees the workspace and the handle.  NULL is allowed. */
+lf_status lf_destroy(lf_handle* h);
+
+/* Message of the last error on this handle ("" if none); valid until the next call on the handle.
+ * With h == NULL: message of the last failed lf_create in this thread. */
+const char* lf_last_error(const lf_handle* h);
+
+lf_status lf_get_info(const lf_handle* h, lf_info* out);
+
+/* ABI self-description for bindings: version and struct sizes
+ * (which: 0 geometry, 1 params, 2 seeds, 3 hits, 4 tracks, 5 debug, 6 info). */
+uint32_t lf_abi_version(void);
+size_t lf_sizeof(int which);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LF_H */

@@ -1,0 +1,371 @@
+/*
+ * lf_api.cu -- C-ABI entry points of include/lf.h: handle management, host-side constants,
+ * launch sequence.  No torch types; the caller's framework only supplies device memory and a stream.
+ */
+#include "../../include/lf.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "lf_kernels.cuh"
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct HostBufs { /* device staging for lf_run_host */
+  float* seeds = nullptr;      /* 5 * max_seeds */
+  uint32_t* seed_off = nullptr;
+  float* hits = nullptr;
+  uint32_t* seg_off = nullptr;
+  int32_t *hit_idx = nullptr, *seed_idx = nullptr, *n_hits = nullptr;
+  float *state = nullptr, *quality = nullptr;
+  uint32_t *ev_off = nullptr, *n_tracks = nullptr;
+  uint32_t* pinned_count = nullptr; /* host, pinned */
+  bool ready = false;
+};
+
+} // namespace
+
+struct lf_handle {
+  lf::Consts C;
+  lf_geometry G;
+  lf_params P;
+  size_t max_events, max_seeds, max_hits;
+  int device;
+  int sm_count, ctas_per_sm, grid, regs;
+  int smem_bytes, stage_cap;
+  /* workspace */
+  int32_t *ws_rec, *ws_nh, *ws_rank, *ws_event;
+  uint32_t *ev_count, *ev_off, *ticket;
+  size_t workspace_bytes;
+  HostBufs hb;
+  std::string err;
+};
+
+namespace {
+
+lf_status fail(lf_handle* h, lf_status st, const std::string& msg) {
+  if (h) h->err = msg; else g_create_error = msg;
+  return st;
+}
+
+#define LF_CUDA(h, call)                                                                              \
+  do {                                                                                                \
+    cudaError_t e_ = (call);                                                                          \
+    if (e_ != cudaSuccess)                                                                            \
+      return fail((h), LF_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_));              \
+  } while (0)
+
+bool uv_layer(int l) { return (l & 3) == 1 || (l & 3) == 2; }
+
+/* Host-side constants in fp32, one rounding per operation.
+ * Built with -ffp-contract=off; volatile stores keep every intermediate a genuine float. */
+void make_consts(const lf_geometry& G, const lf_params& P, lf::Consts& c) {
+  std::memset(&c, 0, sizeof(c));
+  const float one = 1.0f, milli = 0.001f;
+  c.z_seed = G.z_seed; c.z_mag = G.z_mag; c.kick = G.kick;
+  c.dr = G.d_ratio * 1000.0f;
+  c.K[0] = G.k_first; c.K[1] = G.k_last;
+  for (int i = 0; i < 5; ++i) c.poly[i] = G.qop_poly[i];
+  c.polarity = G.polarity;
+  c.mag_dz_seed = c.z_mag - c.z_seed;
+  for (int l = 0; l < lf::NL; ++l) {
+    c.z[l] = G.z[l];
+    c.tana[l] = G.tan_alpha[l];
+    c.inv_tan[l] = uv_layer(l) ? one / c.tana[l] : 0.0f;
+    c.dzs[l] = c.z[l] - c.z_seed;
+    c.dzm[l] = c.z[l] - c.z_mag;
+    const float dz = c.z[l] - G.z_ref;
+    c.d[l] = dz * milli;
+    const float dd = c.d[l] * c.d[l];
+    const float curv = one + c.dr * c.d[l];
+    c.w[l] = dd * curv;
+  }
+  for (int s = 0; s < 2; ++s) {
+    const int a = s ? 3 : 0, b = a + 4, cc = a + 8;
+    c.inv_dz_ac[s] = one / (c.z[cc] - c.z[a]);
+    c.zmag_a[s] = c.z_mag - c.z[a];
+    c.D10[s] = c.d[b] - c.d[a];
+    c.D20[s] = c.d[cc] - c.d[a];
+    c.W10[s] = c.w[b] - c.w[a];
+    c.W20[s] = c.w[cc] - c.w[a];
+    const float p1 = c.W20[s] * c.D10[s];
+    const float p2 = c.W10[s] * c.D20[s];
+    c.inv_det[s] = one / (p1 - p2);
+    c.inv_D10[s] = one / c.D10[s];
+  }
+  c.dz_state = G.z_state - c.z_seed;
+  const float dzst = G.z_state - G.z_ref;
+  c.ds = dzst * milli;
+  const float ds2 = c.ds * c.ds;
+  const float curv_s = one + c.dr * c.ds;
+  c.ws = ds2 * curv_s;
+  const float two_ds = 2.0f * c.ds;
+  const float three_dr = 3.0f * c.dr;
+  c.dws = two_ds + three_dr * ds2;
+  c.T_triplet = P.T_triplet; c.T_x = P.T_x; c.T_uv_slope = P.T_uv_slope; c.T_uv_min = P.T_uv_min;
+  c.T_ty = P.T_ty; c.inv_Tx = one / P.T_x; c.inv_Ty = one / P.T_y; c.T_Q = P.T_Q;
+  for (int i = 0; i < 4; ++i) c.C_nhits[i] = P.C_nhits[i];
+  c.n_window = P.n_window; c.n_triplets = P.n_triplets; c.min_hits = P.min_hits;
+  c.xtol_base = P.xtol_base; c.xtol_inv_p = P.xtol_inv_p; c.x_asym = P.x_asym; c.uv_half_width = P.uv_half_width;
+  c.p_same_bend = P.p_same_bend; c.mag_tol_base = P.mag_tol_base; c.mag_tol_inv_p = P.mag_tol_inv_p;
+  c.mag_tol_tx = P.mag_tol_tx; c.mag_tol_max = P.mag_tol_max;
+}
+
+const char* validate(const lf_geometry& G, const lf_params& P) {
+  if (G.n_layers != LF_N_LAYERS) return "geometry.n_layers must be 12";
+  for (int l = 0; l < LF_N_LAYERS; ++l) {
+    if (!std::isfinite(G.z[l]) || !std::isfinite(G.tan_alpha[l])) return "geometry: non-finite layer constant";
+    if (l > 0 && !(G.z[l] > G.z[l - 1])) return "geometry.z must be strictly ascending";
+    if (uv_layer(l) ? (G.tan_alpha[l] == 0.0f) : (G.tan_alpha[l] != 0.0f))
+      return "geometry.tan_alpha must be 0 on x layers (0,3 mod 4) and non-zero on u/v layers (1,2 mod 4)";
+  }
+  if (!(G.z_mag > G.z_seed) || !(G.z[0] > G.z_mag)) return "geometry: need z_seed < z_mag < z[0]";
+  if (G.polarity != 1 && G.polarity != -1) return "geometry.polarity must be +1 or -1";
+  if (P.n_window < 2 || P.n_window > LF_MAX_WINDOW) return "params.n_window out of [2, LF_MAX_WINDOW]";
+  if (P.n_triplets < 1 || P.n_triplets > LF_MAX_TRIPLETS) return "params.n_triplets out of [1, LF_MAX_TRIPLETS]";
+  if (P.min_hits < 4 || P.min_hits > 12) return "params.min_hits out of [4, 12]";
+  if (!(P.T_triplet > 0) || !(P.T_x > 0) || !(P.T_y > 0) || !(P.T_uv_min > 0) || !(P.T_Q > 0) || !(P.T_ty > 0))
+    return "params: tolerances must be positive";
+  if (P.hit_storage != 0 && P.hit_storage != 1) return "params.hit_storage must be 0 or 1";
+  return nullptr;
+}
+
+template <bool DEBUG>
+lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
+                 const lf_debug* dbg, cudaStream_t st) {
+  if (n_events > 0) {
+    lf::TrackArgs A;
+    std::memset(&A, 0, sizeof(A));
+    A.sx = seeds->x; A.sy = seeds->y; A.stx = seeds->tx; A.sty = seeds->ty; A.sqop = seeds->qop;
+    A.seed_off = seeds->event_offsets;
+    A.hx = hits->x; A.seg_off = hits->seg_offsets;
+    A.n_events = (uint32_t)n_events;
+    A.ws_rec = h->ws_rec; A.ws_nh = h->ws_nh; A.ws_rank = h->ws_rank; A.ws_event = h->ws_event;
+    A.ev_count = h->ev_count; A.ticket = h->ticket;
+    A.stage_cap = h->stage_cap;
+    if (dbg) {
+      A.dbg.win_first = dbg->win_first; A.dbg.win_count = dbg->win_count; A.dbg.n_triplets = dbg->n_triplets;
+      A.dbg.trip_hits = dbg->trip_hits; A.dbg.trip_set = dbg->trip_set; A.dbg.trip_chi2 = dbg->trip_chi2;
+      A.dbg.cand_hits = dbg->cand_hits; A.dbg.cand_quality = dbg->cand_quality;
+    }
+    const int grid = (int)std::min<size_t>((size_t)h->grid, n_events);
+    lf::lf_track_kernel<DEBUG><<<grid, lf::CTA_THREADS, h->smem_bytes, st>>>(h->C, A);
+  }
+  lf::lf_scan_kernel<<<1, 1024, 0, st>>>(h->ev_count, (uint32_t)n_events, h->ev_off, out->event_offsets,
+                                         out->n_tracks, h->ticket);
+  if (n_events > 0 && seeds->n_seeds > 0) {
+    const size_t total = seeds->n_seeds * lf::REC_WORDS;
+    const unsigned blocks = (unsigned)((total + 255) / 256);
+    lf::lf_compact_kernel<<<blocks, 256, 0, st>>>(h->ws_rec, h->ws_rank, h->ws_event, h->ev_off, seeds->n_seeds,
+                                                  out->hit_idx, out->seed_idx, out->n_hits, out->state, out->quality);
+  }
+  LF_CUDA(h, cudaGetLastError());
+  return LF_OK;
+}
+
+lf_status check_run_args(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out) {
+  if (!h) return LF_ERR_INVALID_ARG;
+  if (!seeds || !hits || !out) return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL seeds/hits/out");
+  if (!seeds->event_offsets || !hits->seg_offsets || !out->event_offsets || !out->n_tracks)
+    return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL offset table or n_tracks pointer");
+  if (seeds->n_seeds > 0 && (!seeds->x || !seeds->y || !seeds->tx || !seeds->ty || !seeds->qop))
+    return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL seed array");
+  if (hits->n_hits > 0 && !hits->x) return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL hit array");
+  if (seeds->n_seeds > 0 && (!out->hit_idx || !out->seed_idx || !out->n_hits || !out->state || !out->quality))
+    return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL output array");
+  if (n_events == 0 && (seeds->n_seeds != 0 || hits->n_hits != 0))
+    return fail(h, LF_ERR_INVALID_ARG, "lf_run: n_events == 0 with non-empty seeds or hits");
+  if (n_events > h->max_events || seeds->n_seeds > h->max_seeds || hits->n_hits > h->max_hits)
+    return fail(h, LF_ERR_CAPACITY, "lf_run: batch exceeds the maxima given to lf_create");
+  if (hits->n_hits >= (size_t)0x7fffffff) return fail(h, LF_ERR_CAPACITY, "lf_run: hit indices must fit int32");
+  if (out->capacity < seeds->n_seeds)
+    return fail(h, LF_ERR_CAPACITY, "lf_run: out->capacity must be >= seeds->n_seeds");
+  return LF_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+uint32_t lf_abi_version(void) { return LF_ABI_VERSION; }
+
+size_t lf_sizeof(int which) {
+  switch (which) {
+    case 0: return sizeof(lf_geometry);
+    case 1: return sizeof(lf_params);
+    case 2: return sizeof(lf_seeds);
+    case 3: return sizeof(lf_hits);
+    case 4: return sizeof(lf_tracks);
+    case 5: return sizeof(lf_debug);
+    case 6: return sizeof(lf_info);
+    default: return 0;
+  }
+}
+
+const char* lf_last_error(const lf_handle* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t max_events, size_t max_seeds,
+                    size_t max_hits, lf_handle** out) {
+  if (!geometry || !params || !out) return fail(nullptr, LF_ERR_INVALID_ARG, "lf_create: NULL argument");
+  *out = nullptr;
+  if (const char* why = validate(*geometry, *params)) return fail(nullptr, LF_ERR_INVALID_ARG, std::string("lf_create: ") + why);
+  if (max_hits >= (size_t)0x7fffffff || max_seeds >= (size_t)0x7fffffff || max_events >= (size_t)0x7fffffff / LF_N_LAYERS / 2)
+    return fail(nullptr, LF_ERR_CAPACITY, "lf_create: maxima must fit 32-bit indices");
+  if (params->hit_storage == 1)
+    return fail(nullptr, LF_ERR_UNSUPPORTED, "lf_create: hit_storage = 1 (fp16) is not implemented in this build");
+
+  lf_handle* h = new (std::nothrow) lf_handle();
+  if (!h) return fail(nullptr, LF_ERR_CUDA, "lf_create: out of host memory");
+  h->G = *geometry; h->P = *params;
+  h->max_events = max_events; h->max_seeds = max_seeds; h->max_hits = max_hits;
+  make_consts(*geometry, *params, h->C);
+
+  auto bail = [&](lf_status st, const std::string& msg) { g_create_error = msg; lf_destroy(h); return st; };
+#define LF_CREATE_CUDA(call)                                                                     \
+  do {                                                                                           \
+    cudaError_t e_ = (call);                                                                     \
+    if (e_ != cudaSuccess) return bail(LF_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
+  } while (0)
+
+  LF_CREATE_CUDA(cudaGetDevice(&h->device));
+  cudaDeviceProp prop;
+  LF_CREATE_CUDA(cudaGetDeviceProperties(&prop, h->device));
+  h->sm_count = prop.multiProcessorCount;
+  if (prop.major < 10) return bail(LF_ERR_UNSUPPORTED, "lf_create: this library is built for sm_100a (Blackwell) only");
+
+  /* shared memory: fixed part + one event's hits.  16384 hits (64 KB) covers BASELINE.json's
+   * stress config (about 13.5k hits in the largest event); larger events read global memory. */
+  const size_t fixed = (sizeof(lf::CtaShared) + 15) & ~size_t(15);
+  h->stage_cap = 16384;
+  h->smem_bytes = (int)(fixed + (size_t)h->stage_cap * sizeof(float));
+  LF_CREATE_CUDA(cudaFuncSetAttribute(lf::lf_track_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_bytes));
+  LF_CREATE_CUDA(cudaFuncSetAttribute(lf::lf_track_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_bytes));
+  LF_CREATE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->ctas_per_sm, lf::lf_track_kernel<false>,
+                                                               lf::CTA_THREADS, h->smem_bytes));
+  if (h->ctas_per_sm < 1) return bail(LF_ERR_CUDA, "lf_create: track kernel does not fit on an SM");
+  h->grid = h->sm_count * h->ctas_per_sm;
+  cudaFuncAttributes fa;
+  LF_CREATE_CUDA(cudaFuncGetAttributes(&fa, lf::lf_track_kernel<false>));
+  h->regs = fa.numRegs;
+
+  const size_t ns = std::max<size_t>(max_seeds, 1), ne = std::max<size_t>(max_events, 1);
+  LF_CREATE_CUDA(cudaMalloc(&h->ws_rec, ns * lf::REC_WORDS * sizeof(int32_t)));
+  LF_CREATE_CUDA(cudaMalloc(&h->ws_nh, ns * sizeof(int32_t)));
+  LF_CREATE_CUDA(cudaMalloc(&h->ws_rank, ns * sizeof(int32_t)));
+  LF_CREATE_CUDA(cudaMalloc(&h->ws_event, ns * sizeof(int32_t)));
+  LF_CREATE_CUDA(cudaMalloc(&h->ev_count, ne * sizeof(uint32_t)));
+  LF_CREATE_CUDA(cudaMalloc(&h->ev_off, (ne + 1) * sizeof(uint32_t)));
+  LF_CREATE_CUDA(cudaMalloc(&h->ticket, sizeof(uint32_t)));
+  LF_CREATE_CUDA(cudaMemset(h->ticket, 0, sizeof(uint32_t)));
+  h->workspace_bytes = ns * (lf::REC_WORDS + 3) * sizeof(int32_t) + (2 * ne + 2) * sizeof(uint32_t);
+#undef LF_CREATE_CUDA
+  *out = h;
+  return LF_OK;
+}
+
+lf_status lf_destroy(lf_handle* h) {
+  if (!h) return LF_OK;
+  cudaFree(h->ws_rec); cudaFree(h->ws_nh); cudaFree(h->ws_rank); cudaFree(h->ws_event);
+  cudaFree(h->ev_count); cudaFree(h->ev_off); cudaFree(h->ticket);
+  HostBufs& b = h->hb;
+  cudaFree(b.seeds); cudaFree(b.seed_off); cudaFree(b.hits); cudaFree(b.seg_off);
+  cudaFree(b.hit_idx); cudaFree(b.seed_idx); cudaFree(b.n_hits); cudaFree(b.state); cudaFree(b.quality);
+  cudaFree(b.ev_off); cudaFree(b.n_tracks);
+  if (b.pinned_count) cudaFreeHost(b.pinned_count);
+  delete h;
+  return LF_OK;
+}
+
+lf_status lf_get_info(const lf_handle* h, lf_info* out) {
+  if (!h || !out) return LF_ERR_INVALID_ARG;
+  out->kernels_per_run = 3;
+  out->track_regs = h->regs;
+  out->track_block = lf::CTA_THREADS;
+  out->track_grid = h->grid;
+  out->track_ctas_per_sm = h->ctas_per_sm;
+  out->track_smem_bytes = h->smem_bytes;
+  out->staged_hits_per_event = h->stage_cap - 4;
+  out->sm_count = h->sm_count;
+  out->workspace_bytes = h->workspace_bytes;
+  return LF_OK;
+}
+
+lf_status lf_run(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
+                 void* cuda_stream) {
+  const lf_status st = check_run_args(h, seeds, hits, n_events, out);
+  if (st != LF_OK) return st;
+  h->err.clear();
+  return launch<false>(h, seeds, hits, n_events, out, nullptr, (cudaStream_t)cuda_stream);
+}
+
+lf_status lf_run_debug(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
+                       const lf_debug* debug, void* cuda_stream) {
+  const lf_status st = check_run_args(h, seeds, hits, n_events, out);
+  if (st != LF_OK) return st;
+  if (!debug) return fail(h, LF_ERR_INVALID_ARG, "lf_run_debug: NULL debug");
+  h->err.clear();
+  return launch<true>(h, seeds, hits, n_events, out, debug, (cudaStream_t)cuda_stream);
+}
+
+lf_status lf_run_host(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
+                      void* cuda_stream) {
+  const lf_status st0 = check_run_args(h, seeds, hits, n_events, out);
+  if (st0 != LF_OK) return st0;
+  h->err.clear();
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  HostBufs& b = h->hb;
+  if (!b.ready) {
+    const size_t ns = std::max<size_t>(h->max_seeds, 1), ne = std::max<size_t>(h->max_events, 1);
+    const size_t nh = std::max<size_t>(h->max_hits, 1);
+    LF_CUDA(h, cudaMalloc(&b.seeds, 5 * ns * sizeof(float)));
+    LF_CUDA(h, cudaMalloc(&b.seed_off, (ne + 1) * sizeof(uint32_t)));
+    LF_CUDA(h, cudaMalloc(&b.hits, nh * sizeof(float)));
+    LF_CUDA(h, cudaMalloc(&b.seg_off, (ne * lf::NSEG + 1) * sizeof(uint32_t)));
+    LF_CUDA(h, cudaMalloc(&b.hit_idx, ns * lf::NL * sizeof(int32_t)));
+    LF_CUDA(h, cudaMalloc(&b.seed_idx, ns * sizeof(int32_t)));
+    LF_CUDA(h, cudaMalloc(&b.n_hits, ns * sizeof(int32_t)));
+    LF_CUDA(h, cudaMalloc(&b.state, ns * 5 * sizeof(float)));
+    LF_CUDA(h, cudaMalloc(&b.quality, ns * sizeof(float)));
+    LF_CUDA(h, cudaMalloc(&b.ev_off, (ne + 1) * sizeof(uint32_t)));
+    LF_CUDA(h, cudaMalloc(&b.n_tracks, sizeof(uint32_t)));
+    LF_CUDA(h, cudaMallocHost(&b.pinned_count, sizeof(uint32_t)));
+    b.ready = true;
+  }
+  const size_t ns = seeds->n_seeds, nh = hits->n_hits;
+  const size_t stride = std::max<size_t>(h->max_seeds, 1);
+  const float* src[5] = {seeds->x, seeds->y, seeds->tx, seeds->ty, seeds->qop};
+  for (int i = 0; i < 5 && ns > 0; ++i)
+    LF_CUDA(h, cudaMemcpyAsync(b.seeds + i * stride, src[i], ns * sizeof(float), cudaMemcpyHostToDevice, st));
+  LF_CUDA(h, cudaMemcpyAsync(b.seed_off, seeds->event_offsets, (n_events + 1) * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
+  if (nh > 0) LF_CUDA(h, cudaMemcpyAsync(b.hits, hits->x, nh * sizeof(float), cudaMemcpyHostToDevice, st));
+  LF_CUDA(h, cudaMemcpyAsync(b.seg_off, hits->seg_offsets, (n_events * lf::NSEG + 1) * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
+  lf_seeds ds = {b.seeds, b.seeds + stride, b.seeds + 2 * stride, b.seeds + 3 * stride, b.seeds + 4 * stride, b.seed_off, ns};
+  lf_hits dh = {b.hits, b.seg_off, nh};
+  lf_tracks dt = {b.hit_idx, b.seed_idx, b.n_hits, b.state, b.quality, b.ev_off, b.n_tracks, stride};
+  const lf_status rs = launch<false>(h, &ds, &dh, n_events, &dt, nullptr, st);
+  if (rs != LF_OK) return rs;
+  LF_CUDA(h, cudaMemcpyAsync(b.pinned_count, b.n_tracks, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+  LF_CUDA(h, cudaMemcpyAsync(out->event_offsets, b.ev_off, (n_events + 1) * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+  LF_CUDA(h, cudaStreamSynchronize(st));
+  const size_t nt = *b.pinned_count;
+  *out->n_tracks = (uint32_t)nt;
+  if (nt > 0) {
+    LF_CUDA(h, cudaMemcpyAsync(out->hit_idx, b.hit_idx, nt * lf::NL * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    LF_CUDA(h, cudaMemcpyAsync(out->seed_idx, b.seed_idx, nt * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    LF_CUDA(h, cudaMemcpyAsync(out->n_hits, b.n_hits, nt * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    LF_CUDA(h, cudaMemcpyAsync(out->state, b.state, nt * 5 * sizeof(float), cudaMemcpyDeviceToHost, st));
+    LF_CUDA(h, cudaMemcpyAsync(out->quality, b.quality, nt * sizeof(float), cudaMemcpyDeviceToHost, st));
+    LF_CUDA(h, cudaStreamSynchronize(st));
+  }
+  return LF_OK;
+}
+
+} /* extern "C" */

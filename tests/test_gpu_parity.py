@@ -1,0 +1,201 @@
+"""GPU parity: the CUDA path through the C ABI vs the CPU oracle, element by element (-m gpu)."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2402_14670_b200 import datagen as dg
+
+from parity import assert_debug_equal, assert_tracks_equal
+
+pytestmark = pytest.mark.gpu
+NTHREADS = max(1, (os.cpu_count() or 1))
+
+
+@pytest.fixture(scope="module")
+def lfmod():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2402_14670_b200 import build as cuda_build
+    cuda_build.build()
+    from paper_2402_14670_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def _gpu_run(binding, G, P, b, debug=False):
+    import torch
+    lf = binding.LookingForward(G, P, max(b.n_events, 1), max(b.n_seeds, 1), max(b.n_hits, 1))
+    out = lf.run(binding.DeviceBatch(b), debug=debug)
+    torch.cuda.synchronize()
+    got = out.to_numpy()
+    if debug:
+        got.debug = {k: v.cpu().numpy() for k, v in vars(out.debug_tensors).items()}
+    lf.close()
+    return got
+
+
+def test_config0_tracks_and_stage_boundaries(lfmod, oracle, geometry, params):
+    b = dg.generate_config(0)
+    ref = oracle.run(geometry, params, b, debug=True)
+    got = _gpu_run(lfmod, geometry, params, b, debug=True)
+    assert_debug_equal(got.debug, ref.debug)
+    info = assert_tracks_equal(got, ref, "config 0")
+    assert ref.n_tracks > 150
+    # the non-debug kernel gives the same result
+    got2 = _gpu_run(lfmod, geometry, params, b)
+    assert_tracks_equal(got2, ref, "config 0 (release kernel)")
+    print("config0", info)
+
+
+def test_dense_events_stage_boundaries(lfmod, oracle, geometry, params):
+    """Window cap and top-n cut bind; both polarities; non-default tunables."""
+    cfg = dg.GenConfig("dense", 6, 77, true_fixed=40, fake_mean=8.0, noise_fixed=600, p_min=1.5, smear=0.2)
+    b = dg.generate(cfg)
+    for G, P in ((geometry, params), (dict(geometry, polarity=-1), params),
+                 (dict(geometry, d_ratio=-2.0e-5), dict(params, n_window=9, n_triplets=5, T_x=1.0, T_triplet=4.0)),
+                 (geometry, dict(params, n_window=32, n_triplets=16, T_triplet=30.0, min_hits=8))):
+        ref = oracle.run(G, P, b, debug=True)
+        got = _gpu_run(lfmod, G, P, b, debug=True)
+        assert_debug_equal(got.debug, ref.debug)
+        assert_tracks_equal(got, ref, "dense")
+    assert (ref.debug.n_triplets == 16).sum() > 10
+
+
+def test_config1_full(lfmod, oracle, geometry, params):
+    b = dg.generate_config(1)
+    ref = oracle.run(geometry, params, b, threads=NTHREADS)
+    got = _gpu_run(lfmod, geometry, params, b)
+    print("config1", assert_tracks_equal(got, ref, "config 1"), ref.n_tracks)
+
+
+def test_config1_stage_boundaries_subset(lfmod, oracle, geometry, params):
+    b = dg.generate_config(1, n_events=100)
+    ref = oracle.run(geometry, params, b, debug=True, threads=NTHREADS)
+    got = _gpu_run(lfmod, geometry, params, b, debug=True)
+    assert_debug_equal(got.debug, ref.debug)
+    assert_tracks_equal(got, ref, "config 1 subset")
+
+
+def test_config4_full(lfmod, oracle, geometry, params):
+    b = dg.generate_config(4)
+    ref = oracle.run(geometry, params, b, threads=NTHREADS)
+    got = _gpu_run(lfmod, geometry, params, b)
+    print("config4", assert_tracks_equal(got, ref, "config 4"), ref.n_tracks)
+
+
+def test_config3_full_size(lfmod, oracle, geometry, params):
+    """BASELINE.json configs[3]: 20,000 events in one lf_run, the launch configuration bench.py times."""
+    b = dg.generate_config(3)
+    got = _gpu_run(lfmod, geometry, params, b)
+    ref = oracle.run(geometry, params, b, threads=NTHREADS)
+    print("config3", assert_tracks_equal(got, ref, "config 3"), ref.n_tracks)
+
+
+def test_deterministic(lfmod, geometry, params):
+    b = dg.generate_config(1, n_events=300)
+    a = _gpu_run(lfmod, geometry, params, b)
+    c = _gpu_run(lfmod, geometry, params, b)
+    for k in ("hit_idx", "seed_idx", "n_hits", "event_offsets"):
+        assert np.array_equal(getattr(a, k), getattr(c, k))
+    assert np.array_equal(a.state.view(np.uint32), c.state.view(np.uint32))
+    assert np.array_equal(a.quality.view(np.uint32), c.quality.view(np.uint32))
+
+
+def test_edge_cases(lfmod, oracle, geometry, params):
+    import torch
+    # zero events
+    empty = dg.generate(dg.GenConfig("e", 0, 1))
+    got = _gpu_run(lfmod, geometry, params, empty)
+    assert got.n_tracks == 0 and got.event_offsets.tolist() == [0]
+    # events without seeds; events without hits; a mix of empty and full events
+    noseed = dg.generate(dg.GenConfig("ns", 3, 2, true_fixed=0, noise_fixed=50))
+    got = _gpu_run(lfmod, geometry, params, noseed)
+    assert got.n_tracks == 0 and got.event_offsets.tolist() == [0, 0, 0, 0]
+    b = dg.generate_config(0)
+    nohits = dg.Batch(**{**b.__dict__, "hit_x": np.zeros(0, np.float32),
+                        "seg_offsets": np.zeros(b.n_events * 24 + 1, np.uint32), "hit_track": np.zeros(0, np.int32)})
+    got = _gpu_run(lfmod, geometry, params, nohits)
+    assert got.n_tracks == 0
+    # one hit per segment, duplicates of one x value in every segment
+    one = dg.Batch(**{**b.__dict__})
+    one.hit_x = np.full(b.n_events * 24 * 3, 12.5, np.float32)
+    one.seg_offsets = (np.arange(b.n_events * 24 + 1) * 3).astype(np.uint32)
+    one.hit_track = np.full(one.hit_x.shape[0], -1, np.int32)
+    ref = oracle.run(geometry, params, one, debug=True)
+    got = _gpu_run(lfmod, geometry, params, one, debug=True)
+    assert_debug_equal(got.debug, ref.debug)
+    assert_tracks_equal(got, ref, "duplicates")
+
+
+def test_unaligned_event_starts_and_misaligned_base(lfmod, oracle, geometry, params):
+    """Event hit blocks start at arbitrary 4-byte offsets; also a hit array whose base is not 16-byte aligned."""
+    import torch
+    b = dg.generate_config(1, n_events=40)
+    ref = oracle.run(geometry, params, b)
+    lf = lfmod.LookingForward(geometry, params, b.n_events, b.n_seeds, b.n_hits + 8)
+    for shift in (0, 1, 2, 3):
+        db = lfmod.DeviceBatch(b)
+        big = torch.zeros(b.n_hits + 8, dtype=torch.float32, device=db.device)
+        big[shift:shift + b.n_hits] = db.hit_x
+        db.hit_x = big[shift:shift + b.n_hits]
+        out = lf.run(db)
+        torch.cuda.synchronize()
+        assert_tracks_equal(out.to_numpy(), ref, f"base shift {shift}")
+    lf.close()
+
+
+def test_event_larger_than_stage_buffer(lfmod, oracle, geometry, params):
+    """An event with more hits than the shared-memory stage holds takes the global-memory path."""
+    cfg = dg.GenConfig("huge", 3, 9, true_fixed=60, fake_mean=5.0, noise_fixed=1700)
+    b = dg.generate(cfg)
+    import torch
+    lf = lfmod.LookingForward(geometry, params, b.n_events, b.n_seeds, b.n_hits)
+    assert b.n_hits / b.n_events > lf.info().staged_hits_per_event
+    out = lf.run(lfmod.DeviceBatch(b), debug=True)
+    torch.cuda.synchronize()
+    got = out.to_numpy()
+    got.debug = {k: v.cpu().numpy() for k, v in vars(out.debug_tensors).items()}
+    ref = oracle.run(geometry, params, b, debug=True)
+    assert_debug_equal(got.debug, ref.debug)
+    assert_tracks_equal(got, ref, "huge events")
+    lf.close()
+
+
+def test_run_host_matches_device_path(lfmod, oracle, geometry, params):
+    b = dg.generate_config(1, n_events=200)
+    ref = oracle.run(geometry, params, b, threads=NTHREADS)
+    lf = lfmod.LookingForward(geometry, params, b.n_events, b.n_seeds, b.n_hits)
+    hb = lfmod.HostBatch(b)
+    ht = lfmod.HostTracks(b.n_seeds, b.n_events)
+    for _ in range(2):
+        n = lf.run_host(hb, ht)
+        assert n == ref.n_tracks
+        assert_tracks_equal(ht.to_numpy(), ref, "host path")
+    lf.close()
+
+
+def test_repeated_runs_and_capacity_errors(lfmod, geometry, params):
+    import torch
+    b = dg.generate_config(1, n_events=50)
+    lf = lfmod.LookingForward(geometry, params, b.n_events, b.n_seeds, b.n_hits)
+    db = lfmod.DeviceBatch(b)
+    out = lfmod.TrackBuffers(b.n_seeds, b.n_events, db.device)
+    first = None
+    for _ in range(5):
+        lf.run(db, out)
+        torch.cuda.synchronize()
+        r = out.to_numpy()
+        if first is None:
+            first = r
+        assert r.n_tracks == first.n_tracks and np.array_equal(r.hit_idx, first.hit_idx)
+    small = lfmod.TrackBuffers(b.n_seeds - 1, b.n_events, db.device)
+    with pytest.raises(lfmod.LfError) as ei:
+        lf.run(db, small)
+    assert ei.value.status == lfmod.LF_ERR_CAPACITY
+    lf.close()
+    lf2 = lfmod.LookingForward(geometry, params, 10, 10, 10)
+    with pytest.raises(lfmod.LfError) as ei:
+        lf2.run(db, out)
+    assert ei.value.status == lfmod.LF_ERR_CAPACITY
+    lf2.close()
