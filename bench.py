@@ -1,0 +1,322 @@
+#!/usr/bin/env python
+"""Benchmark of the Looking Forward hot path on B200 (contract: see DESIGN.md "Measurement").
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--events E]
+
+A "step" is one pass of the whole hot path (a1..a7: one lf_run = track kernel + scan + compaction)
+over one batch of synthetic events.  Default workload: BASELINE.json configs[3] (20,000 events at
+Run-3-like occupancy, fp32, a single lf_run on one stream).  Prints ONE JSON line (rank 0).
+
+  value        events/s with inputs resident in HBM (CUDA events around the K steps, max over ranks)
+  e2e          the same metric through lf_run_host: pinned HOST buffers, H2D + D2H inside the timing
+  roofline     dominant kernel (lf_track_kernel): algorithmic bytes per launch / its mean duration,
+               timed live with CUDA events on the launching stream, vs MEASURED_PEAKS.json hbm_gbs
+  cpu_baseline the oracle, as it stands, on the box's host cores on a bounded sample (rank 0, N=1)
+
+--impl reference times the oracle (all host cores via the harness's event sharding) on a bounded
+sample of the same workload; under torchrun only rank 0 works.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+NOMINAL_HBM_GBS = 8000.0   # BASELINE.json north_star: "over 8 TB/s"
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons DURING the timed region (NVML; nvidia-smi as a fallback)."""
+
+    def __init__(self, index: int, period_s: float = 0.02):
+        self.index, self.period = index, period_s
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        self._nvml = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nvml = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nvml = None
+
+    def _reason_names(self, mask: int):
+        n = self._nvml
+        table = (("hw_slowdown", "nvmlClocksEventReasonHwSlowdown", 0x8), ("hw_thermal_slowdown", "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+                 ("sw_thermal_slowdown", "nvmlClocksEventReasonSwThermalSlowdown", 0x20), ("sw_power_cap", "nvmlClocksEventReasonSwPowerCap", 0x4),
+                 ("hw_power_brake", "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80))
+        return [name for name, attr, default in table if mask & getattr(n, attr, default)]
+
+    def _loop(self):
+        n = self._nvml
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(n.nvmlDeviceGetClockInfo(self._h, n.NVML_CLOCK_SM)))
+                try:
+                    mask = int(n.nvmlDeviceGetCurrentClocksEventReasons(self._h))
+                except Exception:
+                    mask = int(n.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                self.reasons.update(self._reason_names(mask))
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def start(self):
+        if self._nvml is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+        if self._nvml is None or not self.samples:
+            return self._smi_once()
+        return {"sm_mhz": float(statistics.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples), "source": "nvml during timed region"}
+
+    def _smi_once(self):
+        import subprocess
+        try:
+            out = subprocess.run(["nvidia-smi", f"--id={self.index}", "--query-gpu=clocks.sm,clocks.max.sm,clocks_event_reasons.active",
+                                  "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=20).stdout.strip().split(",")
+            return {"sm_mhz": float(out[0]), "sm_max_mhz": float(out[1]), "reasons": [out[2].strip()], "samples": 1,
+                    "source": "nvidia-smi after timed region (NVML unavailable)"}
+        except Exception as e:  # pragma: no cover
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [f"unavailable: {e}"], "samples": 0}
+
+
+def algorithmic_bytes(batch, n_tracks: int) -> int:
+    """Unique HBM bytes the method must move: inputs read once, tracks written once."""
+    return int(4 * batch.n_hits + batch.seg_offsets.nbytes + 20 * batch.n_seeds + batch.seed_offsets.nbytes
+               + 80 * n_tracks + 4 * (batch.n_events + 1) + 4)
+
+
+def oracle_rate(batch, threads: int, geometry, params):
+    from oracle import lf_oracle
+    t0 = time.perf_counter()
+    r = lf_oracle.run(geometry, params, batch, threads=threads)
+    dt = time.perf_counter() - t0
+    return batch.n_events / dt, dt, r
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, bounded sample per step."""
+    from paper_2402_14670_b200 import datagen, sharding
+    rank, _, world = sharding.dist_env()
+    if rank != 0:
+        return 0
+    cfg = datagen.CONFIGS[args.config]
+    G, P = datagen.toy_geometry(), datagen.default_params()
+    cores = os.cpu_count() or 1
+    probe = datagen.generate(cfg, n_events=min(200, args.events or cfg.n_events))
+    rate, _, _ = oracle_rate(probe, cores, G, P)
+    budget = min(0.5, 150.0 / max(args.steps + args.warmup, 1))
+    n_sample = int(min(max(rate * budget, 50), 2000, args.events or cfg.n_events))
+    batch = datagen.generate(cfg, n_events=n_sample)
+    for _ in range(args.warmup):
+        oracle_rate(batch, cores, G, P)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_rate(batch, cores, G, P)
+    dt = time.perf_counter() - t0
+    value = n_sample * args.steps / dt
+    sample = f"first {n_sample} events of {cfg.name} per step (seed {cfg.seed}); oracle sharded over {cores} threads by the harness"
+    line = {
+        "impl": "reference", "metric": "events_per_s", "value": value, "unit": "events/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{cfg.name}: Run-3-like occupancy, fp32 (bounded sample)", "events_per_step": n_sample,
+                   "seeds_per_step": batch.n_seeds, "hits_per_step": batch.n_hits},
+        "seeds_per_s": batch.n_seeds * args.steps / dt,
+        "cpu_baseline": {"value": value, "unit": "events/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    from paper_2402_14670_b200 import binding, datagen, sharding
+    rank, local_rank, world = sharding.dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg = datagen.CONFIGS[args.config]
+    if world > 1:  # weak scaling: every rank gets its own batch of the same recipe
+        cfg = datagen.with_overrides(cfg, seed=cfg.seed + 7919 * rank)
+    G = datagen.toy_geometry()
+    P = dict(datagen.default_params(), hit_storage=cfg.hit_storage)
+    t_gen = time.perf_counter()
+    batch = datagen.generate(cfg, n_events=args.events)
+    t_gen = time.perf_counter() - t_gen
+
+    lf = binding.LookingForward(G, P, batch.n_events, batch.n_seeds, batch.n_hits)
+    info = lf.info()
+    db = binding.DeviceBatch(batch, dev)
+    out = binding.TrackBuffers(batch.n_seeds, batch.n_events, dev)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            torch.distributed.barrier()
+
+    for _ in range(max(args.warmup, 3)):
+        lf.run(db, out, stream)
+    barrier()
+    n_tracks = int(out.n_tracks.cpu()[0])
+
+    # ---- timed region: K steps, inputs resident in HBM, per-kernel CUDA events recorded by the library
+    lf.set_profiling(True)
+    sampler = ClockSampler(local_rank)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.start()
+    e0.record(stream)
+    for _ in range(args.steps):
+        lf.run(db, out, stream)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    local_ms = e0.elapsed_time(e1)
+    k_track, k_scan, k_compact = lf.kernel_times()
+    lf.set_profiling(False)
+    total_ms, (tot_events, tot_seeds, tot_tracks) = sharding.reduce_job(
+        local_ms, [batch.n_events, batch.n_seeds, n_tracks], dev)
+    ms_per_step = total_ms / args.steps
+    value = tot_events / (ms_per_step * 1e-3)
+
+    # ---- end to end through lf_run_host (pinned host buffers; H2D + D2H inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        hb = binding.HostBatch(batch)
+        ht = binding.HostTracks(batch.n_seeds, batch.n_events)
+        for _ in range(2):
+            lf.run_host(hb, ht, stream)
+        k_e2e = max(3, min(args.steps, 10))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(k_e2e):
+            n_host = lf.run_host(hb, ht, stream)
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) * 1e3
+        assert n_host == n_tracks, "host path and device path disagree on the track count"
+        e2e_ms, _ = sharding.reduce_job(dt, [0], dev)
+        e2e = {"value": tot_events / (e2e_ms / k_e2e * 1e-3), "unit": "events/s", "h2d_bytes_per_step": hb.h2d_bytes(),
+               "d2h_bytes_per_step": ht.d2h_bytes(n_tracks), "ms_per_step": e2e_ms / k_e2e, "steps": k_e2e,
+               "api": "lf_run_host (pinned host buffers, synchronous)"}
+        del hb, ht
+
+    if rank != 0:
+        return 0
+
+    # ---- roofline of the dominant kernel
+    peak, peak_src = measured_peaks()
+    alg = algorithmic_bytes(batch, n_tracks)
+    achieved = alg / (k_track * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "kernel": "lf_track_kernel", "kernel_ms": k_track, "algorithmic_bytes_per_launch": alg,
+                "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                "note": "path is ALU/issue-bound, not HBM-bound (DESIGN.md 'Rooflines'); HBM fraction reported because the metric asks for it"}
+    traffic_file = os.path.join(ROOT, "profiles", "track_kernel_traffic.txt")
+    if os.path.exists(traffic_file):
+        try:
+            roofline["traffic"] = json.load(open(traffic_file)).get("dram_bytes_per_launch")
+        except Exception:
+            pass
+
+    # ---- CPU baseline: the oracle as it stands (single thread), bounded sample; plus an all-cores figure
+    cpu = None
+    extra = {}
+    if world == 1 and not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        n1 = min(batch.n_events, args.cpu_events)
+        sub = batch.slice_events(0, n1)
+        rate1, dt1, ref = oracle_rate(sub, 1, G, P)
+        cpu = {"value": rate1, "unit": "events/s", "cores": 1, "kind": "oracle",
+               "sample": f"first {n1} events of the same batch, single thread, {dt1:.1f} s"}
+        got_prefix = int(out.event_offsets[n1].item())
+        extra["oracle_check"] = {"events": n1, "gpu_tracks": got_prefix, "oracle_tracks": int(ref.n_tracks),
+                                 "equal": got_prefix == int(ref.n_tracks)}
+        nall = min(batch.n_events, args.cpu_events * min(cores, 8))
+        rate_all, dt_all, _ = oracle_rate(batch.slice_events(0, nall), cores, G, P)
+        extra["cpu_baseline_all_cores"] = {"value": rate_all, "unit": "events/s", "cores": cores, "kind": "oracle",
+                                           "sample": f"first {nall} events, harness shards events over {cores} threads, {dt_all:.1f} s"}
+
+    in_bytes = batch.input_bytes()
+    line = {
+        "metric": "events_per_s", "value": value, "unit": "events/s", "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{cfg.name}: {batch.n_events} events per GPU, Run-3-like occupancy, fp32, one lf_run on one stream",
+                   "events_per_gpu": batch.n_events, "seeds_per_gpu": batch.n_seeds, "hits_per_gpu": batch.n_hits,
+                   "tracks_per_step_per_gpu": n_tracks,
+                   "l2": f"no flush: inputs ({in_bytes / 1e6:.0f} MB) + outputs exceed the 126 MB L2",
+                   "sharding": "events, no data-path collective"},
+        "seeds_per_s": tot_seeds / (ms_per_step * 1e-3),
+        "tracks_per_s": tot_tracks / (ms_per_step * 1e-3),
+        "e2e": e2e, "gpu_launches": info.kernels_per_run * args.steps, "clocks": clocks, "roofline": roofline,
+        "cpu_baseline": cpu,
+        "kernels": {"track_ms": k_track, "scan_ms": k_scan, "compact_ms": k_compact, "track_regs": info.track_regs,
+                    "track_ctas_per_sm": info.track_ctas_per_sm, "track_grid": info.track_grid,
+                    "track_block": info.track_block, "track_smem_bytes": info.track_smem_bytes},
+        "context": {"paper_hlt1_sequence_khz_a5000": 130, "paper_lf_share": 0.20,
+                    "note": "paper numbers are whole-HLT1 on RTX A5000 (PAPER.md:342): context, not a target"},
+        "generation_s": t_gen,
+    }
+    line.update(extra)
+    print(json.dumps(line))
+    lf.close()
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--config", type=int, default=3, choices=[0, 1, 3, 4])
+    ap.add_argument("--events", type=int, default=None, help="override the number of events (default: the config's)")
+    ap.add_argument("--cpu-events", type=int, default=1500, help="events of the single-thread oracle sample")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

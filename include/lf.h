@@ -169,6 +169,14 @@ const char* lf_last_error(const lf_handle* h);
 
 lf_status lf_get_info(const lf_handle* h, lf_info* out);
 
+/* Per-kernel device timing for benchmarks.  With profiling enabled, lf_run / lf_run_debug record CUDA
+ * events on `cuda_stream` around each of their kernels (no synchronisation added).  After the caller
+ * has synchronised the stream, lf_kernel_times writes the mean durations in milliseconds over the runs
+ * recorded since profiling was enabled (the last 256 at most): ms[0] track kernel (a1..a6), ms[1]
+ * offset scan, ms[2] compaction (a7).  LF_ERR_INVALID_ARG if profiling is off or no run was recorded. */
+lf_status lf_set_profiling(lf_handle* h, int enabled);
+lf_status lf_kernel_times(lf_handle* h, float ms[3]);
+
 /* ABI self-description for bindings: version and struct sizes
  * (which: 0 geometry, 1 params, 2 seeds, 3 hits, 4 tracks, 5 debug, 6 info). */
 uint32_t lf_abi_version(void);

@@ -107,6 +107,10 @@ def load_library() -> C.CDLL:
     lib.lf_destroy.argtypes = [C.c_void_p]
     lib.lf_get_info.restype = C.c_int
     lib.lf_get_info.argtypes = [C.c_void_p, C.POINTER(lf_info)]
+    lib.lf_set_profiling.restype = C.c_int
+    lib.lf_set_profiling.argtypes = [C.c_void_p, C.c_int]
+    lib.lf_kernel_times.restype = C.c_int
+    lib.lf_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_float * 3)]
     if lib.lf_abi_version() != 1:
         raise ImportError("liblf_b200.so: ABI version mismatch")
     for i, st in enumerate(_STRUCTS):
@@ -204,6 +208,15 @@ class LookingForward:
         inf = lf_info()
         self._check(self._lib.lf_get_info(self._h, C.byref(inf)))
         return SimpleNamespace(**{n: getattr(inf, n) for n, _ in lf_info._fields_})
+
+    def set_profiling(self, enabled: bool):
+        self._check(self._lib.lf_set_profiling(self._h, 1 if enabled else 0))
+
+    def kernel_times(self):
+        """Mean (track, scan, compact) milliseconds of the profiled runs; the stream must be synchronised."""
+        ms = (C.c_float * 3)()
+        self._check(self._lib.lf_kernel_times(self._h, C.byref(ms)))
+        return tuple(float(v) for v in ms)
 
     # -- device path -----------------------------------------------------------------------------
     def run(self, db: DeviceBatch, out: Optional[TrackBuffers] = None, stream=None, debug: bool = False):

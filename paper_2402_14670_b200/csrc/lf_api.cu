@@ -18,6 +18,7 @@
 namespace {
 
 thread_local std::string g_create_error;
+constexpr size_t PROF_RING = 256;
 
 struct HostBufs { /* device staging for lf_run_host */
   float* seeds = nullptr;      /* 5 * max_seeds */
@@ -46,6 +47,9 @@ struct lf_handle {
   uint32_t *ev_count, *ev_off, *ticket;
   size_t workspace_bytes;
   HostBufs hb;
+  bool profiling = false;
+  size_t prof_runs = 0;                 /* runs recorded since profiling was enabled */
+  cudaEvent_t (*prof_ev)[4] = nullptr;  /* ring of PROF_RING event quadruples */
   std::string err;
 };
 
@@ -141,6 +145,9 @@ const char* validate(const lf_geometry& G, const lf_params& P) {
 template <bool DEBUG>
 lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
                  const lf_debug* dbg, cudaStream_t st) {
+  const bool prof = h->profiling;
+  cudaEvent_t* pe = prof ? h->prof_ev[h->prof_runs % PROF_RING] : nullptr;
+  if (prof) LF_CUDA(h, cudaEventRecord(pe[0], st));
   if (n_events > 0) {
     lf::TrackArgs A;
     std::memset(&A, 0, sizeof(A));
@@ -159,13 +166,19 @@ lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_
     const int grid = (int)std::min<size_t>((size_t)h->grid, n_events);
     lf::lf_track_kernel<DEBUG><<<grid, lf::CTA_THREADS, h->smem_bytes, st>>>(h->C, A);
   }
+  if (prof) LF_CUDA(h, cudaEventRecord(pe[1], st));
   lf::lf_scan_kernel<<<1, 1024, 0, st>>>(h->ev_count, (uint32_t)n_events, h->ev_off, out->event_offsets,
                                          out->n_tracks, h->ticket);
+  if (prof) LF_CUDA(h, cudaEventRecord(pe[2], st));
   if (n_events > 0 && seeds->n_seeds > 0) {
     const size_t total = seeds->n_seeds * lf::REC_WORDS;
     const unsigned blocks = (unsigned)((total + 255) / 256);
     lf::lf_compact_kernel<<<blocks, 256, 0, st>>>(h->ws_rec, h->ws_rank, h->ws_event, h->ev_off, seeds->n_seeds,
                                                   out->hit_idx, out->seed_idx, out->n_hits, out->state, out->quality);
+  }
+  if (prof) {
+    LF_CUDA(h, cudaEventRecord(pe[3], st));
+    ++h->prof_runs;
   }
   LF_CUDA(h, cudaGetLastError());
   return LF_OK;
@@ -280,6 +293,12 @@ lf_status lf_destroy(lf_handle* h) {
   cudaFree(b.hit_idx); cudaFree(b.seed_idx); cudaFree(b.n_hits); cudaFree(b.state); cudaFree(b.quality);
   cudaFree(b.ev_off); cudaFree(b.n_tracks);
   if (b.pinned_count) cudaFreeHost(b.pinned_count);
+  if (h->prof_ev) {
+    for (size_t i = 0; i < PROF_RING; ++i)
+      for (cudaEvent_t e : h->prof_ev[i])
+        if (e) cudaEventDestroy(e);
+    delete[] h->prof_ev;
+  }
   delete h;
   return LF_OK;
 }
@@ -295,6 +314,34 @@ lf_status lf_get_info(const lf_handle* h, lf_info* out) {
   out->staged_hits_per_event = h->stage_cap - 4;
   out->sm_count = h->sm_count;
   out->workspace_bytes = h->workspace_bytes;
+  return LF_OK;
+}
+
+lf_status lf_set_profiling(lf_handle* h, int enabled) {
+  if (!h) return LF_ERR_INVALID_ARG;
+  if (enabled && !h->prof_ev) {
+    h->prof_ev = new (std::nothrow) cudaEvent_t[PROF_RING][4]();
+    if (!h->prof_ev) return fail(h, LF_ERR_CUDA, "lf_set_profiling: out of host memory");
+    for (size_t i = 0; i < PROF_RING; ++i)
+      for (cudaEvent_t& e : h->prof_ev[i]) LF_CUDA(h, cudaEventCreate(&e));
+  }
+  h->profiling = enabled != 0;
+  h->prof_runs = 0;
+  return LF_OK;
+}
+
+lf_status lf_kernel_times(lf_handle* h, float ms[3]) {
+  if (!h || !ms) return LF_ERR_INVALID_ARG;
+  if (!h->profiling || h->prof_runs == 0) return fail(h, LF_ERR_INVALID_ARG, "lf_kernel_times: no profiled run recorded");
+  const size_t n = std::min<size_t>(h->prof_runs, PROF_RING);
+  double acc[3] = {0, 0, 0};
+  for (size_t r = 0; r < n; ++r)
+    for (int i = 0; i < 3; ++i) {
+      float t = 0.f;
+      LF_CUDA(h, cudaEventElapsedTime(&t, h->prof_ev[r][i], h->prof_ev[r][i + 1]));
+      acc[i] += t;
+    }
+  for (int i = 0; i < 3; ++i) ms[i] = (float)(acc[i] / (double)n);
   return LF_OK;
 }
 
