@@ -115,6 +115,18 @@ def algorithmic_bytes(batch, n_tracks: int) -> int:
                + 80 * n_tracks + 4 * (batch.n_events + 1) + 4)
 
 
+def kernel_bytes(batch, n_tracks: int, n_triplets: int) -> dict:
+    """Algorithmic HBM bytes per launch of each event kernel: every kernel stages the
+    event's hits once and reads/writes its own per-seed tables once."""
+    H, S, E = batch.n_hits, batch.n_seeds, batch.n_events
+    common = 4 * H + batch.seg_offsets.nbytes + batch.seed_offsets.nbytes
+    trip = (2 * n_triplets + 1) * S
+    return {"window": common + 20 * S + 48 * S,
+            "seed": common + 12 * S + 48 * S + trip,
+            "fit": common + 12 * S + 48 * S + trip + 80 * n_tracks + 12 * S + 4 * E,
+            "compact": 92 * S + 80 * n_tracks + 4 * E}
+
+
 def oracle_rate(batch, threads: int, geometry, params):
     from oracle import lf_oracle
     t0 = time.perf_counter()
@@ -210,7 +222,7 @@ def run_ours(args):
     barrier()
     clocks = sampler.stop()
     local_ms = e0.elapsed_time(e1)
-    k_track, k_scan, k_compact = lf.kernel_times()
+    ktimes = dict(zip(binding.KERNEL_NAMES, lf.kernel_times()))
     lf.set_profiling(False)
     total_ms, (tot_events, tot_seeds, tot_tracks) = sharding.reduce_job(
         local_ms, [batch.n_events, batch.n_seeds, n_tracks], dev)
@@ -241,18 +253,26 @@ def run_ours(args):
     if rank != 0:
         return 0
 
-    # ---- roofline of the dominant kernel
+    # ---- roofline of the dominant kernel (the slowest of the three event kernels)
     peak, peak_src = measured_peaks()
-    alg = algorithmic_bytes(batch, n_tracks)
-    achieved = alg / (k_track * 1e-3) / 1e9
+    kb = kernel_bytes(batch, n_tracks, int(P["n_triplets"]))
+    dom = max(("window", "seed", "fit"), key=lambda k: ktimes[k])
+    achieved = kb[dom] / (ktimes[dom] * 1e-3) / 1e9
+    path_bytes = algorithmic_bytes(batch, n_tracks)
+    path_gbs = path_bytes / (local_ms / args.steps * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "kernel": "lf_track_kernel", "kernel_ms": k_track, "algorithmic_bytes_per_launch": alg,
-                "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                "traffic": None, "kernel": f"lf_{dom}_kernel", "kernel_ms": ktimes[dom],
+                "algorithmic_bytes_per_launch": kb[dom], "peak_source": peak_src,
+                "whole_path": {"algorithmic_bytes_per_step": path_bytes, "achieved_gbs": path_gbs, "frac_of_measured": path_gbs / peak,
+                               "frac_of_nominal_8TBs": path_gbs / NOMINAL_HBM_GBS},
                 "note": "path is ALU/issue-bound, not HBM-bound (DESIGN.md 'Rooflines'); HBM fraction reported because the metric asks for it"}
-    traffic_file = os.path.join(ROOT, "profiles", "track_kernel_traffic.txt")
+    traffic_file = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.txt")
     if os.path.exists(traffic_file):
         try:
-            roofline["traffic"] = json.load(open(traffic_file)).get("dram_bytes_per_launch")
+            tr = json.load(open(traffic_file))
+            if tr.get("kernel") == roofline["kernel"]:
+                roofline["traffic"] = tr.get("dram_bytes_per_launch")
+                roofline["traffic_source"] = tr.get("source")
         except Exception:
             pass
 
@@ -288,9 +308,11 @@ def run_ours(args):
         "tracks_per_s": tot_tracks / (ms_per_step * 1e-3),
         "e2e": e2e, "gpu_launches": info.kernels_per_run * args.steps, "clocks": clocks, "roofline": roofline,
         "cpu_baseline": cpu,
-        "kernels": {"track_ms": k_track, "scan_ms": k_scan, "compact_ms": k_compact, "track_regs": info.track_regs,
-                    "track_ctas_per_sm": info.track_ctas_per_sm, "track_grid": info.track_grid,
-                    "track_block": info.track_block, "track_smem_bytes": info.track_smem_bytes},
+        "kernels": {"ms": ktimes, "algorithmic_bytes": kb,
+                    "launch": {n: {"regs": info.regs[i], "block": info.block[i], "grid": info.grid[i],
+                                   "ctas_per_sm": info.ctas_per_sm[i], "smem_bytes": info.smem_bytes[i]}
+                               for i, n in enumerate(("window", "seed", "fit"))},
+                    "staged_hits_per_event": info.staged_hits_per_event},
         "context": {"paper_hlt1_sequence_khz_a5000": 130, "paper_lf_share": 0.20,
                     "note": "paper numbers are whole-HLT1 on RTX A5000 (PAPER.md:342): context, not a target"},
         "generation_s": t_gen,

@@ -124,19 +124,27 @@ typedef struct {
   float* cand_quality;  /* n_seeds*NT: Q; -1 = failed the hit-count rule; -2 = failed the t_y cut */
 } lf_debug;
 
-/* What the library launches, for benchmarks and occupancy reports (HOST struct, filled by lf_get_info). */
+/* What the library launches, for benchmarks and occupancy reports (HOST struct, filled by lf_get_info).
+ * Per-kernel arrays are indexed LF_K_WINDOW, LF_K_SEED, LF_K_FIT (the three event kernels). */
+#define LF_K_WINDOW 0
+#define LF_K_SEED 1
+#define LF_K_FIT 2
+#define LF_N_KERNELS 5 /* + LF_K_SCAN = 3, LF_K_COMPACT = 4 in lf_kernel_times */
 typedef struct {
-  int32_t kernels_per_run;       /* kernel launches one lf_run enqueues */
-  int32_t track_regs, track_block, track_grid, track_ctas_per_sm;
-  int32_t track_smem_bytes;      /* dynamic shared memory of the track kernel */
+  int32_t kernels_per_run;       /* kernel launches one lf_run enqueues (5) */
+  int32_t regs[3], block[3], grid[3], ctas_per_sm[3];
+  int32_t smem_bytes[3];         /* dynamic shared memory per CTA */
   int32_t staged_hits_per_event; /* events with more hits than this read hits from global memory */
   int32_t sm_count;
   size_t workspace_bytes;
 } lf_info;
 
 /* Creates a context for batches of at most max_events / max_seeds / max_hits.  Validates geometry
- * and params, uploads constants, allocates the workspace (max_seeds*88 + max_events*4 bytes on the
- * current CUDA device).  *out is set only on LF_OK.  HOST pointers. */
+ * and params, uploads constants, allocates the workspace (about max_seeds*(141 + 2*n_triplets) +
+ * max_events*8 bytes on the current CUDA device).  The shared-memory stage for one event's hits is sized
+ * from the maxima: 1.5 * max_hits / max_events + 512 hits, clamped to [2048, 16384]; larger events are
+ * still processed correctly, reading their hits from global memory.  *out is set only on LF_OK.
+ * HOST pointers. */
 lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t max_events,
                     size_t max_seeds, size_t max_hits, lf_handle** out);
 
@@ -172,10 +180,11 @@ lf_status lf_get_info(const lf_handle* h, lf_info* out);
 /* Per-kernel device timing for benchmarks.  With profiling enabled, lf_run / lf_run_debug record CUDA
  * events on `cuda_stream` around each of their kernels (no synchronisation added).  After the caller
  * has synchronised the stream, lf_kernel_times writes the mean durations in milliseconds over the runs
- * recorded since profiling was enabled (the last 256 at most): ms[0] track kernel (a1..a6), ms[1]
- * offset scan, ms[2] compaction (a7).  LF_ERR_INVALID_ARG if profiling is off or no run was recorded. */
+ * recorded since profiling was enabled (the last 256 at most): ms[0] window kernel (a1, a2), ms[1] seeding
+ * kernel (a3), ms[2] fit kernel (a4..a6), ms[3] offset scan, ms[4] compaction (a7).
+ * LF_ERR_INVALID_ARG if profiling is off or no run was recorded. */
 lf_status lf_set_profiling(lf_handle* h, int enabled);
-lf_status lf_kernel_times(lf_handle* h, float ms[3]);
+lf_status lf_kernel_times(lf_handle* h, float ms[LF_N_KERNELS]);
 
 /* ABI self-description for bindings: version and struct sizes
  * (which: 0 geometry, 1 params, 2 seeds, 3 hits, 4 tracks, 5 debug, 6 info). */

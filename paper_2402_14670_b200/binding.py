@@ -70,9 +70,12 @@ class lf_debug(C.Structure):
 
 
 class lf_info(C.Structure):
-    _fields_ = [("kernels_per_run", C.c_int32), ("track_regs", C.c_int32), ("track_block", C.c_int32),
-                ("track_grid", C.c_int32), ("track_ctas_per_sm", C.c_int32), ("track_smem_bytes", C.c_int32),
+    _fields_ = [("kernels_per_run", C.c_int32), ("regs", C.c_int32 * 3), ("block", C.c_int32 * 3),
+                ("grid", C.c_int32 * 3), ("ctas_per_sm", C.c_int32 * 3), ("smem_bytes", C.c_int32 * 3),
                 ("staged_hits_per_event", C.c_int32), ("sm_count", C.c_int32), ("workspace_bytes", C.c_size_t)]
+
+
+KERNEL_NAMES = ("window", "seed", "fit", "scan", "compact")
 
 
 _STRUCTS = (lf_geometry, lf_params, lf_seeds, lf_hits, lf_tracks, lf_debug, lf_info)
@@ -110,7 +113,7 @@ def load_library() -> C.CDLL:
     lib.lf_set_profiling.restype = C.c_int
     lib.lf_set_profiling.argtypes = [C.c_void_p, C.c_int]
     lib.lf_kernel_times.restype = C.c_int
-    lib.lf_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_float * 3)]
+    lib.lf_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_float * 5)]
     if lib.lf_abi_version() != 1:
         raise ImportError("liblf_b200.so: ABI version mismatch")
     for i, st in enumerate(_STRUCTS):
@@ -207,14 +210,15 @@ class LookingForward:
     def info(self) -> SimpleNamespace:
         inf = lf_info()
         self._check(self._lib.lf_get_info(self._h, C.byref(inf)))
-        return SimpleNamespace(**{n: getattr(inf, n) for n, _ in lf_info._fields_})
+        conv = lambda v: list(v) if hasattr(v, "__len__") else v
+        return SimpleNamespace(**{n: conv(getattr(inf, n)) for n, _ in lf_info._fields_})
 
     def set_profiling(self, enabled: bool):
         self._check(self._lib.lf_set_profiling(self._h, 1 if enabled else 0))
 
     def kernel_times(self):
-        """Mean (track, scan, compact) milliseconds of the profiled runs; the stream must be synchronised."""
-        ms = (C.c_float * 3)()
+        """Mean (window, seed, fit, scan, compact) milliseconds of the profiled runs; the stream must be synchronised."""
+        ms = (C.c_float * 5)()
         self._check(self._lib.lf_kernel_times(self._h, C.byref(ms)))
         return tuple(float(v) for v in ms)
 

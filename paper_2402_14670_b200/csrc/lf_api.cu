@@ -19,6 +19,7 @@ namespace {
 
 thread_local std::string g_create_error;
 constexpr size_t PROF_RING = 256;
+constexpr int N_PROF_EV = LF_N_KERNELS + 1;
 
 struct HostBufs { /* device staging for lf_run_host */
   float* seeds = nullptr;      /* 5 * max_seeds */
@@ -40,16 +41,19 @@ struct lf_handle {
   lf_params P;
   size_t max_events, max_seeds, max_hits;
   int device;
-  int sm_count, ctas_per_sm, grid, regs;
-  int smem_bytes, stage_cap;
+  int sm_count, stage_cap;
+  int regs[3], grid[3], ctas_per_sm[3], smem_bytes[3]; /* window, seed, fit kernels */
   /* workspace */
+  uint32_t* win;
+  uint16_t* trip_code;
+  uint8_t* n_trip;
   int32_t *ws_rec, *ws_nh, *ws_rank, *ws_event;
-  uint32_t *ev_count, *ev_off, *ticket;
+  uint32_t *ev_count, *ev_off, *tickets;
   size_t workspace_bytes;
   HostBufs hb;
   bool profiling = false;
   size_t prof_runs = 0;                 /* runs recorded since profiling was enabled */
-  cudaEvent_t (*prof_ev)[4] = nullptr;  /* ring of PROF_RING event quadruples */
+  cudaEvent_t (*prof_ev)[N_PROF_EV] = nullptr;  /* ring of PROF_RING event sets */
   std::string err;
 };
 
@@ -96,6 +100,7 @@ void make_consts(const lf_geometry& G, const lf_params& P, lf::Consts& c) {
     const int a = s ? 3 : 0, b = a + 4, cc = a + 8;
     c.inv_dz_ac[s] = one / (c.z[cc] - c.z[a]);
     c.zmag_a[s] = c.z_mag - c.z[a];
+    c.inv_r[s] = one / (c.inv_dz_ac[s] * c.zmag_a[s]); /* bracket of the h2 interval only (not a decision) */
     c.D10[s] = c.d[b] - c.d[a];
     c.D20[s] = c.d[cc] - c.d[a];
     c.W10[s] = c.w[b] - c.w[a];
@@ -148,36 +153,49 @@ lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_
   const bool prof = h->profiling;
   cudaEvent_t* pe = prof ? h->prof_ev[h->prof_runs % PROF_RING] : nullptr;
   if (prof) LF_CUDA(h, cudaEventRecord(pe[0], st));
-  if (n_events > 0) {
-    lf::TrackArgs A;
-    std::memset(&A, 0, sizeof(A));
-    A.sx = seeds->x; A.sy = seeds->y; A.stx = seeds->tx; A.sty = seeds->ty; A.sqop = seeds->qop;
-    A.seed_off = seeds->event_offsets;
-    A.hx = hits->x; A.seg_off = hits->seg_offsets;
-    A.n_events = (uint32_t)n_events;
-    A.ws_rec = h->ws_rec; A.ws_nh = h->ws_nh; A.ws_rank = h->ws_rank; A.ws_event = h->ws_event;
-    A.ev_count = h->ev_count; A.ticket = h->ticket;
-    A.stage_cap = h->stage_cap;
-    if (dbg) {
-      A.dbg.win_first = dbg->win_first; A.dbg.win_count = dbg->win_count; A.dbg.n_triplets = dbg->n_triplets;
-      A.dbg.trip_hits = dbg->trip_hits; A.dbg.trip_set = dbg->trip_set; A.dbg.trip_chi2 = dbg->trip_chi2;
-      A.dbg.cand_hits = dbg->cand_hits; A.dbg.cand_quality = dbg->cand_quality;
-    }
-    const int grid = (int)std::min<size_t>((size_t)h->grid, n_events);
-    lf::lf_track_kernel<DEBUG><<<grid, lf::CTA_THREADS, h->smem_bytes, st>>>(h->C, A);
+  lf::EventArgs A;
+  std::memset(&A, 0, sizeof(A));
+  A.sx = seeds->x; A.sy = seeds->y; A.stx = seeds->tx; A.sty = seeds->ty; A.sqop = seeds->qop;
+  A.seed_off = seeds->event_offsets;
+  A.hx = hits->x; A.seg_off = hits->seg_offsets;
+  A.n_events = (uint32_t)n_events;
+  A.stage_cap = h->stage_cap;
+  A.win = h->win; A.trip_code = h->trip_code; A.n_trip = h->n_trip;
+  A.ws_rec = h->ws_rec; A.ws_nh = h->ws_nh; A.ws_rank = h->ws_rank; A.ws_event = h->ws_event;
+  A.ev_count = h->ev_count;
+  if (dbg) {
+    A.dbg.win_first = dbg->win_first; A.dbg.win_count = dbg->win_count; A.dbg.n_triplets = dbg->n_triplets;
+    A.dbg.trip_hits = dbg->trip_hits; A.dbg.trip_set = dbg->trip_set; A.dbg.trip_chi2 = dbg->trip_chi2;
+    A.dbg.cand_hits = dbg->cand_hits; A.dbg.cand_quality = dbg->cand_quality;
+  }
+  const bool work = n_events > 0;
+  auto grid_of = [&](int k) { return (int)std::min<size_t>((size_t)h->grid[k], n_events); };
+  if (work) {
+    A.ticket = h->tickets + 0;
+    lf::lf_window_kernel<DEBUG><<<grid_of(0), lf::WIN_THREADS, h->smem_bytes[0], st>>>(h->C, A);
   }
   if (prof) LF_CUDA(h, cudaEventRecord(pe[1], st));
-  lf::lf_scan_kernel<<<1, 1024, 0, st>>>(h->ev_count, (uint32_t)n_events, h->ev_off, out->event_offsets,
-                                         out->n_tracks, h->ticket);
+  if (work) {
+    A.ticket = h->tickets + 1;
+    lf::lf_seed_kernel<DEBUG><<<grid_of(1), lf::SEED_THREADS, h->smem_bytes[1], st>>>(h->C, A);
+  }
   if (prof) LF_CUDA(h, cudaEventRecord(pe[2], st));
-  if (n_events > 0 && seeds->n_seeds > 0) {
+  if (work) {
+    A.ticket = h->tickets + 2;
+    lf::lf_fit_kernel<DEBUG><<<grid_of(2), lf::FIT_THREADS, h->smem_bytes[2], st>>>(h->C, A);
+  }
+  if (prof) LF_CUDA(h, cudaEventRecord(pe[3], st));
+  lf::lf_scan_kernel<<<1, 1024, 0, st>>>(h->ev_count, (uint32_t)n_events, h->ev_off, out->event_offsets,
+                                         out->n_tracks, h->tickets);
+  if (prof) LF_CUDA(h, cudaEventRecord(pe[4], st));
+  if (work && seeds->n_seeds > 0) {
     const size_t total = seeds->n_seeds * lf::REC_WORDS;
     const unsigned blocks = (unsigned)((total + 255) / 256);
     lf::lf_compact_kernel<<<blocks, 256, 0, st>>>(h->ws_rec, h->ws_rank, h->ws_event, h->ev_off, seeds->n_seeds,
                                                   out->hit_idx, out->seed_idx, out->n_hits, out->state, out->quality);
   }
   if (prof) {
-    LF_CUDA(h, cudaEventRecord(pe[3], st));
+    LF_CUDA(h, cudaEventRecord(pe[5], st));
     ++h->prof_runs;
   }
   LF_CUDA(h, cudaGetLastError());
@@ -254,31 +272,47 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   h->sm_count = prop.multiProcessorCount;
   if (prop.major < 10) return bail(LF_ERR_UNSUPPORTED, "lf_create: this library is built for sm_100a (Blackwell) only");
 
-  /* shared memory: fixed part + one event's hits.  16384 hits (64 KB) covers BASELINE.json's
-   * stress config (about 13.5k hits in the largest event); larger events read global memory. */
-  const size_t fixed = (sizeof(lf::CtaShared) + 15) & ~size_t(15);
-  h->stage_cap = 16384;
-  h->smem_bytes = (int)(fixed + (size_t)h->stage_cap * sizeof(float));
-  LF_CREATE_CUDA(cudaFuncSetAttribute(lf::lf_track_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_bytes));
-  LF_CREATE_CUDA(cudaFuncSetAttribute(lf::lf_track_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_bytes));
-  LF_CREATE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->ctas_per_sm, lf::lf_track_kernel<false>,
-                                                               lf::CTA_THREADS, h->smem_bytes));
-  if (h->ctas_per_sm < 1) return bail(LF_ERR_CUDA, "lf_create: track kernel does not fit on an SM");
-  h->grid = h->sm_count * h->ctas_per_sm;
-  cudaFuncAttributes fa;
-  LF_CREATE_CUDA(cudaFuncGetAttributes(&fa, lf::lf_track_kernel<false>));
-  h->regs = fa.numRegs;
+  /* Shared-memory stage for one event's hits, sized from the maxima (include/lf.h, lf_create):
+   * 1.5 x the mean event + 512 hits, clamped to [2048, 16384].  Larger events read global memory. */
+  {
+    const double mean_hits = (double)max_hits / (double)std::max<size_t>(max_events, 1);
+    size_t cap = (size_t)(1.5 * mean_hits) + 512;
+    cap = (cap + 255) & ~size_t(255);
+    h->stage_cap = (int)std::min<size_t>(std::max<size_t>(cap, 2048), 16384);
+  }
+  const size_t stage_bytes = (size_t)lf::HDR_BYTES + (size_t)h->stage_cap * sizeof(float);
+  h->smem_bytes[0] = (int)stage_bytes;
+  h->smem_bytes[1] = (int)(stage_bytes + sizeof(lf::SeedTables));
+  h->smem_bytes[2] = (int)(stage_bytes + lf::fit_tables_bytes(params->n_triplets));
+  const void* kern[3][2] = {{(const void*)lf::lf_window_kernel<false>, (const void*)lf::lf_window_kernel<true>},
+                            {(const void*)lf::lf_seed_kernel<false>, (const void*)lf::lf_seed_kernel<true>},
+                            {(const void*)lf::lf_fit_kernel<false>, (const void*)lf::lf_fit_kernel<true>}};
+  const int threads[3] = {lf::WIN_THREADS, lf::SEED_THREADS, lf::FIT_THREADS};
+  for (int k = 0; k < 3; ++k) {
+    for (int d = 0; d < 2; ++d)
+      LF_CREATE_CUDA(cudaFuncSetAttribute(kern[k][d], cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_bytes[k]));
+    LF_CREATE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->ctas_per_sm[k], kern[k][0], threads[k], h->smem_bytes[k]));
+    if (h->ctas_per_sm[k] < 1) return bail(LF_ERR_CUDA, "lf_create: an event kernel does not fit on an SM");
+    h->grid[k] = h->sm_count * h->ctas_per_sm[k];
+    cudaFuncAttributes fa;
+    LF_CREATE_CUDA(cudaFuncGetAttributes(&fa, kern[k][0]));
+    h->regs[k] = fa.numRegs;
+  }
 
   const size_t ns = std::max<size_t>(max_seeds, 1), ne = std::max<size_t>(max_events, 1);
+  const size_t nt = (size_t)params->n_triplets;
+  LF_CREATE_CUDA(cudaMalloc(&h->win, ns * lf::NL * sizeof(uint32_t)));
+  LF_CREATE_CUDA(cudaMalloc(&h->trip_code, ns * nt * sizeof(uint16_t)));
+  LF_CREATE_CUDA(cudaMalloc(&h->n_trip, ns));
   LF_CREATE_CUDA(cudaMalloc(&h->ws_rec, ns * lf::REC_WORDS * sizeof(int32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ws_nh, ns * sizeof(int32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ws_rank, ns * sizeof(int32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ws_event, ns * sizeof(int32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ev_count, ne * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ev_off, (ne + 1) * sizeof(uint32_t)));
-  LF_CREATE_CUDA(cudaMalloc(&h->ticket, sizeof(uint32_t)));
-  LF_CREATE_CUDA(cudaMemset(h->ticket, 0, sizeof(uint32_t)));
-  h->workspace_bytes = ns * (lf::REC_WORDS + 3) * sizeof(int32_t) + (2 * ne + 2) * sizeof(uint32_t);
+  LF_CREATE_CUDA(cudaMalloc(&h->tickets, lf::N_TICKETS * sizeof(uint32_t)));
+  LF_CREATE_CUDA(cudaMemset(h->tickets, 0, lf::N_TICKETS * sizeof(uint32_t)));
+  h->workspace_bytes = ns * (lf::NL * 4 + nt * 2 + 1 + (lf::REC_WORDS + 3) * 4) + (2 * ne + 1 + lf::N_TICKETS) * sizeof(uint32_t);
 #undef LF_CREATE_CUDA
   *out = h;
   return LF_OK;
@@ -286,8 +320,9 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
 
 lf_status lf_destroy(lf_handle* h) {
   if (!h) return LF_OK;
+  cudaFree(h->win); cudaFree(h->trip_code); cudaFree(h->n_trip);
   cudaFree(h->ws_rec); cudaFree(h->ws_nh); cudaFree(h->ws_rank); cudaFree(h->ws_event);
-  cudaFree(h->ev_count); cudaFree(h->ev_off); cudaFree(h->ticket);
+  cudaFree(h->ev_count); cudaFree(h->ev_off); cudaFree(h->tickets);
   HostBufs& b = h->hb;
   cudaFree(b.seeds); cudaFree(b.seed_off); cudaFree(b.hits); cudaFree(b.seg_off);
   cudaFree(b.hit_idx); cudaFree(b.seed_idx); cudaFree(b.n_hits); cudaFree(b.state); cudaFree(b.quality);
@@ -305,12 +340,15 @@ lf_status lf_destroy(lf_handle* h) {
 
 lf_status lf_get_info(const lf_handle* h, lf_info* out) {
   if (!h || !out) return LF_ERR_INVALID_ARG;
-  out->kernels_per_run = 3;
-  out->track_regs = h->regs;
-  out->track_block = lf::CTA_THREADS;
-  out->track_grid = h->grid;
-  out->track_ctas_per_sm = h->ctas_per_sm;
-  out->track_smem_bytes = h->smem_bytes;
+  out->kernels_per_run = LF_N_KERNELS;
+  const int threads[3] = {lf::WIN_THREADS, lf::SEED_THREADS, lf::FIT_THREADS};
+  for (int k = 0; k < 3; ++k) {
+    out->regs[k] = h->regs[k];
+    out->block[k] = threads[k];
+    out->grid[k] = h->grid[k];
+    out->ctas_per_sm[k] = h->ctas_per_sm[k];
+    out->smem_bytes[k] = h->smem_bytes[k];
+  }
   out->staged_hits_per_event = h->stage_cap - 4;
   out->sm_count = h->sm_count;
   out->workspace_bytes = h->workspace_bytes;
@@ -320,7 +358,7 @@ lf_status lf_get_info(const lf_handle* h, lf_info* out) {
 lf_status lf_set_profiling(lf_handle* h, int enabled) {
   if (!h) return LF_ERR_INVALID_ARG;
   if (enabled && !h->prof_ev) {
-    h->prof_ev = new (std::nothrow) cudaEvent_t[PROF_RING][4]();
+    h->prof_ev = new (std::nothrow) cudaEvent_t[PROF_RING][N_PROF_EV]();
     if (!h->prof_ev) return fail(h, LF_ERR_CUDA, "lf_set_profiling: out of host memory");
     for (size_t i = 0; i < PROF_RING; ++i)
       for (cudaEvent_t& e : h->prof_ev[i]) LF_CUDA(h, cudaEventCreate(&e));
@@ -330,18 +368,18 @@ lf_status lf_set_profiling(lf_handle* h, int enabled) {
   return LF_OK;
 }
 
-lf_status lf_kernel_times(lf_handle* h, float ms[3]) {
+lf_status lf_kernel_times(lf_handle* h, float ms[LF_N_KERNELS]) {
   if (!h || !ms) return LF_ERR_INVALID_ARG;
   if (!h->profiling || h->prof_runs == 0) return fail(h, LF_ERR_INVALID_ARG, "lf_kernel_times: no profiled run recorded");
   const size_t n = std::min<size_t>(h->prof_runs, PROF_RING);
-  double acc[3] = {0, 0, 0};
+  double acc[LF_N_KERNELS] = {0, 0, 0, 0, 0};
   for (size_t r = 0; r < n; ++r)
-    for (int i = 0; i < 3; ++i) {
+    for (int i = 0; i < LF_N_KERNELS; ++i) {
       float t = 0.f;
       LF_CUDA(h, cudaEventElapsedTime(&t, h->prof_ev[r][i], h->prof_ev[r][i + 1]));
       acc[i] += t;
     }
-  for (int i = 0; i < 3; ++i) ms[i] = (float)(acc[i] / (double)n);
+  for (int i = 0; i < LF_N_KERNELS; ++i) ms[i] = (float)(acc[i] / (double)n);
   return LF_OK;
 }
 

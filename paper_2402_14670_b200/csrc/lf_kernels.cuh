@@ -1,22 +1,25 @@
 /*
  * lf_kernels.cuh -- sm_100a device code of the Looking Forward hot path (include/lf.h, a1..a7).
  *
- * Execution model:
- *   lf_track_kernel    persistent CTAs take events from an atomic ticket.  The event's 24 x-sorted
- *                      hit segments are contiguous in HBM, so one 1-D bulk async copy (TMA,
- *                      cp.async.bulk + mbarrier) stages the whole event into shared memory; the
- *                      CTA's warps then take seeds from a shared counter, ONE WARP PER SEED:
- *                        a1/a2  lanes 0..23 = (layer, edge): 24 binary searches in parallel;
- *                        a3     lanes = h2 hits of the window, loop over h0; ballot-compacted
- *                               survivors are finished lane-per-doublet (binary-search closest h1);
- *                               top-n by rank selection on 64-bit (chi2, set, h0, h2) keys;
- *                        a4/a5  lanes = (triplet, layer) pairs, binary-search closest hit;
- *                        a6     lanes = candidates, sequential-order fp32 fit (the oracle's
- *                               summation order), warp min-reduce on (Q, order) keys.
- *                      At the end of an event the CTA ranks its found tracks in seed order.
- *   lf_scan_kernel     exclusive scan of the per-event track counts -> event_offsets, n_tracks.
- *   lf_compact_kernel  stream compaction: per-seed records -> dense SoA outputs in (event, seed)
- *                      order, one thread per (seed, word), coalesced.
+ * Execution model.  Three event kernels share one skeleton: persistent CTAs take
+ * events from an atomic ticket; the event's 24 x-sorted hit segments are contiguous in HBM, so one
+ * 1-D bulk async copy (TMA: cp.async.bulk + mbarrier, SASS UBLKCP) stages the whole event into shared
+ * memory.  Each kernel then maps threads to the natural work item of its stage:
+ *
+ *   lf_window_kernel  a1/a2  one thread per (seed, layer, window edge): branch-free binary searches,
+ *                            edge pairs exchange by shuffle, n_window cap; packed window words to HBM.
+ *   lf_seed_kernel    a3     one warp per seed, lanes = h0 hits.  For a fixed h0 the h2 hits that pass
+ *                            the magnet-opening cut form a contiguous x interval: a binary search finds a
+ *                            conservative superset, the exact fp32 predicate then decides (bit-exact
+ *                            with the all-pairs definition).  Survivors are ballot-compacted and
+ *                            finished lane-per-doublet (closest h1, chi2 cut); rank selection on
+ *                            64-bit (chi2, set, h0, h2) keys keeps the n smallest, sorted.
+ *   lf_fit_kernel     a4-a6  one thread per candidate: parabola through the triplet, closest hit in the
+ *                            9 other windows, hit-count rule, fp32 fit in the oracle's summation order, Q.
+ *                            Then one thread per seed picks the lowest Q and writes the track record;
+ *                            the CTA ranks the event's tracks in seed order.
+ *   lf_scan_kernel    a7     exclusive scan of per-event track counts -> event_offsets, n_tracks.
+ *   lf_compact_kernel a7     stream compaction: per-seed records -> dense SoA outputs, coalesced.
  *
  * Arithmetic contract: fp32, one rounding per operation, in the order DESIGN.md "Canonical
  * arithmetic" lists (compile with -fmad=false, no fast-math; '/' is IEEE division).  This file is
@@ -30,19 +33,23 @@ namespace lf {
 
 constexpr int NL = 12;
 constexpr int NSEG = 24;
-constexpr int WARPS_PER_CTA = 8;
-constexpr int CTA_THREADS = WARPS_PER_CTA * 32;
 constexpr int REC_WORDS = 20;  /* 12 hit idx, seed, n_hits, 5 state, Q */
 constexpr int TRIP_BUF = 64;   /* per-warp triplet key buffer */
 constexpr int MAX_NT = 16;     /* == LF_MAX_TRIPLETS */
+constexpr int WIN_THREADS = 256;
+constexpr int SEED_WARPS = 8;
+constexpr int SEED_THREADS = SEED_WARPS * 32;
+constexpr int FIT_THREADS = 256;
+constexpr int FIT_CHUNK = 256; /* seeds of one event handled per pass of the fit kernel (== FIT_THREADS) */
+constexpr int N_TICKETS = 4;
 constexpr unsigned FULL = 0xffffffffu;
-constexpr unsigned NO_HIT = 0xFFu;
+constexpr float INTERVAL_MARGIN = 0.1f; /* mm added to the magnet tolerance when bracketing h2 (superset only) */
 
 /* Geometry-derived constants and tunables, computed once on the host in fp32 (lf_api.cu). */
 struct Consts {
   float z[NL], tana[NL], inv_tan[NL], dzs[NL], dzm[NL], d[NL], w[NL];
   float z_seed, z_mag, kick, dr, K[2], poly[5], mag_dz_seed;
-  float inv_dz_ac[2], zmag_a[2], D10[2], D20[2], W10[2], W20[2], inv_det[2], inv_D10[2];
+  float inv_dz_ac[2], zmag_a[2], inv_r[2], D10[2], D20[2], W10[2], W20[2], inv_det[2], inv_D10[2];
   float dz_state, ds, ws, dws;
   int polarity;
   float T_triplet, T_x, T_uv_slope, T_uv_min, T_ty, inv_Tx, inv_Ty, T_Q, C_nhits[4];
@@ -58,37 +65,41 @@ struct DebugOut {
   float* cand_quality;
 };
 
-struct TrackArgs {
+/* Arguments common to the three event kernels + the per-stage tables (library workspace). */
+struct EventArgs {
   const float *sx, *sy, *stx, *sty, *sqop;
   const uint32_t* seed_off;
   const float* hx;
   const uint32_t* seg_off;
   uint32_t n_events;
-  int32_t* ws_rec;     /* n_seeds * REC_WORDS */
-  int32_t* ws_nh;      /* n_seeds: n_hits of the seed's track, 0 = none */
-  int32_t* ws_rank;    /* n_seeds: rank among the event's tracks, -1 = none */
-  int32_t* ws_event;   /* n_seeds: event of the seed */
-  uint32_t* ev_count;  /* n_events */
-  uint32_t* ticket;    /* 1 */
-  int stage_cap;       /* floats of shared memory available for one event's hits */
+  int stage_cap;        /* floats of shared memory available for one event's hits */
+  uint32_t* ticket;     /* this kernel's event ticket */
+  uint32_t* win;        /* n_seeds*12: (first_in_event << 6) | count */
+  uint16_t* trip_code;  /* n_seeds*NT: set<<15 | h0<<10 | h2<<5 | h1 (window-relative), sorted */
+  uint8_t* n_trip;      /* n_seeds */
+  int32_t* ws_rec;      /* n_seeds * REC_WORDS */
+  int32_t* ws_nh;       /* n_seeds: 1 if the seed has a track, else 0 */
+  int32_t* ws_rank;     /* n_seeds: rank among the event's tracks, -1 = none */
+  int32_t* ws_event;    /* n_seeds: event of the seed */
+  uint32_t* ev_count;   /* n_events */
   DebugOut dbg;
 };
 
-struct __align__(16) WarpScratch {
-  unsigned long long trip[TRIP_BUF];
-  uint16_t dq[64];
-  uint8_t ext[MAX_NT][16];
-  int32_t rec[REC_WORDS];
-  int32_t pad[12];
-};
-
-struct __align__(16) CtaShared {
+/* Head of the dynamic shared memory of every event kernel; the staged hits follow it. */
+struct __align__(16) CtaHeader {
   unsigned long long mbar;
-  int seg[NSEG + 3];
-  int ev, next_seed;
-  int warp_tot[WARPS_PER_CTA];
-  float g_tana[NL], g_dzs[NL], g_dzm[NL], g_d[NL], g_w[NL];
-  WarpScratch ws[WARPS_PER_CTA];
+  int seg[NSEG + 1];
+  int ev;
+  int nsteps; /* binary-search steps that cover the event's longest segment */
+  int warp_tot[8];
+  int pad[1];
+};
+constexpr int HDR_BYTES = (sizeof(CtaHeader) + 15) & ~15;
+
+struct EventCtx {
+  uint32_t ev, h0;
+  int nh, skew;
+  bool staged;
 };
 
 /* ---------------------------------------------------------------- PTX helpers (TMA 1-D bulk copy) */
@@ -123,10 +134,9 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 
 __device__ __forceinline__ bool is_uv(int l) { return ((l & 3) == 1) || ((l & 3) == 2); }
 
-/* The one dynamic shared-memory array of the track kernel: CtaShared, then the staged hits. */
+/* The one dynamic shared-memory array: CtaHeader, staged hits, then the kernel's own tables. */
 extern __shared__ __align__(16) unsigned char lf_smem[];
-constexpr size_t FIXED_SMEM = (sizeof(CtaShared) + 15) & ~size_t(15);
-__device__ __forceinline__ float* stage_buf() { return reinterpret_cast<float*>(lf_smem + FIXED_SMEM); }
+__device__ __forceinline__ float* stage_buf() { return reinterpret_cast<float*>(lf_smem + HDR_BYTES); }
 
 /* View of the current event's hits, indexed event-relative.  Staged: shared memory (LDS);
  * fallback for events larger than the stage buffer: read-only global loads. */
@@ -143,36 +153,186 @@ struct HitView<false> {
   __device__ __forceinline__ float operator[](int i) const { return __ldg(p + i); }
 };
 
-/* Closest hit to `pred` in the x-sorted window [f, f+n): binary search for the first x >= pred, then
- * compare the two neighbours; ties -> lower index, including runs of equal distance on the low side
- * (equals a linear argmin with strict '<').  Returns the event-relative index, or -1 if n == 0. */
+/* Takes the next event and stages its hits.  Called by every thread of the CTA; returns false when
+ * the batch is exhausted.  Hit i of the event then lives at stage_buf()[skew + i]. */
+__device__ __forceinline__ bool fetch_event(const EventArgs& A, uint32_t& phase, EventCtx& E) {
+  CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
+  float* buf = stage_buf();
+  const int tid = threadIdx.x;
+  __syncthreads(); /* previous event fully retired: header, stage buffer and tables reusable */
+  if (tid == 0) H.ev = (int)atomicAdd(A.ticket, 1u);
+  __syncthreads();
+  E.ev = (uint32_t)H.ev;
+  if (E.ev >= A.n_events) return false;
+  const uint32_t* so = A.seg_off + (size_t)E.ev * NSEG;
+  E.h0 = so[0];
+  E.nh = (int)(so[NSEG] - E.h0);
+  if (tid <= NSEG) H.seg[tid] = (int)(so[tid] - E.h0);
+  if (tid < 32) { /* longest segment -> number of binary-search steps */
+    int len = (tid < NSEG) ? (int)(so[tid + 1] - so[tid]) : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) len = max(len, __shfl_xor_sync(FULL, len, o));
+    if (tid == 0) H.nsteps = 32 - __clz(len);
+  }
+  const float* gsrc = A.hx + E.h0;
+  E.staged = E.nh + 4 <= A.stage_cap;
+  E.skew = (int)((reinterpret_cast<uintptr_t>(gsrc) >> 2) & 3);
+  if (E.staged) {
+    /* the 16-byte aligned interior goes by TMA, the ragged head/tail by plain loads */
+    const int head = min(E.nh, (4 - E.skew) & 3);
+    const int bulk = (E.nh - head) & ~3;
+    const int tail = E.nh - head - bulk;
+    if (tid == 0 && bulk > 0) {
+      fence_proxy_async();
+      mbar_expect_tx(&H.mbar, (uint32_t)bulk * 4u);
+      bulk_g2s(buf + E.skew + head, gsrc + head, (uint32_t)bulk * 4u, &H.mbar);
+    }
+    if (tid < head) buf[E.skew + tid] = gsrc[tid];
+    if (tid >= 32 && tid < 32 + tail) buf[E.skew + head + bulk + (tid - 32)] = gsrc[head + bulk + (tid - 32)];
+    if (bulk > 0) {
+      if (tid == 0) mbar_wait(&H.mbar, phase); /* one thread polls; the barrier below publishes */
+      phase ^= 1u;
+    }
+  }
+  __syncthreads();
+  return true;
+}
+
+/* Branch-free binary search over the x-sorted range [b, e): b + number of leading elements with
+ * x < v (inclusive == false: lower bound) or x <= v (inclusive == true: upper bound).
+ * Needs 2^nsteps > e - b. */
+template <class HV>
+__device__ __forceinline__ int bound_search(const HV& hx, int b, int e, float v, bool inclusive, int nsteps) {
+  int pos = b;
+  for (int s = nsteps - 1; s >= 0; --s) {
+    const int probe = pos + (1 << s);
+    if (probe <= e) {
+      const float xm = hx[probe - 1];
+      if (inclusive ? (xm <= v) : (xm < v)) pos = probe;
+    }
+  }
+  return pos;
+}
+
+/* Closest hit to `pred` in the x-sorted window [f, f+n), n <= 32: first x >= pred by binary search,
+ * then compare the two neighbours; ties -> lower index, including runs of equal distance on the low
+ * side (equals a linear argmin with strict '<').  Returns the event-relative index, or -1 if n == 0. */
 template <class HV>
 __device__ __forceinline__ int closest_hit(const HV& hx, int f, int n, float pred) {
   if (n <= 0) return -1;
-  int pos = f, cnt = n;
-  while (cnt > 0) {
-    const int half = cnt >> 1;
-    const int mid = pos + half;
-    if (hx[mid] < pred) { pos = mid + 1; cnt -= half + 1; } else { cnt = half; }
+  const int e = f + n;
+  int pos = f;
+#pragma unroll
+  for (int s = 5; s >= 0; --s) {
+    const int probe = pos + (1 << s);
+    if (probe <= e && hx[probe - 1] < pred) pos = probe;
   }
-  int k;
-  if (pos == f) {
-    k = f;
-  } else {
-    k = pos - 1;
-    float dk = pred - hx[k];
-    if (pos < f + n) {
-      const float dh = hx[pos] - pred;
-      if (!(dk <= dh)) return pos;
-    }
-    while (k > f && (pred - hx[k - 1]) == dk) --k;
+  if (pos == f) return f;
+  int k = pos - 1;
+  const float dk = pred - hx[k];
+  if (pos < e) {
+    const float dh = hx[pos] - pred;
+    if (!(dk <= dh)) return pos;
   }
+  while (k > f && (pred - hx[k - 1]) == dk) --k;
   return k;
 }
 
+/* ============================================================================================
+ * a1/a2: search windows.  One thread per (seed, layer, edge).
+ * ============================================================================================ */
+template <bool DEBUG, bool STAGED>
+__device__ __forceinline__ void windows_of_event(const Consts& C, const EventArgs& A, const CtaHeader& H,
+                                                 const EventCtx& E, const HitView<STAGED>& hx) {
+  const int tid = threadIdx.x;
+  const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
+  const int n_items = (int)(s1 - s0) * NSEG;
+  const int nsteps = H.nsteps;
+  const bool pol_pos = C.polarity > 0;
+  for (int base = 0; base < n_items; base += WIN_THREADS) {
+    const int it = base + tid;
+    const bool act = it < n_items;
+    const int sl = act ? it / NSEG : 0;
+    const int j = act ? it - sl * NSEG : 0;
+    const int layer = j >> 1;
+    const bool upper = (j & 1) != 0;
+    const uint32_t seed = s0 + (uint32_t)sl;
+    /* a1: pT-kick extrapolation */
+    const float x = __ldg(A.sx + seed), y = __ldg(A.sy + seed), tx = __ldg(A.stx + seed), ty = __ldg(A.sty + seed);
+    const float qop = __ldg(A.sqop + seed);
+    const float aq = fmaxf(fabsf(qop), 1e-6f);
+    const float x_mag = x + tx * C.mag_dz_seed;
+    const float txp = tx + C.kick * qop;
+    const int zone = (ty >= 0.0f) ? 1 : 0;
+    const float xc = x_mag + txp * C.dzm[layer];
+    float lo, hi;
+    if (!is_uv(layer)) { /* PAPER.md:181-200, Eq. (3) */
+      const float x_tol = C.xtol_base + C.xtol_inv_p * aq;
+      const bool q_pos = qop > 0.0f;
+      const float a_left = (q_pos == pol_pos) ? C.x_asym : 0.0f;
+      const float a_right = (q_pos != pol_pos) ? C.x_asym : 0.0f;
+      lo = (xc - x_tol) - a_left;
+      hi = (xc + x_tol) + a_right;
+    } else { /* PAPER.md:202 */
+      const float yl = y + ty * C.dzs[layer];
+      const float ctr = xc + yl * C.tana[layer];
+      lo = ctr - C.uv_half_width;
+      hi = ctr + C.uv_half_width;
+    }
+    const int sb = H.seg[layer * 2 + zone], se = H.seg[layer * 2 + zone + 1];
+    /* lower edge: first x >= lo; upper edge: first x > hi */
+    const int pos = bound_search(hx, sb, act ? se : sb, upper ? hi : lo, upper, nsteps);
+    const int other = __shfl_xor_sync(FULL, pos, 1);
+    int first = upper ? other : pos;
+    int last = upper ? pos : other;
+    if (last < first) last = first;
+    /* cap to n_window hits, index-symmetric about the geometric centre */
+    const bool capped = act && (last - first > C.n_window);
+    if (__any_sync(FULL, capped)) {
+      const float midv = (lo + hi) * 0.5f;
+      const int cpos = bound_search(hx, first, capped ? last : first, midv, false, nsteps);
+      if (capped) {
+        const int halfw = C.n_window / 2;
+        const int f2 = max(first, cpos - halfw);
+        const int l2 = min(last, cpos + halfw);
+        first = f2;
+        last = l2;
+      }
+    }
+    if (act && !upper) {
+      A.win[(size_t)seed * NL + layer] = ((uint32_t)first << 6) | (uint32_t)(last - first);
+      if (DEBUG) {
+        if (A.dbg.win_first) A.dbg.win_first[(size_t)seed * NL + layer] = (int32_t)(E.h0 + first);
+        if (A.dbg.win_count) A.dbg.win_count[(size_t)seed * NL + layer] = last - first;
+      }
+    }
+  }
+}
+
+template <bool DEBUG>
+__global__ void __launch_bounds__(WIN_THREADS) lf_window_kernel(const __grid_constant__ Consts C,
+                                                                const __grid_constant__ EventArgs A) {
+  CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
+  if (threadIdx.x == 0) mbar_init(&H.mbar, 1);
+  uint32_t phase = 0;
+  EventCtx E;
+  while (fetch_event(A, phase, E)) {
+    if (E.staged) windows_of_event<DEBUG, true>(C, A, H, E, HitView<true>{E.skew});
+    else windows_of_event<DEBUG, false>(C, A, H, E, HitView<false>{A.hx + E.h0});
+  }
+}
+
+/* ============================================================================================
+ * a3: triplet seeding.  One warp per seed.
+ * ============================================================================================ */
+struct __align__(16) SeedScratch {
+  unsigned long long trip[TRIP_BUF];
+  uint16_t dq[64];
+};
+
 /* Rank selection on the warp's triplet keys: keeps the `keep` smallest of `n` (<= TRIP_BUF) unique
  * 64-bit keys and leaves them SORTED ascending in W.trip[0..min(n,keep)).  PAPER.md:221. */
-__device__ __forceinline__ int select_smallest(WarpScratch& W, int n, int keep, int lane) {
+__device__ __forceinline__ int select_smallest(SeedScratch& W, int n, int keep, int lane) {
   const unsigned long long k0 = (lane < n) ? W.trip[lane] : ~0ull;
   const unsigned long long k1 = (lane + 32 < n) ? W.trip[lane + 32] : ~0ull;
   int r0 = 0, r1 = 0;
@@ -190,18 +350,18 @@ __device__ __forceinline__ int select_smallest(WarpScratch& W, int n, int keep, 
 
 /* Finishes the queued doublets, one per lane: x1_expected, closest h1, chi2 cut. */
 template <class HV>
-__device__ __forceinline__ void finish_doublets(const Consts& C, const HV& hx, WarpScratch& W,
-                                                int qcount, int& tcount, int wf, int wn, int lane) {
+__device__ __forceinline__ void finish_doublets(const Consts& C, const HV& hx, SeedScratch& W, int qcount, int& tcount,
+                                                uint32_t winw, int lane) {
   for (int base = 0; base < qcount; base += 32) {
     const int e = base + lane;
     const bool act = e < qcount;
     const unsigned code = act ? W.dq[e] : 0u;
     const int set = (code >> 10) & 1, i0 = (code >> 5) & 31, i2 = code & 31;
     const int la = set ? 3 : 0;
-    const int fa = __shfl_sync(FULL, wf, la);
-    const int fb = __shfl_sync(FULL, wf, la + 4);
-    const int nb = __shfl_sync(FULL, wn, la + 4);
-    const int fc = __shfl_sync(FULL, wf, la + 8);
+    const int fa = (int)(__shfl_sync(FULL, winw, la) >> 6);
+    const uint32_t wb = __shfl_sync(FULL, winw, la + 4);
+    const int fc = (int)(__shfl_sync(FULL, winw, la + 8) >> 6);
+    const int fb = (int)(wb >> 6), nb = (int)(wb & 63u);
     bool pass = false;
     unsigned long long key = 0;
     if (act) {
@@ -230,270 +390,235 @@ __device__ __forceinline__ void finish_doublets(const Consts& C, const HV& hx, W
   }
 }
 
-/* One warp follows one seed through a1..a6 and leaves its record in the per-seed workspace. */
 template <bool DEBUG, class HV>
-__device__ __forceinline__ void process_seed(const Consts& C, const TrackArgs& A, const CtaShared& S,
-                                             const HV& hx, uint32_t h0, uint32_t seed,
-                                             WarpScratch& W, int lane) {
-  /* ---- a1: pT-kick extrapolation */
-  const float x = A.sx[seed], y = A.sy[seed], tx = A.stx[seed], ty = A.sty[seed], qop = A.sqop[seed];
+__device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& A, const HV& hx, uint32_t h0,
+                                              uint32_t seed, SeedScratch& W, int lane) {
+  const float x = __ldg(A.sx + seed), tx = __ldg(A.stx + seed), qop = __ldg(A.sqop + seed);
   const float aq = fmaxf(fabsf(qop), 1e-6f);
   const float p = 1.0f / aq;
   const float x_mag = x + tx * C.mag_dz_seed;
-  const float txp = tx + C.kick * qop;
-  const int zone = (ty >= 0.0f) ? 1 : 0;
-  /* ---- a2: windows.  lanes 0..11: lower edge of layer `lane`; lanes 12..23: upper edge */
-  const float x_tol = C.xtol_base + C.xtol_inv_p * aq;
-  const bool q_pos = qop > 0.0f, pol_pos = C.polarity > 0;
-  const float a_left = (q_pos == pol_pos) ? C.x_asym : 0.0f; /* Eq. (3) */
-  const float a_right = (q_pos != pol_pos) ? C.x_asym : 0.0f;
-  const int wl = lane < 12 ? lane : (lane < 24 ? lane - 12 : 0);
-  const bool wuv = is_uv(wl);
-  const float d_reg = S.g_d[wl], w_reg = S.g_w[wl];
-  const float xc = x_mag + txp * S.g_dzm[wl];
-  const float yl = y + ty * S.g_dzs[wl];
-  const float yt = wuv ? yl * S.g_tana[wl] : 0.0f;
-  float lo, hi;
-  if (!wuv) {
-    lo = (xc - x_tol) - a_left;
-    hi = (xc + x_tol) + a_right;
-  } else {
-    const float ctr = xc + yt;
-    lo = ctr - C.uv_half_width;
-    hi = ctr + C.uv_half_width;
-  }
-  const int sb = S.seg[wl * 2 + zone], se = S.seg[wl * 2 + zone + 1];
-  /* lower edge: first x >= lo; upper edge: first x > hi */
-  const bool upper = lane >= 12;
-  const float v = upper ? hi : lo;
-  int pos = sb, cnt = (lane < 24) ? (se - sb) : 0;
-  while (__any_sync(FULL, cnt > 0)) {
-    if (cnt > 0) {
-      const int half = cnt >> 1;
-      const int mid = pos + half;
-      const float xm = hx[mid];
-      const bool right = upper ? (xm <= v) : (xm < v);
-      if (right) { pos = mid + 1; cnt -= half + 1; } else { cnt = half; }
-    }
-  }
-  int first = __shfl_sync(FULL, pos, wl);
-  int last = __shfl_sync(FULL, pos, wl + 12);
-  if (last < first) last = first;
-  /* cap to n_window hits, index-symmetric about the geometric centre */
-  const bool capped = (lane < 12) && (last - first > C.n_window);
-  {
-    const float midv = (lo + hi) * 0.5f;
-    int cpos = first, ccnt = capped ? (last - first) : 0;
-    while (__any_sync(FULL, ccnt > 0)) {
-      if (ccnt > 0) {
-        const int half = ccnt >> 1;
-        const int mid = cpos + half;
-        if (hx[mid] < midv) { cpos = mid + 1; ccnt -= half + 1; } else { ccnt = half; }
-      }
-    }
-    if (capped) {
-      const int halfw = C.n_window / 2;
-      const int f2 = max(first, cpos - halfw);
-      const int l2 = min(last, cpos + halfw);
-      first = f2;
-      last = l2;
-    }
-  }
-  const int wf = first;        /* event-relative index of the window's first hit (lanes 0..11) */
-  const int wn = last - first; /* hits in the window */
-  if (DEBUG && lane < 12) {
-    if (A.dbg.win_first) A.dbg.win_first[(size_t)seed * NL + lane] = (int32_t)(h0 + wf);
-    if (A.dbg.win_count) A.dbg.win_count[(size_t)seed * NL + lane] = wn;
-  }
-
-  /* ---- a3: triplet seeding */
+  /* lanes 0..11 hold the packed window of layer `lane` */
+  const uint32_t winw = (lane < NL) ? A.win[(size_t)seed * NL + lane] : 0u;
   int qcount = 0, tcount = 0;
   const unsigned lt_mask = (1u << lane) - 1u;
   const bool low_p = p < C.p_same_bend;
   const float tol0 = C.mag_tol_base + C.mag_tol_inv_p * aq;
-#pragma unroll
+#pragma unroll 1
   for (int set = 0; set < 2; ++set) {
     const int la = set ? 3 : 0;
-    const int fa = __shfl_sync(FULL, wf, la), na = __shfl_sync(FULL, wn, la);
-    const int nb = __shfl_sync(FULL, wn, la + 4);
-    const int fc = __shfl_sync(FULL, wf, la + 8), nc = __shfl_sync(FULL, wn, la + 8);
-    if (na > 0 && nb > 0 && nc > 0) {
-      const float x2 = (lane < nc) ? hx[fc + lane] : 0.0f;
-      const float xa = (lane < na) ? hx[fa + lane] : 0.0f;
-      const float inv_dz = C.inv_dz_ac[set], zmag_a = C.zmag_a[set];
-      for (int i0 = 0; i0 < na; ++i0) {
-        const float x0 = __shfl_sync(FULL, xa, i0);
-        const float t = (x2 - x0) * inv_dz;
-        bool ok = lane < nc;
-        /* filter 1: same bending direction below p_same_bend */
-        if (low_p) ok = ok && ((t - tx) * qop > 0.0f);
-        /* filter 2: opening at the magnet centre */
-        const float x_at_mag = x0 + t * zmag_a;
-        const float tol = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * fabsf(t));
-        ok = ok && (fabsf(x_at_mag - x_mag) < tol);
-        const unsigned m = __ballot_sync(FULL, ok);
-        if (m) {
-          if (ok) W.dq[qcount + __popc(m & lt_mask)] = (uint16_t)((set << 10) | (i0 << 5) | lane);
-          qcount += __popc(m);
-          if (qcount > 32) {
-            __syncwarp();
-            finish_doublets(C, hx, W, qcount, tcount, wf, wn, lane);
-            qcount = 0;
-          }
+    const uint32_t wa = __shfl_sync(FULL, winw, la), wb = __shfl_sync(FULL, winw, la + 4), wc = __shfl_sync(FULL, winw, la + 8);
+    const int fa = (int)(wa >> 6), na = (int)(wa & 63u), nb = (int)(wb & 63u);
+    const int fc = (int)(wc >> 6), nc = (int)(wc & 63u);
+    if (na == 0 || nb == 0 || nc == 0) continue;
+    const float inv_dz = C.inv_dz_ac[set], zmag_a = C.zmag_a[set], inv_r = C.inv_r[set];
+    /* lanes = h0.  |x0 + t*zmag_a - x_mag| < tol is linear in x2 (t = (x2-x0)*inv_dz, slope
+     * r = inv_dz*zmag_a < 0) and tol <= tol_sup, so the survivors lie inside
+     * x2 in (x0 + (tol_sup - A)/r, x0 + (-tol_sup - A)/r), A = x0 - x_mag.  The margin in tol_sup
+     * (0.1 mm >> fp32 rounding of these expressions) makes the bracket a strict superset. */
+    const bool have = lane < na;
+    const float x0 = have ? hx[fa + lane] : 0.0f;
+    const float xc_lo = hx[fc], xc_hi = hx[fc + nc - 1];
+    const float tmax = fmaxf(fabsf((xc_lo - x0) * inv_dz), fabsf((xc_hi - x0) * inv_dz));
+    const float tol_sup = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * tmax) + INTERVAL_MARGIN;
+    const float Aoff = x0 - x_mag;
+    const float x2_lo = x0 + (tol_sup - Aoff) * inv_r;
+    const float x2_hi = x0 + (-tol_sup - Aoff) * inv_r;
+    const int ec = fc + nc;
+    int j = ec;
+    if (have) {
+      j = fc;
+#pragma unroll
+      for (int s = 5; s >= 0; --s) {
+        const int probe = j + (1 << s);
+        if (probe <= ec && hx[probe - 1] < x2_lo) j = probe;
+      }
+    }
+    /* walk the bracket; the exact predicate below is the definition */
+    bool more = j < ec;
+    while (__any_sync(FULL, more)) {
+      bool ok = false;
+      if (more) {
+        const float x2 = hx[j];
+        if (x2 > x2_hi) {
+          more = false;
+        } else {
+          const float t = (x2 - x0) * inv_dz;
+          ok = true;
+          if (low_p) ok = (t - tx) * qop > 0.0f; /* filter 1: same bending direction */
+          const float x_at_mag = x0 + t * zmag_a;
+          const float tol = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * fabsf(t));
+          ok = ok && (fabsf(x_at_mag - x_mag) < tol); /* filter 2: opening at the magnet centre */
+        }
+      }
+      const unsigned m = __ballot_sync(FULL, ok);
+      if (m) {
+        if (ok) W.dq[qcount + __popc(m & lt_mask)] = (uint16_t)((set << 10) | (lane << 5) | (j - fc));
+        qcount += __popc(m);
+        if (qcount > 32) {
+          __syncwarp();
+          finish_doublets(C, hx, W, qcount, tcount, winw, lane);
+          qcount = 0;
+        }
+      }
+      if (more) {
+        ++j;
+        more = j < ec;
+      }
+    }
+  }
+  __syncwarp();
+  if (qcount > 0) finish_doublets(C, hx, W, qcount, tcount, winw, lane);
+  if (tcount > 0) tcount = select_smallest(W, tcount, C.n_triplets, lane); /* sorted in (chi2,set,h0,h2) order */
+  const int ntr = tcount;
+  const int NT = C.n_triplets;
+  if (lane == 0) A.n_trip[seed] = (uint8_t)ntr;
+  const bool mine = lane < ntr;
+  const unsigned long long key = mine ? W.trip[lane] : 0ull;
+  if (lane < NT) A.trip_code[(size_t)seed * NT + lane] = (uint16_t)((unsigned)key & 0xFFFFu);
+  if (DEBUG) {
+    const unsigned low = (unsigned)key;
+    const int set = (low >> 15) & 1, la = set ? 3 : 0;
+    const int fa = (int)(__shfl_sync(FULL, winw, la) >> 6), fb = (int)(__shfl_sync(FULL, winw, la + 4) >> 6);
+    const int fc = (int)(__shfl_sync(FULL, winw, la + 8) >> 6);
+    if (lane == 0 && A.dbg.n_triplets) A.dbg.n_triplets[seed] = ntr;
+    if (lane < NT) {
+      const size_t o = (size_t)seed * NT + lane;
+      if (A.dbg.trip_set) A.dbg.trip_set[o] = mine ? set : -1;
+      if (A.dbg.trip_chi2) A.dbg.trip_chi2[o] = mine ? __uint_as_float((unsigned)(key >> 32)) : -1.0f;
+      if (A.dbg.trip_hits) {
+        A.dbg.trip_hits[o * 3 + 0] = mine ? (int32_t)(h0 + fa + ((low >> 10) & 31)) : -1;
+        A.dbg.trip_hits[o * 3 + 1] = mine ? (int32_t)(h0 + fb + (low & 31)) : -1;
+        A.dbg.trip_hits[o * 3 + 2] = mine ? (int32_t)(h0 + fc + ((low >> 5) & 31)) : -1;
+      }
+    }
+  }
+  __syncwarp();
+}
+
+struct __align__(16) SeedTables {
+  int next_seed;
+  int pad[3];
+  SeedScratch ws[SEED_WARPS];
+};
+
+template <bool DEBUG>
+__global__ void __launch_bounds__(SEED_THREADS) lf_seed_kernel(const __grid_constant__ Consts C,
+                                                               const __grid_constant__ EventArgs A) {
+  CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
+  SeedTables& T = *reinterpret_cast<SeedTables*>(lf_smem + HDR_BYTES + (size_t)A.stage_cap * sizeof(float));
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (threadIdx.x == 0) {
+    mbar_init(&H.mbar, 1);
+    T.next_seed = 0;
+  }
+  uint32_t phase = 0;
+  EventCtx E;
+  while (fetch_event(A, phase, E)) {
+    const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
+    SeedScratch& W = T.ws[warp];
+    for (;;) {
+      int k = 0;
+      if (lane == 0) k = atomicAdd(&T.next_seed, 1);
+      k = __shfl_sync(FULL, k, 0);
+      if (s0 + (uint32_t)k >= s1) break;
+      if (E.staged) seed_triplets<DEBUG>(C, A, HitView<true>{E.skew}, E.h0, s0 + (uint32_t)k, W, lane);
+      else seed_triplets<DEBUG>(C, A, HitView<false>{A.hx + E.h0}, E.h0, s0 + (uint32_t)k, W, lane);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) T.next_seed = 0; /* published by fetch_event's barriers */
+  }
+}
+
+/* ============================================================================================
+ * a4-a6: extension, fit, quality, best per seed.  One thread per candidate, then one per seed.
+ * ============================================================================================ */
+struct FitOut {
+  float Q;
+  bool enough, ty_ok;
+};
+
+/* Evaluates candidate `code` of a seed: extension to the 9 other layers, hit-count rule, fit, Q.
+ * With `rec` != nullptr also computes q/p and the state and writes the 20-word track record. */
+template <bool DEBUG, class HV>
+__device__ __noinline__ FitOut eval_candidate(const Consts& C, const HV& hx, const uint32_t* winw, float y, float tx,
+                                              float ty, unsigned code, uint32_t h0, int32_t* rec, uint32_t seed,
+                                              int32_t* dbg_hits) {
+  const int set = (code >> 15) & 1, la = set ? 3 : 0;
+  int idx[NL];   /* event-relative hit index per layer or -1 */
+  float sv[NL];  /* its stored coordinate */
+  /* Eq. (4) parameters: exact parabola through the three triplet hits */
+  const int i0 = (int)(winw[la] >> 6) + (int)((code >> 10) & 31);
+  const int i1 = (int)(winw[la + 4] >> 6) + (int)(code & 31);
+  const int i2 = (int)(winw[la + 8] >> 6) + (int)((code >> 5) & 31);
+  const float x0 = hx[i0], x1 = hx[i1], x2 = hx[i2];
+  const float X10 = x1 - x0, X20 = x2 - x0;
+  const float D10 = set ? C.D10[1] : C.D10[0], D20 = set ? C.D20[1] : C.D20[0];
+  const float W10 = set ? C.W10[1] : C.W10[0];
+  const float c0 = (X20 * D10 - X10 * D20) * (set ? C.inv_det[1] : C.inv_det[0]);
+  const float t0 = (X10 - c0 * W10) * (set ? C.inv_D10[1] : C.inv_D10[0]);
+  const float a0 = (x0 - t0 * (set ? C.d[3] : C.d[0])) - c0 * (set ? C.w[3] : C.w[0]);
+  const float T_uv = fmaxf(C.T_uv_min, C.T_uv_slope * (fabsf(tx) + fabsf(ty)));
+  int n = 0, n_uv = 0;
+  bool st_uv[3] = {false, false, false};
+  float yt[NL];
+#pragma unroll
+  for (int l = 0; l < NL; ++l) {
+    const bool uv = is_uv(l);
+    yt[l] = uv ? (y + ty * C.dzs[l]) * C.tana[l] : 0.0f;
+    idx[l] = -1;
+    sv[l] = 0.0f;
+    if (!uv && (l & 3) == la) { /* the triplet's own layers: la, la+4, la+8 */
+      idx[l] = (l < 4) ? i0 : (l < 8 ? i1 : i2);
+      sv[l] = (l < 4) ? x0 : (l < 8 ? x1 : x2);
+      ++n;
+    } else {
+      float pred = (a0 + t0 * C.d[l]) + c0 * C.w[l];
+      if (uv) pred = pred + yt[l];
+      const uint32_t ww = winw[l];
+      const int k = closest_hit(hx, (int)(ww >> 6), (int)(ww & 63u), pred);
+      if (k >= 0) {
+        const float xk = hx[k];
+        const float dx = xk - pred;
+        const float chi2 = dx * dx;
+        if (chi2 < (uv ? T_uv : C.T_x)) {
+          idx[l] = k;
+          sv[l] = xk;
+          ++n;
+          if (uv) { ++n_uv; st_uv[l >> 2] = true; }
         }
       }
     }
   }
-  __syncwarp();
-  if (qcount > 0) finish_doublets(C, hx, W, qcount, tcount, wf, wn, lane);
-  if (tcount > 0) tcount = select_smallest(W, tcount, C.n_triplets, lane); /* sorted in (chi2,set,h0,h2) order */
-  const int ntr = tcount;
-  const int NT = C.n_triplets;
-
-  if (DEBUG) {
-    /* triplet table; hit indices need the window bases held by lanes 0..11, so every lane shuffles */
-    const bool have = lane < ntr;
-    const unsigned long long key = have ? W.trip[lane] : 0ull;
-    const unsigned low = (unsigned)key;
-    const int set = (low >> 15) & 1, la = set ? 3 : 0;
-    const int fa = __shfl_sync(FULL, wf, la), fb = __shfl_sync(FULL, wf, la + 4), fc = __shfl_sync(FULL, wf, la + 8);
-    if (lane == 0 && A.dbg.n_triplets) A.dbg.n_triplets[seed] = ntr;
-    if (lane < NT) {
-      const size_t o = (size_t)seed * NT + lane;
-      if (A.dbg.trip_set) A.dbg.trip_set[o] = have ? set : -1;
-      if (A.dbg.trip_chi2) A.dbg.trip_chi2[o] = have ? __uint_as_float((unsigned)(key >> 32)) : -1.0f;
-      if (A.dbg.trip_hits) {
-        A.dbg.trip_hits[o * 3 + 0] = have ? (int32_t)(h0 + fa + ((low >> 10) & 31)) : -1;
-        A.dbg.trip_hits[o * 3 + 1] = have ? (int32_t)(h0 + fb + (low & 31)) : -1;
-        A.dbg.trip_hits[o * 3 + 2] = have ? (int32_t)(h0 + fc + ((low >> 5) & 31)) : -1;
-      }
-      if (A.dbg.cand_quality) A.dbg.cand_quality[o] = -1.0f;
-      if (A.dbg.cand_hits)
-        for (int l = 0; l < NL; ++l) A.dbg.cand_hits[o * NL + l] = -1;
-    }
-  }
-
-  if (ntr == 0) {
-    if (lane == 0) A.ws_nh[seed] = 0;
-    return;
-  }
-
-  /* ---- a4/a5: extension, lanes = (triplet, other layer) */
-  const float T_uv = fmaxf(C.T_uv_min, C.T_uv_slope * (fabsf(tx) + fabsf(ty)));
-  for (int base = 0; base < ntr * 9; base += 32) {
-    const int tau = base + lane;
-    const bool act = tau < ntr * 9;
-    const int trip = act ? tau / 9 : 0;
-    const int li = act ? tau - trip * 9 : 0;
-    const unsigned low = (unsigned)W.trip[trip];
-    const int set = (low >> 15) & 1, i0 = (low >> 10) & 31, i2 = (low >> 5) & 31, i1 = low & 31;
-    const int la = set ? 3 : 0;
-    const int l = li + li / 3 + (1 - set); /* the 9 layers outside the set, ascending */
-    const int fa = __shfl_sync(FULL, wf, la), fb = __shfl_sync(FULL, wf, la + 4), fc = __shfl_sync(FULL, wf, la + 8);
-    const int fl = __shfl_sync(FULL, wf, l), nl = __shfl_sync(FULL, wn, l);
-    const float yt_l = __shfl_sync(FULL, yt, l);
-    const float d_l = __shfl_sync(FULL, d_reg, l), w_l = __shfl_sync(FULL, w_reg, l);
-    if (act) {
-      /* Eq. (4) parameters: exact parabola through the three triplet hits */
-      const float x0 = hx[fa + i0], x1 = hx[fb + i1], x2 = hx[fc + i2];
-      const float X10 = x1 - x0, X20 = x2 - x0;
-      const float D10 = set ? C.D10[1] : C.D10[0], D20 = set ? C.D20[1] : C.D20[0];
-      const float W10 = set ? C.W10[1] : C.W10[0];
-      const float c0 = (X20 * D10 - X10 * D20) * (set ? C.inv_det[1] : C.inv_det[0]);
-      const float t0 = (X10 - c0 * W10) * (set ? C.inv_D10[1] : C.inv_D10[0]);
-      const float a0 = (x0 - t0 * (set ? C.d[3] : C.d[0])) - c0 * (set ? C.w[3] : C.w[0]);
-      const bool uv = is_uv(l);
-      float pred = (a0 + t0 * d_l) + c0 * w_l;
-      if (uv) pred = pred + yt_l;
-      const int k = closest_hit(hx, fl, nl, pred);
-      unsigned code = NO_HIT;
-      if (k >= 0) {
-        const float dx = hx[k] - pred;
-        const float chi2 = dx * dx;
-        if (chi2 < (uv ? T_uv : C.T_x)) code = (unsigned)(k - fl);
-      }
-      W.ext[trip][l] = (uint8_t)code;
-      if (li == 0) {
-        W.ext[trip][la] = (uint8_t)i0;
-        W.ext[trip][la + 4] = (uint8_t)i1;
-        W.ext[trip][la + 8] = (uint8_t)i2;
-      }
-    }
-  }
-  __syncwarp();
-
-  /* ---- a6: lanes = candidates.  Hit-count rule, fit, Q */
-  const bool cand = lane < ntr;
-  const int row = cand ? lane : 0;
-  const uint32_t* rowp = reinterpret_cast<const uint32_t*>(&W.ext[row][0]);
-  const uint32_t cw0 = rowp[0], cw1 = rowp[1], cw2 = rowp[2];
-  int n = 0, n_uv = 0;
-  bool st_uv[3] = {false, false, false};
+  if (DEBUG && dbg_hits) {
 #pragma unroll
-  for (int l = 0; l < NL; ++l) {
-    const uint32_t wsel = (l < 4) ? cw0 : (l < 8 ? cw1 : cw2);
-    const bool present = ((wsel >> (8 * (l & 3))) & 0xFFu) != NO_HIT;
-    if (present) {
-      ++n;
-      if (is_uv(l)) { ++n_uv; st_uv[l >> 2] = true; }
-    }
+    for (int l = 0; l < NL; ++l) dbg_hits[l] = idx[l] >= 0 ? (int32_t)(h0 + idx[l]) : -1;
   }
-  const bool enough = cand && (n >= C.min_hits) && st_uv[0] && st_uv[1] && st_uv[2];
+  FitOut out;
+  out.Q = 0.0f;
+  out.ty_ok = false;
+  /* at least min_hits hits and at least one u/v hit per station */
+  out.enough = (n >= C.min_hits) && st_uv[0] && st_uv[1] && st_uv[2];
+  if (!out.enough) return out;
 
-  if (DEBUG && A.dbg.cand_hits) {
-#pragma unroll
-    for (int l = 0; l < NL; ++l) {
-      const uint32_t wsel = (l < 4) ? cw0 : (l < 8 ? cw1 : cw2);
-      const unsigned code = (wsel >> (8 * (l & 3))) & 0xFFu;
-      const int f_l = __shfl_sync(FULL, wf, l);
-      if (cand) A.dbg.cand_hits[((size_t)seed * NT + lane) * NL + l] = (code != NO_HIT) ? (int32_t)(h0 + f_l + code) : -1;
-    }
-  }
-
-  if (!__any_sync(FULL, enough)) {
-    if (lane == 0) A.ws_nh[seed] = 0;
-    return;
-  }
-
-  /* triplet parabola again, now for the candidate this lane owns */
-  const unsigned low = (unsigned)W.trip[row];
-  const int set = (low >> 15) & 1, la = set ? 3 : 0;
-  float a0, t0, c0;
-  {
-    const int fa = __shfl_sync(FULL, wf, la), fb = __shfl_sync(FULL, wf, la + 4), fc = __shfl_sync(FULL, wf, la + 8);
-    const float x0 = hx[fa + ((low >> 10) & 31)], x1 = hx[fb + (low & 31)], x2 = hx[fc + ((low >> 5) & 31)];
-    const float X10 = x1 - x0, X20 = x2 - x0;
-    const float D10 = set ? C.D10[1] : C.D10[0], D20 = set ? C.D20[1] : C.D20[0];
-    const float W10 = set ? C.W10[1] : C.W10[0];
-    c0 = (X20 * D10 - X10 * D20) * (set ? C.inv_det[1] : C.inv_det[0]);
-    t0 = (X10 - c0 * W10) * (set ? C.inv_D10[1] : C.inv_D10[0]);
-    a0 = (x0 - t0 * (set ? C.d[3] : C.d[0])) - c0 * (set ? C.w[3] : C.w[0]);
-  }
   const float inv_Tuv = 1.0f / T_uv;
   /* x fit on the residuals to the triplet parabola: sums in ascending layer order */
   float r[NL];
   float S1 = 0.f, Sd = 0.f, Sw = 0.f, Sdd = 0.f, Sdw = 0.f, Sww = 0.f, Sr = 0.f, Sdr = 0.f, Swr = 0.f;
 #pragma unroll
   for (int l = 0; l < NL; ++l) {
-    const uint32_t wsel = (l < 4) ? cw0 : (l < 8 ? cw1 : cw2);
-    const unsigned code = (wsel >> (8 * (l & 3))) & 0xFFu;
-    const bool present = code != NO_HIT;
-    const int f_l = __shfl_sync(FULL, wf, l);
-    const float yt_l = __shfl_sync(FULL, yt, l);
-    const float s_i = hx[present ? (f_l + (int)code) : 0];
-    const float dl = C.d[l], wl_ = C.w[l];
-    const float m = s_i - yt_l;
-    r[l] = m - ((a0 + t0 * dl) + c0 * wl_);
-    if (present) {
+    const float dl = C.d[l], wl = C.w[l];
+    const float m = sv[l] - yt[l];
+    r[l] = m - ((a0 + t0 * dl) + c0 * wl);
+    if (idx[l] >= 0) {
       S1 = S1 + 1.0f;
       Sd = Sd + dl;
-      Sw = Sw + wl_;
+      Sw = Sw + wl;
       Sdd = Sdd + dl * dl;
-      Sdw = Sdw + dl * wl_;
-      Sww = Sww + wl_ * wl_;
+      Sdw = Sdw + dl * wl;
+      Sww = Sww + wl * wl;
       Sr = Sr + r[l];
       Sdr = Sdr + dl * r[l];
-      Swr = Swr + wl_ * r[l];
+      Swr = Swr + wl * r[l];
     }
   }
   const float C00 = Sdd * Sww - Sdw * Sdw;
@@ -511,14 +636,13 @@ __device__ __forceinline__ void process_seed(const Consts& C, const TrackArgs& A
   float Qx = 0.f, U1 = 0.f, Ud = 0.f, Udd = 0.f, Ur = 0.f, Udr = 0.f;
 #pragma unroll
   for (int l = 0; l < NL; ++l) {
-    const uint32_t wsel = (l < 4) ? cw0 : (l < 8 ? cw1 : cw2);
-    const bool present = ((wsel >> (8 * (l & 3))) & 0xFFu) != NO_HIT;
-    const float dl = C.d[l], wl_ = C.w[l];
-    const float e = r[l] - ((da + dt * dl) + dc * wl_);
+    const float dl = C.d[l], wl = C.w[l];
+    const float e = r[l] - ((da + dt * dl) + dc * wl);
     const float chi2 = e * e;
+    rho[l] = 0.f;
     if (is_uv(l)) {
       rho[l] = e * C.inv_tan[l];
-      if (present) {
+      if (idx[l] >= 0) {
         Qx = Qx + chi2 * inv_Tuv;
         U1 = U1 + 1.0f;
         Ud = Ud + dl;
@@ -526,175 +650,197 @@ __device__ __forceinline__ void process_seed(const Consts& C, const TrackArgs& A
         Ur = Ur + rho[l];
         Udr = Udr + dl * rho[l];
       }
-    } else {
-      rho[l] = 0.f;
-      if (present) Qx = Qx + chi2 * C.inv_Tx;
+    } else if (idx[l] >= 0) {
+      Qx = Qx + chi2 * C.inv_Tx;
     }
   }
+  /* y line on the u/v hits */
   const float det2 = U1 * Udd - Ud * Ud;
   const float inv2 = 1.0f / det2;
   const float dy0 = (Udd * Ur - Ud * Udr) * inv2;
   const float dtym = (U1 * Udr - Ud * Ur) * inv2;
   const float dty = dtym * 0.001f;
-  const bool ty_ok = fabsf(dty) < C.T_ty; /* PAPER.md:264 */
+  out.ty_ok = fabsf(dty) < C.T_ty;
   float Qy = 0.f;
 #pragma unroll
   for (int l = 0; l < NL; ++l) {
     if (!is_uv(l)) continue;
-    const uint32_t wsel = (l < 4) ? cw0 : (l < 8 ? cw1 : cw2);
-    const bool present = ((wsel >> (8 * (l & 3))) & 0xFFu) != NO_HIT;
     const float ey = rho[l] - (dy0 + dtym * C.d[l]);
-    if (present) Qy = Qy + (ey * ey) * C.inv_Ty;
+    if (idx[l] >= 0) Qy = Qy + (ey * ey) * C.inv_Ty;
   }
   const int ci = min(3, max(0, n - 9));
   const float Cn = (ci == 0) ? C.C_nhits[0] : (ci == 1 ? C.C_nhits[1] : (ci == 2 ? C.C_nhits[2] : C.C_nhits[3]));
-  const float Q = (Qx / (float)(n - 3) + Qy / (float)(n_uv - 2)) * Cn; /* Eq. (6) */
-  if (DEBUG && enough && A.dbg.cand_quality) A.dbg.cand_quality[(size_t)seed * NT + lane] = ty_ok ? Q : -2.0f;
+  out.Q = (Qx / (float)(n - 3) + Qy / (float)(n_uv - 2)) * Cn; /* Eq. (6) */
 
-  /* PAPER.md:279: accept Q < T_Q, keep the lowest Q; ties -> earlier in (chi2,set,h0,h2) order */
-  const bool valid = enough && ty_ok && (Q < C.T_Q);
-  unsigned long long qk = valid ? (((unsigned long long)__float_as_uint(Q) << 32) | (unsigned)lane) : ~0ull;
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    const unsigned long long other = __shfl_xor_sync(FULL, qk, o);
-    qk = other < qk ? other : qk;
-  }
-  if (qk == ~0ull) {
-    if (lane == 0) A.ws_nh[seed] = 0;
-    return;
-  }
-  const int winner = (int)(qk & 31u);
-  /* record: hit indices need the window bases (lanes 0..11), so every lane shuffles */
-#pragma unroll
-  for (int l = 0; l < NL; ++l) {
-    const uint32_t wsel = (l < 4) ? cw0 : (l < 8 ? cw1 : cw2);
-    const unsigned code = (wsel >> (8 * (l & 3))) & 0xFFu;
-    const int f_l = __shfl_sync(FULL, wf, l);
-    if (lane == winner) W.rec[l] = (code != NO_HIT) ? (int32_t)(h0 + f_l + code) : -1;
-  }
-  if (lane == winner) {
-    /* ---- a6 (cont.): momentum from the slope change (Eq. 9) and the state at z_state */
+  if (rec != nullptr) {
+    /* momentum from the slope change (Eq. 9) and the state at z_state */
     const float a = a0 + da, t = t0 + dt, c = c0 + dc;
     const float t_ref = t * 0.001f;
     const float dslope = t_ref - tx;
     const float F = C.poly[0] + dslope * (C.poly[1] + dslope * (C.poly[2] + dslope * (C.poly[3] + dslope * C.poly[4])));
-    W.rec[12] = (int32_t)seed;
-    W.rec[13] = n;
-    W.rec[14] = __float_as_int((a + t * C.ds) + c * C.ws);
-    W.rec[15] = __float_as_int((y + ty * C.dz_state) + (dy0 + dtym * C.ds));
-    W.rec[16] = __float_as_int((t + c * C.dws) * 0.001f);
-    W.rec[17] = __float_as_int(ty + dtym * 0.001f);
-    W.rec[18] = __float_as_int(dslope / F);
-    W.rec[19] = __float_as_int(Q);
-    A.ws_nh[seed] = n;
+    int4* r4 = reinterpret_cast<int4*>(rec);
+    int o[REC_WORDS];
+#pragma unroll
+    for (int l = 0; l < NL; ++l) o[l] = idx[l] >= 0 ? (int32_t)(h0 + idx[l]) : -1;
+    o[12] = (int32_t)seed;
+    o[13] = n;
+    o[14] = __float_as_int((a + t * C.ds) + c * C.ws);
+    o[15] = __float_as_int((y + ty * C.dz_state) + (dy0 + dtym * C.ds));
+    o[16] = __float_as_int((t + c * C.dws) * 0.001f);
+    o[17] = __float_as_int(ty + dtym * 0.001f);
+    o[18] = __float_as_int(dslope / F);
+    o[19] = __float_as_int(out.Q);
+#pragma unroll
+    for (int q = 0; q < REC_WORDS / 4; ++q) r4[q] = make_int4(o[4 * q], o[4 * q + 1], o[4 * q + 2], o[4 * q + 3]);
   }
-  __syncwarp();
-  if (lane < REC_WORDS) A.ws_rec[(size_t)seed * REC_WORDS + lane] = W.rec[lane];
-  __syncwarp();
+  return out;
+}
+
+/* Per-chunk tables of the fit kernel (after the staged hits in shared memory). */
+struct FitTables {
+  uint32_t* win;   /* FIT_CHUNK*12 packed windows */
+  float* sp;       /* FIT_CHUNK*4: y, tx, ty, (unused) */
+  int* pref;       /* FIT_CHUNK+1: exclusive prefix of candidates per seed */
+  uint16_t* item;  /* FIT_CHUNK*NT: seed_local<<4 | k */
+  float* Q;        /* FIT_CHUNK*NT: Q, or +inf if the candidate is not acceptable */
+};
+__host__ __device__ inline size_t fit_tables_bytes(int nt) {
+  return (size_t)FIT_CHUNK * NL * 4 + (size_t)FIT_CHUNK * 4 * 4 + (size_t)(FIT_CHUNK + 4) * 4 +
+         (((size_t)FIT_CHUNK * nt * 2 + 15) & ~size_t(15)) + (size_t)FIT_CHUNK * nt * 4;
+}
+
+template <bool DEBUG, bool STAGED>
+__device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, CtaHeader& H, const EventCtx& E,
+                                          const HitView<STAGED>& hx, const FitTables& T) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
+  const int ns = (int)(s1 - s0);
+  const int NT = C.n_triplets;
+  const float INF = __int_as_float(0x7f800000);
+  int ev_tracks = 0;
+  for (int cb = 0; cb < ns; cb += FIT_CHUNK) {
+    const int cn = min(FIT_CHUNK, ns - cb);
+    const uint32_t sbase = s0 + (uint32_t)cb;
+    /* ---- stage the chunk's windows, seed parameters and candidate counts */
+    for (int i = tid; i < cn * NL; i += FIT_THREADS) T.win[i] = A.win[(size_t)sbase * NL + i];
+    int my_n = 0;
+    if (tid < cn) {
+      const uint32_t seed = sbase + (uint32_t)tid;
+      T.sp[tid * 4 + 0] = __ldg(A.sy + seed);
+      T.sp[tid * 4 + 1] = __ldg(A.stx + seed);
+      T.sp[tid * 4 + 2] = __ldg(A.sty + seed);
+      my_n = (int)A.n_trip[seed];
+    }
+    /* exclusive prefix of candidate counts over the chunk (FIT_CHUNK == FIT_THREADS) */
+    int incl = my_n;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int v = __shfl_up_sync(FULL, incl, o);
+      if (lane >= o) incl += v;
+    }
+    if (lane == 31) H.warp_tot[warp] = incl;
+    __syncthreads();
+    int woff = 0, total = 0;
+#pragma unroll
+    for (int wq = 0; wq < FIT_THREADS / 32; ++wq) {
+      const int tq = H.warp_tot[wq];
+      woff += (wq < warp) ? tq : 0;
+      total += tq;
+    }
+    const int excl = woff + incl - my_n;
+    if (tid < cn) {
+      T.pref[tid] = excl;
+      for (int k = 0; k < my_n; ++k) T.item[excl + k] = (uint16_t)((tid << 4) | k);
+    }
+    if (tid == 0) T.pref[cn] = total;
+    __syncthreads();
+    /* ---- one thread per candidate: extension + fit + Q */
+    for (int it = tid; it < total; it += FIT_THREADS) {
+      const unsigned im = T.item[it];
+      const int sl = (int)(im >> 4), k = (int)(im & 15u);
+      const uint32_t seed = sbase + (uint32_t)sl;
+      const unsigned code = A.trip_code[(size_t)seed * NT + k];
+      int32_t* dh = (DEBUG && A.dbg.cand_hits) ? A.dbg.cand_hits + ((size_t)seed * NT + k) * NL : nullptr;
+      const FitOut fo = eval_candidate<DEBUG>(C, hx, T.win + sl * NL, T.sp[sl * 4 + 0], T.sp[sl * 4 + 1], T.sp[sl * 4 + 2],
+                                              code, E.h0, nullptr, seed, dh);
+      /* accepted if Q < T_Q (and the t_y cut holds) */
+      T.Q[it] = (fo.enough && fo.ty_ok && (fo.Q < C.T_Q)) ? fo.Q : INF;
+      if (DEBUG && A.dbg.cand_quality) A.dbg.cand_quality[(size_t)seed * NT + k] = fo.enough ? (fo.ty_ok ? fo.Q : -2.0f) : -1.0f;
+    }
+    __syncthreads();
+    /* ---- one thread per seed: lowest Q wins, ties -> earlier in (chi2,set,h0,h2) order */
+    bool found = false;
+    if (tid < cn) {
+      const uint32_t seed = sbase + (uint32_t)tid;
+      const int b = T.pref[tid], e = T.pref[tid + 1];
+      float best = INF;
+      int bk = -1;
+      for (int i = b; i < e; ++i) {
+        const float q = T.Q[i];
+        if (q < best) { best = q; bk = i - b; }
+      }
+      if (DEBUG) {
+        for (int k = e - b; k < NT; ++k) {
+          if (A.dbg.cand_quality) A.dbg.cand_quality[(size_t)seed * NT + k] = -1.0f;
+          if (A.dbg.cand_hits)
+            for (int l = 0; l < NL; ++l) A.dbg.cand_hits[((size_t)seed * NT + k) * NL + l] = -1;
+        }
+      }
+      if (bk >= 0) {
+        const unsigned code = A.trip_code[(size_t)seed * NT + bk];
+        eval_candidate<false>(C, hx, T.win + tid * NL, T.sp[tid * 4 + 0], T.sp[tid * 4 + 1], T.sp[tid * 4 + 2], code, E.h0,
+                              A.ws_rec + (size_t)seed * REC_WORDS, seed, nullptr);
+        found = true;
+      }
+      A.ws_nh[seed] = found ? 1 : 0;
+    }
+    /* ---- rank the chunk's tracks in seed order (a7, first half) */
+    const unsigned m = __ballot_sync(FULL, found);
+    if (lane == 0) H.warp_tot[warp] = __popc(m);
+    __syncthreads();
+    int off = 0, tot = 0;
+#pragma unroll
+    for (int wq = 0; wq < FIT_THREADS / 32; ++wq) {
+      const int tq = H.warp_tot[wq];
+      off += (wq < warp) ? tq : 0;
+      tot += tq;
+    }
+    if (tid < cn) {
+      A.ws_rank[sbase + tid] = found ? (ev_tracks + off + __popc(m & ((1u << lane) - 1u))) : -1;
+      A.ws_event[sbase + tid] = (int32_t)E.ev;
+    }
+    ev_tracks += tot;
+    __syncthreads();
+  }
+  if (tid == 0) A.ev_count[E.ev] = (uint32_t)ev_tracks;
 }
 
 template <bool DEBUG>
-__global__ void __launch_bounds__(CTA_THREADS) lf_track_kernel(const __grid_constant__ Consts C,
-                                                               const __grid_constant__ TrackArgs A) {
-  CtaShared& S = *reinterpret_cast<CtaShared*>(lf_smem);
-  float* buf = stage_buf();
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  if (tid == 0) mbar_init(&S.mbar, 1);
-  if (tid < NL) {
-    S.g_tana[tid] = C.tana[tid];
-    S.g_dzs[tid] = C.dzs[tid];
-    S.g_dzm[tid] = C.dzm[tid];
-    S.g_d[tid] = C.d[tid];
-    S.g_w[tid] = C.w[tid];
-  }
-  __syncthreads();
+__global__ void __launch_bounds__(FIT_THREADS) lf_fit_kernel(const __grid_constant__ Consts C,
+                                                             const __grid_constant__ EventArgs A) {
+  CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
+  unsigned char* tb = lf_smem + HDR_BYTES + (size_t)A.stage_cap * sizeof(float);
+  const int NT = C.n_triplets;
+  FitTables T;
+  T.win = reinterpret_cast<uint32_t*>(tb);
+  T.sp = reinterpret_cast<float*>(tb + (size_t)FIT_CHUNK * NL * 4);
+  T.pref = reinterpret_cast<int*>(tb + (size_t)FIT_CHUNK * NL * 4 + (size_t)FIT_CHUNK * 16);
+  unsigned char* ib = tb + (size_t)FIT_CHUNK * NL * 4 + (size_t)FIT_CHUNK * 16 + (size_t)(FIT_CHUNK + 4) * 4;
+  T.item = reinterpret_cast<uint16_t*>(ib);
+  T.Q = reinterpret_cast<float*>(ib + (((size_t)FIT_CHUNK * NT * 2 + 15) & ~size_t(15)));
+  if (threadIdx.x == 0) mbar_init(&H.mbar, 1);
   uint32_t phase = 0;
-  for (;;) {
-    if (tid == 0) {
-      S.ev = (int)atomicAdd(A.ticket, 1u);
-      S.next_seed = 0;
-    }
-    __syncthreads(); /* (A) previous event fully retired: buf, seg, counters reusable */
-    const uint32_t ev = (uint32_t)S.ev;
-    if (ev >= A.n_events) break;
-    const uint32_t* so = A.seg_off + (size_t)ev * NSEG;
-    const uint32_t h0 = so[0], h1 = so[NSEG];
-    if (tid <= NSEG) S.seg[tid] = (int)(so[tid] - h0);
-    const int nh = (int)(h1 - h0);
-    const float* gsrc = A.hx + h0;
-    const bool staged = nh + 4 <= A.stage_cap;
-    const int skew = (int)((reinterpret_cast<uintptr_t>(gsrc) >> 2) & 3);
-    if (staged) {
-      /* Stage the event: hit i lives at buf[skew + i]; the 16-byte aligned interior goes by TMA. */
-      const int head = min(nh, (4 - skew) & 3);
-      const int bulk = (nh - head) & ~3;
-      const int tail = nh - head - bulk;
-      if (tid == 0 && bulk > 0) {
-        fence_proxy_async();
-        mbar_expect_tx(&S.mbar, (uint32_t)bulk * 4u);
-        bulk_g2s(buf + skew + head, gsrc + head, (uint32_t)bulk * 4u, &S.mbar);
-      }
-      if (tid < head) buf[skew + tid] = gsrc[tid];
-      if (tid >= 32 && tid < 32 + tail) buf[skew + head + bulk + (tid - 32)] = gsrc[head + bulk + (tid - 32)];
-      if (bulk > 0) {
-        mbar_wait(&S.mbar, phase);
-        phase ^= 1u;
-      }
-    }
-    __syncthreads(); /* (B) seg table and head/tail hits visible */
-    const uint32_t s0 = A.seed_off[ev], s1 = A.seed_off[ev + 1];
-    WarpScratch& W = S.ws[warp];
-    if (staged) {
-      const HitView<true> hv{skew};
-      for (;;) {
-        int k = 0;
-        if (lane == 0) k = atomicAdd(&S.next_seed, 1);
-        k = __shfl_sync(FULL, k, 0);
-        if (s0 + (uint32_t)k >= s1) break;
-        process_seed<DEBUG>(C, A, S, hv, h0, s0 + (uint32_t)k, W, lane);
-      }
-    } else {
-      const HitView<false> hv{gsrc};
-      for (;;) {
-        int k = 0;
-        if (lane == 0) k = atomicAdd(&S.next_seed, 1);
-        k = __shfl_sync(FULL, k, 0);
-        if (s0 + (uint32_t)k >= s1) break;
-        process_seed<DEBUG>(C, A, S, hv, h0, s0 + (uint32_t)k, W, lane);
-      }
-    }
-    __syncthreads(); /* (C) every seed of the event has its ws_nh flag */
-    /* rank the event's tracks in seed order (a7, first half) */
-    const int ns = (int)(s1 - s0);
-    int base = 0;
-    for (int c = 0; c < ns; c += CTA_THREADS) {
-      const int i = c + tid;
-      const bool flag = (i < ns) && (__ldcg(A.ws_nh + s0 + i) > 0);
-      const unsigned m = __ballot_sync(FULL, flag);
-      if (lane == 0) S.warp_tot[warp] = __popc(m);
-      __syncthreads();
-      int off = 0, tot = 0;
-#pragma unroll
-      for (int wq = 0; wq < WARPS_PER_CTA; ++wq) {
-        const int tq = S.warp_tot[wq];
-        off += (wq < warp) ? tq : 0;
-        tot += tq;
-      }
-      if (i < ns) {
-        A.ws_rank[s0 + i] = flag ? (base + off + __popc(m & ((1u << lane) - 1u))) : -1;
-        A.ws_event[s0 + i] = (int32_t)ev;
-      }
-      base += tot;
-      __syncthreads();
-    }
-    if (tid == 0) A.ev_count[ev] = (uint32_t)base;
+  EventCtx E;
+  while (fetch_event(A, phase, E)) {
+    if (E.staged) fit_event<DEBUG, true>(C, A, H, E, HitView<true>{E.skew}, T);
+    else fit_event<DEBUG, false>(C, A, H, E, HitView<false>{A.hx + E.h0}, T);
   }
 }
 
-/* Exclusive scan of per-event track counts (single CTA); also re-arms the event ticket. */
+/* Exclusive scan of per-event track counts (single CTA); also re-arms the event tickets. */
 __global__ void __launch_bounds__(1024) lf_scan_kernel(const uint32_t* __restrict__ ev_count, uint32_t n_events,
                                                        uint32_t* __restrict__ ev_off_ws, uint32_t* __restrict__ out_off,
-                                                       uint32_t* __restrict__ n_tracks, uint32_t* ticket) {
+                                                       uint32_t* __restrict__ n_tracks, uint32_t* tickets) {
   __shared__ uint32_t warp_tot[32];
   __shared__ uint32_t carry;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -733,8 +879,8 @@ __global__ void __launch_bounds__(1024) lf_scan_kernel(const uint32_t* __restric
   if (tid == 0) {
     out_off[n_events] = carry;
     *n_tracks = carry;
-    *ticket = 0u;
   }
+  if (tid < N_TICKETS) tickets[tid] = 0u;
 }
 
 /* Stream compaction (a7): one thread per (seed, record word); coalesced reads of the per-seed
