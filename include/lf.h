@@ -142,7 +142,7 @@ typedef struct {
 /* Creates a context for batches of at most max_events / max_seeds / max_hits.  Validates geometry
  * and params, uploads constants, allocates the workspace (about max_seeds*(141 + 2*n_triplets) +
  * max_events*8 bytes on the current CUDA device).  The shared-memory stage for one event's hits is sized
- * from the maxima: 1.5 * max_hits / max_events + 512 hits, clamped to [2048, 16384]; larger events are
+ * from the maxima: 1.25 * max_hits / max_events + 512 hits, clamped to [2048, 16384]; larger events are
  * still processed correctly, reading their hits from global memory.  *out is set only on LF_OK.
  * HOST pointers. */
 lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t max_events,

@@ -273,10 +273,10 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   if (prop.major < 10) return bail(LF_ERR_UNSUPPORTED, "lf_create: this library is built for sm_100a (Blackwell) only");
 
   /* Shared-memory stage for one event's hits, sized from the maxima (include/lf.h, lf_create):
-   * 1.5 x the mean event + 512 hits, clamped to [2048, 16384].  Larger events read global memory. */
+   * 1.25 x the mean event + 512 hits, clamped to [2048, 16384].  Larger events read global memory. */
   {
     const double mean_hits = (double)max_hits / (double)std::max<size_t>(max_events, 1);
-    size_t cap = (size_t)(1.5 * mean_hits) + 512;
+    size_t cap = (size_t)(1.25 * mean_hits) + 512;
     cap = (cap + 255) & ~size_t(255);
     h->stage_cap = (int)std::min<size_t>(std::max<size_t>(cap, 2048), 16384);
   }

@@ -8,16 +8,18 @@
  *
  *   lf_window_kernel  a1/a2  one thread per (seed, layer, window edge): branch-free binary searches,
  *                            edge pairs exchange by shuffle, n_window cap; packed window words to HBM.
- *   lf_seed_kernel    a3     one warp per seed, lanes = h0 hits.  For a fixed h0 the h2 hits that pass
- *                            the magnet-opening cut form a contiguous x interval: a binary search finds a
- *                            conservative superset, the exact fp32 predicate then decides (bit-exact
- *                            with the all-pairs definition).  Survivors are ballot-compacted and
- *                            finished lane-per-doublet (closest h1, chi2 cut); rank selection on
- *                            64-bit (chi2, set, h0, h2) keys keeps the n smallest, sorted.
+ *   lf_seed_kernel    a3     one warp per seed.  For a fixed h0 the h2 hits that pass the magnet-opening
+ *                            cut form a contiguous x interval: lanes = h0 bracket a conservative superset
+ *                            by two binary searches; a warp prefix scan of the bracket sizes re-maps the
+ *                            work to lanes = candidate doublets, where the exact fp32 predicate decides
+ *                            (bit-exact with the all-pairs definition) and the closest h1 / chi2 cut
+ *                            follow in the same lane; rank selection on 64-bit (chi2, set, h0, h2) keys
+ *                            keeps the n smallest, sorted.
  *   lf_fit_kernel     a4-a6  one thread per candidate: parabola through the triplet, closest hit in the
- *                            9 other windows, hit-count rule, fp32 fit in the oracle's summation order, Q.
- *                            Then one thread per seed picks the lowest Q and writes the track record;
- *                            the CTA ranks the event's tracks in seed order.
+ *                            9 other windows, hit-count rule; accepted candidates are ballot-compacted
+ *                            into a per-warp queue and fitted in dense batches of 32 (fp32 fit in the
+ *                            oracle's summation order, Q).  Then one thread per seed picks the lowest Q
+ *                            and writes the track record; the CTA ranks the event's tracks in seed order.
  *   lf_scan_kernel    a7     exclusive scan of per-event track counts -> event_offsets, n_tracks.
  *   lf_compact_kernel a7     stream compaction: per-seed records -> dense SoA outputs, coalesced.
  *
@@ -327,7 +329,6 @@ __global__ void __launch_bounds__(WIN_THREADS) lf_window_kernel(const __grid_con
  * ============================================================================================ */
 struct __align__(16) SeedScratch {
   unsigned long long trip[TRIP_BUF];
-  uint16_t dq[64];
 };
 
 /* Rank selection on the warp's triplet keys: keeps the `keep` smallest of `n` (<= TRIP_BUF) unique
@@ -336,58 +337,20 @@ __device__ __forceinline__ int select_smallest(SeedScratch& W, int n, int keep, 
   const unsigned long long k0 = (lane < n) ? W.trip[lane] : ~0ull;
   const unsigned long long k1 = (lane + 32 < n) ? W.trip[lane + 32] : ~0ull;
   int r0 = 0, r1 = 0;
-  for (int j = 0; j < n; ++j) {
-    const unsigned long long kj = W.trip[j];
-    r0 += (kj < k0) ? 1 : 0;
-    r1 += (kj < k1) ? 1 : 0;
+  if (n <= 32) {
+    for (int j = 0; j < n; ++j) r0 += (W.trip[j] < k0) ? 1 : 0;
+  } else {
+    for (int j = 0; j < n; ++j) {
+      const unsigned long long kj = W.trip[j];
+      r0 += (kj < k0) ? 1 : 0;
+      r1 += (kj < k1) ? 1 : 0;
+    }
   }
   __syncwarp();
   if (lane < n && r0 < keep) W.trip[r0] = k0;
   if (lane + 32 < n && r1 < keep) W.trip[r1] = k1;
   __syncwarp();
   return n < keep ? n : keep;
-}
-
-/* Finishes the queued doublets, one per lane: x1_expected, closest h1, chi2 cut. */
-template <class HV>
-__device__ __forceinline__ void finish_doublets(const Consts& C, const HV& hx, SeedScratch& W, int qcount, int& tcount,
-                                                uint32_t winw, int lane) {
-  for (int base = 0; base < qcount; base += 32) {
-    const int e = base + lane;
-    const bool act = e < qcount;
-    const unsigned code = act ? W.dq[e] : 0u;
-    const int set = (code >> 10) & 1, i0 = (code >> 5) & 31, i2 = code & 31;
-    const int la = set ? 3 : 0;
-    const int fa = (int)(__shfl_sync(FULL, winw, la) >> 6);
-    const uint32_t wb = __shfl_sync(FULL, winw, la + 4);
-    const int fc = (int)(__shfl_sync(FULL, winw, la + 8) >> 6);
-    const int fb = (int)(wb >> 6), nb = (int)(wb & 63u);
-    bool pass = false;
-    unsigned long long key = 0;
-    if (act) {
-      const float x0 = hx[fa + i0], x2 = hx[fc + i2];
-      const float t = (x2 - x0) * (set ? C.inv_dz_ac[1] : C.inv_dz_ac[0]);
-      const float zb = set ? C.z[7] : C.z[4], za = set ? C.z[3] : C.z[0];
-      const float x1e = zb * t + (x0 - t * za) * (set ? C.K[1] : C.K[0]);
-      const int k = closest_hit(hx, fb, nb, x1e);
-      if (k >= 0) {
-        const float dx = hx[k] - x1e;
-        const float chi2 = dx * dx;
-        if (chi2 < C.T_triplet) {
-          pass = true;
-          key = ((unsigned long long)__float_as_uint(chi2) << 32) |
-                (unsigned)((set << 15) | (i0 << 10) | (i2 << 5) | (k - fb));
-        }
-      }
-    }
-    const unsigned m = __ballot_sync(FULL, pass);
-    if (m) {
-      if (tcount > 32) tcount = select_smallest(W, tcount, C.n_triplets, lane);
-      if (pass) W.trip[tcount + __popc(m & ((1u << lane) - 1u))] = key;
-      tcount += __popc(m);
-      __syncwarp();
-    }
-  }
 }
 
 template <bool DEBUG, class HV>
@@ -399,7 +362,7 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
   const float x_mag = x + tx * C.mag_dz_seed;
   /* lanes 0..11 hold the packed window of layer `lane` */
   const uint32_t winw = (lane < NL) ? A.win[(size_t)seed * NL + lane] : 0u;
-  int qcount = 0, tcount = 0;
+  int tcount = 0;
   const unsigned lt_mask = (1u << lane) - 1u;
   const bool low_p = p < C.p_same_bend;
   const float tol0 = C.mag_tol_base + C.mag_tol_inv_p * aq;
@@ -407,67 +370,87 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
   for (int set = 0; set < 2; ++set) {
     const int la = set ? 3 : 0;
     const uint32_t wa = __shfl_sync(FULL, winw, la), wb = __shfl_sync(FULL, winw, la + 4), wc = __shfl_sync(FULL, winw, la + 8);
-    const int fa = (int)(wa >> 6), na = (int)(wa & 63u), nb = (int)(wb & 63u);
+    const int fa = (int)(wa >> 6), na = (int)(wa & 63u), fb = (int)(wb >> 6), nb = (int)(wb & 63u);
     const int fc = (int)(wc >> 6), nc = (int)(wc & 63u);
     if (na == 0 || nb == 0 || nc == 0) continue;
     const float inv_dz = C.inv_dz_ac[set], zmag_a = C.zmag_a[set], inv_r = C.inv_r[set];
+    const float zb = C.z[la + 4], za = C.z[la], Kx1 = C.K[set];
     /* lanes = h0.  |x0 + t*zmag_a - x_mag| < tol is linear in x2 (t = (x2-x0)*inv_dz, slope
      * r = inv_dz*zmag_a < 0) and tol <= tol_sup, so the survivors lie inside
-     * x2 in (x0 + (tol_sup - A)/r, x0 + (-tol_sup - A)/r), A = x0 - x_mag.  The margin in tol_sup
+     * x2 in [x0 + (tol_sup - A)/r, x0 + (-tol_sup - A)/r], A = x0 - x_mag.  The margin in tol_sup
      * (0.1 mm >> fp32 rounding of these expressions) makes the bracket a strict superset. */
     const bool have = lane < na;
     const float x0 = have ? hx[fa + lane] : 0.0f;
-    const float xc_lo = hx[fc], xc_hi = hx[fc + nc - 1];
+    const int ec = fc + nc;
+    const float xc_lo = hx[fc], xc_hi = hx[ec - 1];
     const float tmax = fmaxf(fabsf((xc_lo - x0) * inv_dz), fabsf((xc_hi - x0) * inv_dz));
     const float tol_sup = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * tmax) + INTERVAL_MARGIN;
     const float Aoff = x0 - x_mag;
     const float x2_lo = x0 + (tol_sup - Aoff) * inv_r;
     const float x2_hi = x0 + (-tol_sup - Aoff) * inv_r;
-    const int ec = fc + nc;
-    int j = ec;
-    if (have) {
-      j = fc;
+    int jlo = fc, jhi = fc; /* first x2 >= x2_lo; first x2 > x2_hi */
 #pragma unroll
-      for (int s = 5; s >= 0; --s) {
-        const int probe = j + (1 << s);
-        if (probe <= ec && hx[probe - 1] < x2_lo) j = probe;
-      }
+    for (int s = 5; s >= 0; --s) {
+      const int pl = jlo + (1 << s), ph = jhi + (1 << s);
+      if (pl <= ec && hx[pl - 1] < x2_lo) jlo = pl;
+      if (ph <= ec && hx[ph - 1] <= x2_hi) jhi = ph;
     }
-    /* walk the bracket; the exact predicate below is the definition */
-    bool more = j < ec;
-    while (__any_sync(FULL, more)) {
-      bool ok = false;
-      if (more) {
+    const int cnt = have ? max(jhi - jlo, 0) : 0;
+    /* dense lane-per-candidate evaluation: inclusive scan of the per-h0 counts */
+    int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int v = __shfl_up_sync(FULL, incl, o);
+      if (lane >= o) incl += v;
+    }
+    const int total = __shfl_sync(FULL, incl, 31);
+    for (int base = 0; base < total; base += 32) {
+      const int tau = base + lane;
+      const bool act = tau < total;
+      int owner = 0; /* number of lanes whose inclusive count is <= tau == the h0 lane owning candidate tau */
+#pragma unroll
+      for (int s = 4; s >= 0; --s) {
+        const int probe = owner + (1 << s);
+        const int v = __shfl_sync(FULL, incl, probe - 1);
+        if (v <= tau) owner = probe;
+      }
+      owner = min(owner, 31);
+      const int before = __shfl_sync(FULL, incl, owner) - __shfl_sync(FULL, cnt, owner);
+      const int j = __shfl_sync(FULL, jlo, owner) + (tau - before);
+      const float x0o = __shfl_sync(FULL, x0, owner);
+      bool pass = false;
+      unsigned long long key = 0;
+      if (act) {
+        /* the exact predicate is the definition */
         const float x2 = hx[j];
-        if (x2 > x2_hi) {
-          more = false;
-        } else {
-          const float t = (x2 - x0) * inv_dz;
-          ok = true;
-          if (low_p) ok = (t - tx) * qop > 0.0f; /* filter 1: same bending direction */
-          const float x_at_mag = x0 + t * zmag_a;
-          const float tol = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * fabsf(t));
-          ok = ok && (fabsf(x_at_mag - x_mag) < tol); /* filter 2: opening at the magnet centre */
+        const float t = (x2 - x0o) * inv_dz;
+        bool ok = true;
+        if (low_p) ok = (t - tx) * qop > 0.0f; /* filter 1: same bending direction */
+        const float x_at_mag = x0o + t * zmag_a;
+        const float tol = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * fabsf(t));
+        ok = ok && (fabsf(x_at_mag - x_mag) < tol); /* filter 2: opening at the magnet centre */
+        if (ok) {
+          /* x1_expected, closest h1, chi2 cut */
+          const float x1e = zb * t + (x0o - t * za) * Kx1;
+          const int k = closest_hit(hx, fb, nb, x1e);
+          const float dx = hx[k] - x1e;
+          const float chi2 = dx * dx;
+          if (chi2 < C.T_triplet) {
+            pass = true;
+            key = ((unsigned long long)__float_as_uint(chi2) << 32) |
+                  (unsigned)((set << 15) | (owner << 10) | ((j - fc) << 5) | (k - fb));
+          }
         }
       }
-      const unsigned m = __ballot_sync(FULL, ok);
+      const unsigned m = __ballot_sync(FULL, pass);
       if (m) {
-        if (ok) W.dq[qcount + __popc(m & lt_mask)] = (uint16_t)((set << 10) | (lane << 5) | (j - fc));
-        qcount += __popc(m);
-        if (qcount > 32) {
-          __syncwarp();
-          finish_doublets(C, hx, W, qcount, tcount, winw, lane);
-          qcount = 0;
-        }
-      }
-      if (more) {
-        ++j;
-        more = j < ec;
+        if (tcount > 32) tcount = select_smallest(W, tcount, C.n_triplets, lane);
+        if (pass) W.trip[tcount + __popc(m & lt_mask)] = key;
+        tcount += __popc(m);
+        __syncwarp();
       }
     }
   }
-  __syncwarp();
-  if (qcount > 0) finish_doublets(C, hx, W, qcount, tcount, winw, lane);
   if (tcount > 0) tcount = select_smallest(W, tcount, C.n_triplets, lane); /* sorted in (chi2,set,h0,h2) order */
   const int ntr = tcount;
   const int NT = C.n_triplets;
@@ -502,7 +485,7 @@ struct __align__(16) SeedTables {
 };
 
 template <bool DEBUG>
-__global__ void __launch_bounds__(SEED_THREADS) lf_seed_kernel(const __grid_constant__ Consts C,
+__global__ void __launch_bounds__(SEED_THREADS, 6) lf_seed_kernel(const __grid_constant__ Consts C,
                                                                const __grid_constant__ EventArgs A) {
   CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
   SeedTables& T = *reinterpret_cast<SeedTables*>(lf_smem + HDR_BYTES + (size_t)A.stage_cap * sizeof(float));
@@ -530,86 +513,113 @@ __global__ void __launch_bounds__(SEED_THREADS) lf_seed_kernel(const __grid_cons
 }
 
 /* ============================================================================================
- * a4-a6: extension, fit, quality, best per seed.  One thread per candidate, then one per seed.
+ * a4-a6: extension, fit, quality, best per seed.
+ *   E  one thread per candidate: closest hit in the 9 layers outside the triplet (uniform loop),
+ *      hit-count rule; accepted candidates are ballot-compacted into a per-warp queue;
+ *   F  one thread per queued candidate (dense batches of 32): fp32 fit in ascending layer order, Q;
+ *   B  one thread per seed: lowest Q wins, the winner is re-evaluated to write the track record.
  * ============================================================================================ */
-struct FitOut {
-  float Q;
-  bool enough, ty_ok;
-};
 
-/* Evaluates candidate `code` of a seed: extension to the 9 other layers, hit-count rule, fit, Q.
- * With `rec` != nullptr also computes q/p and the state and writes the 20-word track record. */
-template <bool DEBUG, class HV>
-__device__ __noinline__ FitOut eval_candidate(const Consts& C, const HV& hx, const uint32_t* winw, float y, float tx,
-                                              float ty, unsigned code, uint32_t h0, int32_t* rec, uint32_t seed,
-                                              int32_t* dbg_hits) {
+/* Hit codes of a candidate: byte l = window-relative index of the hit on layer l, 0xFF = none. */
+struct CandHits {
+  uint32_t w[3];
+  int n, n_uv;
+  bool enough;
+};
+__device__ __forceinline__ unsigned code_of(const CandHits& h, int l) { return (h.w[l >> 2] >> (8 * (l & 3))) & 0xFFu; }
+
+/* Eq. (4) parameters: exact parabola through the three triplet hits. */
+template <class HV>
+__device__ __forceinline__ void triplet_parabola(const Consts& C, const HV& hx, const uint32_t* winw, unsigned code,
+                                                 float& a0, float& t0, float& c0) {
   const int set = (code >> 15) & 1, la = set ? 3 : 0;
-  int idx[NL];   /* event-relative hit index per layer or -1 */
-  float sv[NL];  /* its stored coordinate */
-  /* Eq. (4) parameters: exact parabola through the three triplet hits */
-  const int i0 = (int)(winw[la] >> 6) + (int)((code >> 10) & 31);
-  const int i1 = (int)(winw[la + 4] >> 6) + (int)(code & 31);
-  const int i2 = (int)(winw[la + 8] >> 6) + (int)((code >> 5) & 31);
-  const float x0 = hx[i0], x1 = hx[i1], x2 = hx[i2];
+  const float x0 = hx[(int)(winw[la] >> 6) + (int)((code >> 10) & 31)];
+  const float x1 = hx[(int)(winw[la + 4] >> 6) + (int)(code & 31)];
+  const float x2 = hx[(int)(winw[la + 8] >> 6) + (int)((code >> 5) & 31)];
   const float X10 = x1 - x0, X20 = x2 - x0;
   const float D10 = set ? C.D10[1] : C.D10[0], D20 = set ? C.D20[1] : C.D20[0];
   const float W10 = set ? C.W10[1] : C.W10[0];
-  const float c0 = (X20 * D10 - X10 * D20) * (set ? C.inv_det[1] : C.inv_det[0]);
-  const float t0 = (X10 - c0 * W10) * (set ? C.inv_D10[1] : C.inv_D10[0]);
-  const float a0 = (x0 - t0 * (set ? C.d[3] : C.d[0])) - c0 * (set ? C.w[3] : C.w[0]);
+  c0 = (X20 * D10 - X10 * D20) * (set ? C.inv_det[1] : C.inv_det[0]);
+  t0 = (X10 - c0 * W10) * (set ? C.inv_D10[1] : C.inv_D10[0]);
+  a0 = (x0 - t0 * (set ? C.d[3] : C.d[0])) - c0 * (set ? C.w[3] : C.w[0]);
+}
+
+/* a4/a5: extension of one triplet to the 9 other layers + hit-count rule.
+ * `geo` is the shared-memory copy of the per-layer constants: d, w, dzs, tana (12 floats each). */
+template <class HV>
+__device__ __noinline__ CandHits extend_candidate(const Consts& C, const HV& hx, const uint32_t* winw, const float* geo,
+                                                  float y, float tx, float ty, unsigned code) {
+  const int set = (code >> 15) & 1, la = set ? 3 : 0;
+  float a0, t0, c0;
+  triplet_parabola(C, hx, winw, code, a0, t0, c0);
   const float T_uv = fmaxf(C.T_uv_min, C.T_uv_slope * (fabsf(tx) + fabsf(ty)));
-  int n = 0, n_uv = 0;
-  bool st_uv[3] = {false, false, false};
-  float yt[NL];
+  CandHits h;
+  h.w[0] = h.w[1] = h.w[2] = 0xFFFFFFFFu;
+  /* the triplet's own hits on layers la, la+4, la+8 */
+  const unsigned sh = 8u * (unsigned)la;
+  h.w[0] = (h.w[0] & ~(0xFFu << sh)) | (((code >> 10) & 31u) << sh);
+  h.w[1] = (h.w[1] & ~(0xFFu << sh)) | ((code & 31u) << sh);
+  h.w[2] = (h.w[2] & ~(0xFFu << sh)) | (((code >> 5) & 31u) << sh);
+  int n = 3, n_uv = 0;
+  unsigned st_mask = 0;
 #pragma unroll
-  for (int l = 0; l < NL; ++l) {
-    const bool uv = is_uv(l);
-    yt[l] = uv ? (y + ty * C.dzs[l]) * C.tana[l] : 0.0f;
-    idx[l] = -1;
-    sv[l] = 0.0f;
-    if (!uv && (l & 3) == la) { /* the triplet's own layers: la, la+4, la+8 */
-      idx[l] = (l < 4) ? i0 : (l < 8 ? i1 : i2);
-      sv[l] = (l < 4) ? x0 : (l < 8 ? x1 : x2);
-      ++n;
-    } else {
-      float pred = (a0 + t0 * C.d[l]) + c0 * C.w[l];
-      if (uv) pred = pred + yt[l];
-      const uint32_t ww = winw[l];
-      const int k = closest_hit(hx, (int)(ww >> 6), (int)(ww & 63u), pred);
-      if (k >= 0) {
-        const float xk = hx[k];
-        const float dx = xk - pred;
-        const float chi2 = dx * dx;
-        if (chi2 < (uv ? T_uv : C.T_x)) {
-          idx[l] = k;
-          sv[l] = xk;
-          ++n;
-          if (uv) { ++n_uv; st_uv[l >> 2] = true; }
-        }
+  for (int li = 0; li < 9; ++li) {
+    const int l = li + li / 3 + (1 - set); /* the 9 layers outside the set, ascending */
+    const bool uv = (li % 3) != (set ? 0 : 2); /* set 0: layers 1,2,3 -> u,v,x; set 1: 0,1,2 -> x,u,v */
+    float pred = (a0 + t0 * geo[l]) + c0 * geo[NL + l];
+    if (uv) pred = pred + (y + ty * geo[2 * NL + l]) * geo[3 * NL + l];
+    const uint32_t ww = winw[l];
+    const int f = (int)(ww >> 6);
+    const int k = closest_hit(hx, f, (int)(ww & 63u), pred);
+    if (k >= 0) {
+      const float dx = hx[k] - pred;
+      const float chi2 = dx * dx;
+      if (chi2 < (uv ? T_uv : C.T_x)) {
+        const unsigned s8 = 8u * (unsigned)(l & 3);
+        const unsigned v = (unsigned)(k - f);
+        if (li < 3) h.w[0] = (h.w[0] & ~(0xFFu << s8)) | (v << s8);
+        else if (li < 6) h.w[1] = (h.w[1] & ~(0xFFu << s8)) | (v << s8);
+        else h.w[2] = (h.w[2] & ~(0xFFu << s8)) | (v << s8);
+        ++n;
+        if (uv) { ++n_uv; st_mask |= 1u << (li / 3); }
       }
     }
   }
-  if (DEBUG && dbg_hits) {
-#pragma unroll
-    for (int l = 0; l < NL; ++l) dbg_hits[l] = idx[l] >= 0 ? (int32_t)(h0 + idx[l]) : -1;
-  }
-  FitOut out;
-  out.Q = 0.0f;
-  out.ty_ok = false;
+  h.n = n;
+  h.n_uv = n_uv;
   /* at least min_hits hits and at least one u/v hit per station */
-  out.enough = (n >= C.min_hits) && st_uv[0] && st_uv[1] && st_uv[2];
-  if (!out.enough) return out;
+  h.enough = (n >= C.min_hits) && (st_mask == 7u);
+  return h;
+}
 
+struct FitOut {
+  float Q;
+  bool ty_ok;
+};
+
+/* a6: fit of an accepted candidate.  With `rec` != nullptr also computes q/p and the
+ * state (Eq. 9) and writes the 20-word track record. */
+template <class HV>
+__device__ __noinline__ FitOut fit_candidate(const Consts& C, const HV& hx, const uint32_t* winw, float y, float tx,
+                                             float ty, unsigned code, const CandHits& h, uint32_t h0, uint32_t seed,
+                                             int32_t* rec) {
+  float a0, t0, c0;
+  triplet_parabola(C, hx, winw, code, a0, t0, c0);
+  const float T_uv = fmaxf(C.T_uv_min, C.T_uv_slope * (fabsf(tx) + fabsf(ty)));
   const float inv_Tuv = 1.0f / T_uv;
   /* x fit on the residuals to the triplet parabola: sums in ascending layer order */
   float r[NL];
   float S1 = 0.f, Sd = 0.f, Sw = 0.f, Sdd = 0.f, Sdw = 0.f, Sww = 0.f, Sr = 0.f, Sdr = 0.f, Swr = 0.f;
 #pragma unroll
   for (int l = 0; l < NL; ++l) {
+    const unsigned cd = code_of(h, l);
+    const bool present = cd != 0xFFu;
     const float dl = C.d[l], wl = C.w[l];
-    const float m = sv[l] - yt[l];
+    const float s_i = hx[present ? ((int)(winw[l] >> 6) + (int)cd) : 0];
+    const float yt = is_uv(l) ? (y + ty * C.dzs[l]) * C.tana[l] : 0.0f;
+    const float m = s_i - yt;
     r[l] = m - ((a0 + t0 * dl) + c0 * wl);
-    if (idx[l] >= 0) {
+    if (present) {
       S1 = S1 + 1.0f;
       Sd = Sd + dl;
       Sw = Sw + wl;
@@ -632,25 +642,24 @@ __device__ __noinline__ FitOut eval_candidate(const Consts& C, const HV& hx, con
   const float da = ((C00 * Sr + C01 * Sdr) + C02 * Swr) * inv;
   const float dt = ((C01 * Sr + C11 * Sdr) + C12 * Swr) * inv;
   const float dc = ((C02 * Sr + C12 * Sdr) + C22 * Swr) * inv;
-  float rho[NL];
   float Qx = 0.f, U1 = 0.f, Ud = 0.f, Udd = 0.f, Ur = 0.f, Udr = 0.f;
 #pragma unroll
   for (int l = 0; l < NL; ++l) {
+    const bool present = code_of(h, l) != 0xFFu;
     const float dl = C.d[l], wl = C.w[l];
     const float e = r[l] - ((da + dt * dl) + dc * wl);
     const float chi2 = e * e;
-    rho[l] = 0.f;
     if (is_uv(l)) {
-      rho[l] = e * C.inv_tan[l];
-      if (idx[l] >= 0) {
+      r[l] = e * C.inv_tan[l]; /* rho: y residual to the seed's straight line */
+      if (present) {
         Qx = Qx + chi2 * inv_Tuv;
         U1 = U1 + 1.0f;
         Ud = Ud + dl;
         Udd = Udd + dl * dl;
-        Ur = Ur + rho[l];
-        Udr = Udr + dl * rho[l];
+        Ur = Ur + r[l];
+        Udr = Udr + dl * r[l];
       }
-    } else if (idx[l] >= 0) {
+    } else if (present) {
       Qx = Qx + chi2 * C.inv_Tx;
     }
   }
@@ -660,20 +669,20 @@ __device__ __noinline__ FitOut eval_candidate(const Consts& C, const HV& hx, con
   const float dy0 = (Udd * Ur - Ud * Udr) * inv2;
   const float dtym = (U1 * Udr - Ud * Ur) * inv2;
   const float dty = dtym * 0.001f;
+  FitOut out;
   out.ty_ok = fabsf(dty) < C.T_ty; /* PAPER.md:264 */
   float Qy = 0.f;
 #pragma unroll
   for (int l = 0; l < NL; ++l) {
     if (!is_uv(l)) continue;
-    const float ey = rho[l] - (dy0 + dtym * C.d[l]);
-    if (idx[l] >= 0) Qy = Qy + (ey * ey) * C.inv_Ty;
+    const float ey = r[l] - (dy0 + dtym * C.d[l]);
+    if (code_of(h, l) != 0xFFu) Qy = Qy + (ey * ey) * C.inv_Ty;
   }
-  const int ci = min(3, max(0, n - 9));
+  const int ci = min(3, max(0, h.n - 9));
   const float Cn = (ci == 0) ? C.C_nhits[0] : (ci == 1 ? C.C_nhits[1] : (ci == 2 ? C.C_nhits[2] : C.C_nhits[3]));
-  out.Q = (Qx / (float)(n - 3) + Qy / (float)(n_uv - 2)) * Cn; /* Eq. (6) */
+  out.Q = (Qx / (float)(h.n - 3) + Qy / (float)(h.n_uv - 2)) * Cn; /* Eq. (6) */
 
   if (rec != nullptr) {
-    /* momentum from the slope change (Eq. 9) and the state at z_state */
     const float a = a0 + da, t = t0 + dt, c = c0 + dc;
     const float t_ref = t * 0.001f;
     const float dslope = t_ref - tx;
@@ -681,9 +690,12 @@ __device__ __noinline__ FitOut eval_candidate(const Consts& C, const HV& hx, con
     int4* r4 = reinterpret_cast<int4*>(rec);
     int o[REC_WORDS];
 #pragma unroll
-    for (int l = 0; l < NL; ++l) o[l] = idx[l] >= 0 ? (int32_t)(h0 + idx[l]) : -1;
+    for (int l = 0; l < NL; ++l) {
+      const unsigned cd = code_of(h, l);
+      o[l] = (cd != 0xFFu) ? (int32_t)(h0 + (winw[l] >> 6) + cd) : -1;
+    }
     o[12] = (int32_t)seed;
-    o[13] = n;
+    o[13] = h.n;
     o[14] = __float_as_int((a + t * C.ds) + c * C.ws);
     o[15] = __float_as_int((y + ty * C.dz_state) + (dy0 + dtym * C.ds));
     o[16] = __float_as_int((t + c * C.dws) * 0.001f);
@@ -698,15 +710,41 @@ __device__ __noinline__ FitOut eval_candidate(const Consts& C, const HV& hx, con
 
 /* Per-chunk tables of the fit kernel (after the staged hits in shared memory). */
 struct FitTables {
+  float* geo;      /* 4*12: d, w, dzs, tana */
   uint32_t* win;   /* FIT_CHUNK*12 packed windows */
   float* sp;       /* FIT_CHUNK*4: y, tx, ty, (unused) */
   int* pref;       /* FIT_CHUNK+1: exclusive prefix of candidates per seed */
   uint16_t* item;  /* FIT_CHUNK*NT: seed_local<<4 | k */
   float* Q;        /* FIT_CHUNK*NT: Q, or +inf if the candidate is not acceptable */
+  uint4* queue;    /* (FIT_THREADS/32) warps * 64 entries: hit codes (3 words) + item | n<<16 | n_uv<<24 */
 };
 __host__ __device__ inline size_t fit_tables_bytes(int nt) {
-  return (size_t)FIT_CHUNK * NL * 4 + (size_t)FIT_CHUNK * 4 * 4 + (size_t)(FIT_CHUNK + 4) * 4 +
-         (((size_t)FIT_CHUNK * nt * 2 + 15) & ~size_t(15)) + (size_t)FIT_CHUNK * nt * 4;
+  return 4 * NL * 4 + (size_t)FIT_CHUNK * NL * 4 + (size_t)FIT_CHUNK * 4 * 4 + (size_t)(FIT_CHUNK + 4) * 4 +
+         (((size_t)FIT_CHUNK * nt * 2 + 15) & ~size_t(15)) + (size_t)FIT_CHUNK * nt * 4 + (size_t)(FIT_THREADS / 32) * 64 * 16;
+}
+
+/* F on one dense batch of the warp's queue: entries [0, cnt), cnt <= 32. */
+template <bool DEBUG, class HV>
+__device__ __forceinline__ void fit_batch(const Consts& C, const EventArgs& A, const HV& hx, const FitTables& T,
+                                          const uint4* q, int cnt, uint32_t sbase, uint32_t h0, int lane) {
+  if (lane < cnt) {
+    const uint4 e = q[lane];
+    const int it = (int)(e.w & 0xFFFFu);
+    CandHits h;
+    h.w[0] = e.x; h.w[1] = e.y; h.w[2] = e.z;
+    h.n = (int)((e.w >> 16) & 0xFFu);
+    h.n_uv = (int)(e.w >> 24);
+    h.enough = true;
+    const unsigned im = T.item[it];
+    const int sl = (int)(im >> 4), k = (int)(im & 15u);
+    const uint32_t seed = sbase + (uint32_t)sl;
+    const unsigned code = A.trip_code[(size_t)seed * C.n_triplets + k];
+    const FitOut fo = fit_candidate(C, hx, T.win + sl * NL, T.sp[sl * 4 + 0], T.sp[sl * 4 + 1], T.sp[sl * 4 + 2], code, h,
+                                    h0, seed, nullptr);
+    /* accepted if Q < T_Q (and the t_y cut holds) */
+    T.Q[it] = (fo.ty_ok && (fo.Q < C.T_Q)) ? fo.Q : __int_as_float(0x7f800000);
+    if (DEBUG && A.dbg.cand_quality) A.dbg.cand_quality[(size_t)seed * C.n_triplets + k] = fo.ty_ok ? fo.Q : -2.0f;
+  }
 }
 
 template <bool DEBUG, bool STAGED>
@@ -717,6 +755,7 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
   const int ns = (int)(s1 - s0);
   const int NT = C.n_triplets;
   const float INF = __int_as_float(0x7f800000);
+  uint4* myq = T.queue + warp * 64;
   int ev_tracks = 0;
   for (int cb = 0; cb < ns; cb += FIT_CHUNK) {
     const int cn = min(FIT_CHUNK, ns - cb);
@@ -731,7 +770,7 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
       T.sp[tid * 4 + 2] = __ldg(A.sty + seed);
       my_n = (int)A.n_trip[seed];
     }
-    /* exclusive prefix of candidate counts over the chunk (FIT_CHUNK == FIT_THREADS) */
+    /* exclusive prefix of candidate counts over the chunk (FIT_CHUNK <= FIT_THREADS) */
     int incl = my_n;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -754,21 +793,50 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
     }
     if (tid == 0) T.pref[cn] = total;
     __syncthreads();
-    /* ---- one thread per candidate: extension + fit + Q */
-    for (int it = tid; it < total; it += FIT_THREADS) {
-      const unsigned im = T.item[it];
-      const int sl = (int)(im >> 4), k = (int)(im & 15u);
-      const uint32_t seed = sbase + (uint32_t)sl;
-      const unsigned code = A.trip_code[(size_t)seed * NT + k];
-      int32_t* dh = (DEBUG && A.dbg.cand_hits) ? A.dbg.cand_hits + ((size_t)seed * NT + k) * NL : nullptr;
-      const FitOut fo = eval_candidate<DEBUG>(C, hx, T.win + sl * NL, T.sp[sl * 4 + 0], T.sp[sl * 4 + 1], T.sp[sl * 4 + 2],
-                                              code, E.h0, nullptr, seed, dh);
-      /* accepted if Q < T_Q (and the t_y cut holds) */
-      T.Q[it] = (fo.enough && fo.ty_ok && (fo.Q < C.T_Q)) ? fo.Q : INF;
-      if (DEBUG && A.dbg.cand_quality) A.dbg.cand_quality[(size_t)seed * NT + k] = fo.enough ? (fo.ty_ok ? fo.Q : -2.0f) : -1.0f;
+    /* ---- E: one thread per candidate; accepted candidates go to the warp's queue; F on dense batches */
+    int qn = 0;
+    for (int base = 0; base < total; base += FIT_THREADS) {
+      const int it = base + tid;
+      bool enough = false;
+      CandHits h;
+      if (it < total) {
+        const unsigned im = T.item[it];
+        const int sl = (int)(im >> 4), k = (int)(im & 15u);
+        const uint32_t seed = sbase + (uint32_t)sl;
+        const unsigned code = A.trip_code[(size_t)seed * NT + k];
+        h = extend_candidate(C, hx, T.win + sl * NL, T.geo, T.sp[sl * 4 + 0], T.sp[sl * 4 + 1], T.sp[sl * 4 + 2], code);
+        enough = h.enough;
+        if (!enough) T.Q[it] = INF;
+        if (DEBUG) {
+          if (A.dbg.cand_hits)
+            for (int l = 0; l < NL; ++l) {
+              const unsigned cd = code_of(h, l);
+              A.dbg.cand_hits[((size_t)seed * NT + k) * NL + l] = (cd != 0xFFu) ? (int32_t)(E.h0 + (T.win[sl * NL + l] >> 6) + cd) : -1;
+            }
+          if (A.dbg.cand_quality && !enough) A.dbg.cand_quality[(size_t)seed * NT + k] = -1.0f;
+        }
+      }
+      const unsigned m = __ballot_sync(FULL, enough);
+      if (m) {
+        if (enough)
+          myq[qn + __popc(m & ((1u << lane) - 1u))] =
+              make_uint4(h.w[0], h.w[1], h.w[2], (unsigned)it | ((unsigned)h.n << 16) | ((unsigned)h.n_uv << 24));
+        qn += __popc(m);
+        __syncwarp();
+        if (qn >= 32) {
+          fit_batch<DEBUG>(C, A, hx, T, myq, 32, sbase, E.h0, lane);
+          __syncwarp();
+          const uint4 carry = (lane + 32 < qn) ? myq[lane + 32] : make_uint4(0, 0, 0, 0);
+          __syncwarp();
+          qn -= 32;
+          if (lane < qn) myq[lane] = carry;
+          __syncwarp();
+        }
+      }
     }
+    if (qn > 0) fit_batch<DEBUG>(C, A, hx, T, myq, qn, sbase, E.h0, lane);
     __syncthreads();
-    /* ---- one thread per seed: lowest Q wins, ties -> earlier in (chi2,set,h0,h2) order */
+    /* ---- B: one thread per seed: lowest Q wins, ties -> earlier in (chi2,set,h0,h2) order */
     bool found = false;
     if (tid < cn) {
       const uint32_t seed = sbase + (uint32_t)tid;
@@ -786,11 +854,12 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
             for (int l = 0; l < NL; ++l) A.dbg.cand_hits[((size_t)seed * NT + k) * NL + l] = -1;
         }
       }
-      if (bk >= 0) {
+      found = bk >= 0;
+      if (found) {
         const unsigned code = A.trip_code[(size_t)seed * NT + bk];
-        eval_candidate<false>(C, hx, T.win + tid * NL, T.sp[tid * 4 + 0], T.sp[tid * 4 + 1], T.sp[tid * 4 + 2], code, E.h0,
-                              A.ws_rec + (size_t)seed * REC_WORDS, seed, nullptr);
-        found = true;
+        const float y = T.sp[tid * 4 + 0], tx = T.sp[tid * 4 + 1], ty = T.sp[tid * 4 + 2];
+        const CandHits h = extend_candidate(C, hx, T.win + tid * NL, T.geo, y, tx, ty, code);
+        fit_candidate(C, hx, T.win + tid * NL, y, tx, ty, code, h, E.h0, seed, A.ws_rec + (size_t)seed * REC_WORDS);
       }
       A.ws_nh[seed] = found ? 1 : 0;
     }
@@ -816,19 +885,32 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
 }
 
 template <bool DEBUG>
-__global__ void __launch_bounds__(FIT_THREADS) lf_fit_kernel(const __grid_constant__ Consts C,
-                                                             const __grid_constant__ EventArgs A) {
+__global__ void __launch_bounds__(FIT_THREADS, 3) lf_fit_kernel(const __grid_constant__ Consts C,
+                                                                const __grid_constant__ EventArgs A) {
   CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
   unsigned char* tb = lf_smem + HDR_BYTES + (size_t)A.stage_cap * sizeof(float);
   const int NT = C.n_triplets;
   FitTables T;
+  T.geo = reinterpret_cast<float*>(tb);
+  tb += 4 * NL * 4;
   T.win = reinterpret_cast<uint32_t*>(tb);
-  T.sp = reinterpret_cast<float*>(tb + (size_t)FIT_CHUNK * NL * 4);
-  T.pref = reinterpret_cast<int*>(tb + (size_t)FIT_CHUNK * NL * 4 + (size_t)FIT_CHUNK * 16);
-  unsigned char* ib = tb + (size_t)FIT_CHUNK * NL * 4 + (size_t)FIT_CHUNK * 16 + (size_t)(FIT_CHUNK + 4) * 4;
-  T.item = reinterpret_cast<uint16_t*>(ib);
-  T.Q = reinterpret_cast<float*>(ib + (((size_t)FIT_CHUNK * NT * 2 + 15) & ~size_t(15)));
+  tb += (size_t)FIT_CHUNK * NL * 4;
+  T.sp = reinterpret_cast<float*>(tb);
+  tb += (size_t)FIT_CHUNK * 16;
+  T.pref = reinterpret_cast<int*>(tb);
+  tb += (size_t)(FIT_CHUNK + 4) * 4;
+  T.item = reinterpret_cast<uint16_t*>(tb);
+  tb += ((size_t)FIT_CHUNK * NT * 2 + 15) & ~size_t(15);
+  T.Q = reinterpret_cast<float*>(tb);
+  tb += (size_t)FIT_CHUNK * NT * 4;
+  T.queue = reinterpret_cast<uint4*>(tb);
   if (threadIdx.x == 0) mbar_init(&H.mbar, 1);
+  if (threadIdx.x < NL) {
+    T.geo[threadIdx.x] = C.d[threadIdx.x];
+    T.geo[NL + threadIdx.x] = C.w[threadIdx.x];
+    T.geo[2 * NL + threadIdx.x] = C.dzs[threadIdx.x];
+    T.geo[3 * NL + threadIdx.x] = C.tana[threadIdx.x];
+  }
   uint32_t phase = 0;
   EventCtx E;
   while (fetch_event(A, phase, E)) {
