@@ -331,7 +331,7 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--config", type=int, default=3, choices=[0, 1, 3, 4])
+    ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--events", type=int, default=None, help="override the number of events (default: the config's)")
     ap.add_argument("--cpu-events", type=int, default=1500, help="events of the single-thread oracle sample")
     ap.add_argument("--no-e2e", action="store_true")

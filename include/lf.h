@@ -79,8 +79,10 @@ typedef struct {
                                                                  1 <= n_triplets <= LF_MAX_TRIPLETS */
   float xtol_base, xtol_inv_p, x_asym, uv_half_width;         /* 150, 2000, 100, 800 */
   float p_same_bend, mag_tol_base, mag_tol_inv_p, mag_tol_tx, mag_tol_max; /* 5, 8, 60, 20, 40 */
-  int32_t hit_storage;                                        /* 0 = fp32; 1 = fp16 copy of the hits for windows +
-                                                                 seeding, fp32 extension and fit */
+  int32_t hit_storage;                                        /* 0 = fp32 (bit-exact reference path); 1 = the library keeps
+                                                                 an fp16 copy of the hits (block-offset encoding) that the
+                                                                 window and seeding kernels read; extension and fit stay on
+                                                                 the fp32 hits (BASELINE.json configs[2]) */
 } lf_params;
 
 /* Input seeds: upstream track states at z_seed, SoA, all events back to back. */
@@ -131,7 +133,7 @@ typedef struct {
 #define LF_K_FIT 2
 #define LF_N_KERNELS 5 /* + LF_K_SCAN = 3, LF_K_COMPACT = 4 in lf_kernel_times */
 typedef struct {
-  int32_t kernels_per_run;       /* kernel launches one lf_run enqueues (5) */
+  int32_t kernels_per_run;       /* kernel launches one lf_run enqueues (5; 6 with hit_storage = 1) */
   int32_t regs[3], block[3], grid[3], ctas_per_sm[3];
   int32_t smem_bytes[3];         /* dynamic shared memory per CTA */
   int32_t staged_hits_per_event; /* events with more hits than this read hits from global memory */

@@ -44,6 +44,8 @@ struct lf_handle {
   int sm_count, stage_cap;
   int regs[3], grid[3], ctas_per_sm[3], smem_bytes[3]; /* window, seed, fit kernels */
   /* workspace */
+  __half* hx16;     /* hit_storage = 1 only */
+  float* origin16;
   uint32_t* win;
   uint16_t* trip_code;
   uint8_t* n_trip;
@@ -170,6 +172,14 @@ lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_
   }
   const bool work = n_events > 0;
   auto grid_of = [&](int k) { return (int)std::min<size_t>((size_t)h->grid[k], n_events); };
+  const bool half_hits = h->P.hit_storage == 1;
+  if (work && half_hits) {
+    /* fp16 copy of the hits for the window and seeding kernels (timed with the window kernel) */
+    const int pg = (int)std::min<size_t>((size_t)h->sm_count * 8, n_events);
+    lf::lf_pack_hits_kernel<<<pg, 256, 0, st>>>(hits->x, hits->seg_offsets, (uint32_t)n_events, h->hx16, h->origin16);
+    A.hx16 = h->hx16;
+    A.origin16 = h->origin16;
+  }
   if (work) {
     A.ticket = h->tickets + 0;
     lf::lf_window_kernel<DEBUG><<<grid_of(0), lf::WIN_THREADS, h->smem_bytes[0], st>>>(h->C, A);
@@ -180,6 +190,8 @@ lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_
     lf::lf_seed_kernel<DEBUG><<<grid_of(1), lf::SEED_THREADS, h->smem_bytes[1], st>>>(h->C, A);
   }
   if (prof) LF_CUDA(h, cudaEventRecord(pe[2], st));
+  A.hx16 = nullptr; /* extension and fit always read the fp32 hits */
+  A.origin16 = nullptr;
   if (work) {
     A.ticket = h->tickets + 2;
     lf::lf_fit_kernel<DEBUG><<<grid_of(2), lf::FIT_THREADS, h->smem_bytes[2], st>>>(h->C, A);
@@ -250,8 +262,6 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   if (const char* why = validate(*geometry, *params)) return fail(nullptr, LF_ERR_INVALID_ARG, std::string("lf_create: ") + why);
   if (max_hits >= (size_t)0x7fffffff || max_seeds >= (size_t)0x7fffffff || max_events >= (size_t)0x7fffffff / LF_N_LAYERS / 2)
     return fail(nullptr, LF_ERR_CAPACITY, "lf_create: maxima must fit 32-bit indices");
-  if (params->hit_storage == 1)
-    return fail(nullptr, LF_ERR_UNSUPPORTED, "lf_create: hit_storage = 1 (fp16) is not implemented in this build");
 
   lf_handle* h = new (std::nothrow) lf_handle();
   if (!h) return fail(nullptr, LF_ERR_CUDA, "lf_create: out of host memory");
@@ -301,6 +311,11 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
 
   const size_t ns = std::max<size_t>(max_seeds, 1), ne = std::max<size_t>(max_events, 1);
   const size_t nt = (size_t)params->n_triplets;
+  if (params->hit_storage == 1) {
+    const size_t nh = std::max<size_t>(max_hits, 1);
+    LF_CREATE_CUDA(cudaMalloc(&h->hx16, nh * sizeof(__half)));
+    LF_CREATE_CUDA(cudaMalloc(&h->origin16, ((nh >> 5) + ne * lf::NSEG + 2) * sizeof(float)));
+  }
   LF_CREATE_CUDA(cudaMalloc(&h->win, ns * lf::NL * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->trip_code, ns * nt * sizeof(uint16_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->n_trip, ns));
@@ -320,6 +335,7 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
 
 lf_status lf_destroy(lf_handle* h) {
   if (!h) return LF_OK;
+  cudaFree(h->hx16); cudaFree(h->origin16);
   cudaFree(h->win); cudaFree(h->trip_code); cudaFree(h->n_trip);
   cudaFree(h->ws_rec); cudaFree(h->ws_nh); cudaFree(h->ws_rank); cudaFree(h->ws_event);
   cudaFree(h->ev_count); cudaFree(h->ev_off); cudaFree(h->tickets);
@@ -340,7 +356,7 @@ lf_status lf_destroy(lf_handle* h) {
 
 lf_status lf_get_info(const lf_handle* h, lf_info* out) {
   if (!h || !out) return LF_ERR_INVALID_ARG;
-  out->kernels_per_run = LF_N_KERNELS;
+  out->kernels_per_run = LF_N_KERNELS + (h->P.hit_storage == 1 ? 1 : 0);
   const int threads[3] = {lf::WIN_THREADS, lf::SEED_THREADS, lf::FIT_THREADS};
   for (int k = 0; k < 3; ++k) {
     out->regs[k] = h->regs[k];

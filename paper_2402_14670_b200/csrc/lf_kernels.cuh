@@ -28,6 +28,7 @@
  * written from PAPER.md + DESIGN.md and shares nothing with oracle/.
  */
 #pragma once
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -73,6 +74,10 @@ struct EventArgs {
   const uint32_t* seed_off;
   const float* hx;
   const uint32_t* seg_off;
+  /* hit_storage = 1: fp16 copy of the hits (block-offset encoding, see lf_pack_hits_kernel); the window
+   * and seed kernels stage from it when hx16 != nullptr */
+  const __half* hx16;
+  const float* origin16;
   uint32_t n_events;
   int stage_cap;        /* floats of shared memory available for one event's hits */
   uint32_t* ticket;     /* this kernel's event ticket */
@@ -179,7 +184,16 @@ __device__ __forceinline__ bool fetch_event(const EventArgs& A, uint32_t& phase,
   const float* gsrc = A.hx + E.h0;
   E.staged = E.nh + 4 <= A.stage_cap;
   E.skew = (int)((reinterpret_cast<uintptr_t>(gsrc) >> 2) & 3);
-  if (E.staged) {
+  if (E.staged && A.hx16 != nullptr) {
+    /* fp16 hit storage: decode x~ = origin(block) + half into the fp32 stage, segment by segment */
+    for (int sg = 0; sg < NSEG; ++sg) {
+      const uint32_t S = so[sg];
+      const int len = (int)(so[sg + 1] - S);
+      const uint32_t slot0 = (S >> 5) + (E.ev * NSEG + (uint32_t)sg);
+      for (int i = tid; i < len; i += blockDim.x)
+        buf[E.skew + (int)(S - E.h0) + i] = __ldg(A.origin16 + slot0 + (uint32_t)(i >> 5)) + __half2float(A.hx16[S + i]);
+    }
+  } else if (E.staged) {
     /* the 16-byte aligned interior goes by TMA, the ragged head/tail by plain loads */
     const int head = min(E.nh, (4 - E.skew) & 3);
     const int bulk = (E.nh - head) & ~3;
@@ -916,6 +930,31 @@ __global__ void __launch_bounds__(FIT_THREADS, 3) lf_fit_kernel(const __grid_con
   while (fetch_event(A, phase, E)) {
     if (E.staged) fit_event<DEBUG, true>(C, A, H, E, HitView<true>{E.skew}, T);
     else fit_event<DEBUG, false>(C, A, H, E, HitView<false>{A.hx + E.h0}, T);
+  }
+}
+
+/* hit_storage = 1 (BASELINE.json configs[2]; "store hit data in fp16 in addition to fp32"):
+ * writes the fp16 copy of the hits.  Block-offset encoding: inside every (event, layer, zone) segment,
+ * consecutive hits form blocks of 32; a block's origin is the fp32 coordinate of its 17th hit (or its last
+ * one if shorter); each hit stores half(x - origin), so |offset| stays within half a block's x span
+ * (ulp <= 0.25 mm at Run-3 occupancy).  The origin slot of block b of global segment g starting at hit S is
+ * (S >> 5) + g + b: slots of different segments never overlap, so the index alone locates the origin. */
+__global__ void __launch_bounds__(256) lf_pack_hits_kernel(const float* __restrict__ hx, const uint32_t* __restrict__ seg_off,
+                                                           uint32_t n_events, __half* __restrict__ hx16,
+                                                           float* __restrict__ origin16) {
+  for (uint32_t ev = blockIdx.x; ev < n_events; ev += gridDim.x) {
+    const uint32_t* so = seg_off + (size_t)ev * NSEG;
+    for (int sg = 0; sg < NSEG; ++sg) {
+      const uint32_t S = so[sg];
+      const int len = (int)(so[sg + 1] - S);
+      const uint32_t slot0 = (S >> 5) + (ev * NSEG + (uint32_t)sg);
+      for (int i = threadIdx.x; i < len; i += blockDim.x) {
+        const int b0 = i & ~31;
+        const float o = hx[S + b0 + min(16, len - b0 - 1)];
+        hx16[S + i] = __float2half_rn(hx[S + i] - o);
+        if ((i & 31) == 0) origin16[slot0 + (uint32_t)(i >> 5)] = o;
+      }
+    }
   }
 }
 

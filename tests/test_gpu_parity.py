@@ -199,3 +199,30 @@ def test_repeated_runs_and_capacity_errors(lfmod, geometry, params):
         lf2.run(db, out)
     assert ei.value.status == lfmod.LF_ERR_CAPACITY
     lf2.close()
+
+
+def test_config2_fp16_hit_storage(lfmod, oracle, geometry, params):
+    """BASELINE.json configs[2]: fp16 storage of the hits for windows + seeding, fp32 fit.
+    Rule: >= 99.5 % of the fp32 oracle's tracks reproduced with identical hit lists, and the truth-matched
+    efficiency within 0.2 % absolute."""
+    from paper_2402_14670_b200 import truth
+    b = dg.generate_config(2)
+    assert dg.CONFIGS[2].hit_storage == 1
+    ref = oracle.run(geometry, params, b, threads=NTHREADS)
+    got = _gpu_run(lfmod, geometry, dict(params, hit_storage=1), b)
+    common, ig, ir = np.intersect1d(got.seed_idx, ref.seed_idx, return_indices=True)
+    same = (got.hit_idx[ig] == ref.hit_idx[ir]).all(1)
+    frac = same.sum() / ref.n_tracks
+    e_got = truth.evaluate(b, got.hit_idx, got.n_hits)
+    e_ref = truth.evaluate(b, ref.hit_idx, ref.n_hits)
+    print(f"config2 fp16: identical hit lists {frac:.5f} of {ref.n_tracks}; tracks {got.n_tracks}; "
+          f"eff {e_got.efficiency:.5f} vs {e_ref.efficiency:.5f}; ghost {e_got.ghost_rate:.5f} vs {e_ref.ghost_rate:.5f}")
+    assert frac >= 0.995
+    assert abs(e_got.efficiency - e_ref.efficiency) <= 0.002
+    # identical hit lists went through the fp32 fit; the winning triplet (the fit's expansion point) may
+    # differ, so states agree to fp32 rounding noise (cf. test_f32_build_matches_f64_build), not bitwise
+    d = np.abs(got.state[ig][same].astype(np.float64) - ref.state[ir][same].astype(np.float64))
+    assert d[:, 0].max() <= 2e-3 and d[:, 1].max() <= 2e-2 and d[:, 2].max() <= 3e-6 and d[:, 3].max() <= 3e-5
+    # the fp16 path is deterministic too
+    got2 = _gpu_run(lfmod, geometry, dict(params, hit_storage=1), b)
+    assert np.array_equal(got.hit_idx, got2.hit_idx) and np.array_equal(got.state.view(np.uint32), got2.state.view(np.uint32))
