@@ -110,6 +110,8 @@ def load_library() -> C.CDLL:
     lib.lf_destroy.argtypes = [C.c_void_p]
     lib.lf_get_info.restype = C.c_int
     lib.lf_get_info.argtypes = [C.c_void_p, C.POINTER(lf_info)]
+    lib.lf_set_host_chunk_events.restype = C.c_int
+    lib.lf_set_host_chunk_events.argtypes = [C.c_void_p, C.c_size_t]
     lib.lf_set_profiling.restype = C.c_int
     lib.lf_set_profiling.argtypes = [C.c_void_p, C.c_int]
     lib.lf_kernel_times.restype = C.c_int
@@ -258,6 +260,10 @@ class LookingForward:
         self._check(self._lib.lf_run_host(self._h, C.byref(seeds), C.byref(hits), hb.n_events, C.byref(tr),
                                           self._stream_ptr(stream)))
         return int(out.n_tracks[0])
+
+    def set_host_chunk_events(self, min_events_per_chunk: int):
+        """``lf_set_host_chunk_events``: pipeline granularity of :meth:`run_host`."""
+        self._check(self._lib.lf_set_host_chunk_events(self._h, int(min_events_per_chunk)))
 
     def close(self):
         if getattr(self, "_h", None) and self._h.value:

@@ -20,6 +20,10 @@ namespace {
 thread_local std::string g_create_error;
 constexpr size_t PROF_RING = 256;
 constexpr int N_PROF_EV = LF_N_KERNELS + 1;
+/* lf_run_host pipelines the batch in chunks of events: H2D of chunk c+1, kernels of chunk c and D2H of
+ * chunk c-1 overlap (PCIe is full duplex).  At most HOST_MAX_CHUNKS chunks of at least HOST_CHUNK_EVENTS. */
+constexpr int HOST_MAX_CHUNKS = 16;
+constexpr size_t HOST_CHUNK_EVENTS = 1024;
 
 struct HostBufs { /* device staging for lf_run_host */
   float* seeds = nullptr;      /* 5 * max_seeds */
@@ -28,8 +32,10 @@ struct HostBufs { /* device staging for lf_run_host */
   uint32_t* seg_off = nullptr;
   int32_t *hit_idx = nullptr, *seed_idx = nullptr, *n_hits = nullptr;
   float *state = nullptr, *quality = nullptr;
-  uint32_t *ev_off = nullptr, *n_tracks = nullptr;
-  uint32_t* pinned_count = nullptr; /* host, pinned */
+  uint32_t *ev_off = nullptr, *n_tracks = nullptr; /* ne + HOST_MAX_CHUNKS + 1; HOST_MAX_CHUNKS */
+  uint32_t* pinned_count = nullptr; /* host, pinned: HOST_MAX_CHUNKS counts, then the chunk-relative event offsets */
+  cudaStream_t s_h2d = nullptr, s_cnt = nullptr, s_d2h = nullptr; /* library-owned copy streams */
+  cudaEvent_t ev_start = nullptr, ev_h2d[HOST_MAX_CHUNKS] = {}, ev_comp[HOST_MAX_CHUNKS] = {}, ev_cnt[HOST_MAX_CHUNKS] = {};
   bool ready = false;
 };
 
@@ -53,6 +59,7 @@ struct lf_handle {
   uint32_t *ev_count, *ev_off, *tickets;
   size_t workspace_bytes;
   HostBufs hb;
+  size_t host_chunk_events = HOST_CHUNK_EVENTS;
   bool profiling = false;
   size_t prof_runs = 0;                 /* runs recorded since profiling was enabled */
   cudaEvent_t (*prof_ev)[N_PROF_EV] = nullptr;  /* ring of PROF_RING event sets */
@@ -151,7 +158,7 @@ const char* validate(const lf_geometry& G, const lf_params& P) {
 
 template <bool DEBUG>
 lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
-                 const lf_debug* dbg, cudaStream_t st) {
+                 const lf_debug* dbg, cudaStream_t st, size_t seed_base = 0) {
   const bool prof = h->profiling;
   cudaEvent_t* pe = prof ? h->prof_ev[h->prof_runs % PROF_RING] : nullptr;
   if (prof) LF_CUDA(h, cudaEventRecord(pe[0], st));
@@ -203,7 +210,7 @@ lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_
   if (work && seeds->n_seeds > 0) {
     const size_t total = seeds->n_seeds * lf::REC_WORDS;
     const unsigned blocks = (unsigned)((total + 255) / 256);
-    lf::lf_compact_kernel<<<blocks, 256, 0, st>>>(h->ws_rec, h->ws_rank, h->ws_event, h->ev_off, seeds->n_seeds,
+    lf::lf_compact_kernel<<<blocks, 256, 0, st>>>(h->ws_rec, h->ws_rank, h->ws_event, h->ev_off, seed_base, seeds->n_seeds,
                                                   out->hit_idx, out->seed_idx, out->n_hits, out->state, out->quality);
   }
   if (prof) {
@@ -344,6 +351,15 @@ lf_status lf_destroy(lf_handle* h) {
   cudaFree(b.hit_idx); cudaFree(b.seed_idx); cudaFree(b.n_hits); cudaFree(b.state); cudaFree(b.quality);
   cudaFree(b.ev_off); cudaFree(b.n_tracks);
   if (b.pinned_count) cudaFreeHost(b.pinned_count);
+  if (b.s_h2d) cudaStreamDestroy(b.s_h2d);
+  if (b.s_cnt) cudaStreamDestroy(b.s_cnt);
+  if (b.s_d2h) cudaStreamDestroy(b.s_d2h);
+  if (b.ev_start) cudaEventDestroy(b.ev_start);
+  for (int c = 0; c < HOST_MAX_CHUNKS; ++c) {
+    if (b.ev_h2d[c]) cudaEventDestroy(b.ev_h2d[c]);
+    if (b.ev_comp[c]) cudaEventDestroy(b.ev_comp[c]);
+    if (b.ev_cnt[c]) cudaEventDestroy(b.ev_cnt[c]);
+  }
   if (h->prof_ev) {
     for (size_t i = 0; i < PROF_RING; ++i)
       for (cudaEvent_t e : h->prof_ev[i])
@@ -416,11 +432,27 @@ lf_status lf_run_debug(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits,
   return launch<true>(h, seeds, hits, n_events, out, debug, (cudaStream_t)cuda_stream);
 }
 
+lf_status lf_set_host_chunk_events(lf_handle* h, size_t min_events_per_chunk) {
+  if (!h) return LF_ERR_INVALID_ARG;
+  if (min_events_per_chunk == 0) return fail(h, LF_ERR_INVALID_ARG, "lf_set_host_chunk_events: must be >= 1");
+  h->host_chunk_events = min_events_per_chunk;
+  return LF_OK;
+}
+
 lf_status lf_run_host(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
                       void* cuda_stream) {
   const lf_status st0 = check_run_args(h, seeds, hits, n_events, out);
   if (st0 != LF_OK) return st0;
   h->err.clear();
+  const uint32_t* so = seeds->event_offsets; /* HOST tables: the chunking reads them */
+  const uint32_t* go = hits->seg_offsets;
+  if (so[0] != 0 || go[0] != 0 || so[n_events] != seeds->n_seeds || go[n_events * lf::NSEG] != hits->n_hits)
+    return fail(h, LF_ERR_INVALID_ARG, "lf_run_host: offset tables do not match n_seeds / n_hits");
+  if (n_events == 0) {
+    out->event_offsets[0] = 0;
+    *out->n_tracks = 0;
+    return LF_OK;
+  }
   cudaStream_t st = (cudaStream_t)cuda_stream;
   HostBufs& b = h->hb;
   if (!b.ready) {
@@ -435,37 +467,84 @@ lf_status lf_run_host(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
     LF_CUDA(h, cudaMalloc(&b.n_hits, ns * sizeof(int32_t)));
     LF_CUDA(h, cudaMalloc(&b.state, ns * 5 * sizeof(float)));
     LF_CUDA(h, cudaMalloc(&b.quality, ns * sizeof(float)));
-    LF_CUDA(h, cudaMalloc(&b.ev_off, (ne + 1) * sizeof(uint32_t)));
-    LF_CUDA(h, cudaMalloc(&b.n_tracks, sizeof(uint32_t)));
-    LF_CUDA(h, cudaMallocHost(&b.pinned_count, sizeof(uint32_t)));
+    LF_CUDA(h, cudaMalloc(&b.ev_off, (ne + HOST_MAX_CHUNKS + 1) * sizeof(uint32_t)));
+    LF_CUDA(h, cudaMalloc(&b.n_tracks, HOST_MAX_CHUNKS * sizeof(uint32_t)));
+    LF_CUDA(h, cudaMallocHost(&b.pinned_count, (ne + 2 * HOST_MAX_CHUNKS + 1) * sizeof(uint32_t)));
+    LF_CUDA(h, cudaStreamCreateWithFlags(&b.s_h2d, cudaStreamNonBlocking));
+    LF_CUDA(h, cudaStreamCreateWithFlags(&b.s_cnt, cudaStreamNonBlocking));
+    LF_CUDA(h, cudaStreamCreateWithFlags(&b.s_d2h, cudaStreamNonBlocking));
+    LF_CUDA(h, cudaEventCreateWithFlags(&b.ev_start, cudaEventDisableTiming));
+    for (int c = 0; c < HOST_MAX_CHUNKS; ++c) {
+      LF_CUDA(h, cudaEventCreateWithFlags(&b.ev_h2d[c], cudaEventDisableTiming));
+      LF_CUDA(h, cudaEventCreateWithFlags(&b.ev_comp[c], cudaEventDisableTiming));
+      LF_CUDA(h, cudaEventCreateWithFlags(&b.ev_cnt[c], cudaEventDisableTiming));
+    }
     b.ready = true;
   }
-  const size_t ns = seeds->n_seeds, nh = hits->n_hits;
   const size_t stride = std::max<size_t>(h->max_seeds, 1);
+  const int n_chunks = (int)std::min<size_t>(HOST_MAX_CHUNKS, std::max<size_t>(1, n_events / h->host_chunk_events));
+  auto chunk_begin = [&](int c) { return (size_t)(((unsigned long long)n_events * (unsigned)c) / (unsigned)n_chunks); };
+  uint32_t* pin_cnt = b.pinned_count;
+  uint32_t* pin_off = b.pinned_count + HOST_MAX_CHUNKS; /* chunk c's n+1 relative offsets start at e0 + c */
+
+  /* the copy streams start after whatever the caller queued on `cuda_stream` before this call */
+  LF_CUDA(h, cudaEventRecord(b.ev_start, st));
+  LF_CUDA(h, cudaStreamWaitEvent(b.s_h2d, b.ev_start, 0));
+  LF_CUDA(h, cudaStreamWaitEvent(b.s_cnt, b.ev_start, 0));
+  LF_CUDA(h, cudaStreamWaitEvent(b.s_d2h, b.ev_start, 0));
+
+  /* ---- host -> device: the offset tables once, then seeds and hits chunk by chunk */
+  LF_CUDA(h, cudaMemcpyAsync(b.seed_off, so, (n_events + 1) * sizeof(uint32_t), cudaMemcpyHostToDevice, b.s_h2d));
+  LF_CUDA(h, cudaMemcpyAsync(b.seg_off, go, (n_events * lf::NSEG + 1) * sizeof(uint32_t), cudaMemcpyHostToDevice, b.s_h2d));
   const float* src[5] = {seeds->x, seeds->y, seeds->tx, seeds->ty, seeds->qop};
-  for (int i = 0; i < 5 && ns > 0; ++i)
-    LF_CUDA(h, cudaMemcpyAsync(b.seeds + i * stride, src[i], ns * sizeof(float), cudaMemcpyHostToDevice, st));
-  LF_CUDA(h, cudaMemcpyAsync(b.seed_off, seeds->event_offsets, (n_events + 1) * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
-  if (nh > 0) LF_CUDA(h, cudaMemcpyAsync(b.hits, hits->x, nh * sizeof(float), cudaMemcpyHostToDevice, st));
-  LF_CUDA(h, cudaMemcpyAsync(b.seg_off, hits->seg_offsets, (n_events * lf::NSEG + 1) * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
-  lf_seeds ds = {b.seeds, b.seeds + stride, b.seeds + 2 * stride, b.seeds + 3 * stride, b.seeds + 4 * stride, b.seed_off, ns};
-  lf_hits dh = {b.hits, b.seg_off, nh};
-  lf_tracks dt = {b.hit_idx, b.seed_idx, b.n_hits, b.state, b.quality, b.ev_off, b.n_tracks, stride};
-  const lf_status rs = launch<false>(h, &ds, &dh, n_events, &dt, nullptr, st);
-  if (rs != LF_OK) return rs;
-  LF_CUDA(h, cudaMemcpyAsync(b.pinned_count, b.n_tracks, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
-  LF_CUDA(h, cudaMemcpyAsync(out->event_offsets, b.ev_off, (n_events + 1) * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
-  LF_CUDA(h, cudaStreamSynchronize(st));
-  const size_t nt = *b.pinned_count;
-  *out->n_tracks = (uint32_t)nt;
-  if (nt > 0) {
-    LF_CUDA(h, cudaMemcpyAsync(out->hit_idx, b.hit_idx, nt * lf::NL * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-    LF_CUDA(h, cudaMemcpyAsync(out->seed_idx, b.seed_idx, nt * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-    LF_CUDA(h, cudaMemcpyAsync(out->n_hits, b.n_hits, nt * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-    LF_CUDA(h, cudaMemcpyAsync(out->state, b.state, nt * 5 * sizeof(float), cudaMemcpyDeviceToHost, st));
-    LF_CUDA(h, cudaMemcpyAsync(out->quality, b.quality, nt * sizeof(float), cudaMemcpyDeviceToHost, st));
-    LF_CUDA(h, cudaStreamSynchronize(st));
+  for (int c = 0; c < n_chunks; ++c) {
+    const size_t e0 = chunk_begin(c), e1 = chunk_begin(c + 1);
+    const size_t s0 = so[e0], s1 = so[e1], g0 = go[e0 * lf::NSEG], g1 = go[e1 * lf::NSEG];
+    for (int i = 0; i < 5 && s1 > s0; ++i)
+      LF_CUDA(h, cudaMemcpyAsync(b.seeds + i * stride + s0, src[i] + s0, (s1 - s0) * sizeof(float), cudaMemcpyHostToDevice, b.s_h2d));
+    if (g1 > g0) LF_CUDA(h, cudaMemcpyAsync(b.hits + g0, hits->x + g0, (g1 - g0) * sizeof(float), cudaMemcpyHostToDevice, b.s_h2d));
+    LF_CUDA(h, cudaEventRecord(b.ev_h2d[c], b.s_h2d));
   }
+  /* ---- kernels on the caller's stream, chunk by chunk; the counts follow on their own stream */
+  for (int c = 0; c < n_chunks; ++c) {
+    const size_t e0 = chunk_begin(c), e1 = chunk_begin(c + 1);
+    const size_t s0 = so[e0], s1 = so[e1], g0 = go[e0 * lf::NSEG], g1 = go[e1 * lf::NSEG];
+    LF_CUDA(h, cudaStreamWaitEvent(st, b.ev_h2d[c], 0));
+    lf_seeds ds = {b.seeds, b.seeds + stride, b.seeds + 2 * stride, b.seeds + 3 * stride, b.seeds + 4 * stride,
+                   b.seed_off + e0, s1 - s0};
+    lf_hits dh = {b.hits, b.seg_off + e0 * lf::NSEG, g1 - g0};
+    lf_tracks dt = {b.hit_idx + s0 * lf::NL, b.seed_idx + s0, b.n_hits + s0, b.state + s0 * 5, b.quality + s0,
+                    b.ev_off + e0 + c, b.n_tracks + c, stride - s0};
+    const lf_status rs = launch<false>(h, &ds, &dh, e1 - e0, &dt, nullptr, st, s0);
+    if (rs != LF_OK) return rs;
+    LF_CUDA(h, cudaEventRecord(b.ev_comp[c], st));
+    LF_CUDA(h, cudaStreamWaitEvent(b.s_cnt, b.ev_comp[c], 0));
+    LF_CUDA(h, cudaMemcpyAsync(pin_cnt + c, b.n_tracks + c, sizeof(uint32_t), cudaMemcpyDeviceToHost, b.s_cnt));
+    LF_CUDA(h, cudaMemcpyAsync(pin_off + e0 + c, b.ev_off + e0 + c, (e1 - e0) * sizeof(uint32_t), cudaMemcpyDeviceToHost, b.s_cnt));
+    LF_CUDA(h, cudaEventRecord(b.ev_cnt[c], b.s_cnt));
+  }
+  /* ---- device -> host: as soon as a chunk's count is known its tracks go to their final dense position */
+  size_t running = 0;
+  for (int c = 0; c < n_chunks; ++c) {
+    const size_t e0 = chunk_begin(c), e1 = chunk_begin(c + 1);
+    const size_t s0 = so[e0];
+    LF_CUDA(h, cudaEventSynchronize(b.ev_cnt[c]));
+    const size_t nt = pin_cnt[c];
+    if (nt > 0) {
+      LF_CUDA(h, cudaMemcpyAsync(out->hit_idx + running * lf::NL, b.hit_idx + s0 * lf::NL, nt * lf::NL * sizeof(int32_t), cudaMemcpyDeviceToHost, b.s_d2h));
+      LF_CUDA(h, cudaMemcpyAsync(out->seed_idx + running, b.seed_idx + s0, nt * sizeof(int32_t), cudaMemcpyDeviceToHost, b.s_d2h));
+      LF_CUDA(h, cudaMemcpyAsync(out->n_hits + running, b.n_hits + s0, nt * sizeof(int32_t), cudaMemcpyDeviceToHost, b.s_d2h));
+      LF_CUDA(h, cudaMemcpyAsync(out->state + running * 5, b.state + s0 * 5, nt * 5 * sizeof(float), cudaMemcpyDeviceToHost, b.s_d2h));
+      LF_CUDA(h, cudaMemcpyAsync(out->quality + running, b.quality + s0, nt * sizeof(float), cudaMemcpyDeviceToHost, b.s_d2h));
+    }
+    const uint32_t* rel = pin_off + e0 + c;
+    for (size_t e = e0; e < e1; ++e) out->event_offsets[e] = (uint32_t)(running + rel[e - e0]);
+    running += nt;
+  }
+  out->event_offsets[n_events] = (uint32_t)running;
+  *out->n_tracks = (uint32_t)running;
+  LF_CUDA(h, cudaStreamSynchronize(b.s_d2h));
+  LF_CUDA(h, cudaStreamSynchronize(st));
   return LF_OK;
 }
 

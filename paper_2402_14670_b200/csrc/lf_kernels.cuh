@@ -1008,10 +1008,12 @@ __global__ void __launch_bounds__(1024) lf_scan_kernel(const uint32_t* __restric
  * records, dense SoA writes in (event, seed) order. */
 __global__ void __launch_bounds__(256) lf_compact_kernel(const int32_t* __restrict__ ws_rec, const int32_t* __restrict__ ws_rank,
                                                          const int32_t* __restrict__ ws_event, const uint32_t* __restrict__ ev_off,
-                                                         size_t n_seeds, int32_t* __restrict__ hit_idx, int32_t* __restrict__ seed_idx,
-                                                         int32_t* __restrict__ n_hits, float* __restrict__ state, float* __restrict__ quality) {
-  const size_t gid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+                                                         size_t seed_base, size_t n_seeds, int32_t* __restrict__ hit_idx,
+                                                         int32_t* __restrict__ seed_idx, int32_t* __restrict__ n_hits,
+                                                         float* __restrict__ state, float* __restrict__ quality) {
+  size_t gid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (gid >= n_seeds * REC_WORDS) return;
+  gid += seed_base * REC_WORDS; /* the batch's seeds are [seed_base, seed_base + n_seeds) */
   const size_t seed = gid / REC_WORDS;
   const int wd = (int)(gid - seed * REC_WORDS);
   const int rank = ws_rank[seed];

@@ -172,6 +172,24 @@ def test_run_host_matches_device_path(lfmod, oracle, geometry, params):
         n = lf.run_host(hb, ht)
         assert n == ref.n_tracks
         assert_tracks_equal(ht.to_numpy(), ref, "host path")
+    # the chunked pipeline (H2D / kernels / D2H overlapped) gives the same dense output for any chunking,
+    # with pinned and with pageable host memory
+    for chunk, pin in ((7, True), (16, True), (64, False), (199, True)):
+        lf.set_host_chunk_events(chunk)
+        hb2, ht2 = lfmod.HostBatch(b, pin=pin), lfmod.HostTracks(b.n_seeds, b.n_events, pin=pin)
+        assert lf.run_host(hb2, ht2) == ref.n_tracks
+        assert_tracks_equal(ht2.to_numpy(), ref, f"host path, chunks of >= {chunk} events")
+    lf.close()
+    # fp16 hit storage goes through the same pipeline: chunked == unchunked
+    P16 = dict(params, hit_storage=1)
+    lf = lfmod.LookingForward(geometry, P16, b.n_events, b.n_seeds, b.n_hits)
+    ht_a, ht_b = lfmod.HostTracks(b.n_seeds, b.n_events), lfmod.HostTracks(b.n_seeds, b.n_events)
+    lf.run_host(hb, ht_a)
+    lf.set_host_chunk_events(13)
+    lf.run_host(hb, ht_b)
+    a, c = ht_a.to_numpy(), ht_b.to_numpy()
+    assert a.n_tracks == c.n_tracks and np.array_equal(a.hit_idx, c.hit_idx) and np.array_equal(a.event_offsets, c.event_offsets)
+    assert np.array_equal(a.state.view(np.uint32), c.state.view(np.uint32))
     lf.close()
 
 
