@@ -56,7 +56,7 @@ struct lf_handle {
   uint16_t* trip_code;
   uint8_t* n_trip;
   int32_t *ws_rec, *ws_nh, *ws_rank, *ws_event;
-  uint32_t *ev_count, *ev_off, *tickets;
+  uint32_t *ev_count, *ev_off, *ev_dup, *tickets;
   size_t workspace_bytes;
   HostBufs hb;
   size_t host_chunk_events = HOST_CHUNK_EVENTS;
@@ -172,6 +172,7 @@ lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_
   A.win = h->win; A.trip_code = h->trip_code; A.n_trip = h->n_trip;
   A.ws_rec = h->ws_rec; A.ws_nh = h->ws_nh; A.ws_rank = h->ws_rank; A.ws_event = h->ws_event;
   A.ev_count = h->ev_count;
+  A.ev_dup = h->ev_dup;
   if (dbg) {
     A.dbg.win_first = dbg->win_first; A.dbg.win_count = dbg->win_count; A.dbg.n_triplets = dbg->n_triplets;
     A.dbg.trip_hits = dbg->trip_hits; A.dbg.trip_set = dbg->trip_set; A.dbg.trip_chi2 = dbg->trip_chi2;
@@ -332,9 +333,10 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   LF_CREATE_CUDA(cudaMalloc(&h->ws_event, ns * sizeof(int32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ev_count, ne * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ev_off, (ne + 1) * sizeof(uint32_t)));
+  LF_CREATE_CUDA(cudaMalloc(&h->ev_dup, ne * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->tickets, lf::N_TICKETS * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMemset(h->tickets, 0, lf::N_TICKETS * sizeof(uint32_t)));
-  h->workspace_bytes = ns * (lf::NL * 4 + nt * 2 + 1 + (lf::REC_WORDS + 3) * 4) + (2 * ne + 1 + lf::N_TICKETS) * sizeof(uint32_t);
+  h->workspace_bytes = ns * (lf::NL * 4 + nt * 2 + 1 + (lf::REC_WORDS + 3) * 4) + (3 * ne + 1 + lf::N_TICKETS) * sizeof(uint32_t);
 #undef LF_CREATE_CUDA
   *out = h;
   return LF_OK;
@@ -345,7 +347,7 @@ lf_status lf_destroy(lf_handle* h) {
   cudaFree(h->hx16); cudaFree(h->origin16);
   cudaFree(h->win); cudaFree(h->trip_code); cudaFree(h->n_trip);
   cudaFree(h->ws_rec); cudaFree(h->ws_nh); cudaFree(h->ws_rank); cudaFree(h->ws_event);
-  cudaFree(h->ev_count); cudaFree(h->ev_off); cudaFree(h->tickets);
+  cudaFree(h->ev_count); cudaFree(h->ev_off); cudaFree(h->ev_dup); cudaFree(h->tickets);
   HostBufs& b = h->hb;
   cudaFree(b.seeds); cudaFree(b.seed_off); cudaFree(b.hits); cudaFree(b.seg_off);
   cudaFree(b.hit_idx); cudaFree(b.seed_idx); cudaFree(b.n_hits); cudaFree(b.state); cudaFree(b.quality);

@@ -89,6 +89,7 @@ struct EventArgs {
   int32_t* ws_rank;     /* n_seeds: rank among the event's tracks, -1 = none */
   int32_t* ws_event;    /* n_seeds: event of the seed */
   uint32_t* ev_count;   /* n_events */
+  uint32_t* ev_dup;     /* n_events: written by the window kernel, != 0 if two neighbouring staged hits are equal */
   DebugOut dbg;
 };
 
@@ -99,7 +100,7 @@ struct __align__(16) CtaHeader {
   int ev;
   int nsteps; /* binary-search steps that cover the event's longest segment */
   int warp_tot[8];
-  int pad[1];
+  int dup; /* != 0: the event may hold equal neighbouring hits (closest_hit must resolve runs of ties) */
 };
 constexpr int HDR_BYTES = (sizeof(CtaHeader) + 15) & ~15;
 
@@ -181,6 +182,7 @@ __device__ __forceinline__ bool fetch_event(const EventArgs& A, uint32_t& phase,
     for (int o = 16; o > 0; o >>= 1) len = max(len, __shfl_xor_sync(FULL, len, o));
     if (tid == 0) H.nsteps = 32 - __clz(len);
   }
+  if (tid == 32) H.dup = (int)A.ev_dup[E.ev]; /* meaningful in the seed and fit kernels only */
   const float* gsrc = A.hx + E.h0;
   E.staged = E.nh + 4 <= A.stage_cap;
   E.skew = (int)((reinterpret_cast<uintptr_t>(gsrc) >> 2) & 3);
@@ -232,9 +234,10 @@ __device__ __forceinline__ int bound_search(const HV& hx, int b, int e, float v,
 
 /* Closest hit to `pred` in the x-sorted window [f, f+n), n <= 32: first x >= pred by binary search,
  * then compare the two neighbours; ties -> lower index, including runs of equal distance on the low
- * side (equals a linear argmin with strict '<').  Returns the event-relative index, or -1 if n == 0. */
+ * side (equals a linear argmin with strict '<'); such a run needs two equal neighbouring hits, so the
+ * walk is skipped when the event has none (`dup` == false).  Returns the event-relative index, or -1 if n == 0. */
 template <class HV>
-__device__ __forceinline__ int closest_hit(const HV& hx, int f, int n, float pred) {
+__device__ __forceinline__ int closest_hit(const HV& hx, int f, int n, float pred, bool dup) {
   if (n <= 0) return -1;
   const int e = f + n;
   int pos = f;
@@ -250,7 +253,8 @@ __device__ __forceinline__ int closest_hit(const HV& hx, int f, int n, float pre
     const float dh = hx[pos] - pred;
     if (!(dk <= dh)) return pos;
   }
-  while (k > f && (pred - hx[k - 1]) == dk) --k;
+  if (dup) /* only events with equal neighbouring hits can have a run of ties */
+    while (k > f && (pred - hx[k - 1]) == dk) --k;
   return k;
 }
 
@@ -325,6 +329,17 @@ __device__ __forceinline__ void windows_of_event(const Consts& C, const EventArg
   }
 }
 
+/* ev_dup[event] = 1 iff two neighbouring hits of the event (as the kernels see them) are equal.  Only then can
+ * "closest hit" meet a run of equal distances, so the seed and fit kernels skip the tie walk otherwise.
+ * Conservative across segment boundaries (a false positive only costs the walk). */
+template <class HV>
+__device__ __forceinline__ void flag_equal_neighbours(const EventArgs& A, const EventCtx& E, const HV& hx) {
+  int dup = 0;
+  for (int i = threadIdx.x; i + 1 < E.nh; i += WIN_THREADS) dup |= (hx[i] == hx[i + 1]) ? 1 : 0;
+  dup = __syncthreads_or(dup);
+  if (threadIdx.x == 0) A.ev_dup[E.ev] = (uint32_t)dup;
+}
+
 template <bool DEBUG>
 __global__ void __launch_bounds__(WIN_THREADS) lf_window_kernel(const __grid_constant__ Consts C,
                                                                 const __grid_constant__ EventArgs A) {
@@ -333,8 +348,13 @@ __global__ void __launch_bounds__(WIN_THREADS) lf_window_kernel(const __grid_con
   uint32_t phase = 0;
   EventCtx E;
   while (fetch_event(A, phase, E)) {
-    if (E.staged) windows_of_event<DEBUG, true>(C, A, H, E, HitView<true>{E.skew});
-    else windows_of_event<DEBUG, false>(C, A, H, E, HitView<false>{A.hx + E.h0});
+    if (E.staged) {
+      flag_equal_neighbours(A, E, HitView<true>{E.skew});
+      windows_of_event<DEBUG, true>(C, A, H, E, HitView<true>{E.skew});
+    } else {
+      flag_equal_neighbours(A, E, HitView<false>{A.hx + E.h0});
+      windows_of_event<DEBUG, false>(C, A, H, E, HitView<false>{A.hx + E.h0});
+    }
   }
 }
 
@@ -367,102 +387,131 @@ __device__ __forceinline__ int select_smallest(SeedScratch& W, int n, int keep, 
   return n < keep ? n : keep;
 }
 
+/* Number of the warp's 32 lane values `xv` (ascending over the lanes, +inf padded) that are < v
+ * (INCLUSIVE == false) or <= v (true): binary search by shuffles, every lane with its own v. */
+template <bool INCLUSIVE>
+__device__ __forceinline__ int lanes_below(float xv, float v) {
+  int pos = 0;
+#pragma unroll
+  for (int s = 16; s >= 1; s >>= 1) {
+    const float xm = __shfl_sync(FULL, xv, pos + s - 1);
+    if (INCLUSIVE ? (xm <= v) : (xm < v)) pos += s;
+  }
+  const float xm = __shfl_sync(FULL, xv, pos); /* pos <= 31 here */
+  if (INCLUSIVE ? (xm <= v) : (xm < v)) pos += 1;
+  return pos;
+}
+
 template <bool DEBUG, class HV>
 __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& A, const HV& hx, uint32_t h0,
-                                              uint32_t seed, SeedScratch& W, int lane) {
+                                              uint32_t seed, SeedScratch& W, int lane, bool dup) {
   const float x = __ldg(A.sx + seed), tx = __ldg(A.stx + seed), qop = __ldg(A.sqop + seed);
   const float aq = fmaxf(fabsf(qop), 1e-6f);
   const float p = 1.0f / aq;
   const float x_mag = x + tx * C.mag_dz_seed;
   /* lanes 0..11 hold the packed window of layer `lane` */
   const uint32_t winw = (lane < NL) ? A.win[(size_t)seed * NL + lane] : 0u;
-  int tcount = 0;
   const unsigned lt_mask = (1u << lane) - 1u;
   const bool low_p = p < C.p_same_bend;
   const float tol0 = C.mag_tol_base + C.mag_tol_inv_p * aq;
-#pragma unroll 1
+  const float INF = __int_as_float(0x7f800000);
+  /* ---- per layer set: lanes = h0.  |x0 + t*zmag_a - x_mag| < tol is linear in x2 (t = (x2-x0)*inv_dz, slope
+   * r = inv_dz*zmag_a < 0) and tol <= tol_sup, so the survivors lie inside
+   * x2 in [x0 + (tol_sup - A)/r, x0 + (-tol_sup - A)/r], A = x0 - x_mag.  The margin in tol_sup (0.1 mm >> fp32
+   * rounding of these expressions) makes the bracket a strict superset; the h2 window sits one hit per lane,
+   * so both bracket ends are shuffle searches. */
+  float x0s[2];
+  int fbs[2], nbs[2], fcs[2];
+  unsigned cnt_p = 0, jlo_p = 0; /* set 0 in the low half-word, set 1 in the high one */
+#pragma unroll
   for (int set = 0; set < 2; ++set) {
     const int la = set ? 3 : 0;
     const uint32_t wa = __shfl_sync(FULL, winw, la), wb = __shfl_sync(FULL, winw, la + 4), wc = __shfl_sync(FULL, winw, la + 8);
-    const int fa = (int)(wa >> 6), na = (int)(wa & 63u), fb = (int)(wb >> 6), nb = (int)(wb & 63u);
-    const int fc = (int)(wc >> 6), nc = (int)(wc & 63u);
-    if (na == 0 || nb == 0 || nc == 0) continue;
-    const float inv_dz = C.inv_dz_ac[set], zmag_a = C.zmag_a[set], inv_r = C.inv_r[set];
-    const float zb = C.z[la + 4], za = C.z[la], Kx1 = C.K[set];
-    /* lanes = h0.  |x0 + t*zmag_a - x_mag| < tol is linear in x2 (t = (x2-x0)*inv_dz, slope
-     * r = inv_dz*zmag_a < 0) and tol <= tol_sup, so the survivors lie inside
-     * x2 in [x0 + (tol_sup - A)/r, x0 + (-tol_sup - A)/r], A = x0 - x_mag.  The margin in tol_sup
-     * (0.1 mm >> fp32 rounding of these expressions) makes the bracket a strict superset. */
+    const int fa = (int)(wa >> 6), na = (int)(wa & 63u), nc = (int)(wc & 63u);
+    fbs[set] = (int)(wb >> 6);
+    nbs[set] = (int)(wb & 63u);
+    fcs[set] = (int)(wc >> 6);
+    x0s[set] = 0.0f;
+    if (na == 0 || nbs[set] == 0 || nc == 0) continue; /* warp-uniform */
+    const float inv_dz = C.inv_dz_ac[set], inv_r = C.inv_r[set];
     const bool have = lane < na;
     const float x0 = have ? hx[fa + lane] : 0.0f;
-    const int ec = fc + nc;
-    const float xc_lo = hx[fc], xc_hi = hx[ec - 1];
+    const float x2v = (lane < nc) ? hx[fcs[set] + lane] : INF;
+    const float xc_lo = __shfl_sync(FULL, x2v, 0), xc_hi = __shfl_sync(FULL, x2v, nc - 1);
     const float tmax = fmaxf(fabsf((xc_lo - x0) * inv_dz), fabsf((xc_hi - x0) * inv_dz));
     const float tol_sup = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * tmax) + INTERVAL_MARGIN;
     const float Aoff = x0 - x_mag;
-    const float x2_lo = x0 + (tol_sup - Aoff) * inv_r;
-    const float x2_hi = x0 + (-tol_sup - Aoff) * inv_r;
-    int jlo = fc, jhi = fc; /* first x2 >= x2_lo; first x2 > x2_hi */
-#pragma unroll
-    for (int s = 5; s >= 0; --s) {
-      const int pl = jlo + (1 << s), ph = jhi + (1 << s);
-      if (pl <= ec && hx[pl - 1] < x2_lo) jlo = pl;
-      if (ph <= ec && hx[ph - 1] <= x2_hi) jhi = ph;
-    }
+    const int jlo = lanes_below<false>(x2v, x0 + (tol_sup - Aoff) * inv_r);  /* first x2 >= lower end */
+    const int jhi = lanes_below<true>(x2v, x0 + (-tol_sup - Aoff) * inv_r);  /* first x2 > upper end */
     const int cnt = have ? max(jhi - jlo, 0) : 0;
-    /* dense lane-per-candidate evaluation: inclusive scan of the per-h0 counts */
-    int incl = cnt;
+    x0s[set] = x0;
+    cnt_p |= (unsigned)cnt << (16 * set);
+    jlo_p |= (unsigned)jlo << (16 * set);
+  }
+  /* ---- dense lane-per-candidate evaluation over both sets: inclusive scan of the per-h0 counts */
+  unsigned incl_p = cnt_p;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int v = __shfl_up_sync(FULL, incl, o);
-      if (lane >= o) incl += v;
+  for (int o = 1; o < 32; o <<= 1) {
+    const unsigned v = __shfl_up_sync(FULL, incl_p, o);
+    if (lane >= o) incl_p += v;
+  }
+  const unsigned tot_p = __shfl_sync(FULL, incl_p, 31);
+  const int total0 = (int)(tot_p & 0xFFFFu), total = total0 + (int)(tot_p >> 16);
+  int tcount = 0;
+  for (int base = 0; base < total; base += 32) {
+    const int tau = base + lane;
+    const bool act = tau < total;
+    const int set = (tau >= total0) ? 1 : 0;
+    const int ts = set ? tau - total0 : tau;
+    const unsigned sel = set ? 0x4432u : 0x4410u; /* __byte_perm selector: this set's half-word */
+    int owner = 0; /* number of lanes whose inclusive count is <= ts == the h0 lane owning candidate ts */
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) {
+      const unsigned v = __shfl_sync(FULL, incl_p, owner + s - 1);
+      if ((int)__byte_perm(v, 0u, sel) <= ts) owner += s;
     }
-    const int total = __shfl_sync(FULL, incl, 31);
-    for (int base = 0; base < total; base += 32) {
-      const int tau = base + lane;
-      const bool act = tau < total;
-      int owner = 0; /* number of lanes whose inclusive count is <= tau == the h0 lane owning candidate tau */
-#pragma unroll
-      for (int s = 4; s >= 0; --s) {
-        const int probe = owner + (1 << s);
-        const int v = __shfl_sync(FULL, incl, probe - 1);
-        if (v <= tau) owner = probe;
-      }
-      owner = min(owner, 31);
-      const int before = __shfl_sync(FULL, incl, owner) - __shfl_sync(FULL, cnt, owner);
-      const int j = __shfl_sync(FULL, jlo, owner) + (tau - before);
-      const float x0o = __shfl_sync(FULL, x0, owner);
-      bool pass = false;
-      unsigned long long key = 0;
-      if (act) {
-        /* the exact predicate is the definition */
-        const float x2 = hx[j];
-        const float t = (x2 - x0o) * inv_dz;
-        bool ok = true;
-        if (low_p) ok = (t - tx) * qop > 0.0f; /* filter 1: same bending direction */
-        const float x_at_mag = x0o + t * zmag_a;
-        const float tol = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * fabsf(t));
-        ok = ok && (fabsf(x_at_mag - x_mag) < tol); /* filter 2: opening at the magnet centre */
-        if (ok) {
-          /* x1_expected, closest h1, chi2 cut */
-          const float x1e = zb * t + (x0o - t * za) * Kx1;
-          const int k = closest_hit(hx, fb, nb, x1e);
-          const float dx = hx[k] - x1e;
-          const float chi2 = dx * dx;
-          if (chi2 < C.T_triplet) {
-            pass = true;
-            key = ((unsigned long long)__float_as_uint(chi2) << 32) |
-                  (unsigned)((set << 15) | (owner << 10) | ((j - fc) << 5) | (k - fb));
-          }
+    owner = min(owner, 31);
+    const unsigned ip = __shfl_sync(FULL, incl_p, owner), cp = __shfl_sync(FULL, cnt_p, owner);
+    const unsigned jp = __shfl_sync(FULL, jlo_p, owner);
+    const int before = (int)__byte_perm(ip, 0u, sel) - (int)__byte_perm(cp, 0u, sel);
+    const int j = (int)__byte_perm(jp, 0u, sel) + (ts - before); /* h2 index inside its window */
+    const float xa = __shfl_sync(FULL, x0s[0], owner), xb = __shfl_sync(FULL, x0s[1], owner);
+    const float x0o = set ? xb : xa;
+    bool pass = false;
+    unsigned long long key = 0;
+    if (act) {
+      /* the exact predicate is the definition */
+      const int la = set ? 3 : 0;
+      const int fb = set ? fbs[1] : fbs[0], nb = set ? nbs[1] : nbs[0], fc = set ? fcs[1] : fcs[0];
+      const float inv_dz = set ? C.inv_dz_ac[1] : C.inv_dz_ac[0], zmag_a = set ? C.zmag_a[1] : C.zmag_a[0];
+      const float x2 = hx[fc + j];
+      const float t = (x2 - x0o) * inv_dz;
+      bool ok = true;
+      if (low_p) ok = (t - tx) * qop > 0.0f; /* filter 1: same bending direction */
+      const float x_at_mag = x0o + t * zmag_a;
+      const float tol = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * fabsf(t));
+      ok = ok && (fabsf(x_at_mag - x_mag) < tol); /* filter 2: opening at the magnet centre */
+      if (ok) {
+        /* x1_expected, closest h1, chi2 cut */
+        const float zb = set ? C.z[7] : C.z[4], za = set ? C.z[3] : C.z[0], Kx1 = set ? C.K[1] : C.K[0];
+        const float x1e = zb * t + (x0o - t * za) * Kx1;
+        const int k = closest_hit(hx, fb, nb, x1e, dup);
+        const float dx = hx[k] - x1e;
+        const float chi2 = dx * dx;
+        if (chi2 < C.T_triplet) {
+          pass = true;
+          key = ((unsigned long long)__float_as_uint(chi2) << 32) |
+                (unsigned)((set << 15) | (owner << 10) | (j << 5) | (k - fb));
         }
       }
-      const unsigned m = __ballot_sync(FULL, pass);
-      if (m) {
-        if (tcount > 32) tcount = select_smallest(W, tcount, C.n_triplets, lane);
-        if (pass) W.trip[tcount + __popc(m & lt_mask)] = key;
-        tcount += __popc(m);
-        __syncwarp();
-      }
+      (void)la;
+    }
+    const unsigned m = __ballot_sync(FULL, pass);
+    if (m) {
+      if (tcount > 32) tcount = select_smallest(W, tcount, C.n_triplets, lane);
+      if (pass) W.trip[tcount + __popc(m & lt_mask)] = key;
+      tcount += __popc(m);
+      __syncwarp();
     }
   }
   if (tcount > 0) tcount = select_smallest(W, tcount, C.n_triplets, lane); /* sorted in (chi2,set,h0,h2) order */
@@ -499,7 +548,7 @@ struct __align__(16) SeedTables {
 };
 
 template <bool DEBUG>
-__global__ void __launch_bounds__(SEED_THREADS, 6) lf_seed_kernel(const __grid_constant__ Consts C,
+__global__ void __launch_bounds__(SEED_THREADS, 5) lf_seed_kernel(const __grid_constant__ Consts C,
                                                                const __grid_constant__ EventArgs A) {
   CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
   SeedTables& T = *reinterpret_cast<SeedTables*>(lf_smem + HDR_BYTES + (size_t)A.stage_cap * sizeof(float));
@@ -513,13 +562,17 @@ __global__ void __launch_bounds__(SEED_THREADS, 6) lf_seed_kernel(const __grid_c
   while (fetch_event(A, phase, E)) {
     const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
     SeedScratch& W = T.ws[warp];
-    for (;;) {
+    const bool dup = H.dup != 0;
+    for (;;) { /* the warps of the CTA share the event's seeds, two per ticket */
       int k = 0;
-      if (lane == 0) k = atomicAdd(&T.next_seed, 1);
+      if (lane == 0) k = atomicAdd(&T.next_seed, 2);
       k = __shfl_sync(FULL, k, 0);
       if (s0 + (uint32_t)k >= s1) break;
-      if (E.staged) seed_triplets<DEBUG>(C, A, HitView<true>{E.skew}, E.h0, s0 + (uint32_t)k, W, lane);
-      else seed_triplets<DEBUG>(C, A, HitView<false>{A.hx + E.h0}, E.h0, s0 + (uint32_t)k, W, lane);
+      const int kend = min(k + 2, (int)(s1 - s0));
+      for (; k < kend; ++k) {
+        if (E.staged) seed_triplets<DEBUG>(C, A, HitView<true>{E.skew}, E.h0, s0 + (uint32_t)k, W, lane, dup);
+        else seed_triplets<DEBUG>(C, A, HitView<false>{A.hx + E.h0}, E.h0, s0 + (uint32_t)k, W, lane, dup);
+      }
     }
     __syncthreads();
     if (threadIdx.x == 0) T.next_seed = 0; /* published by fetch_event's barriers */
@@ -562,7 +615,7 @@ __device__ __forceinline__ void triplet_parabola(const Consts& C, const HV& hx, 
  * `geo` is the shared-memory copy of the per-layer constants: d, w, dzs, tana (12 floats each). */
 template <class HV>
 __device__ __noinline__ CandHits extend_candidate(const Consts& C, const HV& hx, const uint32_t* winw, const float* geo,
-                                                  float y, float tx, float ty, unsigned code) {
+                                                  float y, float tx, float ty, unsigned code, bool dup) {
   const int set = (code >> 15) & 1, la = set ? 3 : 0;
   float a0, t0, c0;
   triplet_parabola(C, hx, winw, code, a0, t0, c0);
@@ -584,7 +637,7 @@ __device__ __noinline__ CandHits extend_candidate(const Consts& C, const HV& hx,
     if (uv) pred = pred + (y + ty * geo[2 * NL + l]) * geo[3 * NL + l];
     const uint32_t ww = winw[l];
     const int f = (int)(ww >> 6);
-    const int k = closest_hit(hx, f, (int)(ww & 63u), pred);
+    const int k = closest_hit(hx, f, (int)(ww & 63u), pred, dup);
     if (k >= 0) {
       const float dx = hx[k] - pred;
       const float chi2 = dx * dx;
@@ -770,6 +823,7 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
   const int NT = C.n_triplets;
   const float INF = __int_as_float(0x7f800000);
   uint4* myq = T.queue + warp * 64;
+  const bool dup = H.dup != 0;
   int ev_tracks = 0;
   for (int cb = 0; cb < ns; cb += FIT_CHUNK) {
     const int cn = min(FIT_CHUNK, ns - cb);
@@ -818,7 +872,7 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
         const int sl = (int)(im >> 4), k = (int)(im & 15u);
         const uint32_t seed = sbase + (uint32_t)sl;
         const unsigned code = A.trip_code[(size_t)seed * NT + k];
-        h = extend_candidate(C, hx, T.win + sl * NL, T.geo, T.sp[sl * 4 + 0], T.sp[sl * 4 + 1], T.sp[sl * 4 + 2], code);
+        h = extend_candidate(C, hx, T.win + sl * NL, T.geo, T.sp[sl * 4 + 0], T.sp[sl * 4 + 1], T.sp[sl * 4 + 2], code, dup);
         enough = h.enough;
         if (!enough) T.Q[it] = INF;
         if (DEBUG) {
@@ -872,7 +926,7 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
       if (found) {
         const unsigned code = A.trip_code[(size_t)seed * NT + bk];
         const float y = T.sp[tid * 4 + 0], tx = T.sp[tid * 4 + 1], ty = T.sp[tid * 4 + 2];
-        const CandHits h = extend_candidate(C, hx, T.win + tid * NL, T.geo, y, tx, ty, code);
+        const CandHits h = extend_candidate(C, hx, T.win + tid * NL, T.geo, y, tx, ty, code, dup);
         fit_candidate(C, hx, T.win + tid * NL, y, tx, ty, code, h, E.h0, seed, A.ws_rec + (size_t)seed * REC_WORDS);
       }
       A.ws_nh[seed] = found ? 1 : 0;
