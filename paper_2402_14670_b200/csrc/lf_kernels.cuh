@@ -235,9 +235,11 @@ __device__ __forceinline__ int bound_search(const HV& hx, int b, int e, float v,
 /* Closest hit to `pred` in the x-sorted window [f, f+n), n <= 32: first x >= pred by binary search,
  * then compare the two neighbours; ties -> lower index, including runs of equal distance on the low
  * side (equals a linear argmin with strict '<'); such a run needs two equal neighbouring hits, so the
- * walk is skipped when the event has none (`dup` == false).  Returns the event-relative index, or -1 if n == 0. */
+ * walk is skipped when the event has none (`dup` == false).  Returns the event-relative index, or -1 if
+ * n == 0, and in `dist` the distance |x - pred| of that hit (x - pred and pred - x round to the same
+ * magnitude, so dist*dist is bit-identical to (x - pred)^2).  Generic version (global-memory view). */
 template <class HV>
-__device__ __forceinline__ int closest_hit(const HV& hx, int f, int n, float pred, bool dup) {
+__device__ __forceinline__ int closest_hit(const HV& hx, int f, int n, float pred, bool dup, float& dist) {
   if (n <= 0) return -1;
   const int e = f + n;
   int pos = f;
@@ -246,16 +248,108 @@ __device__ __forceinline__ int closest_hit(const HV& hx, int f, int n, float pre
     const int probe = pos + (1 << s);
     if (probe <= e && hx[probe - 1] < pred) pos = probe;
   }
-  if (pos == f) return f;
+  if (pos == f) {
+    dist = hx[f] - pred;
+    return f;
+  }
   int k = pos - 1;
   const float dk = pred - hx[k];
   if (pos < e) {
     const float dh = hx[pos] - pred;
-    if (!(dk <= dh)) return pos;
+    if (!(dk <= dh)) {
+      dist = dh;
+      return pos;
+    }
   }
+  dist = dk;
   if (dup) /* only events with equal neighbouring hits can have a run of ties */
     while (k > f && (pred - hx[k - 1]) == dk) --k;
   return k;
+}
+
+/* The same on the staged hits: positions are 32-bit shared-memory byte addresses, so one search step is
+ * add, bound check, LDS, compare, select. */
+__device__ __forceinline__ float lds_f32(uint32_t addr) {
+  float v;
+  asm("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ int closest_hit(const HitView<true>& hx, int f, int n, float pred, bool dup, float& dist) {
+  if (n <= 0) return -1;
+  const uint32_t a = smem_u32(stage_buf()) + 4u * (uint32_t)(hx.off + f);
+  const uint32_t end = a + 4u * (uint32_t)n;
+  uint32_t p = a;
+#pragma unroll
+  for (uint32_t s = 128u; s >= 4u; s >>= 1) {
+    const uint32_t q = p + s;
+    if (q <= end && lds_f32(q - 4u) < pred) p = q;
+  }
+  if (p == a) {
+    dist = lds_f32(a) - pred;
+    return f;
+  }
+  const float dk = pred - lds_f32(p - 4u);
+  if (p < end) {
+    const float dh = lds_f32(p) - pred;
+    if (!(dk <= dh)) {
+      dist = dh;
+      return f + (int)((p - a) >> 2);
+    }
+  }
+  dist = dk;
+  uint32_t k = p - 4u;
+  if (dup)
+    while (k > a && (pred - lds_f32(k - 4u)) == dk) k -= 4u;
+  return f + (int)((k - a) >> 2);
+}
+
+/* G independent closest-hit searches in lockstep, branch-free: the G chains of dependent LDS overlap
+ * (instruction-level parallelism instead of occupancy).  ww[g] is the packed window (first << 6 | count),
+ * krel[g] the index of the closest hit inside its window (-1 and dist = +inf if the window is empty). */
+template <int G>
+__device__ __forceinline__ void closest_group(const HitView<true>& hx, const uint32_t (&ww)[G], const float (&pred)[G],
+                                              bool dup, int (&krel)[G], float (&dist)[G]) {
+  const float INF = __int_as_float(0x7f800000);
+  const uint32_t base = smem_u32(stage_buf()) + 4u * (uint32_t)hx.off;
+  uint32_t a[G], end[G], p[G];
+#pragma unroll
+  for (int g = 0; g < G; ++g) {
+    a[g] = base + 4u * (ww[g] >> 6);
+    end[g] = a[g] + 4u * (ww[g] & 63u);
+    p[g] = a[g];
+  }
+#pragma unroll
+  for (uint32_t s = 128u; s >= 4u; s >>= 1) {
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+      const uint32_t q = p[g] + s;
+      const float x = (q <= end[g]) ? lds_f32(q - 4u) : INF;
+      p[g] = (x < pred[g]) ? q : p[g];
+    }
+  }
+#pragma unroll
+  for (int g = 0; g < G; ++g) {
+    const float xl = (p[g] > a[g]) ? lds_f32(p[g] - 4u) : -INF;
+    const float xh = (p[g] < end[g]) ? lds_f32(p[g]) : INF;
+    const float dk = pred[g] - xl, dh = xh - pred[g];
+    const bool right = !(dk <= dh); /* ties -> lower index */
+    uint32_t k = right ? p[g] : p[g] - 4u;
+    dist[g] = right ? dh : dk;
+    if (dup && !right)
+      while (k > a[g] && (pred[g] - lds_f32(k - 4u)) == dk) k -= 4u;
+    krel[g] = (int)(k - a[g]) >> 2;
+  }
+}
+template <int G>
+__device__ __forceinline__ void closest_group(const HitView<false>& hx, const uint32_t (&ww)[G], const float (&pred)[G],
+                                              bool dup, int (&krel)[G], float (&dist)[G]) {
+#pragma unroll
+  for (int g = 0; g < G; ++g) {
+    const int f = (int)(ww[g] >> 6);
+    dist[g] = __int_as_float(0x7f800000);
+    const int k = closest_hit(hx, f, (int)(ww[g] & 63u), pred[g], dup, dist[g]);
+    krel[g] = (k < 0) ? -1 : k - f;
+  }
 }
 
 /* ============================================================================================
@@ -495,8 +589,8 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
         /* x1_expected, closest h1, chi2 cut */
         const float zb = set ? C.z[7] : C.z[4], za = set ? C.z[3] : C.z[0], Kx1 = set ? C.K[1] : C.K[0];
         const float x1e = zb * t + (x0o - t * za) * Kx1;
-        const int k = closest_hit(hx, fb, nb, x1e, dup);
-        const float dx = hx[k] - x1e;
+        float dx;
+        const int k = closest_hit(hx, fb, nb, x1e, dup, dx);
         const float chi2 = dx * dx;
         if (chi2 < C.T_triplet) {
           pass = true;
@@ -621,36 +715,46 @@ __device__ __noinline__ CandHits extend_candidate(const Consts& C, const HV& hx,
   triplet_parabola(C, hx, winw, code, a0, t0, c0);
   const float T_uv = fmaxf(C.T_uv_min, C.T_uv_slope * (fabsf(tx) + fabsf(ty)));
   CandHits h;
-  h.w[0] = h.w[1] = h.w[2] = 0xFFFFFFFFu;
-  /* the triplet's own hits on layers la, la+4, la+8 */
-  const unsigned sh = 8u * (unsigned)la;
-  h.w[0] = (h.w[0] & ~(0xFFu << sh)) | (((code >> 10) & 31u) << sh);
-  h.w[1] = (h.w[1] & ~(0xFFu << sh)) | ((code & 31u) << sh);
-  h.w[2] = (h.w[2] & ~(0xFFu << sh)) | (((code >> 5) & 31u) << sh);
+  /* per station: the triplet's own hit (byte 0 for set 0, byte 3 for set 1) and the three other layers,
+   * searched in lockstep */
+  const unsigned trip[3] = {(code >> 10) & 31u, code & 31u, (code >> 5) & 31u};
+  const unsigned tsh = set ? 24u : 0u, sh0 = set ? 0u : 8u;
   int n = 3, n_uv = 0;
   unsigned st_mask = 0;
 #pragma unroll
-  for (int li = 0; li < 9; ++li) {
-    const int l = li + li / 3 + (1 - set); /* the 9 layers outside the set, ascending */
-    const bool uv = (li % 3) != (set ? 0 : 2); /* set 0: layers 1,2,3 -> u,v,x; set 1: 0,1,2 -> x,u,v */
-    float pred = (a0 + t0 * geo[l]) + c0 * geo[NL + l];
-    if (uv) pred = pred + (y + ty * geo[2 * NL + l]) * geo[3 * NL + l];
-    const uint32_t ww = winw[l];
-    const int f = (int)(ww >> 6);
-    const int k = closest_hit(hx, f, (int)(ww & 63u), pred, dup);
-    if (k >= 0) {
-      const float dx = hx[k] - pred;
-      const float chi2 = dx * dx;
-      if (chi2 < (uv ? T_uv : C.T_x)) {
-        const unsigned s8 = 8u * (unsigned)(l & 3);
-        const unsigned v = (unsigned)(k - f);
-        if (li < 3) h.w[0] = (h.w[0] & ~(0xFFu << s8)) | (v << s8);
-        else if (li < 6) h.w[1] = (h.w[1] & ~(0xFFu << s8)) | (v << s8);
-        else h.w[2] = (h.w[2] & ~(0xFFu << s8)) | (v << s8);
+  for (int st = 0; st < 3; ++st) {
+    const int l0 = st * 4 + (1 - set); /* layers l0, l0+1, l0+2: set 0 -> u, v, x; set 1 -> x, u, v */
+    uint32_t ww[3];
+    float pred[3], dist[3];
+    int krel[3];
+#pragma unroll
+    for (int g = 0; g < 3; ++g) {
+      const int l = l0 + g;
+      ww[g] = winw[l];
+      pred[g] = (a0 + t0 * geo[l]) + c0 * geo[NL + l];
+    }
+    /* stereo layers: + y(z_l) * tan(alpha_l) */
+    if (set) {
+      pred[1] = pred[1] + (y + ty * geo[2 * NL + l0 + 1]) * geo[3 * NL + l0 + 1];
+      pred[2] = pred[2] + (y + ty * geo[2 * NL + l0 + 2]) * geo[3 * NL + l0 + 2];
+    } else {
+      pred[0] = pred[0] + (y + ty * geo[2 * NL + l0]) * geo[3 * NL + l0];
+      pred[1] = pred[1] + (y + ty * geo[2 * NL + l0 + 1]) * geo[3 * NL + l0 + 1];
+    }
+    closest_group<3>(hx, ww, pred, dup, krel, dist);
+    unsigned w = (trip[st] << tsh) | (0x00FFFFFFu << sh0);
+#pragma unroll
+    for (int g = 0; g < 3; ++g) {
+      const bool uv = set ? (g != 0) : (g != 2);
+      const float chi2 = dist[g] * dist[g];
+      if (chi2 < (uv ? T_uv : C.T_x)) { /* an empty window gives chi2 = +inf */
+        const unsigned sh = sh0 + 8u * (unsigned)g;
+        w = (w & ~(0xFFu << sh)) | ((unsigned)krel[g] << sh);
         ++n;
-        if (uv) { ++n_uv; st_mask |= 1u << (li / 3); }
+        if (uv) { ++n_uv; st_mask |= 1u << st; }
       }
     }
+    h.w[st] = w;
   }
   h.n = n;
   h.n_uv = n_uv;
