@@ -115,15 +115,17 @@ def algorithmic_bytes(batch, n_tracks: int) -> int:
                + 80 * n_tracks + 4 * (batch.n_events + 1) + 4)
 
 
-def kernel_bytes(batch, n_tracks: int, n_triplets: int) -> dict:
+def kernel_bytes(batch, n_tracks: int, n_triplets: int, n_acc: int = 0) -> dict:
     """Algorithmic HBM bytes per launch of each event kernel: every kernel stages the
     event's hits once and reads/writes its own per-seed tables once."""
     H, S, E = batch.n_hits, batch.n_seeds, batch.n_events
     common = 4 * H + batch.seg_offsets.nbytes + batch.seed_offsets.nbytes
     trip = (2 * n_triplets + 1) * S
-    return {"window": common + 20 * S + 48 * S,
+    acc = 16 * n_acc  # one 16-byte record per candidate that passed the hit-count rule
+    return {"window": common + 20 * S + 48 * S + 4 * E,
             "seed": common + 12 * S + 48 * S + trip,
-            "fit": common + 12 * S + 48 * S + trip + 80 * n_tracks + 12 * S + 4 * E,
+            "extend": common + 12 * S + 48 * S + trip + acc + 4 * S + 4 * E,
+            "fit": common + 4 * E + acc + n_acc * (48 + 12 + 2) + 80 * n_tracks + 16 * S,
             "compact": 92 * S + 80 * n_tracks + 4 * E}
 
 
@@ -208,6 +210,7 @@ def run_ours(args):
         lf.run(db, out, stream)
     barrier()
     n_tracks = int(out.n_tracks.cpu()[0])
+    n_acc, n_dup_events = lf.run_counters()
 
     # ---- timed region: K steps, inputs resident in HBM, per-kernel CUDA events recorded by the library
     lf.set_profiling(True)
@@ -255,8 +258,8 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel (the slowest of the three event kernels)
     peak, peak_src = measured_peaks()
-    kb = kernel_bytes(batch, n_tracks, int(P["n_triplets"]))
-    dom = max(("window", "seed", "fit"), key=lambda k: ktimes[k])
+    kb = kernel_bytes(batch, n_tracks, int(P["n_triplets"]), n_acc)
+    dom = max(binding.EVENT_KERNELS, key=lambda k: ktimes[k])
     achieved = kb[dom] / (ktimes[dom] * 1e-3) / 1e9
     path_bytes = algorithmic_bytes(batch, n_tracks)
     path_gbs = path_bytes / (local_ms / args.steps * 1e-3) / 1e9
@@ -301,7 +304,7 @@ def run_ours(args):
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"{cfg.name}: {batch.n_events} events per GPU, Run-3-like occupancy, fp32, one lf_run on one stream",
                    "events_per_gpu": batch.n_events, "seeds_per_gpu": batch.n_seeds, "hits_per_gpu": batch.n_hits,
-                   "tracks_per_step_per_gpu": n_tracks,
+                   "tracks_per_step_per_gpu": n_tracks, "accepted_candidates_per_step": n_acc, "events_with_equal_hits": n_dup_events,
                    "l2": f"no flush: inputs ({in_bytes / 1e6:.0f} MB) + outputs exceed the 126 MB L2",
                    "sharding": "events, no data-path collective"},
         "seeds_per_s": tot_seeds / (ms_per_step * 1e-3),
@@ -311,7 +314,7 @@ def run_ours(args):
         "kernels": {"ms": ktimes, "algorithmic_bytes": kb,
                     "launch": {n: {"regs": info.regs[i], "block": info.block[i], "grid": info.grid[i],
                                    "ctas_per_sm": info.ctas_per_sm[i], "smem_bytes": info.smem_bytes[i]}
-                               for i, n in enumerate(("window", "seed", "fit"))},
+                               for i, n in enumerate(binding.EVENT_KERNELS)},
                     "staged_hits_per_event": info.staged_hits_per_event},
         "context": {"paper_hlt1_sequence_khz_a5000": 130, "paper_lf_share": 0.20,
                     "note": "paper numbers are whole-HLT1 on RTX A5000 (PAPER.md:342): context, not a target"},

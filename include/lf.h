@@ -39,7 +39,7 @@
 extern "C" {
 #endif
 
-#define LF_ABI_VERSION 1u
+#define LF_ABI_VERSION 2u
 #define LF_N_LAYERS 12   /* three T-stations, x-u-v-x each */
 #define LF_N_ZONES 2     /* lower / upper half */
 #define LF_MAX_WINDOW 32   /* largest params.n_window this build supports (one warp lane per hit) */
@@ -127,23 +127,25 @@ typedef struct {
 } lf_debug;
 
 /* What the library launches, for benchmarks and occupancy reports (HOST struct, filled by lf_get_info).
- * Per-kernel arrays are indexed LF_K_WINDOW, LF_K_SEED, LF_K_FIT (the three event kernels). */
-#define LF_K_WINDOW 0
-#define LF_K_SEED 1
-#define LF_K_FIT 2
-#define LF_N_KERNELS 5 /* + LF_K_SCAN = 3, LF_K_COMPACT = 4 in lf_kernel_times */
+ * Per-kernel arrays are indexed LF_K_WINDOW .. LF_K_FIT (the four event kernels). */
+#define LF_K_WINDOW 0  /* a1, a2 */
+#define LF_K_SEED 1    /* a3 */
+#define LF_K_EXTEND 2  /* a4, a5 */
+#define LF_K_FIT 3     /* a6 + ranking of the event's tracks */
+#define LF_N_EVENT_KERNELS 4
+#define LF_N_KERNELS 6 /* + LF_K_SCAN = 4, LF_K_COMPACT = 5 (a7) in lf_kernel_times */
 typedef struct {
-  int32_t kernels_per_run;       /* kernel launches one lf_run enqueues (5; 6 with hit_storage = 1) */
-  int32_t regs[3], block[3], grid[3], ctas_per_sm[3];
-  int32_t smem_bytes[3];         /* dynamic shared memory per CTA */
+  int32_t kernels_per_run;       /* kernel launches one lf_run enqueues (6; 7 with hit_storage = 1) */
+  int32_t regs[LF_N_EVENT_KERNELS], block[LF_N_EVENT_KERNELS], grid[LF_N_EVENT_KERNELS], ctas_per_sm[LF_N_EVENT_KERNELS];
+  int32_t smem_bytes[LF_N_EVENT_KERNELS]; /* dynamic shared memory per CTA */
   int32_t staged_hits_per_event; /* events with more hits than this read hits from global memory */
   int32_t sm_count;
   size_t workspace_bytes;
 } lf_info;
 
 /* Creates a context for batches of at most max_events / max_seeds / max_hits.  Validates geometry
- * and params, uploads constants, allocates the workspace (about max_seeds*(141 + 2*n_triplets) +
- * max_events*8 bytes on the current CUDA device).  The shared-memory stage for one event's hits is sized
+ * and params, uploads constants, allocates the workspace (about max_seeds*(141 + 18*n_triplets) +
+ * max_events*16 bytes on the current CUDA device, sized for 180 GB parts).  The shared-memory stage for one event's hits is sized
  * from the maxima: 1.25 * max_hits / max_events + 512 hits, clamped to [2048, 16384]; larger events are
  * still processed correctly, reading their hits from global memory.  *out is set only on LF_OK.
  * HOST pointers. */
@@ -193,10 +195,17 @@ lf_status lf_get_info(const lf_handle* h, lf_info* out);
  * events on `cuda_stream` around each of their kernels (no synchronisation added).  After the caller
  * has synchronised the stream, lf_kernel_times writes the mean durations in milliseconds over the runs
  * recorded since profiling was enabled (the last 256 at most): ms[0] window kernel (a1, a2), ms[1] seeding
- * kernel (a3), ms[2] fit kernel (a4..a6), ms[3] offset scan, ms[4] compaction (a7).
+ * kernel (a3), ms[2] extension kernel (a4, a5), ms[3] fit kernel (a6), ms[4] offset scan, ms[5] compaction (a7).
  * LF_ERR_INVALID_ARG if profiling is off or no run was recorded. */
 lf_status lf_set_profiling(lf_handle* h, int enabled);
 lf_status lf_kernel_times(lf_handle* h, float ms[LF_N_KERNELS]);
+
+/* Work counters of the most recent lf_run / lf_run_debug on this handle (for lf_run_host: of its last chunk),
+ * for benchmarks: counters[0] = candidates that passed the hit-count rule (16-byte records handed from the
+ * extension kernel to the fit kernel), counters[1] = events holding two equal neighbouring hits.
+ * SYNCHRONOUS: waits for the device, then reads two per-event tables back. */
+#define LF_N_COUNTERS 2
+lf_status lf_run_counters(lf_handle* h, uint64_t counters[LF_N_COUNTERS]);
 
 /* ABI self-description for bindings: version and struct sizes
  * (which: 0 geometry, 1 params, 2 seeds, 3 hits, 4 tracks, 5 debug, 6 info). */

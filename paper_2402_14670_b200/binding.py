@@ -70,12 +70,13 @@ class lf_debug(C.Structure):
 
 
 class lf_info(C.Structure):
-    _fields_ = [("kernels_per_run", C.c_int32), ("regs", C.c_int32 * 3), ("block", C.c_int32 * 3),
-                ("grid", C.c_int32 * 3), ("ctas_per_sm", C.c_int32 * 3), ("smem_bytes", C.c_int32 * 3),
+    _fields_ = [("kernels_per_run", C.c_int32), ("regs", C.c_int32 * 4), ("block", C.c_int32 * 4),
+                ("grid", C.c_int32 * 4), ("ctas_per_sm", C.c_int32 * 4), ("smem_bytes", C.c_int32 * 4),
                 ("staged_hits_per_event", C.c_int32), ("sm_count", C.c_int32), ("workspace_bytes", C.c_size_t)]
 
 
-KERNEL_NAMES = ("window", "seed", "fit", "scan", "compact")
+KERNEL_NAMES = ("window", "seed", "extend", "fit", "scan", "compact")
+EVENT_KERNELS = KERNEL_NAMES[:4]
 
 
 _STRUCTS = (lf_geometry, lf_params, lf_seeds, lf_hits, lf_tracks, lf_debug, lf_info)
@@ -112,11 +113,13 @@ def load_library() -> C.CDLL:
     lib.lf_get_info.argtypes = [C.c_void_p, C.POINTER(lf_info)]
     lib.lf_set_host_chunk_events.restype = C.c_int
     lib.lf_set_host_chunk_events.argtypes = [C.c_void_p, C.c_size_t]
+    lib.lf_run_counters.restype = C.c_int
+    lib.lf_run_counters.argtypes = [C.c_void_p, C.POINTER(C.c_uint64 * 2)]
     lib.lf_set_profiling.restype = C.c_int
     lib.lf_set_profiling.argtypes = [C.c_void_p, C.c_int]
     lib.lf_kernel_times.restype = C.c_int
-    lib.lf_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_float * 5)]
-    if lib.lf_abi_version() != 1:
+    lib.lf_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_float * 6)]
+    if lib.lf_abi_version() != 2:
         raise ImportError("liblf_b200.so: ABI version mismatch")
     for i, st in enumerate(_STRUCTS):
         if lib.lf_sizeof(i) != C.sizeof(st):
@@ -219,8 +222,8 @@ class LookingForward:
         self._check(self._lib.lf_set_profiling(self._h, 1 if enabled else 0))
 
     def kernel_times(self):
-        """Mean (window, seed, fit, scan, compact) milliseconds of the profiled runs; the stream must be synchronised."""
-        ms = (C.c_float * 5)()
+        """Mean (window, seed, extend, fit, scan, compact) milliseconds of the profiled runs; the stream must be synchronised."""
+        ms = (C.c_float * 6)()
         self._check(self._lib.lf_kernel_times(self._h, C.byref(ms)))
         return tuple(float(v) for v in ms)
 
@@ -260,6 +263,12 @@ class LookingForward:
         self._check(self._lib.lf_run_host(self._h, C.byref(seeds), C.byref(hits), hb.n_events, C.byref(tr),
                                           self._stream_ptr(stream)))
         return int(out.n_tracks[0])
+
+    def run_counters(self):
+        """``lf_run_counters`` (synchronous): (accepted candidates, events with equal neighbouring hits) of the last run."""
+        c = (C.c_uint64 * 2)()
+        self._check(self._lib.lf_run_counters(self._h, C.byref(c)))
+        return int(c[0]), int(c[1])
 
     def set_host_chunk_events(self, min_events_per_chunk: int):
         """``lf_set_host_chunk_events``: pipeline granularity of :meth:`run_host`."""

@@ -12,6 +12,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "lf_kernels.cuh"
 
@@ -48,7 +49,7 @@ struct lf_handle {
   size_t max_events, max_seeds, max_hits;
   int device;
   int sm_count, stage_cap;
-  int regs[3], grid[3], ctas_per_sm[3], smem_bytes[3]; /* window, seed, fit kernels */
+  int regs[4], grid[4], ctas_per_sm[4], smem_bytes[4]; /* window, seed, extend, fit kernels */
   /* workspace */
   __half* hx16;     /* hit_storage = 1 only */
   float* origin16;
@@ -56,10 +57,13 @@ struct lf_handle {
   uint16_t* trip_code;
   uint8_t* n_trip;
   int32_t *ws_rec, *ws_nh, *ws_rank, *ws_event;
-  uint32_t *ev_count, *ev_off, *ev_dup, *tickets;
+  uint32_t *ev_count, *ev_off, *ev_dup, *ev_acc, *tickets;
+  uint4* acc_rec;
+  lf::FitLut* fit_lut;
   size_t workspace_bytes;
   HostBufs hb;
   size_t host_chunk_events = HOST_CHUNK_EVENTS;
+  size_t last_events = 0; /* n_events of the most recent launch (lf_run_counters) */
   bool profiling = false;
   size_t prof_runs = 0;                 /* runs recorded since profiling was enabled */
   cudaEvent_t (*prof_ev)[N_PROF_EV] = nullptr;  /* ring of PROF_RING event sets */
@@ -137,6 +141,37 @@ void make_consts(const lf_geometry& G, const lf_params& P, lf::Consts& c) {
   c.mag_tol_tx = P.mag_tol_tx; c.mag_tol_max = P.mag_tol_max;
 }
 
+/* Geometry sums and cofactors of the two least-squares fits for every 12-bit hit-presence mask, in the
+ * canonical fp32 order (sums over the present layers in ascending layer order; DESIGN.md "Canonical
+ * arithmetic" a6).  Masks that cannot occur (singular systems) hold inf/nan and are never read. */
+void make_fit_lut(const lf::Consts& c, lf::FitLut* lut) {
+  for (unsigned m = 0; m < (1u << lf::NL); ++m) {
+    volatile float S1 = 0.f, Sd = 0.f, Sw = 0.f, Sdd = 0.f, Sdw = 0.f, Sww = 0.f, U1 = 0.f, Ud = 0.f, Udd = 0.f;
+    for (int l = 0; l < lf::NL; ++l) {
+      if (!((m >> l) & 1u)) continue;
+      const float dl = c.d[l], wl = c.w[l];
+      const float dd = dl * dl, dw = dl * wl, ww = wl * wl;
+      S1 = S1 + 1.0f; Sd = Sd + dl; Sw = Sw + wl; Sdd = Sdd + dd; Sdw = Sdw + dw; Sww = Sww + ww;
+      if (uv_layer(l)) { U1 = U1 + 1.0f; Ud = Ud + dl; Udd = Udd + dd; }
+    }
+    auto mul = [](float a, float b) { volatile float r = a * b; return (float)r; };
+    lf::FitLut& L = lut[m];
+    L.C00 = mul(Sdd, Sww) - mul(Sdw, Sdw);
+    L.C01 = mul(Sdw, Sw) - mul(Sd, Sww);
+    L.C02 = mul(Sd, Sdw) - mul(Sdd, Sw);
+    L.C11 = mul(S1, Sww) - mul(Sw, Sw);
+    L.C12 = mul(Sd, Sw) - mul(S1, Sdw);
+    L.C22 = mul(S1, Sdd) - mul(Sd, Sd);
+    volatile float det = mul(S1, L.C00) + mul(Sd, L.C01);
+    det = det + mul(Sw, L.C02);
+    L.inv_det = 1.0f / det;
+    L.pad0 = 0.f;
+    L.U1 = U1; L.Ud = Ud; L.Udd = Udd;
+    const float det2 = mul(U1, Udd) - mul(Ud, Ud);
+    L.inv_det2 = 1.0f / det2;
+  }
+}
+
 const char* validate(const lf_geometry& G, const lf_params& P) {
   if (G.n_layers != LF_N_LAYERS) return "geometry.n_layers must be 12";
   for (int l = 0; l < LF_N_LAYERS; ++l) {
@@ -173,11 +208,13 @@ lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_
   A.ws_rec = h->ws_rec; A.ws_nh = h->ws_nh; A.ws_rank = h->ws_rank; A.ws_event = h->ws_event;
   A.ev_count = h->ev_count;
   A.ev_dup = h->ev_dup;
+  A.acc_rec = h->acc_rec; A.ev_acc = h->ev_acc; A.fit_lut = h->fit_lut;
   if (dbg) {
     A.dbg.win_first = dbg->win_first; A.dbg.win_count = dbg->win_count; A.dbg.n_triplets = dbg->n_triplets;
     A.dbg.trip_hits = dbg->trip_hits; A.dbg.trip_set = dbg->trip_set; A.dbg.trip_chi2 = dbg->trip_chi2;
     A.dbg.cand_hits = dbg->cand_hits; A.dbg.cand_quality = dbg->cand_quality;
   }
+  h->last_events = n_events;
   const bool work = n_events > 0;
   auto grid_of = [&](int k) { return (int)std::min<size_t>((size_t)h->grid[k], n_events); };
   const bool half_hits = h->P.hit_storage == 1;
@@ -202,12 +239,17 @@ lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_
   A.origin16 = nullptr;
   if (work) {
     A.ticket = h->tickets + 2;
-    lf::lf_fit_kernel<DEBUG><<<grid_of(2), lf::FIT_THREADS, h->smem_bytes[2], st>>>(h->C, A);
+    lf::lf_extend_kernel<DEBUG><<<grid_of(2), lf::FIT_THREADS, h->smem_bytes[2], st>>>(h->C, A);
   }
   if (prof) LF_CUDA(h, cudaEventRecord(pe[3], st));
+  if (work) {
+    A.ticket = h->tickets + 3;
+    lf::lf_fit_kernel<DEBUG><<<grid_of(3), lf::FIT_THREADS, h->smem_bytes[3], st>>>(h->C, A);
+  }
+  if (prof) LF_CUDA(h, cudaEventRecord(pe[4], st));
   lf::lf_scan_kernel<<<1, 1024, 0, st>>>(h->ev_count, (uint32_t)n_events, h->ev_off, out->event_offsets,
                                          out->n_tracks, h->tickets);
-  if (prof) LF_CUDA(h, cudaEventRecord(pe[4], st));
+  if (prof) LF_CUDA(h, cudaEventRecord(pe[5], st));
   if (work && seeds->n_seeds > 0) {
     const size_t total = seeds->n_seeds * lf::REC_WORDS;
     const unsigned blocks = (unsigned)((total + 255) / 256);
@@ -215,7 +257,7 @@ lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_
                                                   out->hit_idx, out->seed_idx, out->n_hits, out->state, out->quality);
   }
   if (prof) {
-    LF_CUDA(h, cudaEventRecord(pe[5], st));
+    LF_CUDA(h, cudaEventRecord(pe[6], st));
     ++h->prof_runs;
   }
   LF_CUDA(h, cudaGetLastError());
@@ -301,12 +343,14 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   const size_t stage_bytes = (size_t)lf::HDR_BYTES + (size_t)h->stage_cap * sizeof(float);
   h->smem_bytes[0] = (int)stage_bytes;
   h->smem_bytes[1] = (int)(stage_bytes + sizeof(lf::SeedTables));
-  h->smem_bytes[2] = (int)(stage_bytes + lf::fit_tables_bytes(params->n_triplets));
-  const void* kern[3][2] = {{(const void*)lf::lf_window_kernel<false>, (const void*)lf::lf_window_kernel<true>},
+  h->smem_bytes[2] = (int)(stage_bytes + lf::ext_tables_bytes(params->n_triplets));
+  h->smem_bytes[3] = (int)(stage_bytes + lf::FIT_TABLES_BYTES);
+  const void* kern[4][2] = {{(const void*)lf::lf_window_kernel<false>, (const void*)lf::lf_window_kernel<true>},
                             {(const void*)lf::lf_seed_kernel<false>, (const void*)lf::lf_seed_kernel<true>},
+                            {(const void*)lf::lf_extend_kernel<false>, (const void*)lf::lf_extend_kernel<true>},
                             {(const void*)lf::lf_fit_kernel<false>, (const void*)lf::lf_fit_kernel<true>}};
-  const int threads[3] = {lf::WIN_THREADS, lf::SEED_THREADS, lf::FIT_THREADS};
-  for (int k = 0; k < 3; ++k) {
+  const int threads[4] = {lf::WIN_THREADS, lf::SEED_THREADS, lf::FIT_THREADS, lf::FIT_THREADS};
+  for (int k = 0; k < 4; ++k) {
     for (int d = 0; d < 2; ++d)
       LF_CREATE_CUDA(cudaFuncSetAttribute(kern[k][d], cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_bytes[k]));
     LF_CREATE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->ctas_per_sm[k], kern[k][0], threads[k], h->smem_bytes[k]));
@@ -334,9 +378,18 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   LF_CREATE_CUDA(cudaMalloc(&h->ev_count, ne * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ev_off, (ne + 1) * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ev_dup, ne * sizeof(uint32_t)));
+  LF_CREATE_CUDA(cudaMalloc(&h->ev_acc, ne * sizeof(uint32_t)));
+  LF_CREATE_CUDA(cudaMalloc(&h->acc_rec, ns * nt * sizeof(uint4)));
+  {
+    std::vector<lf::FitLut> lut(1u << lf::NL);
+    make_fit_lut(h->C, lut.data());
+    LF_CREATE_CUDA(cudaMalloc(&h->fit_lut, lut.size() * sizeof(lf::FitLut)));
+    LF_CREATE_CUDA(cudaMemcpy(h->fit_lut, lut.data(), lut.size() * sizeof(lf::FitLut), cudaMemcpyHostToDevice));
+  }
   LF_CREATE_CUDA(cudaMalloc(&h->tickets, lf::N_TICKETS * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMemset(h->tickets, 0, lf::N_TICKETS * sizeof(uint32_t)));
-  h->workspace_bytes = ns * (lf::NL * 4 + nt * 2 + 1 + (lf::REC_WORDS + 3) * 4) + (3 * ne + 1 + lf::N_TICKETS) * sizeof(uint32_t);
+  h->workspace_bytes = ns * (lf::NL * 4 + nt * (2 + sizeof(uint4)) + 1 + (lf::REC_WORDS + 3) * 4) +
+                       (4 * ne + 1 + lf::N_TICKETS) * sizeof(uint32_t) + (sizeof(lf::FitLut) << lf::NL);
 #undef LF_CREATE_CUDA
   *out = h;
   return LF_OK;
@@ -347,7 +400,7 @@ lf_status lf_destroy(lf_handle* h) {
   cudaFree(h->hx16); cudaFree(h->origin16);
   cudaFree(h->win); cudaFree(h->trip_code); cudaFree(h->n_trip);
   cudaFree(h->ws_rec); cudaFree(h->ws_nh); cudaFree(h->ws_rank); cudaFree(h->ws_event);
-  cudaFree(h->ev_count); cudaFree(h->ev_off); cudaFree(h->ev_dup); cudaFree(h->tickets);
+  cudaFree(h->ev_count); cudaFree(h->ev_off); cudaFree(h->ev_dup); cudaFree(h->ev_acc); cudaFree(h->acc_rec); cudaFree(h->fit_lut); cudaFree(h->tickets);
   HostBufs& b = h->hb;
   cudaFree(b.seeds); cudaFree(b.seed_off); cudaFree(b.hits); cudaFree(b.seg_off);
   cudaFree(b.hit_idx); cudaFree(b.seed_idx); cudaFree(b.n_hits); cudaFree(b.state); cudaFree(b.quality);
@@ -375,8 +428,8 @@ lf_status lf_destroy(lf_handle* h) {
 lf_status lf_get_info(const lf_handle* h, lf_info* out) {
   if (!h || !out) return LF_ERR_INVALID_ARG;
   out->kernels_per_run = LF_N_KERNELS + (h->P.hit_storage == 1 ? 1 : 0);
-  const int threads[3] = {lf::WIN_THREADS, lf::SEED_THREADS, lf::FIT_THREADS};
-  for (int k = 0; k < 3; ++k) {
+  const int threads[4] = {lf::WIN_THREADS, lf::SEED_THREADS, lf::FIT_THREADS, lf::FIT_THREADS};
+  for (int k = 0; k < 4; ++k) {
     out->regs[k] = h->regs[k];
     out->block[k] = threads[k];
     out->grid[k] = h->grid[k];
@@ -386,6 +439,22 @@ lf_status lf_get_info(const lf_handle* h, lf_info* out) {
   out->staged_hits_per_event = h->stage_cap - 4;
   out->sm_count = h->sm_count;
   out->workspace_bytes = h->workspace_bytes;
+  return LF_OK;
+}
+
+lf_status lf_run_counters(lf_handle* h, uint64_t counters[LF_N_COUNTERS]) {
+  if (!h || !counters) return LF_ERR_INVALID_ARG;
+  for (int i = 0; i < LF_N_COUNTERS; ++i) counters[i] = 0;
+  const size_t ne = h->last_events;
+  if (ne == 0) return LF_OK;
+  std::vector<uint32_t> acc(ne), dup(ne);
+  LF_CUDA(h, cudaDeviceSynchronize());
+  LF_CUDA(h, cudaMemcpy(acc.data(), h->ev_acc, ne * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+  LF_CUDA(h, cudaMemcpy(dup.data(), h->ev_dup, ne * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+  for (size_t e = 0; e < ne; ++e) {
+    counters[0] += acc[e];
+    counters[1] += dup[e] ? 1u : 0u;
+  }
   return LF_OK;
 }
 
@@ -406,7 +475,7 @@ lf_status lf_kernel_times(lf_handle* h, float ms[LF_N_KERNELS]) {
   if (!h || !ms) return LF_ERR_INVALID_ARG;
   if (!h->profiling || h->prof_runs == 0) return fail(h, LF_ERR_INVALID_ARG, "lf_kernel_times: no profiled run recorded");
   const size_t n = std::min<size_t>(h->prof_runs, PROF_RING);
-  double acc[LF_N_KERNELS] = {0, 0, 0, 0, 0};
+  double acc[LF_N_KERNELS] = {0, 0, 0, 0, 0, 0};
   for (size_t r = 0; r < n; ++r)
     for (int i = 0; i < LF_N_KERNELS; ++i) {
       float t = 0.f;

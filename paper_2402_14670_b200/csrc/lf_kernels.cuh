@@ -44,7 +44,7 @@ constexpr int SEED_WARPS = 8;
 constexpr int SEED_THREADS = SEED_WARPS * 32;
 constexpr int FIT_THREADS = 256;
 constexpr int FIT_CHUNK = 256; /* seeds of one event handled per pass of the fit kernel (== FIT_THREADS) */
-constexpr int N_TICKETS = 4;
+constexpr int N_TICKETS = 4; /* window, seed, extend, fit */
 constexpr unsigned FULL = 0xffffffffu;
 constexpr float INTERVAL_MARGIN = 0.1f; /* mm added to the magnet tolerance when bracketing h2 (superset only) */
 
@@ -60,6 +60,8 @@ struct Consts {
   float xtol_base, xtol_inv_p, x_asym, uv_half_width;
   float p_same_bend, mag_tol_base, mag_tol_inv_p, mag_tol_tx, mag_tol_max;
 };
+
+struct FitLut;
 
 struct DebugOut {
   int32_t *win_first, *win_count, *n_triplets, *trip_hits, *trip_set;
@@ -89,6 +91,10 @@ struct EventArgs {
   int32_t* ws_rank;     /* n_seeds: rank among the event's tracks, -1 = none */
   int32_t* ws_event;    /* n_seeds: event of the seed */
   uint32_t* ev_count;   /* n_events */
+  uint4* acc_rec;       /* n_seeds*NT: candidates that passed the hit-count rule: 3 words of hit codes (byte l = hit of
+                           layer l inside its window, 0xFF = none), seed inside the event | k << 28; dense per event */
+  uint32_t* ev_acc;     /* n_events: number of such records of the event */
+  const struct FitLut* fit_lut; /* 4096: per presence mask */
   uint32_t* ev_dup;     /* n_events: written by the window kernel, != 0 if two neighbouring staged hits are equal */
   DebugOut dbg;
 };
@@ -575,7 +581,6 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
     unsigned long long key = 0;
     if (act) {
       /* the exact predicate is the definition */
-      const int la = set ? 3 : 0;
       const int fb = set ? fbs[1] : fbs[0], nb = set ? nbs[1] : nbs[0], fc = set ? fcs[1] : fcs[0];
       const float inv_dz = set ? C.inv_dz_ac[1] : C.inv_dz_ac[0], zmag_a = set ? C.zmag_a[1] : C.zmag_a[0];
       const float x2 = hx[fc + j];
@@ -598,7 +603,6 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
                 (unsigned)((set << 15) | (owner << 10) | (j << 5) | (k - fb));
         }
       }
-      (void)la;
     }
     const unsigned m = __ballot_sync(FULL, pass);
     if (m) {
@@ -674,11 +678,7 @@ __global__ void __launch_bounds__(SEED_THREADS, 5) lf_seed_kernel(const __grid_c
 }
 
 /* ============================================================================================
- * a4-a6: extension, fit, quality, best per seed.
- *   E  one thread per candidate: closest hit in the 9 layers outside the triplet (uniform loop),
- *      hit-count rule; accepted candidates are ballot-compacted into a per-warp queue;
- *   F  one thread per queued candidate (dense batches of 32): fp32 fit in ascending layer order, Q;
- *   B  one thread per seed: lowest Q wins, the winner is re-evaluated to write the track record.
+ * a4-a6: extension (lf_extend_kernel), then fit, quality, best per seed (lf_fit_kernel).
  * ============================================================================================ */
 
 /* Hit codes of a candidate: byte l = window-relative index of the hit on layer l, 0xFF = none. */
@@ -763,172 +763,41 @@ __device__ __noinline__ CandHits extend_candidate(const Consts& C, const HV& hx,
   return h;
 }
 
-struct FitOut {
-  float Q;
-  bool ty_ok;
+/* Per-mask constants of the two least-squares fits (computed once in lf_create, fp32, the canonical order):
+ * the geometry sums depend only on which layers hold a hit. */
+struct __align__(16) FitLut {
+  float C00, C01, C02, C11; /* cofactors of the 3x3 normal matrix of (1, d, w) over the present layers */
+  float C12, C22, inv_det, pad0;
+  float U1, Ud, Udd, inv_det2; /* 2x2 normal matrix of (1, d) over the present u/v layers */
 };
 
-/* a6: fit of an accepted candidate.  With `rec` != nullptr also computes q/p and the
- * state (Eq. 9) and writes the 20-word track record. */
-template <class HV>
-__device__ __noinline__ FitOut fit_candidate(const Consts& C, const HV& hx, const uint32_t* winw, float y, float tx,
-                                             float ty, unsigned code, const CandHits& h, uint32_t h0, uint32_t seed,
-                                             int32_t* rec) {
-  float a0, t0, c0;
-  triplet_parabola(C, hx, winw, code, a0, t0, c0);
-  const float T_uv = fmaxf(C.T_uv_min, C.T_uv_slope * (fabsf(tx) + fabsf(ty)));
-  const float inv_Tuv = 1.0f / T_uv;
-  /* x fit on the residuals to the triplet parabola: sums in ascending layer order */
-  float r[NL];
-  float S1 = 0.f, Sd = 0.f, Sw = 0.f, Sdd = 0.f, Sdw = 0.f, Sww = 0.f, Sr = 0.f, Sdr = 0.f, Swr = 0.f;
-#pragma unroll
-  for (int l = 0; l < NL; ++l) {
-    const unsigned cd = code_of(h, l);
-    const bool present = cd != 0xFFu;
-    const float dl = C.d[l], wl = C.w[l];
-    const float s_i = hx[present ? ((int)(winw[l] >> 6) + (int)cd) : 0];
-    const float yt = is_uv(l) ? (y + ty * C.dzs[l]) * C.tana[l] : 0.0f;
-    const float m = s_i - yt;
-    r[l] = m - ((a0 + t0 * dl) + c0 * wl);
-    if (present) {
-      S1 = S1 + 1.0f;
-      Sd = Sd + dl;
-      Sw = Sw + wl;
-      Sdd = Sdd + dl * dl;
-      Sdw = Sdw + dl * wl;
-      Sww = Sww + wl * wl;
-      Sr = Sr + r[l];
-      Sdr = Sdr + dl * r[l];
-      Swr = Swr + wl * r[l];
-    }
-  }
-  const float C00 = Sdd * Sww - Sdw * Sdw;
-  const float C01 = Sdw * Sw - Sd * Sww;
-  const float C02 = Sd * Sdw - Sdd * Sw;
-  const float C11 = S1 * Sww - Sw * Sw;
-  const float C12 = Sd * Sw - S1 * Sdw;
-  const float C22 = S1 * Sdd - Sd * Sd;
-  const float det = (S1 * C00 + Sd * C01) + Sw * C02;
-  const float inv = 1.0f / det;
-  const float da = ((C00 * Sr + C01 * Sdr) + C02 * Swr) * inv;
-  const float dt = ((C01 * Sr + C11 * Sdr) + C12 * Swr) * inv;
-  const float dc = ((C02 * Sr + C12 * Sdr) + C22 * Swr) * inv;
-  float Qx = 0.f, U1 = 0.f, Ud = 0.f, Udd = 0.f, Ur = 0.f, Udr = 0.f;
-#pragma unroll
-  for (int l = 0; l < NL; ++l) {
-    const bool present = code_of(h, l) != 0xFFu;
-    const float dl = C.d[l], wl = C.w[l];
-    const float e = r[l] - ((da + dt * dl) + dc * wl);
-    const float chi2 = e * e;
-    if (is_uv(l)) {
-      r[l] = e * C.inv_tan[l]; /* rho: y residual to the seed's straight line */
-      if (present) {
-        Qx = Qx + chi2 * inv_Tuv;
-        U1 = U1 + 1.0f;
-        Ud = Ud + dl;
-        Udd = Udd + dl * dl;
-        Ur = Ur + r[l];
-        Udr = Udr + dl * r[l];
-      }
-    } else if (present) {
-      Qx = Qx + chi2 * C.inv_Tx;
-    }
-  }
-  /* y line on the u/v hits */
-  const float det2 = U1 * Udd - Ud * Ud;
-  const float inv2 = 1.0f / det2;
-  const float dy0 = (Udd * Ur - Ud * Udr) * inv2;
-  const float dtym = (U1 * Udr - Ud * Ur) * inv2;
-  const float dty = dtym * 0.001f;
-  FitOut out;
-  out.ty_ok = fabsf(dty) < C.T_ty;
-  float Qy = 0.f;
-#pragma unroll
-  for (int l = 0; l < NL; ++l) {
-    if (!is_uv(l)) continue;
-    const float ey = r[l] - (dy0 + dtym * C.d[l]);
-    if (code_of(h, l) != 0xFFu) Qy = Qy + (ey * ey) * C.inv_Ty;
-  }
-  const int ci = min(3, max(0, h.n - 9));
-  const float Cn = (ci == 0) ? C.C_nhits[0] : (ci == 1 ? C.C_nhits[1] : (ci == 2 ? C.C_nhits[2] : C.C_nhits[3]));
-  out.Q = (Qx / (float)(h.n - 3) + Qy / (float)(h.n_uv - 2)) * Cn; /* Eq. (6) */
-
-  if (rec != nullptr) {
-    const float a = a0 + da, t = t0 + dt, c = c0 + dc;
-    const float t_ref = t * 0.001f;
-    const float dslope = t_ref - tx;
-    const float F = C.poly[0] + dslope * (C.poly[1] + dslope * (C.poly[2] + dslope * (C.poly[3] + dslope * C.poly[4])));
-    int4* r4 = reinterpret_cast<int4*>(rec);
-    int o[REC_WORDS];
-#pragma unroll
-    for (int l = 0; l < NL; ++l) {
-      const unsigned cd = code_of(h, l);
-      o[l] = (cd != 0xFFu) ? (int32_t)(h0 + (winw[l] >> 6) + cd) : -1;
-    }
-    o[12] = (int32_t)seed;
-    o[13] = h.n;
-    o[14] = __float_as_int((a + t * C.ds) + c * C.ws);
-    o[15] = __float_as_int((y + ty * C.dz_state) + (dy0 + dtym * C.ds));
-    o[16] = __float_as_int((t + c * C.dws) * 0.001f);
-    o[17] = __float_as_int(ty + dtym * 0.001f);
-    o[18] = __float_as_int(dslope / F);
-    o[19] = __float_as_int(out.Q);
-#pragma unroll
-    for (int q = 0; q < REC_WORDS / 4; ++q) r4[q] = make_int4(o[4 * q], o[4 * q + 1], o[4 * q + 2], o[4 * q + 3]);
-  }
-  return out;
-}
-
-/* Per-chunk tables of the fit kernel (after the staged hits in shared memory). */
-struct FitTables {
+/* ---- E: lf_extend_kernel (a4, a5).  One thread per triplet candidate of the event; candidates passing
+ * the hit-count rule are written as 16-byte records, densely and in (seed, k) order, into the event's
+ * slice of `acc_rec` (slice start = first seed of the event * n_triplets). */
+struct ExtTables {
   float* geo;      /* 4*12: d, w, dzs, tana */
   uint32_t* win;   /* FIT_CHUNK*12 packed windows */
   float* sp;       /* FIT_CHUNK*4: y, tx, ty, (unused) */
-  int* pref;       /* FIT_CHUNK+1: exclusive prefix of candidates per seed */
+  int* pref;       /* FIT_CHUNK+4: exclusive prefix of candidates per seed */
   uint16_t* item;  /* FIT_CHUNK*NT: seed_local<<4 | k */
-  float* Q;        /* FIT_CHUNK*NT: Q, or +inf if the candidate is not acceptable */
-  uint4* queue;    /* (FIT_THREADS/32) warps * 64 entries: hit codes (3 words) + item | n<<16 | n_uv<<24 */
+  int* wcnt;       /* 2 * 8: accepted candidates per warp, double-buffered by pass */
 };
-__host__ __device__ inline size_t fit_tables_bytes(int nt) {
+__host__ __device__ inline size_t ext_tables_bytes(int nt) {
   return 4 * NL * 4 + (size_t)FIT_CHUNK * NL * 4 + (size_t)FIT_CHUNK * 4 * 4 + (size_t)(FIT_CHUNK + 4) * 4 +
-         (((size_t)FIT_CHUNK * nt * 2 + 15) & ~size_t(15)) + (size_t)FIT_CHUNK * nt * 4 + (size_t)(FIT_THREADS / 32) * 64 * 16;
-}
-
-/* F on one dense batch of the warp's queue: entries [0, cnt), cnt <= 32. */
-template <bool DEBUG, class HV>
-__device__ __forceinline__ void fit_batch(const Consts& C, const EventArgs& A, const HV& hx, const FitTables& T,
-                                          const uint4* q, int cnt, uint32_t sbase, uint32_t h0, int lane) {
-  if (lane < cnt) {
-    const uint4 e = q[lane];
-    const int it = (int)(e.w & 0xFFFFu);
-    CandHits h;
-    h.w[0] = e.x; h.w[1] = e.y; h.w[2] = e.z;
-    h.n = (int)((e.w >> 16) & 0xFFu);
-    h.n_uv = (int)(e.w >> 24);
-    h.enough = true;
-    const unsigned im = T.item[it];
-    const int sl = (int)(im >> 4), k = (int)(im & 15u);
-    const uint32_t seed = sbase + (uint32_t)sl;
-    const unsigned code = A.trip_code[(size_t)seed * C.n_triplets + k];
-    const FitOut fo = fit_candidate(C, hx, T.win + sl * NL, T.sp[sl * 4 + 0], T.sp[sl * 4 + 1], T.sp[sl * 4 + 2], code, h,
-                                    h0, seed, nullptr);
-    /* accepted if Q < T_Q (and the t_y cut holds) */
-    T.Q[it] = (fo.ty_ok && (fo.Q < C.T_Q)) ? fo.Q : __int_as_float(0x7f800000);
-    if (DEBUG && A.dbg.cand_quality) A.dbg.cand_quality[(size_t)seed * C.n_triplets + k] = fo.ty_ok ? fo.Q : -2.0f;
-  }
+         (((size_t)FIT_CHUNK * nt * 2 + 15) & ~size_t(15)) + 16 * 4;
 }
 
 template <bool DEBUG, bool STAGED>
-__device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, CtaHeader& H, const EventCtx& E,
-                                          const HitView<STAGED>& hx, const FitTables& T) {
+__device__ __forceinline__ void extend_event(const Consts& C, const EventArgs& A, CtaHeader& H, const EventCtx& E,
+                                             const HitView<STAGED>& hx, const ExtTables& T) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
   const int ns = (int)(s1 - s0);
   const int NT = C.n_triplets;
-  const float INF = __int_as_float(0x7f800000);
-  uint4* myq = T.queue + warp * 64;
   const bool dup = H.dup != 0;
-  int ev_tracks = 0;
+  uint4* rec = A.acc_rec + (size_t)s0 * NT;
+  uint32_t ev_acc = 0;
+  int parity = 0;
   for (int cb = 0; cb < ns; cb += FIT_CHUNK) {
     const int cn = min(FIT_CHUNK, ns - cb);
     const uint32_t sbase = s0 + (uint32_t)cb;
@@ -941,6 +810,14 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
       T.sp[tid * 4 + 1] = __ldg(A.stx + seed);
       T.sp[tid * 4 + 2] = __ldg(A.sty + seed);
       my_n = (int)A.n_trip[seed];
+      A.ws_nh[seed] = 0; /* set by the fit kernel if the seed gets a track */
+      if (DEBUG) {
+        for (int k = my_n; k < NT; ++k) {
+          if (A.dbg.cand_quality) A.dbg.cand_quality[(size_t)seed * NT + k] = -1.0f;
+          if (A.dbg.cand_hits)
+            for (int l = 0; l < NL; ++l) A.dbg.cand_hits[((size_t)seed * NT + k) * NL + l] = -1;
+        }
+      }
     }
     /* exclusive prefix of candidate counts over the chunk (FIT_CHUNK <= FIT_THREADS) */
     int incl = my_n;
@@ -963,14 +840,13 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
       T.pref[tid] = excl;
       for (int k = 0; k < my_n; ++k) T.item[excl + k] = (uint16_t)((tid << 4) | k);
     }
-    if (tid == 0) T.pref[cn] = total;
     __syncthreads();
-    /* ---- E: one thread per candidate; accepted candidates go to the warp's queue; F on dense batches */
-    int qn = 0;
+    /* ---- one thread per candidate; the accepted ones are appended in candidate order */
     for (int base = 0; base < total; base += FIT_THREADS) {
       const int it = base + tid;
       bool enough = false;
       CandHits h;
+      unsigned tag = 0;
       if (it < total) {
         const unsigned im = T.item[it];
         const int sl = (int)(im >> 4), k = (int)(im & 15u);
@@ -978,7 +854,7 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
         const unsigned code = A.trip_code[(size_t)seed * NT + k];
         h = extend_candidate(C, hx, T.win + sl * NL, T.geo, T.sp[sl * 4 + 0], T.sp[sl * 4 + 1], T.sp[sl * 4 + 2], code, dup);
         enough = h.enough;
-        if (!enough) T.Q[it] = INF;
+        tag = (unsigned)(cb + sl) | ((unsigned)k << 28); /* seed inside the event, candidate index */
         if (DEBUG) {
           if (A.dbg.cand_hits)
             for (int l = 0; l < NL; ++l) {
@@ -989,53 +865,232 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
         }
       }
       const unsigned m = __ballot_sync(FULL, enough);
-      if (m) {
-        if (enough)
-          myq[qn + __popc(m & ((1u << lane) - 1u))] =
-              make_uint4(h.w[0], h.w[1], h.w[2], (unsigned)it | ((unsigned)h.n << 16) | ((unsigned)h.n_uv << 24));
-        qn += __popc(m);
-        __syncwarp();
-        if (qn >= 32) {
-          fit_batch<DEBUG>(C, A, hx, T, myq, 32, sbase, E.h0, lane);
-          __syncwarp();
-          const uint4 carry = (lane + 32 < qn) ? myq[lane + 32] : make_uint4(0, 0, 0, 0);
-          __syncwarp();
-          qn -= 32;
-          if (lane < qn) myq[lane] = carry;
-          __syncwarp();
-        }
+      int* wc = T.wcnt + parity * 8;
+      if (lane == 0) wc[warp] = __popc(m);
+      __syncthreads();
+      int off = 0, tot = 0;
+#pragma unroll
+      for (int wq = 0; wq < FIT_THREADS / 32; ++wq) {
+        const int tq = wc[wq];
+        off += (wq < warp) ? tq : 0;
+        tot += tq;
       }
+      if (enough) rec[ev_acc + (uint32_t)(off + __popc(m & ((1u << lane) - 1u)))] = make_uint4(h.w[0], h.w[1], h.w[2], tag);
+      ev_acc += (uint32_t)tot;
+      parity ^= 1;
     }
-    if (qn > 0) fit_batch<DEBUG>(C, A, hx, T, myq, qn, sbase, E.h0, lane);
+    __syncthreads(); /* the tables are restaged by the next chunk */
+  }
+  if (tid == 0) A.ev_acc[E.ev] = ev_acc;
+}
+
+template <bool DEBUG>
+__global__ void __launch_bounds__(FIT_THREADS, 4) lf_extend_kernel(const __grid_constant__ Consts C,
+                                                                   const __grid_constant__ EventArgs A) {
+  CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
+  unsigned char* tb = lf_smem + HDR_BYTES + (size_t)A.stage_cap * sizeof(float);
+  const int NT = C.n_triplets;
+  ExtTables T;
+  T.geo = reinterpret_cast<float*>(tb);
+  tb += 4 * NL * 4;
+  T.win = reinterpret_cast<uint32_t*>(tb);
+  tb += (size_t)FIT_CHUNK * NL * 4;
+  T.sp = reinterpret_cast<float*>(tb);
+  tb += (size_t)FIT_CHUNK * 16;
+  T.pref = reinterpret_cast<int*>(tb);
+  tb += (size_t)(FIT_CHUNK + 4) * 4;
+  T.item = reinterpret_cast<uint16_t*>(tb);
+  tb += ((size_t)FIT_CHUNK * NT * 2 + 15) & ~size_t(15);
+  T.wcnt = reinterpret_cast<int*>(tb);
+  if (threadIdx.x == 0) mbar_init(&H.mbar, 1);
+  if (threadIdx.x < NL) {
+    T.geo[threadIdx.x] = C.d[threadIdx.x];
+    T.geo[NL + threadIdx.x] = C.w[threadIdx.x];
+    T.geo[2 * NL + threadIdx.x] = C.dzs[threadIdx.x];
+    T.geo[3 * NL + threadIdx.x] = C.tana[threadIdx.x];
+  }
+  uint32_t phase = 0;
+  EventCtx E;
+  while (fetch_event(A, phase, E)) {
+    if (E.staged) extend_event<DEBUG, true>(C, A, H, E, HitView<true>{E.skew}, T);
+    else extend_event<DEBUG, false>(C, A, H, E, HitView<false>{A.hx + E.h0}, T);
+  }
+}
+
+/* ---- F: lf_fit_kernel (a6 + ranking).  One thread per accepted candidate, a pass of FIT_THREADS records at a
+ * time; the records of a seed are adjacent and a pass ends on a seed boundary, so after one barrier the lowest
+ * (Q, k) of every seed is known (64-bit atomicMin in shared memory) and the winning thread still holds its fit
+ * in registers: it writes the 20-word track record (q/p from Eq. 9, state at z_state).  Then the CTA ranks the
+ * event's tracks in seed order. */
+struct FitTables {
+  unsigned long long* best; /* 2 * FIT_THREADS: lowest (Q bits << 32 | k) per seed of the pass, double-buffered */
+  int* next_b;              /* 2: first left-over record of a pass (consumed one barrier later) */
+  int* wcnt;                /* 2 * 8: seed changes per warp */
+};
+constexpr size_t FIT_TABLES_BYTES = 2 * FIT_THREADS * 8 + 16 + 16 * 4;
+
+template <bool DEBUG, bool STAGED>
+__device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, CtaHeader& H, const EventCtx& E,
+                                          const HitView<STAGED>& hx, const FitTables& T) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
+  const int ns = (int)(s1 - s0);
+  const int NT = C.n_triplets;
+  const uint4* rec = A.acc_rec + (size_t)s0 * NT;
+  const int n_acc = (int)A.ev_acc[E.ev];
+  const unsigned SIE = 0x0FFFFFFFu;
+  int parity = 0;
+  for (int b = 0; b < n_acc; parity ^= 1) {
+    unsigned long long* best = T.best + parity * FIT_THREADS;
+    int* wc = T.wcnt + parity * 8;
+    best[tid] = ~0ull;
+    const int t = b + tid;
+    const bool have = t < n_acc;
+    const uint4 r = have ? __ldg(rec + t) : make_uint4(0, 0, 0, 0xFFFFFFFFu);
+    const unsigned sie = r.w & SIE;
+    const int k = (int)(r.w >> 28);
+    unsigned prev_sie = __shfl_up_sync(FULL, sie, 1);
+    if (lane == 0) prev_sie = (tid > 0 && have) ? (__ldg(&rec[t - 1].w) & SIE) : 0xFFFFFFFEu;
+    /* a seed whose records continue in the next pass is left to that pass (a seed has < FIT_THREADS records) */
+    const unsigned nxt_sie = (b + FIT_THREADS < n_acc) ? (__ldg(&rec[b + FIT_THREADS].w) & SIE) : 0xFFFFFFFEu;
+    const bool mine = have && sie != nxt_sie;
+    if (have && !mine && prev_sie != nxt_sie) T.next_b[parity] = t; /* first left-over record: single writer */
+    const uint32_t seed = s0 + sie;
+    /* dense index of the record's seed inside the pass: number of seed changes up to this record */
+    const unsigned chg = __ballot_sync(FULL, have && sie != prev_sie);
+    if (lane == 0) wc[warp] = __popc(chg);
     __syncthreads();
-    /* ---- B: one thread per seed: lowest Q wins, ties -> earlier in (chi2,set,h0,h2) order */
-    bool found = false;
-    if (tid < cn) {
-      const uint32_t seed = sbase + (uint32_t)tid;
-      const int b = T.pref[tid], e = T.pref[tid + 1];
-      float best = INF;
-      int bk = -1;
-      for (int i = b; i < e; ++i) {
-        const float q = T.Q[i];
-        if (q < best) { best = q; bk = i - b; }
+    if (tid == 0) T.next_b[parity ^ 1] = 0x7FFFFFFF; /* re-armed for the next pass; its readers are past the barrier */
+    int slot = __popc(chg & ((2u << lane) - 1u)) - 1;
+#pragma unroll
+    for (int wq = 0; wq < FIT_THREADS / 32; ++wq) slot += (wq < warp) ? wc[wq] : 0;
+    /* ---- the fit, sums in ascending layer order */
+    float a0 = 0.f, t0 = 0.f, c0 = 0.f, da = 0.f, dt = 0.f, dc = 0.f, dy0 = 0.f, dtym = 0.f, Q = 0.f, y = 0.f, tx = 0.f, ty = 0.f;
+    uint32_t wf[NL];
+    int n = 0;
+    unsigned long long key = ~0ull;
+    if (mine) {
+      const uint4* wp = reinterpret_cast<const uint4*>(A.win + (size_t)seed * NL);
+      const uint4 w0 = __ldg(wp), w1 = __ldg(wp + 1), w2 = __ldg(wp + 2);
+      wf[0] = w0.x; wf[1] = w0.y; wf[2] = w0.z; wf[3] = w0.w; wf[4] = w1.x; wf[5] = w1.y; wf[6] = w1.z; wf[7] = w1.w;
+      wf[8] = w2.x; wf[9] = w2.y; wf[10] = w2.z; wf[11] = w2.w;
+      y = __ldg(A.sy + seed);
+      tx = __ldg(A.stx + seed);
+      ty = __ldg(A.sty + seed);
+      const unsigned code = A.trip_code[(size_t)seed * NT + k];
+      CandHits h;
+      h.w[0] = r.x; h.w[1] = r.y; h.w[2] = r.z;
+      unsigned mask = 0;
+#pragma unroll
+      for (int l = 0; l < NL; ++l) {
+        const unsigned cd = code_of(h, l);
+        wf[l] = (wf[l] >> 6) + cd; /* event-relative hit index (meaningless if the layer has no hit) */
+        mask |= (cd != 0xFFu) ? (1u << l) : 0u;
       }
-      if (DEBUG) {
-        for (int k = e - b; k < NT; ++k) {
-          if (A.dbg.cand_quality) A.dbg.cand_quality[(size_t)seed * NT + k] = -1.0f;
-          if (A.dbg.cand_hits)
-            for (int l = 0; l < NL; ++l) A.dbg.cand_hits[((size_t)seed * NT + k) * NL + l] = -1;
+      n = __popc(mask);
+      const int n_uv = __popc(mask & 0x666u);
+      {
+        const int set = (code >> 15) & 1;
+        const float x0 = hx[(int)(set ? wf[3] : wf[0])], x1 = hx[(int)(set ? wf[7] : wf[4])], x2 = hx[(int)(set ? wf[11] : wf[8])];
+        const float X10 = x1 - x0, X20 = x2 - x0;
+        const float D10 = set ? C.D10[1] : C.D10[0], D20 = set ? C.D20[1] : C.D20[0];
+        const float W10 = set ? C.W10[1] : C.W10[0];
+        c0 = (X20 * D10 - X10 * D20) * (set ? C.inv_det[1] : C.inv_det[0]);
+        t0 = (X10 - c0 * W10) * (set ? C.inv_D10[1] : C.inv_D10[0]);
+        a0 = (x0 - t0 * (set ? C.d[3] : C.d[0])) - c0 * (set ? C.w[3] : C.w[0]);
+      }
+      const float4* lut = reinterpret_cast<const float4*>(A.fit_lut + mask);
+      const float4 LA = __ldg(lut), LB = __ldg(lut + 1), LY = __ldg(lut + 2);
+      const float T_uv = fmaxf(C.T_uv_min, C.T_uv_slope * (fabsf(tx) + fabsf(ty)));
+      const float inv_Tuv = 1.0f / T_uv;
+      /* x fit on the residuals to the triplet parabola */
+      float rr[NL];
+      float Sr = 0.f, Sdr = 0.f, Swr = 0.f;
+#pragma unroll
+      for (int l = 0; l < NL; ++l) {
+        const bool present = (mask >> l) & 1u;
+        const float dl = C.d[l], wl = C.w[l];
+        const float s_i = hx[present ? (int)wf[l] : 0];
+        const float yt = is_uv(l) ? (y + ty * C.dzs[l]) * C.tana[l] : 0.0f;
+        const float mm = s_i - yt;
+        rr[l] = mm - ((a0 + t0 * dl) + c0 * wl);
+        if (present) {
+          Sr = Sr + rr[l];
+          Sdr = Sdr + dl * rr[l];
+          Swr = Swr + wl * rr[l];
         }
       }
-      found = bk >= 0;
-      if (found) {
-        const unsigned code = A.trip_code[(size_t)seed * NT + bk];
-        const float y = T.sp[tid * 4 + 0], tx = T.sp[tid * 4 + 1], ty = T.sp[tid * 4 + 2];
-        const CandHits h = extend_candidate(C, hx, T.win + tid * NL, T.geo, y, tx, ty, code, dup);
-        fit_candidate(C, hx, T.win + tid * NL, y, tx, ty, code, h, E.h0, seed, A.ws_rec + (size_t)seed * REC_WORDS);
+      da = ((LA.x * Sr + LA.y * Sdr) + LA.z * Swr) * LB.z;
+      dt = ((LA.y * Sr + LA.w * Sdr) + LB.x * Swr) * LB.z;
+      dc = ((LA.z * Sr + LB.x * Sdr) + LB.y * Swr) * LB.z;
+      float Qx = 0.f, Ur = 0.f, Udr = 0.f;
+#pragma unroll
+      for (int l = 0; l < NL; ++l) {
+        const bool present = (mask >> l) & 1u;
+        const float dl = C.d[l], wl = C.w[l];
+        const float e = rr[l] - ((da + dt * dl) + dc * wl);
+        const float chi2 = e * e;
+        if (is_uv(l)) {
+          rr[l] = e * C.inv_tan[l]; /* rho: y residual to the seed's straight line */
+          if (present) {
+            Qx = Qx + chi2 * inv_Tuv;
+            Ur = Ur + rr[l];
+            Udr = Udr + dl * rr[l];
+          }
+        } else if (present) {
+          Qx = Qx + chi2 * C.inv_Tx;
+        }
       }
-      A.ws_nh[seed] = found ? 1 : 0;
+      /* y line on the u/v hits */
+      dy0 = (LY.z * Ur - LY.y * Udr) * LY.w;
+      dtym = (LY.x * Udr - LY.y * Ur) * LY.w;
+      const bool ty_ok = fabsf(dtym * 0.001f) < C.T_ty;
+      float Qy = 0.f;
+#pragma unroll
+      for (int l = 0; l < NL; ++l) {
+        if (!is_uv(l)) continue;
+        const float ey = rr[l] - (dy0 + dtym * C.d[l]);
+        if ((mask >> l) & 1u) Qy = Qy + (ey * ey) * C.inv_Ty;
+      }
+      const int ci = min(3, max(0, n - 9));
+      const float Cn = (ci == 0) ? C.C_nhits[0] : (ci == 1 ? C.C_nhits[1] : (ci == 2 ? C.C_nhits[2] : C.C_nhits[3]));
+      Q = (Qx / (float)(n - 3) + Qy / (float)(n_uv - 2)) * Cn; /* Eq. (6) */
+      if (DEBUG && A.dbg.cand_quality) A.dbg.cand_quality[(size_t)seed * NT + k] = ty_ok ? Q : -2.0f;
+      /* accepted if Q < T_Q (and the t_y cut holds); lowest Q wins, ties -> lower k */
+      if (ty_ok && (Q < C.T_Q)) {
+        key = ((unsigned long long)__float_as_uint(Q) << 32) | (unsigned)k;
+        atomicMin(best + slot, key);
+      }
+#pragma unroll
+      for (int l = 0; l < NL; ++l) wf[l] = ((mask >> l) & 1u) ? (E.h0 + wf[l]) : 0xFFFFFFFFu; /* global hit index or -1 */
     }
-    /* ---- rank the chunk's tracks in seed order (a7, first half) */
+    __syncthreads();
+    if (key != ~0ull && best[slot] == key) {
+      /* the seed's track: q/p (Eq. 9) and the state at z_state */
+      const float a = a0 + da, tt = t0 + dt, c = c0 + dc;
+      const float t_ref = tt * 0.001f;
+      const float dslope = t_ref - tx;
+      const float F = C.poly[0] + dslope * (C.poly[1] + dslope * (C.poly[2] + dslope * (C.poly[3] + dslope * C.poly[4])));
+      int4* r4 = reinterpret_cast<int4*>(A.ws_rec + (size_t)seed * REC_WORDS);
+      r4[0] = make_int4((int)wf[0], (int)wf[1], (int)wf[2], (int)wf[3]);
+      r4[1] = make_int4((int)wf[4], (int)wf[5], (int)wf[6], (int)wf[7]);
+      r4[2] = make_int4((int)wf[8], (int)wf[9], (int)wf[10], (int)wf[11]);
+      r4[3] = make_int4((int32_t)seed, n, __float_as_int((a + tt * C.ds) + c * C.ws),
+                        __float_as_int((y + ty * C.dz_state) + (dy0 + dtym * C.ds)));
+      r4[4] = make_int4(__float_as_int((tt + c * C.dws) * 0.001f), __float_as_int(ty + dtym * 0.001f),
+                        __float_as_int(dslope / F), __float_as_int(Q));
+      A.ws_nh[seed] = 1;
+    }
+    b = min(T.next_b[parity], b + FIT_THREADS); /* next pass: the first record left over, else the next FIT_THREADS */
+  }
+  __syncthreads(); /* the track flags of this CTA's seeds are visible to all its threads */
+  if (tid == 0) T.next_b[0] = T.next_b[1] = 0x7FFFFFFF;
+  /* ---- rank the event's tracks in seed order (a7, first half) */
+  int ev_tracks = 0;
+  for (int cb = 0; cb < ns; cb += FIT_THREADS) {
+    const bool in = cb + tid < ns;
+    const uint32_t seed = s0 + (uint32_t)(cb + tid);
+    const bool found = in && A.ws_nh[seed] != 0;
     const unsigned m = __ballot_sync(FULL, found);
     if (lane == 0) H.warp_tot[warp] = __popc(m);
     __syncthreads();
@@ -1046,9 +1101,9 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
       off += (wq < warp) ? tq : 0;
       tot += tq;
     }
-    if (tid < cn) {
-      A.ws_rank[sbase + tid] = found ? (ev_tracks + off + __popc(m & ((1u << lane) - 1u))) : -1;
-      A.ws_event[sbase + tid] = (int32_t)E.ev;
+    if (in) {
+      A.ws_rank[seed] = found ? (ev_tracks + off + __popc(m & ((1u << lane) - 1u))) : -1;
+      A.ws_event[seed] = (int32_t)E.ev;
     }
     ev_tracks += tot;
     __syncthreads();
@@ -1061,27 +1116,13 @@ __global__ void __launch_bounds__(FIT_THREADS, 3) lf_fit_kernel(const __grid_con
                                                                 const __grid_constant__ EventArgs A) {
   CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
   unsigned char* tb = lf_smem + HDR_BYTES + (size_t)A.stage_cap * sizeof(float);
-  const int NT = C.n_triplets;
   FitTables T;
-  T.geo = reinterpret_cast<float*>(tb);
-  tb += 4 * NL * 4;
-  T.win = reinterpret_cast<uint32_t*>(tb);
-  tb += (size_t)FIT_CHUNK * NL * 4;
-  T.sp = reinterpret_cast<float*>(tb);
-  tb += (size_t)FIT_CHUNK * 16;
-  T.pref = reinterpret_cast<int*>(tb);
-  tb += (size_t)(FIT_CHUNK + 4) * 4;
-  T.item = reinterpret_cast<uint16_t*>(tb);
-  tb += ((size_t)FIT_CHUNK * NT * 2 + 15) & ~size_t(15);
-  T.Q = reinterpret_cast<float*>(tb);
-  tb += (size_t)FIT_CHUNK * NT * 4;
-  T.queue = reinterpret_cast<uint4*>(tb);
-  if (threadIdx.x == 0) mbar_init(&H.mbar, 1);
-  if (threadIdx.x < NL) {
-    T.geo[threadIdx.x] = C.d[threadIdx.x];
-    T.geo[NL + threadIdx.x] = C.w[threadIdx.x];
-    T.geo[2 * NL + threadIdx.x] = C.dzs[threadIdx.x];
-    T.geo[3 * NL + threadIdx.x] = C.tana[threadIdx.x];
+  T.best = reinterpret_cast<unsigned long long*>(tb);
+  T.next_b = reinterpret_cast<int*>(tb + 2 * FIT_THREADS * 8);
+  T.wcnt = T.next_b + 4;
+  if (threadIdx.x == 0) {
+    mbar_init(&H.mbar, 1);
+    T.next_b[0] = T.next_b[1] = 0x7FFFFFFF;
   }
   uint32_t phase = 0;
   EventCtx E;
