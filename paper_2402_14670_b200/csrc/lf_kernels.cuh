@@ -40,6 +40,7 @@ constexpr int REC_WORDS = 20;  /* 12 hit idx, seed, n_hits, 5 state, Q */
 constexpr int TRIP_BUF = 64;   /* per-warp triplet key buffer */
 constexpr int MAX_NT = 16;     /* == LF_MAX_TRIPLETS */
 constexpr int WIN_THREADS = 256;
+constexpr int EDGE_STEPS = 6;  /* window-edge searches span n_window + 1 hits: 2^EDGE_STEPS > LF_MAX_WINDOW + 1 */
 constexpr int SEED_WARPS = 8;
 constexpr int SEED_THREADS = SEED_WARPS * 32;
 constexpr int FIT_THREADS = 256;
@@ -154,18 +155,61 @@ __device__ __forceinline__ float* stage_buf() { return reinterpret_cast<float*>(
 
 /* View of the current event's hits, indexed event-relative.  Staged: shared memory (LDS);
  * fallback for events larger than the stage buffer: read-only global loads. */
+__device__ __forceinline__ float lds_f32(uint32_t addr) {
+  float v;
+  asm("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+  return v;
+}
+/* Besides operator[], a view hands out positions (`pos_t`) for searches whose steps are "advance, bound check,
+ * load, compare, select": 32-bit shared-memory byte addresses for the staged hits, pointers otherwise. */
 template <bool STAGED>
 struct HitView;
 template <>
 struct HitView<true> {
   int off; /* skew of the event inside the stage buffer */
   __device__ __forceinline__ float operator[](int i) const { return stage_buf()[off + i]; }
+  typedef uint32_t pos_t;
+  __device__ __forceinline__ pos_t pos(int i) const { return smem_u32(stage_buf()) + 4u * (uint32_t)(off + i); }
+  static __device__ __forceinline__ pos_t adv(pos_t p, int n) { return p + 4u * (uint32_t)n; }
+  static __device__ __forceinline__ float before(pos_t p) { return lds_f32(p - 4u); } /* the hit in front of p */
+  static __device__ __forceinline__ int diff(pos_t a, pos_t b) { return (int)(a - b) >> 2; }
 };
 template <>
 struct HitView<false> {
   const float* p;
   __device__ __forceinline__ float operator[](int i) const { return __ldg(p + i); }
+  typedef const float* pos_t;
+  __device__ __forceinline__ pos_t pos(int i) const { return p + i; }
+  static __device__ __forceinline__ pos_t adv(pos_t q, int n) { return q + n; }
+  static __device__ __forceinline__ float before(pos_t q) { return __ldg(q - 1); }
+  static __device__ __forceinline__ int diff(pos_t a, pos_t b) { return (int)(a - b); }
 };
+
+/* Branch-free binary search over the x-sorted positions [a, e): a + number of leading hits with x < v
+ * (INCLUSIVE == false: lower bound) or x <= v (true: upper bound).  Needs 2^NSTEPS > e - a. */
+template <int NSTEPS, bool INCLUSIVE, class HV>
+__device__ __forceinline__ typename HV::pos_t bound_pos(typename HV::pos_t a, typename HV::pos_t e, float v) {
+  typename HV::pos_t p = a;
+#pragma unroll
+  for (int s = NSTEPS - 1; s >= 0; --s) {
+    const typename HV::pos_t q = HV::adv(p, 1 << s);
+    if (q <= e) {
+      const float xm = HV::before(q);
+      if (INCLUSIVE ? (xm <= v) : (xm < v)) p = q;
+    }
+  }
+  return p;
+}
+template <class HV>
+__device__ __forceinline__ typename HV::pos_t lower_pos(typename HV::pos_t a, typename HV::pos_t e, float v, int nsteps) {
+  if (nsteps <= 8) return bound_pos<8, false, HV>(a, e, v);
+  typename HV::pos_t p = a;
+  for (int s = nsteps - 1; s >= 0; --s) {
+    const typename HV::pos_t q = HV::adv(p, 1 << s);
+    if (q <= e && HV::before(q) < v) p = q;
+  }
+  return p;
+}
 
 /* Takes the next event and stages its hits.  Called by every thread of the CTA; returns false when
  * the batch is exhausted.  Hit i of the event then lives at stage_buf()[skew + i]. */
@@ -222,22 +266,6 @@ __device__ __forceinline__ bool fetch_event(const EventArgs& A, uint32_t& phase,
   return true;
 }
 
-/* Branch-free binary search over the x-sorted range [b, e): b + number of leading elements with
- * x < v (inclusive == false: lower bound) or x <= v (inclusive == true: upper bound).
- * Needs 2^nsteps > e - b. */
-template <class HV>
-__device__ __forceinline__ int bound_search(const HV& hx, int b, int e, float v, bool inclusive, int nsteps) {
-  int pos = b;
-  for (int s = nsteps - 1; s >= 0; --s) {
-    const int probe = pos + (1 << s);
-    if (probe <= e) {
-      const float xm = hx[probe - 1];
-      if (inclusive ? (xm <= v) : (xm < v)) pos = probe;
-    }
-  }
-  return pos;
-}
-
 /* Closest hit to `pred` in the x-sorted window [f, f+n), n <= 32: first x >= pred by binary search,
  * then compare the two neighbours; ties -> lower index, including runs of equal distance on the low
  * side (equals a linear argmin with strict '<'); such a run needs two equal neighbouring hits, so the
@@ -275,11 +303,6 @@ __device__ __forceinline__ int closest_hit(const HV& hx, int f, int n, float pre
 
 /* The same on the staged hits: positions are 32-bit shared-memory byte addresses, so one search step is
  * add, bound check, LDS, compare, select. */
-__device__ __forceinline__ float lds_f32(uint32_t addr) {
-  float v;
-  asm("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
-  return v;
-}
 __device__ __forceinline__ int closest_hit(const HitView<true>& hx, int f, int n, float pred, bool dup, float& dist) {
   if (n <= 0) return -1;
   const uint32_t a = smem_u32(stage_buf()) + 4u * (uint32_t)(hx.off + f);
@@ -364,18 +387,17 @@ __device__ __forceinline__ void closest_group(const HitView<false>& hx, const ui
 template <bool DEBUG, bool STAGED>
 __device__ __forceinline__ void windows_of_event(const Consts& C, const EventArgs& A, const CtaHeader& H,
                                                  const EventCtx& E, const HitView<STAGED>& hx) {
+  typedef HitView<STAGED> HV;
+  typedef typename HV::pos_t pos_t;
   const int tid = threadIdx.x;
   const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
-  const int n_items = (int)(s1 - s0) * NSEG;
+  const int n_items = (int)(s1 - s0) * NL;
   const int nsteps = H.nsteps;
   const bool pol_pos = C.polarity > 0;
-  for (int base = 0; base < n_items; base += WIN_THREADS) {
-    const int it = base + tid;
-    const bool act = it < n_items;
-    const int sl = act ? it / NSEG : 0;
-    const int j = act ? it - sl * NSEG : 0;
-    const int layer = j >> 1;
-    const bool upper = (j & 1) != 0;
+  const int halfw = C.n_window / 2, reach = C.n_window + 1;
+  for (int it = tid; it < n_items; it += WIN_THREADS) {
+    const int sl = it / NL;
+    const int layer = it - sl * NL;
     const uint32_t seed = s0 + (uint32_t)sl;
     /* a1: pT-kick extrapolation */
     const float x = __ldg(A.sx + seed), y = __ldg(A.sy + seed), tx = __ldg(A.stx + seed), ty = __ldg(A.sty + seed);
@@ -400,31 +422,26 @@ __device__ __forceinline__ void windows_of_event(const Consts& C, const EventArg
       hi = ctr + C.uv_half_width;
     }
     const int sb = H.seg[layer * 2 + zone], se = H.seg[layer * 2 + zone + 1];
-    /* lower edge: first x >= lo; upper edge: first x > hi */
-    const int pos = bound_search(hx, sb, act ? se : sb, upper ? hi : lo, upper, nsteps);
-    const int other = __shfl_xor_sync(FULL, pos, 1);
-    int first = upper ? other : pos;
-    int last = upper ? pos : other;
-    if (last < first) last = first;
-    /* cap to n_window hits, index-symmetric about the geometric centre */
-    const bool capped = act && (last - first > C.n_window);
-    if (__any_sync(FULL, capped)) {
-      const float midv = (lo + hi) * 0.5f;
-      const int cpos = bound_search(hx, first, capped ? last : first, midv, false, nsteps);
-      if (capped) {
-        const int halfw = C.n_window / 2;
-        const int f2 = max(first, cpos - halfw);
-        const int l2 = min(last, cpos + halfw);
-        first = f2;
-        last = l2;
-      }
+    /* a2.  With c = lower_bound(mid) the window [first, last) = [lower_bound(lo), upper_bound(hi))
+     * is capped to [max(first, c - n/2), min(last, c + n/2)) iff it holds more than n = n_window hits.  Both
+     * the test and the result only need first and last clipped to c -/+ (n + 1), so after one search over
+     * the segment the two edges are short searches next to c (lo <= mid <= hi puts c inside the window). */
+    const pos_t pb = hx.pos(sb), pe = hx.pos(se);
+    const float midv = (lo + hi) * 0.5f;
+    const pos_t pc = lower_pos<HV>(pb, pe, midv, nsteps);
+    const int c = sb + HV::diff(pc, pb);
+    const int fmin = max(sb, c - reach), lmax = min(se, c + reach);
+    const pos_t pf = bound_pos<EDGE_STEPS, false, HV>(hx.pos(fmin), pc, lo);   /* first x >= lo, not below c - (n+1) */
+    const pos_t pl = bound_pos<EDGE_STEPS, true, HV>(pc, hx.pos(lmax), hi);    /* first x > hi, not above c + (n+1) */
+    int first = fmin + HV::diff(pf, hx.pos(fmin)), last = c + HV::diff(pl, pc);
+    if (last - first > C.n_window) {
+      first = max(first, c - halfw);
+      last = min(last, c + halfw);
     }
-    if (act && !upper) {
-      A.win[(size_t)seed * NL + layer] = ((uint32_t)first << 6) | (uint32_t)(last - first);
-      if (DEBUG) {
-        if (A.dbg.win_first) A.dbg.win_first[(size_t)seed * NL + layer] = (int32_t)(E.h0 + first);
-        if (A.dbg.win_count) A.dbg.win_count[(size_t)seed * NL + layer] = last - first;
-      }
+    A.win[(size_t)seed * NL + layer] = ((uint32_t)first << 6) | (uint32_t)(last - first);
+    if (DEBUG) {
+      if (A.dbg.win_first) A.dbg.win_first[(size_t)seed * NL + layer] = (int32_t)(E.h0 + first);
+      if (A.dbg.win_count) A.dbg.win_count[(size_t)seed * NL + layer] = last - first;
     }
   }
 }
@@ -710,7 +727,7 @@ __device__ __forceinline__ void triplet_parabola(const Consts& C, const HV& hx, 
 template <class HV>
 __device__ __noinline__ CandHits extend_candidate(const Consts& C, const HV& hx, const uint32_t* winw, const float* geo,
                                                   float y, float tx, float ty, unsigned code, bool dup) {
-  const int set = (code >> 15) & 1, la = set ? 3 : 0;
+  const int set = (code >> 15) & 1;
   float a0, t0, c0;
   triplet_parabola(C, hx, winw, code, a0, t0, c0);
   const float T_uv = fmaxf(C.T_uv_min, C.T_uv_slope * (fabsf(tx) + fabsf(ty)));
