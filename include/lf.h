@@ -103,7 +103,7 @@ typedef struct {
  * capacity >= seeds->n_seeds is required (at most one track per seed), so no
  * overflow is possible and no host synchronisation is needed to size anything. */
 typedef struct {
-  int32_t* hit_idx;        /* capacity*12: global hit index used on each layer, or -1 */
+  int32_t* hit_idx;        /* capacity*12: global hit index used on each layer, or -1; 16-byte aligned (lf_run) */
   int32_t* seed_idx;       /* capacity: global index of the seed the track extends */
   int32_t* n_hits;         /* capacity: number of hits (>= params.min_hits) */
   float* state;            /* capacity*5: x, y, tx, ty, q/p at geometry.z_state */

@@ -251,7 +251,7 @@ lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_
                                          out->n_tracks, h->tickets);
   if (prof) LF_CUDA(h, cudaEventRecord(pe[5], st));
   if (work && seeds->n_seeds > 0) {
-    const size_t total = seeds->n_seeds * lf::REC_WORDS;
+    const size_t total = seeds->n_seeds * (lf::REC_WORDS / 4);
     const unsigned blocks = (unsigned)((total + 255) / 256);
     lf::lf_compact_kernel<<<blocks, 256, 0, st>>>(h->ws_rec, h->ws_rank, h->ws_event, h->ev_off, seed_base, seeds->n_seeds,
                                                   out->hit_idx, out->seed_idx, out->n_hits, out->state, out->quality);
@@ -274,6 +274,8 @@ lf_status check_run_args(lf_handle* h, const lf_seeds* seeds, const lf_hits* hit
   if (hits->n_hits > 0 && !hits->x) return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL hit array");
   if (seeds->n_seeds > 0 && (!out->hit_idx || !out->seed_idx || !out->n_hits || !out->state || !out->quality))
     return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL output array");
+  if ((reinterpret_cast<uintptr_t>(out->hit_idx) & 15u) != 0)
+    return fail(h, LF_ERR_INVALID_ARG, "lf_run: out->hit_idx must be 16-byte aligned");
   if (n_events == 0 && (seeds->n_seeds != 0 || hits->n_hits != 0))
     return fail(h, LF_ERR_INVALID_ARG, "lf_run: n_events == 0 with non-empty seeds or hits");
   if (n_events > h->max_events || seeds->n_seeds > h->max_seeds || hits->n_hits > h->max_hits)

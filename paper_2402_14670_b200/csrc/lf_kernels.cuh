@@ -1129,7 +1129,7 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
 }
 
 template <bool DEBUG>
-__global__ void __launch_bounds__(FIT_THREADS, 3) lf_fit_kernel(const __grid_constant__ Consts C,
+__global__ void __launch_bounds__(FIT_THREADS, 4) lf_fit_kernel(const __grid_constant__ Consts C,
                                                                 const __grid_constant__ EventArgs A) {
   CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
   unsigned char* tb = lf_smem + HDR_BYTES + (size_t)A.stage_cap * sizeof(float);
@@ -1220,27 +1220,36 @@ __global__ void __launch_bounds__(1024) lf_scan_kernel(const uint32_t* __restric
   if (tid < N_TICKETS) tickets[tid] = 0u;
 }
 
-/* Stream compaction (a7): one thread per (seed, record word); coalesced reads of the per-seed
- * records, dense SoA writes in (event, seed) order. */
+/* Stream compaction (a7): one thread per (seed, 16-byte quarter of its record); coalesced 16-byte reads of
+ * the per-seed records, dense SoA writes in (event, seed) order (16-byte stores for the hit lists). */
 __global__ void __launch_bounds__(256) lf_compact_kernel(const int32_t* __restrict__ ws_rec, const int32_t* __restrict__ ws_rank,
                                                          const int32_t* __restrict__ ws_event, const uint32_t* __restrict__ ev_off,
                                                          size_t seed_base, size_t n_seeds, int32_t* __restrict__ hit_idx,
                                                          int32_t* __restrict__ seed_idx, int32_t* __restrict__ n_hits,
                                                          float* __restrict__ state, float* __restrict__ quality) {
+  constexpr int Q4 = REC_WORDS / 4; /* 5 quarters: 3 of hit indices, (seed, n, x, y), (tx, ty, q/p, Q) */
   size_t gid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (gid >= n_seeds * REC_WORDS) return;
-  gid += seed_base * REC_WORDS; /* the batch's seeds are [seed_base, seed_base + n_seeds) */
-  const size_t seed = gid / REC_WORDS;
-  const int wd = (int)(gid - seed * REC_WORDS);
+  if (gid >= n_seeds * Q4) return;
+  gid += seed_base * Q4; /* the batch's seeds are [seed_base, seed_base + n_seeds) */
+  const size_t seed = gid / Q4;
+  const int q = (int)(gid - seed * Q4);
   const int rank = ws_rank[seed];
   if (rank < 0) return;
   const size_t dst = (size_t)ev_off[ws_event[seed]] + (size_t)rank;
-  const int32_t v = ws_rec[gid];
-  if (wd < 12) hit_idx[dst * NL + wd] = v;
-  else if (wd == 12) seed_idx[dst] = v;
-  else if (wd == 13) n_hits[dst] = v;
-  else if (wd < 19) state[dst * 5 + (wd - 14)] = __int_as_float(v);
-  else quality[dst] = __int_as_float(v);
+  const int4 v = reinterpret_cast<const int4*>(ws_rec)[gid];
+  if (q < 3) {
+    reinterpret_cast<int4*>(hit_idx)[dst * 3 + q] = v;
+  } else if (q == 3) {
+    seed_idx[dst] = v.x;
+    n_hits[dst] = v.y;
+    state[dst * 5 + 0] = __int_as_float(v.z);
+    state[dst * 5 + 1] = __int_as_float(v.w);
+  } else {
+    state[dst * 5 + 2] = __int_as_float(v.x);
+    state[dst * 5 + 3] = __int_as_float(v.y);
+    state[dst * 5 + 4] = __int_as_float(v.z);
+    quality[dst] = __int_as_float(v.w);
+  }
 }
 
 } // namespace lf
