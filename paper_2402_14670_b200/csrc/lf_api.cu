@@ -114,6 +114,7 @@ void make_consts(const lf_geometry& G, const lf_params& P, lf::Consts& c) {
     c.inv_dz_ac[s] = one / (c.z[cc] - c.z[a]);
     c.zmag_a[s] = c.z_mag - c.z[a];
     c.inv_r[s] = one / (c.inv_dz_ac[s] * c.zmag_a[s]); /* bracket of the h2 interval only (not a decision) */
+    c.inv_abs_zmag_a[s] = one / std::fabs(c.zmag_a[s]);  /* idem */
     c.D10[s] = c.d[b] - c.d[a];
     c.D20[s] = c.d[cc] - c.d[a];
     c.W10[s] = c.w[b] - c.w[a];

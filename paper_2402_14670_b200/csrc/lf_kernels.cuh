@@ -53,7 +53,7 @@ constexpr float INTERVAL_MARGIN = 0.1f; /* mm added to the magnet tolerance when
 struct Consts {
   float z[NL], tana[NL], inv_tan[NL], dzs[NL], dzm[NL], d[NL], w[NL];
   float z_seed, z_mag, kick, dr, K[2], poly[5], mag_dz_seed;
-  float inv_dz_ac[2], zmag_a[2], inv_r[2], D10[2], D20[2], W10[2], W20[2], inv_det[2], inv_D10[2];
+  float inv_dz_ac[2], zmag_a[2], inv_r[2], inv_abs_zmag_a[2], D10[2], D20[2], W10[2], W20[2], inv_det[2], inv_D10[2];
   float dz_state, ds, ws, dws;
   int polarity;
   float T_triplet, T_x, T_uv_slope, T_uv_min, T_ty, inv_Tx, inv_Ty, T_Q, C_nhits[4];
@@ -533,7 +533,7 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
   const float tol0 = C.mag_tol_base + C.mag_tol_inv_p * aq;
   const float INF = __int_as_float(0x7f800000);
   /* ---- per layer set: lanes = h0.  |x0 + t*zmag_a - x_mag| < tol is linear in x2 (t = (x2-x0)*inv_dz, slope
-   * r = inv_dz*zmag_a < 0) and tol <= tol_sup, so the survivors lie inside
+   * r = inv_dz*zmag_a < 0) and tol <= tol_sup (tol is monotone in |t|), so the survivors lie inside
    * x2 in [x0 + (tol_sup - A)/r, x0 + (-tol_sup - A)/r], A = x0 - x_mag.  The margin in tol_sup (0.1 mm >> fp32
    * rounding of these expressions) makes the bracket a strict superset; the h2 window sits one hit per lane,
    * so both bracket ends are shuffle searches. */
@@ -550,14 +550,14 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
     fcs[set] = (int)(wc >> 6);
     x0s[set] = 0.0f;
     if (na == 0 || nbs[set] == 0 || nc == 0) continue; /* warp-uniform */
-    const float inv_dz = C.inv_dz_ac[set], inv_r = C.inv_r[set];
+    const float inv_r = C.inv_r[set];
     const bool have = lane < na;
     const float x0 = have ? hx[fa + lane] : 0.0f;
     const float x2v = (lane < nc) ? hx[fcs[set] + lane] : INF;
-    const float xc_lo = __shfl_sync(FULL, x2v, 0), xc_hi = __shfl_sync(FULL, x2v, nc - 1);
-    const float tmax = fmaxf(fabsf((xc_lo - x0) * inv_dz), fabsf((xc_hi - x0) * inv_dz));
-    const float tol_sup = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * tmax) + INTERVAL_MARGIN;
+    /* a survivor has |A + t*zmag_a| < tol <= tol_max, so |t| <= (|A| + tol_max)/|zmag_a| =: tmax */
     const float Aoff = x0 - x_mag;
+    const float tmax = (fabsf(Aoff) + C.mag_tol_max) * C.inv_abs_zmag_a[set];
+    const float tol_sup = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * tmax) + INTERVAL_MARGIN;
     const int jlo = lanes_below<false>(x2v, x0 + (tol_sup - Aoff) * inv_r);  /* first x2 >= lower end */
     const int jhi = lanes_below<true>(x2v, x0 + (-tol_sup - Aoff) * inv_r);  /* first x2 > upper end */
     const int cnt = have ? max(jhi - jlo, 0) : 0;
