@@ -3,14 +3,15 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--events E]
 
-A "step" is one pass of the whole hot path (a1..a7: one lf_run = track kernel + scan + compaction)
+A "step" is one pass of the whole hot path (a1..a7: one lf_run = window, seed, extend, fit, scan, compact kernels)
 over one batch of synthetic events.  Default workload: BASELINE.json configs[3] (20,000 events at
 Run-3-like occupancy, fp32, a single lf_run on one stream).  Prints ONE JSON line (rank 0).
 
   value        events/s with inputs resident in HBM (CUDA events around the K steps, max over ranks)
   e2e          the same metric through lf_run_host: pinned HOST buffers, H2D + D2H inside the timing
-  roofline     dominant kernel (lf_track_kernel): algorithmic bytes per launch / its mean duration,
-               timed live with CUDA events on the launching stream, vs MEASURED_PEAKS.json hbm_gbs
+  roofline     dominant kernel (the slowest event kernel): algorithmic bytes per launch / its mean duration,
+               timed live with CUDA events on the launching stream, vs MEASURED_PEAKS.json hbm_gbs;
+               roofline.alu = the issue-rate roofline that actually bounds it
   cpu_baseline the oracle, as it stands, on the box's host cores on a bounded sample (rank 0, N=1)
 
 --impl reference times the oracle (all host cores via the harness's event sharding) on a bounded
@@ -276,6 +277,22 @@ def run_ours(args):
             if tr.get("kernel") == roofline["kernel"]:
                 roofline["traffic"] = tr.get("dram_bytes_per_launch")
                 roofline["traffic_source"] = tr.get("source")
+            # what actually bounds the path: the warp-instruction issue rate.
+            # peak = SMs x 4 schedulers x 1 warp-instruction/clock x max SM clock; achieved = EXECUTED warp-instructions
+            # per launch (counted by ncu, profiles/) / the kernel's live duration: a utilisation, not algorithmic work.
+            wi = tr.get("all_kernels_warp_inst_per_launch", {})
+            if dom in wi and tr.get("kernel") == roofline["kernel"]:
+                sm_mhz = float(clocks.get("sm_max_mhz") or 1965.0)
+                peak_issue = 148 * 4 * sm_mhz * 1e6 / 1e9
+                ach = wi[dom] / (ktimes[dom] * 1e-3) / 1e9
+                ev_k = [k for k in binding.EVENT_KERNELS if k in wi]
+                extra_alu = {"bound": "alu", "achieved": ach, "peak": peak_issue, "unit": "G warp-inst/s", "frac": ach / peak_issue,
+                             "kernel": roofline["kernel"], "warp_inst_per_launch": wi[dom],
+                             "event_kernels_frac": sum(wi[k] for k in ev_k) / (sum(ktimes[k] for k in ev_k) * 1e-3) / 1e9 / peak_issue,
+                             "peak_source": "148 SMs x 4 schedulers x 1 warp-inst/clk x sm_max_mhz (B300_MICROARCH.md issue model)",
+                             "count_source": tr.get("source"),
+                             "note": "executed instructions from the committed ncu capture of this workload, not algorithmic work"}
+                roofline["alu"] = extra_alu
         except Exception:
             pass
 
