@@ -9,9 +9,9 @@ Run-3-like occupancy, fp32, a single lf_run on one stream).  Prints ONE JSON lin
 
   value        events/s with inputs resident in HBM (CUDA events around the K steps, max over ranks)
   e2e          the same metric through lf_run_host: pinned HOST buffers, H2D + D2H inside the timing
-  roofline     dominant kernel (the slowest event kernel): algorithmic bytes per launch / its mean duration,
-               timed live with CUDA events on the launching stream, vs MEASURED_PEAKS.json hbm_gbs;
-               roofline.alu = the issue-rate roofline that actually bounds it
+  roofline     dominant kernel (the slowest event kernel), timed live with CUDA events on the launching stream:
+               "bound": "alu" = warp-instruction issue rate vs 148 SMs x 4 schedulers x clock (what bounds the path,
+               DESIGN.md section 7); roofline.hbm = algorithmic bytes per launch / duration vs MEASURED_PEAKS.json hbm_gbs
   cpu_baseline the oracle, as it stands, on the box's host cores on a bounded sample (rank 0, N=1)
 
 --impl reference times the oracle (all host cores via the harness's event sharding) on a bounded
@@ -257,42 +257,46 @@ def run_ours(args):
     if rank != 0:
         return 0
 
-    # ---- roofline of the dominant kernel (the slowest of the three event kernels)
+    # ---- roofline of the dominant kernel (the slowest of the four event kernels).  The path is bound by the plain
+    # ALU / warp-instruction issue rate, so the top-level object is the "alu" roofline; the HBM
+    # roofline BASELINE.json's metric asks for sits beside it under "hbm" (same keys, algorithmic bytes).
     peak, peak_src = measured_peaks()
     kb = kernel_bytes(batch, n_tracks, int(P["n_triplets"]), n_acc)
     dom = max(binding.EVENT_KERNELS, key=lambda k: ktimes[k])
     achieved = kb[dom] / (ktimes[dom] * 1e-3) / 1e9
     path_bytes = algorithmic_bytes(batch, n_tracks)
     path_gbs = path_bytes / (local_ms / args.steps * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "kernel": f"lf_{dom}_kernel", "kernel_ms": ktimes[dom],
-                "algorithmic_bytes_per_launch": kb[dom], "peak_source": peak_src,
-                "whole_path": {"algorithmic_bytes_per_step": path_bytes, "achieved_gbs": path_gbs, "frac_of_measured": path_gbs / peak,
-                               "frac_of_nominal_8TBs": path_gbs / NOMINAL_HBM_GBS},
-                "note": "path is ALU/issue-bound, not HBM-bound (DESIGN.md 'Rooflines'); HBM fraction reported because the metric asks for it"}
+    hbm = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+           "traffic": None, "kernel": f"lf_{dom}_kernel", "kernel_ms": ktimes[dom],
+           "algorithmic_bytes_per_launch": kb[dom], "peak_source": peak_src,
+           "whole_path": {"algorithmic_bytes_per_step": path_bytes, "achieved_gbs": path_gbs, "frac_of_measured": path_gbs / peak,
+                          "frac_of_nominal_8TBs": path_gbs / NOMINAL_HBM_GBS},
+           "note": "the path is not HBM-bound; this fraction is reported because BASELINE.json's metric asks for it"}
+    roofline = hbm
     traffic_file = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.txt")
     if os.path.exists(traffic_file):
         try:
             tr = json.load(open(traffic_file))
-            if tr.get("kernel") == roofline["kernel"]:
-                roofline["traffic"] = tr.get("dram_bytes_per_launch")
-                roofline["traffic_source"] = tr.get("source")
-            # what actually bounds the path: the warp-instruction issue rate.
+            if tr.get("kernel") == hbm["kernel"]:
+                hbm["traffic"] = tr.get("dram_bytes_per_launch")
+                hbm["traffic_source"] = tr.get("source")
             # peak = SMs x 4 schedulers x 1 warp-instruction/clock x max SM clock; achieved = EXECUTED warp-instructions
-            # per launch (counted by ncu, profiles/) / the kernel's live duration: a utilisation, not algorithmic work.
+            # per launch (counted by ncu on this workload, profiles/) / the kernel's live duration.
             wi = tr.get("all_kernels_warp_inst_per_launch", {})
-            if dom in wi and tr.get("kernel") == roofline["kernel"]:
+            if dom in wi and tr.get("kernel") == hbm["kernel"]:
                 sm_mhz = float(clocks.get("sm_max_mhz") or 1965.0)
                 peak_issue = 148 * 4 * sm_mhz * 1e6 / 1e9
                 ach = wi[dom] / (ktimes[dom] * 1e-3) / 1e9
                 ev_k = [k for k in binding.EVENT_KERNELS if k in wi]
-                extra_alu = {"bound": "alu", "achieved": ach, "peak": peak_issue, "unit": "G warp-inst/s", "frac": ach / peak_issue,
-                             "kernel": roofline["kernel"], "warp_inst_per_launch": wi[dom],
-                             "event_kernels_frac": sum(wi[k] for k in ev_k) / (sum(ktimes[k] for k in ev_k) * 1e-3) / 1e9 / peak_issue,
-                             "peak_source": "148 SMs x 4 schedulers x 1 warp-inst/clk x sm_max_mhz (B300_MICROARCH.md issue model)",
-                             "count_source": tr.get("source"),
-                             "note": "executed instructions from the committed ncu capture of this workload, not algorithmic work"}
-                roofline["alu"] = extra_alu
+                roofline = {"bound": "alu", "achieved": ach, "peak": peak_issue, "unit": "G warp-inst/s", "frac": ach / peak_issue,
+                            "traffic": hbm["traffic"], "kernel": hbm["kernel"], "kernel_ms": ktimes[dom],
+                            "warp_inst_per_launch": wi[dom], "warp_inst_per_seed": wi[dom] / batch.n_seeds,
+                            "event_kernels_frac": sum(wi[k] for k in ev_k) / (sum(ktimes[k] for k in ev_k) * 1e-3) / 1e9 / peak_issue,
+                            "peak_source": "148 SMs x 4 schedulers x 1 warp-inst/clk x sm_max_mhz (B300_MICROARCH.md issue model; DESIGN.md section 7)",
+                            "count_source": tr.get("source"),
+                            "note": "issue-slot utilisation: executed warp-instructions (ncu capture of this workload) over the live kernel "
+                                    "time; the remaining lever is the instruction count per seed, tracked in warp_inst_per_seed",
+                            "hbm": hbm}
         except Exception:
             pass
 
@@ -353,7 +357,7 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--events", type=int, default=None, help="override the number of events (default: the config's)")
-    ap.add_argument("--cpu-events", type=int, default=1500, help="events of the single-thread oracle sample")
+    ap.add_argument("--cpu-events", type=int, default=6000, help="events of the single-thread oracle sample")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
