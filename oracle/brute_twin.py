@@ -44,7 +44,9 @@ def run(G: dict, P: dict, b) -> SimpleNamespace:
     so = np.asarray(b.seed_offsets, dtype=np.int64)
     n_window, n_trip, min_hits = int(P["n_window"]), int(P["n_triplets"]), int(P["min_hits"])
     pf = {k: (f(v) if not isinstance(v, (list, tuple)) else [f(t) for t in v]) for k, v in P.items()
-          if k not in ("n_window", "n_triplets", "min_hits", "hit_storage")}
+          if k not in ("n_window", "n_triplets", "min_hits", "hit_storage", "mode")}
+    mode = int(P.get("mode", 0))
+    n_sides = 2 if mode == 1 else 1  # no-UT: LEFT and RIGHT windows of Eq. (8), followed separately
 
     def basis(zz):
         dz = zz - z_ref
@@ -55,32 +57,55 @@ def run(G: dict, P: dict, b) -> SimpleNamespace:
         return np.array([0.0, 1.0, 2.0 * dz + 3.0 * d_ratio * dz * dz])
 
     tracks = []
-    win_first = np.zeros((b.seed_x.shape[0], NL), np.int64)
-    win_count = np.zeros((b.seed_x.shape[0], NL), np.int64)
+    win_first = np.zeros((b.seed_x.shape[0] * n_sides, NL), np.int64)
+    win_count = np.zeros((b.seed_x.shape[0] * n_sides, NL), np.int64)
     all_trips = []
     ev_off = [0]
     for ev in range(b.n_events):
         for si in range(so[ev], so[ev + 1]):
-            x, y, tx, ty, qop = (float(b.seed_x[si]), float(b.seed_y[si]), float(b.seed_tx[si]),
-                                 float(b.seed_ty[si]), float(b.seed_qop[si]))
-            aq = max(abs(qop), 1e-6)
-            p = 1.0 / aq
+            x, y, tx, ty = float(b.seed_x[si]), float(b.seed_y[si]), float(b.seed_tx[si]), float(b.seed_ty[si])
+            qop = float(b.seed_qop[si]) if mode == 0 else 0.0
             x_mag = x + tx * (z_mag - z_seed)
-            txp = tx + kick * qop
             zone = 1 if ty >= 0 else 0
-            x_tol = pf["xtol_base"] + pf["xtol_inv_p"] / p
-            q = 1 if qop > 0 else -1
-            a_left = pf["x_asym"] if q * pol > 0 else 0.0
-            a_right = pf["x_asym"] if q * pol < 0 else 0.0
             yl = y + ty * (z - z_seed)
-            windows = []
-            for l in range(NL):
-                xc = x_mag + txp * (z[l] - z_mag)
-                if _is_uv(l):
-                    ctr = xc + yl[l] * tana[l]
-                    lo, hi = ctr - pf["uv_half_width"], ctr + pf["uv_half_width"]
+            best = None
+            for side in range(n_sides):
+              row = si * n_sides + side
+              if mode == 0:
+                aq = max(abs(qop), 1e-6)
+                p = 1.0 / aq
+                txp = tx + kick * qop
+                x_tol = pf["xtol_base"] + pf["xtol_inv_p"] / p
+                q = 1 if qop > 0 else -1
+                a_left = pf["x_asym"] if q * pol > 0 else 0.0
+                a_right = pf["x_asym"] if q * pol < 0 else 0.0
+              else:
+                # assumed momentum = the tighter of p_min and pT_min / sin(theta)
+                slope2 = tx * tx + ty * ty
+                p = pf["velo_p_min"]
+                if slope2 > 0.0:
+                    p = max(p, pf["velo_pt_min"] * np.sqrt(1.0 + slope2) / np.sqrt(slope2))
                 else:
-                    lo, hi = xc - x_tol - a_left, xc + x_tol + a_right
+                    p = np.inf
+                ip = 1.0 / p
+                c = pf["xtol_poly"]
+                # Eq. (7), term by term as printed
+                x_tol = ip * (c[0] + c[1] * tx + c[2] * tx ** 2 + ty ** 2 * (c[3] + c[4] * tx + c[5] * tx ** 2)
+                              + ip * (c[6] * tx + c[7] * ip))
+              windows = []
+              for l in range(NL):
+                if mode == 0:
+                    xc = x_mag + txp * (z[l] - z_mag)
+                    if _is_uv(l):
+                        ctr = xc + yl[l] * tana[l]
+                        lo, hi = ctr - pf["uv_half_width"], ctr + pf["uv_half_width"]
+                    else:
+                        lo, hi = xc - x_tol - a_left, xc + x_tol + a_right
+                else:
+                    # Eq. (8) about the straight-line extrapolation
+                    ctr = x + tx * (z[l] - z_seed) + (yl[l] * tana[l] if _is_uv(l) else 0.0)
+                    tol = pf["uv_half_width"] if _is_uv(l) else x_tol
+                    lo, hi = ((ctr - tol, ctr + pf["x_overlap"]) if side == 0 else (ctr - pf["x_overlap"], ctr + tol))
                 s0, s1 = seg[ev * 24 + l * 2 + zone], seg[ev * 24 + l * 2 + zone + 1]
                 members = [i for i in range(s0, s1) if lo <= hx[i] <= hi]
                 members.sort(key=lambda i: (hx[i], i))
@@ -89,72 +114,71 @@ def run(G: dict, P: dict, b) -> SimpleNamespace:
                     c_rank = sum(1 for i in members if hx[i] < mid)
                     members = [i for r, i in enumerate(members) if c_rank - n_window // 2 <= r < c_rank + n_window // 2]
                 windows.append(members)
-                win_count[si, l] = len(members)
-                win_first[si, l] = members[0] if members else -1
-            # ---- seeding
-            trips = []
-            for s, (la, lb, lc) in enumerate(SETS):
-                for i0 in windows[la]:
-                    for i2 in windows[lc]:
-                        t = (hx[i2] - hx[i0]) / (z[lc] - z[la])
-                        if p < pf["p_same_bend"] and not ((t - tx) * qop > 0):
-                            continue
-                        tol = min(pf["mag_tol_max"], pf["mag_tol_base"] + pf["mag_tol_inv_p"] / p + pf["mag_tol_tx"] * abs(t))
-                        if not abs(hx[i0] + t * (z_mag - z[la]) - x_mag) < tol:
-                            continue
-                        if not windows[lb]:
-                            continue
-                        x1e = z[lb] * t + (hx[i0] - t * z[la]) * K[s]
-                        i1 = min(windows[lb], key=lambda i: (abs(hx[i] - x1e), i))
-                        chi2 = (hx[i1] - x1e) ** 2
-                        if chi2 < pf["T_triplet"]:
-                            trips.append((chi2, s, i0, i2, i1))
-            trips.sort()
-            trips = trips[:n_trip]
-            all_trips.append(trips)
-            # ---- extension + fit
-            T_uv = max(pf["T_uv_min"], pf["T_uv_slope"] * (abs(tx) + abs(ty)))
-            best = None
-            for (chi2_t, s, i0, i2, i1) in trips:
-                la, lb, lc = SETS[s]
-                A3 = np.array([basis(z[la]), basis(z[lb]), basis(z[lc])])
-                par0 = np.linalg.solve(A3, np.array([hx[i0], hx[i1], hx[i2]]))
-                hit = [-1] * NL
-                hit[la], hit[lb], hit[lc] = i0, i1, i2
-                for l in range(NL):
-                    if l in (la, lb, lc) or not windows[l]:
-                        continue
-                    pred = float(basis(z[l]) @ par0) + (yl[l] * tana[l] if _is_uv(l) else 0.0)
-                    k = min(windows[l], key=lambda i: (abs(hx[i] - pred), i))
-                    if (hx[k] - pred) ** 2 < (T_uv if _is_uv(l) else pf["T_x"]):
-                        hit[l] = k
-                layers = [l for l in range(NL) if hit[l] >= 0]
-                uv = [l for l in layers if _is_uv(l)]
-                n, n_uv = len(layers), len(uv)
-                if n < min_hits or any(not any((l >> 2) == st for l in uv) for st in range(3)):
-                    continue
-                A = np.array([basis(z[l]) for l in layers])
-                m = np.array([hx[hit[l]] - yl[l] * tana[l] for l in layers])
-                par, *_ = np.linalg.lstsq(A, m, rcond=None)
-                res = m - A @ par
-                Qx = sum(res[j] ** 2 / (T_uv if _is_uv(l) else pf["T_x"]) for j, l in enumerate(layers))
-                Ay = np.array([[1.0, z[l] - z_ref] for l in uv])
-                yi = np.array([(hx[hit[l]] - float(basis(z[l]) @ par)) / tana[l] for l in uv])
-                ypar, *_ = np.linalg.lstsq(Ay, yi, rcond=None)
-                # seed line in the same parameterisation: y(z) = y + ty (z - z_seed)
-                ty_fit = ypar[1]
-                if not abs(ty_fit - ty) < pf["T_ty"]:
-                    continue
-                Qy = float(np.sum((yi - Ay @ ypar) ** 2)) / pf["T_y"]
-                Q = (Qx / (n - 3) + Qy / (n_uv - 2)) * pf["C_nhits"][min(3, max(0, n - 9))]
-                if not Q < pf["T_Q"]:
-                    continue
-                if best is None or Q < best[0]:
-                    dslope = par[1] - tx
-                    F = sum(c * dslope ** k for k, c in enumerate(poly))
-                    state = [float(basis(z_state) @ par), ypar[0] + ypar[1] * (z_state - z_ref),
-                             float(dbasis(z_state) @ par), ty_fit, dslope / F]
-                    best = (Q, hit, n, state)
+                win_count[row, l] = len(members)
+                win_first[row, l] = members[0] if members else -1
+              # ---- seeding
+              trips = []
+              for s, (la, lb, lc) in enumerate(SETS):
+                  for i0 in windows[la]:
+                      for i2 in windows[lc]:
+                          t = (hx[i2] - hx[i0]) / (z[lc] - z[la])
+                          if mode == 0 and p < pf["p_same_bend"] and not ((t - tx) * qop > 0):
+                              continue
+                          tol = min(pf["mag_tol_max"], pf["mag_tol_base"] + pf["mag_tol_inv_p"] / p + pf["mag_tol_tx"] * abs(t))
+                          if not abs(hx[i0] + t * (z_mag - z[la]) - x_mag) < tol:
+                              continue
+                          if not windows[lb]:
+                              continue
+                          x1e = z[lb] * t + (hx[i0] - t * z[la]) * K[s]
+                          i1 = min(windows[lb], key=lambda i: (abs(hx[i] - x1e), i))
+                          chi2 = (hx[i1] - x1e) ** 2
+                          if chi2 < pf["T_triplet"]:
+                              trips.append((chi2, s, i0, i2, i1))
+              trips.sort()
+              trips = trips[:n_trip]
+              all_trips.append(trips)
+              # ---- extension + fit
+              T_uv = max(pf["T_uv_min"], pf["T_uv_slope"] * (abs(tx) + abs(ty)))
+              for (chi2_t, s, i0, i2, i1) in trips:
+                  la, lb, lc = SETS[s]
+                  A3 = np.array([basis(z[la]), basis(z[lb]), basis(z[lc])])
+                  par0 = np.linalg.solve(A3, np.array([hx[i0], hx[i1], hx[i2]]))
+                  hit = [-1] * NL
+                  hit[la], hit[lb], hit[lc] = i0, i1, i2
+                  for l in range(NL):
+                      if l in (la, lb, lc) or not windows[l]:
+                          continue
+                      pred = float(basis(z[l]) @ par0) + (yl[l] * tana[l] if _is_uv(l) else 0.0)
+                      k = min(windows[l], key=lambda i: (abs(hx[i] - pred), i))
+                      if (hx[k] - pred) ** 2 < (T_uv if _is_uv(l) else pf["T_x"]):
+                          hit[l] = k
+                  layers = [l for l in range(NL) if hit[l] >= 0]
+                  uv = [l for l in layers if _is_uv(l)]
+                  n, n_uv = len(layers), len(uv)
+                  if n < min_hits or any(not any((l >> 2) == st for l in uv) for st in range(3)):
+                      continue
+                  A = np.array([basis(z[l]) for l in layers])
+                  m = np.array([hx[hit[l]] - yl[l] * tana[l] for l in layers])
+                  par, *_ = np.linalg.lstsq(A, m, rcond=None)
+                  res = m - A @ par
+                  Qx = sum(res[j] ** 2 / (T_uv if _is_uv(l) else pf["T_x"]) for j, l in enumerate(layers))
+                  Ay = np.array([[1.0, z[l] - z_ref] for l in uv])
+                  yi = np.array([(hx[hit[l]] - float(basis(z[l]) @ par)) / tana[l] for l in uv])
+                  ypar, *_ = np.linalg.lstsq(Ay, yi, rcond=None)
+                  # seed line in the same parameterisation: y(z) = y + ty (z - z_seed)
+                  ty_fit = ypar[1]
+                  if not abs(ty_fit - ty) < pf["T_ty"]:
+                      continue
+                  Qy = float(np.sum((yi - Ay @ ypar) ** 2)) / pf["T_y"]
+                  Q = (Qx / (n - 3) + Qy / (n_uv - 2)) * pf["C_nhits"][min(3, max(0, n - 9))]
+                  if not Q < pf["T_Q"]:
+                      continue
+                  if best is None or Q < best[0]:
+                      dslope = par[1] - tx
+                      F = sum(c * dslope ** k for k, c in enumerate(poly))
+                      state = [float(basis(z_state) @ par), ypar[0] + ypar[1] * (z_state - z_ref),
+                               float(dbasis(z_state) @ par), ty_fit, dslope / F]
+                      best = (Q, hit, n, state)
             if best is not None:
                 tracks.append((si, best[1], best[2], best[3], best[0]))
         ev_off.append(len(tracks))

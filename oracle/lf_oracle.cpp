@@ -12,6 +12,9 @@
  *   O5 u/v extension
  *   O6 fit + quality    PAPER.md:238-279 (Eq. 5, 6, Table 4)
  *   O7 momentum, state  PAPER.md:327-338 (Eq. 9), 388
+ *   no-UT tuning        PAPER.md:285-325 (Eq. 7, 8, Table 5): params.mode == 1 replaces O1/O2 by a
+ *                       straight-line extrapolation with double-sided windows and follows each window
+ *                       side (charge assumption) separately through O3..O6 (N1..N9)
  *
  * Arithmetic: every floating-point operation is done in `Real` (float in the reference build,
  * double in the pin build) in exactly the order written below, one rounding per operation
@@ -127,7 +130,7 @@ int closest_idx(const float* x, const Window& wdw, Real pred) {
 
 struct SeedState {
   Real x, y, tx, ty, qop;
-  Real aq, p, x_mag, txp;
+  Real aq, p, x_mag, txp;  /* mode 1: aq = 1/p of the assumed minimum momentum, qop and txp unused */
   Real yl[NL], yt[NL];  /* y at each layer; y*tan_alpha */
   int zone;
   Window win[NL];
@@ -180,6 +183,53 @@ void extrapolate_and_windows(const Geo& g, const lfo_params& P, const float* hx,
   }
 }
 
+/* no-UT O1 + O2 for one window side (0 = LEFT, 1 = RIGHT of Eq. 8). */
+void velo_windows(const Geo& g, const lfo_params& P, const float* hx, const uint32_t* seg, int side,
+                  SeedState& s) {
+  /* the momentum is set to the tighter (larger) of p_min and pT_min / sin(theta);
+   * as 1/p: min(1/p_min, sin(theta)/pT_min), sin^2(theta) = (tx^2+ty^2)/(1+tx^2+ty^2)  (N2). */
+  const Real s2 = s.tx * s.tx + s.ty * s.ty;
+  const Real sin_theta = std::sqrt(s2 / (RC(1.0) + s2));
+  const Real inv_p = std::min(RC(1.0) / Real(P.velo_p_min), sin_theta * (RC(1.0) / Real(P.velo_pt_min)));
+  s.aq = inv_p;
+  s.p = RC(1.0) / std::max(inv_p, RC(1e-6));
+  s.x_mag = s.x + s.tx * g.mag_dz_seed;
+  s.txp = s.tx;
+  s.zone = (s.ty >= 0) ? 1 : 0; /* t_y still chooses the half */
+  /* Eq. (7) with Table 5. */
+  Real c[8];
+  for (int i = 0; i < 8; ++i) c[i] = Real(P.xtol_poly[i]);
+  const Real x_tol = inv_p * (((c[0] + s.tx * (c[1] + c[2] * s.tx)) +
+                               (s.ty * s.ty) * (c[3] + s.tx * (c[4] + c[5] * s.tx))) +
+                              inv_p * (c[6] * s.tx + c[7] * inv_p));
+  for (int l = 0; l < NL; ++l) {
+    /* straight-line extrapolation of the VELO track to the layer */
+    const Real xe = s.x + s.tx * g.dzs[l];
+    s.yl[l] = s.y + s.ty * g.dzs[l];
+    s.yt[l] = is_uv(l) ? s.yl[l] * g.tana[l] : RC(0.0);
+    const Real ctr = is_uv(l) ? xe + s.yt[l] : xe;                 /* PAPER.md:321 (as PAPER.md:202) */
+    const Real tol = is_uv(l) ? Real(P.uv_half_width) : x_tol;     /* 1200 mm on u/v */
+    /* Eq. (8) */
+    const Real lo = (side == 0) ? ctr - tol : ctr - Real(P.x_overlap);
+    const Real hi = (side == 0) ? ctr + Real(P.x_overlap) : ctr + tol;
+    const int sb = int(seg[l * 2 + s.zone]), se = int(seg[l * 2 + s.zone + 1]);
+    int first = lower_idx(hx, sb, se, lo);
+    int last = upper_idx(hx, sb, se, hi);
+    if (last < first) last = first;
+    /* at most n_window hits, symmetric about the centre of each window (C4) */
+    if (last - first > P.n_window) {
+      const Real mid = (lo + hi) * RC(0.5);
+      const int cidx = lower_idx(hx, first, last, mid);
+      const int half = P.n_window / 2;
+      const int f2 = std::max(first, cidx - half);
+      const int l2 = std::min(last, cidx + half);
+      first = f2; last = l2;
+    }
+    s.win[l].first = first;
+    s.win[l].count = last - first;
+  }
+}
+
 /* O3: all doublets of both layer sets, two filters, h1 lookup, top n by chi2. */
 void triplet_seeding(const Geo& g, const lfo_params& P, const float* hx, const SeedState& s,
                      std::vector<Triplet>& out) {
@@ -192,7 +242,8 @@ void triplet_seeding(const Geo& g, const lfo_params& P, const float* hx, const S
         const Real x0 = hx[i0], x2 = hx[i2];
         const Real t = (x2 - x0) * g.inv_dz_ac[set];
         /* filter 1 (C7): below 5 GeV the doublet must bend like the seed's charge */
-        if (s.p < Real(P.p_same_bend) && !((t - s.tx) * s.qop > 0)) continue;
+        /* (no-UT: the VELO track has no momentum or charge, so the filter does not exist) */
+        if (P.mode == 0 && s.p < Real(P.p_same_bend) && !((t - s.tx) * s.qop > 0)) continue;
         /* filter 2 (C6): opening at the magnet centre */
         const Real x_at_mag = x0 + t * g.zmag_a[set];
         const Real tol = std::min(Real(P.mag_tol_max),
@@ -347,6 +398,9 @@ extern "C" int lf_oracle_run(const lfo_geometry* G, const lfo_params* P, const l
                              const lfo_hits* hits, size_t n_events, lfo_tracks* out, lfo_debug* dbg) {
   if (!G || !P || !seeds || !hits || !out) return 1;
   if (G->n_layers != NL || P->n_window < 2 || P->n_triplets < 1) return 1;
+  if (P->mode != 0 && P->mode != 1) return 1;
+  if (P->mode == 0 && !seeds->qop) return 1;
+  const int n_sides = (P->mode == 1) ? 2 : 1;
   if (!out->event_offsets || !out->n_tracks) return 1;
   const Geo g = make_geo(*G);
   const float* hx = hits->x;
@@ -359,43 +413,49 @@ extern "C" int lf_oracle_run(const lfo_geometry* G, const lfo_params* P, const l
     for (uint32_t si = seeds->event_offsets[ev]; si < seeds->event_offsets[ev + 1]; ++si) {
       SeedState s;
       s.x = seeds->x[si]; s.y = seeds->y[si]; s.tx = seeds->tx[si]; s.ty = seeds->ty[si];
-      s.qop = seeds->qop[si];
-      extrapolate_and_windows(g, *P, hx, seg, s);
-      triplet_seeding(g, *P, hx, s, trips);
-      if (dbg) {
-        for (int l = 0; l < NL; ++l) {
-          if (dbg->win_first) dbg->win_first[size_t(si) * NL + l] = s.win[l].first;
-          if (dbg->win_count) dbg->win_count[size_t(si) * NL + l] = s.win[l].count;
-        }
-        if (dbg->n_triplets) dbg->n_triplets[si] = int(trips.size());
-        for (int k = 0; k < NT; ++k) {
-          const bool have = k < int(trips.size());
-          const size_t o = size_t(si) * NT + k;
-          if (dbg->trip_hits) {
-            dbg->trip_hits[o * 3 + 0] = have ? trips[k].i0 : -1;
-            dbg->trip_hits[o * 3 + 1] = have ? trips[k].i1 : -1;
-            dbg->trip_hits[o * 3 + 2] = have ? trips[k].i2 : -1;
-          }
-          if (dbg->trip_set) dbg->trip_set[o] = have ? trips[k].set : -1;
-          if (dbg->trip_chi2) dbg->trip_chi2[o] = have ? float(trips[k].chi2) : -1.0f;
-          if (dbg->cand_quality) dbg->cand_quality[o] = -1.0f;
-          if (dbg->cand_hits) for (int l = 0; l < NL; ++l) dbg->cand_hits[o * NL + l] = -1;
-        }
-      }
-      /* O4..O6 for each kept triplet; accept Q < T_Q, keep the lowest Q (C15, C16). */
+      s.qop = (P->mode == 0) ? Real(seeds->qop[si]) : RC(0.0);
+      /* accept Q < T_Q, keep the lowest Q (C15, C16).  no-UT: each window side (charge
+       * assumption) is followed on its own; the lowest Q over both sides is kept (N8). */
       bool have_best = false;
       Candidate best;
-      for (int k = 0; k < int(trips.size()); ++k) {
-        Candidate cd;
-        extend(g, *P, hx, s, trips[k], cd);
-        const size_t o = size_t(si) * NT + k;
-        if (dbg && dbg->cand_hits) for (int l = 0; l < NL; ++l) dbg->cand_hits[o * NL + l] = cd.hit[l];
-        if (!cd.enough) continue;
-        fit_quality(g, *P, hx, s, cd);
-        if (dbg && dbg->cand_quality) dbg->cand_quality[o] = cd.ty_ok ? float(cd.Q) : -2.0f;
-        if (!cd.ty_ok) continue;
-        if (!(cd.Q < Real(P->T_Q))) continue;
-        if (!have_best || cd.Q < best.Q) { best = cd; have_best = true; }
+      for (int side = 0; side < n_sides; ++side) {
+        if (P->mode == 0) extrapolate_and_windows(g, *P, hx, seg, s);
+        else velo_windows(g, *P, hx, seg, side, s);
+        triplet_seeding(g, *P, hx, s, trips);
+        const size_t row = size_t(si) * n_sides + side;
+        if (dbg) {
+          for (int l = 0; l < NL; ++l) {
+            if (dbg->win_first) dbg->win_first[row * NL + l] = s.win[l].first;
+            if (dbg->win_count) dbg->win_count[row * NL + l] = s.win[l].count;
+          }
+          if (dbg->n_triplets) dbg->n_triplets[row] = int(trips.size());
+          for (int k = 0; k < NT; ++k) {
+            const bool have = k < int(trips.size());
+            const size_t o = row * NT + k;
+            if (dbg->trip_hits) {
+              dbg->trip_hits[o * 3 + 0] = have ? trips[k].i0 : -1;
+              dbg->trip_hits[o * 3 + 1] = have ? trips[k].i1 : -1;
+              dbg->trip_hits[o * 3 + 2] = have ? trips[k].i2 : -1;
+            }
+            if (dbg->trip_set) dbg->trip_set[o] = have ? trips[k].set : -1;
+            if (dbg->trip_chi2) dbg->trip_chi2[o] = have ? float(trips[k].chi2) : -1.0f;
+            if (dbg->cand_quality) dbg->cand_quality[o] = -1.0f;
+            if (dbg->cand_hits) for (int l = 0; l < NL; ++l) dbg->cand_hits[o * NL + l] = -1;
+          }
+        }
+        /* O4..O6 for each kept triplet */
+        for (int k = 0; k < int(trips.size()); ++k) {
+          Candidate cd;
+          extend(g, *P, hx, s, trips[k], cd);
+          const size_t o = row * NT + k;
+          if (dbg && dbg->cand_hits) for (int l = 0; l < NL; ++l) dbg->cand_hits[o * NL + l] = cd.hit[l];
+          if (!cd.enough) continue;
+          fit_quality(g, *P, hx, s, cd);
+          if (dbg && dbg->cand_quality) dbg->cand_quality[o] = cd.ty_ok ? float(cd.Q) : -2.0f;
+          if (!cd.ty_ok) continue;
+          if (!(cd.Q < Real(P->T_Q))) continue;
+          if (!have_best || cd.Q < best.Q) { best = cd; have_best = true; }
+        }
       }
       if (!have_best) continue;
       if (n_out >= out->capacity) return 3;

@@ -15,7 +15,8 @@
  *   - invariants on every config; LSQ fits vs numpy.linalg.lstsq in float64; windows vs
  *     numpy.searchsorted; fp32 build vs fp64 build of this same file.
  * Parity-unpinned BY THE PAPER (pinned only by DESIGN.md's reading): the magnet-tolerance formula
- * (C6), the T_uv floor (C12), which chi^2 enters Q (C13).
+ * (C6), the T_uv floor (C12), which chi^2 enters Q (C13); in the no-UT mode: whether the triplet cap
+ * is per charge assumption or per track (N6).
  */
 #ifndef LF_ORACLE_H
 #define LF_ORACLE_H
@@ -49,6 +50,11 @@ typedef struct {
   float xtol_base, xtol_inv_p, x_asym, uv_half_width;           /* PAPER.md:191-202 */
   float p_same_bend, mag_tol_base, mag_tol_inv_p, mag_tol_tx, mag_tol_max; /* PAPER.md:210-211 */
   int32_t hit_storage;                                          /* ignored: the oracle is always fp32 storage */
+  /* "no-UT" tuning (PAPER.md:285-325): VELO seeds without momentum, double-sided windows. */
+  int32_t mode;                 /* 0 = with UT (sections VI.A-D), 1 = no-UT (section VI.E) */
+  float velo_p_min, velo_pt_min; /* assumed minimum momentum / transverse momentum, GeV: 5, 1 (PAPER.md:289) */
+  float xtol_poly[8];           /* c0..c7 of Eq. (7), Table 5 (PAPER.md:293, 311-315) */
+  float x_overlap;              /* overlap of the two windows of Eq. (8): 5 mm (PAPER.md:319) */
 } lfo_params;
 
 typedef struct {
@@ -72,7 +78,9 @@ typedef struct {
   size_t capacity;         /* rows available in the arrays above */
 } lfo_tracks;
 
-/* Optional stage-boundary outputs (any pointer may be NULL).  NT = params.n_triplets. */
+/* Optional stage-boundary outputs (any pointer may be NULL).  NT = params.n_triplets.
+ * Rows are "followed tracks": mode 0 one per seed (row = seed); mode 1 one per (seed, window side),
+ * row = 2*seed + side, side 0 = LEFT, 1 = RIGHT of Eq. (8); read n_seeds below as the number of rows. */
 typedef struct {
   int32_t* win_first;     /* n_seeds*12: global index of the first hit of the (capped) window */
   int32_t* win_count;     /* n_seeds*12 */

@@ -56,7 +56,9 @@ class _Params(C.Structure):
                 ("uv_half_width", C.c_float),
                 ("p_same_bend", C.c_float), ("mag_tol_base", C.c_float), ("mag_tol_inv_p", C.c_float),
                 ("mag_tol_tx", C.c_float), ("mag_tol_max", C.c_float),
-                ("hit_storage", C.c_int32)]
+                ("hit_storage", C.c_int32),
+                ("mode", C.c_int32), ("velo_p_min", C.c_float), ("velo_pt_min", C.c_float),
+                ("xtol_poly", C.c_float * 8), ("x_overlap", C.c_float)]
 
 
 _FP = C.POINTER(C.c_float)
@@ -113,6 +115,7 @@ def _p(a: np.ndarray, t):
 
 
 def _run_one(lib, geo, par, b, n_triplets: int, debug: bool):
+    n_sides = 2 if int(par.mode) == 1 else 1  # rows of the debug tables per seed (lf_oracle.h)
     f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
     u32 = lambda a: np.ascontiguousarray(a, dtype=np.uint32)
     sx, sy, stx, sty, sq = f32(b.seed_x), f32(b.seed_y), f32(b.seed_tx), f32(b.seed_ty), f32(b.seed_qop)
@@ -132,12 +135,12 @@ def _run_one(lib, geo, par, b, n_triplets: int, debug: bool):
     dbg_ptr = None
     dbg = None
     if debug:
-        nt = n_triplets
+        nt, rows = n_triplets, cap * n_sides
         dbg = SimpleNamespace(
-            win_first=np.zeros((cap, NL), np.int32), win_count=np.zeros((cap, NL), np.int32),
-            n_triplets=np.zeros(cap, np.int32), trip_hits=np.full((cap, nt, 3), -1, np.int32),
-            trip_set=np.full((cap, nt), -1, np.int32), trip_chi2=np.full((cap, nt), -1, np.float32),
-            cand_hits=np.full((cap, nt, NL), -1, np.int32), cand_quality=np.full((cap, nt), -1, np.float32))
+            win_first=np.zeros((rows, NL), np.int32), win_count=np.zeros((rows, NL), np.int32),
+            n_triplets=np.zeros(rows, np.int32), trip_hits=np.full((rows, nt, 3), -1, np.int32),
+            trip_set=np.full((rows, nt), -1, np.int32), trip_chi2=np.full((rows, nt), -1, np.float32),
+            cand_hits=np.full((rows, nt, NL), -1, np.int32), cand_quality=np.full((rows, nt), -1, np.float32))
         d = _Debug(_p(dbg.win_first, _IP), _p(dbg.win_count, _IP), _p(dbg.n_triplets, _IP),
                    _p(dbg.trip_hits, _IP), _p(dbg.trip_set, _IP), _p(dbg.trip_chi2, _FP),
                    _p(dbg.cand_hits, _IP), _p(dbg.cand_quality, _FP))
@@ -151,7 +154,7 @@ def _run_one(lib, geo, par, b, n_triplets: int, debug: bool):
                           debug=None)
     if dbg is not None:
         for k, v in vars(dbg).items():
-            setattr(dbg, k, v[:n_seeds])
+            setattr(dbg, k, v[:n_seeds * n_sides])
         res.debug = dbg
     return res
 

@@ -99,7 +99,20 @@ def default_params() -> Dict[str, object]:
         "p_same_bend": 5.0, "mag_tol_base": 8.0, "mag_tol_inv_p": 60.0, "mag_tol_tx": 20.0,
         "mag_tol_max": 40.0,
         "hit_storage": 0,
+        # no-UT tuning; inactive while mode == 0
+        "mode": 0, "velo_p_min": 5.0, "velo_pt_min": 1.0,
+        "xtol_poly": [4824.3, 426.3, 7071.1, 12080.4, 14077.8, 13909.3, 9315.3, 3209.5],  # Table 5
+        "x_overlap": 5.0,
     }
+
+
+def no_ut_params() -> Dict[str, object]:
+    """Table 3 "Forward no-UT" column + section VI.E: VELO seeds without
+    momentum, double-sided windows of Eq. (7)/(8) with Table 5, u/v tolerance 1200 mm, 64 hits per window,
+    20 triplets, fixed 10 mm tolerance at the magnet, no same-bend filter (N1..N9)."""
+    return dict(default_params(), mode=1, T_triplet=2.0, T_x=0.5, T_uv_slope=15.0, T_ty=0.003,
+                n_window=64, n_triplets=20, uv_half_width=1200.0,
+                p_same_bend=0.0, mag_tol_base=10.0, mag_tol_inv_p=0.0, mag_tol_tx=0.0, mag_tol_max=10.0)
 
 
 def toy_x_at(x_mag, txp, dtx, z):
