@@ -13,6 +13,11 @@
  *   a6 fit, quality factor Q, best per seed, q/p  PAPER.md:238-279 (Eq. 5, 6), 327-338 (Eq. 9)
  *   a7 stream compaction into dense track lists   north_star (c)
  *
+ * params.mode = 1 selects the "no-UT" tuning of the same path (section VI.E): the seeds are
+ * VELO tracks without momentum or charge; a1/a2 become a straight-line extrapolation with the double-sided
+ * windows of Eq. (7)/(8) and Table 5; each window side (charge assumption) is followed separately through
+ * a3..a6 and the lowest Q over both sides is kept (readings N1..N9).
+ *
  * All of it runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.  The readings of
  * the points the paper leaves open are listed in DESIGN.md ("Readings", C1..C22).
  *
@@ -39,11 +44,13 @@
 extern "C" {
 #endif
 
-#define LF_ABI_VERSION 2u
+#define LF_ABI_VERSION 3u
 #define LF_N_LAYERS 12   /* three T-stations, x-u-v-x each */
 #define LF_N_ZONES 2     /* lower / upper half */
-#define LF_MAX_WINDOW 32   /* largest params.n_window this build supports (one warp lane per hit) */
-#define LF_MAX_TRIPLETS 16 /* largest params.n_triplets this build supports */
+#define LF_MAX_WINDOW 32   /* largest params.n_window of the narrow kernels (one warp lane per hit) */
+#define LF_MAX_TRIPLETS 16 /* largest params.n_triplets of the narrow kernels */
+#define LF_MAX_WINDOW_WIDE 64   /* largest params.n_window at all: beyond LF_MAX_WINDOW / LF_MAX_TRIPLETS, and always */
+#define LF_MAX_TRIPLETS_WIDE 32 /* in the no-UT mode, the library runs the wide build of its kernels */
 
 typedef struct lf_handle lf_handle; /* opaque; owned by the library */
 
@@ -75,19 +82,26 @@ typedef struct {
 typedef struct {
   float T_triplet, T_x, T_uv_slope, T_uv_min, T_ty, T_y, T_Q; /* 8, 2, 50, 0.5, 0.02, 800, 0.5 */
   float C_nhits[4];                                           /* C(n) for n = 9..12: 5, 1, 0.8, 0.5 */
-  int32_t n_window, n_triplets, min_hits;                     /* 32, 12, 9;  2 <= n_window <= LF_MAX_WINDOW,
-                                                                 1 <= n_triplets <= LF_MAX_TRIPLETS */
+  int32_t n_window, n_triplets, min_hits;                     /* 32, 12, 9 (no-UT: 64, 20, 9);  2 <= n_window <=
+                                                                 LF_MAX_WINDOW_WIDE, 1 <= n_triplets <= LF_MAX_TRIPLETS_WIDE */
   float xtol_base, xtol_inv_p, x_asym, uv_half_width;         /* 150, 2000, 100, 800 */
   float p_same_bend, mag_tol_base, mag_tol_inv_p, mag_tol_tx, mag_tol_max; /* 5, 8, 60, 20, 40 */
   int32_t hit_storage;                                        /* 0 = fp32 (bit-exact reference path); 1 = the library keeps
                                                                  an fp16 copy of the hits (block-offset encoding) that the
                                                                  window and seeding kernels read; extension and fit stay on
-                                                                 the fp32 hits (BASELINE.json configs[2]) */
+                                                                 the fp32 hits (BASELINE.json configs[2]);
+                                                                 mode 0 with the narrow limits only (LF_ERR_UNSUPPORTED otherwise) */
+  /* no-UT tuning; read only when mode == 1 */
+  int32_t mode;                  /* 0 = with UT (sections VI.A-D); 1 = no-UT (section VI.E): seeds->qop is not read, the same-bend
+                                    filter does not exist, the magnet tolerance uses the assumed 1/p where q/p stood */
+  float velo_p_min, velo_pt_min; /* assumed minimum momentum / transverse momentum, GeV: 5, 1; > 0 */
+  float xtol_poly[8];            /* c0..c7 of Eq. (7), Table 5 */
+  float x_overlap;               /* overlap of the LEFT and RIGHT windows of Eq. (8): 5 mm */
 } lf_params;
 
 /* Input seeds: upstream track states at z_seed, SoA, all events back to back. */
 typedef struct {
-  const float *x, *y, *tx, *ty, *qop; /* n_seeds each */
+  const float *x, *y, *tx, *ty, *qop; /* n_seeds each; qop is not read (may be NULL) when params.mode == 1 */
   const uint32_t* event_offsets;      /* n_events + 1; seeds of event e are [off[e], off[e+1]) */
   size_t n_seeds;                     /* == event_offsets[n_events] (caller's knowledge; no device read-back) */
 } lf_seeds;
@@ -114,7 +128,9 @@ typedef struct {
 } lf_tracks;
 
 /* Optional stage-boundary outputs for parity tests (device pointers; any may be NULL).
- * NT = params.n_triplets.  Indices are global hit indices; -1 = none. */
+ * NT = params.n_triplets.  Indices are global hit indices; -1 = none.  Rows are followed tracks: one per seed
+ * (row = seed) when mode == 0; one per (seed, window side) when mode == 1, row = 2*seed + side with side 0 =
+ * LEFT and 1 = RIGHT window of Eq. (8): read n_seeds below as the number of rows. */
 typedef struct {
   int32_t* win_first;   /* n_seeds*12: first hit of the (capped) search window (undefined if empty) */
   int32_t* win_count;   /* n_seeds*12: hits in the window (<= n_window) */
@@ -145,7 +161,7 @@ typedef struct {
 
 /* Creates a context for batches of at most max_events / max_seeds / max_hits.  Validates geometry
  * and params, uploads constants, allocates the workspace (about max_seeds*(141 + 18*n_triplets) +
- * max_events*16 bytes on the current CUDA device, sized for 180 GB parts).  The shared-memory stage for one event's hits is sized
+ * max_events*16 bytes, roughly twice that in the no-UT mode, on the current CUDA device, sized for 180 GB parts).  The shared-memory stage for one event's hits is sized
  * from the maxima: 1.25 * max_hits / max_events + 512 hits, clamped to [2048, 16384]; larger events are
  * still processed correctly, reading their hits from global memory.  *out is set only on LF_OK.
  * HOST pointers. */

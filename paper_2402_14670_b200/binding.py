@@ -45,7 +45,9 @@ class lf_params(C.Structure):
                 ("uv_half_width", C.c_float),
                 ("p_same_bend", C.c_float), ("mag_tol_base", C.c_float), ("mag_tol_inv_p", C.c_float),
                 ("mag_tol_tx", C.c_float), ("mag_tol_max", C.c_float),
-                ("hit_storage", C.c_int32)]
+                ("hit_storage", C.c_int32),
+                ("mode", C.c_int32), ("velo_p_min", C.c_float), ("velo_pt_min", C.c_float),
+                ("xtol_poly", C.c_float * 8), ("x_overlap", C.c_float)]
 
 
 class lf_seeds(C.Structure):
@@ -119,7 +121,7 @@ def load_library() -> C.CDLL:
     lib.lf_set_profiling.argtypes = [C.c_void_p, C.c_int]
     lib.lf_kernel_times.restype = C.c_int
     lib.lf_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_float * 6)]
-    if lib.lf_abi_version() != 2:
+    if lib.lf_abi_version() != 3:
         raise ImportError("liblf_b200.so: ABI version mismatch")
     for i, st in enumerate(_STRUCTS):
         if lib.lf_sizeof(i) != C.sizeof(st):
@@ -241,7 +243,9 @@ class LookingForward:
             self._check(self._lib.lf_run(self._h, C.byref(seeds), C.byref(hits), db.n_events, C.byref(tr), sp))
             return out
         import torch
-        nt, ns, dev = int(self.params["n_triplets"]), max(db.n_seeds, 1), db.device
+        # one row per followed track: per seed, or per (seed, window side) in the no-UT mode (include/lf.h, lf_debug)
+        sides = 2 if int(self.params.get("mode", 0)) == 1 else 1
+        nt, ns, dev = int(self.params["n_triplets"]), max(db.n_seeds, 1) * sides, db.device
         i32 = lambda *shape: torch.full(shape, -1, dtype=torch.int32, device=dev)
         f32 = lambda *shape: torch.full(shape, -1.0, dtype=torch.float32, device=dev)
         d = SimpleNamespace(win_first=i32(ns, NL), win_count=i32(ns, NL), n_triplets=i32(ns), trip_hits=i32(ns, nt, 3),

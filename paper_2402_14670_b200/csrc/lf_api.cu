@@ -53,8 +53,10 @@ struct lf_handle {
   /* workspace */
   __half* hx16;     /* hit_storage = 1 only */
   float* origin16;
+  bool wide;        /* the wide build of the event kernels runs (no-UT mode, or caps beyond the narrow limits) */
+  int sides;        /* followed tracks (rows) per seed: 2 in the no-UT mode */
   uint32_t* win;
-  uint16_t* trip_code;
+  void* trip_code;
   uint8_t* n_trip;
   int32_t *ws_rec, *ws_nh, *ws_rank, *ws_event;
   uint32_t *ev_count, *ev_off, *ev_dup, *ev_acc, *tickets;
@@ -140,6 +142,14 @@ void make_consts(const lf_geometry& G, const lf_params& P, lf::Consts& c) {
   c.xtol_base = P.xtol_base; c.xtol_inv_p = P.xtol_inv_p; c.x_asym = P.x_asym; c.uv_half_width = P.uv_half_width;
   c.p_same_bend = P.p_same_bend; c.mag_tol_base = P.mag_tol_base; c.mag_tol_inv_p = P.mag_tol_inv_p;
   c.mag_tol_tx = P.mag_tol_tx; c.mag_tol_max = P.mag_tol_max;
+  c.mode = P.mode;
+  c.sides = (P.mode == 1) ? 2 : 1;
+  if (P.mode == 1) {
+    c.inv_p_min = one / P.velo_p_min;
+    c.inv_pt_min = one / P.velo_pt_min;
+    for (int i = 0; i < 8; ++i) c.xtol_poly[i] = P.xtol_poly[i];
+    c.x_overlap = P.x_overlap;
+  }
 }
 
 /* Geometry sums and cofactors of the two least-squares fits for every 12-bit hit-presence mask, in the
@@ -183,8 +193,15 @@ const char* validate(const lf_geometry& G, const lf_params& P) {
   }
   if (!(G.z_mag > G.z_seed) || !(G.z[0] > G.z_mag)) return "geometry: need z_seed < z_mag < z[0]";
   if (G.polarity != 1 && G.polarity != -1) return "geometry.polarity must be +1 or -1";
-  if (P.n_window < 2 || P.n_window > LF_MAX_WINDOW) return "params.n_window out of [2, LF_MAX_WINDOW]";
-  if (P.n_triplets < 1 || P.n_triplets > LF_MAX_TRIPLETS) return "params.n_triplets out of [1, LF_MAX_TRIPLETS]";
+  if (P.n_window < 2 || P.n_window > LF_MAX_WINDOW_WIDE) return "params.n_window out of [2, LF_MAX_WINDOW_WIDE]";
+  if (P.n_triplets < 1 || P.n_triplets > LF_MAX_TRIPLETS_WIDE) return "params.n_triplets out of [1, LF_MAX_TRIPLETS_WIDE]";
+  if (P.mode != 0 && P.mode != 1) return "params.mode must be 0 (with UT) or 1 (no-UT)";
+  if (P.mode == 1) {
+    if (!(P.velo_p_min > 0) || !(P.velo_pt_min > 0)) return "params: velo_p_min and velo_pt_min must be positive";
+    for (int i = 0; i < 8; ++i)
+      if (!std::isfinite(P.xtol_poly[i])) return "params.xtol_poly: non-finite coefficient";
+    if (!std::isfinite(P.x_overlap)) return "params.x_overlap: non-finite";
+  }
   if (P.min_hits < 4 || P.min_hits > 12) return "params.min_hits out of [4, 12]";
   if (!(P.T_triplet > 0) || !(P.T_x > 0) || !(P.T_y > 0) || !(P.T_uv_min > 0) || !(P.T_Q > 0) || !(P.T_ty > 0))
     return "params: tolerances must be positive";
@@ -192,8 +209,12 @@ const char* validate(const lf_geometry& G, const lf_params& P) {
   return nullptr;
 }
 
-template <bool DEBUG>
-lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
+bool use_wide(const lf_params& P) {
+  return P.mode == 1 || P.n_window > LF_MAX_WINDOW || P.n_triplets > LF_MAX_TRIPLETS;
+}
+
+template <bool DEBUG, bool WIDE>
+lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
                  const lf_debug* dbg, cudaStream_t st, size_t seed_base = 0) {
   const bool prof = h->profiling;
   cudaEvent_t* pe = prof ? h->prof_ev[h->prof_runs % PROF_RING] : nullptr;
@@ -228,24 +249,24 @@ lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_
   }
   if (work) {
     A.ticket = h->tickets + 0;
-    lf::lf_window_kernel<DEBUG><<<grid_of(0), lf::WIN_THREADS, h->smem_bytes[0], st>>>(h->C, A);
+    lf::lf_window_kernel<DEBUG, WIDE><<<grid_of(0), lf::WIN_THREADS, h->smem_bytes[0], st>>>(h->C, A);
   }
   if (prof) LF_CUDA(h, cudaEventRecord(pe[1], st));
   if (work) {
     A.ticket = h->tickets + 1;
-    lf::lf_seed_kernel<DEBUG><<<grid_of(1), lf::SEED_THREADS, h->smem_bytes[1], st>>>(h->C, A);
+    lf::lf_seed_kernel<DEBUG, WIDE><<<grid_of(1), lf::SEED_THREADS, h->smem_bytes[1], st>>>(h->C, A);
   }
   if (prof) LF_CUDA(h, cudaEventRecord(pe[2], st));
   A.hx16 = nullptr; /* extension and fit always read the fp32 hits */
   A.origin16 = nullptr;
   if (work) {
     A.ticket = h->tickets + 2;
-    lf::lf_extend_kernel<DEBUG><<<grid_of(2), lf::FIT_THREADS, h->smem_bytes[2], st>>>(h->C, A);
+    lf::lf_extend_kernel<DEBUG, WIDE><<<grid_of(2), lf::FIT_THREADS, h->smem_bytes[2], st>>>(h->C, A);
   }
   if (prof) LF_CUDA(h, cudaEventRecord(pe[3], st));
   if (work) {
     A.ticket = h->tickets + 3;
-    lf::lf_fit_kernel<DEBUG><<<grid_of(3), lf::FIT_THREADS, h->smem_bytes[3], st>>>(h->C, A);
+    lf::lf_fit_kernel<DEBUG, WIDE><<<grid_of(3), lf::FIT_THREADS, h->smem_bytes[3], st>>>(h->C, A);
   }
   if (prof) LF_CUDA(h, cudaEventRecord(pe[4], st));
   lf::lf_scan_kernel<<<1, 1024, 0, st>>>(h->ev_count, (uint32_t)n_events, h->ev_off, out->event_offsets,
@@ -265,12 +286,19 @@ lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_
   return LF_OK;
 }
 
+template <bool DEBUG>
+lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
+                 const lf_debug* dbg, cudaStream_t st, size_t seed_base = 0) {
+  return h->wide ? launch_impl<DEBUG, true>(h, seeds, hits, n_events, out, dbg, st, seed_base)
+                 : launch_impl<DEBUG, false>(h, seeds, hits, n_events, out, dbg, st, seed_base);
+}
+
 lf_status check_run_args(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out) {
   if (!h) return LF_ERR_INVALID_ARG;
   if (!seeds || !hits || !out) return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL seeds/hits/out");
   if (!seeds->event_offsets || !hits->seg_offsets || !out->event_offsets || !out->n_tracks)
     return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL offset table or n_tracks pointer");
-  if (seeds->n_seeds > 0 && (!seeds->x || !seeds->y || !seeds->tx || !seeds->ty || !seeds->qop))
+  if (seeds->n_seeds > 0 && (!seeds->x || !seeds->y || !seeds->tx || !seeds->ty || (!seeds->qop && h->P.mode == 0)))
     return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL seed array");
   if (hits->n_hits > 0 && !hits->x) return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL hit array");
   if (seeds->n_seeds > 0 && (!out->hit_idx || !out->seed_idx || !out->n_hits || !out->state || !out->quality))
@@ -313,6 +341,8 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   if (!geometry || !params || !out) return fail(nullptr, LF_ERR_INVALID_ARG, "lf_create: NULL argument");
   *out = nullptr;
   if (const char* why = validate(*geometry, *params)) return fail(nullptr, LF_ERR_INVALID_ARG, std::string("lf_create: ") + why);
+  if (params->hit_storage == 1 && use_wide(*params))
+    return fail(nullptr, LF_ERR_UNSUPPORTED, "lf_create: hit_storage = 1 needs mode 0 with n_window <= 32 and n_triplets <= 16");
   if (max_hits >= (size_t)0x7fffffff || max_seeds >= (size_t)0x7fffffff || max_events >= (size_t)0x7fffffff / LF_N_LAYERS / 2)
     return fail(nullptr, LF_ERR_CAPACITY, "lf_create: maxima must fit 32-bit indices");
 
@@ -321,6 +351,8 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   h->G = *geometry; h->P = *params;
   h->max_events = max_events; h->max_seeds = max_seeds; h->max_hits = max_hits;
   make_consts(*geometry, *params, h->C);
+  h->wide = use_wide(*params);
+  h->sides = h->C.sides;
 
   auto bail = [&](lf_status st, const std::string& msg) { g_create_error = msg; lf_destroy(h); return st; };
 #define LF_CREATE_CUDA(call)                                                                     \
@@ -348,10 +380,15 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   h->smem_bytes[1] = (int)(stage_bytes + sizeof(lf::SeedTables));
   h->smem_bytes[2] = (int)(stage_bytes + lf::ext_tables_bytes(params->n_triplets));
   h->smem_bytes[3] = (int)(stage_bytes + lf::FIT_TABLES_BYTES);
-  const void* kern[4][2] = {{(const void*)lf::lf_window_kernel<false>, (const void*)lf::lf_window_kernel<true>},
-                            {(const void*)lf::lf_seed_kernel<false>, (const void*)lf::lf_seed_kernel<true>},
-                            {(const void*)lf::lf_extend_kernel<false>, (const void*)lf::lf_extend_kernel<true>},
-                            {(const void*)lf::lf_fit_kernel<false>, (const void*)lf::lf_fit_kernel<true>}};
+  const void* kern_n[4][2] = {{(const void*)lf::lf_window_kernel<false, false>, (const void*)lf::lf_window_kernel<true, false>},
+                              {(const void*)lf::lf_seed_kernel<false, false>, (const void*)lf::lf_seed_kernel<true, false>},
+                              {(const void*)lf::lf_extend_kernel<false, false>, (const void*)lf::lf_extend_kernel<true, false>},
+                              {(const void*)lf::lf_fit_kernel<false, false>, (const void*)lf::lf_fit_kernel<true, false>}};
+  const void* kern_w[4][2] = {{(const void*)lf::lf_window_kernel<false, true>, (const void*)lf::lf_window_kernel<true, true>},
+                              {(const void*)lf::lf_seed_kernel<false, true>, (const void*)lf::lf_seed_kernel<true, true>},
+                              {(const void*)lf::lf_extend_kernel<false, true>, (const void*)lf::lf_extend_kernel<true, true>},
+                              {(const void*)lf::lf_fit_kernel<false, true>, (const void*)lf::lf_fit_kernel<true, true>}};
+  const void* (*kern)[2] = h->wide ? kern_w : kern_n;
   const int threads[4] = {lf::WIN_THREADS, lf::SEED_THREADS, lf::FIT_THREADS, lf::FIT_THREADS};
   for (int k = 0; k < 4; ++k) {
     for (int d = 0; d < 2; ++d)
@@ -366,14 +403,16 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
 
   const size_t ns = std::max<size_t>(max_seeds, 1), ne = std::max<size_t>(max_events, 1);
   const size_t nt = (size_t)params->n_triplets;
+  const size_t nrows = ns * (size_t)h->sides; /* followed tracks */
+  const size_t code_bytes = h->wide ? sizeof(uint32_t) : sizeof(uint16_t);
   if (params->hit_storage == 1) {
     const size_t nh = std::max<size_t>(max_hits, 1);
     LF_CREATE_CUDA(cudaMalloc(&h->hx16, nh * sizeof(__half)));
     LF_CREATE_CUDA(cudaMalloc(&h->origin16, ((nh >> 5) + ne * lf::NSEG + 2) * sizeof(float)));
   }
-  LF_CREATE_CUDA(cudaMalloc(&h->win, ns * lf::NL * sizeof(uint32_t)));
-  LF_CREATE_CUDA(cudaMalloc(&h->trip_code, ns * nt * sizeof(uint16_t)));
-  LF_CREATE_CUDA(cudaMalloc(&h->n_trip, ns));
+  LF_CREATE_CUDA(cudaMalloc(&h->win, nrows * lf::NL * sizeof(uint32_t)));
+  LF_CREATE_CUDA(cudaMalloc(&h->trip_code, nrows * nt * code_bytes));
+  LF_CREATE_CUDA(cudaMalloc(&h->n_trip, nrows));
   LF_CREATE_CUDA(cudaMalloc(&h->ws_rec, ns * lf::REC_WORDS * sizeof(int32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ws_nh, ns * sizeof(int32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ws_rank, ns * sizeof(int32_t)));
@@ -382,7 +421,7 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   LF_CREATE_CUDA(cudaMalloc(&h->ev_off, (ne + 1) * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ev_dup, ne * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ev_acc, ne * sizeof(uint32_t)));
-  LF_CREATE_CUDA(cudaMalloc(&h->acc_rec, ns * nt * sizeof(uint4)));
+  LF_CREATE_CUDA(cudaMalloc(&h->acc_rec, nrows * nt * sizeof(uint4)));
   {
     std::vector<lf::FitLut> lut(1u << lf::NL);
     make_fit_lut(h->C, lut.data());
@@ -391,7 +430,7 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   }
   LF_CREATE_CUDA(cudaMalloc(&h->tickets, lf::N_TICKETS * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMemset(h->tickets, 0, lf::N_TICKETS * sizeof(uint32_t)));
-  h->workspace_bytes = ns * (lf::NL * 4 + nt * (2 + sizeof(uint4)) + 1 + (lf::REC_WORDS + 3) * 4) +
+  h->workspace_bytes = nrows * (lf::NL * 4 + nt * (code_bytes + sizeof(uint4)) + 1) + ns * (lf::REC_WORDS + 3) * 4 +
                        (4 * ne + 1 + lf::N_TICKETS) * sizeof(uint32_t) + (sizeof(lf::FitLut) << lf::NL);
 #undef LF_CREATE_CUDA
   *out = h;
@@ -575,7 +614,8 @@ lf_status lf_run_host(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
     const size_t e0 = chunk_begin(c), e1 = chunk_begin(c + 1);
     const size_t s0 = so[e0], s1 = so[e1], g0 = go[e0 * lf::NSEG], g1 = go[e1 * lf::NSEG];
     for (int i = 0; i < 5 && s1 > s0; ++i)
-      LF_CUDA(h, cudaMemcpyAsync(b.seeds + i * stride + s0, src[i] + s0, (s1 - s0) * sizeof(float), cudaMemcpyHostToDevice, b.s_h2d));
+      if (src[i]) /* qop may be NULL in the no-UT mode */
+        LF_CUDA(h, cudaMemcpyAsync(b.seeds + i * stride + s0, src[i] + s0, (s1 - s0) * sizeof(float), cudaMemcpyHostToDevice, b.s_h2d));
     if (g1 > g0) LF_CUDA(h, cudaMemcpyAsync(b.hits + g0, hits->x + g0, (g1 - g0) * sizeof(float), cudaMemcpyHostToDevice, b.s_h2d));
     LF_CUDA(h, cudaEventRecord(b.ev_h2d[c], b.s_h2d));
   }

@@ -32,15 +32,37 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 namespace lf {
 
 constexpr int NL = 12;
 constexpr int NSEG = 24;
 constexpr int REC_WORDS = 20;  /* 12 hit idx, seed, n_hits, 5 state, Q */
 constexpr int TRIP_BUF = 64;   /* per-warp triplet key buffer */
-constexpr int MAX_NT = 16;     /* == LF_MAX_TRIPLETS */
+constexpr int MAX_NT = 16;     /* == LF_MAX_TRIPLETS (narrow kernels) */
+constexpr int MAX_NT_WIDE = 32; /* == LF_MAX_TRIPLETS_WIDE */
 constexpr int WIN_THREADS = 256;
-constexpr int EDGE_STEPS = 6;  /* window-edge searches span n_window + 1 hits: 2^EDGE_STEPS > LF_MAX_WINDOW + 1 */
+/* Two builds of every event kernel (template parameter WIDE):
+ *   narrow  n_window <= 32, n_triplets <= 16, one followed track ("row") per seed: the with-UT tuning; a search
+ *           window fits one hit per lane, window-relative hit indices take 5 bits;
+ *   wide    n_window <= 64, n_triplets <= 32, `sides` rows per seed (row = seed*sides + side): the no-UT tuning
+ *           (two window sides per VELO track, 64 hits, 20 triplets), and the with-UT
+ *           tuning with caps beyond the narrow limits (sides = 1). */
+template <bool WIDE>
+struct Fmt {
+  static constexpr int WB = WIDE ? 7 : 6;             /* bits of the hit count in a packed window word */
+  static constexpr uint32_t WMASK = (1u << WB) - 1u;
+  static constexpr int IB = WIDE ? 6 : 5;             /* bits of a window-relative hit index in a triplet code */
+  static constexpr uint32_t IMASK = (1u << IB) - 1u;
+  static constexpr int EDGE_STEPS = WIDE ? 7 : 6;     /* window-edge searches span n_window + 1 hits */
+  static constexpr uint32_t TOPB = WIDE ? 256u : 128u; /* first stride (bytes) of a search inside one window */
+  static constexpr int KB = WIDE ? 5 : 4;             /* bits of the triplet index k */
+  static constexpr int SIE_BITS = WIDE ? 26 : 28;     /* record tag: seed inside the event | side << 26 | k << 27 (wide) */
+  static constexpr uint32_t SIE = (1u << SIE_BITS) - 1u;
+  static constexpr int K_SHIFT = WIDE ? 27 : 28;
+  typedef typename std::conditional<WIDE, uint32_t, uint16_t>::type code_t; /* stored triplet code */
+};
 constexpr int SEED_WARPS = 8;
 constexpr int SEED_THREADS = SEED_WARPS * 32;
 constexpr int FIT_THREADS = 256;
@@ -60,6 +82,10 @@ struct Consts {
   int n_window, n_triplets, min_hits;
   float xtol_base, xtol_inv_p, x_asym, uv_half_width;
   float p_same_bend, mag_tol_base, mag_tol_inv_p, mag_tol_tx, mag_tol_max;
+  /* no-UT tuning */
+  int mode, sides;                 /* mode 1: sides = 2 (LEFT / RIGHT windows of Eq. 8) */
+  float inv_p_min, inv_pt_min;     /* 1 / velo_p_min, 1 / velo_pt_min */
+  float xtol_poly[8], x_overlap;   /* Eq. (7) / Table 5; Eq. (8) */
 };
 
 struct FitLut;
@@ -84,16 +110,18 @@ struct EventArgs {
   uint32_t n_events;
   int stage_cap;        /* floats of shared memory available for one event's hits */
   uint32_t* ticket;     /* this kernel's event ticket */
-  uint32_t* win;        /* n_seeds*12: (first_in_event << 6) | count */
-  uint16_t* trip_code;  /* n_seeds*NT: set<<15 | h0<<10 | h2<<5 | h1 (window-relative), sorted */
-  uint8_t* n_trip;      /* n_seeds */
+  /* per followed track ("row" = seed*sides + side; narrow kernels: row = seed) */
+  uint32_t* win;        /* n_rows*12: (first_in_event << WB) | count */
+  void* trip_code;      /* n_rows*NT Fmt::code_t: set<<3IB | h0<<2IB | h2<<IB | h1 (window-relative), sorted */
+  uint8_t* n_trip;      /* n_rows */
   int32_t* ws_rec;      /* n_seeds * REC_WORDS */
   int32_t* ws_nh;       /* n_seeds: 1 if the seed has a track, else 0 */
   int32_t* ws_rank;     /* n_seeds: rank among the event's tracks, -1 = none */
   int32_t* ws_event;    /* n_seeds: event of the seed */
   uint32_t* ev_count;   /* n_events */
-  uint4* acc_rec;       /* n_seeds*NT: candidates that passed the hit-count rule: 3 words of hit codes (byte l = hit of
-                           layer l inside its window, 0xFF = none), seed inside the event | k << 28; dense per event */
+  uint4* acc_rec;       /* n_rows*NT: candidates that passed the hit-count rule: 3 words of hit codes (byte l = hit of
+                           layer l inside its window, 0xFF = none), then the tag seed inside the event | k << 28
+                           (wide: | side << 26 | k << 27); dense per event */
   uint32_t* ev_acc;     /* n_events: number of such records of the event */
   const struct FitLut* fit_lut; /* 4096: per presence mask */
   uint32_t* ev_dup;     /* n_events: written by the window kernel, != 0 if two neighbouring staged hits are equal */
@@ -272,13 +300,13 @@ __device__ __forceinline__ bool fetch_event(const EventArgs& A, uint32_t& phase,
  * walk is skipped when the event has none (`dup` == false).  Returns the event-relative index, or -1 if
  * n == 0, and in `dist` the distance |x - pred| of that hit (x - pred and pred - x round to the same
  * magnitude, so dist*dist is bit-identical to (x - pred)^2).  Generic version (global-memory view). */
-template <class HV>
+template <bool WIDE, class HV>
 __device__ __forceinline__ int closest_hit(const HV& hx, int f, int n, float pred, bool dup, float& dist) {
   if (n <= 0) return -1;
   const int e = f + n;
   int pos = f;
 #pragma unroll
-  for (int s = 5; s >= 0; --s) {
+  for (int s = Fmt<WIDE>::EDGE_STEPS - 1; s >= 0; --s) {
     const int probe = pos + (1 << s);
     if (probe <= e && hx[probe - 1] < pred) pos = probe;
   }
@@ -303,13 +331,14 @@ __device__ __forceinline__ int closest_hit(const HV& hx, int f, int n, float pre
 
 /* The same on the staged hits: positions are 32-bit shared-memory byte addresses, so one search step is
  * add, bound check, LDS, compare, select. */
+template <bool WIDE>
 __device__ __forceinline__ int closest_hit(const HitView<true>& hx, int f, int n, float pred, bool dup, float& dist) {
   if (n <= 0) return -1;
   const uint32_t a = smem_u32(stage_buf()) + 4u * (uint32_t)(hx.off + f);
   const uint32_t end = a + 4u * (uint32_t)n;
   uint32_t p = a;
 #pragma unroll
-  for (uint32_t s = 128u; s >= 4u; s >>= 1) {
+  for (uint32_t s = Fmt<WIDE>::TOPB; s >= 4u; s >>= 1) {
     const uint32_t q = p + s;
     if (q <= end && lds_f32(q - 4u) < pred) p = q;
   }
@@ -335,7 +364,7 @@ __device__ __forceinline__ int closest_hit(const HitView<true>& hx, int f, int n
 /* G independent closest-hit searches in lockstep, branch-free: the G chains of dependent LDS overlap
  * (instruction-level parallelism instead of occupancy).  ww[g] is the packed window (first << 6 | count),
  * krel[g] the index of the closest hit inside its window (-1 and dist = +inf if the window is empty). */
-template <int G>
+template <int G, bool WIDE>
 __device__ __forceinline__ void closest_group(const HitView<true>& hx, const uint32_t (&ww)[G], const float (&pred)[G],
                                               bool dup, int (&krel)[G], float (&dist)[G]) {
   const float INF = __int_as_float(0x7f800000);
@@ -343,12 +372,12 @@ __device__ __forceinline__ void closest_group(const HitView<true>& hx, const uin
   uint32_t a[G], end[G], p[G];
 #pragma unroll
   for (int g = 0; g < G; ++g) {
-    a[g] = base + 4u * (ww[g] >> 6);
-    end[g] = a[g] + 4u * (ww[g] & 63u);
+    a[g] = base + 4u * (ww[g] >> Fmt<WIDE>::WB);
+    end[g] = a[g] + 4u * (ww[g] & Fmt<WIDE>::WMASK);
     p[g] = a[g];
   }
 #pragma unroll
-  for (uint32_t s = 128u; s >= 4u; s >>= 1) {
+  for (uint32_t s = Fmt<WIDE>::TOPB; s >= 4u; s >>= 1) {
 #pragma unroll
     for (int g = 0; g < G; ++g) {
       const uint32_t q = p[g] + s;
@@ -369,14 +398,14 @@ __device__ __forceinline__ void closest_group(const HitView<true>& hx, const uin
     krel[g] = (int)(k - a[g]) >> 2;
   }
 }
-template <int G>
+template <int G, bool WIDE>
 __device__ __forceinline__ void closest_group(const HitView<false>& hx, const uint32_t (&ww)[G], const float (&pred)[G],
                                               bool dup, int (&krel)[G], float (&dist)[G]) {
 #pragma unroll
   for (int g = 0; g < G; ++g) {
-    const int f = (int)(ww[g] >> 6);
+    const int f = (int)(ww[g] >> Fmt<WIDE>::WB);
     dist[g] = __int_as_float(0x7f800000);
-    const int k = closest_hit(hx, f, (int)(ww[g] & 63u), pred[g], dup, dist[g]);
+    const int k = closest_hit<WIDE>(hx, f, (int)(ww[g] & Fmt<WIDE>::WMASK), pred[g], dup, dist[g]);
     krel[g] = (k < 0) ? -1 : k - f;
   }
 }
@@ -384,64 +413,93 @@ __device__ __forceinline__ void closest_group(const HitView<false>& hx, const ui
 /* ============================================================================================
  * a1/a2: search windows.  One thread per (seed, layer, edge).
  * ============================================================================================ */
-template <bool DEBUG, bool STAGED>
+template <bool DEBUG, bool WIDE, bool STAGED>
 __device__ __forceinline__ void windows_of_event(const Consts& C, const EventArgs& A, const CtaHeader& H,
                                                  const EventCtx& E, const HitView<STAGED>& hx) {
   typedef HitView<STAGED> HV;
   typedef typename HV::pos_t pos_t;
+  typedef Fmt<WIDE> F;
   const int tid = threadIdx.x;
   const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
-  const int n_items = (int)(s1 - s0) * NL;
+  const int sides = WIDE ? C.sides : 1;
+  const int per_seed = sides * NL;
+  const int n_items = (int)(s1 - s0) * per_seed;
   const int nsteps = H.nsteps;
   const bool pol_pos = C.polarity > 0;
   const int halfw = C.n_window / 2, reach = C.n_window + 1;
   for (int it = tid; it < n_items; it += WIN_THREADS) {
-    const int sl = it / NL;
-    const int layer = it - sl * NL;
+    const int sl = it / per_seed;
+    const int rem = it - sl * per_seed;
+    const int side = WIDE ? rem / NL : 0;
+    const int layer = rem - side * NL;
     const uint32_t seed = s0 + (uint32_t)sl;
-    /* a1: pT-kick extrapolation */
+    const size_t row = (size_t)seed * sides + side;
     const float x = __ldg(A.sx + seed), y = __ldg(A.sy + seed), tx = __ldg(A.stx + seed), ty = __ldg(A.sty + seed);
-    const float qop = __ldg(A.sqop + seed);
-    const float aq = fmaxf(fabsf(qop), 1e-6f);
-    const float x_mag = x + tx * C.mag_dz_seed;
-    const float txp = tx + C.kick * qop;
-    const int zone = (ty >= 0.0f) ? 1 : 0; /* PAPER.md:165 */
-    const float xc = x_mag + txp * C.dzm[layer];
+    const int zone = (ty >= 0.0f) ? 1 : 0; /* PAPER.md:165, 289 */
     float lo, hi;
-    if (!is_uv(layer)) { /* PAPER.md:181-200, Eq. (3) */
-      const float x_tol = C.xtol_base + C.xtol_inv_p * aq;
-      const bool q_pos = qop > 0.0f;
-      const float a_left = (q_pos == pol_pos) ? C.x_asym : 0.0f;
-      const float a_right = (q_pos != pol_pos) ? C.x_asym : 0.0f;
-      lo = (xc - x_tol) - a_left;
-      hi = (xc + x_tol) + a_right;
-    } else { /* PAPER.md:202 */
-      const float yl = y + ty * C.dzs[layer];
-      const float ctr = xc + yl * C.tana[layer];
-      lo = ctr - C.uv_half_width;
-      hi = ctr + C.uv_half_width;
+    if (WIDE && C.mode == 1) {
+      /* no-UT: straight-line extrapolation of the VELO track, assumed minimum momentum,
+       * x_tol of Eq. (7), double-sided windows of Eq. (8) */
+      const float s2 = tx * tx + ty * ty;
+      const float sin_theta = sqrtf(s2 / (1.0f + s2));
+      const float inv_p = fminf(C.inv_p_min, sin_theta * C.inv_pt_min);
+      const float xe = x + tx * C.dzs[layer];
+      float ctr = xe, tol;
+      if (is_uv(layer)) {
+        const float yl = y + ty * C.dzs[layer];
+        ctr = xe + yl * C.tana[layer];
+        tol = C.uv_half_width;
+      } else {
+        const float* c = C.xtol_poly;
+        tol = inv_p * (((c[0] + tx * (c[1] + c[2] * tx)) + (ty * ty) * (c[3] + tx * (c[4] + c[5] * tx))) +
+                       inv_p * (c[6] * tx + c[7] * inv_p));
+      }
+      lo = (side == 0) ? ctr - tol : ctr - C.x_overlap;
+      hi = (side == 0) ? ctr + C.x_overlap : ctr + tol;
+    } else {
+      /* a1: pT-kick extrapolation */
+      const float qop = __ldg(A.sqop + seed);
+      const float aq = fmaxf(fabsf(qop), 1e-6f);
+      const float x_mag = x + tx * C.mag_dz_seed;
+      const float txp = tx + C.kick * qop;
+      const float xc = x_mag + txp * C.dzm[layer];
+      if (!is_uv(layer)) { /* PAPER.md:181-200, Eq. (3) */
+        const float x_tol = C.xtol_base + C.xtol_inv_p * aq;
+        const bool q_pos = qop > 0.0f;
+        const float a_left = (q_pos == pol_pos) ? C.x_asym : 0.0f;
+        const float a_right = (q_pos != pol_pos) ? C.x_asym : 0.0f;
+        lo = (xc - x_tol) - a_left;
+        hi = (xc + x_tol) + a_right;
+      } else {
+        const float yl = y + ty * C.dzs[layer];
+        const float ctr = xc + yl * C.tana[layer];
+        lo = ctr - C.uv_half_width;
+        hi = ctr + C.uv_half_width;
+      }
     }
     const int sb = H.seg[layer * 2 + zone], se = H.seg[layer * 2 + zone + 1];
     /* a2.  With c = lower_bound(mid) the window [first, last) = [lower_bound(lo), upper_bound(hi))
      * is capped to [max(first, c - n/2), min(last, c + n/2)) iff it holds more than n = n_window hits.  Both
      * the test and the result only need first and last clipped to c -/+ (n + 1), so after one search over
-     * the segment the two edges are short searches next to c (lo <= mid <= hi puts c inside the window). */
+     * the segment the two edges are short searches next to c (lo <= mid <= hi puts c inside the window;
+     * an empty interval lo > hi, possible in the no-UT mode with a negative x_tol, gives first >= last = empty). */
     const pos_t pb = hx.pos(sb), pe = hx.pos(se);
     const float midv = (lo + hi) * 0.5f;
     const pos_t pc = lower_pos<HV>(pb, pe, midv, nsteps);
     const int c = sb + HV::diff(pc, pb);
     const int fmin = max(sb, c - reach), lmax = min(se, c + reach);
-    const pos_t pf = bound_pos<EDGE_STEPS, false, HV>(hx.pos(fmin), pc, lo);   /* first x >= lo, not below c - (n+1) */
-    const pos_t pl = bound_pos<EDGE_STEPS, true, HV>(pc, hx.pos(lmax), hi);    /* first x > hi, not above c + (n+1) */
+    const pos_t pf = bound_pos<F::EDGE_STEPS, false, HV>(hx.pos(fmin), pc, lo);   /* first x >= lo, not below c - (n+1) */
+    const pos_t pl = bound_pos<F::EDGE_STEPS, true, HV>(pc, hx.pos(lmax), hi);    /* first x > hi, not above c + (n+1) */
     int first = fmin + HV::diff(pf, hx.pos(fmin)), last = c + HV::diff(pl, pc);
     if (last - first > C.n_window) {
       first = max(first, c - halfw);
       last = min(last, c + halfw);
     }
-    A.win[(size_t)seed * NL + layer] = ((uint32_t)first << 6) | (uint32_t)(last - first);
+    if (WIDE && last < first) last = first;
+    A.win[row * NL + layer] = ((uint32_t)first << F::WB) | (uint32_t)(last - first);
     if (DEBUG) {
-      if (A.dbg.win_first) A.dbg.win_first[(size_t)seed * NL + layer] = (int32_t)(E.h0 + first);
-      if (A.dbg.win_count) A.dbg.win_count[(size_t)seed * NL + layer] = last - first;
+      if (A.dbg.win_first) A.dbg.win_first[row * NL + layer] = (int32_t)(E.h0 + first);
+      if (A.dbg.win_count) A.dbg.win_count[row * NL + layer] = last - first;
     }
   }
 }
@@ -457,7 +515,7 @@ __device__ __forceinline__ void flag_equal_neighbours(const EventArgs& A, const 
   if (threadIdx.x == 0) A.ev_dup[E.ev] = (uint32_t)dup;
 }
 
-template <bool DEBUG>
+template <bool DEBUG, bool WIDE>
 __global__ void __launch_bounds__(WIN_THREADS) lf_window_kernel(const __grid_constant__ Consts C,
                                                                 const __grid_constant__ EventArgs A) {
   CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
@@ -467,10 +525,10 @@ __global__ void __launch_bounds__(WIN_THREADS) lf_window_kernel(const __grid_con
   while (fetch_event(A, phase, E)) {
     if (E.staged) {
       flag_equal_neighbours(A, E, HitView<true>{E.skew});
-      windows_of_event<DEBUG, true>(C, A, H, E, HitView<true>{E.skew});
+      windows_of_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>{E.skew});
     } else {
       flag_equal_neighbours(A, E, HitView<false>{A.hx + E.h0});
-      windows_of_event<DEBUG, false>(C, A, H, E, HitView<false>{A.hx + E.h0});
+      windows_of_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>{A.hx + E.h0});
     }
   }
 }
@@ -612,7 +670,7 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
         const float zb = set ? C.z[7] : C.z[4], za = set ? C.z[3] : C.z[0], Kx1 = set ? C.K[1] : C.K[0];
         const float x1e = zb * t + (x0o - t * za) * Kx1;
         float dx;
-        const int k = closest_hit(hx, fb, nb, x1e, dup, dx);
+        const int k = closest_hit<false>(hx, fb, nb, x1e, dup, dx);
         const float chi2 = dx * dx;
         if (chi2 < C.T_triplet) {
           pass = true;
@@ -635,7 +693,7 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
   if (lane == 0) A.n_trip[seed] = (uint8_t)ntr;
   const bool mine = lane < ntr;
   const unsigned long long key = mine ? W.trip[lane] : 0ull;
-  if (lane < NT) A.trip_code[(size_t)seed * NT + lane] = (uint16_t)((unsigned)key & 0xFFFFu);
+  if (lane < NT) static_cast<uint16_t*>(A.trip_code)[(size_t)seed * NT + lane] = (uint16_t)((unsigned)key & 0xFFFFu);
   if (DEBUG) {
     const unsigned low = (unsigned)key;
     const int set = (low >> 15) & 1, la = set ? 3 : 0;
@@ -656,15 +714,147 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
   __syncwarp();
 }
 
+/* a3 in the wide build (windows of up to 64 hits, `sides` rows per seed).  One warp per
+ * row.  Same scheme as seed_triplets, one (layer set, block of 32 h0 hits) at a time: lanes = h0 bracket the h2
+ * interval that can pass the magnet-opening cut (binary searches over the h2 window in shared memory), a prefix
+ * scan of the bracket sizes re-maps lanes to candidate doublets, the exact fp32 predicate decides, closest h1 and
+ * chi2 cut follow in the same lane.  In the no-UT mode the assumed 1/p of PAPER.md:289 stands where q/p stood and
+ * the same-bend filter does not exist (a VELO track has no momentum or charge). */
+template <bool DEBUG, class HV>
+__device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventArgs& A, const HV& hx, uint32_t h0,
+                                                   uint32_t seed, int side, SeedScratch& W, int lane, bool dup) {
+  typedef Fmt<true> F;
+  typedef typename HV::pos_t pos_t;
+  const size_t row = (size_t)seed * C.sides + side;
+  const float x = __ldg(A.sx + seed), tx = __ldg(A.stx + seed);
+  const bool no_ut = C.mode == 1;
+  float qop = 0.0f, aq;
+  if (no_ut) {
+    const float ty = __ldg(A.sty + seed);
+    const float s2 = tx * tx + ty * ty;
+    const float sin_theta = sqrtf(s2 / (1.0f + s2));
+    aq = fminf(C.inv_p_min, sin_theta * C.inv_pt_min);
+  } else {
+    qop = __ldg(A.sqop + seed);
+    aq = fmaxf(fabsf(qop), 1e-6f);
+  }
+  const float p = 1.0f / aq;
+  const float x_mag = x + tx * C.mag_dz_seed;
+  const uint32_t winw = (lane < NL) ? A.win[row * NL + lane] : 0u;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  const bool low_p = !no_ut && (p < C.p_same_bend);
+  const float tol0 = C.mag_tol_base + C.mag_tol_inv_p * aq;
+  int tcount = 0;
+#pragma unroll 1
+  for (int set = 0; set < 2; ++set) {
+    const int la = set ? 3 : 0;
+    const uint32_t wa = __shfl_sync(FULL, winw, la), wb = __shfl_sync(FULL, winw, la + 4), wc = __shfl_sync(FULL, winw, la + 8);
+    const int fa = (int)(wa >> F::WB), na = (int)(wa & F::WMASK), fb = (int)(wb >> F::WB), nb = (int)(wb & F::WMASK);
+    const int fc = (int)(wc >> F::WB), nc = (int)(wc & F::WMASK);
+    if (na == 0 || nb == 0 || nc == 0) continue; /* warp-uniform */
+    const float inv_r = C.inv_r[set], inv_dz = C.inv_dz_ac[set], zmag_a = C.zmag_a[set];
+    const float zb = C.z[la + 4], za = C.z[la], Kx1 = C.K[set];
+    const pos_t pc0 = hx.pos(fc), pc1 = hx.pos(fc + nc);
+#pragma unroll 1
+    for (int sub = 0; sub < na; sub += 32) {
+      const bool have = sub + lane < na;
+      const float x0 = have ? hx[fa + sub + lane] : 0.0f;
+      /* a survivor has |A + t*zmag_a| < tol <= tol_max, so |t| <= (|A| + tol_max)/|zmag_a| =: tmax (see seed_triplets) */
+      const float Aoff = x0 - x_mag;
+      const float tmax = (fabsf(Aoff) + C.mag_tol_max) * C.inv_abs_zmag_a[set];
+      const float tol_sup = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * tmax) + INTERVAL_MARGIN;
+      const int jlo = HV::diff(bound_pos<F::EDGE_STEPS, false, HV>(pc0, pc1, x0 + (tol_sup - Aoff) * inv_r), pc0);
+      const int jhi = HV::diff(bound_pos<F::EDGE_STEPS, true, HV>(pc0, pc1, x0 + (-tol_sup - Aoff) * inv_r), pc0);
+      const int cnt = have ? max(jhi - jlo, 0) : 0;
+      int incl = cnt;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(FULL, incl, o);
+        if (lane >= o) incl += v;
+      }
+      const int total = __shfl_sync(FULL, incl, 31);
+      for (int base = 0; base < total; base += 32) {
+        const int tau = base + lane;
+        const bool act = tau < total;
+        int owner = 0; /* number of lanes whose inclusive count is <= tau == the h0 lane owning candidate tau */
+#pragma unroll
+        for (int st = 16; st >= 1; st >>= 1) {
+          const int v = __shfl_sync(FULL, incl, owner + st - 1);
+          if (v <= tau) owner += st;
+        }
+        owner = min(owner, 31);
+        const int before = __shfl_sync(FULL, incl, owner) - __shfl_sync(FULL, cnt, owner);
+        const int j = __shfl_sync(FULL, jlo, owner) + (tau - before); /* h2 index inside its window */
+        const float x0o = __shfl_sync(FULL, x0, owner);
+        bool pass = false;
+        unsigned long long key = 0;
+        if (act) {
+          /* the exact predicate is the definition */
+          const float x2 = hx[fc + j];
+          const float t = (x2 - x0o) * inv_dz;
+          bool ok = true;
+          if (low_p) ok = (t - tx) * qop > 0.0f; /* filter 1: same bending direction */
+          const float x_at_mag = x0o + t * zmag_a;
+          const float tol = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * fabsf(t));
+          ok = ok && (fabsf(x_at_mag - x_mag) < tol); /* filter 2: opening at the magnet centre */
+          if (ok) {
+            const float x1e = zb * t + (x0o - t * za) * Kx1;
+            float dx;
+            const int k = closest_hit<true>(hx, fb, nb, x1e, dup, dx);
+            const float chi2 = dx * dx;
+            if (chi2 < C.T_triplet) {
+              pass = true;
+              key = ((unsigned long long)__float_as_uint(chi2) << 32) |
+                    (unsigned)((set << (3 * F::IB)) | ((sub + owner) << (2 * F::IB)) | (j << F::IB) | (k - fb));
+            }
+          }
+        }
+        const unsigned m = __ballot_sync(FULL, pass);
+        if (m) {
+          if (tcount > 32) tcount = select_smallest(W, tcount, C.n_triplets, lane);
+          if (pass) W.trip[tcount + __popc(m & lt_mask)] = key;
+          tcount += __popc(m);
+          __syncwarp();
+        }
+      }
+    }
+  }
+  if (tcount > 0) tcount = select_smallest(W, tcount, C.n_triplets, lane); /* sorted in (chi2,set,h0,h2) order */
+  const int ntr = tcount;
+  const int NT = C.n_triplets;
+  if (lane == 0) A.n_trip[row] = (uint8_t)ntr;
+  const bool mine = lane < ntr;
+  const unsigned long long key = mine ? W.trip[lane] : 0ull;
+  if (lane < NT) static_cast<uint32_t*>(A.trip_code)[row * NT + lane] = (unsigned)key;
+  if (DEBUG) {
+    const unsigned low = (unsigned)key;
+    const int set = (low >> (3 * F::IB)) & 1, la = set ? 3 : 0;
+    const int fa = (int)(__shfl_sync(FULL, winw, la) >> F::WB), fb = (int)(__shfl_sync(FULL, winw, la + 4) >> F::WB);
+    const int fc = (int)(__shfl_sync(FULL, winw, la + 8) >> F::WB);
+    if (lane == 0 && A.dbg.n_triplets) A.dbg.n_triplets[row] = ntr;
+    if (lane < NT) {
+      const size_t o = row * NT + lane;
+      if (A.dbg.trip_set) A.dbg.trip_set[o] = mine ? set : -1;
+      if (A.dbg.trip_chi2) A.dbg.trip_chi2[o] = mine ? __uint_as_float((unsigned)(key >> 32)) : -1.0f;
+      if (A.dbg.trip_hits) {
+        A.dbg.trip_hits[o * 3 + 0] = mine ? (int32_t)(h0 + fa + ((low >> (2 * F::IB)) & F::IMASK)) : -1;
+        A.dbg.trip_hits[o * 3 + 1] = mine ? (int32_t)(h0 + fb + (low & F::IMASK)) : -1;
+        A.dbg.trip_hits[o * 3 + 2] = mine ? (int32_t)(h0 + fc + ((low >> F::IB) & F::IMASK)) : -1;
+      }
+    }
+  }
+  __syncwarp();
+}
+
 struct __align__(16) SeedTables {
   int next_seed;
   int pad[3];
   SeedScratch ws[SEED_WARPS];
 };
 
-template <bool DEBUG>
-__global__ void __launch_bounds__(SEED_THREADS, 5) lf_seed_kernel(const __grid_constant__ Consts C,
-                                                               const __grid_constant__ EventArgs A) {
+template <bool DEBUG, bool WIDE>
+__global__ void __launch_bounds__(SEED_THREADS, WIDE ? 4 : 5) lf_seed_kernel(const __grid_constant__ Consts C,
+                                                                           const __grid_constant__ EventArgs A) {
   CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
   SeedTables& T = *reinterpret_cast<SeedTables*>(lf_smem + HDR_BYTES + (size_t)A.stage_cap * sizeof(float));
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -676,17 +866,26 @@ __global__ void __launch_bounds__(SEED_THREADS, 5) lf_seed_kernel(const __grid_c
   EventCtx E;
   while (fetch_event(A, phase, E)) {
     const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
+    const int sides = WIDE ? C.sides : 1;
+    const int n_rows = (int)(s1 - s0) * sides;
     SeedScratch& W = T.ws[warp];
     const bool dup = H.dup != 0;
-    for (;;) { /* the warps of the CTA share the event's seeds, two per ticket */
+    for (;;) { /* the warps of the CTA share the event's rows, two per ticket */
       int k = 0;
       if (lane == 0) k = atomicAdd(&T.next_seed, 2);
       k = __shfl_sync(FULL, k, 0);
-      if (s0 + (uint32_t)k >= s1) break;
-      const int kend = min(k + 2, (int)(s1 - s0));
+      if (k >= n_rows) break;
+      const int kend = min(k + 2, n_rows);
       for (; k < kend; ++k) {
-        if (E.staged) seed_triplets<DEBUG>(C, A, HitView<true>{E.skew}, E.h0, s0 + (uint32_t)k, W, lane, dup);
-        else seed_triplets<DEBUG>(C, A, HitView<false>{A.hx + E.h0}, E.h0, s0 + (uint32_t)k, W, lane, dup);
+        if (WIDE) {
+          const uint32_t seed = s0 + (uint32_t)(k / sides);
+          const int side = k - (k / sides) * sides;
+          if (E.staged) seed_triplets_wide<DEBUG>(C, A, HitView<true>{E.skew}, E.h0, seed, side, W, lane, dup);
+          else seed_triplets_wide<DEBUG>(C, A, HitView<false>{A.hx + E.h0}, E.h0, seed, side, W, lane, dup);
+        } else {
+          if (E.staged) seed_triplets<DEBUG>(C, A, HitView<true>{E.skew}, E.h0, s0 + (uint32_t)k, W, lane, dup);
+          else seed_triplets<DEBUG>(C, A, HitView<false>{A.hx + E.h0}, E.h0, s0 + (uint32_t)k, W, lane, dup);
+        }
       }
     }
     __syncthreads();
@@ -707,13 +906,14 @@ struct CandHits {
 __device__ __forceinline__ unsigned code_of(const CandHits& h, int l) { return (h.w[l >> 2] >> (8 * (l & 3))) & 0xFFu; }
 
 /* Eq. (4) parameters: exact parabola through the three triplet hits. */
-template <class HV>
+template <bool WIDE, class HV>
 __device__ __forceinline__ void triplet_parabola(const Consts& C, const HV& hx, const uint32_t* winw, unsigned code,
                                                  float& a0, float& t0, float& c0) {
-  const int set = (code >> 15) & 1, la = set ? 3 : 0;
-  const float x0 = hx[(int)(winw[la] >> 6) + (int)((code >> 10) & 31)];
-  const float x1 = hx[(int)(winw[la + 4] >> 6) + (int)(code & 31)];
-  const float x2 = hx[(int)(winw[la + 8] >> 6) + (int)((code >> 5) & 31)];
+  typedef Fmt<WIDE> F;
+  const int set = (code >> (3 * F::IB)) & 1, la = set ? 3 : 0;
+  const float x0 = hx[(int)(winw[la] >> F::WB) + (int)((code >> (2 * F::IB)) & F::IMASK)];
+  const float x1 = hx[(int)(winw[la + 4] >> F::WB) + (int)(code & F::IMASK)];
+  const float x2 = hx[(int)(winw[la + 8] >> F::WB) + (int)((code >> F::IB) & F::IMASK)];
   const float X10 = x1 - x0, X20 = x2 - x0;
   const float D10 = set ? C.D10[1] : C.D10[0], D20 = set ? C.D20[1] : C.D20[0];
   const float W10 = set ? C.W10[1] : C.W10[0];
@@ -724,17 +924,18 @@ __device__ __forceinline__ void triplet_parabola(const Consts& C, const HV& hx, 
 
 /* a4/a5: extension of one triplet to the 9 other layers + hit-count rule.
  * `geo` is the shared-memory copy of the per-layer constants: d, w, dzs, tana (12 floats each). */
-template <class HV>
+template <bool WIDE, class HV>
 __device__ __noinline__ CandHits extend_candidate(const Consts& C, const HV& hx, const uint32_t* winw, const float* geo,
                                                   float y, float tx, float ty, unsigned code, bool dup) {
-  const int set = (code >> 15) & 1;
+  typedef Fmt<WIDE> F;
+  const int set = (code >> (3 * F::IB)) & 1;
   float a0, t0, c0;
-  triplet_parabola(C, hx, winw, code, a0, t0, c0);
+  triplet_parabola<WIDE>(C, hx, winw, code, a0, t0, c0);
   const float T_uv = fmaxf(C.T_uv_min, C.T_uv_slope * (fabsf(tx) + fabsf(ty)));
   CandHits h;
   /* per station: the triplet's own hit (byte 0 for set 0, byte 3 for set 1) and the three other layers,
    * searched in lockstep */
-  const unsigned trip[3] = {(code >> 10) & 31u, code & 31u, (code >> 5) & 31u};
+  const unsigned trip[3] = {(code >> (2 * F::IB)) & F::IMASK, code & F::IMASK, (code >> F::IB) & F::IMASK};
   const unsigned tsh = set ? 24u : 0u, sh0 = set ? 0u : 8u;
   int n = 3, n_uv = 0;
   unsigned st_mask = 0;
@@ -758,7 +959,7 @@ __device__ __noinline__ CandHits extend_candidate(const Consts& C, const HV& hx,
       pred[0] = pred[0] + (y + ty * geo[2 * NL + l0]) * geo[3 * NL + l0];
       pred[1] = pred[1] + (y + ty * geo[2 * NL + l0 + 1]) * geo[3 * NL + l0 + 1];
     }
-    closest_group<3>(hx, ww, pred, dup, krel, dist);
+    closest_group<3, WIDE>(hx, ww, pred, dup, krel, dist);
     unsigned w = (trip[st] << tsh) | (0x00FFFFFFu << sh0);
 #pragma unroll
     for (int g = 0; g < 3; ++g) {
@@ -804,35 +1005,41 @@ __host__ __device__ inline size_t ext_tables_bytes(int nt) {
          (((size_t)FIT_CHUNK * nt * 2 + 15) & ~size_t(15)) + 16 * 4;
 }
 
-template <bool DEBUG, bool STAGED>
+template <bool DEBUG, bool WIDE, bool STAGED>
 __device__ __forceinline__ void extend_event(const Consts& C, const EventArgs& A, CtaHeader& H, const EventCtx& E,
                                              const HitView<STAGED>& hx, const ExtTables& T) {
+  typedef Fmt<WIDE> F;
+  typedef typename F::code_t code_t;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
-  const int ns = (int)(s1 - s0);
+  const int sides = WIDE ? C.sides : 1;
+  const int nr = (int)(s1 - s0) * sides;        /* rows (followed tracks) of the event */
+  const size_t row0 = (size_t)s0 * sides;       /* first row of the event */
   const int NT = C.n_triplets;
   const bool dup = H.dup != 0;
-  uint4* rec = A.acc_rec + (size_t)s0 * NT;
+  const code_t* trip_code = static_cast<const code_t*>(A.trip_code);
+  uint4* rec = A.acc_rec + row0 * NT;
   uint32_t ev_acc = 0;
   int parity = 0;
-  for (int cb = 0; cb < ns; cb += FIT_CHUNK) {
-    const int cn = min(FIT_CHUNK, ns - cb);
-    const uint32_t sbase = s0 + (uint32_t)cb;
+  for (int cb = 0; cb < nr; cb += FIT_CHUNK) { /* FIT_CHUNK is even: a chunk starts on a seed boundary */
+    const int cn = min(FIT_CHUNK, nr - cb);
+    const size_t rbase = row0 + (size_t)cb;
     /* ---- stage the chunk's windows, seed parameters and candidate counts */
-    for (int i = tid; i < cn * NL; i += FIT_THREADS) T.win[i] = A.win[(size_t)sbase * NL + i];
+    for (int i = tid; i < cn * NL; i += FIT_THREADS) T.win[i] = A.win[rbase * NL + i];
     int my_n = 0;
     if (tid < cn) {
-      const uint32_t seed = sbase + (uint32_t)tid;
+      const size_t row = rbase + (size_t)tid;
+      const uint32_t seed = WIDE ? (uint32_t)(row / (size_t)sides) : (uint32_t)row;
       T.sp[tid * 4 + 0] = __ldg(A.sy + seed);
       T.sp[tid * 4 + 1] = __ldg(A.stx + seed);
       T.sp[tid * 4 + 2] = __ldg(A.sty + seed);
-      my_n = (int)A.n_trip[seed];
+      my_n = (int)A.n_trip[row];
       A.ws_nh[seed] = 0; /* set by the fit kernel if the seed gets a track */
       if (DEBUG) {
         for (int k = my_n; k < NT; ++k) {
-          if (A.dbg.cand_quality) A.dbg.cand_quality[(size_t)seed * NT + k] = -1.0f;
+          if (A.dbg.cand_quality) A.dbg.cand_quality[row * NT + k] = -1.0f;
           if (A.dbg.cand_hits)
-            for (int l = 0; l < NL; ++l) A.dbg.cand_hits[((size_t)seed * NT + k) * NL + l] = -1;
+            for (int l = 0; l < NL; ++l) A.dbg.cand_hits[(row * NT + k) * NL + l] = -1;
         }
       }
     }
@@ -855,7 +1062,7 @@ __device__ __forceinline__ void extend_event(const Consts& C, const EventArgs& A
     const int excl = woff + incl - my_n;
     if (tid < cn) {
       T.pref[tid] = excl;
-      for (int k = 0; k < my_n; ++k) T.item[excl + k] = (uint16_t)((tid << 4) | k);
+      for (int k = 0; k < my_n; ++k) T.item[excl + k] = (uint16_t)((tid << F::KB) | k);
     }
     __syncthreads();
     /* ---- one thread per candidate; the accepted ones are appended in candidate order */
@@ -866,19 +1073,22 @@ __device__ __forceinline__ void extend_event(const Consts& C, const EventArgs& A
       unsigned tag = 0;
       if (it < total) {
         const unsigned im = T.item[it];
-        const int sl = (int)(im >> 4), k = (int)(im & 15u);
-        const uint32_t seed = sbase + (uint32_t)sl;
-        const unsigned code = A.trip_code[(size_t)seed * NT + k];
-        h = extend_candidate(C, hx, T.win + sl * NL, T.geo, T.sp[sl * 4 + 0], T.sp[sl * 4 + 1], T.sp[sl * 4 + 2], code, dup);
+        const int rl = (int)(im >> F::KB), k = (int)(im & ((1u << F::KB) - 1u));
+        const size_t row = rbase + (size_t)rl;
+        const unsigned code = trip_code[row * NT + k];
+        h = extend_candidate<WIDE>(C, hx, T.win + rl * NL, T.geo, T.sp[rl * 4 + 0], T.sp[rl * 4 + 1], T.sp[rl * 4 + 2], code, dup);
         enough = h.enough;
-        tag = (unsigned)(cb + sl) | ((unsigned)k << 28); /* seed inside the event, candidate index */
+        /* seed inside the event, (side,) candidate index */
+        const int re = cb + rl;
+        tag = WIDE ? ((unsigned)(re / sides) | ((unsigned)(re - (re / sides) * sides) << F::SIE_BITS) | ((unsigned)k << F::K_SHIFT))
+                   : ((unsigned)re | ((unsigned)k << F::K_SHIFT));
         if (DEBUG) {
           if (A.dbg.cand_hits)
             for (int l = 0; l < NL; ++l) {
               const unsigned cd = code_of(h, l);
-              A.dbg.cand_hits[((size_t)seed * NT + k) * NL + l] = (cd != 0xFFu) ? (int32_t)(E.h0 + (T.win[sl * NL + l] >> 6) + cd) : -1;
+              A.dbg.cand_hits[(row * NT + k) * NL + l] = (cd != 0xFFu) ? (int32_t)(E.h0 + (T.win[rl * NL + l] >> F::WB) + cd) : -1;
             }
-          if (A.dbg.cand_quality && !enough) A.dbg.cand_quality[(size_t)seed * NT + k] = -1.0f;
+          if (A.dbg.cand_quality && !enough) A.dbg.cand_quality[row * NT + k] = -1.0f;
         }
       }
       const unsigned m = __ballot_sync(FULL, enough);
@@ -901,7 +1111,7 @@ __device__ __forceinline__ void extend_event(const Consts& C, const EventArgs& A
   if (tid == 0) A.ev_acc[E.ev] = ev_acc;
 }
 
-template <bool DEBUG>
+template <bool DEBUG, bool WIDE>
 __global__ void __launch_bounds__(FIT_THREADS, 4) lf_extend_kernel(const __grid_constant__ Consts C,
                                                                    const __grid_constant__ EventArgs A) {
   CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
@@ -929,8 +1139,8 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_extend_kernel(const __grid_
   uint32_t phase = 0;
   EventCtx E;
   while (fetch_event(A, phase, E)) {
-    if (E.staged) extend_event<DEBUG, true>(C, A, H, E, HitView<true>{E.skew}, T);
-    else extend_event<DEBUG, false>(C, A, H, E, HitView<false>{A.hx + E.h0}, T);
+    if (E.staged) extend_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>{E.skew}, T);
+    else extend_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>{A.hx + E.h0}, T);
   }
 }
 
@@ -946,16 +1156,18 @@ struct FitTables {
 };
 constexpr size_t FIT_TABLES_BYTES = 2 * FIT_THREADS * 8 + 16 + 16 * 4;
 
-template <bool DEBUG, bool STAGED>
+template <bool DEBUG, bool WIDE, bool STAGED>
 __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, CtaHeader& H, const EventCtx& E,
                                           const HitView<STAGED>& hx, const FitTables& T) {
+  typedef Fmt<WIDE> F;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
   const int ns = (int)(s1 - s0);
+  const int sides = WIDE ? C.sides : 1;
   const int NT = C.n_triplets;
-  const uint4* rec = A.acc_rec + (size_t)s0 * NT;
+  const uint4* rec = A.acc_rec + (size_t)s0 * sides * NT;
   const int n_acc = (int)A.ev_acc[E.ev];
-  const unsigned SIE = 0x0FFFFFFFu;
+  const unsigned SIE = F::SIE;
   int parity = 0;
   for (int b = 0; b < n_acc; parity ^= 1) {
     unsigned long long* best = T.best + parity * FIT_THREADS;
@@ -965,7 +1177,9 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
     const bool have = t < n_acc;
     const uint4 r = have ? __ldg(rec + t) : make_uint4(0, 0, 0, 0xFFFFFFFFu);
     const unsigned sie = r.w & SIE;
-    const int k = (int)(r.w >> 28);
+    const int k = (int)(r.w >> F::K_SHIFT);
+    /* wide: the records of a seed's sides are adjacent (side 0 first) and compete for the seed's track */
+    const int side = WIDE ? (int)((r.w >> F::SIE_BITS) & 1u) : 0;
     unsigned prev_sie = __shfl_up_sync(FULL, sie, 1);
     if (lane == 0) prev_sie = (tid > 0 && have) ? (__ldg(&rec[t - 1].w) & SIE) : 0xFFFFFFFEu;
     /* a seed whose records continue in the next pass is left to that pass (a seed has < FIT_THREADS records) */
@@ -987,27 +1201,28 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
     int n = 0;
     unsigned long long key = ~0ull;
     if (mine) {
-      const uint4* wp = reinterpret_cast<const uint4*>(A.win + (size_t)seed * NL);
+      const size_t row = (size_t)seed * sides + side;
+      const uint4* wp = reinterpret_cast<const uint4*>(A.win + row * NL);
       const uint4 w0 = __ldg(wp), w1 = __ldg(wp + 1), w2 = __ldg(wp + 2);
       wf[0] = w0.x; wf[1] = w0.y; wf[2] = w0.z; wf[3] = w0.w; wf[4] = w1.x; wf[5] = w1.y; wf[6] = w1.z; wf[7] = w1.w;
       wf[8] = w2.x; wf[9] = w2.y; wf[10] = w2.z; wf[11] = w2.w;
       y = __ldg(A.sy + seed);
       tx = __ldg(A.stx + seed);
       ty = __ldg(A.sty + seed);
-      const unsigned code = A.trip_code[(size_t)seed * NT + k];
+      const unsigned code = static_cast<const typename F::code_t*>(A.trip_code)[row * NT + k];
       CandHits h;
       h.w[0] = r.x; h.w[1] = r.y; h.w[2] = r.z;
       unsigned mask = 0;
 #pragma unroll
       for (int l = 0; l < NL; ++l) {
         const unsigned cd = code_of(h, l);
-        wf[l] = (wf[l] >> 6) + cd; /* event-relative hit index (meaningless if the layer has no hit) */
+        wf[l] = (wf[l] >> F::WB) + cd; /* event-relative hit index (meaningless if the layer has no hit) */
         mask |= (cd != 0xFFu) ? (1u << l) : 0u;
       }
       n = __popc(mask);
       const int n_uv = __popc(mask & 0x666u);
       {
-        const int set = (code >> 15) & 1;
+        const int set = (code >> (3 * F::IB)) & 1;
         const float x0 = hx[(int)(set ? wf[3] : wf[0])], x1 = hx[(int)(set ? wf[7] : wf[4])], x2 = hx[(int)(set ? wf[11] : wf[8])];
         const float X10 = x1 - x0, X20 = x2 - x0;
         const float D10 = set ? C.D10[1] : C.D10[0], D20 = set ? C.D20[1] : C.D20[0];
@@ -1072,10 +1287,10 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
       const int ci = min(3, max(0, n - 9));
       const float Cn = (ci == 0) ? C.C_nhits[0] : (ci == 1 ? C.C_nhits[1] : (ci == 2 ? C.C_nhits[2] : C.C_nhits[3]));
       Q = (Qx / (float)(n - 3) + Qy / (float)(n_uv - 2)) * Cn; /* Eq. (6) */
-      if (DEBUG && A.dbg.cand_quality) A.dbg.cand_quality[(size_t)seed * NT + k] = ty_ok ? Q : -2.0f;
-      /* accepted if Q < T_Q (and the t_y cut holds); lowest Q wins, ties -> lower k */
+      if (DEBUG && A.dbg.cand_quality) A.dbg.cand_quality[row * NT + k] = ty_ok ? Q : -2.0f;
+      /* accepted if Q < T_Q (and the t_y cut holds); lowest Q wins, ties -> lower (side, k) */
       if (ty_ok && (Q < C.T_Q)) {
-        key = ((unsigned long long)__float_as_uint(Q) << 32) | (unsigned)k;
+        key = ((unsigned long long)__float_as_uint(Q) << 32) | (unsigned)((side << F::KB) | k);
         atomicMin(best + slot, key);
       }
 #pragma unroll
@@ -1128,7 +1343,7 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
   if (tid == 0) A.ev_count[E.ev] = (uint32_t)ev_tracks;
 }
 
-template <bool DEBUG>
+template <bool DEBUG, bool WIDE>
 __global__ void __launch_bounds__(FIT_THREADS, 4) lf_fit_kernel(const __grid_constant__ Consts C,
                                                                 const __grid_constant__ EventArgs A) {
   CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
@@ -1144,8 +1359,8 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_fit_kernel(const __grid_con
   uint32_t phase = 0;
   EventCtx E;
   while (fetch_event(A, phase, E)) {
-    if (E.staged) fit_event<DEBUG, true>(C, A, H, E, HitView<true>{E.skew}, T);
-    else fit_event<DEBUG, false>(C, A, H, E, HitView<false>{A.hx + E.h0}, T);
+    if (E.staged) fit_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>{E.skew}, T);
+    else fit_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>{A.hx + E.h0}, T);
   }
 }
 

@@ -34,7 +34,7 @@ def test_struct_sizes_match_binding(lib):
     from paper_2402_14670_b200 import binding
     for i, st in enumerate(binding._STRUCTS):
         assert lib.lf_sizeof(i) == ctypes.sizeof(st)
-    assert lib.lf_sizeof(99) == 0 and lib.lf_abi_version() == 2
+    assert lib.lf_sizeof(99) == 0 and lib.lf_abi_version() == 3
 
 
 def test_argument_validation_needs_no_gpu(lib, geometry, params):
@@ -43,11 +43,17 @@ def test_argument_validation_needs_no_gpu(lib, geometry, params):
     h = ctypes.c_void_p()
     assert lib.lf_create(None, None, 1, 1, 1, ctypes.byref(h)) == bd.LF_ERR_INVALID_ARG
     g = bd._fill(bd.lf_geometry(), geometry)
-    for bad_params, why in ((dict(params, n_window=64), "n_window"), (dict(params, n_triplets=0), "n_triplets"),
+    for bad_params, why in ((dict(params, n_window=65), "n_window"), (dict(params, n_triplets=0), "n_triplets"),
+                            (dict(params, n_triplets=33), "n_triplets"), (dict(params, mode=2), "mode"),
+                            (dict(params, mode=1, velo_pt_min=0.0), "velo_pt_min"),
                             (dict(params, min_hits=2), "min_hits"), (dict(params, T_x=0.0), "positive")):
         p = bd._fill(bd.lf_params(), bad_params)
         assert lib.lf_create(ctypes.byref(g), ctypes.byref(p), 1, 1, 1, ctypes.byref(h)) == bd.LF_ERR_INVALID_ARG
         assert why in lib.lf_last_error(None).decode()
+    # fp16 hit storage exists for the narrow with-UT kernels only
+    for unsupported in (dict(params, hit_storage=1, mode=1), dict(params, hit_storage=1, n_window=64)):
+        p = bd._fill(bd.lf_params(), unsupported)
+        assert lib.lf_create(ctypes.byref(g), ctypes.byref(p), 1, 1, 1, ctypes.byref(h)) == bd.LF_ERR_UNSUPPORTED
     p = bd._fill(bd.lf_params(), params)
     for bad_geo in (dict(geometry, n_layers=8), dict(geometry, polarity=0),
                     dict(geometry, tan_alpha=[0.0] * 12), dict(geometry, z=list(reversed(geometry["z"])))):
