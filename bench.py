@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """Benchmark of the Looking Forward hot path on B200 (contract: see DESIGN.md "Measurement").
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--events E]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--events E] [--tuning with-ut|no-ut]
 
 A "step" is one pass of the whole hot path (a1..a7: one lf_run = window, seed, extend, fit, scan, compact kernels)
 over one batch of synthetic events.  Default workload: BASELINE.json configs[3] (20,000 events at
@@ -116,18 +116,27 @@ def algorithmic_bytes(batch, n_tracks: int) -> int:
                + 80 * n_tracks + 4 * (batch.n_events + 1) + 4)
 
 
-def kernel_bytes(batch, n_tracks: int, n_triplets: int, n_acc: int = 0) -> dict:
+def kernel_bytes(batch, n_tracks: int, n_triplets: int, n_acc: int = 0, sides: int = 1, wide: bool = False) -> dict:
     """Algorithmic HBM bytes per launch of each event kernel: every kernel stages the
-    event's hits once and reads/writes its own per-seed tables once."""
+    event's hits once and reads/writes its own tables once.  Tables are per followed track (row): one per seed, or
+    one per (seed, window side) in the no-UT tuning; the wide kernels store 4-byte triplet codes."""
     H, S, E = batch.n_hits, batch.n_seeds, batch.n_events
+    R, cb = S * sides, (4 if wide else 2)
     common = 4 * H + batch.seg_offsets.nbytes + batch.seed_offsets.nbytes
-    trip = (2 * n_triplets + 1) * S
+    trip = (cb * n_triplets + 1) * R
     acc = 16 * n_acc  # one 16-byte record per candidate that passed the hit-count rule
-    return {"window": common + 20 * S + 48 * S + 4 * E,
-            "seed": common + 12 * S + 48 * S + trip,
-            "extend": common + 12 * S + 48 * S + trip + acc + 4 * S + 4 * E,
-            "fit": common + 4 * E + acc + n_acc * (48 + 12 + 2) + 80 * n_tracks + 16 * S,
+    return {"window": common + (16 if sides == 2 else 20) * S + 48 * R + 4 * E,
+            "seed": common + 12 * S + 48 * R + trip,
+            "extend": common + 12 * S + 48 * R + trip + acc + 4 * S + 4 * E,
+            "fit": common + 4 * E + acc + n_acc * (48 + 12 + cb) + 80 * n_tracks + 16 * S,
             "compact": 92 * S + 80 * n_tracks + 4 * E}
+
+
+def tuning_params(args, datagen, cfg):
+    """--tuning with-ut: Table 3 "Forward" column (BASELINE.json configs); no-ut: section VI.E."""
+    if args.tuning == "no-ut":
+        return datagen.no_ut_params()
+    return dict(datagen.default_params(), hit_storage=cfg.hit_storage)
 
 
 def oracle_rate(batch, threads: int, geometry, params):
@@ -145,7 +154,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     cfg = datagen.CONFIGS[args.config]
-    G, P = datagen.toy_geometry(), datagen.default_params()
+    G, P = datagen.toy_geometry(), tuning_params(args, datagen, cfg)
     cores = os.cpu_count() or 1
     probe = datagen.generate(cfg, n_events=min(200, args.events or cfg.n_events))
     rate, _, _ = oracle_rate(probe, cores, G, P)
@@ -164,7 +173,7 @@ def run_reference(args):
         "impl": "reference", "metric": "events_per_s", "value": value, "unit": "events/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"{cfg.name}: Run-3-like occupancy, fp32 (bounded sample)", "events_per_step": n_sample,
+        "config": {"workload": f"{cfg.name}: Run-3-like occupancy, fp32, {args.tuning} tuning (bounded sample)", "events_per_step": n_sample,
                    "seeds_per_step": batch.n_seeds, "hits_per_step": batch.n_hits},
         "seeds_per_s": batch.n_seeds * args.steps / dt,
         "cpu_baseline": {"value": value, "unit": "events/s", "cores": cores, "kind": "oracle", "sample": sample},
@@ -191,7 +200,9 @@ def run_ours(args):
     if world > 1:  # weak scaling: every rank gets its own batch of the same recipe
         cfg = datagen.with_overrides(cfg, seed=cfg.seed + 7919 * rank)
     G = datagen.toy_geometry()
-    P = dict(datagen.default_params(), hit_storage=cfg.hit_storage)
+    P = tuning_params(args, datagen, cfg)
+    no_ut = int(P["mode"]) == 1
+    wide = no_ut or int(P["n_window"]) > 32 or int(P["n_triplets"]) > 16
     t_gen = time.perf_counter()
     batch = datagen.generate(cfg, n_events=args.events)
     t_gen = time.perf_counter() - t_gen
@@ -261,7 +272,7 @@ def run_ours(args):
     # ALU / warp-instruction issue rate, so the top-level object is the "alu" roofline; the HBM
     # roofline BASELINE.json's metric asks for sits beside it under "hbm" (same keys, algorithmic bytes).
     peak, peak_src = measured_peaks()
-    kb = kernel_bytes(batch, n_tracks, int(P["n_triplets"]), n_acc)
+    kb = kernel_bytes(batch, n_tracks, int(P["n_triplets"]), n_acc, sides=2 if no_ut else 1, wide=wide)
     dom = max(binding.EVENT_KERNELS, key=lambda k: ktimes[k])
     achieved = kb[dom] / (ktimes[dom] * 1e-3) / 1e9
     path_bytes = algorithmic_bytes(batch, n_tracks)
@@ -273,7 +284,7 @@ def run_ours(args):
                           "frac_of_nominal_8TBs": path_gbs / NOMINAL_HBM_GBS},
            "note": "the path is not HBM-bound; this fraction is reported because BASELINE.json's metric asks for it"}
     roofline = hbm
-    traffic_file = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.txt")
+    traffic_file = os.path.join(ROOT, "profiles", "dominant_kernel_traffic_noUT.txt" if no_ut else "dominant_kernel_traffic.txt")
     if os.path.exists(traffic_file):
         try:
             tr = json.load(open(traffic_file))
@@ -323,7 +334,9 @@ def run_ours(args):
         "metric": "events_per_s", "value": value, "unit": "events/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"{cfg.name}: {batch.n_events} events per GPU, Run-3-like occupancy, fp32, one lf_run on one stream",
+        "config": {"workload": f"{cfg.name}: {batch.n_events} events per GPU, Run-3-like occupancy, fp32, one lf_run on one stream"
+                               + (", no-UT tuning (PAPER.md:285-325)" if no_ut else ""),
+                   "tuning": args.tuning,
                    "events_per_gpu": batch.n_events, "seeds_per_gpu": batch.n_seeds, "hits_per_gpu": batch.n_hits,
                    "tracks_per_step_per_gpu": n_tracks, "accepted_candidates_per_step": n_acc, "events_with_equal_hits": n_dup_events,
                    "l2": f"no flush: inputs ({in_bytes / 1e6:.0f} MB) + outputs exceed the 126 MB L2",
@@ -356,6 +369,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--tuning", choices=["with-ut", "no-ut"], default="with-ut",
+                    help="with-ut: BASELINE.json's headline (default); no-ut: the no-UT tuning of PAPER.md:285-325 on the same events")
     ap.add_argument("--events", type=int, default=None, help="override the number of events (default: the config's)")
     ap.add_argument("--cpu-events", type=int, default=6000, help="events of the single-thread oracle sample")
     ap.add_argument("--no-e2e", action="store_true")

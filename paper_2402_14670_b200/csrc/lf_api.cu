@@ -377,7 +377,7 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   }
   const size_t stage_bytes = (size_t)lf::HDR_BYTES + (size_t)h->stage_cap * sizeof(float);
   h->smem_bytes[0] = (int)stage_bytes;
-  h->smem_bytes[1] = (int)(stage_bytes + sizeof(lf::SeedTables));
+  h->smem_bytes[1] = (int)(stage_bytes + (h->wide ? sizeof(lf::SeedTables<true>) : sizeof(lf::SeedTables<false>)));
   h->smem_bytes[2] = (int)(stage_bytes + lf::ext_tables_bytes(params->n_triplets));
   h->smem_bytes[3] = (int)(stage_bytes + lf::FIT_TABLES_BYTES);
   const void* kern_n[4][2] = {{(const void*)lf::lf_window_kernel<false, false>, (const void*)lf::lf_window_kernel<true, false>},

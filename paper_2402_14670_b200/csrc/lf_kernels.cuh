@@ -715,14 +715,24 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
 }
 
 /* a3 in the wide build (windows of up to 64 hits, `sides` rows per seed).  One warp per
- * row.  Same scheme as seed_triplets, one (layer set, block of 32 h0 hits) at a time: lanes = h0 bracket the h2
- * interval that can pass the magnet-opening cut (binary searches over the h2 window in shared memory), a prefix
- * scan of the bracket sizes re-maps lanes to candidate doublets, the exact fp32 predicate decides, closest h1 and
- * chi2 cut follow in the same lane.  In the no-UT mode the assumed 1/p of PAPER.md:289 stands where q/p stood and
- * the same-bend filter does not exist (a VELO track has no momentum or charge). */
+ * row.  Same scheme as seed_triplets over four groups of 32 h0 hits (layer set x half of the h0 window): lanes =
+ * h0 bracket the h2 interval that can pass the magnet-opening cut (binary searches over the h2 window in shared
+ * memory) and leave (running candidate count, bracket start, x0) in the warp's scratch; then ONE dense pass maps
+ * lanes to candidate doublets (binary search of the candidate number in the 128 running counts), where the exact
+ * fp32 predicate decides and closest h1 / chi2 cut follow in the same lane.  In the no-UT mode the assumed 1/p
+ * of PAPER.md:289 stands where q/p stood and the same-bend filter does not exist (a VELO track has no momentum
+ * or charge). */
+struct __align__(16) SeedScratchWide {
+  unsigned long long trip[TRIP_BUF];
+  uint32_t incl[128]; /* entry e = set*64 + h0: candidates of entries 0..e */
+  uint32_t jx[128];   /* first h2 index of the bracket | candidates before the entry << 8 */
+  float x0[128];
+};
+__device__ __forceinline__ SeedScratch& trip_part(SeedScratchWide& W) { return *reinterpret_cast<SeedScratch*>(W.trip); }
+
 template <bool DEBUG, class HV>
 __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventArgs& A, const HV& hx, uint32_t h0,
-                                                   uint32_t seed, int side, SeedScratch& W, int lane, bool dup) {
+                                                   uint32_t seed, int side, SeedScratchWide& W, int lane, bool dup) {
   typedef Fmt<true> F;
   typedef typename HV::pos_t pos_t;
   const size_t row = (size_t)seed * C.sides + side;
@@ -744,19 +754,27 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
   const unsigned lt_mask = (1u << lane) - 1u;
   const bool low_p = !no_ut && (p < C.p_same_bend);
   const float tol0 = C.mag_tol_base + C.mag_tol_inv_p * aq;
-  int tcount = 0;
-#pragma unroll 1
+  /* ---- brackets: four groups of 32 h0 hits */
+  int fbs[2], nbs[2], fcs[2];
+  int total = 0; /* warp-uniform running number of candidate doublets */
+#pragma unroll
   for (int set = 0; set < 2; ++set) {
     const int la = set ? 3 : 0;
     const uint32_t wa = __shfl_sync(FULL, winw, la), wb = __shfl_sync(FULL, winw, la + 4), wc = __shfl_sync(FULL, winw, la + 8);
-    const int fa = (int)(wa >> F::WB), na = (int)(wa & F::WMASK), fb = (int)(wb >> F::WB), nb = (int)(wb & F::WMASK);
-    const int fc = (int)(wc >> F::WB), nc = (int)(wc & F::WMASK);
-    if (na == 0 || nb == 0 || nc == 0) continue; /* warp-uniform */
-    const float inv_r = C.inv_r[set], inv_dz = C.inv_dz_ac[set], zmag_a = C.zmag_a[set];
-    const float zb = C.z[la + 4], za = C.z[la], Kx1 = C.K[set];
-    const pos_t pc0 = hx.pos(fc), pc1 = hx.pos(fc + nc);
-#pragma unroll 1
-    for (int sub = 0; sub < na; sub += 32) {
+    const int fa = (int)(wa >> F::WB), na = (int)(wa & F::WMASK), nc = (int)(wc & F::WMASK);
+    fbs[set] = (int)(wb >> F::WB);
+    nbs[set] = (int)(wb & F::WMASK);
+    fcs[set] = (int)(wc >> F::WB);
+    const bool set_on = na != 0 && nbs[set] != 0 && nc != 0; /* warp-uniform */
+    const float inv_r = C.inv_r[set];
+    const pos_t pc0 = hx.pos(fcs[set]), pc1 = hx.pos(fcs[set] + nc);
+#pragma unroll
+    for (int sub = 0; sub < 64; sub += 32) {
+      const int e = set * 64 + sub + lane;
+      if (!set_on || sub >= na) { /* warp-uniform: no candidates from this group */
+        W.incl[e] = (uint32_t)total;
+        continue;
+      }
       const bool have = sub + lane < na;
       const float x0 = have ? hx[fa + sub + lane] : 0.0f;
       /* a survivor has |A + t*zmag_a| < tol <= tol_max, so |t| <= (|A| + tol_max)/|zmag_a| =: tmax (see seed_triplets) */
@@ -772,65 +790,75 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
         const int v = __shfl_up_sync(FULL, incl, o);
         if (lane >= o) incl += v;
       }
-      const int total = __shfl_sync(FULL, incl, 31);
-      for (int base = 0; base < total; base += 32) {
-        const int tau = base + lane;
-        const bool act = tau < total;
-        int owner = 0; /* number of lanes whose inclusive count is <= tau == the h0 lane owning candidate tau */
+      incl += total;
+      W.incl[e] = (uint32_t)incl;
+      W.jx[e] = (uint32_t)jlo | ((uint32_t)(incl - cnt) << 8);
+      W.x0[e] = x0;
+      total = __shfl_sync(FULL, incl, 31);
+    }
+  }
+  __syncwarp();
+  /* ---- dense lane-per-candidate evaluation over all groups */
+  int tcount = 0;
+  SeedScratch& WT = trip_part(W);
+  for (int base = 0; base < total; base += 32) {
+    const int tau = base + lane;
+    const bool act = tau < total;
+    int e = 0; /* number of entries whose running count is <= tau == the entry owning candidate tau */
 #pragma unroll
-        for (int st = 16; st >= 1; st >>= 1) {
-          const int v = __shfl_sync(FULL, incl, owner + st - 1);
-          if (v <= tau) owner += st;
-        }
-        owner = min(owner, 31);
-        const int before = __shfl_sync(FULL, incl, owner) - __shfl_sync(FULL, cnt, owner);
-        const int j = __shfl_sync(FULL, jlo, owner) + (tau - before); /* h2 index inside its window */
-        const float x0o = __shfl_sync(FULL, x0, owner);
-        bool pass = false;
-        unsigned long long key = 0;
-        if (act) {
-          /* the exact predicate is the definition */
-          const float x2 = hx[fc + j];
-          const float t = (x2 - x0o) * inv_dz;
-          bool ok = true;
-          if (low_p) ok = (t - tx) * qop > 0.0f; /* filter 1: same bending direction */
-          const float x_at_mag = x0o + t * zmag_a;
-          const float tol = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * fabsf(t));
-          ok = ok && (fabsf(x_at_mag - x_mag) < tol); /* filter 2: opening at the magnet centre */
-          if (ok) {
-            const float x1e = zb * t + (x0o - t * za) * Kx1;
-            float dx;
-            const int k = closest_hit<true>(hx, fb, nb, x1e, dup, dx);
-            const float chi2 = dx * dx;
-            if (chi2 < C.T_triplet) {
-              pass = true;
-              key = ((unsigned long long)__float_as_uint(chi2) << 32) |
-                    (unsigned)((set << (3 * F::IB)) | ((sub + owner) << (2 * F::IB)) | (j << F::IB) | (k - fb));
-            }
-          }
-        }
-        const unsigned m = __ballot_sync(FULL, pass);
-        if (m) {
-          if (tcount > 32) tcount = select_smallest(W, tcount, C.n_triplets, lane);
-          if (pass) W.trip[tcount + __popc(m & lt_mask)] = key;
-          tcount += __popc(m);
-          __syncwarp();
+    for (int st = 64; st >= 1; st >>= 1)
+      if (W.incl[e + st - 1] <= (uint32_t)tau) e += st;
+    e = min(e, 127);
+    bool pass = false;
+    unsigned long long key = 0;
+    if (act) {
+      const uint32_t jx = W.jx[e];
+      const float x0o = W.x0[e];
+      const int set = e >> 6, h0i = e & 63;
+      const int j = (int)(jx & 0xFFu) + (tau - (int)(jx >> 8)); /* h2 index inside its window */
+      /* the exact predicate is the definition */
+      const int fb = set ? fbs[1] : fbs[0], nb = set ? nbs[1] : nbs[0], fc = set ? fcs[1] : fcs[0];
+      const float inv_dz = set ? C.inv_dz_ac[1] : C.inv_dz_ac[0], zmag_a = set ? C.zmag_a[1] : C.zmag_a[0];
+      const float x2 = hx[fc + j];
+      const float t = (x2 - x0o) * inv_dz;
+      bool ok = true;
+      if (low_p) ok = (t - tx) * qop > 0.0f; /* filter 1: same bending direction */
+      const float x_at_mag = x0o + t * zmag_a;
+      const float tol = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * fabsf(t));
+      ok = ok && (fabsf(x_at_mag - x_mag) < tol); /* filter 2: opening at the magnet centre */
+      if (ok) {
+        const float zb = set ? C.z[7] : C.z[4], za = set ? C.z[3] : C.z[0], Kx1 = set ? C.K[1] : C.K[0];
+        const float x1e = zb * t + (x0o - t * za) * Kx1;
+        float dx;
+        const int k = closest_hit<true>(hx, fb, nb, x1e, dup, dx);
+        const float chi2 = dx * dx;
+        if (chi2 < C.T_triplet) {
+          pass = true;
+          key = ((unsigned long long)__float_as_uint(chi2) << 32) |
+                (unsigned)((set << (3 * F::IB)) | (h0i << (2 * F::IB)) | (j << F::IB) | (k - fb));
         }
       }
     }
+    const unsigned m = __ballot_sync(FULL, pass);
+    if (m) {
+      if (tcount > 32) tcount = select_smallest(WT, tcount, C.n_triplets, lane);
+      if (pass) WT.trip[tcount + __popc(m & lt_mask)] = key;
+      tcount += __popc(m);
+      __syncwarp();
+    }
   }
-  if (tcount > 0) tcount = select_smallest(W, tcount, C.n_triplets, lane); /* sorted in (chi2,set,h0,h2) order */
+  if (tcount > 0) tcount = select_smallest(WT, tcount, C.n_triplets, lane); /* sorted in (chi2,set,h0,h2) order */
   const int ntr = tcount;
   const int NT = C.n_triplets;
   if (lane == 0) A.n_trip[row] = (uint8_t)ntr;
   const bool mine = lane < ntr;
-  const unsigned long long key = mine ? W.trip[lane] : 0ull;
-  if (lane < NT) static_cast<uint32_t*>(A.trip_code)[row * NT + lane] = (unsigned)key;
+  const unsigned long long key = mine ? WT.trip[lane] : 0ull;
+  if (mine) static_cast<uint32_t*>(A.trip_code)[row * NT + lane] = (unsigned)key; /* codes beyond n_trip are never read */
   if (DEBUG) {
     const unsigned low = (unsigned)key;
     const int set = (low >> (3 * F::IB)) & 1, la = set ? 3 : 0;
-    const int fa = (int)(__shfl_sync(FULL, winw, la) >> F::WB), fb = (int)(__shfl_sync(FULL, winw, la + 4) >> F::WB);
-    const int fc = (int)(__shfl_sync(FULL, winw, la + 8) >> F::WB);
+    const int fa = (int)(__shfl_sync(FULL, winw, la) >> F::WB);
+    const int fb = set ? fbs[1] : fbs[0], fc = set ? fcs[1] : fcs[0];
     if (lane == 0 && A.dbg.n_triplets) A.dbg.n_triplets[row] = ntr;
     if (lane < NT) {
       const size_t o = row * NT + lane;
@@ -846,17 +874,18 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
   __syncwarp();
 }
 
+template <bool WIDE>
 struct __align__(16) SeedTables {
   int next_seed;
   int pad[3];
-  SeedScratch ws[SEED_WARPS];
+  typename std::conditional<WIDE, SeedScratchWide, SeedScratch>::type ws[SEED_WARPS];
 };
 
 template <bool DEBUG, bool WIDE>
 __global__ void __launch_bounds__(SEED_THREADS, WIDE ? 4 : 5) lf_seed_kernel(const __grid_constant__ Consts C,
                                                                            const __grid_constant__ EventArgs A) {
   CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
-  SeedTables& T = *reinterpret_cast<SeedTables*>(lf_smem + HDR_BYTES + (size_t)A.stage_cap * sizeof(float));
+  SeedTables<WIDE>& T = *reinterpret_cast<SeedTables<WIDE>*>(lf_smem + HDR_BYTES + (size_t)A.stage_cap * sizeof(float));
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (threadIdx.x == 0) {
     mbar_init(&H.mbar, 1);
@@ -868,7 +897,7 @@ __global__ void __launch_bounds__(SEED_THREADS, WIDE ? 4 : 5) lf_seed_kernel(con
     const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
     const int sides = WIDE ? C.sides : 1;
     const int n_rows = (int)(s1 - s0) * sides;
-    SeedScratch& W = T.ws[warp];
+    auto& W = T.ws[warp];
     const bool dup = H.dup != 0;
     for (;;) { /* the warps of the CTA share the event's rows, two per ticket */
       int k = 0;
@@ -877,7 +906,7 @@ __global__ void __launch_bounds__(SEED_THREADS, WIDE ? 4 : 5) lf_seed_kernel(con
       if (k >= n_rows) break;
       const int kend = min(k + 2, n_rows);
       for (; k < kend; ++k) {
-        if (WIDE) {
+        if constexpr (WIDE) {
           const uint32_t seed = s0 + (uint32_t)(k / sides);
           const int side = k - (k / sides) * sides;
           if (E.staged) seed_triplets_wide<DEBUG>(C, A, HitView<true>{E.skew}, E.h0, seed, side, W, lane, dup);
