@@ -24,7 +24,7 @@ constexpr int N_PROF_EV = LF_N_KERNELS + 1;
 /* lf_run_host pipelines the batch in chunks of events: H2D of chunk c+1, kernels of chunk c and D2H of
  * chunk c-1 overlap (PCIe is full duplex).  At most HOST_MAX_CHUNKS chunks of at least HOST_CHUNK_EVENTS. */
 constexpr int HOST_MAX_CHUNKS = 16;
-constexpr size_t HOST_CHUNK_EVENTS = 1024;
+constexpr size_t HOST_CHUNK_EVENTS = 2048; /* measured on config 3: 8-10 chunks beat 16 (11.1 vs 11.6 ms) */
 
 struct HostBufs { /* device staging for lf_run_host */
   float* seeds = nullptr;      /* 5 * max_seeds */

@@ -8,6 +8,8 @@
 * occupancy scan (Fig. 11-12): the same quantities against the event occupancy (tracks, fake seeds
   and noise hits scaled together - the stand-in for the number of pp collisions per event).
 
+* concurrent streams: the same batch cut into event ranges that run on several CUDA streams at once.
+
 Everything runs through the C ABI on cuda:0 (no CPU fallback); efficiencies use the generator's truth
 (`truth.evaluate`, the paper's 70 % matching rule).  Prints a markdown report.
 """
@@ -54,11 +56,48 @@ def measure(binding, truth, G, P, batch, steps: int):
                 tracks=r.n_tracks)
 
 
+def measure_streams(binding, G, P, batch, n_streams: int, steps: int):
+    """The batch cut into `n_streams` event ranges, each with its own handle and CUDA stream, all in flight together
+    (the paper's way of filling the GPU: several streams, each with its own batch of events)."""
+    import torch
+    from . import sharding
+    ranges = sharding.event_ranges(batch.seed_offsets, n_streams)
+    parts = [batch.slice_events(e0, e1) for e0, e1 in ranges]
+    lfs = [binding.LookingForward(G, P, p.n_events, p.n_seeds, p.n_hits) for p in parts]
+    dbs = [binding.DeviceBatch(p) for p in parts]
+    outs = [binding.TrackBuffers(p.n_seeds, p.n_events, dbs[0].device) for p in parts]
+    streams = [torch.cuda.Stream() for _ in parts]
+    main = torch.cuda.current_stream()
+
+    def step():
+        for lf, db, out, st in zip(lfs, dbs, outs, streams):
+            lf.run(db, out, st)
+    for _ in range(3):
+        step()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(main)
+    for st in streams:
+        st.wait_stream(main)
+    for _ in range(steps):
+        step()
+    for st in streams:
+        main.wait_stream(st)
+    e1.record(main)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    tracks = sum(int(o.n_tracks.cpu()[0]) for o in outs)
+    for lf in lfs:
+        lf.close()
+    return dict(ms=ms, events_per_s=batch.n_events / (ms * 1e-3), tracks=tracks)
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--events", type=int, default=4000, help="events of the Run-3-like batch (configs[1] recipe)")
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--out", default=None, help="also write the report to this file")
+    ap.add_argument("--sections", default="window,occupancy,streams", help="comma list of window, occupancy, streams")
     args = ap.parse_args(argv)
     import torch
     if not torch.cuda.is_available():
@@ -81,7 +120,24 @@ def main(argv=None):
                          f"{100 * m['eff_kin']:.2f} % | {100 * m['eff_all']:.2f} % | {100 * m['ghost']:.2f} % | {m['tracks']} |")
         lines.append("")
 
-    # ---- n_window scans (Fig. 10), with-UT tuning
+    sections = set(args.sections.split(","))
+    P0, P1 = datagen.default_params(), datagen.no_ut_params()
+    if "window" in sections:
+        scan_window(binding, truth, datagen, G, base, args, table, hits_per_seg)
+    if "occupancy" in sections:
+        scan_occupancy(binding, truth, datagen, G, args, table)
+    if "streams" in sections:
+        scan_streams(binding, datagen, G, args, lines)
+    report = "\n".join(lines)
+    print(report)
+    if args.out:
+        with open(args.out, "w") as fh:
+            fh.write(report + "\n")
+    return 0
+
+
+def scan_window(binding, truth, datagen, G, base, args, table, hits_per_seg):
+    # ---- n_window scans (Fig. 10)
     P0 = datagen.default_params()
     rows = [(str(nw), measure(binding, truth, G, dict(P0, n_window=nw), base, args.steps)) for nw in (4, 8, 12, 16, 24, 32, 48, 64)]
     table(f"n_window scan, with-UT tuning, window tolerances fixed ({args.events} events, {hits_per_seg:.0f} hits per layer half; "
@@ -96,7 +152,11 @@ def main(argv=None):
     rows = [(str(nw), measure(binding, truth, G, dict(P1, n_window=nw), base, args.steps)) for nw in (16, 32, 48, 64)]
     table("n_window scan, no-UT tuning (PAPER.md:323: 64)", rows, "n_window")
 
+
+
+def scan_occupancy(binding, truth, datagen, G, args, table):
     # ---- occupancy scan (Fig. 11, 12)
+    P0, P1 = datagen.default_params(), datagen.no_ut_params()
     rows_ut, rows_no = [], []
     for f in (0.25, 0.5, 1.0, 1.5, 2.0, 3.0):
         c = datagen.CONFIGS[1]
@@ -108,12 +168,18 @@ def main(argv=None):
         rows_no.append((label, measure(binding, truth, G, P1, b, args.steps)))
     table("occupancy scan, with-UT tuning (x 1 = BASELINE.json configs[1] occupancy)", rows_ut, "occupancy")
     table("occupancy scan, no-UT tuning", rows_no, "occupancy")
-    report = "\n".join(lines)
-    print(report)
-    if args.out:
-        with open(args.out, "w") as fh:
-            fh.write(report + "\n")
-    return 0
+
+
+def scan_streams(binding, datagen, G, args, lines):
+    # ---- concurrent streams
+    P0 = datagen.default_params()
+    big = datagen.generate(datagen.with_overrides(datagen.CONFIGS[1], seed=2001), n_events=5 * args.events)
+    lines.extend([f"## concurrent streams, with-UT tuning ({big.n_events} events cut into equal-seed-count ranges, one handle and one stream each)", "",
+                  "| streams | ms/step | events/s | tracks |", "|---|---|---|---|"])
+    for ns in (1, 2, 4, 8):
+        m = measure_streams(binding, G, P0, big, ns, args.steps)
+        lines.append(f"| {ns} | {m['ms']:.3f} | {m['events_per_s'] / 1e6:.2f} M | {m['tracks']} |")
+    lines.append("")
 
 
 if __name__ == "__main__":
