@@ -44,7 +44,7 @@
 extern "C" {
 #endif
 
-#define LF_ABI_VERSION 3u
+#define LF_ABI_VERSION 4u
 #define LF_N_LAYERS 12   /* three T-stations, x-u-v-x each */
 #define LF_N_ZONES 2     /* lower / upper half */
 #define LF_MAX_WINDOW 32   /* largest params.n_window of the narrow kernels (one warp lane per hit) */
@@ -75,6 +75,13 @@ typedef struct {
   float x_half, y_half;          /* acceptance; used by generators only, ignored by the library */
   float z_state;                 /* z at which the output state is evaluated */
   int32_t polarity;              /* +1 = MU, -1 = MD; selects the asymmetric window edge (Eq. 3) */
+  /* Full Eq. (9): the coefficient of dSlope^i is a 2-D polynomial in the seed's slopes,
+   * c_i(tx, ty) = sum_j qop_poly2d[i][j] * tx^k * ty^m over the terms the field symmetries allow, k + m <= 6:
+   *   even i: (k,m) = (0,0) (2,0) (0,2) (4,0) (2,2) (0,4) (6,0) (4,2) (2,4) (0,6)
+   *   odd  i: (k,m) = (1,0) (3,0) (1,2) (5,0) (3,2) (1,4); slots 6..9 are not read.
+   * qop_mode = 0: c_i = qop_poly[i] (constants); qop_mode = 1: the table (qop_poly is then not read). */
+  int32_t qop_mode;
+  float qop_poly2d[5][10];
 } lf_geometry;
 
 /* Tunables: Table 3 "Forward" column, Table 4 and the DESIGN.md readings.

@@ -37,6 +37,11 @@ def run(G: dict, P: dict, b) -> SimpleNamespace:
     z_seed, z_mag, kick, z_ref, d_ratio = f(G["z_seed"]), f(G["z_mag"]), f(G["kick"]), f(G["z_ref"]), f(G["d_ratio"])
     K = (f(G["k_first"]), f(G["k_last"]))
     poly = [f(c) for c in G["qop_poly"]]
+    qop_mode = int(G.get("qop_mode", 0))
+    poly2d = [[f(c) for c in row] for row in G.get("qop_poly2d", [[0.0] * 10] * 5)]
+    # Eq. (9): exponents (k, m) of tx^k ty^m allowed by the field symmetries, k + m <= 6
+    even_terms = [(k, m) for d in (0, 2, 4, 6) for k in range(d, -1, -2) for m in [d - k]]
+    odd_terms = [(k, m) for d in (1, 3, 5) for k in range(d, 0, -2) for m in [d - k]]
     z_state = f(G["z_state"])
     pol = int(G["polarity"])
     hx = np.asarray(b.hit_x, dtype=np.float64)
@@ -175,7 +180,12 @@ def run(G: dict, P: dict, b) -> SimpleNamespace:
                       continue
                   if best is None or Q < best[0]:
                       dslope = par[1] - tx
-                      F = sum(c * dslope ** k for k, c in enumerate(poly))
+                      if qop_mode == 0:
+                          coef = poly
+                      else:
+                          coef = [sum(a * tx ** k * ty ** m for a, (k, m) in zip(poly2d[i], even_terms if i % 2 == 0 else odd_terms))
+                                  for i in range(5)]
+                      F = sum(c * dslope ** k for k, c in enumerate(coef))
                       state = [float(basis(z_state) @ par), ypar[0] + ypar[1] * (z_state - z_ref),
                                float(dbasis(z_state) @ par), ty_fit, dslope / F]
                       best = (Q, hit, n, state)

@@ -57,6 +57,8 @@ struct Geo {
   Real D10[2], D20[2], W10[2], W20[2], inv_det[2], inv_D10[2]; /* 3-point solve (C11) */
   Real dz_state, ds, ws, dws;           /* output state plane (C19) */
   int polarity;
+  int qop_mode;
+  Real poly2d[5][10];
 };
 
 Geo make_geo(const lfo_geometry& G) {
@@ -66,6 +68,9 @@ Geo make_geo(const lfo_geometry& G) {
   g.K[0] = G.k_first; g.K[1] = G.k_last;
   for (int i = 0; i < 5; ++i) g.poly[i] = G.qop_poly[i];
   g.polarity = G.polarity;
+  g.qop_mode = G.qop_mode;
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j < 10; ++j) g.poly2d[i][j] = G.qop_poly2d[i][j];
   g.mag_dz_seed = g.z_mag - g.z_seed;
   for (int l = 0; l < NL; ++l) {
     g.z[l] = G.z[l];
@@ -265,6 +270,24 @@ void triplet_seeding(const Geo& g, const lfo_params& P, const float* hx, const S
   if (int(out.size()) > P.n_triplets) out.resize(P.n_triplets);
 }
 
+/* Coefficients c_0..c_4 of Eq. (9) for a seed with slopes (tx, ty): constants, or 2-D
+ * polynomials in the slopes with the terms the field symmetries allow (term order: lf_oracle.h). */
+void eq9_coefficients(const Geo& g, Real tx, Real ty, Real c[5]) {
+  if (g.qop_mode == 0) {
+    for (int i = 0; i < 5; ++i) c[i] = g.poly[i];
+    return;
+  }
+  const Real u = tx * tx, v = ty * ty;
+  const Real uu = u * u, uv = u * v, vv = v * v;
+  const Real mono[10] = {RC(1.0), u, v, uu, uv, vv, uu * u, uu * v, u * vv, vv * v};
+  for (int i = 0; i < 5; ++i) {
+    const int n_terms = (i % 2 == 0) ? 10 : 6;
+    Real acc = g.poly2d[i][0];
+    for (int j = 1; j < n_terms; ++j) acc = acc + g.poly2d[i][j] * mono[j];
+    c[i] = (i % 2 == 0) ? acc : tx * acc;   /* odd i: tx^(2a+1) ty^(2b) = tx * (tx^2)^a (ty^2)^b */
+  }
+}
+
 struct Candidate {
   int hit[NL];       /* global hit index per layer or -1 */
   int n, n_uv;
@@ -399,6 +422,7 @@ extern "C" int lf_oracle_run(const lfo_geometry* G, const lfo_params* P, const l
   if (!G || !P || !seeds || !hits || !out) return 1;
   if (G->n_layers != NL || P->n_window < 2 || P->n_triplets < 1) return 1;
   if (P->mode != 0 && P->mode != 1) return 1;
+  if (G->qop_mode != 0 && G->qop_mode != 1) return 1;
   if (P->mode == 0 && !seeds->qop) return 1;
   const int n_sides = (P->mode == 1) ? 2 : 1;
   if (!out->event_offsets || !out->n_tracks) return 1;
@@ -462,7 +486,9 @@ extern "C" int lf_oracle_run(const lfo_geometry* G, const lfo_params* P, const l
       /* O7: q/p from the slope change, state at z_state. */
       const Real t_ref = best.t * RC(0.001);
       const Real dslope = t_ref - s.tx;
-      const Real F = g.poly[0] + dslope * (g.poly[1] + dslope * (g.poly[2] + dslope * (g.poly[3] + dslope * g.poly[4])));
+      Real cq[5];
+      eq9_coefficients(g, s.tx, s.ty, cq);
+      const Real F = cq[0] + dslope * (cq[1] + dslope * (cq[2] + dslope * (cq[3] + dslope * cq[4])));
       const Real qop_out = dslope / F;
       const Real x_out = (best.a + best.t * g.ds) + best.c * g.ws;
       const Real tx_out = (best.t + best.c * g.dws) * RC(0.001);

@@ -41,6 +41,11 @@ typedef struct {
   float x_half, y_half;           /* acceptance (generator only; unused here) */
   float z_state;                  /* z of the output state */
   int32_t polarity;               /* +1 = MU, -1 = MD (Eq. 3) */
+  /* Full Eq. (9): c_i(tx, ty) = sum_j qop_poly2d[i][j] tx^k ty^m over the terms allowed by the
+   * field symmetries, k + m <= 6.  Even i: (k,m) = (0,0) (2,0) (0,2) (4,0) (2,2) (0,4) (6,0) (4,2) (2,4) (0,6);
+   * odd i: (1,0) (3,0) (1,2) (5,0) (3,2) (1,4), slots 6..9 unused.  qop_mode 0: c_i = qop_poly[i] (constants). */
+  int32_t qop_mode;
+  float qop_poly2d[5][10];
 } lfo_geometry;
 
 typedef struct {

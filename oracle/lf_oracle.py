@@ -44,7 +44,7 @@ class _Geometry(C.Structure):
                 ("z_ref", C.c_float), ("d_ratio", C.c_float),
                 ("k_first", C.c_float), ("k_last", C.c_float), ("qop_poly", C.c_float * 5),
                 ("x_half", C.c_float), ("y_half", C.c_float), ("z_state", C.c_float),
-                ("polarity", C.c_int32)]
+                ("polarity", C.c_int32), ("qop_mode", C.c_int32), ("qop_poly2d", (C.c_float * 10) * 5)]
 
 
 class _Params(C.Structure):
@@ -87,7 +87,9 @@ class _Debug(C.Structure):
 def _fill(struct, values: Dict[str, object]):
     for name, ctype in struct._fields_:
         v = values[name]
-        if isinstance(v, (list, tuple, np.ndarray)):
+        if isinstance(v, (list, tuple, np.ndarray)) and len(v) and isinstance(v[0], (list, tuple, np.ndarray)):
+            setattr(struct, name, ctype(*[ctype._type_(*[float(t) for t in row]) for row in v]))
+        elif isinstance(v, (list, tuple, np.ndarray)):
             setattr(struct, name, ctype(*[float(t) for t in v]))
         else:
             setattr(struct, name, v)

@@ -33,7 +33,7 @@ class lf_geometry(C.Structure):
                 ("z_ref", C.c_float), ("d_ratio", C.c_float),
                 ("k_first", C.c_float), ("k_last", C.c_float), ("qop_poly", C.c_float * 5),
                 ("x_half", C.c_float), ("y_half", C.c_float), ("z_state", C.c_float),
-                ("polarity", C.c_int32)]
+                ("polarity", C.c_int32), ("qop_mode", C.c_int32), ("qop_poly2d", (C.c_float * 10) * 5)]
 
 
 class lf_params(C.Structure):
@@ -121,7 +121,7 @@ def load_library() -> C.CDLL:
     lib.lf_set_profiling.argtypes = [C.c_void_p, C.c_int]
     lib.lf_kernel_times.restype = C.c_int
     lib.lf_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_float * 6)]
-    if lib.lf_abi_version() != 3:
+    if lib.lf_abi_version() != 4:
         raise ImportError("liblf_b200.so: ABI version mismatch")
     for i, st in enumerate(_STRUCTS):
         if lib.lf_sizeof(i) != C.sizeof(st):
@@ -133,7 +133,9 @@ def load_library() -> C.CDLL:
 def _fill(struct, values: Dict[str, object]):
     for name, ctype in struct._fields_:
         v = values[name]
-        if isinstance(v, (list, tuple, np.ndarray)):
+        if isinstance(v, (list, tuple, np.ndarray)) and len(v) and isinstance(v[0], (list, tuple, np.ndarray)):
+            setattr(struct, name, ctype(*[ctype._type_(*[float(t) for t in row]) for row in v]))
+        elif isinstance(v, (list, tuple, np.ndarray)):
             setattr(struct, name, ctype(*[float(t) for t in v]))
         else:
             setattr(struct, name, v)

@@ -142,6 +142,9 @@ void make_consts(const lf_geometry& G, const lf_params& P, lf::Consts& c) {
   c.xtol_base = P.xtol_base; c.xtol_inv_p = P.xtol_inv_p; c.x_asym = P.x_asym; c.uv_half_width = P.uv_half_width;
   c.p_same_bend = P.p_same_bend; c.mag_tol_base = P.mag_tol_base; c.mag_tol_inv_p = P.mag_tol_inv_p;
   c.mag_tol_tx = P.mag_tol_tx; c.mag_tol_max = P.mag_tol_max;
+  c.qop_mode = G.qop_mode;
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j < 10; ++j) c.poly2d[i][j] = G.qop_poly2d[i][j];
   c.mode = P.mode;
   c.sides = (P.mode == 1) ? 2 : 1;
   if (P.mode == 1) {
@@ -193,6 +196,11 @@ const char* validate(const lf_geometry& G, const lf_params& P) {
   }
   if (!(G.z_mag > G.z_seed) || !(G.z[0] > G.z_mag)) return "geometry: need z_seed < z_mag < z[0]";
   if (G.polarity != 1 && G.polarity != -1) return "geometry.polarity must be +1 or -1";
+  if (G.qop_mode != 0 && G.qop_mode != 1) return "geometry.qop_mode must be 0 (constants) or 1 (2-D polynomials)";
+  if (G.qop_mode == 1)
+    for (int i = 0; i < 5; ++i)
+      for (int j = 0; j < ((i % 2 == 0) ? 10 : 6); ++j)
+        if (!std::isfinite(G.qop_poly2d[i][j])) return "geometry.qop_poly2d: non-finite coefficient";
   if (P.n_window < 2 || P.n_window > LF_MAX_WINDOW_WIDE) return "params.n_window out of [2, LF_MAX_WINDOW_WIDE]";
   if (P.n_triplets < 1 || P.n_triplets > LF_MAX_TRIPLETS_WIDE) return "params.n_triplets out of [1, LF_MAX_TRIPLETS_WIDE]";
   if (P.mode != 0 && P.mode != 1) return "params.mode must be 0 (with UT) or 1 (no-UT)";

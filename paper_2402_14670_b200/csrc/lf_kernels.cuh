@@ -86,6 +86,9 @@ struct Consts {
   int mode, sides;                 /* mode 1: sides = 2 (LEFT / RIGHT windows of Eq. 8) */
   float inv_p_min, inv_pt_min;     /* 1 / velo_p_min, 1 / velo_pt_min */
   float xtol_poly[8], x_overlap;   /* Eq. (7) / Table 5; Eq. (8) */
+  /* full Eq. (9) */
+  int qop_mode;
+  float poly2d[5][10];
 };
 
 struct FitLut;
@@ -1173,6 +1176,28 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_extend_kernel(const __grid_
   }
 }
 
+/* Coefficients c_0..c_4 of Eq. (9) for a seed with slopes (tx, ty): constants, or 2-D polynomials
+ * in the slopes over the terms the field symmetries allow (term order: include/lf.h, lf_geometry.qop_poly2d).
+ * Even i: sum_j a_ij mono_j over 10 monomials in u = tx^2, v = ty^2; odd i: tx * (sum over the first 6). */
+__device__ __forceinline__ void eq9_coefficients(const Consts& C, float tx, float ty, float (&c)[5]) {
+  if (C.qop_mode == 0) {
+#pragma unroll
+    for (int i = 0; i < 5; ++i) c[i] = C.poly[i];
+    return;
+  }
+  const float u = tx * tx, v = ty * ty;
+  const float uu = u * u, uv = u * v, vv = v * v;
+  const float mono[10] = {1.0f, u, v, uu, uv, vv, uu * u, uu * v, u * vv, vv * v};
+#pragma unroll
+  for (int i = 0; i < 5; ++i) {
+    const int n_terms = (i % 2 == 0) ? 10 : 6;
+    float acc = C.poly2d[i][0];
+#pragma unroll
+    for (int j = 1; j < n_terms; ++j) acc = acc + C.poly2d[i][j] * mono[j];
+    c[i] = (i % 2 == 0) ? acc : tx * acc;
+  }
+}
+
 /* ---- F: lf_fit_kernel (a6 + ranking).  One thread per accepted candidate, a pass of FIT_THREADS records at a
  * time; the records of a seed are adjacent and a pass ends on a seed boundary, so after one barrier the lowest
  * (Q, k) of every seed is known (64-bit atomicMin in shared memory) and the winning thread still holds its fit
@@ -1331,7 +1356,9 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
       const float a = a0 + da, tt = t0 + dt, c = c0 + dc;
       const float t_ref = tt * 0.001f;
       const float dslope = t_ref - tx;
-      const float F = C.poly[0] + dslope * (C.poly[1] + dslope * (C.poly[2] + dslope * (C.poly[3] + dslope * C.poly[4])));
+      float cq[5];
+      eq9_coefficients(C, tx, ty, cq);
+      const float F = cq[0] + dslope * (cq[1] + dslope * (cq[2] + dslope * (cq[3] + dslope * cq[4])));
       int4* r4 = reinterpret_cast<int4*>(A.ws_rec + (size_t)seed * REC_WORDS);
       r4[0] = make_int4((int)wf[0], (int)wf[1], (int)wf[2], (int)wf[3]);
       r4[1] = make_int4((int)wf[4], (int)wf[5], (int)wf[6], (int)wf[7]);

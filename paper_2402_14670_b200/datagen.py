@@ -81,6 +81,10 @@ def toy_geometry(polarity: int = 1) -> Dict[str, object]:
         "k_last": _toy_k(z[3], z[7], z[11]),
         # Eq. (9) reduced to a constant (C18): slope at z_ref includes the quadratic term
         "qop_poly": [TOY_KICK * (1.0 + 2.0 * TOY_C2 * (TOY_Z_REF - TOY_Z0)), 0.0, 0.0, 0.0, 0.0],
+        # full Eq. (9): coefficients of dSlope^i as 2-D polynomials in the seed slopes; inactive
+        # while qop_mode == 0.  `momentum_fit.fit_qop_poly2d` produces them from toy tracks.
+        "qop_mode": 0,
+        "qop_poly2d": [[0.0] * 10 for _ in range(5)],
         "x_half": TOY_X_HALF,
         "y_half": TOY_Y_HALF,
         "z_state": z[11],
@@ -115,6 +119,20 @@ def no_ut_params() -> Dict[str, object]:
                 p_same_bend=0.0, mag_tol_base=10.0, mag_tol_inv_p=0.0, mag_tol_tx=0.0, mag_tol_max=10.0)
 
 
+def toy_dtx(tx, ty, qop, field_ax: float = 0.0, field_ay: float = 0.0):
+    """Change of the x slope across the magnet.  BASELINE.json's TOY field: kick * q/p.  With a non-uniform field
+    (`field_ax`, `field_ay` != 0; stand-in for LHCb's field map) the kick acts on the normalised slope
+    as in Eq. (2) with an integrated field that grows with the entry slopes:
+    n(t) = t / sqrt(1 + t^2 + ty^2),  n(tx_out) = n(tx_in) + kick * q/p * (1 + ax tx^2 + ay ty^2)."""
+    if field_ax == 0.0 and field_ay == 0.0:
+        return TOY_KICK * qop
+    n_in = tx / np.sqrt(1.0 + tx * tx + ty * ty)
+    n_out = n_in + TOY_KICK * qop * (1.0 + field_ax * tx * tx + field_ay * ty * ty)
+    n_out = np.clip(n_out, -0.95, 0.95)
+    tx_out = n_out * np.sqrt((1.0 + ty * ty) / (1.0 - n_out * n_out))
+    return tx_out - tx
+
+
 def toy_x_at(x_mag, txp, dtx, z):
     """TOY truth x(z) downstream of the magnet (BASELINE.json configs[0])."""
     return x_mag + txp * (z - TOY_Z_MAG) + TOY_C2 * dtx * (z - TOY_Z0) ** 2
@@ -145,6 +163,8 @@ class GenConfig:
     eff: float = 0.98                   # per-layer hit efficiency
     zpv_sigma: float = 60.0             # origin spread along z, mm (C20)
     hit_storage: int = 0                # 0 fp32, 1 fp16 storage for windows + seeding
+    field_ax: float = 0.0               # non-uniform field (toy_dtx); 0, 0 = BASELINE.json's TOY kick
+    field_ay: float = 0.0
 
 
 CONFIGS: Dict[int, GenConfig] = {
@@ -263,7 +283,7 @@ def _gen_chunk(cfg: GenConfig, chunk_idx: int, n_ev: int) -> _Chunk:
     trk_event = np.repeat(np.arange(n_ev, dtype=np.int64), n_true)
     x, y, tx, ty, qop = states(nt)
     x_mag = x + tx * (TOY_Z_MAG - TOY_Z_SEED)
-    dtx = TOY_KICK * qop
+    dtx = toy_dtx(tx, ty, qop, cfg.field_ax, cfg.field_ay)
     txp = tx + dtx
     xt = toy_x_at(x_mag[:, None], txp[:, None], dtx[:, None], z[None, :])
     yt = y[:, None] + ty[:, None] * (z[None, :] - TOY_Z_SEED)

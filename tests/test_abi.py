@@ -34,7 +34,7 @@ def test_struct_sizes_match_binding(lib):
     from paper_2402_14670_b200 import binding
     for i, st in enumerate(binding._STRUCTS):
         assert lib.lf_sizeof(i) == ctypes.sizeof(st)
-    assert lib.lf_sizeof(99) == 0 and lib.lf_abi_version() == 3
+    assert lib.lf_sizeof(99) == 0 and lib.lf_abi_version() == 4
 
 
 def test_argument_validation_needs_no_gpu(lib, geometry, params):
@@ -55,7 +55,7 @@ def test_argument_validation_needs_no_gpu(lib, geometry, params):
         p = bd._fill(bd.lf_params(), unsupported)
         assert lib.lf_create(ctypes.byref(g), ctypes.byref(p), 1, 1, 1, ctypes.byref(h)) == bd.LF_ERR_UNSUPPORTED
     p = bd._fill(bd.lf_params(), params)
-    for bad_geo in (dict(geometry, n_layers=8), dict(geometry, polarity=0),
+    for bad_geo in (dict(geometry, n_layers=8), dict(geometry, polarity=0), dict(geometry, qop_mode=2),
                     dict(geometry, tan_alpha=[0.0] * 12), dict(geometry, z=list(reversed(geometry["z"])))):
         gg = bd._fill(bd.lf_geometry(), bad_geo)
         assert lib.lf_create(ctypes.byref(gg), ctypes.byref(p), 1, 1, 1, ctypes.byref(h)) == bd.LF_ERR_INVALID_ARG
