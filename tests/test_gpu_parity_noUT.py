@@ -165,3 +165,21 @@ def test_noUT_run_host_and_determinism(lfmod, oracle, geometry, nparams):
     c = _gpu_run(lfmod, geometry, nparams, b)
     assert np.array_equal(a.hit_idx, c.hit_idx) and np.array_equal(a.state.view(np.uint32), c.state.view(np.uint32))
     assert np.array_equal(a.quality.view(np.uint32), c.quality.view(np.uint32))
+
+
+def test_full_eq9_table_both_tunings(lfmod, oracle, geometry, params, nparams):
+    """geometry.qop_mode = 1: q/p from the 2-D polynomial table, in a non-uniform toy field,
+    narrow kernels (with UT) and wide kernels (no-UT); also the mirrored event (negated stereo angles, polarity)."""
+    from paper_2402_14670_b200 import momentum_fit as mf
+    table = mf.fit_qop_poly2d(0.8, 1.5)
+    G1 = dict(geometry, qop_mode=1, qop_poly2d=table)
+    b = dg.generate(dg.with_overrides(dg.CONFIGS[1], field_ax=0.8, field_ay=1.5, seed=3001), n_events=300)
+    for P, what in ((params, "Eq. 9 table, with UT"), (nparams, "Eq. 9 table, no-UT")):
+        info, ref = _both(lfmod, oracle, G1, P, b, what, debug=False)
+        assert ref.n_tracks > 10000
+        # the table changes q/p and nothing else
+        ref0 = oracle.run(geometry, P, b, threads=NTHREADS)
+        assert np.array_equal(ref.hit_idx, ref0.hit_idx) and np.array_equal(ref.state[:, :4], ref0.state[:, :4])
+        assert np.max(np.abs(ref.state[:, 4] / ref0.state[:, 4] - 1.0)) > 0.02
+    Gm = dict(G1, polarity=-1, tan_alpha=[-t for t in geometry["tan_alpha"]])
+    _both(lfmod, oracle, Gm, params, b, "Eq. 9 table, mirrored geometry", debug=False)
