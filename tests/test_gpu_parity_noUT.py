@@ -183,3 +183,14 @@ def test_full_eq9_table_both_tunings(lfmod, oracle, geometry, params, nparams):
         assert np.max(np.abs(ref.state[:, 4] / ref0.state[:, 4] - 1.0)) > 0.02
     Gm = dict(G1, polarity=-1, tan_alpha=[-t for t in geometry["tan_alpha"]])
     _both(lfmod, oracle, Gm, params, b, "Eq. 9 table, mirrored geometry", debug=False)
+
+
+def test_scan_script_runs(lfmod, tmp_path):
+    """`python -m paper_2402_14670_b200.scan` (the Fig. 10-12 analogue) on a small batch: report written, rates positive."""
+    from paper_2402_14670_b200 import scan
+    out = tmp_path / "scan.md"
+    assert scan.main(["--events", "150", "--steps", "1", "--sections", "window,streams", "--out", str(out)]) == 0
+    text = out.read_text()
+    assert "n_window scan" in text and "concurrent streams" in text
+    rows = [l for l in text.splitlines() if l.startswith("| 32 |")]
+    assert rows and float(rows[0].split("|")[5].strip().rstrip(" %")) > 95.0   # efficiency (p > 5, pT > 1) at n_window = 32
