@@ -205,6 +205,14 @@ lf_status lf_run_host(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
  * chunks is min(16, max(1, n_events / min_events_per_chunk)). */
 lf_status lf_set_host_chunk_events(lf_handle* h, size_t min_events_per_chunk);
 
+/* Checks, on the device, the input preconditions lf_run relies on but does not check (see "Conventions"): segment
+ * offsets monotone, starting at 0 and ending at n_hits; stored coordinates finite and ascending inside every
+ * segment; seed offsets monotone, starting at 0 and ending at n_seeds; seed states finite (q/p only when params.mode
+ * == 0).  Arguments as for lf_run (HOST structs holding DEVICE pointers); `out` is not needed.  SYNCHRONOUS: waits
+ * for `cuda_stream`.  Returns LF_OK, or LF_ERR_INVALID_ARG with lf_last_error naming the kind of violation and the
+ * index of one offending segment / hit / event / seed.  A debugging aid: not part of the hot path. */
+lf_status lf_validate_inputs(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, void* cuda_stream);
+
 /* Frees the workspace and the handle.  NULL is allowed. */
 lf_status lf_destroy(lf_handle* h);
 

@@ -106,6 +106,8 @@ def load_library() -> C.CDLL:
         fn = getattr(lib, name)
         fn.restype = C.c_int
         fn.argtypes = [C.c_void_p, C.POINTER(lf_seeds), C.POINTER(lf_hits), C.c_size_t, C.POINTER(lf_tracks), C.c_void_p]
+    lib.lf_validate_inputs.restype = C.c_int
+    lib.lf_validate_inputs.argtypes = [C.c_void_p, C.POINTER(lf_seeds), C.POINTER(lf_hits), C.c_size_t, C.c_void_p]
     lib.lf_run_debug.restype = C.c_int
     lib.lf_run_debug.argtypes = [C.c_void_p, C.POINTER(lf_seeds), C.POINTER(lf_hits), C.c_size_t, C.POINTER(lf_tracks),
                                  C.POINTER(lf_debug), C.c_void_p]
@@ -257,6 +259,13 @@ class LookingForward:
         self._check(self._lib.lf_run_debug(self._h, C.byref(seeds), C.byref(hits), db.n_events, C.byref(tr), C.byref(dbg), sp))
         out.debug_tensors = d
         return out
+
+    def validate_inputs(self, db: DeviceBatch, stream=None) -> None:
+        """``lf_validate_inputs`` (synchronous): raises LfError naming the violated precondition."""
+        seeds = lf_seeds(db.seed_x.data_ptr(), db.seed_y.data_ptr(), db.seed_tx.data_ptr(), db.seed_ty.data_ptr(),
+                         db.seed_qop.data_ptr(), db.seed_offsets.data_ptr(), db.n_seeds)
+        hits = lf_hits(db.hit_x.data_ptr(), db.seg_offsets.data_ptr(), db.n_hits)
+        self._check(self._lib.lf_validate_inputs(self._h, C.byref(seeds), C.byref(hits), db.n_events, self._stream_ptr(stream)))
 
     # -- host path (end to end) ------------------------------------------------------------------
     def run_host(self, hb: "HostBatch", out: "HostTracks", stream=None) -> int:

@@ -553,6 +553,38 @@ lf_status lf_run_debug(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits,
   return launch<true>(h, seeds, hits, n_events, out, debug, (cudaStream_t)cuda_stream);
 }
 
+lf_status lf_validate_inputs(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, void* cuda_stream) {
+  if (!h) return LF_ERR_INVALID_ARG;
+  if (!seeds || !hits || !seeds->event_offsets || !hits->seg_offsets)
+    return fail(h, LF_ERR_INVALID_ARG, "lf_validate_inputs: NULL seeds/hits or offset table");
+  if (seeds->n_seeds > 0 && (!seeds->x || !seeds->y || !seeds->tx || !seeds->ty || (!seeds->qop && h->P.mode == 0)))
+    return fail(h, LF_ERR_INVALID_ARG, "lf_validate_inputs: NULL seed array");
+  if (hits->n_hits > 0 && !hits->x) return fail(h, LF_ERR_INVALID_ARG, "lf_validate_inputs: NULL hit array");
+  if (n_events > h->max_events || seeds->n_seeds > h->max_seeds || hits->n_hits > h->max_hits)
+    return fail(h, LF_ERR_CAPACITY, "lf_validate_inputs: batch exceeds the maxima given to lf_create");
+  h->err.clear();
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  uint32_t* res = h->ev_count; /* 4 words of the workspace serve as the result; no lf_run may be in flight on the handle */
+  if (h->max_events < 4) return fail(h, LF_ERR_CAPACITY, "lf_validate_inputs: needs a handle created for at least 4 events");
+  LF_CUDA(h, cudaMemsetAsync(res, 0, 4 * sizeof(uint32_t), st));
+  const int blocks = std::max(1, std::min<int>(h->sm_count * 8, (int)((n_events * lf::NSEG + 7) / 8) + 1));
+  lf::lf_validate_kernel<<<blocks, 256, 0, st>>>(hits->x, hits->seg_offsets, (uint32_t)n_events, (uint32_t)hits->n_hits,
+                                               seeds->event_offsets, (uint32_t)seeds->n_seeds, seeds->x, seeds->y, seeds->tx,
+                                               seeds->ty, h->P.mode == 0 ? seeds->qop : nullptr, res);
+  LF_CUDA(h, cudaGetLastError());
+  uint32_t host[4] = {0, 0, 0, 0};
+  LF_CUDA(h, cudaMemcpyAsync(host, res, sizeof(host), cudaMemcpyDeviceToHost, st));
+  LF_CUDA(h, cudaStreamSynchronize(st));
+  if (host[0] == 0) return LF_OK;
+  std::string msg = "lf_validate_inputs:";
+  if (host[0] & lf::BAD_SEG_OFFSETS) msg += " seg_offsets not monotone / not ending at n_hits (segment " + std::to_string(host[1]) + ");";
+  if (host[0] & lf::BAD_HIT_ORDER) msg += " hits not ascending inside a segment (hit " + std::to_string(host[2]) + ");";
+  if (host[0] & lf::BAD_HIT_VALUE) msg += " non-finite hit coordinate (hit " + std::to_string(host[2]) + ");";
+  if (host[0] & lf::BAD_SEED_OFFSETS) msg += " seed event_offsets not monotone / not ending at n_seeds (event " + std::to_string(host[3]) + ");";
+  if (host[0] & lf::BAD_SEED_VALUE) msg += " non-finite seed state (seed " + std::to_string(host[3]) + ");";
+  return fail(h, LF_ERR_INVALID_ARG, msg);
+}
+
 lf_status lf_set_host_chunk_events(lf_handle* h, size_t min_events_per_chunk) {
   if (!h) return LF_ERR_INVALID_ARG;
   if (min_events_per_chunk == 0) return fail(h, LF_ERR_INVALID_ARG, "lf_set_host_chunk_events: must be >= 1");

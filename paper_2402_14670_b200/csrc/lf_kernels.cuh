@@ -1445,6 +1445,42 @@ __global__ void __launch_bounds__(256) lf_pack_hits_kernel(const float* __restri
   }
 }
 
+/* lf_validate_inputs: the preconditions lf_run does not check (include/lf.h "Conventions").  One warp per
+ * (event, layer, zone) segment, grid-stride; result[0] = OR of the violation bits, result[1..3] = index of a
+ * violation of each kind (any one of them). */
+constexpr uint32_t BAD_SEG_OFFSETS = 1u, BAD_HIT_ORDER = 2u, BAD_SEED_OFFSETS = 4u, BAD_SEED_VALUE = 8u, BAD_HIT_VALUE = 16u;
+__global__ void __launch_bounds__(256) lf_validate_kernel(const float* __restrict__ hx, const uint32_t* __restrict__ seg_off,
+                                                          uint32_t n_events, uint32_t n_hits, const uint32_t* __restrict__ seed_off,
+                                                          uint32_t n_seeds, const float* __restrict__ sx, const float* __restrict__ sy,
+                                                          const float* __restrict__ stx, const float* __restrict__ sty,
+                                                          const float* __restrict__ sqop, uint32_t* __restrict__ result) {
+  const uint32_t lane = threadIdx.x & 31u;
+  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
+  const uint32_t n_seg = n_events * NSEG;
+  for (uint32_t sg = warp; sg < n_seg; sg += n_warps) {
+    const uint32_t a = seg_off[sg], e = seg_off[sg + 1];
+    if (a > e || e > n_hits) {
+      if (lane == 0) { atomicOr(result, BAD_SEG_OFFSETS); result[1] = sg; }
+      continue;
+    }
+    for (uint32_t i = a + lane; i < e; i += 32u) {
+      const float v = hx[i];
+      if (!isfinite(v)) { atomicOr(result, BAD_HIT_VALUE); result[2] = i; }
+      if (i + 1 < e && !(v <= hx[i + 1])) { atomicOr(result, BAD_HIT_ORDER); result[2] = i; }
+    }
+  }
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, n_thr = gridDim.x * blockDim.x;
+  if (tid == 0 && (seg_off[0] != 0u || seg_off[n_seg] != n_hits)) { atomicOr(result, BAD_SEG_OFFSETS); result[1] = n_seg; }
+  if (tid == 0 && (seed_off[0] != 0u || seed_off[n_events] != n_seeds)) { atomicOr(result, BAD_SEED_OFFSETS); result[3] = n_events; }
+  for (uint32_t ev = tid; ev < n_events; ev += n_thr)
+    if (seed_off[ev] > seed_off[ev + 1]) { atomicOr(result, BAD_SEED_OFFSETS); result[3] = ev; }
+  for (uint32_t s = tid; s < n_seeds; s += n_thr) {
+    bool ok = isfinite(sx[s]) && isfinite(sy[s]) && isfinite(stx[s]) && isfinite(sty[s]);
+    if (sqop != nullptr) ok = ok && isfinite(sqop[s]);
+    if (!ok) { atomicOr(result, BAD_SEED_VALUE); result[3] = s; }
+  }
+}
+
 /* Exclusive scan of per-event track counts (single CTA); also re-arms the event tickets. */
 __global__ void __launch_bounds__(1024) lf_scan_kernel(const uint32_t* __restrict__ ev_count, uint32_t n_events,
                                                        uint32_t* __restrict__ ev_off_ws, uint32_t* __restrict__ out_off,

@@ -244,3 +244,43 @@ def test_config2_fp16_hit_storage(lfmod, oracle, geometry, params):
     # the fp16 path is deterministic too
     got2 = _gpu_run(lfmod, geometry, dict(params, hit_storage=1), b)
     assert np.array_equal(got.hit_idx, got2.hit_idx) and np.array_equal(got.state.view(np.uint32), got2.state.view(np.uint32))
+
+
+def test_validate_inputs(lfmod, geometry, params):
+    """lf_validate_inputs: the preconditions lf_run relies on, checked on the device."""
+    import torch
+    b = dg.generate_config(1, n_events=20)
+    lf = lfmod.LookingForward(geometry, params, b.n_events, b.n_seeds, b.n_hits)
+    lf.validate_inputs(lfmod.DeviceBatch(b))                                   # a generated batch is valid
+    lf.validate_inputs(lfmod.DeviceBatch(dg.generate(dg.GenConfig("e", 0, 1))))  # so is an empty one
+
+    def expect(batch, word, handle=lf):
+        with pytest.raises(lfmod.LfError) as ei:
+            handle.validate_inputs(lfmod.DeviceBatch(batch))
+        assert ei.value.status == lfmod.LF_ERR_INVALID_ARG and word in str(ei.value), str(ei.value)
+
+    hx = b.hit_x.copy()
+    s0 = int(b.seg_offsets[5])
+    hx[s0], hx[s0 + 1] = hx[s0 + 1] + 1.0, hx[s0]
+    expect(dg.Batch(**{**b.__dict__, "hit_x": hx}), "not ascending")
+    hx = b.hit_x.copy()
+    hx[7] = np.inf
+    expect(dg.Batch(**{**b.__dict__, "hit_x": hx}), "non-finite hit")
+    so = b.seg_offsets.copy()
+    so[10], so[11] = so[11], so[10] + (1 if so[10] == so[11] else 0)
+    expect(dg.Batch(**{**b.__dict__, "seg_offsets": so}), "seg_offsets")
+    eo = b.seed_offsets.copy()
+    eo[3] = eo[4] + 1
+    expect(dg.Batch(**{**b.__dict__, "seed_offsets": eo}), "seed event_offsets")
+    q = b.seed_qop.copy()
+    q[11] = np.nan
+    bad_q = dg.Batch(**{**b.__dict__, "seed_qop": q})
+    expect(bad_q, "non-finite seed")
+    lf.close()
+    # q/p is not an input of the no-UT mode
+    lf1 = lfmod.LookingForward(geometry, dg.no_ut_params(), b.n_events, b.n_seeds, b.n_hits)
+    lf1.validate_inputs(lfmod.DeviceBatch(bad_q))
+    tx = b.seed_tx.copy()
+    tx[0] = np.nan
+    expect(dg.Batch(**{**b.__dict__, "seed_tx": tx}), "non-finite seed", lf1)
+    lf1.close()
