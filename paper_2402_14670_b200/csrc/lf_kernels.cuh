@@ -957,7 +957,7 @@ __device__ __forceinline__ void triplet_parabola(const Consts& C, const HV& hx, 
 /* a4/a5: extension of one triplet to the 9 other layers + hit-count rule.
  * `geo` is the shared-memory copy of the per-layer constants: d, w, dzs, tana (12 floats each). */
 template <bool WIDE, class HV>
-__device__ __noinline__ CandHits extend_candidate(const Consts& C, const HV& hx, const uint32_t* winw, const float* geo,
+__device__ __forceinline__ CandHits extend_candidate(const Consts& C, const HV& hx, const uint32_t* winw, const float* geo,
                                                   float y, float tx, float ty, unsigned code, bool dup) {
   typedef Fmt<WIDE> F;
   const int set = (code >> (3 * F::IB)) & 1;
