@@ -190,7 +190,8 @@ lf_status lf_run_debug(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits,
 
 /* End-to-end variant: every pointer inside `seeds`, `hits`, `out` is a HOST pointer (pinned memory
  * makes the copies asynchronous and lets them overlap the kernels).  The batch is pipelined in chunks of
- * events (at most 16 chunks of at least 2048 events, see lf_set_host_chunk_events): the host->device copy
+ * events (the seeds of the whole batch first; then the hits in at most 13 equal chunks of at least 2048 events, see
+ * lf_set_host_chunk_events, the last of them cut into four shrinking pieces to shorten the pipeline's tail): the host->device copy
  * of chunk c+1, the kernels of chunk c (on `cuda_stream`) and the device->host copy of the tracks of chunk
  * c-1 (library-owned copy streams, ordered after the work already queued on `cuda_stream`) run
  * concurrently; device buffers are library-owned, allocated on first use and sized by lf_create's maxima.
@@ -201,8 +202,8 @@ lf_status lf_run_debug(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits,
 lf_status lf_run_host(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events,
                       lf_tracks* out, void* cuda_stream);
 
-/* Smallest number of events lf_run_host puts in one pipeline chunk (default 2048; >= 1).  The number of
- * chunks is min(16, max(1, n_events / min_events_per_chunk)). */
+/* Smallest number of events lf_run_host puts in one equal pipeline chunk (default 2048; >= 1).  The number of
+ * equal chunks is min(13, max(1, n_events / min_events_per_chunk)); the last one is cut into four pieces. */
 lf_status lf_set_host_chunk_events(lf_handle* h, size_t min_events_per_chunk);
 
 /* Checks, on the device, the input preconditions lf_run relies on but does not check (see "Conventions"): segment

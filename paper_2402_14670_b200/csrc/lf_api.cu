@@ -635,8 +635,24 @@ lf_status lf_run_host(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
     b.ready = true;
   }
   const size_t stride = std::max<size_t>(h->max_seeds, 1);
-  const int n_chunks = (int)std::min<size_t>(HOST_MAX_CHUNKS, std::max<size_t>(1, n_events / h->host_chunk_events));
-  auto chunk_begin = [&](int c) { return (size_t)(((unsigned long long)n_events * (unsigned)c) / (unsigned)n_chunks); };
+  /* Chunk boundaries.  The pipeline is bound by the host->device copies, so what is left after the last byte has
+   * arrived (kernels + device->host copy of the LAST chunk) is pure latency: equal chunks of at least
+   * host_chunk_events events, the last of them cut into four pieces of 40 / 27 / 18 / 15 % so that this tail is short
+   * while every piece's kernels still hide behind the next piece's copy. */
+  size_t bounds[HOST_MAX_CHUNKS + 1];
+  int n_chunks = 0;
+  {
+    const int base = (int)std::min<size_t>(HOST_MAX_CHUNKS - 3, std::max<size_t>(1, n_events / h->host_chunk_events));
+    for (int c = 0; c < base; ++c) bounds[n_chunks++] = (size_t)(((unsigned long long)n_events * (unsigned)c) / (unsigned)base);
+    const size_t last0 = bounds[n_chunks - 1], last_n = n_events - last0;
+    if (last_n >= 64) {
+      bounds[n_chunks++] = last0 + (last_n * 40) / 100;
+      bounds[n_chunks++] = last0 + (last_n * 67) / 100;
+      bounds[n_chunks++] = last0 + (last_n * 85) / 100;
+    }
+    bounds[n_chunks] = n_events;
+  }
+  auto chunk_begin = [&](int c) { return bounds[c]; };
   uint32_t* pin_cnt = b.pinned_count;
   uint32_t* pin_off = b.pinned_count + HOST_MAX_CHUNKS; /* chunk c's n+1 relative offsets start at e0 + c */
 
@@ -649,13 +665,15 @@ lf_status lf_run_host(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
   /* ---- host -> device: the offset tables once, then seeds and hits chunk by chunk */
   LF_CUDA(h, cudaMemcpyAsync(b.seed_off, so, (n_events + 1) * sizeof(uint32_t), cudaMemcpyHostToDevice, b.s_h2d));
   LF_CUDA(h, cudaMemcpyAsync(b.seg_off, go, (n_events * lf::NSEG + 1) * sizeof(uint32_t), cudaMemcpyHostToDevice, b.s_h2d));
+  /* the seeds of the whole batch go first, in five copies (15 % of the input bytes): per-chunk seed copies would add
+   * 5 x n_chunks small transfers, each with its fixed cost, to the stream that bounds the pipeline */
   const float* src[5] = {seeds->x, seeds->y, seeds->tx, seeds->ty, seeds->qop};
+  for (int i = 0; i < 5 && seeds->n_seeds > 0; ++i)
+    if (src[i]) /* qop may be NULL in the no-UT mode */
+      LF_CUDA(h, cudaMemcpyAsync(b.seeds + i * stride, src[i], seeds->n_seeds * sizeof(float), cudaMemcpyHostToDevice, b.s_h2d));
   for (int c = 0; c < n_chunks; ++c) {
     const size_t e0 = chunk_begin(c), e1 = chunk_begin(c + 1);
-    const size_t s0 = so[e0], s1 = so[e1], g0 = go[e0 * lf::NSEG], g1 = go[e1 * lf::NSEG];
-    for (int i = 0; i < 5 && s1 > s0; ++i)
-      if (src[i]) /* qop may be NULL in the no-UT mode */
-        LF_CUDA(h, cudaMemcpyAsync(b.seeds + i * stride + s0, src[i] + s0, (s1 - s0) * sizeof(float), cudaMemcpyHostToDevice, b.s_h2d));
+    const size_t g0 = go[e0 * lf::NSEG], g1 = go[e1 * lf::NSEG];
     if (g1 > g0) LF_CUDA(h, cudaMemcpyAsync(b.hits + g0, hits->x + g0, (g1 - g0) * sizeof(float), cudaMemcpyHostToDevice, b.s_h2d));
     LF_CUDA(h, cudaEventRecord(b.ev_h2d[c], b.s_h2d));
   }
