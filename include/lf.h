@@ -33,6 +33,8 @@
  *     coordinate s = x + y*tan_alpha is ASCENDING (precondition, not checked).  Offsets are
  *     monotone.  q/p is finite.
  *   - Output order contract: tracks are ordered by (event, seed index); at most one per seed.
+ *   - Limits: n_hits, n_seeds < 2^31 per call; at most 2^26 seeds and 2^25 hits in one event (packed per-event
+ *     indices in the library's tables); n_window <= 64, n_triplets <= 32.
  */
 #ifndef LF_H
 #define LF_H
