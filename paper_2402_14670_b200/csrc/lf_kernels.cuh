@@ -1028,12 +1028,11 @@ struct ExtTables {
   float* geo;      /* 4*12: d, w, dzs, tana */
   uint32_t* win;   /* FIT_CHUNK*12 packed windows */
   float* sp;       /* FIT_CHUNK*4: y, tx, ty, (unused) */
-  int* pref;       /* FIT_CHUNK+4: exclusive prefix of candidates per seed */
   uint16_t* item;  /* FIT_CHUNK*NT: seed_local<<4 | k */
   int* wcnt;       /* 2 * 8: accepted candidates per warp, double-buffered by pass */
 };
 __host__ __device__ inline size_t ext_tables_bytes(int nt) {
-  return 4 * NL * 4 + (size_t)FIT_CHUNK * NL * 4 + (size_t)FIT_CHUNK * 4 * 4 + (size_t)(FIT_CHUNK + 4) * 4 +
+  return 4 * NL * 4 + (size_t)FIT_CHUNK * NL * 4 + (size_t)FIT_CHUNK * 4 * 4 +
          (((size_t)FIT_CHUNK * nt * 2 + 15) & ~size_t(15)) + 16 * 4;
 }
 
@@ -1093,7 +1092,6 @@ __device__ __forceinline__ void extend_event(const Consts& C, const EventArgs& A
     }
     const int excl = woff + incl - my_n;
     if (tid < cn) {
-      T.pref[tid] = excl;
       for (int k = 0; k < my_n; ++k) T.item[excl + k] = (uint16_t)((tid << F::KB) | k);
     }
     __syncthreads();
@@ -1156,8 +1154,6 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_extend_kernel(const __grid_
   tb += (size_t)FIT_CHUNK * NL * 4;
   T.sp = reinterpret_cast<float*>(tb);
   tb += (size_t)FIT_CHUNK * 16;
-  T.pref = reinterpret_cast<int*>(tb);
-  tb += (size_t)(FIT_CHUNK + 4) * 4;
   T.item = reinterpret_cast<uint16_t*>(tb);
   tb += ((size_t)FIT_CHUNK * NT * 2 + 15) & ~size_t(15);
   T.wcnt = reinterpret_cast<int*>(tb);
