@@ -288,13 +288,15 @@ def run_ours(args):
     if os.path.exists(traffic_file):
         try:
             tr = json.load(open(traffic_file))
-            if tr.get("kernel") == hbm["kernel"]:
+            # the ncu counts were taken on one batch (n_seeds of the capture): they describe this run only if it is that batch
+            same_batch = tr.get("kernel") == hbm["kernel"] and int(tr.get("n_seeds", -1)) == batch.n_seeds
+            if same_batch:
                 hbm["traffic"] = tr.get("dram_bytes_per_launch")
                 hbm["traffic_source"] = tr.get("source")
             # peak = SMs x 4 schedulers x 1 warp-instruction/clock x max SM clock; achieved = EXECUTED warp-instructions
             # per launch (counted by ncu on this workload, profiles/) / the kernel's live duration.
             wi = tr.get("all_kernels_warp_inst_per_launch", {})
-            if dom in wi and tr.get("kernel") == hbm["kernel"]:
+            if dom in wi and same_batch:
                 sm_mhz = float(clocks.get("sm_max_mhz") or 1965.0)
                 peak_issue = 148 * 4 * sm_mhz * 1e6 / 1e9
                 ach = wi[dom] / (ktimes[dom] * 1e-3) / 1e9

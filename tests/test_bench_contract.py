@@ -1,0 +1,55 @@
+"""bench.py prints ONE JSON line with the keys the driver and the judge read (both arms)."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+BASE_KEYS = {"metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+             "vs_baseline", "dtype", "data", "config", "e2e", "cpu_baseline"}
+
+
+def _run(args, timeout=600):
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py")] + args, capture_output=True, text=True,
+                         timeout=timeout, cwd=ROOT)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [l for l in res.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1, f"bench.py must print exactly one line, got {len(lines)}"
+    return json.loads(lines[0])
+
+
+@pytest.mark.parametrize("tuning", ["with-ut", "no-ut"])
+def test_reference_arm_line(tuning):
+    """--impl reference times the oracle on the host cores: no GPU needed."""
+    d = _run(["--impl", "reference", "--steps", "1", "--warmup", "0", "--events", "60", "--tuning", tuning])
+    assert BASE_KEYS <= set(d) and d["impl"] == "reference"
+    assert d["metric"] == "events_per_s" and d["unit"] == "events/s" and d["higher_is_better"] is True
+    assert d["value"] > 0 and d["vs_baseline"] is None and d["data"] == "synthetic" and d["dtype"] == "f32"
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1 and d["cpu_baseline"]["value"] == d["value"]
+    assert d["e2e"] == {"value": d["value"], "unit": "events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert "workload" in d["config"] and "model" not in d["config"]
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("tuning", ["with-ut", "no-ut"])
+def test_gpu_arm_line(tuning):
+    d = _run(["--steps", "3", "--warmup", "3", "--events", "400", "--cpu-events", "100", "--tuning", tuning])
+    assert BASE_KEYS | {"roofline", "clocks", "gpu_launches"} <= set(d)
+    assert d["metric"] == "events_per_s" and d["n_gpus"] == 1 and d["steps"] == 3 and d["warmup"] >= 3
+    assert d["value"] > 0 and d["ms_per_step"] > 0 and d["scaling"] == "weak" and d["vs_baseline"] is None
+    assert d["gpu_launches"] == 6 * 3
+    e = d["e2e"]
+    assert e["value"] > 0 and e["value"] < d["value"] and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
+    r = d["roofline"]
+    # the ALU (issue-rate) roofline needs ncu's instruction counts of the SAME batch (profiles/dominant_kernel_traffic*.txt,
+    # taken on the full configs[3] batch): on this small batch only the HBM roofline can be reported
+    assert r["bound"] == "hbm" and 0 < r["frac"] < 1 and r["achieved"] > 0 and r["peak"] > 0 and r["traffic"] is None
+    hbm = r
+    assert hbm["bound"] == "hbm" and hbm["unit"] == "GB/s" and 0 < hbm["frac"] < 1 and hbm["algorithmic_bytes_per_launch"] > 0
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] == 1 and c["value"] > 0 and "sample" in c
+    assert d["oracle_check"]["equal"] is True
+    assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+    assert "workload" in d["config"] and "model" not in d["config"]
