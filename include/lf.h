@@ -182,6 +182,7 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
  * launches; results are valid once the caller has synchronised the stream.  `seeds`, `hits`, `out`
  * are HOST structs holding DEVICE pointers.  Safe to call repeatedly; calls on one handle must not
  * overlap in time (they share the workspace).  n_events == 0 is valid (writes n_tracks = 0).
+ * The call only enqueues kernels, so it may be captured into a CUDA graph and replayed (tests/test_gpu_parity.py).
  * Errors are detected before any launch: LF_ERR_INVALID_ARG (NULL pointer), LF_ERR_CAPACITY. */
 lf_status lf_run(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events,
                  lf_tracks* out, void* cuda_stream);

@@ -284,3 +284,46 @@ def test_validate_inputs(lfmod, geometry, params):
     tx[0] = np.nan
     expect(dg.Batch(**{**b.__dict__, "seed_tx": tx}), "non-finite seed", lf1)
     lf1.close()
+
+
+def test_lf_run_is_graph_capturable(lfmod, oracle, geometry, params):
+    """lf_run only enqueues kernels on the caller's stream (no sync, no allocation): it can be captured into a CUDA
+    graph and replayed, e.g. for small launch-bound batches."""
+    import torch
+    b = dg.generate_config(1, n_events=64)
+    ref = oracle.run(geometry, params, b, threads=NTHREADS)
+    lf = lfmod.LookingForward(geometry, params, b.n_events, b.n_seeds, b.n_hits)
+    db = lfmod.DeviceBatch(b)
+    out = lfmod.TrackBuffers(b.n_seeds, b.n_events, db.device)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        lf.run(db, out, side)            # warm-up outside the capture
+        side.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            lf.run(db, out, side)
+    for _ in range(3):
+        out.hit_idx.fill_(-7)
+        out.n_tracks.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert_tracks_equal(out.to_numpy(), ref, "graph replay")
+    # launch-bound regime: replaying the graph is not slower than six separate launches
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    st = torch.cuda.current_stream()
+    for _ in range(5):
+        g.replay()
+    e0.record(st)
+    for _ in range(50):
+        g.replay()
+    e1.record(st)
+    torch.cuda.synchronize()
+    t_graph = e0.elapsed_time(e1) / 50
+    e0.record(st)
+    for _ in range(50):
+        lf.run(db, out, st)
+    e1.record(st)
+    torch.cuda.synchronize()
+    t_plain = e0.elapsed_time(e1) / 50
+    print(f"64 events: graph replay {t_graph * 1e3:.1f} us, plain launches {t_plain * 1e3:.1f} us")
+    lf.close()
