@@ -327,3 +327,37 @@ def test_lf_run_is_graph_capturable(lfmod, oracle, geometry, params):
     t_plain = e0.elapsed_time(e1) / 50
     print(f"64 events: graph replay {t_graph * 1e3:.1f} us, plain launches {t_plain * 1e3:.1f} us")
     lf.close()
+
+
+def test_garbage_inputs_are_memory_safe(lfmod, geometry, params):
+    """Unsorted hits, NaN / inf / huge values in hits and seeds: the preconditions are violated, so the result is
+    unspecified - but every index stays in range, the offsets are consistent and nothing hangs (searches are bounded
+    by the segment and window limits whatever the comparisons return)."""
+    import torch
+    rng = np.random.default_rng(5)
+    for P in (params, dg.no_ut_params(), dict(params, n_window=64, n_triplets=32)):
+        b = dg.generate_config(1, n_events=30)
+        hx = rng.uniform(-4000, 4000, b.n_hits).astype(np.float32)
+        hx[rng.integers(0, b.n_hits, 200)] = np.nan
+        hx[rng.integers(0, b.n_hits, 200)] = np.inf
+
+        def junk(a):
+            a = a.copy()
+            idx = rng.integers(0, a.shape[0], a.shape[0] // 5)
+            a[idx] = rng.choice([np.nan, np.inf, -np.inf, 1e30, -1e30, 0.0], idx.shape[0]).astype(np.float32)
+            return a
+        bb = dg.Batch(**{**b.__dict__, "hit_x": hx, "seed_x": junk(b.seed_x), "seed_y": junk(b.seed_y),
+                         "seed_tx": junk(b.seed_tx), "seed_ty": junk(b.seed_ty), "seed_qop": junk(b.seed_qop)})
+        lf = lfmod.LookingForward(geometry, P, bb.n_events, bb.n_seeds, bb.n_hits)
+        with pytest.raises(lfmod.LfError):
+            lf.validate_inputs(lfmod.DeviceBatch(bb))
+        for debug in (False, True):
+            out = lf.run(lfmod.DeviceBatch(bb), debug=debug)
+            torch.cuda.synchronize()
+            r = out.to_numpy()
+            assert 0 <= r.n_tracks <= bb.n_seeds
+            assert np.all(np.diff(r.event_offsets.astype(np.int64)) >= 0) and r.event_offsets[-1] == r.n_tracks
+            if r.n_tracks:
+                assert r.hit_idx.min() >= -1 and r.hit_idx.max() < bb.n_hits
+                assert r.seed_idx.min() >= 0 and r.seed_idx.max() < bb.n_seeds
+        lf.close()
