@@ -127,7 +127,7 @@ def run(G: dict, P: dict, b) -> SimpleNamespace:
                   for i0 in windows[la]:
                       for i2 in windows[lc]:
                           t = (hx[i2] - hx[i0]) / (z[lc] - z[la])
-                          if mode == 0 and p < pf["p_same_bend"] and not ((t - tx) * qop > 0):
+                          if mode == 0 and p < pf["p_same_bend"] and not ((t - tx) * (kick * qop) > 0):
                               continue
                           tol = min(pf["mag_tol_max"], pf["mag_tol_base"] + pf["mag_tol_inv_p"] / p + pf["mag_tol_tx"] * abs(t))
                           if not abs(hx[i0] + t * (z_mag - z[la]) - x_mag) < tol:

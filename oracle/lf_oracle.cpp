@@ -246,9 +246,10 @@ void triplet_seeding(const Geo& g, const lfo_params& P, const float* hx, const S
       for (int i2 = wc.first; i2 < wc.first + wc.count; ++i2) {
         const Real x0 = hx[i0], x2 = hx[i2];
         const Real t = (x2 - x0) * g.inv_dz_ac[set];
-        /* filter 1 (C7): below 5 GeV the doublet must bend like the seed's charge */
+        /* filter 1 (C7): below 5 GeV the doublet's slope change t - tx must have the sign of the
+         * expected kick, delta tx = kick * q/p (Eq. 2) */
         /* (no-UT: the VELO track has no momentum or charge, so the filter does not exist) */
-        if (P.mode == 0 && s.p < Real(P.p_same_bend) && !((t - s.tx) * s.qop > 0)) continue;
+        if (P.mode == 0 && s.p < Real(P.p_same_bend) && !((t - s.tx) * (g.kick * s.qop) > 0)) continue;
         /* filter 2 (C6): opening at the magnet centre */
         const Real x_at_mag = x0 + t * g.zmag_a[set];
         const Real tol = std::min(Real(P.mag_tol_max),

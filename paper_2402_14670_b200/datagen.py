@@ -65,22 +65,24 @@ def _toy_k(za: float, zb: float, zc: float) -> float:
     return 1.0 + TOY_C2 * (zb - za) * (zc - zb) / (TOY_Z_MAG - TOY_C2 * (TOY_Z0 ** 2 - za * zc))
 
 
-def toy_geometry(polarity: int = 1) -> Dict[str, object]:
-    """Plain-value description of the TOY geometry (fields of ``lf_geometry``)."""
+def toy_geometry(polarity: int = 1, kick_sign: float = 1.0) -> Dict[str, object]:
+    """Plain-value description of the TOY geometry (fields of ``lf_geometry``).  ``kick_sign = -1`` is the magnet with
+    the field reversed (particles bend the other way; generate the events with ``GenConfig.kick_sign = -1``)."""
     z = TOY_Z
+    kick = math.copysign(TOY_KICK, kick_sign)
     return {
         "n_layers": N_LAYERS,
         "z": list(z),
         "tan_alpha": list(TOY_TAN),
         "z_seed": TOY_Z_SEED,
         "z_mag": TOY_Z_MAG,
-        "kick": TOY_KICK,
+        "kick": kick,
         "z_ref": TOY_Z_REF,
         "d_ratio": 0.0,
         "k_first": _toy_k(z[0], z[4], z[8]),
         "k_last": _toy_k(z[3], z[7], z[11]),
         # Eq. (9) reduced to a constant (DESIGN.md C18): slope at z_ref includes the quadratic term
-        "qop_poly": [TOY_KICK * (1.0 + 2.0 * TOY_C2 * (TOY_Z_REF - TOY_Z0)), 0.0, 0.0, 0.0, 0.0],
+        "qop_poly": [kick * (1.0 + 2.0 * TOY_C2 * (TOY_Z_REF - TOY_Z0)), 0.0, 0.0, 0.0, 0.0],
         # full Eq. (9): coefficients of dSlope^i as 2-D polynomials in the seed slopes (PAPER.md:331-338); inactive
         # while qop_mode == 0.  `momentum_fit.fit_qop_poly2d` produces them from toy tracks.
         "qop_mode": 0,
@@ -165,6 +167,7 @@ class GenConfig:
     hit_storage: int = 0                # 0 fp32, 1 fp16 storage for windows + seeding
     field_ax: float = 0.0               # non-uniform field (toy_dtx); 0, 0 = BASELINE.json's TOY kick
     field_ay: float = 0.0
+    kick_sign: float = 1.0              # -1: reversed field, delta tx = -kick * q/p (pair with toy_geometry(kick_sign=-1))
 
 
 CONFIGS: Dict[int, GenConfig] = {
@@ -283,7 +286,7 @@ def _gen_chunk(cfg: GenConfig, chunk_idx: int, n_ev: int) -> _Chunk:
     trk_event = np.repeat(np.arange(n_ev, dtype=np.int64), n_true)
     x, y, tx, ty, qop = states(nt)
     x_mag = x + tx * (TOY_Z_MAG - TOY_Z_SEED)
-    dtx = toy_dtx(tx, ty, qop, cfg.field_ax, cfg.field_ay)
+    dtx = cfg.kick_sign * toy_dtx(tx, ty, qop, cfg.field_ax, cfg.field_ay)
     txp = tx + dtx
     xt = toy_x_at(x_mag[:, None], txp[:, None], dtx[:, None], z[None, :])
     yt = y[:, None] + ty[:, None] * (z[None, :] - TOY_Z_SEED)

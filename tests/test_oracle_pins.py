@@ -132,6 +132,25 @@ def test_truth_exact_hits_noise_free(oracle, geometry, params, real, tol_x, tol_
     assert np.max(first) < 0.01 ** 2
 
 
+def test_truth_reversed_field(oracle, params):
+    """Reading C7 with the field reversed (kick < 0, polarity -1): the same-bend filter compares the doublet's slope
+    change with the sign of kick * q/p (Eq. 2), so low-momentum truth is still found with exactly its hits.  A filter
+    written as (t - tx) * q/p > 0 would reject every true doublet below p_same_bend here."""
+    G = dg.toy_geometry(polarity=-1, kick_sign=-1.0)
+    cfg = dg.with_overrides(dg.single_track_config(400, seed=13, sigma=0.0, smear=0.0), kick_sign=-1.0, p_max=4.5)
+    b = dg.generate(cfg)
+    assert np.all(1.0 / np.abs(b.trk_qop) < params["p_same_bend"])
+    r = oracle.run(G, params, b, debug=True)
+    full = _full_tracks(b)
+    tid = b.seed_track[r.seed_idx]
+    found = np.zeros(b.n_tracks, bool)
+    found[tid] = True
+    assert full.sum() > 150 and np.all(found[full])
+    sel = full[tid]
+    assert np.all(b.hit_track[r.hit_idx[sel]] == tid[sel][:, None])
+    assert np.max(np.abs(r.state[sel, 4].astype(np.float64) / b.trk_qop[tid[sel]] - 1.0)) < 1e-4
+
+
 def test_truth_measured_hits_found(oracle, geometry, params):
     """sigma = 0.08 mm, 5 % q/p smear, no noise: exactly the generated hits of each >=9-hit track."""
     b = dg.generate(dg.with_overrides(dg.single_track_config(600, seed=12, sigma=0.08, smear=0.05), eff=0.98))
