@@ -10,6 +10,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -60,6 +61,7 @@ struct lf_handle {
   uint8_t* n_trip;
   int32_t *ws_rec, *ws_nh, *ws_rank, *ws_event;
   uint32_t *ev_count, *ev_off, *ev_dup, *ev_acc, *tickets;
+  uint32_t* validate_res; /* 4 words: lf_validate_inputs' violation bits and offending indices */
   uint4* acc_rec;
   lf::FitLut* fit_lut;
   size_t workspace_bytes;
@@ -87,6 +89,22 @@ lf_status fail(lf_handle* h, lf_status st, const std::string& msg) {
   } while (0)
 
 bool uv_layer(int l) { return (l & 3) == 1 || (l & 3) == 2; }
+
+/* cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel function, not to a handle: a later lf_create
+ * with a smaller stage must not lower it under a live handle.  Per (kernel, device) the library keeps the largest
+ * value any handle has asked for and only ever raises the attribute. */
+std::mutex g_attr_mutex;
+constexpr int MAX_DEVICES = 64;
+int g_attr_max[2][4][2][MAX_DEVICES]; /* [wide][kernel][debug][device] */
+
+cudaError_t raise_dynamic_smem(const void* kernel, int wide, int k, int dbg, int device, int bytes) {
+  std::lock_guard<std::mutex> lock(g_attr_mutex);
+  int& cur = g_attr_max[wide][k][dbg][device < 0 || device >= MAX_DEVICES ? 0 : device];
+  if (bytes <= cur) return cudaSuccess;
+  const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) cur = bytes;
+  return e;
+}
 
 /* Host-side constants in fp32, one rounding per operation.
  * Built with -ffp-contract=off; volatile stores keep every intermediate a genuine float. */
@@ -195,6 +213,13 @@ const char* validate(const lf_geometry& G, const lf_params& P) {
       return "geometry.tan_alpha must be 0 on x layers (0,3 mod 4) and non-zero on u/v layers (1,2 mod 4)";
   }
   if (!(G.z_mag > G.z_seed) || !(G.z[0] > G.z_mag)) return "geometry: need z_seed < z_mag < z[0]";
+  {
+    const float gf[] = {G.z_seed, G.z_mag, G.kick, G.z_ref, G.d_ratio, G.k_first, G.k_last, G.z_state,
+                        G.qop_poly[0], G.qop_poly[1], G.qop_poly[2], G.qop_poly[3], G.qop_poly[4]};
+    for (float v : gf)
+      if (!std::isfinite(v)) return "geometry: non-finite constant";
+    if (G.kick == 0.0f) return "geometry.kick must be non-zero (its sign is the bending direction)";
+  }
   if (G.polarity != 1 && G.polarity != -1) return "geometry.polarity must be +1 or -1";
   if (G.qop_mode != 0 && G.qop_mode != 1) return "geometry.qop_mode must be 0 (constants) or 1 (2-D polynomials)";
   if (G.qop_mode == 1)
@@ -214,6 +239,19 @@ const char* validate(const lf_geometry& G, const lf_params& P) {
   if (!(P.T_triplet > 0) || !(P.T_x > 0) || !(P.T_y > 0) || !(P.T_uv_min > 0) || !(P.T_Q > 0) || !(P.T_ty > 0))
     return "params: tolerances must be positive";
   if (P.hit_storage != 0 && P.hit_storage != 1) return "params.hit_storage must be 0 or 1";
+  {
+    /* every tolerance is finite ("no cap" is a large finite number, not inf: the kernels bracket with it) */
+    const float pf[] = {P.T_triplet, P.T_x, P.T_uv_slope, P.T_uv_min, P.T_ty, P.T_y, P.T_Q, P.C_nhits[0], P.C_nhits[1],
+                        P.C_nhits[2], P.C_nhits[3], P.xtol_base, P.xtol_inv_p, P.x_asym, P.uv_half_width, P.p_same_bend,
+                        P.mag_tol_base, P.mag_tol_inv_p, P.mag_tol_tx, P.mag_tol_max};
+    for (float v : pf)
+      if (!std::isfinite(v)) return "params: non-finite tolerance or constant";
+    if (P.T_uv_slope < 0 || P.xtol_base < 0 || P.xtol_inv_p < 0 || P.x_asym < 0 || P.uv_half_width < 0 || P.p_same_bend < 0 ||
+        P.mag_tol_base < 0 || P.mag_tol_inv_p < 0 || P.mag_tol_tx < 0 || P.mag_tol_max < 0)
+      return "params: window and magnet tolerances must be >= 0";
+    for (int i = 0; i < 4; ++i)
+      if (!(P.C_nhits[i] > 0)) return "params.C_nhits must be positive";
+  }
   return nullptr;
 }
 
@@ -400,7 +438,7 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   const int threads[4] = {lf::WIN_THREADS, lf::SEED_THREADS, lf::FIT_THREADS, lf::FIT_THREADS};
   for (int k = 0; k < 4; ++k) {
     for (int d = 0; d < 2; ++d)
-      LF_CREATE_CUDA(cudaFuncSetAttribute(kern[k][d], cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_bytes[k]));
+      LF_CREATE_CUDA(raise_dynamic_smem(kern[k][d], h->wide ? 1 : 0, k, d, h->device, h->smem_bytes[k]));
     LF_CREATE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->ctas_per_sm[k], kern[k][0], threads[k], h->smem_bytes[k]));
     if (h->ctas_per_sm[k] < 1) return bail(LF_ERR_CUDA, "lf_create: an event kernel does not fit on an SM");
     h->grid[k] = h->sm_count * h->ctas_per_sm[k];
@@ -436,6 +474,7 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
     LF_CREATE_CUDA(cudaMalloc(&h->fit_lut, lut.size() * sizeof(lf::FitLut)));
     LF_CREATE_CUDA(cudaMemcpy(h->fit_lut, lut.data(), lut.size() * sizeof(lf::FitLut), cudaMemcpyHostToDevice));
   }
+  LF_CREATE_CUDA(cudaMalloc(&h->validate_res, 4 * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->tickets, lf::N_TICKETS * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMemset(h->tickets, 0, lf::N_TICKETS * sizeof(uint32_t)));
   h->workspace_bytes = nrows * (lf::NL * 4 + nt * (code_bytes + sizeof(uint4)) + 1) + ns * (lf::REC_WORDS + 3) * 4 +
@@ -451,6 +490,7 @@ lf_status lf_destroy(lf_handle* h) {
   cudaFree(h->win); cudaFree(h->trip_code); cudaFree(h->n_trip);
   cudaFree(h->ws_rec); cudaFree(h->ws_nh); cudaFree(h->ws_rank); cudaFree(h->ws_event);
   cudaFree(h->ev_count); cudaFree(h->ev_off); cudaFree(h->ev_dup); cudaFree(h->ev_acc); cudaFree(h->acc_rec); cudaFree(h->fit_lut); cudaFree(h->tickets);
+  cudaFree(h->validate_res);
   HostBufs& b = h->hb;
   cudaFree(b.seeds); cudaFree(b.seed_off); cudaFree(b.hits); cudaFree(b.seg_off);
   cudaFree(b.hit_idx); cudaFree(b.seed_idx); cudaFree(b.n_hits); cudaFree(b.state); cudaFree(b.quality);
@@ -564,9 +604,9 @@ lf_status lf_validate_inputs(lf_handle* h, const lf_seeds* seeds, const lf_hits*
     return fail(h, LF_ERR_CAPACITY, "lf_validate_inputs: batch exceeds the maxima given to lf_create");
   h->err.clear();
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  uint32_t* res = h->ev_count; /* 4 words of the workspace serve as the result; no lf_run may be in flight on the handle */
-  if (h->max_events < 4) return fail(h, LF_ERR_CAPACITY, "lf_validate_inputs: needs a handle created for at least 4 events");
-  LF_CUDA(h, cudaMemsetAsync(res, 0, 4 * sizeof(uint32_t), st));
+  uint32_t* res = h->validate_res; /* word 0: violation bits; words 1..3: smallest offending index of each kind */
+  LF_CUDA(h, cudaMemsetAsync(res, 0, sizeof(uint32_t), st));
+  LF_CUDA(h, cudaMemsetAsync(res + 1, 0xFF, 3 * sizeof(uint32_t), st));
   const int blocks = std::max(1, std::min<int>(h->sm_count * 8, (int)((n_events * lf::NSEG + 7) / 8) + 1));
   lf::lf_validate_kernel<<<blocks, 256, 0, st>>>(hits->x, hits->seg_offsets, (uint32_t)n_events, (uint32_t)hits->n_hits,
                                                seeds->event_offsets, (uint32_t)seeds->n_seeds, seeds->x, seeds->y, seeds->tx,
@@ -592,11 +632,29 @@ lf_status lf_set_host_chunk_events(lf_handle* h, size_t min_events_per_chunk) {
   return LF_OK;
 }
 
+static lf_status run_host_pipeline(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
+                                   void* cuda_stream);
+
 lf_status lf_run_host(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
                       void* cuda_stream) {
   const lf_status st0 = check_run_args(h, seeds, hits, n_events, out);
   if (st0 != LF_OK) return st0;
   h->err.clear();
+  const lf_status rs = run_host_pipeline(h, seeds, hits, n_events, out, cuda_stream);
+  if (rs != LF_OK) {
+    /* an error in the middle of the pipeline: copies from / into the caller's host buffers may still be in flight on
+     * the library's streams; drain them (and the caller's stream) before handing the buffers back */
+    HostBufs& b = h->hb;
+    if (b.s_h2d) cudaStreamSynchronize(b.s_h2d);
+    if (b.s_cnt) cudaStreamSynchronize(b.s_cnt);
+    if (b.s_d2h) cudaStreamSynchronize(b.s_d2h);
+    cudaStreamSynchronize((cudaStream_t)cuda_stream);
+  }
+  return rs;
+}
+
+static lf_status run_host_pipeline(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
+                                   void* cuda_stream) {
   const uint32_t* so = seeds->event_offsets; /* HOST tables: the chunking reads them */
   const uint32_t* go = hits->seg_offsets;
   if (so[0] != 0 || go[0] != 0 || so[n_events] != seeds->n_seeds || go[n_events * lf::NSEG] != hits->n_hits)

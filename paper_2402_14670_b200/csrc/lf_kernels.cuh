@@ -586,6 +586,7 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
   const float x = __ldg(A.sx + seed), tx = __ldg(A.stx + seed), qop = __ldg(A.sqop + seed);
   const float aq = fmaxf(fabsf(qop), 1e-6f);
   const float p = 1.0f / aq;
+  const float kq = C.kick * qop; /* expected slope change across the magnet (Eq. 2) */
   const float x_mag = x + tx * C.mag_dz_seed;
   /* lanes 0..11 hold the packed window of layer `lane` */
   const uint32_t winw = (lane < NL) ? A.win[(size_t)seed * NL + lane] : 0u;
@@ -620,7 +621,8 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
     const float tmax = (fabsf(Aoff) + C.mag_tol_max) * C.inv_abs_zmag_a[set];
     const float tol_sup = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * tmax) + INTERVAL_MARGIN;
     const int jlo = lanes_below<false>(x2v, x0 + (tol_sup - Aoff) * inv_r);  /* first x2 >= lower end */
-    const int jhi = lanes_below<true>(x2v, x0 + (-tol_sup - Aoff) * inv_r);  /* first x2 > upper end */
+    const int jhi = min(nc, lanes_below<true>(x2v, x0 + (-tol_sup - Aoff) * inv_r));  /* first x2 > upper end; the +inf
+                                                                                       padding lanes are not hits */
     const int cnt = have ? max(jhi - jlo, 0) : 0;
     x0s[set] = x0;
     cnt_p |= (unsigned)cnt << (16 * set);
@@ -664,7 +666,7 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
       const float x2 = hx[fc + j];
       const float t = (x2 - x0o) * inv_dz;
       bool ok = true;
-      if (low_p) ok = (t - tx) * qop > 0.0f; /* filter 1: same bending direction */
+      if (low_p) ok = (t - tx) * kq > 0.0f; /* filter 1: same bending direction as the expected kick */
       const float x_at_mag = x0o + t * zmag_a;
       const float tol = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * fabsf(t));
       ok = ok && (fabsf(x_at_mag - x_mag) < tol); /* filter 2: opening at the magnet centre */
@@ -741,15 +743,16 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
   const size_t row = (size_t)seed * C.sides + side;
   const float x = __ldg(A.sx + seed), tx = __ldg(A.stx + seed);
   const bool no_ut = C.mode == 1;
-  float qop = 0.0f, aq;
+  float kq = 0.0f, aq;
   if (no_ut) {
     const float ty = __ldg(A.sty + seed);
     const float s2 = tx * tx + ty * ty;
     const float sin_theta = sqrtf(s2 / (1.0f + s2));
     aq = fminf(C.inv_p_min, sin_theta * C.inv_pt_min);
   } else {
-    qop = __ldg(A.sqop + seed);
+    const float qop = __ldg(A.sqop + seed);
     aq = fmaxf(fabsf(qop), 1e-6f);
+    kq = C.kick * qop; /* expected slope change across the magnet (Eq. 2) */
   }
   const float p = 1.0f / aq;
   const float x_mag = x + tx * C.mag_dz_seed;
@@ -825,7 +828,7 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
       const float x2 = hx[fc + j];
       const float t = (x2 - x0o) * inv_dz;
       bool ok = true;
-      if (low_p) ok = (t - tx) * qop > 0.0f; /* filter 1: same bending direction */
+      if (low_p) ok = (t - tx) * kq > 0.0f; /* filter 1: same bending direction as the expected kick */
       const float x_at_mag = x0o + t * zmag_a;
       const float tol = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * fabsf(t));
       ok = ok && (fabsf(x_at_mag - x_mag) < tol); /* filter 2: opening at the magnet centre */
@@ -1442,8 +1445,8 @@ __global__ void __launch_bounds__(256) lf_pack_hits_kernel(const float* __restri
 }
 
 /* lf_validate_inputs: the preconditions lf_run does not check (include/lf.h "Conventions").  One warp per
- * (event, layer, zone) segment, grid-stride; result[0] = OR of the violation bits, result[1..3] = index of a
- * violation of each kind (any one of them). */
+ * (event, layer, zone) segment, grid-stride; result[0] = OR of the violation bits, result[1..3] = smallest index of
+ * a violation of each kind (segment / hit / event-or-seed), preset to 0xFFFFFFFF by the caller. */
 constexpr uint32_t BAD_SEG_OFFSETS = 1u, BAD_HIT_ORDER = 2u, BAD_SEED_OFFSETS = 4u, BAD_SEED_VALUE = 8u, BAD_HIT_VALUE = 16u;
 __global__ void __launch_bounds__(256) lf_validate_kernel(const float* __restrict__ hx, const uint32_t* __restrict__ seg_off,
                                                           uint32_t n_events, uint32_t n_hits, const uint32_t* __restrict__ seed_off,
@@ -1456,24 +1459,24 @@ __global__ void __launch_bounds__(256) lf_validate_kernel(const float* __restric
   for (uint32_t sg = warp; sg < n_seg; sg += n_warps) {
     const uint32_t a = seg_off[sg], e = seg_off[sg + 1];
     if (a > e || e > n_hits) {
-      if (lane == 0) { atomicOr(result, BAD_SEG_OFFSETS); result[1] = sg; }
+      if (lane == 0) { atomicOr(result, BAD_SEG_OFFSETS); atomicMin(result + 1, sg); }
       continue;
     }
     for (uint32_t i = a + lane; i < e; i += 32u) {
       const float v = hx[i];
-      if (!isfinite(v)) { atomicOr(result, BAD_HIT_VALUE); result[2] = i; }
-      if (i + 1 < e && !(v <= hx[i + 1])) { atomicOr(result, BAD_HIT_ORDER); result[2] = i; }
+      if (!isfinite(v)) { atomicOr(result, BAD_HIT_VALUE); atomicMin(result + 2, i); }
+      if (i + 1 < e && !(v <= hx[i + 1])) { atomicOr(result, BAD_HIT_ORDER); atomicMin(result + 2, i); }
     }
   }
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, n_thr = gridDim.x * blockDim.x;
-  if (tid == 0 && (seg_off[0] != 0u || seg_off[n_seg] != n_hits)) { atomicOr(result, BAD_SEG_OFFSETS); result[1] = n_seg; }
-  if (tid == 0 && (seed_off[0] != 0u || seed_off[n_events] != n_seeds)) { atomicOr(result, BAD_SEED_OFFSETS); result[3] = n_events; }
+  if (tid == 0 && (seg_off[0] != 0u || seg_off[n_seg] != n_hits)) { atomicOr(result, BAD_SEG_OFFSETS); atomicMin(result + 1, n_seg); }
+  if (tid == 0 && (seed_off[0] != 0u || seed_off[n_events] != n_seeds)) { atomicOr(result, BAD_SEED_OFFSETS); atomicMin(result + 3, n_events); }
   for (uint32_t ev = tid; ev < n_events; ev += n_thr)
-    if (seed_off[ev] > seed_off[ev + 1]) { atomicOr(result, BAD_SEED_OFFSETS); result[3] = ev; }
+    if (seed_off[ev] > seed_off[ev + 1]) { atomicOr(result, BAD_SEED_OFFSETS); atomicMin(result + 3, ev); }
   for (uint32_t s = tid; s < n_seeds; s += n_thr) {
     bool ok = isfinite(sx[s]) && isfinite(sy[s]) && isfinite(stx[s]) && isfinite(sty[s]);
     if (sqop != nullptr) ok = ok && isfinite(sqop[s]);
-    if (!ok) { atomicOr(result, BAD_SEED_VALUE); result[3] = s; }
+    if (!ok) { atomicOr(result, BAD_SEED_VALUE); atomicMin(result + 3, s); }
   }
 }
 

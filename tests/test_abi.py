@@ -46,7 +46,9 @@ def test_argument_validation_needs_no_gpu(lib, geometry, params):
     for bad_params, why in ((dict(params, n_window=65), "n_window"), (dict(params, n_triplets=0), "n_triplets"),
                             (dict(params, n_triplets=33), "n_triplets"), (dict(params, mode=2), "mode"),
                             (dict(params, mode=1, velo_pt_min=0.0), "velo_pt_min"),
-                            (dict(params, min_hits=2), "min_hits"), (dict(params, T_x=0.0), "positive")):
+                            (dict(params, min_hits=2), "min_hits"), (dict(params, T_x=0.0), "positive"),
+                            (dict(params, mag_tol_max=float("inf")), "non-finite"), (dict(params, xtol_base=float("nan")), "non-finite"),
+                            (dict(params, uv_half_width=-1.0), ">= 0"), (dict(params, C_nhits=[5.0, 0.0, 0.8, 0.5]), "C_nhits")):
         p = bd._fill(bd.lf_params(), bad_params)
         assert lib.lf_create(ctypes.byref(g), ctypes.byref(p), 1, 1, 1, ctypes.byref(h)) == bd.LF_ERR_INVALID_ARG
         assert why in lib.lf_last_error(None).decode()
@@ -56,7 +58,8 @@ def test_argument_validation_needs_no_gpu(lib, geometry, params):
         assert lib.lf_create(ctypes.byref(g), ctypes.byref(p), 1, 1, 1, ctypes.byref(h)) == bd.LF_ERR_UNSUPPORTED
     p = bd._fill(bd.lf_params(), params)
     for bad_geo in (dict(geometry, n_layers=8), dict(geometry, polarity=0), dict(geometry, qop_mode=2),
-                    dict(geometry, tan_alpha=[0.0] * 12), dict(geometry, z=list(reversed(geometry["z"])))):
+                    dict(geometry, tan_alpha=[0.0] * 12), dict(geometry, z=list(reversed(geometry["z"]))),
+                    dict(geometry, kick=0.0), dict(geometry, kick=float("inf")), dict(geometry, z_ref=float("nan"))):
         gg = bd._fill(bd.lf_geometry(), bad_geo)
         assert lib.lf_create(ctypes.byref(gg), ctypes.byref(p), 1, 1, 1, ctypes.byref(h)) == bd.LF_ERR_INVALID_ARG
     assert lib.lf_destroy(None) == bd.LF_OK

@@ -361,3 +361,34 @@ def test_garbage_inputs_are_memory_safe(lfmod, geometry, params):
                 assert r.hit_idx.min() >= -1 and r.hit_idx.max() < bb.n_hits
                 assert r.seed_idx.min() >= 0 and r.seed_idx.max() < bb.n_seeds
         lf.close()
+
+
+def test_two_live_handles_of_different_size(lfmod, oracle, geometry, params):
+    """The dynamic shared-memory limit is an attribute of the kernel function, not of a handle: creating a handle with a
+    smaller stage (or fewer triplets) after a large one must not break the large one."""
+    import torch
+    big = dg.generate_config(4, n_events=12)        # ~12 000 hits per event: the largest stage
+    small = dg.generate_config(0)
+    lf_big = lfmod.LookingForward(geometry, params, big.n_events, big.n_seeds, big.n_hits)
+    assert max(lf_big.info().smem_bytes) > 48 * 1024
+    lf_small = lfmod.LookingForward(geometry, dict(params, n_triplets=4), small.n_events, small.n_seeds, small.n_hits)
+    assert max(lf_small.info().smem_bytes) < max(lf_big.info().smem_bytes)
+    out_small = lf_small.run(lfmod.DeviceBatch(small))
+    out_big = lf_big.run(lfmod.DeviceBatch(big))    # needs the larger limit that lf_small's creation must not have lowered
+    torch.cuda.synchronize()
+    assert_tracks_equal(out_big.to_numpy(), oracle.run(geometry, params, big), "big handle after a small lf_create")
+    assert_tracks_equal(out_small.to_numpy(), oracle.run(geometry, dict(params, n_triplets=4), small), "small handle")
+    lf_small.close()
+    lf_big.close()
+
+
+def test_reversed_field(lfmod, oracle, params):
+    """kick < 0 with polarity -1 (C7): the same-bend filter follows the sign of kick * q/p."""
+    G = dg.toy_geometry(polarity=-1, kick_sign=-1.0)
+    cfg = dg.with_overrides(dg.CONFIGS[1], kick_sign=-1.0, p_min=1.5)
+    b = dg.generate(cfg, n_events=40)
+    ref = oracle.run(G, params, b, debug=True)
+    assert ref.n_tracks > 0.7 * (b.seed_track >= 0).sum()
+    got = _gpu_run(lfmod, G, params, b, debug=True)
+    assert_tracks_equal(got, ref, "reversed field")
+    assert_debug_equal(got.debug, ref.debug)
