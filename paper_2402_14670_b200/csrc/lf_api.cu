@@ -135,6 +135,7 @@ void make_consts(const lf_geometry& G, const lf_params& P, lf::Consts& c) {
     c.zmag_a[s] = c.z_mag - c.z[a];
     c.inv_r[s] = one / (c.inv_dz_ac[s] * c.zmag_a[s]); /* bracket of the h2 interval only (not a decision) */
     c.inv_abs_zmag_a[s] = one / std::fabs(c.zmag_a[s]);  /* idem */
+    c.tolmax_over_zmag[s] = P.mag_tol_max * c.inv_abs_zmag_a[s]; /* idem */
     c.D10[s] = c.d[b] - c.d[a];
     c.D20[s] = c.d[cc] - c.d[a];
     c.W10[s] = c.w[b] - c.w[a];
@@ -456,7 +457,7 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
     LF_CREATE_CUDA(cudaMalloc(&h->hx16, nh * sizeof(__half)));
     LF_CREATE_CUDA(cudaMalloc(&h->origin16, ((nh >> 5) + ne * lf::NSEG + 2) * sizeof(float)));
   }
-  LF_CREATE_CUDA(cudaMalloc(&h->win, nrows * lf::NL * sizeof(uint32_t)));
+  LF_CREATE_CUDA(cudaMalloc(&h->win, nrows * lf::WIN_ROW * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->trip_code, nrows * nt * code_bytes));
   LF_CREATE_CUDA(cudaMalloc(&h->n_trip, nrows));
   LF_CREATE_CUDA(cudaMalloc(&h->ws_rec, ns * lf::REC_WORDS * sizeof(int32_t)));
@@ -477,7 +478,7 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   LF_CREATE_CUDA(cudaMalloc(&h->validate_res, 4 * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->tickets, lf::N_TICKETS * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMemset(h->tickets, 0, lf::N_TICKETS * sizeof(uint32_t)));
-  h->workspace_bytes = nrows * (lf::NL * 4 + nt * (code_bytes + sizeof(uint4)) + 1) + ns * (lf::REC_WORDS + 3) * 4 +
+  h->workspace_bytes = nrows * (lf::WIN_ROW * 4 + nt * (code_bytes + sizeof(uint4)) + 1) + ns * (lf::REC_WORDS + 3) * 4 +
                        (4 * ne + 1 + lf::N_TICKETS) * sizeof(uint32_t) + (sizeof(lf::FitLut) << lf::NL);
 #undef LF_CREATE_CUDA
   *out = h;

@@ -38,6 +38,8 @@ namespace lf {
 
 constexpr int NL = 12;
 constexpr int NSEG = 24;
+constexpr int WIN_ROW = 16;    /* words per followed track in the window table: 12 packed windows + x_mag, tx, q/p, flags */
+constexpr uint32_t ROW_LOW_P = 1u; /* flags: the seed's momentum is below p_same_bend (filter 1 applies) */
 constexpr int REC_WORDS = 20;  /* 12 hit idx, seed, n_hits, 5 state, Q */
 constexpr int TRIP_BUF = 64;   /* per-warp triplet key buffer */
 constexpr int MAX_NT = 16;     /* == LF_MAX_TRIPLETS (narrow kernels) */
@@ -75,7 +77,7 @@ constexpr float INTERVAL_MARGIN = 0.1f; /* mm added to the magnet tolerance when
 struct Consts {
   float z[NL], tana[NL], inv_tan[NL], dzs[NL], dzm[NL], d[NL], w[NL];
   float z_seed, z_mag, kick, dr, K[2], poly[5], mag_dz_seed;
-  float inv_dz_ac[2], zmag_a[2], inv_r[2], inv_abs_zmag_a[2], D10[2], D20[2], W10[2], W20[2], inv_det[2], inv_D10[2];
+  float inv_dz_ac[2], zmag_a[2], inv_r[2], inv_abs_zmag_a[2], tolmax_over_zmag[2], D10[2], D20[2], W10[2], W20[2], inv_det[2], inv_D10[2];
   float dz_state, ds, ws, dws;
   int polarity;
   float T_triplet, T_x, T_uv_slope, T_uv_min, T_ty, inv_Tx, inv_Ty, T_Q, C_nhits[4];
@@ -114,7 +116,8 @@ struct EventArgs {
   int stage_cap;        /* floats of shared memory available for one event's hits */
   uint32_t* ticket;     /* this kernel's event ticket */
   /* per followed track ("row" = seed*sides + side; narrow kernels: row = seed) */
-  uint32_t* win;        /* n_rows*12: (first_in_event << WB) | count */
+  uint32_t* win;        /* n_rows*WIN_ROW: 12 x ((first_in_event << WB) | count), then x_mag, tx, q/p (mode 1: the assumed
+                           1/p), flags */
   void* trip_code;      /* n_rows*NT Fmt::code_t: set<<3IB | h0<<2IB | h2<<IB | h1 (window-relative), sorted */
   uint8_t* n_trip;      /* n_rows */
   int32_t* ws_rec;      /* n_seeds * REC_WORDS */
@@ -197,22 +200,26 @@ template <bool STAGED>
 struct HitView;
 template <>
 struct HitView<true> {
-  int off; /* skew of the event inside the stage buffer */
-  __device__ __forceinline__ float operator[](int i) const { return stage_buf()[off + i]; }
+  uint32_t base; /* shared-memory byte address of hit 0 of the event */
+  __device__ __forceinline__ explicit HitView(int skew) : base(smem_u32(stage_buf()) + 4u * (uint32_t)skew) {}
+  __device__ __forceinline__ float operator[](int i) const { return lds_f32(base + 4u * (uint32_t)i); }
   typedef uint32_t pos_t;
-  __device__ __forceinline__ pos_t pos(int i) const { return smem_u32(stage_buf()) + 4u * (uint32_t)(off + i); }
+  __device__ __forceinline__ pos_t pos(int i) const { return base + 4u * (uint32_t)i; }
   static __device__ __forceinline__ pos_t adv(pos_t p, int n) { return p + 4u * (uint32_t)n; }
   static __device__ __forceinline__ float before(pos_t p) { return lds_f32(p - 4u); } /* the hit in front of p */
+  static __device__ __forceinline__ float at(pos_t p) { return lds_f32(p); }
   static __device__ __forceinline__ int diff(pos_t a, pos_t b) { return (int)(a - b) >> 2; }
 };
 template <>
 struct HitView<false> {
   const float* p;
+  __device__ __forceinline__ explicit HitView(const float* first) : p(first) {}
   __device__ __forceinline__ float operator[](int i) const { return __ldg(p + i); }
   typedef const float* pos_t;
   __device__ __forceinline__ pos_t pos(int i) const { return p + i; }
   static __device__ __forceinline__ pos_t adv(pos_t q, int n) { return q + n; }
   static __device__ __forceinline__ float before(pos_t q) { return __ldg(q - 1); }
+  static __device__ __forceinline__ float at(pos_t q) { return __ldg(q); }
   static __device__ __forceinline__ int diff(pos_t a, pos_t b) { return (int)(a - b); }
 };
 
@@ -337,7 +344,7 @@ __device__ __forceinline__ int closest_hit(const HV& hx, int f, int n, float pre
 template <bool WIDE>
 __device__ __forceinline__ int closest_hit(const HitView<true>& hx, int f, int n, float pred, bool dup, float& dist) {
   if (n <= 0) return -1;
-  const uint32_t a = smem_u32(stage_buf()) + 4u * (uint32_t)(hx.off + f);
+  const uint32_t a = hx.base + 4u * (uint32_t)f;
   const uint32_t end = a + 4u * (uint32_t)n;
   uint32_t p = a;
 #pragma unroll
@@ -371,7 +378,7 @@ template <int G, bool WIDE>
 __device__ __forceinline__ void closest_group(const HitView<true>& hx, const uint32_t (&ww)[G], const float (&pred)[G],
                                               bool dup, int (&krel)[G], float (&dist)[G]) {
   const float INF = __int_as_float(0x7f800000);
-  const uint32_t base = smem_u32(stage_buf()) + 4u * (uint32_t)hx.off;
+  const uint32_t base = hx.base;
   uint32_t a[G], end[G], p[G];
 #pragma unroll
   for (int g = 0; g < G; ++g) {
@@ -499,7 +506,22 @@ __device__ __forceinline__ void windows_of_event(const Consts& C, const EventArg
       last = min(last, c + halfw);
     }
     if (WIDE && last < first) last = first;
-    A.win[row * NL + layer] = ((uint32_t)first << F::WB) | (uint32_t)(last - first);
+    A.win[row * WIN_ROW + layer] = ((uint32_t)first << F::WB) | (uint32_t)(last - first);
+    if (layer == 0) {
+      /* words 12..15 of the row: what the seeding kernel needs of the seed, so that it reads one 64-byte row */
+      float q3 = 0.0f;
+      uint32_t flags = 0u;
+      if (WIDE && C.mode == 1) {
+        const float s2 = tx * tx + ty * ty;
+        q3 = fminf(C.inv_p_min, sqrtf(s2 / (1.0f + s2)) * C.inv_pt_min); /* the assumed 1/p */
+      } else {
+        q3 = __ldg(A.sqop + seed);
+        const float pmom = 1.0f / fmaxf(fabsf(q3), 1e-6f);
+        flags = (pmom < C.p_same_bend) ? ROW_LOW_P : 0u;
+      }
+      *reinterpret_cast<uint4*>(A.win + row * WIN_ROW + NL) =
+          make_uint4(__float_as_uint(x + tx * C.mag_dz_seed), __float_as_uint(tx), __float_as_uint(q3), flags);
+    }
     if (DEBUG) {
       if (A.dbg.win_first) A.dbg.win_first[row * NL + layer] = (int32_t)(E.h0 + first);
       if (A.dbg.win_count) A.dbg.win_count[row * NL + layer] = last - first;
@@ -519,7 +541,7 @@ __device__ __forceinline__ void flag_equal_neighbours(const EventArgs& A, const 
 }
 
 template <bool DEBUG, bool WIDE>
-__global__ void __launch_bounds__(WIN_THREADS) lf_window_kernel(const __grid_constant__ Consts C,
+__global__ void __launch_bounds__(WIN_THREADS, 8) lf_window_kernel(const __grid_constant__ Consts C,
                                                                 const __grid_constant__ EventArgs A) {
   CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
   if (threadIdx.x == 0) mbar_init(&H.mbar, 1);
@@ -527,11 +549,11 @@ __global__ void __launch_bounds__(WIN_THREADS) lf_window_kernel(const __grid_con
   EventCtx E;
   while (fetch_event(A, phase, E)) {
     if (E.staged) {
-      flag_equal_neighbours(A, E, HitView<true>{E.skew});
-      windows_of_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>{E.skew});
+      flag_equal_neighbours(A, E, HitView<true>(E.skew));
+      windows_of_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>(E.skew));
     } else {
-      flag_equal_neighbours(A, E, HitView<false>{A.hx + E.h0});
-      windows_of_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>{A.hx + E.h0});
+      flag_equal_neighbours(A, E, HitView<false>(A.hx + E.h0));
+      windows_of_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>(A.hx + E.h0));
     }
   }
 }
@@ -539,13 +561,110 @@ __global__ void __launch_bounds__(WIN_THREADS) lf_window_kernel(const __grid_con
 /* ============================================================================================
  * a3: triplet seeding.  One warp per seed.
  * ============================================================================================ */
+/* Closest hit to `pred` in the non-empty x-sorted window [f, e) of at most 2^EDGE_STEPS - 1 hits, branch-free: first
+ * x >= pred by a binary search whose probes beyond the window read +inf, then the two neighbours; ties -> lower index
+ * (equal to a linear argmin with strict '<'; the walk over a run of equal distances runs only in events that hold two
+ * equal neighbouring hits).  Returns the event-relative index and, in `dist`, |x - pred| of that hit (x - pred and
+ * pred - x round to the same magnitude, so dist*dist is bit-identical to (x - pred)^2).  An empty window gives dist = +inf. */
+template <bool WIDE, class HV>
+__device__ __forceinline__ int closest_in_window(const HV& hx, int f, int e, float pred, bool dup, float& dist) {
+  typedef typename HV::pos_t pos_t;
+  const float INF = __int_as_float(0x7f800000);
+  const pos_t a = hx.pos(f), end = hx.pos(e);
+  pos_t p = a;
+#pragma unroll
+  for (int s = Fmt<WIDE>::EDGE_STEPS - 1; s >= 0; --s) {
+    const pos_t q = HV::adv(p, 1 << s);
+    if (q <= end && HV::before(q) < pred) p = q;
+  }
+  const float xl = (p > a) ? HV::before(p) : -INF;
+  const float xh = (p < end) ? HV::at(p) : INF;
+  const float dk = pred - xl, dh = xh - pred;
+  const bool right = !(dk <= dh); /* ties -> lower index */
+  pos_t k = right ? p : HV::adv(p, -1);
+  dist = right ? dh : dk;
+  if (dup && !right)
+    while (k > a && (pred - HV::before(k)) == dk) k = HV::adv(k, -1);
+  return f + HV::diff(k, a);
+}
+
+/* Per-warp scratch of the narrow seeding kernel: the passing triplets in candidate order, i.e. ascending
+ * (set, h0, h2): the chi2 bit pattern (non-negative floats order like their bit patterns) and the 16-bit code. */
 struct __align__(16) SeedScratch {
-  unsigned long long trip[TRIP_BUF];
+  uint32_t chi2[TRIP_BUF];
+  uint16_t code[TRIP_BUF];
+  int4 setw[2]; /* per layer set: first and end of the h1 window, first of the h2 window (event-relative) */
 };
 
-/* Rank selection on the warp's triplet keys: keeps the `keep` smallest of `n` (<= TRIP_BUF) unique
- * 64-bit keys and leaves them SORTED ascending in W.trip[0..min(n,keep)).  PAPER.md:221. */
+/* Rank selection on the warp's triplets: keeps the `keep` smallest of `n` (<= TRIP_BUF) by the key (chi2, position in the
+ * buffer) and leaves them SORTED ascending in W.chi2 / W.code [0, min(n, keep)).  The buffer is in candidate order and a
+ * selection keeps it ordered by the full key, so the position stands for the (set, h0, h2) part of the order key of
+ * DESIGN.md C9.  PAPER.md:221. */
+__device__ __forceinline__ int count_less4(const uint32_t* v, uint32_t c) {
+  const uint4 q = *reinterpret_cast<const uint4*>(v);
+  return ((q.x < c) ? 1 : 0) + ((q.y < c) ? 1 : 0) + ((q.z < c) ? 1 : 0) + ((q.w < c) ? 1 : 0);
+}
 __device__ __forceinline__ int select_smallest(SeedScratch& W, int n, int keep, int lane) {
+  const unsigned lt_mask = (1u << lane) - 1u;
+  if (n <= 32) {
+    /* P = 8, 16 or 32 key slots, 32 / P lanes per key: lane & (P-1) is the key, lane / P the part of the P slots it
+     * compares with (16-byte groups; the slots beyond n are padded with all-ones, which no passing chi2 equals) */
+    if (lane >= n) W.chi2[lane] = 0xFFFFFFFFu;
+    __syncwarp();
+    const int P = (n <= 8) ? 8 : ((n <= 16) ? 16 : 32);
+    const int key = lane & (P - 1);
+    const uint32_t c0 = W.chi2[key];
+    const uint16_t d0 = W.code[key];
+    int r;
+    if (n <= 8) {
+      const uint2 q = *reinterpret_cast<const uint2*>(&W.chi2[(lane >> 3) * 2]);
+      r = ((q.x < c0) ? 1 : 0) + ((q.y < c0) ? 1 : 0);
+      r += __shfl_xor_sync(FULL, r, 8);
+      r += __shfl_xor_sync(FULL, r, 16);
+    } else if (n <= 16) {
+      r = count_less4(&W.chi2[(lane >> 4) * 8], c0) + count_less4(&W.chi2[(lane >> 4) * 8 + 4], c0);
+      r += __shfl_xor_sync(FULL, r, 16);
+    } else {
+      r = 0;
+      for (int j = 0; j < n; j += 4) r += count_less4(&W.chi2[j], c0);
+    }
+    /* equal chi2: the earlier candidate first */
+    r += __popc(__match_any_sync(FULL, c0) & lt_mask & (unsigned)((1ull << P) - 1ull));
+    __syncwarp();
+    if (lane < n && r < keep) {
+      W.chi2[r] = c0;
+      W.code[r] = d0;
+    }
+  } else {
+    const uint32_t c0 = W.chi2[lane];
+    const uint16_t d0 = W.code[lane];
+    const uint32_t c1 = (lane + 32 < n) ? W.chi2[lane + 32] : 0xFFFFFFFFu;
+    const uint16_t d1 = W.code[lane + 32];
+    int r0 = 0, r1 = 0;
+    for (int j = 0; j < n; ++j) {
+      const uint32_t cj = W.chi2[j];
+      r0 += (cj < c0 || (cj == c0 && j < lane)) ? 1 : 0;
+      r1 += (cj < c1 || (cj == c1 && j < lane + 32)) ? 1 : 0;
+    }
+    __syncwarp();
+    if (r0 < keep) {
+      W.chi2[r0] = c0;
+      W.code[r0] = d0;
+    }
+    if (lane + 32 < n && r1 < keep) {
+      W.chi2[r1] = c1;
+      W.code[r1] = d1;
+    }
+  }
+  __syncwarp();
+  return n < keep ? n : keep;
+}
+
+/* The same on 64-bit keys (chi2 bits, code): the wide build. */
+struct __align__(16) SeedScratch64 {
+  unsigned long long trip[TRIP_BUF];
+};
+__device__ __forceinline__ int select_smallest(SeedScratch64& W, int n, int keep, int lane) {
   const unsigned long long k0 = (lane < n) ? W.trip[lane] : ~0ull;
   const unsigned long long k1 = (lane + 32 < n) ? W.trip[lane + 32] : ~0ull;
   int r0 = 0, r1 = 0;
@@ -569,60 +688,90 @@ __device__ __forceinline__ int select_smallest(SeedScratch& W, int n, int keep, 
  * (INCLUSIVE == false) or <= v (true): binary search by shuffles, every lane with its own v. */
 template <bool INCLUSIVE>
 __device__ __forceinline__ int lanes_below(float xv, float v) {
-  int pos = 0;
+  int probe = 15; /* the lane probed next = count so far + step - 1 (one update per step instead of two) */
 #pragma unroll
-  for (int s = 16; s >= 1; s >>= 1) {
-    const float xm = __shfl_sync(FULL, xv, pos + s - 1);
-    if (INCLUSIVE ? (xm <= v) : (xm < v)) pos += s;
+  for (int s = 16; s >= 2; s >>= 1) {
+    const float xm = __shfl_sync(FULL, xv, probe);
+    const bool c = INCLUSIVE ? (xm <= v) : (xm < v);
+    probe += (c ? s : 0) - (s >> 1);
   }
-  const float xm = __shfl_sync(FULL, xv, pos); /* pos <= 31 here */
-  if (INCLUSIVE ? (xm <= v) : (xm < v)) pos += 1;
-  return pos;
+#pragma unroll
+  for (int r = 0; r < 2; ++r) { /* step 1, then the 32nd lane: probe == count <= 31 */
+    const float xm = __shfl_sync(FULL, xv, probe);
+    if (INCLUSIVE ? (xm <= v) : (xm < v)) probe += 1;
+  }
+  return probe;
 }
 
+/* Per layer set: the constants a candidate doublet needs (shared memory, one 32-byte row per set, so that a lane
+ * whose candidate belongs to either set fetches them with two 16-byte loads instead of a select per constant). */
+struct __align__(16) SetConsts {
+  float inv_dz, zmag_a, zb, za;
+  float K, pad0, pad1, pad2;
+};
+__device__ __forceinline__ void fill_set_consts(const Consts& C, SetConsts* sc) {
+  if (threadIdx.x < 2) {
+    const int s = threadIdx.x;
+    sc[s].inv_dz = C.inv_dz_ac[s];
+    sc[s].zmag_a = C.zmag_a[s];
+    sc[s].zb = C.z[s ? 7 : 4];
+    sc[s].za = C.z[s ? 3 : 0];
+    sc[s].K = C.K[s];
+    sc[s].pad0 = sc[s].pad1 = sc[s].pad2 = 0.0f;
+  }
+}
+
+struct SeedEventPtrs { /* the event's slices of the per-row tables */
+  const uint32_t* rows;
+  uint16_t* codes;
+  uint8_t* n_trip;
+  uint32_t s0;
+};
 template <bool DEBUG, class HV>
 __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& A, const HV& hx, uint32_t h0,
-                                              uint32_t seed, SeedScratch& W, int lane, bool dup) {
-  const float x = __ldg(A.sx + seed), tx = __ldg(A.stx + seed), qop = __ldg(A.sqop + seed);
+                                              const SeedEventPtrs& EP, uint32_t k_seed, SeedScratch& W, const SetConsts* SC,
+                                              int lane, bool dup) {
+  constexpr bool STG = std::is_same<HV, HitView<true> >::value; /* staged hits: reading past a window is harmless */
+  const uint32_t* rowp = EP.rows + k_seed * WIN_ROW;
+  /* the seed's row of the window table: lanes 0..11 hold the packed window of layer `lane`, lanes 12..15 x_mag, tx,
+   * q/p and the flags (written by the window kernel) */
+  const uint32_t winw = (lane < WIN_ROW) ? rowp[lane] : 0u;
+  const float x_mag = __uint_as_float(__shfl_sync(FULL, winw, 12)), tx = __uint_as_float(__shfl_sync(FULL, winw, 13));
+  const float qop = __uint_as_float(__shfl_sync(FULL, winw, 14));
+  const bool low_p = (__shfl_sync(FULL, winw, 15) & ROW_LOW_P) != 0u;
   const float aq = fmaxf(fabsf(qop), 1e-6f);
-  const float p = 1.0f / aq;
   const float kq = C.kick * qop; /* expected slope change across the magnet (Eq. 2) */
-  const float x_mag = x + tx * C.mag_dz_seed;
-  /* lanes 0..11 hold the packed window of layer `lane` */
-  const uint32_t winw = (lane < NL) ? A.win[(size_t)seed * NL + lane] : 0u;
   const unsigned lt_mask = (1u << lane) - 1u;
-  const bool low_p = p < C.p_same_bend;
   const float tol0 = C.mag_tol_base + C.mag_tol_inv_p * aq;
   const float INF = __int_as_float(0x7f800000);
   /* ---- per layer set: lanes = h0.  |x0 + t*zmag_a - x_mag| < tol is linear in x2 (t = (x2-x0)*inv_dz, slope
    * r = inv_dz*zmag_a < 0) and tol <= tol_sup (tol is monotone in |t|), so the survivors lie inside
    * x2 in [x0 + (tol_sup - A)/r, x0 + (-tol_sup - A)/r], A = x0 - x_mag.  The margin in tol_sup (0.1 mm >> fp32
-   * rounding of these expressions) makes the bracket a strict superset; the h2 window sits one hit per lane,
-   * so both bracket ends are shuffle searches. */
+   * rounding of these expressions, which may therefore use fused multiply-adds: they bracket, they do not decide)
+   * makes the bracket a strict superset; the h2 window sits one hit per lane, so both bracket ends are shuffle
+   * searches. */
+  const float tol0m = tol0 + INTERVAL_MARGIN, tolmaxm = C.mag_tol_max + INTERVAL_MARGIN;
   float x0s[2];
-  int fbs[2], nbs[2], fcs[2];
   unsigned cnt_p = 0, jlo_p = 0; /* set 0 in the low half-word, set 1 in the high one */
 #pragma unroll
   for (int set = 0; set < 2; ++set) {
     const int la = set ? 3 : 0;
     const uint32_t wa = __shfl_sync(FULL, winw, la), wb = __shfl_sync(FULL, winw, la + 4), wc = __shfl_sync(FULL, winw, la + 8);
-    const int fa = (int)(wa >> 6), na = (int)(wa & 63u), nc = (int)(wc & 63u);
-    fbs[set] = (int)(wb >> 6);
-    nbs[set] = (int)(wb & 63u);
-    fcs[set] = (int)(wc >> 6);
-    x0s[set] = 0.0f;
-    if (na == 0 || nbs[set] == 0 || nc == 0) continue; /* warp-uniform */
-    const float inv_r = C.inv_r[set];
-    const bool have = lane < na;
-    const float x0 = have ? hx[fa + lane] : 0.0f;
-    const float x2v = (lane < nc) ? hx[fcs[set] + lane] : INF;
+    const int fa = (int)(wa >> 6), na = (int)(wa & 63u), fb = (int)(wb >> 6), nb = (int)(wb & 63u);
+    const int fc = (int)(wc >> 6), nc = (int)(wc & 63u);
+    if (lane == set) W.setw[set] = make_int4(fb, fb + nb, fc, 0);
+    const bool have = (lane < na) && (nb != 0); /* no h1 hit, no triplet */
+    const float x0 = (STG || lane < na) ? hx[fa + lane] : 0.0f;
+    const float x2r = (STG || lane < nc) ? hx[fc + lane] : 0.0f;
+    const float x2v = (lane < nc) ? x2r : INF;
     /* a survivor has |A + t*zmag_a| < tol <= tol_max, so |t| <= (|A| + tol_max)/|zmag_a| =: tmax */
     const float Aoff = x0 - x_mag;
-    const float tmax = (fabsf(Aoff) + C.mag_tol_max) * C.inv_abs_zmag_a[set];
-    const float tol_sup = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * tmax) + INTERVAL_MARGIN;
-    const int jlo = lanes_below<false>(x2v, x0 + (tol_sup - Aoff) * inv_r);  /* first x2 >= lower end */
-    const int jhi = min(nc, lanes_below<true>(x2v, x0 + (-tol_sup - Aoff) * inv_r));  /* first x2 > upper end; the +inf
-                                                                                       padding lanes are not hits */
+    const float tmax = __fmaf_rn(fabsf(Aoff), C.inv_abs_zmag_a[set], C.tolmax_over_zmag[set]);
+    const float tol_sup = fminf(tolmaxm, __fmaf_rn(C.mag_tol_tx, tmax, tol0m));
+    const float inv_r = C.inv_r[set];
+    const int jlo = lanes_below<false>(x2v, __fmaf_rn(tol_sup - Aoff, inv_r, x0));           /* first x2 >= lower end */
+    const int jhi = min(nc, lanes_below<true>(x2v, __fmaf_rn(-tol_sup - Aoff, inv_r, x0)));  /* first x2 > upper end; the
+                                                                                     +inf padding lanes are not hits */
     const int cnt = have ? max(jhi - jlo, 0) : 0;
     x0s[set] = x0;
     cnt_p |= (unsigned)cnt << (16 * set);
@@ -637,6 +786,7 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
   }
   const unsigned tot_p = __shfl_sync(FULL, incl_p, 31);
   const int total0 = (int)(tot_p & 0xFFFFu), total = total0 + (int)(tot_p >> 16);
+  __syncwarp(); /* W.setw */
   int tcount = 0;
   for (int base = 0; base < total; base += 32) {
     const int tau = base + lane;
@@ -644,13 +794,17 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
     const int set = (tau >= total0) ? 1 : 0;
     const int ts = set ? tau - total0 : tau;
     const unsigned sel = set ? 0x4432u : 0x4410u; /* __byte_perm selector: this set's half-word */
-    int owner = 0; /* number of lanes whose inclusive count is <= ts == the h0 lane owning candidate ts */
+    int owner = 15; /* ends as the number of lanes whose inclusive count is <= ts == the h0 lane owning candidate ts;
+                       meanwhile the lane probed next (count so far + step - 1) */
 #pragma unroll
-    for (int s = 16; s >= 1; s >>= 1) {
-      const unsigned v = __shfl_sync(FULL, incl_p, owner + s - 1);
-      if ((int)__byte_perm(v, 0u, sel) <= ts) owner += s;
+    for (int s = 16; s >= 2; s >>= 1) {
+      const unsigned v = __shfl_sync(FULL, incl_p, owner);
+      owner += (((int)__byte_perm(v, 0u, sel) <= ts) ? s : 0) - (s >> 1);
     }
-    owner = min(owner, 31);
+    {
+      const unsigned v = __shfl_sync(FULL, incl_p, owner);
+      if ((int)__byte_perm(v, 0u, sel) <= ts) owner += 1;
+    }
     const unsigned ip = __shfl_sync(FULL, incl_p, owner), cp = __shfl_sync(FULL, cnt_p, owner);
     const unsigned jp = __shfl_sync(FULL, jlo_p, owner);
     const int before = (int)__byte_perm(ip, 0u, sel) - (int)__byte_perm(cp, 0u, sel);
@@ -658,36 +812,39 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
     const float xa = __shfl_sync(FULL, x0s[0], owner), xb = __shfl_sync(FULL, x0s[1], owner);
     const float x0o = set ? xb : xa;
     bool pass = false;
-    unsigned long long key = 0;
+    uint32_t chi2b = 0u, code = 0u;
     if (act) {
       /* the exact predicate is the definition */
-      const int fb = set ? fbs[1] : fbs[0], nb = set ? nbs[1] : nbs[0], fc = set ? fcs[1] : fcs[0];
-      const float inv_dz = set ? C.inv_dz_ac[1] : C.inv_dz_ac[0], zmag_a = set ? C.zmag_a[1] : C.zmag_a[0];
-      const float x2 = hx[fc + j];
-      const float t = (x2 - x0o) * inv_dz;
+      const float4 ca = *reinterpret_cast<const float4*>(&SC[set].inv_dz); /* inv_dz, zmag_a, zb, za */
+      const int4 wv = W.setw[set];                                        /* fb, fb + nb, fc */
+      const float x2 = hx[wv.z + j];
+      const float t = (x2 - x0o) * ca.x;
       bool ok = true;
       if (low_p) ok = (t - tx) * kq > 0.0f; /* filter 1: same bending direction as the expected kick */
-      const float x_at_mag = x0o + t * zmag_a;
+      const float x_at_mag = x0o + t * ca.y;
       const float tol = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * fabsf(t));
       ok = ok && (fabsf(x_at_mag - x_mag) < tol); /* filter 2: opening at the magnet centre */
       if (ok) {
         /* x1_expected, closest h1, chi2 cut */
-        const float zb = set ? C.z[7] : C.z[4], za = set ? C.z[3] : C.z[0], Kx1 = set ? C.K[1] : C.K[0];
-        const float x1e = zb * t + (x0o - t * za) * Kx1;
+        const float x1e = ca.z * t + (x0o - t * ca.w) * SC[set].K;
         float dx;
-        const int k = closest_hit<false>(hx, fb, nb, x1e, dup, dx);
+        const int k = closest_in_window<false>(hx, wv.x, wv.y, x1e, dup, dx);
         const float chi2 = dx * dx;
         if (chi2 < C.T_triplet) {
           pass = true;
-          key = ((unsigned long long)__float_as_uint(chi2) << 32) |
-                (unsigned)((set << 15) | (owner << 10) | (j << 5) | (k - fb));
+          chi2b = __float_as_uint(chi2);
+          code = (unsigned)((set << 15) | (owner << 10) | (j << 5) | (k - wv.x));
         }
       }
     }
     const unsigned m = __ballot_sync(FULL, pass);
     if (m) {
       if (tcount > 32) tcount = select_smallest(W, tcount, C.n_triplets, lane);
-      if (pass) W.trip[tcount + __popc(m & lt_mask)] = key;
+      if (pass) {
+        const int slot = tcount + __popc(m & lt_mask);
+        W.chi2[slot] = chi2b;
+        W.code[slot] = (uint16_t)code;
+      }
       tcount += __popc(m);
       __syncwarp();
     }
@@ -695,12 +852,12 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
   if (tcount > 0) tcount = select_smallest(W, tcount, C.n_triplets, lane); /* sorted in (chi2,set,h0,h2) order */
   const int ntr = tcount;
   const int NT = C.n_triplets;
-  if (lane == 0) A.n_trip[seed] = (uint8_t)ntr;
+  if (lane == 0) EP.n_trip[k_seed] = (uint8_t)ntr;
   const bool mine = lane < ntr;
-  const unsigned long long key = mine ? W.trip[lane] : 0ull;
-  if (lane < NT) static_cast<uint16_t*>(A.trip_code)[(size_t)seed * NT + lane] = (uint16_t)((unsigned)key & 0xFFFFu);
+  const unsigned low = mine ? (unsigned)W.code[lane] : 0u;
+  if (lane < NT) EP.codes[k_seed * (uint32_t)NT + (uint32_t)lane] = (uint16_t)low;
   if (DEBUG) {
-    const unsigned low = (unsigned)key;
+    const size_t seed = (size_t)EP.s0 + k_seed;
     const int set = (low >> 15) & 1, la = set ? 3 : 0;
     const int fa = (int)(__shfl_sync(FULL, winw, la) >> 6), fb = (int)(__shfl_sync(FULL, winw, la + 4) >> 6);
     const int fc = (int)(__shfl_sync(FULL, winw, la + 8) >> 6);
@@ -708,7 +865,7 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
     if (lane < NT) {
       const size_t o = (size_t)seed * NT + lane;
       if (A.dbg.trip_set) A.dbg.trip_set[o] = mine ? set : -1;
-      if (A.dbg.trip_chi2) A.dbg.trip_chi2[o] = mine ? __uint_as_float((unsigned)(key >> 32)) : -1.0f;
+      if (A.dbg.trip_chi2) A.dbg.trip_chi2[o] = mine ? __uint_as_float(W.chi2[lane]) : -1.0f;
       if (A.dbg.trip_hits) {
         A.dbg.trip_hits[o * 3 + 0] = mine ? (int32_t)(h0 + fa + ((low >> 10) & 31)) : -1;
         A.dbg.trip_hits[o * 3 + 1] = mine ? (int32_t)(h0 + fb + (low & 31)) : -1;
@@ -733,7 +890,7 @@ struct __align__(16) SeedScratchWide {
   uint32_t jx[128];   /* first h2 index of the bracket | candidates before the entry << 8 */
   float x0[128];
 };
-__device__ __forceinline__ SeedScratch& trip_part(SeedScratchWide& W) { return *reinterpret_cast<SeedScratch*>(W.trip); }
+__device__ __forceinline__ SeedScratch64& trip_part(SeedScratchWide& W) { return *reinterpret_cast<SeedScratch64*>(W.trip); }
 
 template <bool DEBUG, class HV>
 __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventArgs& A, const HV& hx, uint32_t h0,
@@ -756,7 +913,7 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
   }
   const float p = 1.0f / aq;
   const float x_mag = x + tx * C.mag_dz_seed;
-  const uint32_t winw = (lane < NL) ? A.win[row * NL + lane] : 0u;
+  const uint32_t winw = (lane < NL) ? A.win[row * WIN_ROW + lane] : 0u;
   const unsigned lt_mask = (1u << lane) - 1u;
   const bool low_p = !no_ut && (p < C.p_same_bend);
   const float tol0 = C.mag_tol_base + C.mag_tol_inv_p * aq;
@@ -806,7 +963,7 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
   __syncwarp();
   /* ---- dense lane-per-candidate evaluation over all groups */
   int tcount = 0;
-  SeedScratch& WT = trip_part(W);
+  SeedScratch64& WT = trip_part(W);
   for (int base = 0; base < total; base += 32) {
     const int tau = base + lane;
     const bool act = tau < total;
@@ -884,6 +1041,7 @@ template <bool WIDE>
 struct __align__(16) SeedTables {
   int next_seed;
   int pad[3];
+  SetConsts sc[2];
   typename std::conditional<WIDE, SeedScratchWide, SeedScratch>::type ws[SEED_WARPS];
 };
 
@@ -897,6 +1055,7 @@ __global__ void __launch_bounds__(SEED_THREADS, WIDE ? 4 : 5) lf_seed_kernel(con
     mbar_init(&H.mbar, 1);
     T.next_seed = 0;
   }
+  fill_set_consts(C, T.sc); /* published by fetch_event's barriers */
   uint32_t phase = 0;
   EventCtx E;
   while (fetch_event(A, phase, E)) {
@@ -905,21 +1064,27 @@ __global__ void __launch_bounds__(SEED_THREADS, WIDE ? 4 : 5) lf_seed_kernel(con
     const int n_rows = (int)(s1 - s0) * sides;
     auto& W = T.ws[warp];
     const bool dup = H.dup != 0;
-    for (;;) { /* the warps of the CTA share the event's rows, two per ticket */
+    constexpr int PER_TICKET = WIDE ? 2 : 4;
+    SeedEventPtrs EP;
+    EP.rows = A.win + (size_t)s0 * WIN_ROW;
+    EP.codes = static_cast<uint16_t*>(A.trip_code) + (size_t)s0 * C.n_triplets; /* narrow build only */
+    EP.n_trip = A.n_trip + s0;
+    EP.s0 = s0;
+    for (;;) { /* the warps of the CTA share the event's rows, a few per ticket */
       int k = 0;
-      if (lane == 0) k = atomicAdd(&T.next_seed, 2);
+      if (lane == 0) k = atomicAdd(&T.next_seed, PER_TICKET);
       k = __shfl_sync(FULL, k, 0);
       if (k >= n_rows) break;
-      const int kend = min(k + 2, n_rows);
+      const int kend = min(k + PER_TICKET, n_rows);
       for (; k < kend; ++k) {
         if constexpr (WIDE) {
           const uint32_t seed = s0 + (uint32_t)(k / sides);
           const int side = k - (k / sides) * sides;
-          if (E.staged) seed_triplets_wide<DEBUG>(C, A, HitView<true>{E.skew}, E.h0, seed, side, W, lane, dup);
-          else seed_triplets_wide<DEBUG>(C, A, HitView<false>{A.hx + E.h0}, E.h0, seed, side, W, lane, dup);
+          if (E.staged) seed_triplets_wide<DEBUG>(C, A, HitView<true>(E.skew), E.h0, seed, side, W, lane, dup);
+          else seed_triplets_wide<DEBUG>(C, A, HitView<false>(A.hx + E.h0), E.h0, seed, side, W, lane, dup);
         } else {
-          if (E.staged) seed_triplets<DEBUG>(C, A, HitView<true>{E.skew}, E.h0, s0 + (uint32_t)k, W, lane, dup);
-          else seed_triplets<DEBUG>(C, A, HitView<false>{A.hx + E.h0}, E.h0, s0 + (uint32_t)k, W, lane, dup);
+          if (E.staged) seed_triplets<DEBUG>(C, A, HitView<true>(E.skew), E.h0, EP, (uint32_t)k, W, T.sc, lane, dup);
+          else seed_triplets<DEBUG>(C, A, HitView<false>(A.hx + E.h0), E.h0, EP, (uint32_t)k, W, T.sc, lane, dup);
         }
       }
     }
@@ -1059,7 +1224,8 @@ __device__ __forceinline__ void extend_event(const Consts& C, const EventArgs& A
     const int cn = min(FIT_CHUNK, nr - cb);
     const size_t rbase = row0 + (size_t)cb;
     /* ---- stage the chunk's windows, seed parameters and candidate counts */
-    for (int i = tid; i < cn * NL; i += FIT_THREADS) T.win[i] = A.win[rbase * NL + i];
+    for (int i = tid; i < cn * WIN_ROW; i += FIT_THREADS)
+      if ((i & (WIN_ROW - 1)) < NL) T.win[(i >> 4) * NL + (i & (WIN_ROW - 1))] = A.win[rbase * WIN_ROW + i];
     int my_n = 0;
     if (tid < cn) {
       const size_t row = rbase + (size_t)tid;
@@ -1170,8 +1336,8 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_extend_kernel(const __grid_
   uint32_t phase = 0;
   EventCtx E;
   while (fetch_event(A, phase, E)) {
-    if (E.staged) extend_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>{E.skew}, T);
-    else extend_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>{A.hx + E.h0}, T);
+    if (E.staged) extend_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>(E.skew), T);
+    else extend_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>(A.hx + E.h0), T);
   }
 }
 
@@ -1255,7 +1421,7 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
     unsigned long long key = ~0ull;
     if (mine) {
       const size_t row = (size_t)seed * sides + side;
-      const uint4* wp = reinterpret_cast<const uint4*>(A.win + row * NL);
+      const uint4* wp = reinterpret_cast<const uint4*>(A.win + row * WIN_ROW);
       const uint4 w0 = __ldg(wp), w1 = __ldg(wp + 1), w2 = __ldg(wp + 2);
       wf[0] = w0.x; wf[1] = w0.y; wf[2] = w0.z; wf[3] = w0.w; wf[4] = w1.x; wf[5] = w1.y; wf[6] = w1.z; wf[7] = w1.w;
       wf[8] = w2.x; wf[9] = w2.y; wf[10] = w2.z; wf[11] = w2.w;
@@ -1414,8 +1580,8 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_fit_kernel(const __grid_con
   uint32_t phase = 0;
   EventCtx E;
   while (fetch_event(A, phase, E)) {
-    if (E.staged) fit_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>{E.skew}, T);
-    else fit_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>{A.hx + E.h0}, T);
+    if (E.staged) fit_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>(E.skew), T);
+    else fit_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>(A.hx + E.h0), T);
   }
 }
 
