@@ -60,9 +60,10 @@ struct Fmt {
   static constexpr int EDGE_STEPS = WIDE ? 7 : 6;     /* window-edge searches span n_window + 1 hits */
   static constexpr uint32_t TOPB = WIDE ? 256u : 128u; /* first stride (bytes) of a search inside one window */
   static constexpr int KB = WIDE ? 5 : 4;             /* bits of the triplet index k */
-  static constexpr int SIE_BITS = WIDE ? 26 : 28;     /* record tag: seed inside the event | side << 26 | k << 27 (wide) */
+  /* tag of a candidate record: seed inside the event | layer set << 25 | window side << 26 | k << 27 */
+  static constexpr int SIE_BITS = 25;
   static constexpr uint32_t SIE = (1u << SIE_BITS) - 1u;
-  static constexpr int K_SHIFT = WIDE ? 27 : 28;
+  static constexpr int SET_SHIFT = 25, SIDE_SHIFT = 26, K_SHIFT = 27;
   typedef typename std::conditional<WIDE, uint32_t, uint16_t>::type code_t; /* stored triplet code */
 };
 constexpr int SEED_WARPS = 8;
@@ -126,8 +127,8 @@ struct EventArgs {
   int32_t* ws_event;    /* n_seeds: event of the seed */
   uint32_t* ev_count;   /* n_events */
   uint4* acc_rec;       /* n_rows*NT: candidates that passed the hit-count rule: 3 words of hit codes (byte l = hit of
-                           layer l inside its window, 0xFF = none), then the tag seed inside the event | k << 28
-                           (wide: | side << 26 | k << 27); dense per event */
+                           layer l inside its window, 0xFF = none), then the tag seed inside the event | layer set << 25 |
+                           window side << 26 | k << 27; dense per event */
   uint32_t* ev_acc;     /* n_events: number of such records of the event */
   const struct FitLut* fit_lut; /* 4096: per presence mask */
   uint32_t* ev_dup;     /* n_events: written by the window kernel, != 0 if two neighbouring staged hits are equal */
@@ -1070,12 +1071,19 @@ __global__ void __launch_bounds__(SEED_THREADS, WIDE ? 4 : 5) lf_seed_kernel(con
     EP.codes = static_cast<uint16_t*>(A.trip_code) + (size_t)s0 * C.n_triplets; /* narrow build only */
     EP.n_trip = A.n_trip + s0;
     EP.s0 = s0;
-    for (;;) { /* the warps of the CTA share the event's rows, a few per ticket */
-      int k = 0;
-      if (lane == 0) k = atomicAdd(&T.next_seed, PER_TICKET);
-      k = __shfl_sync(FULL, k, 0);
+    /* the warps read one 64-byte row per followed track: pull the event's rows (two per 128-byte line) into L1 now */
+    for (int i = threadIdx.x * 2; i < n_rows; i += SEED_THREADS * 2)
+      asm volatile("prefetch.global.L1 [%0];" ::"l"(A.win + ((size_t)s0 * sides + i) * WIN_ROW));
+    /* the warps of the CTA share the event's rows by tickets: PER_TICKET rows each while many are left, single rows for
+     * the last 24, so that the warps reach the end of the event together */
+    const int n_big = max(n_rows - 24, 0) / PER_TICKET;
+    for (;;) {
+      int t = 0;
+      if (lane == 0) t = atomicAdd(&T.next_seed, 1);
+      t = __shfl_sync(FULL, t, 0);
+      int k = (t < n_big) ? t * PER_TICKET : n_big * PER_TICKET + (t - n_big);
       if (k >= n_rows) break;
-      const int kend = min(k + PER_TICKET, n_rows);
+      const int kend = (t < n_big) ? k + PER_TICKET : k + 1;
       for (; k < kend; ++k) {
         if constexpr (WIDE) {
           const uint32_t seed = s0 + (uint32_t)(k / sides);
@@ -1279,8 +1287,9 @@ __device__ __forceinline__ void extend_event(const Consts& C, const EventArgs& A
         enough = h.enough;
         /* seed inside the event, (side,) candidate index */
         const int re = cb + rl;
-        tag = WIDE ? ((unsigned)(re / sides) | ((unsigned)(re - (re / sides) * sides) << F::SIE_BITS) | ((unsigned)k << F::K_SHIFT))
-                   : ((unsigned)re | ((unsigned)k << F::K_SHIFT));
+        const unsigned set_bit = ((code >> (3 * F::IB)) & 1u) << F::SET_SHIFT;
+        tag = WIDE ? ((unsigned)(re / sides) | set_bit | ((unsigned)(re - (re / sides) * sides) << F::SIDE_SHIFT) | ((unsigned)k << F::K_SHIFT))
+                   : ((unsigned)re | set_bit | ((unsigned)k << F::K_SHIFT));
         if (DEBUG) {
           if (A.dbg.cand_hits)
             for (int l = 0; l < NL; ++l) {
@@ -1395,10 +1404,12 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
     const int t = b + tid;
     const bool have = t < n_acc;
     const uint4 r = have ? __ldg(rec + t) : make_uint4(0, 0, 0, 0xFFFFFFFFu);
+    if (t + FIT_THREADS < n_acc) /* the next pass starts at most FIT_THREADS records further: pull its lines into L1 */
+      asm volatile("prefetch.global.L1 [%0];" ::"l"(rec + t + FIT_THREADS));
     const unsigned sie = r.w & SIE;
     const int k = (int)(r.w >> F::K_SHIFT);
     /* wide: the records of a seed's sides are adjacent (side 0 first) and compete for the seed's track */
-    const int side = WIDE ? (int)((r.w >> F::SIE_BITS) & 1u) : 0;
+    const int side = WIDE ? (int)((r.w >> F::SIDE_SHIFT) & 1u) : 0;
     unsigned prev_sie = __shfl_up_sync(FULL, sie, 1);
     if (lane == 0) prev_sie = (tid > 0 && have) ? (__ldg(&rec[t - 1].w) & SIE) : 0xFFFFFFFEu;
     /* a seed whose records continue in the next pass is left to that pass (a seed has < FIT_THREADS records) */
@@ -1411,6 +1422,16 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
     if (lane == 0) wc[warp] = __popc(chg);
     __syncthreads();
     if (tid == 0) T.next_b[parity ^ 1] = 0x7FFFFFFF; /* re-armed for the next pass; its readers are past the barrier */
+    if (nxt_sie != 0xFFFFFFFEu && tid < 96) {
+      /* the next pass fits seeds nxt_sie, nxt_sie + 1, ...: pull their window rows (two per 128-byte line) and seed
+       * parameters towards L1 while this pass computes */
+      const uint32_t ps = s0 + nxt_sie;
+      const void* pf;
+      if (tid < 64) pf = A.win + ((size_t)ps * sides + 2 * tid) * WIN_ROW;
+      else pf = ((tid < 72) ? A.sy : ((tid < 80) ? A.stx : A.sty)) + ps + 32 * (tid & 7);
+      const bool inside = (tid < 64) ? (ps * sides + 2 * tid < s1 * sides) : (ps + 32 * (tid & 7) < s1);
+      if (inside) asm volatile("prefetch.global.L1 [%0];" ::"l"(pf));
+    }
     int slot = __popc(chg & ((2u << lane) - 1u)) - 1;
 #pragma unroll
     for (int wq = 0; wq < FIT_THREADS / 32; ++wq) slot += (wq < warp) ? wc[wq] : 0;
@@ -1428,7 +1449,6 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
       y = __ldg(A.sy + seed);
       tx = __ldg(A.stx + seed);
       ty = __ldg(A.sty + seed);
-      const unsigned code = static_cast<const typename F::code_t*>(A.trip_code)[row * NT + k];
       CandHits h;
       h.w[0] = r.x; h.w[1] = r.y; h.w[2] = r.z;
       unsigned mask = 0;
@@ -1441,7 +1461,7 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
       n = __popc(mask);
       const int n_uv = __popc(mask & 0x666u);
       {
-        const int set = (code >> (3 * F::IB)) & 1;
+        const int set = (int)((r.w >> F::SET_SHIFT) & 1u);
         const float x0 = hx[(int)(set ? wf[3] : wf[0])], x1 = hx[(int)(set ? wf[7] : wf[4])], x2 = hx[(int)(set ? wf[11] : wf[8])];
         const float X10 = x1 - x0, X20 = x2 - x0;
         const float D10 = set ? C.D10[1] : C.D10[0], D20 = set ? C.D20[1] : C.D20[0];
