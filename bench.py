@@ -9,9 +9,14 @@ Run-3-like occupancy, fp32, a single lf_run on one stream).  Prints ONE JSON lin
 
   value        events/s with inputs resident in HBM (CUDA events around the K steps, max over ranks)
   e2e          the same metric through lf_run_host: pinned HOST buffers, H2D + D2H inside the timing
-  roofline     dominant kernel (the slowest event kernel), timed live with CUDA events on the launching stream:
-               "bound": "alu" = warp-instruction issue rate vs 148 SMs x 4 schedulers x clock (what bounds the path,
-               DESIGN.md section 7); roofline.hbm = algorithmic bytes per launch / duration vs MEASURED_PEAKS.json hbm_gbs
+  roofline     the HBM roofline BASELINE.json's metric names, for the dominant kernel (the slowest event kernel, timed
+               live with CUDA events on the launching stream): algorithmic bytes per launch / duration vs the measured
+               copy bandwidth of MEASURED_PEAKS.json; "traffic" = DRAM bytes per launch from the committed ncu capture
+               when that capture was taken on this very source (sha256 stamp), else null
+  alu_algorithmic_frac  ALGORITHMIC lane-operations per step (the committed model of DESIGN.md section 7, evaluated on this
+               batch's own work counters) / step time / (148 SMs x 128 lanes x sm_max_mhz)
+  issue_utilisation     EXECUTED warp-instructions of the dominant kernel (ncu capture, same sha256 stamp) / its live time /
+               (148 SMs x 4 schedulers x sm_max_mhz): how busy the issue slots are, not a roofline fraction
   cpu_baseline the oracle, as it stands, on the box's host cores on a bounded sample (rank 0, N=1)
 
 --impl reference times the oracle (all host cores via the harness's event sharding) on a bounded
@@ -108,6 +113,57 @@ class ClockSampler:
                     "source": "nvidia-smi after timed region (NVML unavailable)"}
         except Exception as e:  # pragma: no cover
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [f"unavailable: {e}"], "samples": 0}
+
+
+def source_sha256() -> str:
+    """Stamp of the kernel sources a committed ncu capture must carry to describe this build."""
+    import hashlib
+    h = hashlib.sha256()
+    for rel in ("paper_2402_14670_b200/csrc/lf_kernels.cuh", "paper_2402_14670_b200/csrc/lf_api.cu"):
+        with open(os.path.join(ROOT, rel), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()
+
+
+# Algorithmic work model (DESIGN.md section 7, "Algorithmic lane-operations"): lane-operations (one fp32 / int32 ALU
+# operation on one lane) the interval-search formulation of the method needs per work item, at 100 % lane use.
+LANE_OPS = {
+    "per_row": 70,              # a1: extrapolation, 12 layer centres and y positions
+    "per_row_layer_fixed": 10,  # a2: window edges and cap
+    "per_search_step": 2,       # compare + index update of one binary-search step
+    "per_h0_hit": 10,           # a3: bounds of the h2 interval of one h0 hit (+ two searches over <= n_window hits)
+    "per_doublet": 16,          # a3: both filters + x1_expected (+ one closest-hit search in the h1 window)
+    "closest_fixed": 6,         # neighbour compare of a closest-hit search
+    "per_triplet_passing": 12,  # a3: key + insertion into the n smallest
+    "per_triplet_kept": 15,     # a4: parabola through the triplet (+ 9 predictions and closest-hit searches)
+    "per_prediction": 6,        # a4/a5: expected coordinate on one layer
+    "per_accepted": 331,        # a6: residuals, both least-squares fits, chi2 sums, Q
+    "per_track": 60,            # a6/a7: Eq. (9), state, 20-word record moved once
+    "per_seed": 2,              # a7: flag + scan
+}
+
+
+def algorithmic_lane_ops(counters: dict, batch, n_window: int, sides: int) -> dict:
+    """Evaluates the model on the batch's own counters (lf_run_counters after a counting run)."""
+    import math
+    L = LANE_OPS
+    rows = batch.n_seeds * sides
+    seg_len = batch.n_hits / max(batch.n_events * 24, 1)
+    seg_steps = math.ceil(math.log2(seg_len + 1)) if seg_len > 0 else 0
+    win_steps = math.ceil(math.log2(n_window + 1))
+    closest = win_steps * L["per_search_step"] + L["closest_fixed"]
+    h0_hits = counters["window_hits"] / 6.0  # two of the twelve layers open the two layer sets
+    parts = {
+        "a1_a2": rows * (L["per_row"] + 12 * (L["per_row_layer_fixed"] + 2 * seg_steps * L["per_search_step"])),
+        "a3": h0_hits * (L["per_h0_hit"] + 2 * win_steps * L["per_search_step"])
+              + counters["doublets_passing"] * (L["per_doublet"] + closest)
+              + counters["triplets_passing"] * L["per_triplet_passing"],
+        "a4_a5": counters["triplets_kept"] * (L["per_triplet_kept"] + 9 * (L["per_prediction"] + closest)),
+        "a6": counters["accepted_candidates"] * L["per_accepted"] + counters["tracks"] * L["per_track"],
+        "a7": batch.n_seeds * L["per_seed"],
+    }
+    parts["total"] = float(sum(parts.values()))
+    return parts
 
 
 def algorithmic_bytes(batch, n_tracks: int) -> int:
@@ -222,7 +278,13 @@ def run_ours(args):
         lf.run(db, out, stream)
     barrier()
     n_tracks = int(out.n_tracks.cpu()[0])
-    n_acc, n_dup_events = lf.run_counters()
+    # one counting run (debug build of the kernels, untimed): the work items of every stage, for the algorithmic model
+    lf.run_counting(db, out, stream)
+    counters = lf.run_counters()
+    assert counters["tracks"] == n_tracks, "counting run and plain run disagree on the track count"
+    n_acc, n_dup_events = counters["accepted_candidates"], counters["events_with_equal_hits"]
+    lf.run(db, out, stream)
+    barrier()
 
     # ---- timed region: K steps, inputs resident in HBM, per-kernel CUDA events recorded by the library
     lf.set_profiling(True)
@@ -251,7 +313,7 @@ def run_ours(args):
         ht = binding.HostTracks(batch.n_seeds, batch.n_events)
         for _ in range(2):
             lf.run_host(hb, ht, stream)
-        k_e2e = max(3, min(args.steps, 10))
+        k_e2e = max(3, min(args.steps, 10))  # the host path is PCIe-bound and steady: ten steps are enough (e2e.steps says so)
         barrier()
         t0 = time.perf_counter()
         for _ in range(k_e2e):
@@ -268,48 +330,55 @@ def run_ours(args):
     if rank != 0:
         return 0
 
-    # ---- roofline of the dominant kernel (the slowest of the four event kernels).  The path is bound by the plain
-    # ALU / warp-instruction issue rate, so the top-level object is the "alu" roofline; the HBM
-    # roofline BASELINE.json's metric asks for sits beside it under "hbm" (same keys, algorithmic bytes).
+    # ---- roofline of the dominant kernel (the slowest of the four event kernels): the HBM roofline BASELINE.json's metric
+    # names.  The path is bound by instruction issue, not by HBM, so two ALU figures sit beside it
+    # as flat keys: alu_algorithmic_frac (a roofline fraction: algorithmic lane-operations of the committed model) and
+    # issue_utilisation (how busy the issue slots are with whatever the kernel executes: not a roofline fraction).
     peak, peak_src = measured_peaks()
-    kb = kernel_bytes(batch, n_tracks, int(P["n_triplets"]), n_acc, sides=2 if no_ut else 1, wide=wide)
+    sides = 2 if no_ut else 1
+    kb = kernel_bytes(batch, n_tracks, int(P["n_triplets"]), n_acc, sides=sides, wide=wide)
     dom = max(binding.EVENT_KERNELS, key=lambda k: ktimes[k])
     achieved = kb[dom] / (ktimes[dom] * 1e-3) / 1e9
     path_bytes = algorithmic_bytes(batch, n_tracks)
     path_gbs = path_bytes / (local_ms / args.steps * 1e-3) / 1e9
-    hbm = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-           "traffic": None, "kernel": f"lf_{dom}_kernel", "kernel_ms": ktimes[dom],
-           "algorithmic_bytes_per_launch": kb[dom], "peak_source": peak_src,
-           "whole_path": {"algorithmic_bytes_per_step": path_bytes, "achieved_gbs": path_gbs, "frac_of_measured": path_gbs / peak,
-                          "frac_of_nominal_8TBs": path_gbs / NOMINAL_HBM_GBS},
-           "note": "the path is not HBM-bound; this fraction is reported because BASELINE.json's metric asks for it"}
-    roofline = hbm
-    traffic_file = os.path.join(ROOT, "profiles", "dominant_kernel_traffic_noUT.txt" if no_ut else "dominant_kernel_traffic.txt")
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "kernel": f"lf_{dom}_kernel", "kernel_ms": ktimes[dom],
+                "algorithmic_bytes_per_launch": kb[dom], "peak_source": peak_src,
+                "whole_path": {"algorithmic_bytes_per_step": path_bytes, "achieved_gbs": path_gbs, "frac_of_measured": path_gbs / peak,
+                               "frac_of_nominal_8TBs": path_gbs / NOMINAL_HBM_GBS},
+                "note": "the path is not HBM-bound (DESIGN.md section 7); this is the fraction BASELINE.json's metric asks for"}
+    sm_mhz = float(clocks.get("sm_max_mhz") or 1965.0)
+    lane_peak = 148 * 128 * sm_mhz * 1e6
+    model = algorithmic_lane_ops(counters, batch, int(P["n_window"]), sides)
+    alu_frac = model["total"] / (local_ms / args.steps * 1e-3) / lane_peak
+    alu_model = {"lane_ops_per_step": model, "lane_ops_per_seed": model["total"] / max(batch.n_seeds, 1),
+                 "peak_lane_ops_per_s": lane_peak, "peak_source": "148 SMs x 128 fp32/int32 lanes x sm_max_mhz",
+                 "counters": counters, "coefficients": LANE_OPS,
+                 "note": "algorithmic work of the interval-search formulation at 100 % lane use (DESIGN.md section 7), not executed instructions"}
+    issue_util, issue_detail = None, None
+    tag = ("_noUT" if no_ut else "") + (f"_cfg{args.config}" if args.config != 3 else "")
+    traffic_file = os.path.join(ROOT, "profiles", f"dominant_kernel_traffic{tag}.txt")
     if os.path.exists(traffic_file):
         try:
             tr = json.load(open(traffic_file))
-            # the ncu counts were taken on one batch (n_seeds of the capture): they describe this run only if it is that batch
-            same_batch = tr.get("kernel") == hbm["kernel"] and int(tr.get("n_seeds", -1)) == batch.n_seeds
-            if same_batch:
-                hbm["traffic"] = tr.get("dram_bytes_per_launch")
-                hbm["traffic_source"] = tr.get("source")
-            # peak = SMs x 4 schedulers x 1 warp-instruction/clock x max SM clock; achieved = EXECUTED warp-instructions
-            # per launch (counted by ncu on this workload, profiles/) / the kernel's live duration.
-            wi = tr.get("all_kernels_warp_inst_per_launch", {})
-            if dom in wi and same_batch:
-                sm_mhz = float(clocks.get("sm_max_mhz") or 1965.0)
-                peak_issue = 148 * 4 * sm_mhz * 1e6 / 1e9
-                ach = wi[dom] / (ktimes[dom] * 1e-3) / 1e9
-                ev_k = [k for k in binding.EVENT_KERNELS if k in wi]
-                roofline = {"bound": "alu", "achieved": ach, "peak": peak_issue, "unit": "G warp-inst/s", "frac": ach / peak_issue,
-                            "traffic": hbm["traffic"], "kernel": hbm["kernel"], "kernel_ms": ktimes[dom],
-                            "warp_inst_per_launch": wi[dom], "warp_inst_per_seed": wi[dom] / batch.n_seeds,
-                            "event_kernels_frac": sum(wi[k] for k in ev_k) / (sum(ktimes[k] for k in ev_k) * 1e-3) / 1e9 / peak_issue,
-                            "peak_source": "148 SMs x 4 schedulers x 1 warp-inst/clk x sm_max_mhz (B300_MICROARCH.md issue model; DESIGN.md section 7)",
-                            "count_source": tr.get("source"),
-                            "note": "issue-slot utilisation: executed warp-instructions (ncu capture of this workload) over the live kernel "
-                                    "time; the remaining lever is the instruction count per seed, tracked in warp_inst_per_seed",
-                            "hbm": hbm}
+            # the ncu counts describe this run only if they were taken on this source and on this batch
+            same = (tr.get("source_sha256") == source_sha256() and tr.get("kernel") == roofline["kernel"]
+                    and int(tr.get("n_seeds", -1)) == batch.n_seeds)
+            if same:
+                roofline["traffic"] = tr.get("dram_bytes_per_launch")
+                roofline["traffic_source"] = tr.get("source")
+                wi = tr.get("all_kernels_warp_inst_per_launch", {})
+                if dom in wi:
+                    peak_issue = 148 * 4 * sm_mhz * 1e6
+                    issue_util = wi[dom] / (ktimes[dom] * 1e-3) / peak_issue
+                    ev_k = [k for k in binding.EVENT_KERNELS if k in wi]
+                    issue_detail = {"kernel": roofline["kernel"], "warp_inst_per_launch": wi[dom],
+                                    "warp_inst_per_seed": wi[dom] / batch.n_seeds,
+                                    "all_kernels_warp_inst_per_seed": {k: wi[k] / batch.n_seeds for k in ev_k},
+                                    "event_kernels_utilisation": sum(wi[k] for k in ev_k) / (sum(ktimes[k] for k in ev_k) * 1e-3) / peak_issue,
+                                    "peak_warp_inst_per_s": peak_issue, "count_source": tr.get("source")}
+            else:
+                roofline["traffic_note"] = "committed ncu capture was taken on another source or batch (sha256 / n_seeds stamp differs)"
         except Exception:
             pass
 
@@ -336,7 +405,8 @@ def run_ours(args):
         "metric": "events_per_s", "value": value, "unit": "events/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"{cfg.name}: {batch.n_events} events per GPU, Run-3-like occupancy, fp32, one lf_run on one stream"
+        "config": {"workload": f"{cfg.name}: {batch.n_events} events per GPU, {'high' if args.config == 4 else 'Run-3-like'} occupancy, fp32"
+                               + (" with fp16 hit storage" if int(P.get("hit_storage", 0)) == 1 else "") + ", one lf_run on one stream"
                                + (", no-UT tuning (PAPER.md:285-325)" if no_ut else ""),
                    "tuning": args.tuning,
                    "events_per_gpu": batch.n_events, "seeds_per_gpu": batch.n_seeds, "hits_per_gpu": batch.n_hits,
@@ -346,6 +416,7 @@ def run_ours(args):
         "seeds_per_s": tot_seeds / (ms_per_step * 1e-3),
         "tracks_per_s": tot_tracks / (ms_per_step * 1e-3),
         "e2e": e2e, "gpu_launches": info.kernels_per_run * args.steps, "clocks": clocks, "roofline": roofline,
+        "alu_algorithmic_frac": alu_frac, "issue_utilisation": issue_util, "alu_model": alu_model, "issue_detail": issue_detail,
         "cpu_baseline": cpu,
         "kernels": {"ms": ktimes, "algorithmic_bytes": kb,
                     "launch": {n: {"regs": info.regs[i], "block": info.block[i], "grid": info.grid[i],

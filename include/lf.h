@@ -33,7 +33,7 @@
  *     coordinate s = x + y*tan_alpha is ASCENDING (precondition, not checked).  Offsets are
  *     monotone.  q/p is finite.
  *   - Output order contract: tracks are ordered by (event, seed index); at most one per seed.
- *   - Limits: n_hits, n_seeds < 2^31 per call; at most 2^26 seeds and 2^25 hits in one event (packed per-event
+ *   - Limits: n_hits, n_seeds < 2^31 per call; at most 2^25 seeds and 2^25 hits in one event (packed per-event
  *     indices in the library's tables); n_window <= 64, n_triplets <= 32.
  */
 #ifndef LF_H
@@ -46,7 +46,7 @@
 extern "C" {
 #endif
 
-#define LF_ABI_VERSION 4u
+#define LF_ABI_VERSION 5u
 #define LF_N_LAYERS 12   /* three T-stations, x-u-v-x each */
 #define LF_N_ZONES 2     /* lower / upper half */
 #define LF_MAX_WINDOW 32   /* largest params.n_window of the narrow kernels (one warp lane per hit) */
@@ -235,11 +235,19 @@ lf_status lf_get_info(const lf_handle* h, lf_info* out);
 lf_status lf_set_profiling(lf_handle* h, int enabled);
 lf_status lf_kernel_times(lf_handle* h, float ms[LF_N_KERNELS]);
 
-/* Work counters of the most recent lf_run / lf_run_debug on this handle (for lf_run_host: of its last chunk),
- * for benchmarks: counters[0] = candidates that passed the hit-count rule (16-byte records handed from the
- * extension kernel to the fit kernel), counters[1] = events holding two equal neighbouring hits.
- * SYNCHRONOUS: waits for the device, then reads two per-event tables back. */
-#define LF_N_COUNTERS 2
+/* Work counters of the most recent lf_run / lf_run_debug on this handle (for lf_run_host: of its last chunk), for
+ * benchmarks and for the algorithmic work model of DESIGN.md section 7:
+ *   [0] candidates that passed the hit-count rule (16-byte records handed from the extension kernel to the fit kernel)
+ *   [1] events holding two equal neighbouring hits
+ * and, counted only by lf_run_debug (0 after a plain lf_run; any or all pointers of lf_debug may be NULL):
+ *   [2] hits inside the search windows, summed over followed tracks and layers (a2)
+ *   [3] candidate doublets the seeding kernel evaluated (its bracket of the magnet-opening cut; implementation-specific)
+ *   [4] doublets that passed both filters of PAPER.md:210-211 (a3)
+ *   [5] triplets that passed the chi2 cut, before the top-n selection (a3)
+ *   [6] triplets kept = candidates extended (a4, a5)
+ *   [7] tracks written (a6, a7)
+ * SYNCHRONOUS: waits for the device, then reads the tables back. */
+#define LF_N_COUNTERS 8
 lf_status lf_run_counters(lf_handle* h, uint64_t counters[LF_N_COUNTERS]);
 
 /* ABI self-description for bindings: version and struct sizes

@@ -78,6 +78,9 @@ class lf_info(C.Structure):
 
 
 KERNEL_NAMES = ("window", "seed", "extend", "fit", "scan", "compact")
+N_COUNTERS = 8
+COUNTER_NAMES = ("accepted_candidates", "events_with_equal_hits", "window_hits", "doublets_evaluated", "doublets_passing",
+                 "triplets_passing", "triplets_kept", "tracks")
 EVENT_KERNELS = KERNEL_NAMES[:4]
 
 
@@ -118,12 +121,12 @@ def load_library() -> C.CDLL:
     lib.lf_set_host_chunk_events.restype = C.c_int
     lib.lf_set_host_chunk_events.argtypes = [C.c_void_p, C.c_size_t]
     lib.lf_run_counters.restype = C.c_int
-    lib.lf_run_counters.argtypes = [C.c_void_p, C.POINTER(C.c_uint64 * 2)]
+    lib.lf_run_counters.argtypes = [C.c_void_p, C.POINTER(C.c_uint64 * N_COUNTERS)]
     lib.lf_set_profiling.restype = C.c_int
     lib.lf_set_profiling.argtypes = [C.c_void_p, C.c_int]
     lib.lf_kernel_times.restype = C.c_int
     lib.lf_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_float * 6)]
-    if lib.lf_abi_version() != 4:
+    if lib.lf_abi_version() != 5:
         raise ImportError("liblf_b200.so: ABI version mismatch")
     for i, st in enumerate(_STRUCTS):
         if lib.lf_sizeof(i) != C.sizeof(st):
@@ -280,10 +283,23 @@ class LookingForward:
         return int(out.n_tracks[0])
 
     def run_counters(self):
-        """``lf_run_counters`` (synchronous): (accepted candidates, events with equal neighbouring hits) of the last run."""
-        c = (C.c_uint64 * 2)()
+        """``lf_run_counters`` (synchronous): the work counters of the last run as a dict (include/lf.h); entries 2..6 are
+        counted by debug launches only (:meth:`run` with ``debug=True`` or :meth:`run_counting`)."""
+        c = (C.c_uint64 * N_COUNTERS)()
         self._check(self._lib.lf_run_counters(self._h, C.byref(c)))
-        return int(c[0]), int(c[1])
+        return {n: int(v) for n, v in zip(COUNTER_NAMES, c)}
+
+    def run_counting(self, db: "DeviceBatch", out: "TrackBuffers", stream=None):
+        """``lf_run_debug`` with no stage-boundary table requested: the debug build of the kernels, which also counts
+        the work items of every stage (:meth:`run_counters`)."""
+        seeds = lf_seeds(db.seed_x.data_ptr(), db.seed_y.data_ptr(), db.seed_tx.data_ptr(), db.seed_ty.data_ptr(),
+                         db.seed_qop.data_ptr(), db.seed_offsets.data_ptr(), db.n_seeds)
+        hits = lf_hits(db.hit_x.data_ptr(), db.seg_offsets.data_ptr(), db.n_hits)
+        tr = out.c_struct()
+        dbg = lf_debug()
+        self._check(self._lib.lf_run_debug(self._h, C.byref(seeds), C.byref(hits), db.n_events, C.byref(tr), C.byref(dbg),
+                                           self._stream_ptr(stream)))
+        return out
 
     def set_host_chunk_events(self, min_events_per_chunk: int):
         """``lf_set_host_chunk_events``: pipeline granularity of :meth:`run_host`."""

@@ -61,6 +61,8 @@ struct lf_handle {
   uint8_t* n_trip;
   int32_t *ws_rec, *ws_nh, *ws_rank, *ws_event;
   uint32_t *ev_count, *ev_off, *ev_dup, *ev_acc, *tickets;
+  unsigned long long* counters; /* LF_N_COUNTERS: written by the debug build of the kernels */
+  bool counters_valid = false;  /* the most recent launch was a debug launch */
   uint32_t* validate_res; /* 4 words: lf_validate_inputs' violation bits and offending indices */
   uint4* acc_rec;
   lf::FitLut* fit_lut;
@@ -283,6 +285,11 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
     A.dbg.trip_hits = dbg->trip_hits; A.dbg.trip_set = dbg->trip_set; A.dbg.trip_chi2 = dbg->trip_chi2;
     A.dbg.cand_hits = dbg->cand_hits; A.dbg.cand_quality = dbg->cand_quality;
   }
+  if (DEBUG) {
+    A.dbg.counters = h->counters;
+    LF_CUDA(h, cudaMemsetAsync(h->counters, 0, LF_N_COUNTERS * sizeof(unsigned long long), st));
+  }
+  h->counters_valid = DEBUG;
   h->last_events = n_events;
   const bool work = n_events > 0;
   auto grid_of = [&](int k) { return (int)std::min<size_t>((size_t)h->grid[k], n_events); };
@@ -476,6 +483,7 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
     LF_CREATE_CUDA(cudaMemcpy(h->fit_lut, lut.data(), lut.size() * sizeof(lf::FitLut), cudaMemcpyHostToDevice));
   }
   LF_CREATE_CUDA(cudaMalloc(&h->validate_res, 4 * sizeof(uint32_t)));
+  LF_CREATE_CUDA(cudaMalloc(&h->counters, LF_N_COUNTERS * sizeof(unsigned long long)));
   LF_CREATE_CUDA(cudaMalloc(&h->tickets, lf::N_TICKETS * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMemset(h->tickets, 0, lf::N_TICKETS * sizeof(uint32_t)));
   h->workspace_bytes = nrows * (lf::WIN_ROW * 4 + nt * (code_bytes + sizeof(uint4)) + 1) + ns * (lf::REC_WORDS + 3) * 4 +
@@ -492,6 +500,7 @@ lf_status lf_destroy(lf_handle* h) {
   cudaFree(h->ws_rec); cudaFree(h->ws_nh); cudaFree(h->ws_rank); cudaFree(h->ws_event);
   cudaFree(h->ev_count); cudaFree(h->ev_off); cudaFree(h->ev_dup); cudaFree(h->ev_acc); cudaFree(h->acc_rec); cudaFree(h->fit_lut); cudaFree(h->tickets);
   cudaFree(h->validate_res);
+  cudaFree(h->counters);
   HostBufs& b = h->hb;
   cudaFree(b.seeds); cudaFree(b.seed_off); cudaFree(b.hits); cudaFree(b.seg_off);
   cudaFree(b.hit_idx); cudaFree(b.seed_idx); cudaFree(b.n_hits); cudaFree(b.state); cudaFree(b.quality);
@@ -538,13 +547,20 @@ lf_status lf_run_counters(lf_handle* h, uint64_t counters[LF_N_COUNTERS]) {
   for (int i = 0; i < LF_N_COUNTERS; ++i) counters[i] = 0;
   const size_t ne = h->last_events;
   if (ne == 0) return LF_OK;
-  std::vector<uint32_t> acc(ne), dup(ne);
+  std::vector<uint32_t> acc(ne), dup(ne), cnt(ne);
   LF_CUDA(h, cudaDeviceSynchronize());
   LF_CUDA(h, cudaMemcpy(acc.data(), h->ev_acc, ne * sizeof(uint32_t), cudaMemcpyDeviceToHost));
   LF_CUDA(h, cudaMemcpy(dup.data(), h->ev_dup, ne * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+  LF_CUDA(h, cudaMemcpy(cnt.data(), h->ev_count, ne * sizeof(uint32_t), cudaMemcpyDeviceToHost));
   for (size_t e = 0; e < ne; ++e) {
     counters[0] += acc[e];
     counters[1] += dup[e] ? 1u : 0u;
+    counters[7] += cnt[e];
+  }
+  if (h->counters_valid) {
+    unsigned long long dev[LF_N_COUNTERS];
+    LF_CUDA(h, cudaMemcpy(dev, h->counters, sizeof(dev), cudaMemcpyDeviceToHost));
+    for (int i = 2; i <= 6; ++i) counters[i] = dev[i];
   }
   return LF_OK;
 }

@@ -101,6 +101,7 @@ struct DebugOut {
   float* trip_chi2;
   int32_t* cand_hits;
   float* cand_quality;
+  unsigned long long* counters; /* LF_N_COUNTERS work counters of the debug build (include/lf.h, lf_run_counters) */
 };
 
 /* Arguments common to the three event kernels + the per-stage tables (library workspace). */
@@ -526,6 +527,7 @@ __device__ __forceinline__ void windows_of_event(const Consts& C, const EventArg
     if (DEBUG) {
       if (A.dbg.win_first) A.dbg.win_first[row * NL + layer] = (int32_t)(E.h0 + first);
       if (A.dbg.win_count) A.dbg.win_count[row * NL + layer] = last - first;
+      if (A.dbg.counters) atomicAdd(A.dbg.counters + 2, (unsigned long long)(last - first));
     }
   }
 }
@@ -825,6 +827,7 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
       const float x_at_mag = x0o + t * ca.y;
       const float tol = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * fabsf(t));
       ok = ok && (fabsf(x_at_mag - x_mag) < tol); /* filter 2: opening at the magnet centre */
+      if (DEBUG && ok && A.dbg.counters) atomicAdd(A.dbg.counters + 4, 1ull);
       if (ok) {
         /* x1_expected, closest h1, chi2 cut */
         const float x1e = ca.z * t + (x0o - t * ca.w) * SC[set].K;
@@ -839,6 +842,7 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
       }
     }
     const unsigned m = __ballot_sync(FULL, pass);
+    if (DEBUG && lane == 0 && A.dbg.counters) atomicAdd(A.dbg.counters + 5, (unsigned long long)__popc(m));
     if (m) {
       if (tcount > 32) tcount = select_smallest(W, tcount, C.n_triplets, lane);
       if (pass) {
@@ -858,6 +862,10 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
   const unsigned low = mine ? (unsigned)W.code[lane] : 0u;
   if (lane < NT) EP.codes[k_seed * (uint32_t)NT + (uint32_t)lane] = (uint16_t)low;
   if (DEBUG) {
+    if (lane == 0 && A.dbg.counters) {
+      atomicAdd(A.dbg.counters + 3, (unsigned long long)total);
+      atomicAdd(A.dbg.counters + 6, (unsigned long long)ntr);
+    }
     const size_t seed = (size_t)EP.s0 + k_seed;
     const int set = (low >> 15) & 1, la = set ? 3 : 0;
     const int fa = (int)(__shfl_sync(FULL, winw, la) >> 6), fb = (int)(__shfl_sync(FULL, winw, la + 4) >> 6);
@@ -990,6 +998,7 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
       const float x_at_mag = x0o + t * zmag_a;
       const float tol = fminf(C.mag_tol_max, tol0 + C.mag_tol_tx * fabsf(t));
       ok = ok && (fabsf(x_at_mag - x_mag) < tol); /* filter 2: opening at the magnet centre */
+      if (DEBUG && ok && A.dbg.counters) atomicAdd(A.dbg.counters + 4, 1ull);
       if (ok) {
         const float zb = set ? C.z[7] : C.z[4], za = set ? C.z[3] : C.z[0], Kx1 = set ? C.K[1] : C.K[0];
         const float x1e = zb * t + (x0o - t * za) * Kx1;
@@ -1004,6 +1013,7 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
       }
     }
     const unsigned m = __ballot_sync(FULL, pass);
+    if (DEBUG && lane == 0 && A.dbg.counters) atomicAdd(A.dbg.counters + 5, (unsigned long long)__popc(m));
     if (m) {
       if (tcount > 32) tcount = select_smallest(WT, tcount, C.n_triplets, lane);
       if (pass) WT.trip[tcount + __popc(m & lt_mask)] = key;
@@ -1019,6 +1029,10 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
   const unsigned long long key = mine ? WT.trip[lane] : 0ull;
   if (mine) static_cast<uint32_t*>(A.trip_code)[row * NT + lane] = (unsigned)key; /* codes beyond n_trip are never read */
   if (DEBUG) {
+    if (lane == 0 && A.dbg.counters) {
+      atomicAdd(A.dbg.counters + 3, (unsigned long long)total);
+      atomicAdd(A.dbg.counters + 6, (unsigned long long)ntr);
+    }
     const unsigned low = (unsigned)key;
     const int set = (low >> (3 * F::IB)) & 1, la = set ? 3 : 0;
     const int fa = (int)(__shfl_sync(FULL, winw, la) >> F::WB);

@@ -43,11 +43,17 @@ def test_gpu_arm_line(tuning):
     e = d["e2e"]
     assert e["value"] > 0 and e["value"] < d["value"] and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
     r = d["roofline"]
-    # the ALU (issue-rate) roofline needs ncu's instruction counts of the SAME batch (profiles/dominant_kernel_traffic*.txt,
-    # taken on the full configs[3] batch): on this small batch only the HBM roofline can be reported
-    assert r["bound"] == "hbm" and 0 < r["frac"] < 1 and r["achieved"] > 0 and r["peak"] > 0 and r["traffic"] is None
-    hbm = r
-    assert hbm["bound"] == "hbm" and hbm["unit"] == "GB/s" and 0 < hbm["frac"] < 1 and hbm["algorithmic_bytes_per_launch"] > 0
+    # top level = the HBM roofline BASELINE.json's metric names.  ncu's DRAM bytes and instruction counts describe the
+    # full configs[3] batch on the stamped source only (profiles/dominant_kernel_traffic*.txt): on this small batch
+    # "traffic" and "issue_utilisation" must be null, never a stale number
+    assert r["bound"] == "hbm" and r["unit"] == "GB/s" and 0 < r["frac"] < 1 and r["achieved"] > 0 and r["peak"] > 0
+    assert r["traffic"] is None and r["algorithmic_bytes_per_launch"] > 0 and d["issue_utilisation"] is None
+    # the algorithmic ALU fraction comes from the committed model evaluated on this batch's own work counters
+    assert 0 < d["alu_algorithmic_frac"] < 1
+    c = d["alu_model"]["counters"]
+    assert c["tracks"] == d["config"]["tracks_per_step_per_gpu"] and c["window_hits"] > c["doublets_passing"] > 0
+    assert c["doublets_evaluated"] >= c["doublets_passing"] and c["triplets_passing"] >= c["triplets_kept"] >= c["accepted_candidates"] > 0
+    assert abs(sum(v for k, v in d["alu_model"]["lane_ops_per_step"].items() if k != "total") - d["alu_model"]["lane_ops_per_step"]["total"]) < 1
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["cores"] == 1 and c["value"] > 0 and "sample" in c
     assert d["oracle_check"]["equal"] is True
