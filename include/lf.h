@@ -95,11 +95,13 @@ typedef struct {
                                                                  LF_MAX_WINDOW_WIDE, 1 <= n_triplets <= LF_MAX_TRIPLETS_WIDE */
   float xtol_base, xtol_inv_p, x_asym, uv_half_width;         /* 150, 2000, 100, 800 */
   float p_same_bend, mag_tol_base, mag_tol_inv_p, mag_tol_tx, mag_tol_max; /* 5, 8, 60, 20, 40 */
-  int32_t hit_storage;                                        /* 0 = fp32 (bit-exact reference path); 1 = the library keeps
-                                                                 an fp16 copy of the hits (block-offset encoding) that the
-                                                                 window and seeding kernels read; extension and fit stay on
-                                                                 the fp32 hits (BASELINE.json configs[2]);
-                                                                 mode 0 with the narrow limits only (LF_ERR_UNSUPPORTED otherwise) */
+  int32_t hit_storage;                                        /* 0 = fp32 (bit-exact reference path); 1 = the window and
+                                                                 seeding kernels read an fp16 copy of the hits (block-offset
+                                                                 encoding, lf_pack_hits; the caller's, or packed by the
+                                                                 library at every lf_run); extension and fit stay on the
+                                                                 fp32 hits when lf_hits.x is given (BASELINE.json
+                                                                 configs[2]); mode 0 with the narrow limits only
+                                                                 (LF_ERR_UNSUPPORTED otherwise) */
   /* no-UT tuning; read only when mode == 1 */
   int32_t mode;                  /* 0 = with UT (sections VI.A-D); 1 = no-UT (section VI.E): seeds->qop is not read, the same-bend
                                     filter does not exist, the magnet tolerance uses the assumed 1/p where q/p stood */
@@ -117,9 +119,14 @@ typedef struct {
 
 /* Input hits. */
 typedef struct {
-  const float* x;              /* n_hits stored coordinates */
+  const float* x;              /* n_hits stored coordinates (fp32); may be NULL when params.hit_storage == 1 and x16 is given */
   const uint32_t* seg_offsets; /* n_events*24 + 1; segment index = event*24 + layer*2 + zone */
   size_t n_hits;               /* == seg_offsets[n_events*24] */
+  /* params.hit_storage == 1 only (ignored otherwise; both NULL = the library packs `x` itself at every lf_run):
+   * the fp16 copy of the hits in the block-offset encoding lf_pack_hits writes.  With x == NULL every stage reads
+   * this copy (2.125 bytes per hit to move); with x given, extension and fit read the fp32 hits. */
+  const uint16_t* x16;         /* n_hits IEEE binary16 offsets */
+  const float* origin16;       /* lf_origin_slots(n_events, n_hits) block origins */
 } lf_hits;
 
 /* Output tracks (dense, (event, seed) order).  Arrays must hold `capacity` rows;
@@ -208,6 +215,18 @@ lf_status lf_run_host(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
 /* Smallest number of events lf_run_host puts in one equal pipeline chunk (default 2048; >= 1).  The number of
  * equal chunks is min(13, max(1, n_events / min_events_per_chunk)); the last one is cut into four pieces. */
 lf_status lf_set_host_chunk_events(lf_handle* h, size_t min_events_per_chunk);
+
+/* fp16 hit storage (params.hit_storage == 1; "store hit data in fp16 in addition to fp32"; BASELINE.json
+ * configs[2]).  Encoding: inside every (event, layer, zone) segment consecutive hits form blocks of 32; a block's origin
+ * is the fp32 coordinate of its 17th hit (its last one if shorter); every hit stores binary16(x - origin), so the offset
+ * stays within half a block's span (ulp <= 0.25 mm at Run-3 occupancy).  The origin of block b of global segment g that
+ * starts at hit S sits in slot (S >> 5) + g + b: lf_origin_slots(n_events, n_hits) = (n_hits >> 5) + 24 * n_events + 2
+ * slots hold them all.  lf_pack_hits writes both arrays from fp32 hits (DEVICE pointers, asynchronous on `cuda_stream`;
+ * `hits->x` and `hits->seg_offsets` are read); the result can be kept, copied to the host and handed to lf_run /
+ * lf_run_host in lf_hits.x16 / origin16 of later calls with the same offsets. */
+size_t lf_origin_slots(size_t n_events, size_t n_hits);
+lf_status lf_pack_hits(lf_handle* h, const lf_hits* hits, size_t n_events, uint16_t* x16_out, float* origin16_out,
+                       void* cuda_stream);
 
 /* Checks, on the device, the input preconditions lf_run relies on but does not check (see "Conventions"): segment
  * offsets monotone, starting at 0 and ending at n_hits; stored coordinates finite and ascending inside every

@@ -56,7 +56,8 @@ class lf_seeds(C.Structure):
 
 
 class lf_hits(C.Structure):
-    _fields_ = [("x", C.c_void_p), ("seg_offsets", C.c_void_p), ("n_hits", C.c_size_t)]
+    _fields_ = [("x", C.c_void_p), ("seg_offsets", C.c_void_p), ("n_hits", C.c_size_t),
+                ("x16", C.c_void_p), ("origin16", C.c_void_p)]
 
 
 class lf_tracks(C.Structure):
@@ -120,6 +121,10 @@ def load_library() -> C.CDLL:
     lib.lf_get_info.argtypes = [C.c_void_p, C.POINTER(lf_info)]
     lib.lf_set_host_chunk_events.restype = C.c_int
     lib.lf_set_host_chunk_events.argtypes = [C.c_void_p, C.c_size_t]
+    lib.lf_origin_slots.restype = C.c_size_t
+    lib.lf_origin_slots.argtypes = [C.c_size_t, C.c_size_t]
+    lib.lf_pack_hits.restype = C.c_int
+    lib.lf_pack_hits.argtypes = [C.c_void_p, C.POINTER(lf_hits), C.c_size_t, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.lf_run_counters.restype = C.c_int
     lib.lf_run_counters.argtypes = [C.c_void_p, C.POINTER(C.c_uint64 * N_COUNTERS)]
     lib.lf_set_profiling.restype = C.c_int
@@ -162,6 +167,17 @@ class DeviceBatch:
         self.hit_x = t(batch.hit_x)
         self.seg_offsets = t(np.asarray(batch.seg_offsets, dtype=np.uint32).view(np.int32))
         self.device = self.hit_x.device
+        self.hit_x16 = None     # optional fp16 copy (LookingForward.pack_hits); with drop_fp32() the only copy
+        self.origin16 = None
+
+    def drop_fp32(self):
+        """Keeps only the packed fp16 copy of the hits (hit_storage = 1 with every stage reading fp16)."""
+        assert self.hit_x16 is not None, "pack the hits first"
+        self.hit_x = None
+
+    def c_hits(self) -> "lf_hits":
+        p = lambda t: t.data_ptr() if t is not None else None
+        return lf_hits(p(self.hit_x), self.seg_offsets.data_ptr(), self.n_hits, p(self.hit_x16), p(self.origin16))
 
 
 class TrackBuffers:
@@ -243,7 +259,7 @@ class LookingForward:
             out = TrackBuffers(db.n_seeds, db.n_events, db.device)
         seeds = lf_seeds(db.seed_x.data_ptr(), db.seed_y.data_ptr(), db.seed_tx.data_ptr(), db.seed_ty.data_ptr(),
                          db.seed_qop.data_ptr(), db.seed_offsets.data_ptr(), db.n_seeds)
-        hits = lf_hits(db.hit_x.data_ptr(), db.seg_offsets.data_ptr(), db.n_hits)
+        hits = db.c_hits()
         tr = out.c_struct()
         sp = self._stream_ptr(stream)
         if not debug:
@@ -267,15 +283,27 @@ class LookingForward:
         """``lf_validate_inputs`` (synchronous): raises LfError naming the violated precondition."""
         seeds = lf_seeds(db.seed_x.data_ptr(), db.seed_y.data_ptr(), db.seed_tx.data_ptr(), db.seed_ty.data_ptr(),
                          db.seed_qop.data_ptr(), db.seed_offsets.data_ptr(), db.n_seeds)
-        hits = lf_hits(db.hit_x.data_ptr(), db.seg_offsets.data_ptr(), db.n_hits)
+        hits = db.c_hits()
         self._check(self._lib.lf_validate_inputs(self._h, C.byref(seeds), C.byref(hits), db.n_events, self._stream_ptr(stream)))
+
+    def pack_hits(self, db: DeviceBatch, stream=None) -> DeviceBatch:
+        """``lf_pack_hits``: writes the fp16 block-offset copy of ``db``'s hits into ``db.hit_x16`` / ``db.origin16``."""
+        import torch
+        slots = int(self._lib.lf_origin_slots(db.n_events, db.n_hits))
+        db.hit_x16 = torch.empty(max(db.n_hits, 1), dtype=torch.float16, device=db.device)
+        db.origin16 = torch.zeros(slots, dtype=torch.float32, device=db.device)
+        hits = lf_hits(db.hit_x.data_ptr(), db.seg_offsets.data_ptr(), db.n_hits, None, None)
+        self._check(self._lib.lf_pack_hits(self._h, C.byref(hits), db.n_events, db.hit_x16.data_ptr(), db.origin16.data_ptr(),
+                                           self._stream_ptr(stream)))
+        return db
 
     # -- host path (end to end) ------------------------------------------------------------------
     def run_host(self, hb: "HostBatch", out: "HostTracks", stream=None) -> int:
         """``lf_run_host``: host buffers in, host buffers out; returns the number of tracks."""
         seeds = lf_seeds(hb.seed_x.data_ptr(), hb.seed_y.data_ptr(), hb.seed_tx.data_ptr(), hb.seed_ty.data_ptr(),
                          hb.seed_qop.data_ptr(), hb.seed_offsets.data_ptr(), hb.n_seeds)
-        hits = lf_hits(hb.hit_x.data_ptr(), hb.seg_offsets.data_ptr(), hb.n_hits)
+        p = lambda t: t.data_ptr() if t is not None else None
+        hits = lf_hits(p(hb.hit_x), hb.seg_offsets.data_ptr(), hb.n_hits, p(hb.hit_x16), p(hb.origin16))
         tr = lf_tracks(out.hit_idx.data_ptr(), out.seed_idx.data_ptr(), out.n_hits.data_ptr(), out.state.data_ptr(),
                        out.quality.data_ptr(), out.event_offsets.data_ptr(), out.n_tracks.data_ptr(), out.capacity)
         self._check(self._lib.lf_run_host(self._h, C.byref(seeds), C.byref(hits), hb.n_events, C.byref(tr),
@@ -294,7 +322,7 @@ class LookingForward:
         the work items of every stage (:meth:`run_counters`)."""
         seeds = lf_seeds(db.seed_x.data_ptr(), db.seed_y.data_ptr(), db.seed_tx.data_ptr(), db.seed_ty.data_ptr(),
                          db.seed_qop.data_ptr(), db.seed_offsets.data_ptr(), db.n_seeds)
-        hits = lf_hits(db.hit_x.data_ptr(), db.seg_offsets.data_ptr(), db.n_hits)
+        hits = db.c_hits()
         tr = out.c_struct()
         dbg = lf_debug()
         self._check(self._lib.lf_run_debug(self._h, C.byref(seeds), C.byref(hits), db.n_events, C.byref(tr), C.byref(dbg),
@@ -334,11 +362,24 @@ class HostBatch:
         self.seed_offsets = t(np.asarray(batch.seed_offsets, dtype=np.uint32).view(np.int32))
         self.hit_x = t(batch.hit_x)
         self.seg_offsets = t(np.asarray(batch.seg_offsets, dtype=np.uint32).view(np.int32))
+        self.hit_x16 = None
+        self.origin16 = None
+        self._pin = pin
+
+    def use_packed(self, db: DeviceBatch, keep_fp32: bool = False):
+        """Takes the packed fp16 copy of a device batch (LookingForward.pack_hits) as the host input; unless
+        ``keep_fp32`` the fp32 hits are dropped, so that the host path moves 2 bytes per hit plus the origins."""
+        pin = (lambda x: x.pin_memory()) if self._pin else (lambda x: x)
+        self.hit_x16 = pin(db.hit_x16.cpu())
+        self.origin16 = pin(db.origin16.cpu())
+        if not keep_fp32:
+            self.hit_x = None
+        return self
 
     def h2d_bytes(self) -> int:
         ts = (self.seed_x, self.seed_y, self.seed_tx, self.seed_ty, self.seed_qop, self.seed_offsets, self.hit_x,
-              self.seg_offsets)
-        return int(sum(x.numel() * x.element_size() for x in ts))
+              self.seg_offsets, self.hit_x16, self.origin16)
+        return int(sum(x.numel() * x.element_size() for x in ts if x is not None))
 
 
 class HostTracks:

@@ -31,6 +31,8 @@ struct HostBufs { /* device staging for lf_run_host */
   float* seeds = nullptr;      /* 5 * max_seeds */
   uint32_t* seed_off = nullptr;
   float* hits = nullptr;
+  uint16_t* hits16 = nullptr;  /* hit_storage = 1: the caller's packed copy */
+  float* origin16 = nullptr;
   uint32_t* seg_off = nullptr;
   int32_t *hit_idx = nullptr, *seed_idx = nullptr, *n_hits = nullptr;
   float *state = nullptr, *quality = nullptr;
@@ -52,8 +54,9 @@ struct lf_handle {
   int sm_count, stage_cap;
   int regs[4], grid[4], ctas_per_sm[4], smem_bytes[4]; /* window, seed, extend, fit kernels */
   /* workspace */
-  __half* hx16;     /* hit_storage = 1 only */
+  __half* hx16;     /* hit_storage = 1 only: the library's own fp16 copy (when the caller gives none) */
   float* origin16;
+  float* hx_scratch; /* hit_storage = 1 only: fp32 image of events that do not fit the stage (lf_kernels.cuh, fetch_event) */
   bool wide;        /* the wide build of the event kernels runs (no-UT mode, or caps beyond the narrow limits) */
   int sides;        /* followed tracks (rows) per seed: 2 in the no-UT mode */
   uint32_t* win;
@@ -264,7 +267,7 @@ bool use_wide(const lf_params& P) {
 
 template <bool DEBUG, bool WIDE>
 lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
-                 const lf_debug* dbg, cudaStream_t st, size_t seed_base = 0) {
+                 const lf_debug* dbg, cudaStream_t st, size_t seed_base = 0, size_t event_base = 0) {
   const bool prof = h->profiling;
   cudaEvent_t* pe = prof ? h->prof_ev[h->prof_runs % PROF_RING] : nullptr;
   if (prof) LF_CUDA(h, cudaEventRecord(pe[0], st));
@@ -294,25 +297,42 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
   const bool work = n_events > 0;
   auto grid_of = [&](int k) { return (int)std::min<size_t>((size_t)h->grid[k], n_events); };
   const bool half_hits = h->P.hit_storage == 1;
-  if (work && half_hits) {
-    /* fp16 copy of the hits for the window and seeding kernels (timed with the window kernel) */
-    const int pg = (int)std::min<size_t>((size_t)h->sm_count * 8, n_events);
-    lf::lf_pack_hits_kernel<<<pg, 256, 0, st>>>(hits->x, hits->seg_offsets, (uint32_t)n_events, h->hx16, h->origin16);
-    A.hx16 = h->hx16;
-    A.origin16 = h->origin16;
+  const __half* use16 = nullptr;
+  const float* use_origin = nullptr;
+  if (half_hits) {
+    if (hits->x16 && hits->origin16) { /* the caller's fp16 copy */
+      use16 = reinterpret_cast<const __half*>(hits->x16);
+      use_origin = hits->origin16;
+    } else { /* pack the fp32 hits (timed with the window kernel) */
+      if (work && hits->n_hits > 0) {
+        const int pg = (int)std::min<size_t>((size_t)h->sm_count * 8, n_events);
+        lf::lf_pack_hits_kernel<<<pg, 256, 0, st>>>(hits->x, hits->seg_offsets, (uint32_t)n_events, (uint32_t)event_base, h->hx16,
+                                                    h->origin16);
+      }
+      use16 = h->hx16;
+      use_origin = h->origin16;
+    }
+    A.hx16 = use16;
+    A.origin16 = use_origin;
+    A.hx_scratch = h->hx_scratch;
+    A.event_base = (uint32_t)event_base;
   }
   if (work) {
     A.ticket = h->tickets + 0;
+    A.scratch_writer = 1; /* the window kernel decodes oversized events once for all four kernels */
     lf::lf_window_kernel<DEBUG, WIDE><<<grid_of(0), lf::WIN_THREADS, h->smem_bytes[0], st>>>(h->C, A);
   }
   if (prof) LF_CUDA(h, cudaEventRecord(pe[1], st));
+  A.scratch_writer = 0;
   if (work) {
     A.ticket = h->tickets + 1;
     lf::lf_seed_kernel<DEBUG, WIDE><<<grid_of(1), lf::SEED_THREADS, h->smem_bytes[1], st>>>(h->C, A);
   }
   if (prof) LF_CUDA(h, cudaEventRecord(pe[2], st));
-  A.hx16 = nullptr; /* extension and fit always read the fp32 hits */
-  A.origin16 = nullptr;
+  if (hits->x != nullptr) { /* extension and fit read the fp32 hits when the caller gave them */
+    A.hx16 = nullptr;
+    A.origin16 = nullptr;
+  }
   if (work) {
     A.ticket = h->tickets + 2;
     lf::lf_extend_kernel<DEBUG, WIDE><<<grid_of(2), lf::FIT_THREADS, h->smem_bytes[2], st>>>(h->C, A);
@@ -342,9 +362,9 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
 
 template <bool DEBUG>
 lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
-                 const lf_debug* dbg, cudaStream_t st, size_t seed_base = 0) {
-  return h->wide ? launch_impl<DEBUG, true>(h, seeds, hits, n_events, out, dbg, st, seed_base)
-                 : launch_impl<DEBUG, false>(h, seeds, hits, n_events, out, dbg, st, seed_base);
+                 const lf_debug* dbg, cudaStream_t st, size_t seed_base = 0, size_t event_base = 0) {
+  return h->wide ? launch_impl<DEBUG, true>(h, seeds, hits, n_events, out, dbg, st, seed_base, event_base)
+                 : launch_impl<DEBUG, false>(h, seeds, hits, n_events, out, dbg, st, seed_base, event_base);
 }
 
 lf_status check_run_args(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out) {
@@ -354,7 +374,8 @@ lf_status check_run_args(lf_handle* h, const lf_seeds* seeds, const lf_hits* hit
     return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL offset table or n_tracks pointer");
   if (seeds->n_seeds > 0 && (!seeds->x || !seeds->y || !seeds->tx || !seeds->ty || (!seeds->qop && h->P.mode == 0)))
     return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL seed array");
-  if (hits->n_hits > 0 && !hits->x) return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL hit array");
+  if (hits->n_hits > 0 && !hits->x && !(h->P.hit_storage == 1 && hits->x16 && hits->origin16))
+    return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL hit array (x may be NULL only with hit_storage = 1 and x16 + origin16 given)");
   if (seeds->n_seeds > 0 && (!out->hit_idx || !out->seed_idx || !out->n_hits || !out->state || !out->quality))
     return fail(h, LF_ERR_INVALID_ARG, "lf_run: NULL output array");
   if ((reinterpret_cast<uintptr_t>(out->hit_idx) & 15u) != 0)
@@ -462,7 +483,8 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   if (params->hit_storage == 1) {
     const size_t nh = std::max<size_t>(max_hits, 1);
     LF_CREATE_CUDA(cudaMalloc(&h->hx16, nh * sizeof(__half)));
-    LF_CREATE_CUDA(cudaMalloc(&h->origin16, ((nh >> 5) + ne * lf::NSEG + 2) * sizeof(float)));
+    LF_CREATE_CUDA(cudaMalloc(&h->origin16, lf_origin_slots(ne, nh) * sizeof(float)));
+    LF_CREATE_CUDA(cudaMalloc(&h->hx_scratch, nh * sizeof(float)));
   }
   LF_CREATE_CUDA(cudaMalloc(&h->win, nrows * lf::WIN_ROW * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->trip_code, nrows * nt * code_bytes));
@@ -495,14 +517,14 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
 
 lf_status lf_destroy(lf_handle* h) {
   if (!h) return LF_OK;
-  cudaFree(h->hx16); cudaFree(h->origin16);
+  cudaFree(h->hx16); cudaFree(h->origin16); cudaFree(h->hx_scratch);
   cudaFree(h->win); cudaFree(h->trip_code); cudaFree(h->n_trip);
   cudaFree(h->ws_rec); cudaFree(h->ws_nh); cudaFree(h->ws_rank); cudaFree(h->ws_event);
   cudaFree(h->ev_count); cudaFree(h->ev_off); cudaFree(h->ev_dup); cudaFree(h->ev_acc); cudaFree(h->acc_rec); cudaFree(h->fit_lut); cudaFree(h->tickets);
   cudaFree(h->validate_res);
   cudaFree(h->counters);
   HostBufs& b = h->hb;
-  cudaFree(b.seeds); cudaFree(b.seed_off); cudaFree(b.hits); cudaFree(b.seg_off);
+  cudaFree(b.seeds); cudaFree(b.seed_off); cudaFree(b.hits); cudaFree(b.hits16); cudaFree(b.origin16); cudaFree(b.seg_off);
   cudaFree(b.hit_idx); cudaFree(b.seed_idx); cudaFree(b.n_hits); cudaFree(b.state); cudaFree(b.quality);
   cudaFree(b.ev_off); cudaFree(b.n_tracks);
   if (b.pinned_count) cudaFreeHost(b.pinned_count);
@@ -642,6 +664,22 @@ lf_status lf_validate_inputs(lf_handle* h, const lf_seeds* seeds, const lf_hits*
   return fail(h, LF_ERR_INVALID_ARG, msg);
 }
 
+size_t lf_origin_slots(size_t n_events, size_t n_hits) { return (n_hits >> lf::H16_SHIFT) + n_events * lf::NSEG + 2; }
+
+lf_status lf_pack_hits(lf_handle* h, const lf_hits* hits, size_t n_events, uint16_t* x16_out, float* origin16_out,
+                       void* cuda_stream) {
+  if (!h) return LF_ERR_INVALID_ARG;
+  if (!hits || !hits->seg_offsets || (hits->n_hits > 0 && (!hits->x || !x16_out)) || !origin16_out)
+    return fail(h, LF_ERR_INVALID_ARG, "lf_pack_hits: NULL hits / offsets / output");
+  h->err.clear();
+  if (n_events == 0 || hits->n_hits == 0) return LF_OK;
+  const int pg = (int)std::min<size_t>((size_t)h->sm_count * 8, n_events);
+  lf::lf_pack_hits_kernel<<<pg, 256, 0, (cudaStream_t)cuda_stream>>>(hits->x, hits->seg_offsets, (uint32_t)n_events, 0u,
+                                                                    reinterpret_cast<__half*>(x16_out), origin16_out);
+  LF_CUDA(h, cudaGetLastError());
+  return LF_OK;
+}
+
 lf_status lf_set_host_chunk_events(lf_handle* h, size_t min_events_per_chunk) {
   if (!h) return LF_ERR_INVALID_ARG;
   if (min_events_per_chunk == 0) return fail(h, LF_ERR_INVALID_ARG, "lf_set_host_chunk_events: must be >= 1");
@@ -683,12 +721,17 @@ static lf_status run_host_pipeline(lf_handle* h, const lf_seeds* seeds, const lf
   }
   cudaStream_t st = (cudaStream_t)cuda_stream;
   HostBufs& b = h->hb;
+  const bool packed = h->P.hit_storage == 1 && hits->x16 && hits->origin16; /* the caller ships the fp16 copy */
   if (!b.ready) {
     const size_t ns = std::max<size_t>(h->max_seeds, 1), ne = std::max<size_t>(h->max_events, 1);
     const size_t nh = std::max<size_t>(h->max_hits, 1);
     LF_CUDA(h, cudaMalloc(&b.seeds, 5 * ns * sizeof(float)));
     LF_CUDA(h, cudaMalloc(&b.seed_off, (ne + 1) * sizeof(uint32_t)));
     LF_CUDA(h, cudaMalloc(&b.hits, nh * sizeof(float)));
+    if (h->P.hit_storage == 1) {
+      LF_CUDA(h, cudaMalloc(&b.hits16, nh * sizeof(uint16_t)));
+      LF_CUDA(h, cudaMalloc(&b.origin16, lf_origin_slots(ne, nh) * sizeof(float)));
+    }
     LF_CUDA(h, cudaMalloc(&b.seg_off, (ne * lf::NSEG + 1) * sizeof(uint32_t)));
     LF_CUDA(h, cudaMalloc(&b.hit_idx, ns * lf::NL * sizeof(int32_t)));
     LF_CUDA(h, cudaMalloc(&b.seed_idx, ns * sizeof(int32_t)));
@@ -749,7 +792,13 @@ static lf_status run_host_pipeline(lf_handle* h, const lf_seeds* seeds, const lf
   for (int c = 0; c < n_chunks; ++c) {
     const size_t e0 = chunk_begin(c), e1 = chunk_begin(c + 1);
     const size_t g0 = go[e0 * lf::NSEG], g1 = go[e1 * lf::NSEG];
-    if (g1 > g0) LF_CUDA(h, cudaMemcpyAsync(b.hits + g0, hits->x + g0, (g1 - g0) * sizeof(float), cudaMemcpyHostToDevice, b.s_h2d));
+    if (g1 > g0 && hits->x)
+      LF_CUDA(h, cudaMemcpyAsync(b.hits + g0, hits->x + g0, (g1 - g0) * sizeof(float), cudaMemcpyHostToDevice, b.s_h2d));
+    if (g1 > g0 && packed) { /* the packed copy of the chunk: its halves and the origin slots its segments own */
+      LF_CUDA(h, cudaMemcpyAsync(b.hits16 + g0, hits->x16 + g0, (g1 - g0) * sizeof(uint16_t), cudaMemcpyHostToDevice, b.s_h2d));
+      const size_t o0 = (g0 >> lf::H16_SHIFT) + e0 * lf::NSEG, o1 = (g1 >> lf::H16_SHIFT) + e1 * lf::NSEG + 1;
+      LF_CUDA(h, cudaMemcpyAsync(b.origin16 + o0, hits->origin16 + o0, (o1 - o0) * sizeof(float), cudaMemcpyHostToDevice, b.s_h2d));
+    }
     LF_CUDA(h, cudaEventRecord(b.ev_h2d[c], b.s_h2d));
   }
   /* ---- kernels on the caller's stream, chunk by chunk; the counts follow on their own stream */
@@ -759,10 +808,11 @@ static lf_status run_host_pipeline(lf_handle* h, const lf_seeds* seeds, const lf
     LF_CUDA(h, cudaStreamWaitEvent(st, b.ev_h2d[c], 0));
     lf_seeds ds = {b.seeds, b.seeds + stride, b.seeds + 2 * stride, b.seeds + 3 * stride, b.seeds + 4 * stride,
                    b.seed_off + e0, s1 - s0};
-    lf_hits dh = {b.hits, b.seg_off + e0 * lf::NSEG, g1 - g0};
+    lf_hits dh = {hits->x ? b.hits : nullptr, b.seg_off + e0 * lf::NSEG, g1 - g0, packed ? b.hits16 : nullptr,
+                  packed ? b.origin16 : nullptr};
     lf_tracks dt = {b.hit_idx + s0 * lf::NL, b.seed_idx + s0, b.n_hits + s0, b.state + s0 * 5, b.quality + s0,
                     b.ev_off + e0 + c, b.n_tracks + c, stride - s0};
-    const lf_status rs = launch<false>(h, &ds, &dh, e1 - e0, &dt, nullptr, st, s0);
+    const lf_status rs = launch<false>(h, &ds, &dh, e1 - e0, &dt, nullptr, st, s0, e0);
     if (rs != LF_OK) return rs;
     LF_CUDA(h, cudaEventRecord(b.ev_comp[c], st));
     LF_CUDA(h, cudaStreamWaitEvent(b.s_cnt, b.ev_comp[c], 0));

@@ -38,6 +38,7 @@ namespace lf {
 
 constexpr int NL = 12;
 constexpr int NSEG = 24;
+constexpr int H16_SHIFT = 3;   /* fp16 hit storage: 2^H16_SHIFT hits share one fp32 origin (include/lf.h, lf_pack_hits) */
 constexpr int WIN_ROW = 16;    /* words per followed track in the window table: 12 packed windows + x_mag, tx, q/p, flags */
 constexpr uint32_t ROW_LOW_P = 1u; /* flags: the seed's momentum is below p_same_bend (filter 1 applies) */
 constexpr int REC_WORDS = 20;  /* 12 hit idx, seed, n_hits, 5 state, Q */
@@ -114,6 +115,10 @@ struct EventArgs {
    * and seed kernels stage from it when hx16 != nullptr */
   const __half* hx16;
   const float* origin16;
+  uint32_t event_base;  /* index of the launch's first event in the arrays hx16 / origin16 were packed for (lf_run_host chunks) */
+  float* hx_scratch;    /* hit_storage = 1: fp32 image of the events that do not fit the stage (decoded once, by the kernel
+                           launched with scratch_writer != 0; read by all of them through HitView<false>) */
+  int scratch_writer;
   uint32_t n_events;
   int stage_cap;        /* floats of shared memory available for one event's hits */
   uint32_t* ticket;     /* this kernel's event ticket */
@@ -144,6 +149,7 @@ struct __align__(16) CtaHeader {
   int nsteps; /* binary-search steps that cover the event's longest segment */
   int warp_tot[8];
   int dup; /* != 0: the event may hold equal neighbouring hits (closest_hit must resolve runs of ties) */
+  int blk_pref[NSEG + 1]; /* fp16 hit storage: blocks of 32 hits in front of each segment of the event */
 };
 constexpr int HDR_BYTES = (sizeof(CtaHeader) + 15) & ~15;
 
@@ -151,6 +157,7 @@ struct EventCtx {
   uint32_t ev, h0;
   int nh, skew;
   bool staged;
+  const float* gview; /* the event's hits in global memory (events that do not fit the stage) */
 };
 
 /* ---------------------------------------------------------------- PTX helpers (TMA 1-D bulk copy) */
@@ -275,15 +282,38 @@ __device__ __forceinline__ bool fetch_event(const EventArgs& A, uint32_t& phase,
   if (tid == 32) H.dup = (int)A.ev_dup[E.ev]; /* meaningful in the seed and fit kernels only */
   const float* gsrc = A.hx + E.h0;
   E.staged = E.nh + 4 <= A.stage_cap;
-  E.skew = (int)((reinterpret_cast<uintptr_t>(gsrc) >> 2) & 3);
-  if (E.staged && A.hx16 != nullptr) {
-    /* fp16 hit storage: decode x~ = origin(block) + half into the fp32 stage, segment by segment */
-    for (int sg = 0; sg < NSEG; ++sg) {
-      const uint32_t S = so[sg];
-      const int len = (int)(so[sg + 1] - S);
-      const uint32_t slot0 = (S >> 5) + (E.ev * NSEG + (uint32_t)sg);
-      for (int i = tid; i < len; i += blockDim.x)
-        buf[E.skew + (int)(S - E.h0) + i] = __ldg(A.origin16 + slot0 + (uint32_t)(i >> 5)) + __half2float(A.hx16[S + i]);
+  const bool from16 = A.hx16 != nullptr;
+  E.skew = from16 ? 0 : (int)((reinterpret_cast<uintptr_t>(gsrc) >> 2) & 3);
+  E.gview = from16 ? A.hx_scratch + E.h0 : gsrc;
+  if (from16) {
+    /* fp16 hit storage (lf_pack_hits_kernel): x~ = origin(block) + half, blocks of 32 hits counted from the start of
+     * each segment.  One warp decodes one block per trip: a 64-byte load of halves, one origin, 32 fp32 stores into
+     * the stage (or, for an event larger than the stage, into the library's fp32 scratch image, once per lf_run). */
+    if (tid < 32) {
+      const int nb = (tid < NSEG) ? (int)((so[tid + 1] - so[tid] + 31u) >> 5) : 0;
+      int incl = nb;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(FULL, incl, o);
+        if (tid >= o) incl += v;
+      }
+      if (tid <= NSEG) H.blk_pref[tid] = incl - nb; /* entry NSEG = all blocks of the event */
+    }
+    __syncthreads();
+    if (E.staged || A.scratch_writer) {
+      float* dst = E.staged ? buf : A.hx_scratch + E.h0;
+      const int lane = tid & 31, n_blk = H.blk_pref[NSEG];
+      const int pref = (lane < NSEG) ? H.blk_pref[lane] : 0x7FFFFFFF;
+      for (int blk = tid >> 5; blk < n_blk; blk += (int)(blockDim.x >> 5)) {
+        const int sg = __popc(__ballot_sync(FULL, pref <= blk)) - 1; /* the last segment that starts at or before blk */
+        const int b = blk - H.blk_pref[sg];
+        const uint32_t S = so[sg];
+        const int i = 32 * b + lane;
+        if (i < (int)(so[sg + 1] - S))
+          dst[(int)(S - E.h0) + i] = __ldg(A.origin16 + ((S >> H16_SHIFT) + ((A.event_base + E.ev) * NSEG + (uint32_t)sg) + (uint32_t)(i >> H16_SHIFT))) +
+                                     __half2float(A.hx16[S + i]);
+      }
+      if (!E.staged) __threadfence(); /* the scratch image is read back by this CTA and by the later kernels */
     }
   } else if (E.staged) {
     /* the 16-byte aligned interior goes by TMA, the ragged head/tail by plain loads */
@@ -555,8 +585,8 @@ __global__ void __launch_bounds__(WIN_THREADS, 8) lf_window_kernel(const __grid_
       flag_equal_neighbours(A, E, HitView<true>(E.skew));
       windows_of_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>(E.skew));
     } else {
-      flag_equal_neighbours(A, E, HitView<false>(A.hx + E.h0));
-      windows_of_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>(A.hx + E.h0));
+      flag_equal_neighbours(A, E, HitView<false>(E.gview));
+      windows_of_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>(E.gview));
     }
   }
 }
@@ -1103,10 +1133,10 @@ __global__ void __launch_bounds__(SEED_THREADS, WIDE ? 4 : 5) lf_seed_kernel(con
           const uint32_t seed = s0 + (uint32_t)(k / sides);
           const int side = k - (k / sides) * sides;
           if (E.staged) seed_triplets_wide<DEBUG>(C, A, HitView<true>(E.skew), E.h0, seed, side, W, lane, dup);
-          else seed_triplets_wide<DEBUG>(C, A, HitView<false>(A.hx + E.h0), E.h0, seed, side, W, lane, dup);
+          else seed_triplets_wide<DEBUG>(C, A, HitView<false>(E.gview), E.h0, seed, side, W, lane, dup);
         } else {
           if (E.staged) seed_triplets<DEBUG>(C, A, HitView<true>(E.skew), E.h0, EP, (uint32_t)k, W, T.sc, lane, dup);
-          else seed_triplets<DEBUG>(C, A, HitView<false>(A.hx + E.h0), E.h0, EP, (uint32_t)k, W, T.sc, lane, dup);
+          else seed_triplets<DEBUG>(C, A, HitView<false>(E.gview), E.h0, EP, (uint32_t)k, W, T.sc, lane, dup);
         }
       }
     }
@@ -1360,7 +1390,7 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_extend_kernel(const __grid_
   EventCtx E;
   while (fetch_event(A, phase, E)) {
     if (E.staged) extend_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>(E.skew), T);
-    else extend_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>(A.hx + E.h0), T);
+    else extend_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>(E.gview), T);
   }
 }
 
@@ -1615,7 +1645,7 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_fit_kernel(const __grid_con
   EventCtx E;
   while (fetch_event(A, phase, E)) {
     if (E.staged) fit_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>(E.skew), T);
-    else fit_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>(A.hx + E.h0), T);
+    else fit_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>(E.gview), T);
   }
 }
 
@@ -1626,19 +1656,20 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_fit_kernel(const __grid_con
  * (ulp <= 0.25 mm at Run-3 occupancy).  The origin slot of block b of global segment g starting at hit S is
  * (S >> 5) + g + b: slots of different segments never overlap, so the index alone locates the origin. */
 __global__ void __launch_bounds__(256) lf_pack_hits_kernel(const float* __restrict__ hx, const uint32_t* __restrict__ seg_off,
-                                                           uint32_t n_events, __half* __restrict__ hx16,
-                                                           float* __restrict__ origin16) {
+                                                           uint32_t n_events, uint32_t event_base,
+                                                           __half* __restrict__ hx16, float* __restrict__ origin16) {
   for (uint32_t ev = blockIdx.x; ev < n_events; ev += gridDim.x) {
     const uint32_t* so = seg_off + (size_t)ev * NSEG;
     for (int sg = 0; sg < NSEG; ++sg) {
       const uint32_t S = so[sg];
       const int len = (int)(so[sg + 1] - S);
-      const uint32_t slot0 = (S >> 5) + (ev * NSEG + (uint32_t)sg);
+      const uint32_t slot0 = (S >> H16_SHIFT) + ((event_base + ev) * NSEG + (uint32_t)sg);
+      constexpr int BL = 1 << H16_SHIFT;
       for (int i = threadIdx.x; i < len; i += blockDim.x) {
-        const int b0 = i & ~31;
-        const float o = hx[S + b0 + min(16, len - b0 - 1)];
+        const int b0 = i & ~(BL - 1);
+        const float o = hx[S + b0 + min(BL / 2, len - b0 - 1)];
         hx16[S + i] = __float2half_rn(hx[S + i] - o);
-        if ((i & 31) == 0) origin16[slot0 + (uint32_t)(i >> 5)] = o;
+        if ((i & (BL - 1)) == 0) origin16[slot0 + (uint32_t)(i >> H16_SHIFT)] = o;
       }
     }
   }

@@ -392,3 +392,87 @@ def test_reversed_field(lfmod, oracle, params):
     got = _gpu_run(lfmod, G, params, b, debug=True)
     assert_tracks_equal(got, ref, "reversed field")
     assert_debug_equal(got.debug, ref.debug)
+
+
+def _rule_config2(b, got, ref, what, min_same=0.995):
+    """BASELINE.json configs[2] rule: >= 99.5 % identical hit lists, truth-matched efficiency within 0.2 % absolute."""
+    from paper_2402_14670_b200 import truth
+    common, ig, ir = np.intersect1d(got.seed_idx, ref.seed_idx, return_indices=True)
+    same = (got.hit_idx[ig] == ref.hit_idx[ir]).all(1)
+    frac = same.sum() / ref.n_tracks
+    e_got, e_ref = truth.evaluate(b, got.hit_idx, got.n_hits), truth.evaluate(b, ref.hit_idx, ref.n_hits)
+    print(f"{what}: identical hit lists {frac:.5f} of {ref.n_tracks}; eff {e_got.efficiency:.5f} vs {e_ref.efficiency:.5f}")
+    assert frac >= min_same and abs(e_got.efficiency - e_ref.efficiency) <= 0.002
+    return frac
+
+
+def test_config2_packed_input_and_fp16_only(lfmod, oracle, geometry, params):
+    """hit_storage = 1 with the caller's packed copy (lf_pack_hits): identical to the library packing it, and within the
+    configs[2] rule.  With the fp32 hits dropped every stage reads the fp16 copy (2.5 bytes per hit instead of 4; only the
+    packed copy crosses PCIe in lf_run_host): a LOSSY mode outside the configs[2] rule, because extension and fit then
+    see the fp16 rounding (<= 0.03 mm typically) next to a 0.08 mm resolution: the efficiency is unchanged but only about
+    98.5 % of the hit lists stay identical."""
+    import torch
+    b = dg.generate_config(2)
+    P16 = dict(params, hit_storage=1)
+    ref = oracle.run(geometry, params, b, threads=NTHREADS)
+    lf = lfmod.LookingForward(geometry, P16, b.n_events, b.n_seeds, b.n_hits)
+    db = lfmod.DeviceBatch(b)
+    a = lf.run(db)
+    torch.cuda.synchronize()
+    a = a.to_numpy()
+    lf.pack_hits(db)
+    # the packed copy follows the documented encoding: hit = origin(block) + half; the error is half an fp16 ulp of the
+    # offset to the block origin (<= 0.125 mm for offsets below 512 mm, <= 0.25 mm below 1024 mm)
+    x16, org = db.hit_x16.cpu().numpy().astype(np.float32), db.origin16.cpu().numpy()
+    S = np.repeat(b.seg_offsets[:-1].astype(np.int64), np.diff(b.seg_offsets.astype(np.int64)))
+    g = np.repeat(np.arange(b.n_events * 24), np.diff(b.seg_offsets.astype(np.int64)))
+    i = np.arange(b.n_hits) - S
+    dec = org[(S >> 3) + g + (i >> 3)] + x16
+    err = np.abs(dec - b.hit_x)
+    assert err.max() <= 1.0 and np.percentile(err, 99) <= 0.26 and np.median(err) <= 0.07
+    c = lf.run(db)          # x and x16 given: windows + seeding on the caller's copy, extension + fit on fp32
+    torch.cuda.synchronize()
+    c = c.to_numpy()
+    assert c.n_tracks == a.n_tracks and np.array_equal(c.hit_idx, a.hit_idx) and np.array_equal(c.state.view(np.uint32), a.state.view(np.uint32))
+    _rule_config2(b, c, ref, "fp16 windows+seeding, fp32 extension+fit")
+    db.drop_fp32()          # fp16 only
+    d = lf.run(db)
+    torch.cuda.synchronize()
+    d = d.to_numpy()
+    _rule_config2(b, d, ref, "fp16 everywhere (lossy, outside the rule)", min_same=0.98)
+    hb = lfmod.HostBatch(b).use_packed(db)
+    assert hb.hit_x is None and hb.h2d_bytes() < 0.75 * lfmod.HostBatch(b, pin=False).h2d_bytes()
+    ht = lfmod.HostTracks(b.n_seeds, b.n_events)
+    lf.set_host_chunk_events(64)
+    assert lf.run_host(hb, ht) == d.n_tracks
+    e = ht.to_numpy()
+    assert np.array_equal(e.hit_idx, d.hit_idx) and np.array_equal(e.state.view(np.uint32), d.state.view(np.uint32))
+    lf.close()
+
+
+def test_fp16_only_events_larger_than_the_stage(lfmod, oracle, geometry, params):
+    """fp16-only input with events that do not fit the shared-memory stage: the window kernel decodes them once into the
+    library's fp32 scratch image; the result equals the staged decoding of the same packed hits."""
+    import torch
+    cfg = dg.GenConfig("huge16", 6, 19, true_fixed=60, fake_mean=5.0, noise_fixed=1000)
+    b = dg.generate(cfg)
+    P16 = dict(params, hit_storage=1)
+    small = lfmod.LookingForward(geometry, P16, b.n_events, b.n_seeds, b.n_hits)              # stage sized for these events
+    tiny = lfmod.LookingForward(geometry, P16, 100 * b.n_events, b.n_seeds, b.n_hits)         # 2 048-hit stage: all oversize
+    assert b.n_hits / b.n_events <= small.info().staged_hits_per_event
+    assert np.diff(b.seg_offsets[::24].astype(np.int64)).min() > tiny.info().staged_hits_per_event
+    db = lfmod.DeviceBatch(b)
+    small.pack_hits(db)
+    db.drop_fp32()
+    r1 = small.run(db)
+    r2 = tiny.run(db)
+    torch.cuda.synchronize()
+    r1, r2 = r1.to_numpy(), r2.to_numpy()
+    assert r1.n_tracks == r2.n_tracks > 100 and np.array_equal(r1.hit_idx, r2.hit_idx)
+    assert np.array_equal(r1.state.view(np.uint32), r2.state.view(np.uint32))
+    ref = oracle.run(geometry, params, b)
+    common, ig, ir = np.intersect1d(r2.seed_idx, ref.seed_idx, return_indices=True)
+    assert ((r2.hit_idx[ig] == ref.hit_idx[ir]).all(1).sum() / ref.n_tracks) > 0.95  # fp16 everywhere is lossy
+    small.close()
+    tiny.close()
