@@ -192,7 +192,7 @@ def tuning_params(args, datagen, cfg):
     """--tuning with-ut: Table 3 "Forward" column (BASELINE.json configs); no-ut: section VI.E."""
     if args.tuning == "no-ut":
         return datagen.no_ut_params()
-    return dict(datagen.default_params(), hit_storage=cfg.hit_storage)
+    return dict(datagen.default_params(), hit_storage=cfg.hit_storage, seed_arith=1 if args.seed_arith == "fp32" else 0)
 
 
 def oracle_rate(batch, threads: int, geometry, params):
@@ -266,6 +266,11 @@ def run_ours(args):
     lf = binding.LookingForward(G, P, batch.n_events, batch.n_seeds, batch.n_hits)
     info = lf.info()
     db = binding.DeviceBatch(batch, dev)
+    fp16_mode = args.fp16_input if int(P.get("hit_storage", 0)) == 1 else None
+    if fp16_mode in ("caller", "only"):
+        lf.pack_hits(db)
+        if fp16_mode == "only":
+            db.drop_fp32()
     out = binding.TrackBuffers(batch.n_seeds, batch.n_events, dev)
     stream = torch.cuda.current_stream()
 
@@ -310,6 +315,8 @@ def run_ours(args):
     e2e = None
     if not args.no_e2e:
         hb = binding.HostBatch(batch)
+        if fp16_mode in ("caller", "only"):
+            hb.use_packed(db, keep_fp32=(fp16_mode == "caller"))
         ht = binding.HostTracks(batch.n_seeds, batch.n_events)
         for _ in range(2):
             lf.run_host(hb, ht, stream)
@@ -406,9 +413,10 @@ def run_ours(args):
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"{cfg.name}: {batch.n_events} events per GPU, {'high' if args.config == 4 else 'Run-3-like'} occupancy, fp32"
-                               + (" with fp16 hit storage" if int(P.get("hit_storage", 0)) == 1 else "") + ", one lf_run on one stream"
+                               + ((" with fp16 hit storage, " + args.seed_arith + " seeding") if int(P.get("hit_storage", 0)) == 1 else "")
+                               + ", one lf_run on one stream"
                                + (", no-UT tuning (PAPER.md:285-325)" if no_ut else ""),
-                   "tuning": args.tuning,
+                   "tuning": args.tuning, "fp16_input": fp16_mode,
                    "events_per_gpu": batch.n_events, "seeds_per_gpu": batch.n_seeds, "hits_per_gpu": batch.n_hits,
                    "tracks_per_step_per_gpu": n_tracks, "accepted_candidates_per_step": n_acc, "events_with_equal_hits": n_dup_events,
                    "l2": f"no flush: inputs ({in_bytes / 1e6:.0f} MB) + outputs exceed the 126 MB L2",
@@ -444,6 +452,11 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--tuning", choices=["with-ut", "no-ut"], default="with-ut",
                     help="with-ut: BASELINE.json's headline (default); no-ut: the no-UT tuning of PAPER.md:285-325 on the same events")
+    ap.add_argument("--seed-arith", choices=["half2", "fp32"], default="half2",
+                    help="config 2 (fp16 hit storage) only: half2 = pairs of doublets in __half2 (PAPER.md:366), fp32 = one doublet per lane")
+    ap.add_argument("--fp16-input", choices=["library", "caller", "only"], default="library",
+                    help="config 2 only: library = lf_run packs the fp32 hits itself (default); caller = the caller hands the packed "
+                         "copy next to the fp32 hits; only = the packed copy alone (every stage on fp16: lossy, outside configs[2]'s rule)")
     ap.add_argument("--events", type=int, default=None, help="override the number of events (default: the config's)")
     ap.add_argument("--cpu-events", type=int, default=6000, help="events of the single-thread oracle sample")
     ap.add_argument("--no-e2e", action="store_true")

@@ -108,6 +108,9 @@ typedef struct {
   float velo_p_min, velo_pt_min; /* assumed minimum momentum / transverse momentum, GeV: 5, 1; > 0 */
   float xtol_poly[8];            /* c0..c7 of Eq. (7), Table 5 */
   float x_overlap;               /* overlap of the LEFT and RIGHT windows of Eq. (8): 5 mm */
+  /* read only when hit_storage == 1 */
+  int32_t seed_arith;            /* 0 = the seeding kernel evaluates PAIRS of doublets in __half2 ("two combinations at a time",
+                                    PAPER.md:366); 1 = one doublet per lane in fp32 on the decoded fp16 hits (for comparison) */
 } lf_params;
 
 /* Input seeds: upstream track states at z_seed, SoA, all events back to back. */

@@ -47,7 +47,7 @@ class lf_params(C.Structure):
                 ("mag_tol_tx", C.c_float), ("mag_tol_max", C.c_float),
                 ("hit_storage", C.c_int32),
                 ("mode", C.c_int32), ("velo_p_min", C.c_float), ("velo_pt_min", C.c_float),
-                ("xtol_poly", C.c_float * 8), ("x_overlap", C.c_float)]
+                ("xtol_poly", C.c_float * 8), ("x_overlap", C.c_float), ("seed_arith", C.c_int32)]
 
 
 class lf_seeds(C.Structure):

@@ -57,6 +57,7 @@ struct lf_handle {
   __half* hx16;     /* hit_storage = 1 only: the library's own fp16 copy (when the caller gives none) */
   float* origin16;
   float* hx_scratch; /* hit_storage = 1 only: fp32 image of events that do not fit the stage (lf_kernels.cuh, fetch_event) */
+  bool half2;       /* hit_storage = 1: the seeding kernel evaluates pairs of doublets in __half2 (seed_triplets_h2) */
   bool wide;        /* the wide build of the event kernels runs (no-UT mode, or caps beyond the narrow limits) */
   int sides;        /* followed tracks (rows) per seed: 2 in the no-UT mode */
   uint32_t* win;
@@ -100,7 +101,7 @@ bool uv_layer(int l) { return (l & 3) == 1 || (l & 3) == 2; }
  * value any handle has asked for and only ever raises the attribute. */
 std::mutex g_attr_mutex;
 constexpr int MAX_DEVICES = 64;
-int g_attr_max[2][4][2][MAX_DEVICES]; /* [wide][kernel][debug][device] */
+int g_attr_max[3][4][2][MAX_DEVICES]; /* [narrow / wide / narrow half2][kernel][debug][device] */
 
 cudaError_t raise_dynamic_smem(const void* kernel, int wide, int k, int dbg, int device, int bytes) {
   std::lock_guard<std::mutex> lock(g_attr_mutex);
@@ -245,6 +246,7 @@ const char* validate(const lf_geometry& G, const lf_params& P) {
   if (!(P.T_triplet > 0) || !(P.T_x > 0) || !(P.T_y > 0) || !(P.T_uv_min > 0) || !(P.T_Q > 0) || !(P.T_ty > 0))
     return "params: tolerances must be positive";
   if (P.hit_storage != 0 && P.hit_storage != 1) return "params.hit_storage must be 0 or 1";
+  if (P.hit_storage == 1 && P.seed_arith != 0 && P.seed_arith != 1) return "params.seed_arith must be 0 (half2 pairs) or 1 (fp32)";
   {
     /* every tolerance is finite ("no cap" is a large finite number, not inf: the kernels bracket with it) */
     const float pf[] = {P.T_triplet, P.T_x, P.T_uv_slope, P.T_uv_min, P.T_ty, P.T_y, P.T_Q, P.C_nhits[0], P.C_nhits[1],
@@ -326,7 +328,8 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
   A.scratch_writer = 0;
   if (work) {
     A.ticket = h->tickets + 1;
-    lf::lf_seed_kernel<DEBUG, WIDE><<<grid_of(1), lf::SEED_THREADS, h->smem_bytes[1], st>>>(h->C, A);
+    if (!WIDE && h->half2) lf::lf_seed_kernel<DEBUG, false, true><<<grid_of(1), lf::SEED_THREADS, h->smem_bytes[1], st>>>(h->C, A);
+    else lf::lf_seed_kernel<DEBUG, WIDE><<<grid_of(1), lf::SEED_THREADS, h->smem_bytes[1], st>>>(h->C, A);
   }
   if (prof) LF_CUDA(h, cudaEventRecord(pe[2], st));
   if (hits->x != nullptr) { /* extension and fit read the fp32 hits when the caller gave them */
@@ -427,6 +430,7 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   h->max_events = max_events; h->max_seeds = max_seeds; h->max_hits = max_hits;
   make_consts(*geometry, *params, h->C);
   h->wide = use_wide(*params);
+  h->half2 = params->hit_storage == 1 && params->seed_arith != 1;
   h->sides = h->C.sides;
 
   auto bail = [&](lf_status st, const std::string& msg) { g_create_error = msg; lf_destroy(h); return st; };
@@ -452,7 +456,7 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   }
   const size_t stage_bytes = (size_t)lf::HDR_BYTES + (size_t)h->stage_cap * sizeof(float);
   h->smem_bytes[0] = (int)stage_bytes;
-  h->smem_bytes[1] = (int)(stage_bytes + (h->wide ? sizeof(lf::SeedTables<true>) : sizeof(lf::SeedTables<false>)));
+  h->smem_bytes[1] = (int)(stage_bytes + (h->wide ? sizeof(lf::SeedTables<true, false>) : (h->half2 ? sizeof(lf::SeedTables<false, true>) : sizeof(lf::SeedTables<false, false>))));
   h->smem_bytes[2] = (int)(stage_bytes + lf::ext_tables_bytes(params->n_triplets));
   h->smem_bytes[3] = (int)(stage_bytes + lf::FIT_TABLES_BYTES);
   const void* kern_n[4][2] = {{(const void*)lf::lf_window_kernel<false, false>, (const void*)lf::lf_window_kernel<true, false>},
@@ -463,11 +467,13 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
                               {(const void*)lf::lf_seed_kernel<false, true>, (const void*)lf::lf_seed_kernel<true, true>},
                               {(const void*)lf::lf_extend_kernel<false, true>, (const void*)lf::lf_extend_kernel<true, true>},
                               {(const void*)lf::lf_fit_kernel<false, true>, (const void*)lf::lf_fit_kernel<true, true>}};
+  const void* kern_h2[2] = {(const void*)lf::lf_seed_kernel<false, false, true>, (const void*)lf::lf_seed_kernel<true, false, true>};
+  if (h->half2) { kern_n[1][0] = kern_h2[0]; kern_n[1][1] = kern_h2[1]; }
   const void* (*kern)[2] = h->wide ? kern_w : kern_n;
   const int threads[4] = {lf::WIN_THREADS, lf::SEED_THREADS, lf::FIT_THREADS, lf::FIT_THREADS};
   for (int k = 0; k < 4; ++k) {
     for (int d = 0; d < 2; ++d)
-      LF_CREATE_CUDA(raise_dynamic_smem(kern[k][d], h->wide ? 1 : 0, k, d, h->device, h->smem_bytes[k]));
+      LF_CREATE_CUDA(raise_dynamic_smem(kern[k][d], h->wide ? 1 : (h->half2 && k == 1 ? 2 : 0), k, d, h->device, h->smem_bytes[k]));
     LF_CREATE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->ctas_per_sm[k], kern[k][0], threads[k], h->smem_bytes[k]));
     if (h->ctas_per_sm[k] < 1) return bail(LF_ERR_CUDA, "lf_create: an event kernel does not fit on an SM");
     h->grid[k] = h->sm_count * h->ctas_per_sm[k];

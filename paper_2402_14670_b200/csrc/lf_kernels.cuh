@@ -628,6 +628,11 @@ struct __align__(16) SeedScratch {
   uint16_t code[TRIP_BUF];
   int4 setw[2]; /* per layer set: first and end of the h1 window, first of the h2 window (event-relative) */
 };
+/* + the per-h0 references of the half2 pair evaluation (hit_storage = 1): x2 of the first doublet of the h0 hit's
+ * bracket and, for that doublet in fp32, its slope t, its opening at the magnet and its expected x1 */
+struct __align__(16) SeedScratchH2 : SeedScratch {
+  float4 ref[2][32];
+};
 
 /* Rank selection on the warp's triplets: keeps the `keep` smallest of `n` (<= TRIP_BUF) by the key (chi2, position in the
  * buffer) and leaves them SORTED ascending in W.chi2 / W.code [0, min(n, keep)).  The buffer is in candidate order and a
@@ -740,8 +745,15 @@ __device__ __forceinline__ int lanes_below(float xv, float v) {
  * whose candidate belongs to either set fetches them with two 16-byte loads instead of a select per constant). */
 struct __align__(16) SetConsts {
   float inv_dz, zmag_a, zb, za;
-  float K, pad0, pad1, pad2;
+  float K;
+  /* half2 pair evaluation (seed_triplets_h2): both halves hold inv_dz, r = inv_dz * zmag_a, c = inv_dz * (zb - za * K) */
+  uint32_t inv_dz2, r2, c2;
 };
+__device__ __forceinline__ uint32_t h2_bits(float v) {
+  const __half2 h = __float2half2_rn(v);
+  return *reinterpret_cast<const uint32_t*>(&h);
+}
+__device__ __forceinline__ __half2 h2_of(uint32_t bits) { return *reinterpret_cast<const __half2*>(&bits); }
 __device__ __forceinline__ void fill_set_consts(const Consts& C, SetConsts* sc) {
   if (threadIdx.x < 2) {
     const int s = threadIdx.x;
@@ -750,7 +762,9 @@ __device__ __forceinline__ void fill_set_consts(const Consts& C, SetConsts* sc) 
     sc[s].zb = C.z[s ? 7 : 4];
     sc[s].za = C.z[s ? 3 : 0];
     sc[s].K = C.K[s];
-    sc[s].pad0 = sc[s].pad1 = sc[s].pad2 = 0.0f;
+    sc[s].inv_dz2 = h2_bits(C.inv_dz_ac[s]);
+    sc[s].r2 = h2_bits(C.inv_dz_ac[s] * C.zmag_a[s]);
+    sc[s].c2 = h2_bits(C.inv_dz_ac[s] * (C.z[s ? 7 : 4] - C.z[s ? 3 : 0] * C.K[s]));
   }
 }
 
@@ -894,6 +908,182 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
   if (DEBUG) {
     if (lane == 0 && A.dbg.counters) {
       atomicAdd(A.dbg.counters + 3, (unsigned long long)total);
+      atomicAdd(A.dbg.counters + 6, (unsigned long long)ntr);
+    }
+    const size_t seed = (size_t)EP.s0 + k_seed;
+    const int set = (low >> 15) & 1, la = set ? 3 : 0;
+    const int fa = (int)(__shfl_sync(FULL, winw, la) >> 6), fb = (int)(__shfl_sync(FULL, winw, la + 4) >> 6);
+    const int fc = (int)(__shfl_sync(FULL, winw, la + 8) >> 6);
+    if (lane == 0 && A.dbg.n_triplets) A.dbg.n_triplets[seed] = ntr;
+    if (lane < NT) {
+      const size_t o = (size_t)seed * NT + lane;
+      if (A.dbg.trip_set) A.dbg.trip_set[o] = mine ? set : -1;
+      if (A.dbg.trip_chi2) A.dbg.trip_chi2[o] = mine ? __uint_as_float(W.chi2[lane]) : -1.0f;
+      if (A.dbg.trip_hits) {
+        A.dbg.trip_hits[o * 3 + 0] = mine ? (int32_t)(h0 + fa + ((low >> 10) & 31)) : -1;
+        A.dbg.trip_hits[o * 3 + 1] = mine ? (int32_t)(h0 + fb + (low & 31)) : -1;
+        A.dbg.trip_hits[o * 3 + 2] = mine ? (int32_t)(h0 + fc + ((low >> 5) & 31)) : -1;
+      }
+    }
+  }
+  __syncwarp();
+}
+
+/* a3 with fp16 hit storage (params.hit_storage = 1; "Using fp16 allows us to use half-2 vectorized instructions
+ * ... processing two combinations at a time"): the same scheme as seed_triplets, but a lane evaluates a PAIR of
+ * neighbouring doublets (h0, j0) and (h0, j0 + 1) of one h0 hit with __half2 arithmetic.  To keep binary16 accurate the
+ * pair works on small quantities: per h0 hit the first doublet of its bracket is evaluated in fp32 (slope t_ref, opening
+ * at the magnet m_ref, expected x1 e_ref) and a doublet of the bracket differs from it by d = x2 - x2_ref < 2 * 41 mm:
+ *   t = t_ref + d * inv_dz,  opening = m_ref + d * (inv_dz * zmag_a),  x1_expected = e_ref + d * inv_dz * (zb - za * K),
+ * all three exact identities of PAPER.md:210-215.  The closest h1 and the chi2 are fp32 on the decoded hits.  Decisions
+ * are taken in binary16 here, so this kernel is judged by BASELINE.json configs[2]'s rule, not bit for bit. */
+template <bool DEBUG, class HV>
+__device__ __forceinline__ void seed_triplets_h2(const Consts& C, const EventArgs& A, const HV& hx, uint32_t h0,
+                                                 const SeedEventPtrs& EP, uint32_t k_seed, SeedScratchH2& W, const SetConsts* SC,
+                                                 int lane, bool dup) {
+  constexpr bool STG = std::is_same<HV, HitView<true> >::value;
+  const uint32_t* rowp = EP.rows + k_seed * WIN_ROW;
+  const uint32_t winw = (lane < WIN_ROW) ? rowp[lane] : 0u;
+  const float x_mag = __uint_as_float(__shfl_sync(FULL, winw, 12)), tx = __uint_as_float(__shfl_sync(FULL, winw, 13));
+  const float qop = __uint_as_float(__shfl_sync(FULL, winw, 14));
+  const bool low_p = (__shfl_sync(FULL, winw, 15) & ROW_LOW_P) != 0u;
+  const float aq = fmaxf(fabsf(qop), 1e-6f);
+  const float kq = C.kick * qop;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  const float tol0 = C.mag_tol_base + C.mag_tol_inv_p * aq;
+  const float INF = __int_as_float(0x7f800000);
+  const float tol0m = tol0 + INTERVAL_MARGIN, tolmaxm = C.mag_tol_max + INTERVAL_MARGIN;
+  unsigned slots_p = 0, cnt_p = 0, jlo_p = 0; /* set 0 in the low half-word, set 1 in the high one */
+#pragma unroll
+  for (int set = 0; set < 2; ++set) {
+    const int la = set ? 3 : 0;
+    const uint32_t wa = __shfl_sync(FULL, winw, la), wb = __shfl_sync(FULL, winw, la + 4), wc = __shfl_sync(FULL, winw, la + 8);
+    const int fa = (int)(wa >> 6), na = (int)(wa & 63u), fb = (int)(wb >> 6), nb = (int)(wb & 63u);
+    const int fc = (int)(wc >> 6), nc = (int)(wc & 63u);
+    if (lane == set) W.setw[set] = make_int4(fb, fb + nb, fc, fc + nc);
+    const bool have = (lane < na) && (nb != 0);
+    const float x0 = (STG || lane < na) ? hx[fa + lane] : 0.0f;
+    const float x2r = (STG || lane < nc) ? hx[fc + lane] : 0.0f;
+    const float x2v = (lane < nc) ? x2r : INF;
+    const float Aoff = x0 - x_mag;
+    const float tmax = __fmaf_rn(fabsf(Aoff), C.inv_abs_zmag_a[set], C.tolmax_over_zmag[set]);
+    const float tol_sup = fminf(tolmaxm, __fmaf_rn(C.mag_tol_tx, tmax, tol0m));
+    const float inv_r = C.inv_r[set];
+    const int jlo = lanes_below<false>(x2v, __fmaf_rn(tol_sup - Aoff, inv_r, x0));
+    const int jhi = min(nc, lanes_below<true>(x2v, __fmaf_rn(-tol_sup - Aoff, inv_r, x0)));
+    const int cnt = have ? max(jhi - jlo, 0) : 0;
+    /* the bracket's first doublet in fp32: the reference of the h0 hit's pairs */
+    const float x2ref = __shfl_sync(FULL, x2r, min(jlo, 31));
+    const float t_ref = (x2ref - x0) * C.inv_dz_ac[set];
+    const float m_ref = (x0 + t_ref * C.zmag_a[set]) - x_mag;
+    const float e_ref = C.z[set ? 7 : 4] * t_ref + (x0 - t_ref * C.z[set ? 3 : 0]) * C.K[set];
+    W.ref[set][lane] = make_float4(x2ref, t_ref, m_ref, e_ref);
+    slots_p |= (unsigned)((cnt + 1) >> 1) << (16 * set);
+    cnt_p |= (unsigned)cnt << (16 * set);
+    jlo_p |= (unsigned)jlo << (16 * set);
+  }
+  /* ---- dense lane-per-PAIR evaluation over both sets: inclusive scan of the per-h0 pair counts */
+  unsigned incl_p = slots_p;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const unsigned v = __shfl_up_sync(FULL, incl_p, o);
+    if (lane >= o) incl_p += v;
+  }
+  const unsigned tot_p = __shfl_sync(FULL, incl_p, 31);
+  const int total0 = (int)(tot_p & 0xFFFFu), total = total0 + (int)(tot_p >> 16);
+  __syncwarp(); /* W.setw, W.ref */
+  /* seed constants of the pair arithmetic, both halves equal */
+  const __half2 tx2 = __float2half2_rn(tx), tol02 = __float2half2_rn(tol0), tolmax2 = __float2half2_rn(C.mag_tol_max);
+  const __half2 txc2 = __float2half2_rn(C.mag_tol_tx), sgn2 = __float2half2_rn(kq > 0.0f ? 1.0f : (kq < 0.0f ? -1.0f : 0.0f));
+  const __half2 zero2 = __float2half2_rn(0.0f);
+  int tcount = 0, n_eval = 0, n_ok = 0, n_pass = 0;
+  for (int base = 0; base < total; base += 32) {
+    const int tau = base + lane;
+    const bool act = tau < total;
+    const int set = (tau >= total0) ? 1 : 0;
+    const int ts = set ? tau - total0 : tau;
+    const unsigned sel = set ? 0x4432u : 0x4410u;
+    int owner = 15;
+#pragma unroll
+    for (int s = 16; s >= 2; s >>= 1) {
+      const unsigned v = __shfl_sync(FULL, incl_p, owner);
+      owner += (((int)__byte_perm(v, 0u, sel) <= ts) ? s : 0) - (s >> 1);
+    }
+    {
+      const unsigned v = __shfl_sync(FULL, incl_p, owner);
+      if ((int)__byte_perm(v, 0u, sel) <= ts) owner += 1;
+    }
+    const unsigned ip = __shfl_sync(FULL, incl_p, owner), sp = __shfl_sync(FULL, slots_p, owner);
+    const unsigned jp = __shfl_sync(FULL, jlo_p, owner), cp = __shfl_sync(FULL, cnt_p, owner);
+    const int before = (int)__byte_perm(ip, 0u, sel) - (int)__byte_perm(sp, 0u, sel);
+    const int pair = ts - before;                                   /* pair of the h0 hit's bracket */
+    const int j0 = (int)__byte_perm(jp, 0u, sel) + 2 * pair;       /* h2 index of its first doublet */
+    const bool two = 2 * pair + 1 < (int)__byte_perm(cp, 0u, sel); /* the pair's second doublet exists */
+    bool ok[2] = {false, false};
+    float x1e[2] = {0.0f, 0.0f};
+    int4 wv = make_int4(0, 0, 0, 0);
+    if (act) {
+      wv = W.setw[set]; /* fb, fb + nb, fc, fc + nc */
+      const float4 ref = W.ref[set][owner]; /* x2_ref, t_ref, m_ref, e_ref */
+      const float x2a = hx[wv.z + j0];
+      const float x2b = (STG || two) ? hx[wv.z + j0 + 1] : x2a;
+      /* two combinations at a time */
+      const __half2 d2 = __floats2half2_rn(x2a - ref.x, x2b - ref.x);
+      const __half2 t2 = __hfma2(d2, h2_of(SC[set].inv_dz2), __float2half2_rn(ref.y));
+      const __half2 m2 = __hfma2(d2, h2_of(SC[set].r2), __float2half2_rn(ref.z));
+      const __half2 tol2 = __hmin2(tolmax2, __hfma2(__habs2(t2), txc2, tol02));
+      unsigned okm = __hlt2_mask(__habs2(m2), tol2);                                        /* filter 2 */
+      if (low_p) okm &= __hgt2_mask(__hmul2(__hsub2(t2, tx2), sgn2), zero2);                 /* filter 1 */
+      const __half2 e2 = __hmul2(d2, h2_of(SC[set].c2));
+      x1e[0] = ref.w + __low2float(e2);
+      x1e[1] = ref.w + __high2float(e2);
+      ok[0] = (okm & 0xFFFFu) != 0u;
+      ok[1] = two && (okm >> 16) != 0u;
+    }
+    if (DEBUG) {
+      n_eval += __popc(__ballot_sync(FULL, act)) + __popc(__ballot_sync(FULL, act && two));
+      n_ok += __popc(__ballot_sync(FULL, ok[0])) + __popc(__ballot_sync(FULL, ok[1]));
+    }
+#pragma unroll
+    for (int e = 0; e < 2; ++e) { /* the pair's doublets in turn: closest h1 and chi2 cut in fp32 */
+      bool pass = false;
+      uint32_t chi2b = 0u, code = 0u;
+      if (ok[e]) {
+        float dx;
+        const int k = closest_in_window<false>(hx, wv.x, wv.y, x1e[e], dup, dx);
+        const float chi2 = dx * dx;
+        if (chi2 < C.T_triplet) {
+          pass = true;
+          chi2b = __float_as_uint(chi2);
+          code = (unsigned)((set << 15) | (owner << 10) | ((j0 + e) << 5) | (k - wv.x));
+        }
+      }
+      const unsigned m = __ballot_sync(FULL, pass);
+      if (m) {
+        if (DEBUG) n_pass += __popc(m);
+        if (tcount > 32) tcount = select_smallest(W, tcount, C.n_triplets, lane);
+        if (pass) {
+          const int slot = tcount + __popc(m & lt_mask);
+          W.chi2[slot] = chi2b;
+          W.code[slot] = (uint16_t)code;
+        }
+        tcount += __popc(m);
+        __syncwarp();
+      }
+    }
+  }
+  if (tcount > 0) tcount = select_smallest(W, tcount, C.n_triplets, lane);
+  const int ntr = tcount;
+  const int NT = C.n_triplets;
+  if (lane == 0) EP.n_trip[k_seed] = (uint8_t)ntr;
+  const bool mine = lane < ntr;
+  const unsigned low = mine ? (unsigned)W.code[lane] : 0u;
+  if (lane < NT) EP.codes[k_seed * (uint32_t)NT + (uint32_t)lane] = (uint16_t)low;
+  if (DEBUG) {
+    if (lane == 0 && A.dbg.counters) {
+      atomicAdd(A.dbg.counters + 3, (unsigned long long)n_eval);
+      atomicAdd(A.dbg.counters + 4, (unsigned long long)n_ok);
+      atomicAdd(A.dbg.counters + 5, (unsigned long long)n_pass);
       atomicAdd(A.dbg.counters + 6, (unsigned long long)ntr);
     }
     const size_t seed = (size_t)EP.s0 + k_seed;
@@ -1082,19 +1272,21 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
   __syncwarp();
 }
 
-template <bool WIDE>
+template <bool WIDE, bool H2>
 struct __align__(16) SeedTables {
   int next_seed;
   int pad[3];
   SetConsts sc[2];
-  typename std::conditional<WIDE, SeedScratchWide, SeedScratch>::type ws[SEED_WARPS];
+  typename std::conditional<WIDE, SeedScratchWide, typename std::conditional<H2, SeedScratchH2, SeedScratch>::type>::type ws[SEED_WARPS];
 };
 
-template <bool DEBUG, bool WIDE>
+/* H2: the half2 pair evaluation of seed_triplets_h2 (narrow build, hit_storage = 1) */
+template <bool DEBUG, bool WIDE, bool H2 = false>
 __global__ void __launch_bounds__(SEED_THREADS, WIDE ? 4 : 5) lf_seed_kernel(const __grid_constant__ Consts C,
                                                                            const __grid_constant__ EventArgs A) {
+  static_assert(!(WIDE && H2), "the half2 pair evaluation exists in the narrow build only");
   CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
-  SeedTables<WIDE>& T = *reinterpret_cast<SeedTables<WIDE>*>(lf_smem + HDR_BYTES + (size_t)A.stage_cap * sizeof(float));
+  SeedTables<WIDE, H2>& T = *reinterpret_cast<SeedTables<WIDE, H2>*>(lf_smem + HDR_BYTES + (size_t)A.stage_cap * sizeof(float));
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (threadIdx.x == 0) {
     mbar_init(&H.mbar, 1);
@@ -1134,6 +1326,9 @@ __global__ void __launch_bounds__(SEED_THREADS, WIDE ? 4 : 5) lf_seed_kernel(con
           const int side = k - (k / sides) * sides;
           if (E.staged) seed_triplets_wide<DEBUG>(C, A, HitView<true>(E.skew), E.h0, seed, side, W, lane, dup);
           else seed_triplets_wide<DEBUG>(C, A, HitView<false>(E.gview), E.h0, seed, side, W, lane, dup);
+        } else if constexpr (H2) {
+          if (E.staged) seed_triplets_h2<DEBUG>(C, A, HitView<true>(E.skew), E.h0, EP, (uint32_t)k, W, T.sc, lane, dup);
+          else seed_triplets_h2<DEBUG>(C, A, HitView<false>(E.gview), E.h0, EP, (uint32_t)k, W, T.sc, lane, dup);
         } else {
           if (E.staged) seed_triplets<DEBUG>(C, A, HitView<true>(E.skew), E.h0, EP, (uint32_t)k, W, T.sc, lane, dup);
           else seed_triplets<DEBUG>(C, A, HitView<false>(E.gview), E.h0, EP, (uint32_t)k, W, T.sc, lane, dup);

@@ -219,21 +219,24 @@ def test_repeated_runs_and_capacity_errors(lfmod, geometry, params):
     lf2.close()
 
 
-def test_config2_fp16_hit_storage(lfmod, oracle, geometry, params):
-    """BASELINE.json configs[2]: fp16 storage of the hits for windows + seeding, fp32 fit.
+@pytest.mark.parametrize("seed_arith", [0, 1])
+def test_config2_fp16_hit_storage(lfmod, oracle, geometry, params, seed_arith):
+    """BASELINE.json configs[2]: fp16 storage of the hits for windows + seeding, fp32 extension and fit.  seed_arith 0 is
+    the half2 seeding kernel (pairs of doublets in __half2), 1 the fp32 arithmetic on the decoded fp16 hits.
     Rule: >= 99.5 % of the fp32 oracle's tracks reproduced with identical hit lists, and the truth-matched
     efficiency within 0.2 % absolute."""
     from paper_2402_14670_b200 import truth
     b = dg.generate_config(2)
     assert dg.CONFIGS[2].hit_storage == 1
+    P16 = dict(params, hit_storage=1, seed_arith=seed_arith)
     ref = oracle.run(geometry, params, b, threads=NTHREADS)
-    got = _gpu_run(lfmod, geometry, dict(params, hit_storage=1), b)
+    got = _gpu_run(lfmod, geometry, P16, b)
     common, ig, ir = np.intersect1d(got.seed_idx, ref.seed_idx, return_indices=True)
     same = (got.hit_idx[ig] == ref.hit_idx[ir]).all(1)
     frac = same.sum() / ref.n_tracks
     e_got = truth.evaluate(b, got.hit_idx, got.n_hits)
     e_ref = truth.evaluate(b, ref.hit_idx, ref.n_hits)
-    print(f"config2 fp16: identical hit lists {frac:.5f} of {ref.n_tracks}; tracks {got.n_tracks}; "
+    print(f"config2 fp16 (seed_arith {seed_arith}): identical hit lists {frac:.5f} of {ref.n_tracks}; tracks {got.n_tracks}; "
           f"eff {e_got.efficiency:.5f} vs {e_ref.efficiency:.5f}; ghost {e_got.ghost_rate:.5f} vs {e_ref.ghost_rate:.5f}")
     assert frac >= 0.995
     assert abs(e_got.efficiency - e_ref.efficiency) <= 0.002
@@ -242,8 +245,24 @@ def test_config2_fp16_hit_storage(lfmod, oracle, geometry, params):
     d = np.abs(got.state[ig][same].astype(np.float64) - ref.state[ir][same].astype(np.float64))
     assert d[:, 0].max() <= 2e-3 and d[:, 1].max() <= 2e-2 and d[:, 2].max() <= 3e-6 and d[:, 3].max() <= 3e-5
     # the fp16 path is deterministic too
-    got2 = _gpu_run(lfmod, geometry, dict(params, hit_storage=1), b)
+    got2 = _gpu_run(lfmod, geometry, P16, b)
     assert np.array_equal(got.hit_idx, got2.hit_idx) and np.array_equal(got.state.view(np.uint32), got2.state.view(np.uint32))
+    # the stage-boundary tables of the seeding kernel stay consistent in the half2 build: kept triplets are ordered by
+    # chi2, below the cut, and made of hits inside the seed's windows
+    dbg = _gpu_run(lfmod, geometry, P16, dg.generate_config(2, n_events=40), debug=True).debug
+    nt, c = dbg["n_triplets"], dbg["trip_chi2"]
+    for k in range(params["n_triplets"] - 1):
+        both = nt > k + 1
+        assert np.all(c[both, k] <= c[both, k + 1])
+    assert np.all(c[c >= 0] < params["T_triplet"]) and np.all(nt <= params["n_triplets"])
+    for i, l in ((0, (0, 3)), (1, (4, 7)), (2, (8, 11))):
+        h = dbg["trip_hits"][:, :, i]
+        st = dbg["trip_set"]
+        for s_, layer in enumerate(l):
+            m = (st == s_) & (h >= 0)
+            wf = np.broadcast_to(dbg["win_first"][:, layer][:, None], h.shape)[m]
+            wc = np.broadcast_to(dbg["win_count"][:, layer][:, None], h.shape)[m]
+            assert np.all(h[m] >= wf) and np.all(h[m] < wf + wc)
 
 
 def test_validate_inputs(lfmod, geometry, params):
