@@ -248,7 +248,10 @@ def run_ours(args):
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    if world > 1:
+    # under torchrun (any world size, 1 included) the job runs through torch.distributed: NCCL process group, barrier,
+    # max over ranks of the device time
+    distributed = world > 1 or ("RANK" in os.environ and "MASTER_ADDR" in os.environ)
+    if distributed:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
 
@@ -276,7 +279,7 @@ def run_ours(args):
 
     def barrier():
         torch.cuda.synchronize()
-        if world > 1:
+        if distributed:
             torch.distributed.barrier()
 
     for _ in range(max(args.warmup, 3)):
@@ -335,6 +338,9 @@ def run_ours(args):
         del hb, ht
 
     if rank != 0:
+        lf.close()
+        if distributed:
+            torch.distributed.destroy_process_group()
         return 0
 
     # ---- roofline of the dominant kernel (the slowest of the four event kernels): the HBM roofline BASELINE.json's metric
@@ -438,7 +444,7 @@ def run_ours(args):
     line.update(extra)
     print(json.dumps(line))
     lf.close()
-    if world > 1:
+    if distributed:
         torch.distributed.destroy_process_group()
     return 0
 

@@ -36,7 +36,7 @@ def reduce_job(local_ms: float, local_counts, device=None):
     import torch
     import torch.distributed as dist
     counts = [float(c) for c in local_counts]
-    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+    if not (dist.is_available() and dist.is_initialized()):
         return local_ms, counts
     t = torch.tensor([local_ms], dtype=torch.float64, device=device)
     c = torch.tensor(counts, dtype=torch.float64, device=device)

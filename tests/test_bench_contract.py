@@ -59,3 +59,30 @@ def test_gpu_arm_line(tuning):
     assert d["oracle_check"]["equal"] is True
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
     assert "workload" in d["config"] and "model" not in d["config"]
+
+
+def _torchrun(nproc, args, timeout=900):
+    port = 29600 + (os.getpid() % 1500)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={nproc}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.join(ROOT, "bench.py"), "--gpus", str(nproc)] + args
+    res = subprocess.run(cmd, capture_output=True, text=True, timeout=timeout, cwd=ROOT)
+    assert res.returncode == 0, res.stderr[-3000:]
+    lines = [l for l in res.stdout.splitlines() if l.strip().startswith("{")]
+    assert len(lines) == 1, f"exactly one JSON line expected from rank 0, got {len(lines)}"
+    return json.loads(lines[0])
+
+
+@pytest.mark.gpu
+def test_gpu_arm_under_torchrun():
+    """The N > 1 launch path of the contract on the hardware there is: torchrun, NCCL process group, barrier + max over
+    ranks of the device time, rank-seeded batches.  One rank per visible GPU, at most two (this pool hands out one GPU, so
+    this normally runs world size 1 through the same code: NCCL init is skipped only by torch when world == 1 is not
+    launched through torchrun, never here)."""
+    import torch
+    n = min(torch.cuda.device_count(), 2)
+    d = _torchrun(n, ["--steps", "3", "--warmup", "3", "--events", "600", "--no-cpu-baseline"])
+    assert d["n_gpus"] == n and d["scaling"] == "weak" and d["value"] > 0
+    assert d["config"]["events_per_gpu"] == 600
+    # whole-job aggregate: the units all ranks processed over the max-over-ranks time
+    assert abs(d["value"] - n * 600 / (d["ms_per_step"] * 1e-3)) / d["value"] < 1e-6
+    assert d["e2e"]["value"] > 0 and d["gpu_launches"] == 6 * 3
