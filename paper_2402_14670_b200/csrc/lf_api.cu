@@ -52,6 +52,7 @@ struct lf_handle {
   size_t max_events, max_seeds, max_hits;
   int device;
   int sm_count, stage_cap;
+  int stage_cap_x; /* the seeding kernel stages the six x layers only: about half an event */
   int regs[4], grid[4], ctas_per_sm[4], smem_bytes[4]; /* window, seed, extend, fit kernels */
   /* workspace */
   __half* hx16;     /* hit_storage = 1 only: the library's own fp16 copy (when the caller gives none) */
@@ -326,12 +327,14 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
   }
   if (prof) LF_CUDA(h, cudaEventRecord(pe[1], st));
   A.scratch_writer = 0;
+  A.stage_cap = h->stage_cap_x;
   if (work) {
     A.ticket = h->tickets + 1;
     if (!WIDE && h->half2) lf::lf_seed_kernel<DEBUG, false, true><<<grid_of(1), lf::SEED_THREADS, h->smem_bytes[1], st>>>(h->C, A);
     else lf::lf_seed_kernel<DEBUG, WIDE><<<grid_of(1), lf::SEED_THREADS, h->smem_bytes[1], st>>>(h->C, A);
   }
   if (prof) LF_CUDA(h, cudaEventRecord(pe[2], st));
+  A.stage_cap = h->stage_cap;
   if (hits->x != nullptr) { /* extension and fit read the fp32 hits when the caller gave them */
     A.hx16 = nullptr;
     A.origin16 = nullptr;
@@ -455,8 +458,10 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
     h->stage_cap = (int)std::min<size_t>(std::max<size_t>(cap, 2048), 16384);
   }
   const size_t stage_bytes = (size_t)lf::HDR_BYTES + (size_t)h->stage_cap * sizeof(float);
+  h->stage_cap_x = (h->stage_cap / 2 + 256 + 255) & ~255; /* half an event + its fluctuation + the runs' alignment gaps */
+  const size_t stage_bytes_x = (size_t)lf::HDR_BYTES + (size_t)h->stage_cap_x * sizeof(float);
   h->smem_bytes[0] = (int)stage_bytes;
-  h->smem_bytes[1] = (int)(stage_bytes + (h->wide ? sizeof(lf::SeedTables<true, false>) : (h->half2 ? sizeof(lf::SeedTables<false, true>) : sizeof(lf::SeedTables<false, false>))));
+  h->smem_bytes[1] = (int)(stage_bytes_x + (h->wide ? sizeof(lf::SeedTables<true, false>) : (h->half2 ? sizeof(lf::SeedTables<false, true>) : sizeof(lf::SeedTables<false, false>))));
   h->smem_bytes[2] = (int)(stage_bytes + lf::ext_tables_bytes(params->n_triplets));
   h->smem_bytes[3] = (int)(stage_bytes + lf::FIT_TABLES_BYTES);
   const void* kern_n[4][2] = {{(const void*)lf::lf_window_kernel<false, false>, (const void*)lf::lf_window_kernel<true, false>},

@@ -150,6 +150,7 @@ struct __align__(16) CtaHeader {
   int warp_tot[8];
   int dup; /* != 0: the event may hold equal neighbouring hits (closest_hit must resolve runs of ties) */
   int blk_pref[NSEG + 1]; /* fp16 hit storage: blocks of 32 hits in front of each segment of the event */
+  int xdelta[NL];         /* seeding kernel: hit i of an x layer l lives at stage position i - xdelta[l] (fetch_event_x) */
 };
 constexpr int HDR_BYTES = (sizeof(CtaHeader) + 15) & ~15;
 
@@ -329,6 +330,110 @@ __device__ __forceinline__ bool fetch_event(const EventArgs& A, uint32_t& phase,
     if (tid >= 32 && tid < 32 + tail) buf[E.skew + head + bulk + (tid - 32)] = gsrc[head + bulk + (tid - 32)];
     if (bulk > 0) {
       if (tid == 0) mbar_wait(&H.mbar, phase); /* one thread polls; the barrier below publishes */
+      phase ^= 1u;
+    }
+  }
+  __syncthreads();
+  return true;
+}
+
+/* fetch_event for the seeding kernel, which touches the six x layers only (0, 3, 4, 7, 8, 11): they form
+ * four contiguous runs of the event's hits, staged back to back by four bulk copies, so that the stage holds half an
+ * event and large events keep their CTAs per SM.  Hit i (event-relative) of x layer l then lives at stage position
+ * i - H.xdelta[l]; for an event that does not fit even so, xdelta = 0 and the hits are read from global memory. */
+__device__ __forceinline__ bool fetch_event_x(const EventArgs& A, uint32_t& phase, EventCtx& E) {
+  CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
+  float* buf = stage_buf();
+  const int tid = threadIdx.x;
+  __syncthreads();
+  if (tid == 0) H.ev = (int)atomicAdd(A.ticket, 1u);
+  __syncthreads();
+  E.ev = (uint32_t)H.ev;
+  if (E.ev >= A.n_events) return false;
+  const uint32_t* so = A.seg_off + (size_t)E.ev * NSEG;
+  E.h0 = so[0];
+  E.nh = (int)(so[NSEG] - E.h0);
+  if (tid == 32) H.dup = (int)A.ev_dup[E.ev];
+  const bool from16 = A.hx16 != nullptr;
+  E.skew = 0;
+  E.gview = from16 ? A.hx_scratch + E.h0 : A.hx + E.h0;
+  /* the four runs: segments [0,2), [6,10), [14,18), [22,24); stage base of run r keeps the 16-byte phase of its source */
+  int rs[4], rn[4], rb[4];
+  {
+    const int sa[4] = {0, 6, 14, 22}, sb[4] = {2, 10, 18, 24};
+    int pos = 0;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      rs[r] = (int)(so[sa[r]] - E.h0);
+      rn[r] = (int)(so[sb[r]] - so[sa[r]]);
+      const int sk = from16 ? 0 : (int)((reinterpret_cast<uintptr_t>(A.hx + E.h0 + rs[r]) >> 2) & 3);
+      rb[r] = pos + sk;
+      pos = (rb[r] + rn[r] + 3) & ~3;
+    }
+    E.staged = pos + 4 <= A.stage_cap;
+  }
+  if (tid < NL) {
+    const int r = (tid == 0) ? 0 : ((tid <= 4) ? 1 : ((tid <= 8) ? 2 : 3)); /* run of layer tid (x layers only matter) */
+    H.xdelta[tid] = E.staged ? ((r == 0 ? rs[0] - rb[0] : (r == 1 ? rs[1] - rb[1] : (r == 2 ? rs[2] - rb[2] : rs[3] - rb[3])))) : 0;
+  }
+  if (from16) {
+    if (tid < 32) {
+      const int nb = (tid < NSEG) ? (int)((so[tid + 1] - so[tid] + 31u) >> 5) : 0;
+      int incl = nb;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(FULL, incl, o);
+        if (tid >= o) incl += v;
+      }
+      if (tid <= NSEG) H.blk_pref[tid] = incl - nb;
+    }
+    __syncthreads();
+    if (E.staged) { /* oversized events were decoded into the scratch image by the window kernel */
+      const int lane = tid & 31, n_blk = H.blk_pref[NSEG];
+      const int pref = (lane < NSEG) ? H.blk_pref[lane] : 0x7FFFFFFF;
+      for (int blk = tid >> 5; blk < n_blk; blk += (int)(blockDim.x >> 5)) {
+        const int sg = __popc(__ballot_sync(FULL, pref <= blk)) - 1;
+        const int l = sg >> 1;
+        if ((l & 3) != 0 && (l & 3) != 3) continue; /* a u/v layer: not staged here */
+        const int b = blk - H.blk_pref[sg];
+        const uint32_t S = so[sg];
+        const int i = 32 * b + lane;
+        if (i < (int)(so[sg + 1] - S))
+          buf[(int)(S - E.h0) - H.xdelta[l] + i] =
+              __ldg(A.origin16 + ((S >> H16_SHIFT) + ((A.event_base + E.ev) * NSEG + (uint32_t)sg) + (uint32_t)(i >> H16_SHIFT))) +
+              __half2float(A.hx16[S + i]);
+      }
+    }
+  } else if (E.staged) {
+    /* per run: the 16-byte aligned interior by TMA, the ragged head / tail (at most 3 hits each) by plain loads */
+    const float* g0 = A.hx + E.h0;
+    int head[4], bulk[4];
+    uint32_t bytes = 0;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      head[r] = min(rn[r], (4 - (rb[r] & 3)) & 3);
+      bulk[r] = (rn[r] - head[r]) & ~3;
+      bytes += (uint32_t)bulk[r] * 4u;
+    }
+    if (tid == 0 && bytes > 0) {
+      fence_proxy_async();
+      mbar_expect_tx(&H.mbar, bytes);
+#pragma unroll
+      for (int r = 0; r < 4; ++r)
+        if (bulk[r] > 0) bulk_g2s(buf + rb[r] + head[r], g0 + rs[r] + head[r], (uint32_t)bulk[r] * 4u, &H.mbar);
+    }
+    if (tid >= 64 && tid < 96) {
+      const int r = (tid - 64) >> 3, e = (tid - 64) & 7; /* e < 4: head element e; else tail element e - 4 */
+      const int hd = (r == 0) ? head[0] : ((r == 1) ? head[1] : ((r == 2) ? head[2] : head[3]));
+      const int bk = (r == 0) ? bulk[0] : ((r == 1) ? bulk[1] : ((r == 2) ? bulk[2] : bulk[3]));
+      const int n = (r == 0) ? rn[0] : ((r == 1) ? rn[1] : ((r == 2) ? rn[2] : rn[3]));
+      const int s_ = (r == 0) ? rs[0] : ((r == 1) ? rs[1] : ((r == 2) ? rs[2] : rs[3]));
+      const int b_ = (r == 0) ? rb[0] : ((r == 1) ? rb[1] : ((r == 2) ? rb[2] : rb[3]));
+      const int i = (e < 4) ? e : hd + bk + (e - 4);
+      if ((e < 4) ? (e < hd) : (i < n)) buf[b_ + i] = g0[s_ + i];
+    }
+    if (bytes > 0) {
+      if (tid == 0) mbar_wait(&H.mbar, phase);
       phase ^= 1u;
     }
   }
@@ -779,6 +884,7 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
                                               const SeedEventPtrs& EP, uint32_t k_seed, SeedScratch& W, const SetConsts* SC,
                                               int lane, bool dup) {
   constexpr bool STG = std::is_same<HV, HitView<true> >::value; /* staged hits: reading past a window is harmless */
+  const int* XD = reinterpret_cast<const CtaHeader*>(lf_smem)->xdelta;
   const uint32_t* rowp = EP.rows + k_seed * WIN_ROW;
   /* the seed's row of the window table: lanes 0..11 hold the packed window of layer `lane`, lanes 12..15 x_mag, tx,
    * q/p and the flags (written by the window kernel) */
@@ -804,8 +910,9 @@ __device__ __forceinline__ void seed_triplets(const Consts& C, const EventArgs& 
   for (int set = 0; set < 2; ++set) {
     const int la = set ? 3 : 0;
     const uint32_t wa = __shfl_sync(FULL, winw, la), wb = __shfl_sync(FULL, winw, la + 4), wc = __shfl_sync(FULL, winw, la + 8);
-    const int fa = (int)(wa >> 6), na = (int)(wa & 63u), fb = (int)(wb >> 6), nb = (int)(wb & 63u);
-    const int fc = (int)(wc >> 6), nc = (int)(wc & 63u);
+    /* window starts as positions of the compact x-layer stage (fetch_event_x) */
+    const int fa = (int)(wa >> 6) - XD[la], na = (int)(wa & 63u), fb = (int)(wb >> 6) - XD[la + 4], nb = (int)(wb & 63u);
+    const int fc = (int)(wc >> 6) - XD[la + 8], nc = (int)(wc & 63u);
     if (lane == set) W.setw[set] = make_int4(fb, fb + nb, fc, 0);
     const bool have = (lane < na) && (nb != 0); /* no h1 hit, no triplet */
     const float x0 = (STG || lane < na) ? hx[fa + lane] : 0.0f;
@@ -942,6 +1049,7 @@ __device__ __forceinline__ void seed_triplets_h2(const Consts& C, const EventArg
                                                  const SeedEventPtrs& EP, uint32_t k_seed, SeedScratchH2& W, const SetConsts* SC,
                                                  int lane, bool dup) {
   constexpr bool STG = std::is_same<HV, HitView<true> >::value;
+  const int* XD = reinterpret_cast<const CtaHeader*>(lf_smem)->xdelta;
   const uint32_t* rowp = EP.rows + k_seed * WIN_ROW;
   const uint32_t winw = (lane < WIN_ROW) ? rowp[lane] : 0u;
   const float x_mag = __uint_as_float(__shfl_sync(FULL, winw, 12)), tx = __uint_as_float(__shfl_sync(FULL, winw, 13));
@@ -958,8 +1066,9 @@ __device__ __forceinline__ void seed_triplets_h2(const Consts& C, const EventArg
   for (int set = 0; set < 2; ++set) {
     const int la = set ? 3 : 0;
     const uint32_t wa = __shfl_sync(FULL, winw, la), wb = __shfl_sync(FULL, winw, la + 4), wc = __shfl_sync(FULL, winw, la + 8);
-    const int fa = (int)(wa >> 6), na = (int)(wa & 63u), fb = (int)(wb >> 6), nb = (int)(wb & 63u);
-    const int fc = (int)(wc >> 6), nc = (int)(wc & 63u);
+    /* window starts as positions of the compact x-layer stage (fetch_event_x) */
+    const int fa = (int)(wa >> 6) - XD[la], na = (int)(wa & 63u), fb = (int)(wb >> 6) - XD[la + 4], nb = (int)(wb & 63u);
+    const int fc = (int)(wc >> 6) - XD[la + 8], nc = (int)(wc & 63u);
     if (lane == set) W.setw[set] = make_int4(fb, fb + nb, fc, fc + nc);
     const bool have = (lane < na) && (nb != 0);
     const float x0 = (STG || lane < na) ? hx[fa + lane] : 0.0f;
@@ -1126,6 +1235,7 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
                                                    uint32_t seed, int side, SeedScratchWide& W, int lane, bool dup) {
   typedef Fmt<true> F;
   typedef typename HV::pos_t pos_t;
+  const int* XD = reinterpret_cast<const CtaHeader*>(lf_smem)->xdelta;
   const size_t row = (size_t)seed * C.sides + side;
   const float x = __ldg(A.sx + seed), tx = __ldg(A.stx + seed);
   const bool no_ut = C.mode == 1;
@@ -1153,10 +1263,11 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
   for (int set = 0; set < 2; ++set) {
     const int la = set ? 3 : 0;
     const uint32_t wa = __shfl_sync(FULL, winw, la), wb = __shfl_sync(FULL, winw, la + 4), wc = __shfl_sync(FULL, winw, la + 8);
-    const int fa = (int)(wa >> F::WB), na = (int)(wa & F::WMASK), nc = (int)(wc & F::WMASK);
-    fbs[set] = (int)(wb >> F::WB);
+    /* window starts as positions of the compact x-layer stage (fetch_event_x) */
+    const int fa = (int)(wa >> F::WB) - XD[la], na = (int)(wa & F::WMASK), nc = (int)(wc & F::WMASK);
+    fbs[set] = (int)(wb >> F::WB) - XD[la + 4];
     nbs[set] = (int)(wb & F::WMASK);
-    fcs[set] = (int)(wc >> F::WB);
+    fcs[set] = (int)(wc >> F::WB) - XD[la + 8];
     const bool set_on = na != 0 && nbs[set] != 0 && nc != 0; /* warp-uniform */
     const float inv_r = C.inv_r[set];
     const pos_t pc0 = hx.pos(fcs[set]), pc1 = hx.pos(fcs[set] + nc);
@@ -1256,7 +1367,7 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
     const unsigned low = (unsigned)key;
     const int set = (low >> (3 * F::IB)) & 1, la = set ? 3 : 0;
     const int fa = (int)(__shfl_sync(FULL, winw, la) >> F::WB);
-    const int fb = set ? fbs[1] : fbs[0], fc = set ? fcs[1] : fcs[0];
+    const int fb = (set ? fbs[1] : fbs[0]) + XD[la + 4], fc = (set ? fcs[1] : fcs[0]) + XD[la + 8]; /* event-relative again */
     if (lane == 0 && A.dbg.n_triplets) A.dbg.n_triplets[row] = ntr;
     if (lane < NT) {
       const size_t o = row * NT + lane;
@@ -1295,7 +1406,7 @@ __global__ void __launch_bounds__(SEED_THREADS, WIDE ? 4 : 5) lf_seed_kernel(con
   fill_set_consts(C, T.sc); /* published by fetch_event's barriers */
   uint32_t phase = 0;
   EventCtx E;
-  while (fetch_event(A, phase, E)) {
+  while (fetch_event_x(A, phase, E)) {
     const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
     const int sides = WIDE ? C.sides : 1;
     const int n_rows = (int)(s1 - s0) * sides;
