@@ -52,6 +52,7 @@ struct lf_handle {
   size_t max_events, max_seeds, max_hits;
   int device;
   int sm_count, stage_cap;
+  int ext_chunk;   /* rows the extension kernel stages at a time: 256, or 128 if that keeps one more CTA per SM */
   int stage_cap_x; /* the seeding kernel stages the six x layers only: about half an event */
   int regs[4], grid[4], ctas_per_sm[4], smem_bytes[4]; /* window, seed, extend, fit kernels */
   /* workspace */
@@ -281,6 +282,7 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
   A.hx = hits->x; A.seg_off = hits->seg_offsets;
   A.n_events = (uint32_t)n_events;
   A.stage_cap = h->stage_cap;
+  A.ext_chunk = h->ext_chunk;
   A.win = h->win; A.trip_code = h->trip_code; A.n_trip = h->n_trip;
   A.ws_rec = h->ws_rec; A.ws_nh = h->ws_nh; A.ws_rank = h->ws_rank; A.ws_event = h->ws_event;
   A.ev_count = h->ev_count;
@@ -462,7 +464,8 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   const size_t stage_bytes_x = (size_t)lf::HDR_BYTES + (size_t)h->stage_cap_x * sizeof(float);
   h->smem_bytes[0] = (int)stage_bytes;
   h->smem_bytes[1] = (int)(stage_bytes_x + (h->wide ? sizeof(lf::SeedTables<true, false>) : (h->half2 ? sizeof(lf::SeedTables<false, true>) : sizeof(lf::SeedTables<false, false>))));
-  h->smem_bytes[2] = (int)(stage_bytes + lf::ext_tables_bytes(params->n_triplets));
+  h->ext_chunk = lf::FIT_CHUNK;
+  h->smem_bytes[2] = (int)(stage_bytes + lf::ext_tables_bytes(params->n_triplets, h->ext_chunk));
   h->smem_bytes[3] = (int)(stage_bytes + lf::FIT_TABLES_BYTES);
   const void* kern_n[4][2] = {{(const void*)lf::lf_window_kernel<false, false>, (const void*)lf::lf_window_kernel<true, false>},
                               {(const void*)lf::lf_seed_kernel<false, false>, (const void*)lf::lf_seed_kernel<true, false>},
@@ -477,6 +480,18 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   const void* (*kern)[2] = h->wide ? kern_w : kern_n;
   const int threads[4] = {lf::WIN_THREADS, lf::SEED_THREADS, lf::FIT_THREADS, lf::FIT_THREADS};
   for (int k = 0; k < 4; ++k) {
+    if (k == 2) { /* extension kernel: half-size row tables if they buy a resident CTA (large events) */
+      const int small = (int)(stage_bytes + lf::ext_tables_bytes(params->n_triplets, lf::FIT_CHUNK / 2));
+      int occ_big = 0, occ_small = 0;
+      for (int d = 0; d < 2; ++d)
+        LF_CREATE_CUDA(raise_dynamic_smem(kern[k][d], h->wide ? 1 : 0, k, d, h->device, h->smem_bytes[k]));
+      LF_CREATE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_big, kern[k][0], threads[k], h->smem_bytes[k]));
+      LF_CREATE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_small, kern[k][0], threads[k], small));
+      if (occ_small > occ_big) {
+        h->ext_chunk = lf::FIT_CHUNK / 2;
+        h->smem_bytes[k] = small;
+      }
+    }
     for (int d = 0; d < 2; ++d)
       LF_CREATE_CUDA(raise_dynamic_smem(kern[k][d], h->wide ? 1 : (h->half2 && k == 1 ? 2 : 0), k, d, h->device, h->smem_bytes[k]));
     LF_CREATE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->ctas_per_sm[k], kern[k][0], threads[k], h->smem_bytes[k]));

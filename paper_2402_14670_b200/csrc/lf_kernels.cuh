@@ -70,7 +70,8 @@ struct Fmt {
 constexpr int SEED_WARPS = 8;
 constexpr int SEED_THREADS = SEED_WARPS * 32;
 constexpr int FIT_THREADS = 256;
-constexpr int FIT_CHUNK = 256; /* seeds of one event handled per pass of the fit kernel (== FIT_THREADS) */
+constexpr int FIT_CHUNK = 256; /* most rows of one event whose windows the extension kernel stages at a time (<= FIT_THREADS, even);
+                                 EventArgs.ext_chunk is the handle's choice, 256 or 128 */
 constexpr int N_TICKETS = 4; /* window, seed, extend, fit */
 constexpr unsigned FULL = 0xffffffffu;
 constexpr float INTERVAL_MARGIN = 0.1f; /* mm added to the magnet tolerance when bracketing h2 (superset only) */
@@ -121,6 +122,7 @@ struct EventArgs {
   int scratch_writer;
   uint32_t n_events;
   int stage_cap;        /* floats of shared memory available for one event's hits */
+  int ext_chunk;        /* extension kernel: rows staged at a time (lf_create picks the size that keeps most CTAs per SM) */
   uint32_t* ticket;     /* this kernel's event ticket */
   /* per followed track ("row" = seed*sides + side; narrow kernels: row = seed) */
   uint32_t* win;        /* n_rows*WIN_ROW: 12 x ((first_in_event << WB) | count), then x_mag, tx, q/p (mode 1: the assumed
@@ -1557,9 +1559,8 @@ struct ExtTables {
   uint16_t* item;  /* FIT_CHUNK*NT: seed_local<<4 | k */
   int* wcnt;       /* 2 * 8: accepted candidates per warp, double-buffered by pass */
 };
-__host__ __device__ inline size_t ext_tables_bytes(int nt) {
-  return 4 * NL * 4 + (size_t)FIT_CHUNK * NL * 4 + (size_t)FIT_CHUNK * 4 * 4 +
-         (((size_t)FIT_CHUNK * nt * 2 + 15) & ~size_t(15)) + 16 * 4;
+__host__ __device__ inline size_t ext_tables_bytes(int nt, int chunk) {
+  return 4 * NL * 4 + (size_t)chunk * NL * 4 + (size_t)chunk * 4 * 4 + (((size_t)chunk * nt * 2 + 15) & ~size_t(15)) + 16 * 4;
 }
 
 template <bool DEBUG, bool WIDE, bool STAGED>
@@ -1578,8 +1579,9 @@ __device__ __forceinline__ void extend_event(const Consts& C, const EventArgs& A
   uint4* rec = A.acc_rec + row0 * NT;
   uint32_t ev_acc = 0;
   int parity = 0;
-  for (int cb = 0; cb < nr; cb += FIT_CHUNK) { /* FIT_CHUNK is even: a chunk starts on a seed boundary */
-    const int cn = min(FIT_CHUNK, nr - cb);
+  const int CH = A.ext_chunk;
+  for (int cb = 0; cb < nr; cb += CH) { /* the chunk size is even: a chunk starts on a seed boundary */
+    const int cn = min(CH, nr - cb);
     const size_t rbase = row0 + (size_t)cb;
     /* ---- stage the chunk's windows, seed parameters and candidate counts */
     for (int i = tid; i < cn * WIN_ROW; i += FIT_THREADS)
@@ -1679,11 +1681,11 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_extend_kernel(const __grid_
   T.geo = reinterpret_cast<float*>(tb);
   tb += 4 * NL * 4;
   T.win = reinterpret_cast<uint32_t*>(tb);
-  tb += (size_t)FIT_CHUNK * NL * 4;
+  tb += (size_t)A.ext_chunk * NL * 4;
   T.sp = reinterpret_cast<float*>(tb);
-  tb += (size_t)FIT_CHUNK * 16;
+  tb += (size_t)A.ext_chunk * 16;
   T.item = reinterpret_cast<uint16_t*>(tb);
-  tb += ((size_t)FIT_CHUNK * NT * 2 + 15) & ~size_t(15);
+  tb += ((size_t)A.ext_chunk * NT * 2 + 15) & ~size_t(15);
   T.wcnt = reinterpret_cast<int*>(tb);
   if (threadIdx.x == 0) mbar_init(&H.mbar, 1);
   if (threadIdx.x < NL) {
