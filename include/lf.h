@@ -170,7 +170,7 @@ typedef struct {
 #define LF_N_EVENT_KERNELS 4
 #define LF_N_KERNELS 6 /* + LF_K_SCAN = 4, LF_K_COMPACT = 5 (a7) in lf_kernel_times */
 typedef struct {
-  int32_t kernels_per_run;       /* kernel launches one lf_run enqueues (6; 7 with hit_storage = 1) */
+  int32_t kernels_per_run;       /* kernel launches one lf_run enqueues (6; 7 with hit_storage = 1 when the library packs the hits) */
   int32_t regs[LF_N_EVENT_KERNELS], block[LF_N_EVENT_KERNELS], grid[LF_N_EVENT_KERNELS], ctas_per_sm[LF_N_EVENT_KERNELS];
   int32_t smem_bytes[LF_N_EVENT_KERNELS]; /* dynamic shared memory per CTA */
   int32_t staged_hits_per_event; /* events with more hits than this read hits from global memory */
@@ -179,11 +179,12 @@ typedef struct {
 } lf_info;
 
 /* Creates a context for batches of at most max_events / max_seeds / max_hits.  Validates geometry
- * and params, uploads constants, allocates the workspace (about max_seeds*(141 + 18*n_triplets) +
- * max_events*16 bytes, roughly twice that in the no-UT mode, on the current CUDA device, sized for 180 GB parts).  The shared-memory stage for one event's hits is sized
- * from the maxima: 1.25 * max_hits / max_events + 512 hits, clamped to [2048, 16384]; larger events are
- * still processed correctly, reading their hits from global memory.  *out is set only on LF_OK.
- * HOST pointers. */
+ * and params (finite, tolerances >= 0, kick != 0), uploads constants, allocates the workspace (about
+ * max_seeds*(153 + 18*n_triplets) + max_events*16 bytes, roughly twice that in the no-UT mode; with hit_storage = 1
+ * another 6.5 bytes per hit) on the current CUDA device, sized for 180 GB parts.  The shared-memory stage for one event's
+ * hits is sized from the maxima: 1.25 * max_hits / max_events + 512 hits, clamped to [2048, 16384] (the seeding kernel
+ * stages the x layers only, half of that); larger events are still processed correctly, reading their hits from global
+ * memory.  Handles of different sizes may be alive at the same time.  *out is set only on LF_OK.  HOST pointers. */
 lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t max_events,
                     size_t max_seeds, size_t max_hits, lf_handle** out);
 

@@ -1,31 +1,36 @@
 /*
  * lf_kernels.cuh -- sm_100a device code of the Looking Forward hot path (include/lf.h, a1..a7).
  *
- * Execution model.  Three event kernels share one skeleton: persistent CTAs take
- * events from an atomic ticket; the event's 24 x-sorted hit segments are contiguous in HBM, so one
- * 1-D bulk async copy (TMA: cp.async.bulk + mbarrier, SASS UBLKCP) stages the whole event into shared
- * memory.  Each kernel then maps threads to the natural work item of its stage:
+ * Execution model.  Four event kernels share one skeleton: persistent CTAs take events from an
+ * atomic ticket; the event's 24 x-sorted hit segments are contiguous in HBM, so 1-D bulk async copies (TMA:
+ * cp.async.bulk + mbarrier, SASS UBLKCP) stage them into shared memory (fetch_event: the whole event; fetch_event_x:
+ * the six x layers in four runs, for the seeding kernel).  Each kernel then maps threads to the work item of its stage:
  *
- *   lf_window_kernel  a1/a2  one thread per (seed, layer, window edge): branch-free binary searches,
- *                            edge pairs exchange by shuffle, n_window cap; packed window words to HBM.
- *   lf_seed_kernel    a3     one warp per seed.  For a fixed h0 the h2 hits that pass the magnet-opening
- *                            cut form a contiguous x interval: lanes = h0 bracket a conservative superset
- *                            by two binary searches; a warp prefix scan of the bracket sizes re-maps the
- *                            work to lanes = candidate doublets, where the exact fp32 predicate decides
- *                            (bit-exact with the all-pairs definition) and the closest h1 / chi2 cut
- *                            follow in the same lane; rank selection on 64-bit (chi2, set, h0, h2) keys
- *                            keeps the n smallest, sorted.
- *   lf_fit_kernel     a4-a6  one thread per candidate: parabola through the triplet, closest hit in the
- *                            9 other windows, hit-count rule; accepted candidates are ballot-compacted
- *                            into a per-warp queue and fitted in dense batches of 32 (fp32 fit in the
- *                            oracle's summation order, Q).  Then one thread per seed picks the lowest Q
- *                            and writes the track record; the CTA ranks the event's tracks in seed order.
+ *   lf_window_kernel  a1/a2  one thread per (followed track, layer): one branch-free binary search over the segment
+ *                            for the window centre, two short ones for the edges, n_window cap; writes a 64-byte row
+ *                            per followed track: 12 packed windows + x_mag, tx, q/p, flags.
+ *   lf_seed_kernel    a3     one warp per followed track.  For a fixed h0 the h2 hits that pass the magnet-opening
+ *                            cut form a contiguous x interval: lanes = h0 bracket a conservative superset by two
+ *                            shuffle searches; a warp prefix scan of the bracket sizes re-maps the work to lanes =
+ *                            candidate doublets, where the exact fp32 predicate decides (bit-exact with the
+ *                            all-pairs definition) and the closest h1 / chi2 cut follow in the same lane; rank
+ *                            selection on (chi2, candidate order) keeps the n smallest, sorted.  seed_triplets_h2
+ *                            is the same with pairs of doublets evaluated in __half2 (hit_storage = 1);
+ *                            seed_triplets_wide handles windows of up to 64 hits and the no-UT tuning.
+ *   lf_extend_kernel  a4/a5  one thread per triplet: parabola through the triplet, closest hit in the 9 other windows
+ *                            (three searches in lockstep per station), chi2 cuts, hit-count rule; accepted
+ *                            candidates are ballot-compacted in (seed, k) order into 16-byte records.
+ *   lf_fit_kernel     a6     one thread per accepted record: both least-squares fits (geometry sums from a
+ *                            per-presence-mask LUT), Q, lowest (Q, k) per seed by shared-memory atomicMin; the winning
+ *                            thread writes the 20-word track record; the CTA ranks the event's tracks in seed order.
  *   lf_scan_kernel    a7     exclusive scan of per-event track counts -> event_offsets, n_tracks.
  *   lf_compact_kernel a7     stream compaction: per-seed records -> dense SoA outputs, coalesced.
+ *   lf_pack_hits_kernel, lf_validate_kernel: fp16 copy of the hits (hit_storage = 1); input preconditions.
  *
  * Arithmetic contract: fp32, one rounding per operation, in the order DESIGN.md "Canonical
- * arithmetic" lists (compile with -fmad=false, no fast-math; '/' is IEEE division).  This file is
- * written from PAPER.md + DESIGN.md and shares nothing with oracle/.
+ * arithmetic" lists (compile with -fmad=false, no fast-math; '/' is IEEE division; explicit __fmaf_rn appears only
+ * where a value brackets a search and decides nothing).  This file is written from PAPER.md + DESIGN.md and shares
+ * nothing with oracle/.
  */
 #pragma once
 #include <cuda_fp16.h>
