@@ -173,19 +173,23 @@ def algorithmic_bytes(batch, n_tracks: int) -> int:
 
 
 def kernel_bytes(batch, n_tracks: int, n_triplets: int, n_acc: int = 0, sides: int = 1, wide: bool = False) -> dict:
-    """Algorithmic HBM bytes per launch of each event kernel: every kernel stages the
-    event's hits once and reads/writes its own tables once.  Tables are per followed track (row): one per seed, or
-    one per (seed, window side) in the no-UT tuning; the wide kernels store 4-byte triplet codes."""
+    """Algorithmic HBM bytes per launch of each event kernel: every kernel stages the hits it needs
+    once (all twelve layers; the seeding kernel only the six x layers) and reads / writes its own tables once.  Tables are
+    per followed track (row): one per seed, or one per (seed, window side) in the no-UT tuning (64-byte window rows; the
+    wide kernels store 4-byte triplet codes)."""
     H, S, E = batch.n_hits, batch.n_seeds, batch.n_events
     R, cb = S * sides, (4 if wide else 2)
-    common = 4 * H + batch.seg_offsets.nbytes + batch.seed_offsets.nbytes
+    so = np.asarray(batch.seg_offsets).astype(np.int64)
+    seg_len = np.diff(so).reshape(-1, 12, 2).sum(2)          # hits per (event, layer)
+    Hx = int(seg_len[:, [0, 3, 4, 7, 8, 11]].sum())          # hits of the six x layers
+    offs = batch.seg_offsets.nbytes + batch.seed_offsets.nbytes
     trip = (cb * n_triplets + 1) * R
     acc = 16 * n_acc  # one 16-byte record per candidate that passed the hit-count rule
-    return {"window": common + (16 if sides == 2 else 20) * S + 48 * R + 4 * E,
-            "seed": common + 12 * S + 48 * R + trip,
-            "extend": common + 12 * S + 48 * R + trip + acc + 4 * S + 4 * E,
-            "fit": common + 4 * E + acc + n_acc * (48 + 12 + cb) + 80 * n_tracks + 16 * S,
-            "compact": 92 * S + 80 * n_tracks + 4 * E}
+    return {"window": 4 * H + offs + (16 if sides == 2 else 20) * S + 64 * R + 4 * E,
+            "seed": 4 * Hx + offs + 64 * R + trip + 4 * E,
+            "extend": 4 * H + offs + 12 * S + 64 * R + trip + acc + 4 * S + 4 * E,
+            "fit": 4 * H + offs + 4 * E + acc + n_acc * (64 + 12) + 80 * n_tracks + 12 * S,
+            "compact": 88 * S + 80 * n_tracks + 4 * E}
 
 
 def tuning_params(args, datagen, cfg):

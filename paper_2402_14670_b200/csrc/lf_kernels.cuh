@@ -582,10 +582,10 @@ __device__ __forceinline__ void windows_of_event(const Consts& C, const EventArg
   const bool pol_pos = C.polarity > 0;
   const int halfw = C.n_window / 2, reach = C.n_window + 1;
   for (int it = tid; it < n_items; it += WIN_THREADS) {
-    const int sl = it / per_seed;
-    const int rem = it - sl * per_seed;
-    const int side = WIDE ? rem / NL : 0;
-    const int layer = rem - side * NL;
+    const int q12 = it / NL; /* (seed, side) pair; sides is 1 or 2, so no division by a run-time value */
+    const int layer = it - q12 * NL;
+    const int sl = WIDE ? (q12 >> (sides >> 1)) : q12;
+    const int side = WIDE ? (q12 & (sides - 1)) : 0;
     const uint32_t seed = s0 + (uint32_t)sl;
     const size_t row = (size_t)seed * sides + side;
     const float x = __ldg(A.sx + seed), y = __ldg(A.sy + seed), tx = __ldg(A.stx + seed), ty = __ldg(A.sty + seed);
@@ -1244,24 +1244,16 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
   typedef typename HV::pos_t pos_t;
   const int* XD = reinterpret_cast<const CtaHeader*>(lf_smem)->xdelta;
   const size_t row = (size_t)seed * C.sides + side;
-  const float x = __ldg(A.sx + seed), tx = __ldg(A.stx + seed);
   const bool no_ut = C.mode == 1;
-  float kq = 0.0f, aq;
-  if (no_ut) {
-    const float ty = __ldg(A.sty + seed);
-    const float s2 = tx * tx + ty * ty;
-    const float sin_theta = sqrtf(s2 / (1.0f + s2));
-    aq = fminf(C.inv_p_min, sin_theta * C.inv_pt_min);
-  } else {
-    const float qop = __ldg(A.sqop + seed);
-    aq = fmaxf(fabsf(qop), 1e-6f);
-    kq = C.kick * qop; /* expected slope change across the magnet (Eq. 2) */
-  }
-  const float p = 1.0f / aq;
-  const float x_mag = x + tx * C.mag_dz_seed;
-  const uint32_t winw = (lane < NL) ? A.win[row * WIN_ROW + lane] : 0u;
+  /* the row of the window table: lanes 0..11 the packed windows, lanes 12..15 x_mag, tx, q/p (no-UT: the assumed 1/p of
+   * PAPER.md:289) and the flags, written by the window kernel */
+  const uint32_t winw = (lane < WIN_ROW) ? A.win[row * WIN_ROW + lane] : 0u;
+  const float x_mag = __uint_as_float(__shfl_sync(FULL, winw, 12)), tx = __uint_as_float(__shfl_sync(FULL, winw, 13));
+  const float q3 = __uint_as_float(__shfl_sync(FULL, winw, 14));
+  const bool low_p = (__shfl_sync(FULL, winw, 15) & ROW_LOW_P) != 0u;
+  const float aq = no_ut ? q3 : fmaxf(fabsf(q3), 1e-6f);
+  const float kq = no_ut ? 0.0f : C.kick * q3; /* expected slope change across the magnet (Eq. 2) */
   const unsigned lt_mask = (1u << lane) - 1u;
-  const bool low_p = !no_ut && (p < C.p_same_bend);
   const float tol0 = C.mag_tol_base + C.mag_tol_inv_p * aq;
   /* ---- brackets: four groups of 32 h0 hits */
   int fbs[2], nbs[2], fcs[2];
@@ -1341,7 +1333,7 @@ __device__ __forceinline__ void seed_triplets_wide(const Consts& C, const EventA
         const float zb = set ? C.z[7] : C.z[4], za = set ? C.z[3] : C.z[0], Kx1 = set ? C.K[1] : C.K[0];
         const float x1e = zb * t + (x0o - t * za) * Kx1; /* PAPER.md:215 */
         float dx;
-        const int k = closest_hit<true>(hx, fb, nb, x1e, dup, dx);
+        const int k = closest_in_window<true>(hx, fb, fb + nb, x1e, dup, dx);
         const float chi2 = dx * dx;
         if (chi2 < C.T_triplet) {
           pass = true;
@@ -1440,8 +1432,9 @@ __global__ void __launch_bounds__(SEED_THREADS, WIDE ? 4 : 5) lf_seed_kernel(con
       const int kend = (t < n_big) ? k + PER_TICKET : k + 1;
       for (; k < kend; ++k) {
         if constexpr (WIDE) {
-          const uint32_t seed = s0 + (uint32_t)(k / sides);
-          const int side = k - (k / sides) * sides;
+          const int sh = sides >> 1; /* sides is 1 or 2: shifts instead of a division by a run-time value */
+          const uint32_t seed = s0 + (uint32_t)(k >> sh);
+          const int side = k & (sides - 1);
           if (E.staged) seed_triplets_wide<DEBUG>(C, A, HitView<true>(E.skew), E.h0, seed, side, W, lane, dup);
           else seed_triplets_wide<DEBUG>(C, A, HitView<false>(E.gview), E.h0, seed, side, W, lane, dup);
         } else if constexpr (H2) {
@@ -1594,7 +1587,7 @@ __device__ __forceinline__ void extend_event(const Consts& C, const EventArgs& A
     int my_n = 0;
     if (tid < cn) {
       const size_t row = rbase + (size_t)tid;
-      const uint32_t seed = WIDE ? (uint32_t)(row / (size_t)sides) : (uint32_t)row;
+      const uint32_t seed = WIDE ? (uint32_t)(row >> (sides >> 1)) : (uint32_t)row; /* sides is 1 or 2 */
       T.sp[tid * 4 + 0] = __ldg(A.sy + seed);
       T.sp[tid * 4 + 1] = __ldg(A.stx + seed);
       T.sp[tid * 4 + 2] = __ldg(A.sty + seed);
@@ -1645,7 +1638,7 @@ __device__ __forceinline__ void extend_event(const Consts& C, const EventArgs& A
         /* seed inside the event, (side,) candidate index */
         const int re = cb + rl;
         const unsigned set_bit = ((code >> (3 * F::IB)) & 1u) << F::SET_SHIFT;
-        tag = WIDE ? ((unsigned)(re / sides) | set_bit | ((unsigned)(re - (re / sides) * sides) << F::SIDE_SHIFT) | ((unsigned)k << F::K_SHIFT))
+        tag = WIDE ? ((unsigned)(re >> (sides >> 1)) | set_bit | ((unsigned)(re & (sides - 1)) << F::SIDE_SHIFT) | ((unsigned)k << F::K_SHIFT))
                    : ((unsigned)re | set_bit | ((unsigned)k << F::K_SHIFT));
         if (DEBUG) {
           if (A.dbg.cand_hits)
