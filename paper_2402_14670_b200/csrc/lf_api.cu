@@ -282,6 +282,7 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
   A.hx = hits->x; A.seg_off = hits->seg_offsets;
   A.n_events = (uint32_t)n_events;
   A.stage_cap = h->stage_cap;
+  A.stage_cap_x = h->stage_cap_x;
   A.ext_chunk = h->ext_chunk;
   A.win = h->win; A.trip_code = h->trip_code; A.n_trip = h->n_trip;
   A.ws_rec = h->ws_rec; A.ws_nh = h->ws_nh; A.ws_rank = h->ws_rank; A.ws_event = h->ws_event;

@@ -127,6 +127,7 @@ struct EventArgs {
   int scratch_writer;
   uint32_t n_events;
   int stage_cap;        /* floats of shared memory available for one event's hits */
+  int stage_cap_x;      /* the stage of the seeding kernel (fetch_event_x), known to the kernel that writes the fp16 scratch image */
   int ext_chunk;        /* extension kernel: rows staged at a time (lf_create picks the size that keeps most CTAs per SM) */
   uint32_t* ticket;     /* this kernel's event ticket */
   /* per followed track ("row" = seed*sides + side; narrow kernels: row = seed) */
@@ -308,8 +309,15 @@ __device__ __forceinline__ bool fetch_event(const EventArgs& A, uint32_t& phase,
       if (tid <= NSEG) H.blk_pref[tid] = incl - nb; /* entry NSEG = all blocks of the event */
     }
     __syncthreads();
-    if (E.staged || A.scratch_writer) {
-      float* dst = E.staged ? buf : A.hx_scratch + E.h0;
+    /* The scratch writer (the window kernel) also decodes into the scratch image every event that the seeding kernel's
+     * half-size x-layer stage cannot hold (its runs take at most 24 floats of alignment gaps). */
+    bool to_scratch = false;
+    if (A.scratch_writer) {
+      const int nx = (int)((so[2] - so[0]) + (so[10] - so[6]) + (so[18] - so[14]) + (so[24] - so[22]));
+      to_scratch = !E.staged || nx + 28 > A.stage_cap_x;
+    }
+    if (E.staged || to_scratch) {
+      float* scr = A.hx_scratch + E.h0;
       const int lane = tid & 31, n_blk = H.blk_pref[NSEG];
       const int pref = (lane < NSEG) ? H.blk_pref[lane] : 0x7FFFFFFF;
       for (int blk = tid >> 5; blk < n_blk; blk += (int)(blockDim.x >> 5)) {
@@ -317,11 +325,14 @@ __device__ __forceinline__ bool fetch_event(const EventArgs& A, uint32_t& phase,
         const int b = blk - H.blk_pref[sg];
         const uint32_t S = so[sg];
         const int i = 32 * b + lane;
-        if (i < (int)(so[sg + 1] - S))
-          dst[(int)(S - E.h0) + i] = __ldg(A.origin16 + ((S >> H16_SHIFT) + ((A.event_base + E.ev) * NSEG + (uint32_t)sg) + (uint32_t)(i >> H16_SHIFT))) +
-                                     __half2float(A.hx16[S + i]);
+        if (i < (int)(so[sg + 1] - S)) {
+          const float v = __ldg(A.origin16 + ((S >> H16_SHIFT) + ((A.event_base + E.ev) * NSEG + (uint32_t)sg) + (uint32_t)(i >> H16_SHIFT))) +
+                          __half2float(A.hx16[S + i]);
+          if (E.staged) buf[(int)(S - E.h0) + i] = v;
+          if (to_scratch) scr[(int)(S - E.h0) + i] = v;
+        }
       }
-      if (!E.staged) __threadfence(); /* the scratch image is read back by this CTA and by the later kernels */
+      if (to_scratch) __threadfence(); /* the scratch image is read back by this CTA and by the later kernels */
     }
   } else if (E.staged) {
     /* the 16-byte aligned interior goes by TMA, the ragged head/tail by plain loads */

@@ -495,3 +495,56 @@ def test_fp16_only_events_larger_than_the_stage(lfmod, oracle, geometry, params)
     assert ((r2.hit_idx[ig] == ref.hit_idx[ir]).all(1).sum() / ref.n_tracks) > 0.95  # fp16 everywhere is lossy
     small.close()
     tiny.close()
+
+
+def _thin_uv_layers(b, keep=0.12, seed=5):
+    """The same batch with most noise hits of the u/v layers dropped (true hits stay), so that the x layers hold well over
+    half of an event's hits: the seeding kernel's half-size x-layer stage overflows while the full-event stage of the other
+    kernels does not."""
+    from dataclasses import replace
+    rng = np.random.default_rng(seed)
+    so = b.seg_offsets.astype(np.int64)
+    seg_of_hit = np.repeat(np.arange(so.size - 1), np.diff(so))
+    layer = (seg_of_hit % 24) // 2
+    uv = ((layer % 4) == 1) | ((layer % 4) == 2)
+    keep_mask = ~uv | (b.hit_track >= 0) | (rng.uniform(size=b.n_hits) < keep)
+    new_so = np.concatenate([[0], np.cumsum(np.bincount(seg_of_hit[keep_mask], minlength=so.size - 1))]).astype(np.uint32)
+    return replace(b, hit_x=b.hit_x[keep_mask], hit_track=b.hit_track[keep_mask], seg_offsets=new_so)
+
+
+def test_x_layer_stage_overflow(lfmod, oracle, geometry, params):
+    """Events that fit the full-event stage of the window, extension and fit kernels but whose x layers overflow the seeding
+    kernel's half-size stage: fp32 hits are then read from global memory by that kernel alone (bit-identical to the oracle),
+    fp16-only hits from the scratch image the window kernel decodes for exactly these events (identical to the staged
+    decoding of the same packed hits)."""
+    import torch
+    b = _thin_uv_layers(dg.generate(dg.GenConfig("xheavy", 8, 23, true_fixed=40, fake_mean=4.0, noise_fixed=500)))
+    nx = [int(sum(b.seg_offsets[e * 24 + 2 * l + 2] - b.seg_offsets[e * 24 + 2 * l] for l in (0, 3, 4, 7, 8, 11))) for e in range(b.n_events)]
+    nh = np.diff(b.seg_offsets[::24].astype(np.int64))
+    assert min(nx) > 0.7 * nh.max()
+    roomy = lfmod.LookingForward(geometry, params, b.n_events, b.n_seeds, 3 * b.n_hits)      # both stages hold the events
+    tight = lfmod.LookingForward(geometry, params, b.n_events, b.n_seeds, b.n_hits)          # only the full-event stage does
+    cap = tight.info().staged_hits_per_event
+    assert nh.max() <= cap and min(nx) + 28 > cap // 2 + 256 + 256, (nh.max(), min(nx), cap)
+    ref = oracle.run(geometry, params, b, debug=True)
+    for lf in (roomy, tight):
+        out = lf.run(lfmod.DeviceBatch(b), debug=True)
+        torch.cuda.synchronize()
+        got = out.to_numpy()
+        got.debug = {k: v.cpu().numpy() for k, v in vars(out.debug_tensors).items()}
+        assert_debug_equal(got.debug, ref.debug)
+        assert_tracks_equal(got, ref, "x-heavy events")
+        lf.close()
+    P16 = dict(params, hit_storage=1, seed_arith=1)
+    roomy = lfmod.LookingForward(geometry, P16, b.n_events, b.n_seeds, 3 * b.n_hits)
+    tight = lfmod.LookingForward(geometry, P16, b.n_events, b.n_seeds, b.n_hits)
+    db = lfmod.DeviceBatch(b)
+    roomy.pack_hits(db)
+    db.drop_fp32()
+    r1, r2 = roomy.run(db), tight.run(db)
+    torch.cuda.synchronize()
+    r1, r2 = r1.to_numpy(), r2.to_numpy()
+    assert r1.n_tracks == r2.n_tracks > 50 and np.array_equal(r1.hit_idx, r2.hit_idx)
+    assert np.array_equal(r1.state.view(np.uint32), r2.state.view(np.uint32))
+    roomy.close()
+    tight.close()
