@@ -3,7 +3,7 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--events E] [--tuning with-ut|no-ut]
 
-A "step" is one pass of the whole hot path (a1..a7: one lf_run = window, seed, extend, fit, scan, compact kernels)
+A "step" is one pass of the whole hot path (a1..a7: one lf_run = window, seed, extend, fit kernels; the fit kernel also compacts)
 over one batch of synthetic events.  Default workload: BASELINE.json configs[3] (20,000 events at
 Run-3-like occupancy, fp32, a single lf_run on one stream).  Prints ONE JSON line (rank 0).
 
@@ -185,11 +185,13 @@ def kernel_bytes(batch, n_tracks: int, n_triplets: int, n_acc: int = 0, sides: i
     offs = batch.seg_offsets.nbytes + batch.seed_offsets.nbytes
     trip = (cb * n_triplets + 1) * R
     acc = 16 * n_acc  # one 16-byte record per candidate that passed the hit-count rule
-    return {"window": 4 * H + offs + (16 if sides == 2 else 20) * S + 64 * R + 4 * E,
+    # fit (a6 + a7): records, per record its window row and seed parameters, the per-seed track flags; the winners' 80-byte
+    # records and the 4-byte track list written and read back by the same CTA (L2-resident in practice), the dense outputs,
+    # per event its look-back word (zeroed by the window kernel, written twice, read by later events) and its offset
+    return {"window": 4 * H + offs + (16 if sides == 2 else 20) * S + 64 * R + (4 + 8) * E,
             "seed": 4 * Hx + offs + 64 * R + trip + 4 * E,
             "extend": 4 * H + offs + 12 * S + 64 * R + trip + acc + 4 * S + 4 * E,
-            "fit": 4 * H + offs + 4 * E + acc + n_acc * (64 + 12) + 80 * n_tracks + 12 * S,
-            "compact": 88 * S + 80 * n_tracks + 4 * E}
+            "fit": 4 * H + offs + 4 * E + acc + n_acc * (64 + 12) + 4 * S + 2 * 84 * n_tracks + 80 * n_tracks + (8 * 3 + 4) * E}
 
 
 def tuning_params(args, datagen, cfg):

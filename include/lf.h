@@ -46,7 +46,7 @@
 extern "C" {
 #endif
 
-#define LF_ABI_VERSION 5u
+#define LF_ABI_VERSION 6u
 #define LF_N_LAYERS 12   /* three T-stations, x-u-v-x each */
 #define LF_N_ZONES 2     /* lower / upper half */
 #define LF_MAX_WINDOW 32   /* largest params.n_window of the narrow kernels (one warp lane per hit) */
@@ -166,11 +166,12 @@ typedef struct {
 #define LF_K_WINDOW 0  /* a1, a2 */
 #define LF_K_SEED 1    /* a3 */
 #define LF_K_EXTEND 2  /* a4, a5 */
-#define LF_K_FIT 3     /* a6 + ranking of the event's tracks */
+#define LF_K_FIT 3     /* a6, a7: fit, best candidate per seed, and the stream compaction (look-back scan of the events'
+                          track counts + copy of the tracks to their dense position) */
 #define LF_N_EVENT_KERNELS 4
-#define LF_N_KERNELS 6 /* + LF_K_SCAN = 4, LF_K_COMPACT = 5 (a7) in lf_kernel_times */
+#define LF_N_KERNELS 4 /* kernels one lf_run enqueues = entries of lf_kernel_times */
 typedef struct {
-  int32_t kernels_per_run;       /* kernel launches one lf_run enqueues (6; 7 with hit_storage = 1 when the library packs the hits) */
+  int32_t kernels_per_run;       /* kernel launches one lf_run enqueues (4; 5 with hit_storage = 1 when the library packs the hits) */
   int32_t regs[LF_N_EVENT_KERNELS], block[LF_N_EVENT_KERNELS], grid[LF_N_EVENT_KERNELS], ctas_per_sm[LF_N_EVENT_KERNELS];
   int32_t smem_bytes[LF_N_EVENT_KERNELS]; /* dynamic shared memory per CTA */
   int32_t staged_hits_per_event; /* events with more hits than this read hits from global memory */
@@ -180,7 +181,7 @@ typedef struct {
 
 /* Creates a context for batches of at most max_events / max_seeds / max_hits.  Validates geometry
  * and params (finite, tolerances >= 0, kick != 0), uploads constants, allocates the workspace (about
- * max_seeds*(153 + 18*n_triplets) + max_events*16 bytes, roughly twice that in the no-UT mode; with hit_storage = 1
+ * max_seeds*(153 + 18*n_triplets) + max_events*20 bytes, roughly twice that in the no-UT mode; with hit_storage = 1
  * another 6.5 bytes per hit) on the current CUDA device, sized for 180 GB parts.  The shared-memory stage for one event's
  * hits is sized from the maxima: 1.25 * max_hits / max_events + 512 hits, clamped to [2048, 16384] (the seeding kernel
  * stages the x layers only, half of that); larger events are still processed correctly, reading their hits from global
@@ -253,7 +254,7 @@ lf_status lf_get_info(const lf_handle* h, lf_info* out);
  * events on `cuda_stream` around each of their kernels (no synchronisation added).  After the caller
  * has synchronised the stream, lf_kernel_times writes the mean durations in milliseconds over the runs
  * recorded since profiling was enabled (the last 256 at most): ms[0] window kernel (a1, a2), ms[1] seeding
- * kernel (a3), ms[2] extension kernel (a4, a5), ms[3] fit kernel (a6), ms[4] offset scan, ms[5] compaction (a7).
+ * kernel (a3), ms[2] extension kernel (a4, a5), ms[3] fit kernel (a6 and the stream compaction a7).
  * LF_ERR_INVALID_ARG if profiling is off or no run was recorded. */
 lf_status lf_set_profiling(lf_handle* h, int enabled);
 lf_status lf_kernel_times(lf_handle* h, float ms[LF_N_KERNELS]);

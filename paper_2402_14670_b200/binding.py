@@ -78,7 +78,7 @@ class lf_info(C.Structure):
                 ("staged_hits_per_event", C.c_int32), ("sm_count", C.c_int32), ("workspace_bytes", C.c_size_t)]
 
 
-KERNEL_NAMES = ("window", "seed", "extend", "fit", "scan", "compact")
+KERNEL_NAMES = ("window", "seed", "extend", "fit")
 N_COUNTERS = 8
 COUNTER_NAMES = ("accepted_candidates", "events_with_equal_hits", "window_hits", "doublets_evaluated", "doublets_passing",
                  "triplets_passing", "triplets_kept", "tracks")
@@ -130,8 +130,8 @@ def load_library() -> C.CDLL:
     lib.lf_set_profiling.restype = C.c_int
     lib.lf_set_profiling.argtypes = [C.c_void_p, C.c_int]
     lib.lf_kernel_times.restype = C.c_int
-    lib.lf_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_float * 6)]
-    if lib.lf_abi_version() != 5:
+    lib.lf_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_float * len(KERNEL_NAMES))]
+    if lib.lf_abi_version() != 6:
         raise ImportError("liblf_b200.so: ABI version mismatch")
     for i, st in enumerate(_STRUCTS):
         if lib.lf_sizeof(i) != C.sizeof(st):
@@ -247,8 +247,8 @@ class LookingForward:
         self._check(self._lib.lf_set_profiling(self._h, 1 if enabled else 0))
 
     def kernel_times(self):
-        """Mean (window, seed, extend, fit, scan, compact) milliseconds of the profiled runs; the stream must be synchronised."""
-        ms = (C.c_float * 6)()
+        """Mean (window, seed, extend, fit) milliseconds of the profiled runs; the stream must be synchronised."""
+        ms = (C.c_float * len(KERNEL_NAMES))()
         self._check(self._lib.lf_kernel_times(self._h, C.byref(ms)))
         return tuple(float(v) for v in ms)
 

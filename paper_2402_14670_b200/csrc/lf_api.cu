@@ -55,6 +55,7 @@ struct lf_handle {
   int ext_chunk;   /* rows the extension kernel stages at a time: 256, or 128 if that keeps one more CTA per SM */
   int stage_cap_x; /* the seeding kernel stages the six x layers only: about half an event */
   int regs[4], grid[4], ctas_per_sm[4], smem_bytes[4]; /* window, seed, extend, fit kernels */
+  unsigned long long* ev_state; /* look-back words of the fit kernel's stream compaction */
   /* workspace */
   __half* hx16;     /* hit_storage = 1 only: the library's own fp16 copy (when the caller gives none) */
   float* origin16;
@@ -65,8 +66,8 @@ struct lf_handle {
   uint32_t* win;
   void* trip_code;
   uint8_t* n_trip;
-  int32_t *ws_rec, *ws_nh, *ws_rank, *ws_event;
-  uint32_t *ev_count, *ev_off, *ev_dup, *ev_acc, *tickets;
+  int32_t *ws_rec, *ws_nh, *ws_rank;
+  uint32_t *ev_count, *ev_dup, *ev_acc, *tickets;
   unsigned long long* counters; /* LF_N_COUNTERS: written by the debug build of the kernels */
   bool counters_valid = false;  /* the most recent launch was a debug launch */
   uint32_t* validate_res; /* 4 words: lf_validate_inputs' violation bits and offending indices */
@@ -271,7 +272,7 @@ bool use_wide(const lf_params& P) {
 
 template <bool DEBUG, bool WIDE>
 lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
-                 const lf_debug* dbg, cudaStream_t st, size_t seed_base = 0, size_t event_base = 0) {
+                 const lf_debug* dbg, cudaStream_t st, size_t event_base = 0) {
   const bool prof = h->profiling;
   cudaEvent_t* pe = prof ? h->prof_ev[h->prof_runs % PROF_RING] : nullptr;
   if (prof) LF_CUDA(h, cudaEventRecord(pe[0], st));
@@ -285,10 +286,11 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
   A.stage_cap_x = h->stage_cap_x;
   A.ext_chunk = h->ext_chunk;
   A.win = h->win; A.trip_code = h->trip_code; A.n_trip = h->n_trip;
-  A.ws_rec = h->ws_rec; A.ws_nh = h->ws_nh; A.ws_rank = h->ws_rank; A.ws_event = h->ws_event;
+  A.ws_rec = h->ws_rec; A.ws_nh = h->ws_nh; A.ws_rank = h->ws_rank;
   A.ev_count = h->ev_count;
   A.ev_dup = h->ev_dup;
   A.acc_rec = h->acc_rec; A.ev_acc = h->ev_acc; A.fit_lut = h->fit_lut;
+  A.ev_state = h->ev_state;
   if (dbg) {
     A.dbg.win_first = dbg->win_first; A.dbg.win_count = dbg->win_count; A.dbg.n_triplets = dbg->n_triplets;
     A.dbg.trip_hits = dbg->trip_hits; A.dbg.trip_set = dbg->trip_set; A.dbg.trip_chi2 = dbg->trip_chi2;
@@ -348,21 +350,19 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
   }
   if (prof) LF_CUDA(h, cudaEventRecord(pe[3], st));
   if (work) {
+    /* a6 + a7: the fit kernel also scans the events' track counts (look-back) and writes the dense outputs */
+    lf::TrackOut O;
+    O.hit_idx = out->hit_idx; O.seed_idx = out->seed_idx; O.n_hits = out->n_hits; O.state = out->state; O.quality = out->quality;
+    O.event_offsets = out->event_offsets; O.n_tracks = out->n_tracks;
+    O.ev_state = h->ev_state; O.tickets = h->tickets;
     A.ticket = h->tickets + 3;
-    lf::lf_fit_kernel<DEBUG, WIDE><<<grid_of(3), lf::FIT_THREADS, h->smem_bytes[3], st>>>(h->C, A);
-  }
-  if (prof) LF_CUDA(h, cudaEventRecord(pe[4], st));
-  lf::lf_scan_kernel<<<1, 1024, 0, st>>>(h->ev_count, (uint32_t)n_events, h->ev_off, out->event_offsets,
-                                         out->n_tracks, h->tickets);
-  if (prof) LF_CUDA(h, cudaEventRecord(pe[5], st));
-  if (work && seeds->n_seeds > 0) {
-    const size_t total = seeds->n_seeds * (lf::REC_WORDS / 4);
-    const unsigned blocks = (unsigned)((total + 255) / 256);
-    lf::lf_compact_kernel<<<blocks, 256, 0, st>>>(h->ws_rec, h->ws_rank, h->ws_event, h->ev_off, seed_base, seeds->n_seeds,
-                                                  out->hit_idx, out->seed_idx, out->n_hits, out->state, out->quality);
+    lf::lf_fit_kernel<DEBUG, WIDE><<<grid_of(3), lf::FIT_THREADS, h->smem_bytes[3], st>>>(h->C, A, O);
+  } else { /* no events: an empty track list */
+    LF_CUDA(h, cudaMemsetAsync(out->event_offsets, 0, sizeof(uint32_t), st));
+    LF_CUDA(h, cudaMemsetAsync(out->n_tracks, 0, sizeof(uint32_t), st));
   }
   if (prof) {
-    LF_CUDA(h, cudaEventRecord(pe[6], st));
+    LF_CUDA(h, cudaEventRecord(pe[4], st));
     ++h->prof_runs;
   }
   LF_CUDA(h, cudaGetLastError());
@@ -371,9 +371,9 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
 
 template <bool DEBUG>
 lf_status launch(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
-                 const lf_debug* dbg, cudaStream_t st, size_t seed_base = 0, size_t event_base = 0) {
-  return h->wide ? launch_impl<DEBUG, true>(h, seeds, hits, n_events, out, dbg, st, seed_base, event_base)
-                 : launch_impl<DEBUG, false>(h, seeds, hits, n_events, out, dbg, st, seed_base, event_base);
+                 const lf_debug* dbg, cudaStream_t st, size_t event_base = 0) {
+  return h->wide ? launch_impl<DEBUG, true>(h, seeds, hits, n_events, out, dbg, st, event_base)
+                 : launch_impl<DEBUG, false>(h, seeds, hits, n_events, out, dbg, st, event_base);
 }
 
 lf_status check_run_args(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out) {
@@ -519,9 +519,7 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   LF_CREATE_CUDA(cudaMalloc(&h->ws_rec, ns * lf::REC_WORDS * sizeof(int32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ws_nh, ns * sizeof(int32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ws_rank, ns * sizeof(int32_t)));
-  LF_CREATE_CUDA(cudaMalloc(&h->ws_event, ns * sizeof(int32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ev_count, ne * sizeof(uint32_t)));
-  LF_CREATE_CUDA(cudaMalloc(&h->ev_off, (ne + 1) * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ev_dup, ne * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->ev_acc, ne * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->acc_rec, nrows * nt * sizeof(uint4)));
@@ -533,10 +531,12 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   }
   LF_CREATE_CUDA(cudaMalloc(&h->validate_res, 4 * sizeof(uint32_t)));
   LF_CREATE_CUDA(cudaMalloc(&h->counters, LF_N_COUNTERS * sizeof(unsigned long long)));
-  LF_CREATE_CUDA(cudaMalloc(&h->tickets, lf::N_TICKETS * sizeof(uint32_t)));
-  LF_CREATE_CUDA(cudaMemset(h->tickets, 0, lf::N_TICKETS * sizeof(uint32_t)));
-  h->workspace_bytes = nrows * (lf::WIN_ROW * 4 + nt * (code_bytes + sizeof(uint4)) + 1) + ns * (lf::REC_WORDS + 3) * 4 +
-                       (4 * ne + 1 + lf::N_TICKETS) * sizeof(uint32_t) + (sizeof(lf::FitLut) << lf::NL);
+  LF_CREATE_CUDA(cudaMalloc(&h->tickets, (lf::N_TICKETS + 1) * sizeof(uint32_t)));
+  LF_CREATE_CUDA(cudaMemset(h->tickets, 0, (lf::N_TICKETS + 1) * sizeof(uint32_t)));
+  LF_CREATE_CUDA(cudaMalloc(&h->ev_state, ne * sizeof(unsigned long long)));
+  h->workspace_bytes = nrows * (lf::WIN_ROW * 4 + nt * (code_bytes + sizeof(uint4)) + 1) + ns * (lf::REC_WORDS + 2) * 4 +
+                       (3 * ne + 1 + lf::N_TICKETS) * sizeof(uint32_t) + ne * sizeof(unsigned long long) +
+                       (sizeof(lf::FitLut) << lf::NL);
 #undef LF_CREATE_CUDA
   *out = h;
   return LF_OK;
@@ -546,8 +546,8 @@ lf_status lf_destroy(lf_handle* h) {
   if (!h) return LF_OK;
   cudaFree(h->hx16); cudaFree(h->origin16); cudaFree(h->hx_scratch);
   cudaFree(h->win); cudaFree(h->trip_code); cudaFree(h->n_trip);
-  cudaFree(h->ws_rec); cudaFree(h->ws_nh); cudaFree(h->ws_rank); cudaFree(h->ws_event);
-  cudaFree(h->ev_count); cudaFree(h->ev_off); cudaFree(h->ev_dup); cudaFree(h->ev_acc); cudaFree(h->acc_rec); cudaFree(h->fit_lut); cudaFree(h->tickets);
+  cudaFree(h->ws_rec); cudaFree(h->ws_nh); cudaFree(h->ws_rank);
+  cudaFree(h->ev_count); cudaFree(h->ev_dup); cudaFree(h->ev_acc); cudaFree(h->acc_rec); cudaFree(h->fit_lut); cudaFree(h->tickets); cudaFree(h->ev_state);
   cudaFree(h->validate_res);
   cudaFree(h->counters);
   HostBufs& b = h->hb;
@@ -631,7 +631,7 @@ lf_status lf_kernel_times(lf_handle* h, float ms[LF_N_KERNELS]) {
   if (!h || !ms) return LF_ERR_INVALID_ARG;
   if (!h->profiling || h->prof_runs == 0) return fail(h, LF_ERR_INVALID_ARG, "lf_kernel_times: no profiled run recorded");
   const size_t n = std::min<size_t>(h->prof_runs, PROF_RING);
-  double acc[LF_N_KERNELS] = {0, 0, 0, 0, 0, 0};
+  double acc[LF_N_KERNELS] = {};
   for (size_t r = 0; r < n; ++r)
     for (int i = 0; i < LF_N_KERNELS; ++i) {
       float t = 0.f;
@@ -839,7 +839,7 @@ static lf_status run_host_pipeline(lf_handle* h, const lf_seeds* seeds, const lf
                   packed ? b.origin16 : nullptr};
     lf_tracks dt = {b.hit_idx + s0 * lf::NL, b.seed_idx + s0, b.n_hits + s0, b.state + s0 * 5, b.quality + s0,
                     b.ev_off + e0 + c, b.n_tracks + c, stride - s0};
-    const lf_status rs = launch<false>(h, &ds, &dh, e1 - e0, &dt, nullptr, st, s0, e0);
+    const lf_status rs = launch<false>(h, &ds, &dh, e1 - e0, &dt, nullptr, st, e0);
     if (rs != LF_OK) return rs;
     LF_CUDA(h, cudaEventRecord(b.ev_comp[c], st));
     LF_CUDA(h, cudaStreamWaitEvent(b.s_cnt, b.ev_comp[c], 0));

@@ -20,11 +20,12 @@
  *   lf_extend_kernel  a4/a5  one thread per triplet: parabola through the triplet, closest hit in the 9 other windows
  *                            (three searches in lockstep per station), chi2 cuts, hit-count rule; accepted
  *                            candidates are ballot-compacted in (seed, k) order into 16-byte records.
- *   lf_fit_kernel     a6     one thread per accepted record: both least-squares fits (geometry sums from a
+ *   lf_fit_kernel     a6/a7  one thread per accepted record: both least-squares fits (geometry sums from a
  *                            per-presence-mask LUT), Q, lowest (Q, k) per seed by shared-memory atomicMin; the winning
- *                            thread writes the 20-word track record; the CTA ranks the event's tracks in seed order.
- *   lf_scan_kernel    a7     exclusive scan of per-event track counts -> event_offsets, n_tracks.
- *   lf_compact_kernel a7     stream compaction: per-seed records -> dense SoA outputs, coalesced.
+ *                            thread writes the 20-word track record; the CTA lists the event's tracks in seed order.
+ *                            Stream compaction in the same kernel: a decoupled look-back over the events' track counts
+ *                            gives every event its offset in the dense output, and the CTA that fitted the event copies
+ *                            its tracks there (no scan kernel, no compaction kernel).
  *   lf_pack_hits_kernel, lf_validate_kernel: fp16 copy of the hits (hit_storage = 1); input preconditions.
  *
  * Arithmetic contract: fp32, one rounding per operation, in the order DESIGN.md "Canonical
@@ -137,8 +138,7 @@ struct EventArgs {
   uint8_t* n_trip;      /* n_rows */
   int32_t* ws_rec;      /* n_seeds * REC_WORDS */
   int32_t* ws_nh;       /* n_seeds: 1 if the seed has a track, else 0 */
-  int32_t* ws_rank;     /* n_seeds: rank among the event's tracks, -1 = none */
-  int32_t* ws_event;    /* n_seeds: event of the seed */
+  int32_t* ws_rank;     /* n_seeds: the events' track lists: entry (first seed of the event + r) = seed of the event's r-th track */
   uint32_t* ev_count;   /* n_events */
   uint4* acc_rec;       /* n_rows*NT: candidates that passed the hit-count rule: 3 words of hit codes (byte l = hit of
                            layer l inside its window, 0xFF = none), then the tag seed inside the event | layer set << 25 |
@@ -146,6 +146,7 @@ struct EventArgs {
   uint32_t* ev_acc;     /* n_events: number of such records of the event */
   const struct FitLut* fit_lut; /* 4096: per presence mask */
   uint32_t* ev_dup;     /* n_events: written by the window kernel, != 0 if two neighbouring staged hits are equal */
+  unsigned long long* ev_state; /* n_events: look-back words of lf_track_kernel, zeroed by the window kernel */
   DebugOut dbg;
 };
 
@@ -268,8 +269,14 @@ __device__ __forceinline__ typename HV::pos_t lower_pos(typename HV::pos_t a, ty
 }
 
 /* Takes the next event and stages its hits.  Called by every thread of the CTA; returns false when
- * the batch is exhausted.  Hit i of the event then lives at stage_buf()[skew + i]. */
-__device__ __forceinline__ bool fetch_event(const EventArgs& A, uint32_t& phase, EventCtx& E) {
+ * the batch is exhausted.  Hit i of the event then lives at stage_buf()[skew + i].  `while_loading` is called once by
+ * every thread of an event that was taken, after the bulk copy has been issued and before anybody waits for it: work
+ * that does not touch the stage hides behind the copy's latency (lf_track_kernel resolves an earlier event there). */
+struct NoHook {
+  __device__ __forceinline__ void operator()() const {}
+};
+template <class Hook = NoHook>
+__device__ __forceinline__ bool fetch_event(const EventArgs& A, uint32_t& phase, EventCtx& E, Hook while_loading = Hook()) {
   CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
   float* buf = stage_buf();
   const int tid = threadIdx.x;
@@ -346,11 +353,13 @@ __device__ __forceinline__ bool fetch_event(const EventArgs& A, uint32_t& phase,
     }
     if (tid < head) buf[E.skew + tid] = gsrc[tid];
     if (tid >= 32 && tid < 32 + tail) buf[E.skew + head + bulk + (tid - 32)] = gsrc[head + bulk + (tid - 32)];
+    while_loading();
     if (bulk > 0) {
       if (tid == 0) mbar_wait(&H.mbar, phase); /* one thread polls; the barrier below publishes */
       phase ^= 1u;
     }
   }
+  if (from16 || !E.staged) while_loading();
   __syncthreads();
   return true;
 }
@@ -704,6 +713,7 @@ __global__ void __launch_bounds__(WIN_THREADS, 8) lf_window_kernel(const __grid_
   uint32_t phase = 0;
   EventCtx E;
   while (fetch_event(A, phase, E)) {
+    if (threadIdx.x == 0) A.ev_state[E.ev] = 0ull; /* re-arms the look-back word of the event (lf_track_kernel) */
     if (E.staged) {
       flag_equal_neighbours(A, E, HitView<true>(E.skew));
       windows_of_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>(E.skew));
@@ -1733,21 +1743,104 @@ __device__ __forceinline__ void eq9_coefficients(const Consts& C, float tx, floa
   }
 }
 
-/* ---- F: lf_fit_kernel (a6 + ranking).  One thread per accepted candidate, a pass of FIT_THREADS records at a
+/* ---- F: lf_fit_kernel (a6, a7).  One thread per accepted candidate, a pass of FIT_THREADS records at a
  * time; the records of a seed are adjacent and a pass ends on a seed boundary, so after one barrier the lowest
  * (Q, k) of every seed is known (64-bit atomicMin in shared memory) and the winning thread still holds its fit
  * in registers: it writes the 20-word track record (q/p from Eq. 9, state at z_state).  Then the CTA ranks the
- * event's tracks in seed order. */
+ * event's tracks in seed order into the event's dense track list.
+ *
+ * a7 (stream compaction) without a scan or a compaction kernel: the events' track counts are scanned by a decoupled
+ * look-back over `ev_state` (64-bit words: flag << 32 | value; flag 1 = the event's own count, 2 = inclusive prefix).
+ * A CTA publishes its event's count when the event is done and resolves the event's prefix TWO events later, inside
+ * the next-but-one fetch_event while the bulk copy of the new event's hits is in flight: the look-back then meets
+ * counts that were published long ago and does not wait on a running event.  No deadlock either way: tickets are handed
+ * out in event order, so every lower-numbered event is owned by a CTA that is running or done, and publishing a count
+ * waits on nothing.  With the prefix known the CTA copies the event's tracks from its per-seed records (L2-resident:
+ * it wrote them two events ago) to their final dense position, in (event, seed) order; the last CTA out re-arms the
+ * event tickets. */
+struct TrackOut {
+  int32_t *hit_idx, *seed_idx, *n_hits;
+  float *state, *quality;
+  uint32_t *event_offsets, *n_tracks;
+  unsigned long long* ev_state; /* n_events look-back words, zeroed by the window kernel of the same lf_run */
+  uint32_t* tickets;            /* N_TICKETS event tickets + the count of CTAs of this kernel that are done */
+};
+/* CTA-wide scalars that live across events (kept out of registers) */
+enum { TM_EXCL = 0,                                 /* exclusive prefix of the event being resolved */
+       TM_OLD_EV, TM_OLD_S0, TM_OLD_N, TM_OLD_SLOT, /* the event finished two events ago (ev + 1; 0 = none): resolved in
+                                                       the next fetch_event */
+       TM_NEW_EV, TM_NEW_S0, TM_NEW_N, TM_NEW_SLOT, /* the event finished last */
+       TM_SLOT,                                     /* track-list slot of the current event (0..2) */
+       TM_WORDS = 12 };
+constexpr int LIST_CAP = 384; /* tracks of an event whose list is also kept in shared memory until the event is copied out */
 struct FitTables {
   unsigned long long* best; /* 2 * FIT_THREADS: lowest (Q bits << 32 | k) per seed of the pass, double-buffered */
   int* next_b;              /* 2: first left-over record of a pass (consumed one barrier later) */
   int* wcnt;                /* 2 * 8: seed changes per warp */
+  uint32_t* misc;           /* TM_WORDS */
+  uint32_t* list;           /* 3 * LIST_CAP: the track lists (seeds) of the current event and of the two still to be copied out */
 };
-constexpr size_t FIT_TABLES_BYTES = 2 * FIT_THREADS * 8 + 16 + 16 * 4;
+constexpr size_t FIT_TABLES_BYTES = 2 * FIT_THREADS * 8 + 16 + 16 * 4 + TM_WORDS * 4 + 3 * LIST_CAP * 4;
+
+__device__ __forceinline__ unsigned long long ld_state(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_state(unsigned long long* p, unsigned long long v) {
+  asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+/* Decoupled look-back by one warp: exclusive prefix of event `ev` over ev_state; publishes the inclusive prefix. */
+__device__ __forceinline__ uint32_t lookback_publish(unsigned long long* state, int ev, uint32_t n, int lane) {
+  uint32_t excl = 0;
+  for (int idx = ev - 1; idx >= 0; idx -= 32) {
+    const int j = idx - lane;
+    unsigned long long v;
+    do { /* every lower-numbered event belongs to a CTA that is running or done: its count arrives */
+      v = (j >= 0) ? ld_state(state + j) : (2ull << 32);
+    } while (__any_sync(FULL, (uint32_t)(v >> 32) == 0u));
+    const unsigned pm = __ballot_sync(FULL, (uint32_t)(v >> 32) == 2u);
+    const int first = pm ? (__ffs(pm) - 1) : 31; /* the nearest event whose inclusive prefix is known */
+    uint32_t c = (lane <= first) ? (uint32_t)v : 0u;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(FULL, c, o);
+    excl += c;
+    if (pm) break;
+  }
+  if (lane == 0) st_state(state + ev, (2ull << 32) | (unsigned long long)(excl + n));
+  return excl;
+}
+
+/* a7, second half: the tracks of a resolved event go from the per-seed records to their dense final position.  One
+ * thread per track: its five 16-byte loads are in flight together (one L2 round trip per event instead of one per load);
+ * `list` is the event's track list in shared memory, or nullptr if it did not fit (then the global copy is read). */
+__device__ __forceinline__ void copy_out_event(const EventArgs& A, const TrackOut& O, const uint32_t* list, uint32_t s0, int n,
+                                               uint32_t excl) {
+  for (int t = threadIdx.x; t < n; t += FIT_THREADS) {
+    const uint32_t seed = list ? list[t] : (uint32_t)__ldcg(A.ws_rank + s0 + t);
+    const int4* src = reinterpret_cast<const int4*>(A.ws_rec) + (size_t)seed * (REC_WORDS / 4);
+    const int4 h0 = __ldcg(src), h1 = __ldcg(src + 1), h2 = __ldcg(src + 2), p0 = __ldcg(src + 3), p1 = __ldcg(src + 4);
+    const size_t dst = (size_t)excl + (size_t)t;
+    int4* hd = reinterpret_cast<int4*>(O.hit_idx) + dst * 3;
+    hd[0] = h0;
+    hd[1] = h1;
+    hd[2] = h2;
+    O.seed_idx[dst] = p0.x;
+    O.n_hits[dst] = p0.y;
+    float* sd = O.state + dst * 5;
+    sd[0] = __int_as_float(p0.z);
+    sd[1] = __int_as_float(p0.w);
+    sd[2] = __int_as_float(p1.x);
+    sd[3] = __int_as_float(p1.y);
+    sd[4] = __int_as_float(p1.z);
+    O.quality[dst] = __int_as_float(p1.w);
+  }
+}
 
 template <bool DEBUG, bool WIDE, bool STAGED>
-__device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, CtaHeader& H, const EventCtx& E,
-                                          const HitView<STAGED>& hx, const FitTables& T) {
+__device__ __forceinline__ int fit_event(const Consts& C, const EventArgs& A, CtaHeader& H, const EventCtx& E,
+                                         const HitView<STAGED>& hx, const FitTables& T) {
   typedef Fmt<WIDE> F;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
@@ -1798,29 +1891,27 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
     for (int wq = 0; wq < FIT_THREADS / 32; ++wq) slot += (wq < warp) ? wc[wq] : 0;
     /* ---- the fit, sums in ascending layer order */
     float a0 = 0.f, t0 = 0.f, c0 = 0.f, da = 0.f, dt = 0.f, dc = 0.f, dy0 = 0.f, dtym = 0.f, Q = 0.f, y = 0.f, tx = 0.f, ty = 0.f;
-    uint32_t wf[NL];
-    int n = 0;
+    unsigned mask = 0;
+    CandHits h;
+    h.w[0] = r.x; h.w[1] = r.y; h.w[2] = r.z;
     unsigned long long key = ~0ull;
     if (mine) {
       const size_t row = (size_t)seed * sides + side;
       const uint4* wp = reinterpret_cast<const uint4*>(A.win + row * WIN_ROW);
       const uint4 w0 = __ldg(wp), w1 = __ldg(wp + 1), w2 = __ldg(wp + 2);
+      uint32_t wf[NL]; /* event-relative hit index per layer (meaningless if the layer has no hit); dead after the first loop */
       wf[0] = w0.x; wf[1] = w0.y; wf[2] = w0.z; wf[3] = w0.w; wf[4] = w1.x; wf[5] = w1.y; wf[6] = w1.z; wf[7] = w1.w;
       wf[8] = w2.x; wf[9] = w2.y; wf[10] = w2.z; wf[11] = w2.w;
       y = __ldg(A.sy + seed);
       tx = __ldg(A.stx + seed);
       ty = __ldg(A.sty + seed);
-      CandHits h;
-      h.w[0] = r.x; h.w[1] = r.y; h.w[2] = r.z;
-      unsigned mask = 0;
 #pragma unroll
       for (int l = 0; l < NL; ++l) {
         const unsigned cd = code_of(h, l);
-        wf[l] = (wf[l] >> F::WB) + cd; /* event-relative hit index (meaningless if the layer has no hit) */
+        wf[l] = (wf[l] >> F::WB) + cd;
         mask |= (cd != 0xFFu) ? (1u << l) : 0u;
       }
-      n = __popc(mask);
-      const int n_uv = __popc(mask & 0x666u);
+      const int n = __popc(mask), n_uv = __popc(mask & 0x666u);
       {
         const int set = (int)((r.w >> F::SET_SHIFT) & 1u);
         const float x0 = hx[(int)(set ? wf[3] : wf[0])], x1 = hx[(int)(set ? wf[7] : wf[4])], x2 = hx[(int)(set ? wf[11] : wf[8])];
@@ -1893,12 +1984,17 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
         key = ((unsigned long long)__float_as_uint(Q) << 32) | (unsigned)((side << F::KB) | k);
         atomicMin(best + slot, key);
       }
-#pragma unroll
-      for (int l = 0; l < NL; ++l) wf[l] = ((mask >> l) & 1u) ? (E.h0 + wf[l]) : 0xFFFFFFFFu; /* global hit index or -1 */
     }
     __syncthreads();
     if (key != ~0ull && best[slot] == key) {
-      /* the seed's track: q/p (Eq. 9) and the state at z_state */
+      /* the seed's track: its global hit indices (-1 = none; the window row is read again here, by the winner only, rather
+       * than kept in 12 registers across the fit), q/p (Eq. 9) and the state at z_state */
+      const uint4* wp = reinterpret_cast<const uint4*>(A.win + ((size_t)seed * sides + side) * WIN_ROW);
+      const uint4 w0 = __ldg(wp), w1 = __ldg(wp + 1), w2 = __ldg(wp + 2);
+      uint32_t wf[NL] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w, w2.x, w2.y, w2.z, w2.w};
+#pragma unroll
+      for (int l = 0; l < NL; ++l) wf[l] = ((mask >> l) & 1u) ? (E.h0 + (wf[l] >> F::WB) + code_of(h, l)) : 0xFFFFFFFFu;
+      const int n = __popc(mask);
       const float a = a0 + da, tt = t0 + dt, c = c0 + dc;
       const float t_ref = tt * 0.001f;
       const float dslope = t_ref - tx;
@@ -1919,7 +2015,7 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
   }
   __syncthreads(); /* the track flags of this CTA's seeds are visible to all its threads */
   if (tid == 0) T.next_b[0] = T.next_b[1] = 0x7FFFFFFF;
-  /* ---- rank the event's tracks in seed order (a7, first half) */
+  /* ---- the event's track list: its seeds that have a track, in seed order (a7, first half) */
   int ev_tracks = 0;
   for (int cb = 0; cb < ns; cb += FIT_THREADS) {
     const bool in = cb + tid < ns;
@@ -1935,34 +2031,97 @@ __device__ __forceinline__ void fit_event(const Consts& C, const EventArgs& A, C
       off += (wq < warp) ? tq : 0;
       tot += tq;
     }
-    if (in) {
-      A.ws_rank[seed] = found ? (ev_tracks + off + __popc(m & ((1u << lane) - 1u))) : -1;
-      A.ws_event[seed] = (int32_t)E.ev;
+    if (found) {
+      const int pos = ev_tracks + off + __popc(m & ((1u << lane) - 1u));
+      A.ws_rank[s0 + (uint32_t)pos] = (int32_t)seed;
+      if (pos < LIST_CAP) T.list[T.misc[TM_SLOT] * LIST_CAP + pos] = seed;
     }
     ev_tracks += tot;
     __syncthreads();
   }
   if (tid == 0) A.ev_count[E.ev] = (uint32_t)ev_tracks;
+  return ev_tracks;
 }
 
 template <bool DEBUG, bool WIDE>
 __global__ void __launch_bounds__(FIT_THREADS, 4) lf_fit_kernel(const __grid_constant__ Consts C,
-                                                                const __grid_constant__ EventArgs A) {
+                                                                const __grid_constant__ EventArgs A,
+                                                                const __grid_constant__ TrackOut O) {
   CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
   unsigned char* tb = lf_smem + HDR_BYTES + (size_t)A.stage_cap * sizeof(float);
   FitTables T;
   T.best = reinterpret_cast<unsigned long long*>(tb);
   T.next_b = reinterpret_cast<int*>(tb + 2 * FIT_THREADS * 8);
   T.wcnt = T.next_b + 4;
-  if (threadIdx.x == 0) {
+  T.misc = reinterpret_cast<uint32_t*>(T.wcnt + 16);
+  T.list = T.misc + TM_WORDS;
+  const int tid = threadIdx.x;
+  if (tid == 0) {
     mbar_init(&H.mbar, 1);
     T.next_b[0] = T.next_b[1] = 0x7FFFFFFF;
   }
+  if (tid < TM_WORDS) T.misc[tid] = 0u; /* published by fetch_event's barriers */
+  /* Resolves the event in the TM_OLD_* words: look-back by warp 1, which neither issues nor polls the bulk copy.  Called
+   * inside fetch_event (the words it reads were written before fetch_event's first barrier). */
+  auto resolve = [&]() {
+    if ((threadIdx.x >> 5) == 1 && T.misc[TM_OLD_EV] != 0u) {
+      const int ev = (int)T.misc[TM_OLD_EV] - 1;
+      const uint32_t n = T.misc[TM_OLD_N];
+      const uint32_t excl = lookback_publish(O.ev_state, ev, n, threadIdx.x & 31);
+      if ((threadIdx.x & 31) == 0) {
+        T.misc[TM_EXCL] = excl;
+        O.event_offsets[ev] = excl;
+        if (ev == (int)A.n_events - 1) {
+          O.event_offsets[ev + 1] = excl + n;
+          *O.n_tracks = excl + n;
+        }
+      }
+    }
+  };
+  /* after the barrier that follows resolve(): copies the resolved event out and shifts the queue of finished events */
+  auto retire = [&]() {
+    if (T.misc[TM_OLD_EV] != 0u) {
+      const int n = (int)T.misc[TM_OLD_N];
+      copy_out_event(A, O, n <= LIST_CAP ? T.list + T.misc[TM_OLD_SLOT] * LIST_CAP : nullptr, T.misc[TM_OLD_S0], n, T.misc[TM_EXCL]);
+    }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+      T.misc[TM_OLD_EV + threadIdx.x] = T.misc[TM_NEW_EV + threadIdx.x];
+      T.misc[TM_NEW_EV + threadIdx.x] = 0u;
+    }
+  };
   uint32_t phase = 0;
   EventCtx E;
-  while (fetch_event(A, phase, E)) {
-    if (E.staged) fit_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>(E.skew), T);
-    else fit_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>(E.gview), T);
+  while (fetch_event(A, phase, E, resolve)) {
+    retire();
+    int n;
+    if (E.staged) n = fit_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>(E.skew), T);
+    else n = fit_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>(E.gview), T);
+    if (tid == 0) { /* the event is done: publish its count; fetch_event's first barrier publishes the TM_NEW_* words */
+      st_state(O.ev_state + E.ev, (1ull << 32) | (unsigned long long)(uint32_t)n);
+      T.misc[TM_NEW_EV] = E.ev + 1u;
+      T.misc[TM_NEW_S0] = A.seed_off[E.ev];
+      T.misc[TM_NEW_N] = (uint32_t)n;
+      const uint32_t slot = T.misc[TM_SLOT];
+      T.misc[TM_NEW_SLOT] = slot;
+      T.misc[TM_SLOT] = (slot == 2u) ? 0u : slot + 1u; /* three lists in turn: the current event's and the two pending ones' */
+    }
+  }
+  /* the batch is exhausted: resolve what this CTA still holds, in event order */
+#pragma unroll 1
+  for (int r = 0; r < 2; ++r) {
+    resolve();
+    __syncthreads();
+    retire();
+    __syncthreads();
+  }
+  /* the last CTA out re-arms the tickets of all event kernels for the next lf_run */
+  if (tid == 0) {
+    __threadfence();
+    if (atomicAdd(O.tickets + N_TICKETS, 1u) == gridDim.x - 1u) {
+#pragma unroll
+      for (int i = 0; i <= N_TICKETS; ++i) O.tickets[i] = 0u;
+    }
   }
 }
 
@@ -2025,84 +2184,6 @@ __global__ void __launch_bounds__(256) lf_validate_kernel(const float* __restric
     bool ok = isfinite(sx[s]) && isfinite(sy[s]) && isfinite(stx[s]) && isfinite(sty[s]);
     if (sqop != nullptr) ok = ok && isfinite(sqop[s]);
     if (!ok) { atomicOr(result, BAD_SEED_VALUE); atomicMin(result + 3, s); }
-  }
-}
-
-/* Exclusive scan of per-event track counts (single CTA); also re-arms the event tickets. */
-__global__ void __launch_bounds__(1024) lf_scan_kernel(const uint32_t* __restrict__ ev_count, uint32_t n_events,
-                                                       uint32_t* __restrict__ ev_off_ws, uint32_t* __restrict__ out_off,
-                                                       uint32_t* __restrict__ n_tracks, uint32_t* tickets) {
-  __shared__ uint32_t warp_tot[32];
-  __shared__ uint32_t carry;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  if (tid == 0) carry = 0;
-  __syncthreads();
-  for (uint32_t c = 0; c < n_events; c += 1024) {
-    const uint32_t i = c + tid;
-    const uint32_t v = (i < n_events) ? ev_count[i] : 0u;
-    uint32_t incl = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const uint32_t t = __shfl_up_sync(FULL, incl, o);
-      if (lane >= o) incl += t;
-    }
-    if (lane == 31) warp_tot[warp] = incl;
-    __syncthreads();
-    if (warp == 0) {
-      uint32_t wt = warp_tot[lane];
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t t = __shfl_up_sync(FULL, wt, o);
-        if (lane >= o) wt += t;
-      }
-      warp_tot[lane] = wt; /* inclusive over warps */
-    }
-    __syncthreads();
-    const uint32_t excl = carry + (warp > 0 ? warp_tot[warp - 1] : 0u) + (incl - v);
-    if (i < n_events) {
-      ev_off_ws[i] = excl;
-      out_off[i] = excl;
-    }
-    __syncthreads();
-    if (tid == 0) carry += warp_tot[31];
-    __syncthreads();
-  }
-  if (tid == 0) {
-    out_off[n_events] = carry;
-    *n_tracks = carry;
-  }
-  if (tid < N_TICKETS) tickets[tid] = 0u;
-}
-
-/* Stream compaction (a7): one thread per (seed, 16-byte quarter of its record); coalesced 16-byte reads of
- * the per-seed records, dense SoA writes in (event, seed) order (16-byte stores for the hit lists). */
-__global__ void __launch_bounds__(256) lf_compact_kernel(const int32_t* __restrict__ ws_rec, const int32_t* __restrict__ ws_rank,
-                                                         const int32_t* __restrict__ ws_event, const uint32_t* __restrict__ ev_off,
-                                                         size_t seed_base, size_t n_seeds, int32_t* __restrict__ hit_idx,
-                                                         int32_t* __restrict__ seed_idx, int32_t* __restrict__ n_hits,
-                                                         float* __restrict__ state, float* __restrict__ quality) {
-  constexpr int Q4 = REC_WORDS / 4; /* 5 quarters: 3 of hit indices, (seed, n, x, y), (tx, ty, q/p, Q) */
-  size_t gid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (gid >= n_seeds * Q4) return;
-  gid += seed_base * Q4; /* the batch's seeds are [seed_base, seed_base + n_seeds) */
-  const size_t seed = gid / Q4;
-  const int q = (int)(gid - seed * Q4);
-  const int rank = ws_rank[seed];
-  if (rank < 0) return;
-  const size_t dst = (size_t)ev_off[ws_event[seed]] + (size_t)rank;
-  const int4 v = reinterpret_cast<const int4*>(ws_rec)[gid];
-  if (q < 3) {
-    reinterpret_cast<int4*>(hit_idx)[dst * 3 + q] = v;
-  } else if (q == 3) {
-    seed_idx[dst] = v.x;
-    n_hits[dst] = v.y;
-    state[dst * 5 + 0] = __int_as_float(v.z);
-    state[dst * 5 + 1] = __int_as_float(v.w);
-  } else {
-    state[dst * 5 + 2] = __int_as_float(v.x);
-    state[dst * 5 + 3] = __int_as_float(v.y);
-    state[dst * 5 + 4] = __int_as_float(v.z);
-    quality[dst] = __int_as_float(v.w);
   }
 }
 
