@@ -713,7 +713,7 @@ __global__ void __launch_bounds__(WIN_THREADS, 8) lf_window_kernel(const __grid_
   uint32_t phase = 0;
   EventCtx E;
   while (fetch_event(A, phase, E)) {
-    if (threadIdx.x == 0) A.ev_state[E.ev] = 0ull; /* re-arms the look-back word of the event (lf_track_kernel) */
+    if (threadIdx.x == 0) A.ev_state[E.ev] = 0ull; /* re-arms the look-back word of the event (lf_fit_kernel) */
     if (E.staged) {
       flag_equal_neighbours(A, E, HitView<true>(E.skew));
       windows_of_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>(E.skew));
@@ -1643,17 +1643,22 @@ __device__ __forceinline__ void extend_event(const Consts& C, const EventArgs& A
       for (int k = 0; k < my_n; ++k) T.item[excl + k] = (uint16_t)((tid << F::KB) | k);
     }
     __syncthreads();
-    /* ---- one thread per candidate; the accepted ones are appended in candidate order */
+    /* ---- one thread per candidate; the accepted ones are appended in candidate order.  The candidate's item and its
+     * triplet code are fetched one pass ahead. */
+    const unsigned KM = (1u << F::KB) - 1u;
+    unsigned im = (tid < total) ? T.item[tid] : 0u;
+    unsigned code = (tid < total) ? (unsigned)trip_code[(rbase + (size_t)(im >> F::KB)) * NT + (im & KM)] : 0u;
     for (int base = 0; base < total; base += FIT_THREADS) {
       const int it = base + tid;
+      const bool more = it + FIT_THREADS < total;
+      const unsigned im_next = more ? T.item[it + FIT_THREADS] : 0u;
+      const unsigned code_next = more ? (unsigned)trip_code[(rbase + (size_t)(im_next >> F::KB)) * NT + (im_next & KM)] : 0u;
       bool enough = false;
       CandHits h;
       unsigned tag = 0;
       if (it < total) {
-        const unsigned im = T.item[it];
-        const int rl = (int)(im >> F::KB), k = (int)(im & ((1u << F::KB) - 1u));
+        const int rl = (int)(im >> F::KB), k = (int)(im & KM);
         const size_t row = rbase + (size_t)rl;
-        const unsigned code = trip_code[row * NT + k];
         h = extend_candidate<WIDE>(C, hx, T.win + rl * NL, T.geo, T.sp[rl * 4 + 0], T.sp[rl * 4 + 1], T.sp[rl * 4 + 2], code, dup);
         enough = h.enough;
         /* seed inside the event, (side,) candidate index */
@@ -1670,6 +1675,8 @@ __device__ __forceinline__ void extend_event(const Consts& C, const EventArgs& A
           if (A.dbg.cand_quality && !enough) A.dbg.cand_quality[row * NT + k] = -1.0f;
         }
       }
+      im = im_next;
+      code = code_next;
       const unsigned m = __ballot_sync(FULL, enough);
       int* wc = T.wcnt + parity * 8;
       if (lane == 0) wc[warp] = __popc(m);
@@ -1715,7 +1722,30 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_extend_kernel(const __grid_
   }
   uint32_t phase = 0;
   EventCtx E;
-  while (fetch_event(A, phase, E)) {
+  /* while the event's hits are on their way: pull its per-row tables (window rows, triplet counts and codes, seed
+   * parameters; written by the earlier kernels, so in DRAM by now) into L2 */
+  auto prefetch_tables = [&]() {
+    const int tid = threadIdx.x;
+    const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
+    const int sides = WIDE ? C.sides : 1;
+    const size_t row0 = (size_t)s0 * sides, n_rows = (size_t)(s1 - s0) * sides;
+    const char* rows = reinterpret_cast<const char*>(A.win + row0 * WIN_ROW);
+    for (size_t o = (size_t)tid * 128; o < n_rows * WIN_ROW * 4; o += (size_t)FIT_THREADS * 128)
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(rows + o));
+    const size_t cbytes = n_rows * NT * sizeof(typename Fmt<WIDE>::code_t);
+    const char* codes = static_cast<const char*>(A.trip_code) + row0 * NT * sizeof(typename Fmt<WIDE>::code_t);
+    for (size_t o = (size_t)tid * 128; o < cbytes; o += (size_t)FIT_THREADS * 128)
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(codes + o));
+    if (tid < 8) {
+      if ((size_t)tid * 128 < n_rows) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.n_trip + row0 + (size_t)tid * 128));
+    } else if (tid >= 32 && tid < 32 + 3 * 8) {
+      const int a = (tid - 32) >> 3;
+      const size_t o = (size_t)((tid - 32) & 7) * 32;
+      const float* base = (a == 0) ? A.sy : ((a == 1) ? A.stx : A.sty);
+      if (o < (size_t)(s1 - s0)) asm volatile("prefetch.global.L2 [%0];" ::"l"(base + s0 + o));
+    }
+  };
+  while (fetch_event(A, phase, E, prefetch_tables)) {
     if (E.staged) extend_event<DEBUG, WIDE, true>(C, A, H, E, HitView<true>(E.skew), T);
     else extend_event<DEBUG, WIDE, false>(C, A, H, E, HitView<false>(E.gview), T);
   }
@@ -2063,7 +2093,28 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_fit_kernel(const __grid_con
   if (tid < TM_WORDS) T.misc[tid] = 0u; /* published by fetch_event's barriers */
   /* Resolves the event in the TM_OLD_* words: look-back by warp 1, which neither issues nor polls the bulk copy.  Called
    * inside fetch_event (the words it reads were written before fetch_event's first barrier). */
-  auto resolve = [&]() {
+  EventCtx E;
+  auto resolve = [&](bool taken = true) {
+    if (taken && threadIdx.x >= 64) {
+      /* the other warps, while the event's hits are on their way: its records, window rows and seed parameters -> L2 */
+      const int t = threadIdx.x - 64, nthr = FIT_THREADS - 64;
+      const uint32_t s0 = A.seed_off[E.ev], s1 = A.seed_off[E.ev + 1];
+      const int sides = WIDE ? C.sides : 1;
+      const size_t row0 = (size_t)s0 * sides, n_rows = (size_t)(s1 - s0) * sides;
+      const char* recs = reinterpret_cast<const char*>(A.acc_rec + row0 * C.n_triplets);
+      const size_t rbytes = (size_t)A.ev_acc[E.ev] * sizeof(uint4);
+      for (size_t o = (size_t)t * 128; o < rbytes; o += (size_t)nthr * 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(recs + o));
+      const char* rows = reinterpret_cast<const char*>(A.win + row0 * WIN_ROW);
+      for (size_t o = (size_t)t * 128; o < n_rows * WIN_ROW * 4; o += (size_t)nthr * 128)
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(rows + o));
+      if (t < 4 * 8) {
+        const int a = t >> 3;
+        const size_t o = (size_t)(t & 7) * 32;
+        const void* base = (a == 0) ? (const void*)(A.sy + s0 + o) : ((a == 1) ? (const void*)(A.stx + s0 + o)
+                           : ((a == 2) ? (const void*)(A.sty + s0 + o) : (const void*)(A.ws_nh + s0 + o)));
+        if (o < (size_t)(s1 - s0)) asm volatile("prefetch.global.L2 [%0];" ::"l"(base));
+      }
+    }
     if ((threadIdx.x >> 5) == 1 && T.misc[TM_OLD_EV] != 0u) {
       const int ev = (int)T.misc[TM_OLD_EV] - 1;
       const uint32_t n = T.misc[TM_OLD_N];
@@ -2091,7 +2142,6 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_fit_kernel(const __grid_con
     }
   };
   uint32_t phase = 0;
-  EventCtx E;
   while (fetch_event(A, phase, E, resolve)) {
     retire();
     int n;
@@ -2110,7 +2160,7 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_fit_kernel(const __grid_con
   /* the batch is exhausted: resolve what this CTA still holds, in event order */
 #pragma unroll 1
   for (int r = 0; r < 2; ++r) {
-    resolve();
+    resolve(false);
     __syncthreads();
     retire();
     __syncthreads();
