@@ -304,15 +304,30 @@ def run_ours(args):
     lf.set_profiling(True)
     sampler = ClockSampler(local_rank)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # timing rule: the inputs of a step must not be served from L2 left warm by the previous step.  The headline batches are
+    # several times the 126 MB L2; a batch that is not (configs 0, 1, 2) is timed step by step with a 256 MB write between steps
+    flush_l2 = batch.input_bytes() < 2 * 126e6
     barrier()
     sampler.start()
-    e0.record(stream)
-    for _ in range(args.steps):
-        lf.run(db, out, stream)
-    e1.record(stream)
-    barrier()
-    clocks = sampler.stop()
-    local_ms = e0.elapsed_time(e1)
+    if flush_l2:
+        scrub = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for a, b in evs:
+            scrub.zero_()
+            a.record(stream)
+            lf.run(db, out, stream)
+            b.record(stream)
+        barrier()
+        clocks = sampler.stop()
+        local_ms = sum(a.elapsed_time(b) for a, b in evs)
+    else:
+        e0.record(stream)
+        for _ in range(args.steps):
+            lf.run(db, out, stream)
+        e1.record(stream)
+        barrier()
+        clocks = sampler.stop()
+        local_ms = e0.elapsed_time(e1)
     ktimes = dict(zip(binding.KERNEL_NAMES, lf.kernel_times()))
     lf.set_profiling(False)
     total_ms, (tot_events, tot_seeds, tot_tracks) = sharding.reduce_job(
@@ -431,7 +446,8 @@ def run_ours(args):
                    "tuning": args.tuning, "fp16_input": fp16_mode,
                    "events_per_gpu": batch.n_events, "seeds_per_gpu": batch.n_seeds, "hits_per_gpu": batch.n_hits,
                    "tracks_per_step_per_gpu": n_tracks, "accepted_candidates_per_step": n_acc, "events_with_equal_hits": n_dup_events,
-                   "l2": f"no flush: inputs ({in_bytes / 1e6:.0f} MB) + outputs exceed the 126 MB L2",
+                   "l2": (f"flushed: inputs are {in_bytes / 1e6:.0f} MB, so every step is timed on its own after a 256 MB write"
+                          if flush_l2 else f"no flush: inputs ({in_bytes / 1e6:.0f} MB) + outputs exceed the 126 MB L2"),
                    "sharding": "events, no data-path collective"},
         "seeds_per_s": tot_seeds / (ms_per_step * 1e-3),
         "tracks_per_s": tot_tracks / (ms_per_step * 1e-3),

@@ -158,7 +158,7 @@ struct __align__(16) CtaHeader {
   int nsteps; /* binary-search steps that cover the event's longest segment */
   int warp_tot[8];
   int dup; /* != 0: the event may hold equal neighbouring hits (closest_hit must resolve runs of ties) */
-  int blk_pref[NSEG + 1]; /* fp16 hit storage: blocks of 32 hits in front of each segment of the event */
+  int blk_pref[NSEG + 1]; /* fp16 hit storage: decode trips (32 hits each, one per warp pass) in front of each segment of the event */
   int xdelta[NL];         /* seeding kernel: hit i of an x layer l lives at stage position i - xdelta[l] (fetch_event_x) */
 };
 constexpr int HDR_BYTES = (sizeof(CtaHeader) + 15) & ~15;
@@ -302,9 +302,9 @@ __device__ __forceinline__ bool fetch_event(const EventArgs& A, uint32_t& phase,
   E.skew = from16 ? 0 : (int)((reinterpret_cast<uintptr_t>(gsrc) >> 2) & 3);
   E.gview = from16 ? A.hx_scratch + E.h0 : gsrc;
   if (from16) {
-    /* fp16 hit storage (lf_pack_hits_kernel): x~ = origin(block) + half, blocks of 32 hits counted from the start of
-     * each segment.  One warp decodes one block per trip: a 64-byte load of halves, one origin, 32 fp32 stores into
-     * the stage (or, for an event larger than the stage, into the library's fp32 scratch image, once per lf_run). */
+    /* fp16 hit storage (lf_pack_hits_kernel): x~ = origin(block of 8 hits) + half.  One warp decodes one trip of 32 hits
+     * (counted from the start of each segment) at a time: a 64-byte load of halves, the origins, 32 fp32 stores into the
+     * stage (or, for an event larger than the stage, into the library's fp32 scratch image, once per lf_run). */
     if (tid < 32) {
       const int nb = (tid < NSEG) ? (int)((so[tid + 1] - so[tid] + 31u) >> 5) : 0;
       int incl = nb;
@@ -2177,10 +2177,10 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_fit_kernel(const __grid_con
 
 /* hit_storage = 1 (BASELINE.json configs[2]; "store hit data in fp16 in addition to fp32"):
  * writes the fp16 copy of the hits.  Block-offset encoding: inside every (event, layer, zone) segment,
- * consecutive hits form blocks of 32; a block's origin is the fp32 coordinate of its 17th hit (or its last
- * one if shorter); each hit stores half(x - origin), so |offset| stays within half a block's x span
- * (ulp <= 0.25 mm at Run-3 occupancy).  The origin slot of block b of global segment g starting at hit S is
- * (S >> 5) + g + b: slots of different segments never overlap, so the index alone locates the origin. */
+ * consecutive hits form blocks of 2^H16_SHIFT = 8; a block's origin is the fp32 coordinate of its 5th hit (or its
+ * last one if shorter); each hit stores half(x - origin), so |offset| stays within half a block's x span.  The origin
+ * slot of block b of global segment g starting at hit S is (S >> H16_SHIFT) + g + b: slots of different segments never
+ * overlap, so the index alone locates the origin. */
 __global__ void __launch_bounds__(256) lf_pack_hits_kernel(const float* __restrict__ hx, const uint32_t* __restrict__ seg_off,
                                                            uint32_t n_events, uint32_t event_base,
                                                            __half* __restrict__ hx16, float* __restrict__ origin16) {
