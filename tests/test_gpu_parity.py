@@ -567,8 +567,9 @@ def test_stream_compaction_lookback_stress(lfmod, oracle, geometry, params):
     """a7 inside the fit kernel (decoupled look-back over the events' track counts): batches that
     stress the scan rather than the arithmetic.  (1) 40 000 tiny events, most of them without a track, far more events than
     resident CTAs; (2) full events alternating with seedless ones in runs of irregular length, so that CTAs finish their
-    events in an order far from the event order; (3) two handles running on two streams at the same time; (4) the same
-    batch through lf_run_host, whose chunks are separate launches."""
+    events in an order far from the event order; (3) two handles running on two streams at the same time; (4) events with
+    more tracks than the shared-memory track list holds; (5) the tiny events through lf_run_host, whose chunks are separate
+    launches."""
     import torch
     tiny = dg.generate(dg.GenConfig("tiny_events", 40000, 77, true_mean=1.2, fake_mean=0.3, noise_mean=6.0))
     ref = oracle.run(geometry, params, tiny, threads=NTHREADS)
@@ -603,6 +604,11 @@ def test_stream_compaction_lookback_stress(lfmod, oracle, geometry, params):
     assert_tracks_equal(o2.to_numpy(), ref_m, "two handles in flight (mixed events)")
     lf1.close()
     lf2.close()
+    # events with more tracks than the shared-memory track list holds (384): the copy-out reads the global list
+    big = dg.generate(dg.GenConfig("big_events", 24, 78, true_mean=700.0, fake_mean=50.0, noise_mean=100.0))
+    ref_b = oracle.run(geometry, params, big, threads=NTHREADS)
+    assert np.diff(ref_b.event_offsets).min() > 384
+    assert_tracks_equal(_gpu_run(lfmod, geometry, params, big), ref_b, "events with more than 384 tracks")
     # the host path: chunks are separate launches, each with its own look-back
     lf = lfmod.LookingForward(geometry, params, tiny.n_events, tiny.n_seeds, tiny.n_hits)
     lf.set_host_chunk_events(1500)
