@@ -146,7 +146,7 @@ struct EventArgs {
   uint32_t* ev_acc;     /* n_events: number of such records of the event */
   const struct FitLut* fit_lut; /* 4096: per presence mask */
   uint32_t* ev_dup;     /* n_events: written by the window kernel, != 0 if two neighbouring staged hits are equal */
-  unsigned long long* ev_state; /* n_events: look-back words of lf_track_kernel, zeroed by the window kernel */
+  unsigned long long* ev_state; /* n_events: look-back words of the fit kernel's stream compaction, zeroed by the window kernel */
   DebugOut dbg;
 };
 
@@ -271,7 +271,8 @@ __device__ __forceinline__ typename HV::pos_t lower_pos(typename HV::pos_t a, ty
 /* Takes the next event and stages its hits.  Called by every thread of the CTA; returns false when
  * the batch is exhausted.  Hit i of the event then lives at stage_buf()[skew + i].  `while_loading` is called once by
  * every thread of an event that was taken, after the bulk copy has been issued and before anybody waits for it: work
- * that does not touch the stage hides behind the copy's latency (lf_track_kernel resolves an earlier event there). */
+ * that does not touch the stage hides behind the copy's latency (the extension and fit kernels pull the event's tables
+ * into L2 there; the fit kernel also resolves the output offset of an earlier event). */
 struct NoHook {
   __device__ __forceinline__ void operator()() const {}
 };
