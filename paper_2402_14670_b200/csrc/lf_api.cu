@@ -53,6 +53,7 @@ struct lf_handle {
   int device;
   int sm_count, stage_cap;
   int ext_chunk;   /* rows the extension kernel stages at a time: 256, or 128 if that keeps one more CTA per SM */
+  int win_threads; /* threads per CTA of the window kernel: 256, or 512 if that keeps more warps per SM (large stages) */
   int stage_cap_x; /* the seeding kernel stages the six x layers only: about half an event */
   int regs[4], grid[4], ctas_per_sm[4], smem_bytes[4]; /* window, seed, extend, fit kernels */
   unsigned long long* ev_state; /* look-back words of the fit kernel's stream compaction */
@@ -70,6 +71,8 @@ struct lf_handle {
   uint32_t *ev_count, *ev_dup, *ev_acc, *tickets;
   unsigned long long* counters; /* LF_N_COUNTERS: written by the debug build of the kernels */
   bool counters_valid = false;  /* the most recent launch was a debug launch */
+  bool tickets_dirty = false;   /* an lf_run failed between its first and its last launch: the event tickets, which the last
+                                   CTA of the fit kernel re-arms, may be left advanced; the next launch zeroes them first */
   uint32_t* validate_res; /* 4 words: lf_validate_inputs' violation bits and offending indices */
   uint4* acc_rec;
   lf::FitLut* fit_lut;
@@ -275,6 +278,8 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
                  const lf_debug* dbg, cudaStream_t st, size_t event_base = 0) {
   const bool prof = h->profiling;
   cudaEvent_t* pe = prof ? h->prof_ev[h->prof_runs % PROF_RING] : nullptr;
+  if (h->tickets_dirty) LF_CUDA(h, cudaMemsetAsync(h->tickets, 0, (lf::N_TICKETS + 1) * sizeof(uint32_t), st));
+  h->tickets_dirty = true; /* until every kernel of this run has been enqueued */
   if (prof) LF_CUDA(h, cudaEventRecord(pe[0], st));
   lf::EventArgs A;
   std::memset(&A, 0, sizeof(A));
@@ -328,7 +333,7 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
   if (work) {
     A.ticket = h->tickets + 0;
     A.scratch_writer = 1; /* the window kernel decodes oversized events once for all four kernels */
-    lf::lf_window_kernel<DEBUG, WIDE><<<grid_of(0), lf::WIN_THREADS, h->smem_bytes[0], st>>>(h->C, A);
+    lf::lf_window_kernel<DEBUG, WIDE><<<grid_of(0), h->win_threads, h->smem_bytes[0], st>>>(h->C, A);
   }
   if (prof) LF_CUDA(h, cudaEventRecord(pe[1], st));
   A.scratch_writer = 0;
@@ -366,6 +371,7 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
     ++h->prof_runs;
   }
   LF_CUDA(h, cudaGetLastError());
+  h->tickets_dirty = false;
   return LF_OK;
 }
 
@@ -479,8 +485,17 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
   const void* kern_h2[2] = {(const void*)lf::lf_seed_kernel<false, false, true>, (const void*)lf::lf_seed_kernel<true, false, true>};
   if (h->half2) { kern_n[1][0] = kern_h2[0]; kern_n[1][1] = kern_h2[1]; }
   const void* (*kern)[2] = h->wide ? kern_w : kern_n;
-  const int threads[4] = {lf::WIN_THREADS, lf::SEED_THREADS, lf::FIT_THREADS, lf::FIT_THREADS};
+  int threads[4] = {lf::WIN_THREADS, lf::SEED_THREADS, lf::FIT_THREADS, lf::FIT_THREADS};
+  h->win_threads = lf::WIN_THREADS;
   for (int k = 0; k < 4; ++k) {
+    if (k == 0) { /* window kernel: CTAs of 512 threads if they put more warps on an SM (a large stage limits the CTAs) */
+      int occ = 0, occ_big = 0;
+      for (int d = 0; d < 2; ++d)
+        LF_CREATE_CUDA(raise_dynamic_smem(kern[k][d], h->wide ? 1 : 0, k, d, h->device, h->smem_bytes[k]));
+      LF_CREATE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern[k][0], lf::WIN_THREADS, h->smem_bytes[k]));
+      LF_CREATE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_big, kern[k][0], lf::WIN_THREADS_BIG, h->smem_bytes[k]));
+      if (occ_big * lf::WIN_THREADS_BIG > occ * lf::WIN_THREADS) threads[0] = h->win_threads = lf::WIN_THREADS_BIG;
+    }
     if (k == 2) { /* extension kernel: half-size row tables if they buy a resident CTA (large events) */
       const int small = (int)(stage_bytes + lf::ext_tables_bytes(params->n_triplets, lf::FIT_CHUNK / 2));
       int occ_big = 0, occ_small = 0;
@@ -577,7 +592,7 @@ lf_status lf_destroy(lf_handle* h) {
 lf_status lf_get_info(const lf_handle* h, lf_info* out) {
   if (!h || !out) return LF_ERR_INVALID_ARG;
   out->kernels_per_run = LF_N_KERNELS + (h->P.hit_storage == 1 ? 1 : 0);
-  const int threads[4] = {lf::WIN_THREADS, lf::SEED_THREADS, lf::FIT_THREADS, lf::FIT_THREADS};
+  const int threads[4] = {h->win_threads, lf::SEED_THREADS, lf::FIT_THREADS, lf::FIT_THREADS};
   for (int k = 0; k < 4; ++k) {
     out->regs[k] = h->regs[k];
     out->block[k] = threads[k];

@@ -51,7 +51,8 @@ constexpr int REC_WORDS = 20;  /* 12 hit idx, seed, n_hits, 5 state, Q */
 constexpr int TRIP_BUF = 64;   /* per-warp triplet key buffer */
 constexpr int MAX_NT = 16;     /* == LF_MAX_TRIPLETS (narrow kernels) */
 constexpr int MAX_NT_WIDE = 32; /* == LF_MAX_TRIPLETS_WIDE */
-constexpr int WIN_THREADS = 256;
+constexpr int WIN_THREADS = 256;     /* window kernel: threads per CTA ... */
+constexpr int WIN_THREADS_BIG = 512; /* ... or, when a large stage leaves few CTAs per SM, this many (lf_create picks) */
 /* Two builds of every event kernel (template parameter WIDE):
  *   narrow  n_window <= 32, n_triplets <= 16, one followed track ("row") per seed: the with-UT tuning; a search
  *           window fits one hit per lane, window-relative hit indices take 5 bits;
@@ -602,7 +603,7 @@ __device__ __forceinline__ void windows_of_event(const Consts& C, const EventArg
   const int nsteps = H.nsteps;
   const bool pol_pos = C.polarity > 0;
   const int halfw = C.n_window / 2, reach = C.n_window + 1;
-  for (int it = tid; it < n_items; it += WIN_THREADS) {
+  for (int it = tid; it < n_items; it += (int)blockDim.x) {
     const int q12 = it / NL; /* (seed, side) pair; sides is 1 or 2, so no division by a run-time value */
     const int layer = it - q12 * NL;
     const int sl = WIDE ? (q12 >> (sides >> 1)) : q12;
@@ -701,13 +702,13 @@ __device__ __forceinline__ void windows_of_event(const Consts& C, const EventArg
 template <class HV>
 __device__ __forceinline__ void flag_equal_neighbours(const EventArgs& A, const EventCtx& E, const HV& hx) {
   int dup = 0;
-  for (int i = threadIdx.x; i + 1 < E.nh; i += WIN_THREADS) dup |= (hx[i] == hx[i + 1]) ? 1 : 0;
+  for (int i = threadIdx.x; i + 1 < E.nh; i += (int)blockDim.x) dup |= (hx[i] == hx[i + 1]) ? 1 : 0;
   dup = __syncthreads_or(dup);
   if (threadIdx.x == 0) A.ev_dup[E.ev] = (uint32_t)dup;
 }
 
 template <bool DEBUG, bool WIDE>
-__global__ void __launch_bounds__(WIN_THREADS, 8) lf_window_kernel(const __grid_constant__ Consts C,
+__global__ void __launch_bounds__(WIN_THREADS_BIG, 4) lf_window_kernel(const __grid_constant__ Consts C,
                                                                 const __grid_constant__ EventArgs A) {
   CtaHeader& H = *reinterpret_cast<CtaHeader*>(lf_smem);
   if (threadIdx.x == 0) mbar_init(&H.mbar, 1);
