@@ -46,7 +46,7 @@
 extern "C" {
 #endif
 
-#define LF_ABI_VERSION 6u
+#define LF_ABI_VERSION 7u
 #define LF_N_LAYERS 12   /* three T-stations, x-u-v-x each */
 #define LF_N_ZONES 2     /* lower / upper half */
 #define LF_MAX_WINDOW 32   /* largest params.n_window of the narrow kernels (one warp lane per hit) */
@@ -216,6 +216,25 @@ lf_status lf_run_debug(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits,
  * produced for the whole batch (dense, (event, seed) order). */
 lf_status lf_run_host(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events,
                       lf_tracks* out, void* cuda_stream);
+
+/* The same in two halves, for a stream of batches: lf_host_submit enqueues everything that needs no answer from the
+ * device (the host->device copies of the whole batch, the kernels of every chunk on `cuda_stream`, the read-back of the
+ * chunks' track counts) and returns at once; lf_host_collect then places the tracks in the caller's arrays as the chunks
+ * finish and returns when the batch's last byte has arrived (it does not wait for anything queued behind the batch).
+ * LF_HOST_SLOTS batches can be in flight on one handle, each in its own slot (its own device staging, allocated on first
+ * use), so that
+ *     submit(batch 0, slot 0); for (i = 1; i < n; ++i) { submit(batch i, slot i % 2); collect(slot (i - 1) % 2); } collect(last)
+ * copies batch i + 1 to the device while batch i is still being computed and copied back: the stream of batches then runs
+ * at the speed of the host->device link.  lf_run_host(..) == lf_host_submit(.., slot 0) + lf_host_collect(slot 0), except that
+ * lf_host_submit starts its copies at once (the caller's host arrays must be complete when it is called) instead of after the
+ * work already queued on `cuda_stream`.  The host arrays of `seeds`, `hits` and `out` must stay valid and untouched until the
+ * batch has been collected (the structs themselves are copied).  Batches in flight share the handle's workspace, so they must
+ * all use the same `cuda_stream` (LF_ERR_INVALID_ARG otherwise); a slot takes a new batch only after its previous one has been
+ * collected; lf_run and lf_run_host must not be called while a batch is in flight. */
+#define LF_HOST_SLOTS 2
+lf_status lf_host_submit(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events,
+                         lf_tracks* out, void* cuda_stream, int slot);
+lf_status lf_host_collect(lf_handle* h, int slot);
 
 /* Smallest number of events lf_run_host puts in one equal pipeline chunk (default 2048; >= 1).  The number of
  * equal chunks is min(13, max(1, n_events / min_events_per_chunk)); the last one is cut into four pieces. */

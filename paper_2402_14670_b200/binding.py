@@ -110,6 +110,11 @@ def load_library() -> C.CDLL:
         fn = getattr(lib, name)
         fn.restype = C.c_int
         fn.argtypes = [C.c_void_p, C.POINTER(lf_seeds), C.POINTER(lf_hits), C.c_size_t, C.POINTER(lf_tracks), C.c_void_p]
+    lib.lf_host_submit.restype = C.c_int
+    lib.lf_host_submit.argtypes = [C.c_void_p, C.POINTER(lf_seeds), C.POINTER(lf_hits), C.c_size_t, C.POINTER(lf_tracks),
+                                   C.c_void_p, C.c_int]
+    lib.lf_host_collect.restype = C.c_int
+    lib.lf_host_collect.argtypes = [C.c_void_p, C.c_int]
     lib.lf_validate_inputs.restype = C.c_int
     lib.lf_validate_inputs.argtypes = [C.c_void_p, C.POINTER(lf_seeds), C.POINTER(lf_hits), C.c_size_t, C.c_void_p]
     lib.lf_run_debug.restype = C.c_int
@@ -131,7 +136,7 @@ def load_library() -> C.CDLL:
     lib.lf_set_profiling.argtypes = [C.c_void_p, C.c_int]
     lib.lf_kernel_times.restype = C.c_int
     lib.lf_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_float * len(KERNEL_NAMES))]
-    if lib.lf_abi_version() != 6:
+    if lib.lf_abi_version() != 7:
         raise ImportError("liblf_b200.so: ABI version mismatch")
     for i, st in enumerate(_STRUCTS):
         if lib.lf_sizeof(i) != C.sizeof(st):
@@ -298,17 +303,33 @@ class LookingForward:
         return db
 
     # -- host path (end to end) ------------------------------------------------------------------
-    def run_host(self, hb: "HostBatch", out: "HostTracks", stream=None) -> int:
-        """``lf_run_host``: host buffers in, host buffers out; returns the number of tracks."""
+    @staticmethod
+    def _host_structs(hb: "HostBatch", out: "HostTracks"):
         seeds = lf_seeds(hb.seed_x.data_ptr(), hb.seed_y.data_ptr(), hb.seed_tx.data_ptr(), hb.seed_ty.data_ptr(),
                          hb.seed_qop.data_ptr(), hb.seed_offsets.data_ptr(), hb.n_seeds)
         p = lambda t: t.data_ptr() if t is not None else None
         hits = lf_hits(p(hb.hit_x), hb.seg_offsets.data_ptr(), hb.n_hits, p(hb.hit_x16), p(hb.origin16))
         tr = lf_tracks(out.hit_idx.data_ptr(), out.seed_idx.data_ptr(), out.n_hits.data_ptr(), out.state.data_ptr(),
                        out.quality.data_ptr(), out.event_offsets.data_ptr(), out.n_tracks.data_ptr(), out.capacity)
+        return seeds, hits, tr
+
+    def run_host(self, hb: "HostBatch", out: "HostTracks", stream=None) -> int:
+        """``lf_run_host``: host buffers in, host buffers out; returns the number of tracks."""
+        seeds, hits, tr = self._host_structs(hb, out)
         self._check(self._lib.lf_run_host(self._h, C.byref(seeds), C.byref(hits), hb.n_events, C.byref(tr),
                                           self._stream_ptr(stream)))
         return int(out.n_tracks[0])
+
+    def host_submit(self, hb: "HostBatch", out: "HostTracks", slot: int, stream=None):
+        """``lf_host_submit``: enqueue a host batch in ``slot`` (0 or 1) and return at once; ``hb`` and ``out`` must stay
+        alive and untouched until :meth:`host_collect` of that slot."""
+        seeds, hits, tr = self._host_structs(hb, out)
+        self._check(self._lib.lf_host_submit(self._h, C.byref(seeds), C.byref(hits), hb.n_events, C.byref(tr),
+                                             self._stream_ptr(stream), int(slot)))
+
+    def host_collect(self, slot: int):
+        """``lf_host_collect``: wait until the batch submitted to ``slot`` is complete in its host arrays."""
+        self._check(self._lib.lf_host_collect(self._h, int(slot)))
 
     def run_counters(self):
         """``lf_run_counters`` (synchronous): the work counters of the last run as a dict (include/lf.h); entries 2..6 are

@@ -27,7 +27,9 @@ constexpr int N_PROF_EV = LF_N_KERNELS + 1;
 constexpr int HOST_MAX_CHUNKS = 16;
 constexpr size_t HOST_CHUNK_EVENTS = 2048; /* measured on config 3: 8-10 chunks beat 16 (11.1 vs 11.6 ms) */
 
-struct HostBufs { /* device staging for lf_run_host */
+/* One batch in flight through the host path (lf_run_host = slot 0; lf_host_submit / lf_host_collect: LF_HOST_SLOTS of them,
+ * so that the copies of the next batch run while this one is finished): its device staging, events and bookkeeping. */
+struct HostSlot {
   float* seeds = nullptr;      /* 5 * max_seeds */
   uint32_t* seed_off = nullptr;
   float* hits = nullptr;
@@ -38,9 +40,20 @@ struct HostBufs { /* device staging for lf_run_host */
   float *state = nullptr, *quality = nullptr;
   uint32_t *ev_off = nullptr, *n_tracks = nullptr; /* ne + HOST_MAX_CHUNKS + 1; HOST_MAX_CHUNKS */
   uint32_t* pinned_count = nullptr; /* host, pinned: HOST_MAX_CHUNKS counts, then the chunk-relative event offsets */
-  cudaStream_t s_h2d = nullptr, s_cnt = nullptr, s_d2h = nullptr; /* library-owned copy streams */
-  cudaEvent_t ev_start = nullptr, ev_h2d[HOST_MAX_CHUNKS] = {}, ev_comp[HOST_MAX_CHUNKS] = {}, ev_cnt[HOST_MAX_CHUNKS] = {};
+  cudaEvent_t ev_start = nullptr, ev_done = nullptr, ev_h2d[HOST_MAX_CHUNKS] = {}, ev_comp[HOST_MAX_CHUNKS] = {}, ev_cnt[HOST_MAX_CHUNKS] = {};
   bool ready = false;
+  /* the submitted batch, until it has been collected */
+  bool pending = false;
+  cudaStream_t st = nullptr; /* the stream its kernels were enqueued on */
+  lf_tracks out = {};
+  size_t n_events = 0;
+  int n_chunks = 0;
+  size_t bounds[HOST_MAX_CHUNKS + 1] = {}; /* first event of every chunk */
+  size_t first_seed[HOST_MAX_CHUNKS + 1] = {};
+};
+struct HostBufs {
+  cudaStream_t s_h2d = nullptr, s_cnt = nullptr, s_d2h = nullptr; /* library-owned copy streams, shared by the slots */
+  HostSlot slot[LF_HOST_SLOTS];
 };
 
 } // namespace
@@ -565,20 +578,23 @@ lf_status lf_destroy(lf_handle* h) {
   cudaFree(h->ev_count); cudaFree(h->ev_dup); cudaFree(h->ev_acc); cudaFree(h->acc_rec); cudaFree(h->fit_lut); cudaFree(h->tickets); cudaFree(h->ev_state);
   cudaFree(h->validate_res);
   cudaFree(h->counters);
-  HostBufs& b = h->hb;
-  cudaFree(b.seeds); cudaFree(b.seed_off); cudaFree(b.hits); cudaFree(b.hits16); cudaFree(b.origin16); cudaFree(b.seg_off);
-  cudaFree(b.hit_idx); cudaFree(b.seed_idx); cudaFree(b.n_hits); cudaFree(b.state); cudaFree(b.quality);
-  cudaFree(b.ev_off); cudaFree(b.n_tracks);
-  if (b.pinned_count) cudaFreeHost(b.pinned_count);
-  if (b.s_h2d) cudaStreamDestroy(b.s_h2d);
-  if (b.s_cnt) cudaStreamDestroy(b.s_cnt);
-  if (b.s_d2h) cudaStreamDestroy(b.s_d2h);
-  if (b.ev_start) cudaEventDestroy(b.ev_start);
-  for (int c = 0; c < HOST_MAX_CHUNKS; ++c) {
-    if (b.ev_h2d[c]) cudaEventDestroy(b.ev_h2d[c]);
-    if (b.ev_comp[c]) cudaEventDestroy(b.ev_comp[c]);
-    if (b.ev_cnt[c]) cudaEventDestroy(b.ev_cnt[c]);
+  HostBufs& hb = h->hb;
+  for (HostSlot& b : hb.slot) {
+    cudaFree(b.seeds); cudaFree(b.seed_off); cudaFree(b.hits); cudaFree(b.hits16); cudaFree(b.origin16); cudaFree(b.seg_off);
+    cudaFree(b.hit_idx); cudaFree(b.seed_idx); cudaFree(b.n_hits); cudaFree(b.state); cudaFree(b.quality);
+    cudaFree(b.ev_off); cudaFree(b.n_tracks);
+    if (b.pinned_count) cudaFreeHost(b.pinned_count);
+    if (b.ev_start) cudaEventDestroy(b.ev_start);
+    if (b.ev_done) cudaEventDestroy(b.ev_done);
+    for (int c = 0; c < HOST_MAX_CHUNKS; ++c) {
+      if (b.ev_h2d[c]) cudaEventDestroy(b.ev_h2d[c]);
+      if (b.ev_comp[c]) cudaEventDestroy(b.ev_comp[c]);
+      if (b.ev_cnt[c]) cudaEventDestroy(b.ev_cnt[c]);
+    }
   }
+  if (hb.s_h2d) cudaStreamDestroy(hb.s_h2d);
+  if (hb.s_cnt) cudaStreamDestroy(hb.s_cnt);
+  if (hb.s_d2h) cudaStreamDestroy(hb.s_d2h);
   if (h->prof_ev) {
     for (size_t i = 0; i < PROF_RING; ++i)
       for (cudaEvent_t e : h->prof_ev[i])
@@ -729,41 +745,83 @@ lf_status lf_set_host_chunk_events(lf_handle* h, size_t min_events_per_chunk) {
   return LF_OK;
 }
 
-static lf_status run_host_pipeline(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
-                                   void* cuda_stream);
+static lf_status host_submit(lf_handle* h, int slot, const lf_seeds* seeds, const lf_hits* hits, size_t n_events,
+                             lf_tracks* out, void* cuda_stream, bool after_stream);
+static lf_status host_collect(lf_handle* h, int slot);
+
+/* an error in the middle of the pipeline: copies from / into the caller's host buffers may still be in flight on the
+ * library's streams; drain them (and the caller's stream) before handing the buffers back */
+static void host_drain(lf_handle* h, void* cuda_stream) {
+  HostBufs& hb = h->hb;
+  if (hb.s_h2d) cudaStreamSynchronize(hb.s_h2d);
+  if (hb.s_cnt) cudaStreamSynchronize(hb.s_cnt);
+  if (hb.s_d2h) cudaStreamSynchronize(hb.s_d2h);
+  cudaStreamSynchronize((cudaStream_t)cuda_stream);
+  for (HostSlot& b : hb.slot) b.pending = false;
+}
 
 lf_status lf_run_host(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
                       void* cuda_stream) {
   const lf_status st0 = check_run_args(h, seeds, hits, n_events, out);
   if (st0 != LF_OK) return st0;
   h->err.clear();
-  const lf_status rs = run_host_pipeline(h, seeds, hits, n_events, out, cuda_stream);
-  if (rs != LF_OK) {
-    /* an error in the middle of the pipeline: copies from / into the caller's host buffers may still be in flight on
-     * the library's streams; drain them (and the caller's stream) before handing the buffers back */
-    HostBufs& b = h->hb;
-    if (b.s_h2d) cudaStreamSynchronize(b.s_h2d);
-    if (b.s_cnt) cudaStreamSynchronize(b.s_cnt);
-    if (b.s_d2h) cudaStreamSynchronize(b.s_d2h);
-    cudaStreamSynchronize((cudaStream_t)cuda_stream);
-  }
+  for (const HostSlot& b : h->hb.slot)
+    if (b.pending) return fail(h, LF_ERR_INVALID_ARG, "lf_run_host: a batch submitted with lf_host_submit has not been collected");
+  lf_status rs = host_submit(h, 0, seeds, hits, n_events, out, cuda_stream, true);
+  if (rs == LF_OK) rs = host_collect(h, 0);
+  if (rs == LF_ERR_CUDA) host_drain(h, cuda_stream);
   return rs;
 }
 
-static lf_status run_host_pipeline(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
-                                   void* cuda_stream) {
+lf_status lf_host_submit(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, lf_tracks* out,
+                         void* cuda_stream, int slot) {
+  const lf_status st0 = check_run_args(h, seeds, hits, n_events, out);
+  if (st0 != LF_OK) return st0;
+  if (slot < 0 || slot >= LF_HOST_SLOTS) return fail(h, LF_ERR_INVALID_ARG, "lf_host_submit: slot out of range");
+  if (h->hb.slot[slot].pending) return fail(h, LF_ERR_INVALID_ARG, "lf_host_submit: the slot holds a batch that has not been collected");
+  h->err.clear();
+  const lf_status rs = host_submit(h, slot, seeds, hits, n_events, out, cuda_stream, false);
+  if (rs == LF_ERR_CUDA) host_drain(h, cuda_stream); /* failed half-way: nothing stays in flight (argument errors enqueue nothing) */
+  return rs;
+}
+
+lf_status lf_host_collect(lf_handle* h, int slot) {
+  if (!h) return LF_ERR_INVALID_ARG;
+  if (slot < 0 || slot >= LF_HOST_SLOTS) return fail(h, LF_ERR_INVALID_ARG, "lf_host_collect: slot out of range");
+  if (!h->hb.slot[slot].pending) return fail(h, LF_ERR_INVALID_ARG, "lf_host_collect: no batch was submitted to the slot");
+  h->err.clear();
+  const lf_status rs = host_collect(h, slot);
+  if (rs != LF_OK) host_drain(h, nullptr);
+  return rs;
+}
+
+/* First half of the host path: everything that needs no answer from the device.  Enqueues the host -> device copies of
+ * the whole batch (library stream), the kernels of every chunk (caller's stream, each chunk behind its copy) and the small
+ * copies that bring every chunk's track count back (library stream); returns without waiting. */
+static lf_status host_submit(lf_handle* h, int slot, const lf_seeds* seeds, const lf_hits* hits, size_t n_events,
+                             lf_tracks* out, void* cuda_stream, bool after_stream) {
   const uint32_t* so = seeds->event_offsets; /* HOST tables: the chunking reads them */
   const uint32_t* go = hits->seg_offsets;
   if (so[0] != 0 || go[0] != 0 || so[n_events] != seeds->n_seeds || go[n_events * lf::NSEG] != hits->n_hits)
     return fail(h, LF_ERR_INVALID_ARG, "lf_run_host: offset tables do not match n_seeds / n_hits");
-  if (n_events == 0) {
-    out->event_offsets[0] = 0;
-    *out->n_tracks = 0;
-    return LF_OK;
-  }
+  HostBufs& hb = h->hb;
+  HostSlot& b = hb.slot[slot];
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  HostBufs& b = h->hb;
+  for (const HostSlot& o : hb.slot) /* the batches in flight share the workspace: their kernels must run one after the other */
+    if (o.pending && o.st != st)
+      return fail(h, LF_ERR_INVALID_ARG, "lf_host_submit: batches in flight on one handle must use the same cuda_stream");
+  b.out = *out;
+  b.n_events = n_events;
+  b.n_chunks = 0;
+  b.st = st;
+  b.pending = true;
+  if (n_events == 0) return LF_OK;
   const bool packed = h->P.hit_storage == 1 && hits->x16 && hits->origin16; /* the caller ships the fp16 copy */
+  if (!hb.s_h2d) {
+    LF_CUDA(h, cudaStreamCreateWithFlags(&hb.s_h2d, cudaStreamNonBlocking));
+    LF_CUDA(h, cudaStreamCreateWithFlags(&hb.s_cnt, cudaStreamNonBlocking));
+    LF_CUDA(h, cudaStreamCreateWithFlags(&hb.s_d2h, cudaStreamNonBlocking));
+  }
   if (!b.ready) {
     const size_t ns = std::max<size_t>(h->max_seeds, 1), ne = std::max<size_t>(h->max_events, 1);
     const size_t nh = std::max<size_t>(h->max_hits, 1);
@@ -783,10 +841,8 @@ static lf_status run_host_pipeline(lf_handle* h, const lf_seeds* seeds, const lf
     LF_CUDA(h, cudaMalloc(&b.ev_off, (ne + HOST_MAX_CHUNKS + 1) * sizeof(uint32_t)));
     LF_CUDA(h, cudaMalloc(&b.n_tracks, HOST_MAX_CHUNKS * sizeof(uint32_t)));
     LF_CUDA(h, cudaMallocHost(&b.pinned_count, (ne + 2 * HOST_MAX_CHUNKS + 1) * sizeof(uint32_t)));
-    LF_CUDA(h, cudaStreamCreateWithFlags(&b.s_h2d, cudaStreamNonBlocking));
-    LF_CUDA(h, cudaStreamCreateWithFlags(&b.s_cnt, cudaStreamNonBlocking));
-    LF_CUDA(h, cudaStreamCreateWithFlags(&b.s_d2h, cudaStreamNonBlocking));
     LF_CUDA(h, cudaEventCreateWithFlags(&b.ev_start, cudaEventDisableTiming));
+    LF_CUDA(h, cudaEventCreateWithFlags(&b.ev_done, cudaEventDisableTiming));
     for (int c = 0; c < HOST_MAX_CHUNKS; ++c) {
       LF_CUDA(h, cudaEventCreateWithFlags(&b.ev_h2d[c], cudaEventDisableTiming));
       LF_CUDA(h, cudaEventCreateWithFlags(&b.ev_comp[c], cudaEventDisableTiming));
@@ -799,7 +855,7 @@ static lf_status run_host_pipeline(lf_handle* h, const lf_seeds* seeds, const lf
    * arrived (kernels + device->host copy of the LAST chunk) is pure latency: equal chunks of at least
    * host_chunk_events events, the last of them cut into four pieces of 40 / 27 / 18 / 15 % so that this tail is short
    * while every piece's kernels still hide behind the next piece's copy. */
-  size_t bounds[HOST_MAX_CHUNKS + 1];
+  size_t* bounds = b.bounds;
   int n_chunks = 0;
   {
     const int base = (int)std::min<size_t>(HOST_MAX_CHUNKS - 3, std::max<size_t>(1, n_events / h->host_chunk_events));
@@ -812,38 +868,43 @@ static lf_status run_host_pipeline(lf_handle* h, const lf_seeds* seeds, const lf
     }
     bounds[n_chunks] = n_events;
   }
+  b.n_chunks = n_chunks;
+  for (int c = 0; c <= n_chunks; ++c) b.first_seed[c] = so[bounds[c]];
   auto chunk_begin = [&](int c) { return bounds[c]; };
-  uint32_t* pin_cnt = b.pinned_count;
-  uint32_t* pin_off = b.pinned_count + HOST_MAX_CHUNKS; /* chunk c's n+1 relative offsets start at e0 + c */
 
-  /* the copy streams start after whatever the caller queued on `cuda_stream` before this call */
-  LF_CUDA(h, cudaEventRecord(b.ev_start, st));
-  LF_CUDA(h, cudaStreamWaitEvent(b.s_h2d, b.ev_start, 0));
-  LF_CUDA(h, cudaStreamWaitEvent(b.s_cnt, b.ev_start, 0));
-  LF_CUDA(h, cudaStreamWaitEvent(b.s_d2h, b.ev_start, 0));
+  /* lf_run_host: the copy streams start after whatever the caller queued on `cuda_stream` before this call.
+   * lf_host_submit: they start at once, so that this batch's copies run under the previous batch's kernels. */
+  if (after_stream) {
+    LF_CUDA(h, cudaEventRecord(b.ev_start, st));
+    LF_CUDA(h, cudaStreamWaitEvent(hb.s_h2d, b.ev_start, 0));
+    LF_CUDA(h, cudaStreamWaitEvent(hb.s_cnt, b.ev_start, 0));
+    LF_CUDA(h, cudaStreamWaitEvent(hb.s_d2h, b.ev_start, 0));
+  }
 
   /* ---- host -> device: the offset tables once, then seeds and hits chunk by chunk */
-  LF_CUDA(h, cudaMemcpyAsync(b.seed_off, so, (n_events + 1) * sizeof(uint32_t), cudaMemcpyHostToDevice, b.s_h2d));
-  LF_CUDA(h, cudaMemcpyAsync(b.seg_off, go, (n_events * lf::NSEG + 1) * sizeof(uint32_t), cudaMemcpyHostToDevice, b.s_h2d));
+  LF_CUDA(h, cudaMemcpyAsync(b.seed_off, so, (n_events + 1) * sizeof(uint32_t), cudaMemcpyHostToDevice, hb.s_h2d));
+  LF_CUDA(h, cudaMemcpyAsync(b.seg_off, go, (n_events * lf::NSEG + 1) * sizeof(uint32_t), cudaMemcpyHostToDevice, hb.s_h2d));
   /* the seeds of the whole batch go first, in five copies (15 % of the input bytes): per-chunk seed copies would add
    * 5 x n_chunks small transfers, each with its fixed cost, to the stream that bounds the pipeline */
   const float* src[5] = {seeds->x, seeds->y, seeds->tx, seeds->ty, seeds->qop};
   for (int i = 0; i < 5 && seeds->n_seeds > 0; ++i)
     if (src[i]) /* qop may be NULL in the no-UT mode */
-      LF_CUDA(h, cudaMemcpyAsync(b.seeds + i * stride, src[i], seeds->n_seeds * sizeof(float), cudaMemcpyHostToDevice, b.s_h2d));
+      LF_CUDA(h, cudaMemcpyAsync(b.seeds + i * stride, src[i], seeds->n_seeds * sizeof(float), cudaMemcpyHostToDevice, hb.s_h2d));
   for (int c = 0; c < n_chunks; ++c) {
     const size_t e0 = chunk_begin(c), e1 = chunk_begin(c + 1);
     const size_t g0 = go[e0 * lf::NSEG], g1 = go[e1 * lf::NSEG];
     if (g1 > g0 && hits->x)
-      LF_CUDA(h, cudaMemcpyAsync(b.hits + g0, hits->x + g0, (g1 - g0) * sizeof(float), cudaMemcpyHostToDevice, b.s_h2d));
+      LF_CUDA(h, cudaMemcpyAsync(b.hits + g0, hits->x + g0, (g1 - g0) * sizeof(float), cudaMemcpyHostToDevice, hb.s_h2d));
     if (g1 > g0 && packed) { /* the packed copy of the chunk: its halves and the origin slots its segments own */
-      LF_CUDA(h, cudaMemcpyAsync(b.hits16 + g0, hits->x16 + g0, (g1 - g0) * sizeof(uint16_t), cudaMemcpyHostToDevice, b.s_h2d));
+      LF_CUDA(h, cudaMemcpyAsync(b.hits16 + g0, hits->x16 + g0, (g1 - g0) * sizeof(uint16_t), cudaMemcpyHostToDevice, hb.s_h2d));
       const size_t o0 = (g0 >> lf::H16_SHIFT) + e0 * lf::NSEG, o1 = (g1 >> lf::H16_SHIFT) + e1 * lf::NSEG + 1;
-      LF_CUDA(h, cudaMemcpyAsync(b.origin16 + o0, hits->origin16 + o0, (o1 - o0) * sizeof(float), cudaMemcpyHostToDevice, b.s_h2d));
+      LF_CUDA(h, cudaMemcpyAsync(b.origin16 + o0, hits->origin16 + o0, (o1 - o0) * sizeof(float), cudaMemcpyHostToDevice, hb.s_h2d));
     }
-    LF_CUDA(h, cudaEventRecord(b.ev_h2d[c], b.s_h2d));
+    LF_CUDA(h, cudaEventRecord(b.ev_h2d[c], hb.s_h2d));
   }
   /* ---- kernels on the caller's stream, chunk by chunk; the counts follow on their own stream */
+  uint32_t* pin_cnt = b.pinned_count;
+  uint32_t* pin_off = b.pinned_count + HOST_MAX_CHUNKS; /* chunk c's n+1 relative offsets start at e0 + c */
   for (int c = 0; c < n_chunks; ++c) {
     const size_t e0 = chunk_begin(c), e1 = chunk_begin(c + 1);
     const size_t s0 = so[e0], s1 = so[e1], g0 = go[e0 * lf::NSEG], g1 = go[e1 * lf::NSEG];
@@ -857,24 +918,41 @@ static lf_status run_host_pipeline(lf_handle* h, const lf_seeds* seeds, const lf
     const lf_status rs = launch<false>(h, &ds, &dh, e1 - e0, &dt, nullptr, st, e0);
     if (rs != LF_OK) return rs;
     LF_CUDA(h, cudaEventRecord(b.ev_comp[c], st));
-    LF_CUDA(h, cudaStreamWaitEvent(b.s_cnt, b.ev_comp[c], 0));
-    LF_CUDA(h, cudaMemcpyAsync(pin_cnt + c, b.n_tracks + c, sizeof(uint32_t), cudaMemcpyDeviceToHost, b.s_cnt));
-    LF_CUDA(h, cudaMemcpyAsync(pin_off + e0 + c, b.ev_off + e0 + c, (e1 - e0) * sizeof(uint32_t), cudaMemcpyDeviceToHost, b.s_cnt));
-    LF_CUDA(h, cudaEventRecord(b.ev_cnt[c], b.s_cnt));
+    LF_CUDA(h, cudaStreamWaitEvent(hb.s_cnt, b.ev_comp[c], 0));
+    LF_CUDA(h, cudaMemcpyAsync(pin_cnt + c, b.n_tracks + c, sizeof(uint32_t), cudaMemcpyDeviceToHost, hb.s_cnt));
+    LF_CUDA(h, cudaMemcpyAsync(pin_off + e0 + c, b.ev_off + e0 + c, (e1 - e0) * sizeof(uint32_t), cudaMemcpyDeviceToHost, hb.s_cnt));
+    LF_CUDA(h, cudaEventRecord(b.ev_cnt[c], hb.s_cnt));
   }
-  /* ---- device -> host: as soon as a chunk's count is known its tracks go to their final dense position */
+  return LF_OK;
+}
+
+/* Second half: as soon as a chunk's count is known its tracks go to their final dense position in the caller's arrays;
+ * returns when the batch's last byte has arrived.  Does not wait for anything queued behind the batch. */
+static lf_status host_collect(lf_handle* h, int slot) {
+  HostBufs& hb = h->hb;
+  HostSlot& b = hb.slot[slot];
+  lf_tracks* out = &b.out;
+  const size_t n_events = b.n_events;
+  b.pending = false;
+  if (n_events == 0) {
+    out->event_offsets[0] = 0;
+    *out->n_tracks = 0;
+    return LF_OK;
+  }
+  uint32_t* pin_cnt = b.pinned_count;
+  uint32_t* pin_off = b.pinned_count + HOST_MAX_CHUNKS;
   size_t running = 0;
-  for (int c = 0; c < n_chunks; ++c) {
-    const size_t e0 = chunk_begin(c), e1 = chunk_begin(c + 1);
-    const size_t s0 = so[e0];
+  for (int c = 0; c < b.n_chunks; ++c) {
+    const size_t e0 = b.bounds[c], e1 = b.bounds[c + 1];
+    const size_t s0 = b.first_seed[c];
     LF_CUDA(h, cudaEventSynchronize(b.ev_cnt[c]));
     const size_t nt = pin_cnt[c];
     if (nt > 0) {
-      LF_CUDA(h, cudaMemcpyAsync(out->hit_idx + running * lf::NL, b.hit_idx + s0 * lf::NL, nt * lf::NL * sizeof(int32_t), cudaMemcpyDeviceToHost, b.s_d2h));
-      LF_CUDA(h, cudaMemcpyAsync(out->seed_idx + running, b.seed_idx + s0, nt * sizeof(int32_t), cudaMemcpyDeviceToHost, b.s_d2h));
-      LF_CUDA(h, cudaMemcpyAsync(out->n_hits + running, b.n_hits + s0, nt * sizeof(int32_t), cudaMemcpyDeviceToHost, b.s_d2h));
-      LF_CUDA(h, cudaMemcpyAsync(out->state + running * 5, b.state + s0 * 5, nt * 5 * sizeof(float), cudaMemcpyDeviceToHost, b.s_d2h));
-      LF_CUDA(h, cudaMemcpyAsync(out->quality + running, b.quality + s0, nt * sizeof(float), cudaMemcpyDeviceToHost, b.s_d2h));
+      LF_CUDA(h, cudaMemcpyAsync(out->hit_idx + running * lf::NL, b.hit_idx + s0 * lf::NL, nt * lf::NL * sizeof(int32_t), cudaMemcpyDeviceToHost, hb.s_d2h));
+      LF_CUDA(h, cudaMemcpyAsync(out->seed_idx + running, b.seed_idx + s0, nt * sizeof(int32_t), cudaMemcpyDeviceToHost, hb.s_d2h));
+      LF_CUDA(h, cudaMemcpyAsync(out->n_hits + running, b.n_hits + s0, nt * sizeof(int32_t), cudaMemcpyDeviceToHost, hb.s_d2h));
+      LF_CUDA(h, cudaMemcpyAsync(out->state + running * 5, b.state + s0 * 5, nt * 5 * sizeof(float), cudaMemcpyDeviceToHost, hb.s_d2h));
+      LF_CUDA(h, cudaMemcpyAsync(out->quality + running, b.quality + s0, nt * sizeof(float), cudaMemcpyDeviceToHost, hb.s_d2h));
     }
     const uint32_t* rel = pin_off + e0 + c;
     for (size_t e = e0; e < e1; ++e) out->event_offsets[e] = (uint32_t)(running + rel[e - e0]);
@@ -882,8 +960,10 @@ static lf_status run_host_pipeline(lf_handle* h, const lf_seeds* seeds, const lf
   }
   out->event_offsets[n_events] = (uint32_t)running;
   *out->n_tracks = (uint32_t)running;
-  LF_CUDA(h, cudaStreamSynchronize(b.s_d2h));
-  LF_CUDA(h, cudaStreamSynchronize(st));
+  /* the batch's kernels are done (its last count has arrived); wait for its last copy, not for the streams, which may
+   * already hold the next batch */
+  LF_CUDA(h, cudaEventRecord(b.ev_done, hb.s_d2h));
+  LF_CUDA(h, cudaEventSynchronize(b.ev_done));
   return LF_OK;
 }
 

@@ -1723,7 +1723,7 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_extend_kernel(const __grid_
     T.geo[3 * NL + threadIdx.x] = C.tana[threadIdx.x];
   }
   uint32_t phase = 0;
-  EventCtx E;
+  EventCtx E = {};
   /* while the event's hits are on their way: pull its per-row tables (window rows, triplet counts and codes, seed
    * parameters; written by the earlier kernels, so in DRAM by now) into L2 */
   auto prefetch_tables = [&]() {
@@ -2095,7 +2095,7 @@ __global__ void __launch_bounds__(FIT_THREADS, 4) lf_fit_kernel(const __grid_con
   if (tid < TM_WORDS) T.misc[tid] = 0u; /* published by fetch_event's barriers */
   /* Resolves the event in the TM_OLD_* words: look-back by warp 1, which neither issues nor polls the bulk copy.  Called
    * inside fetch_event (the words it reads were written before fetch_event's first barrier). */
-  EventCtx E;
+  EventCtx E = {};
   auto resolve = [&](bool taken = true) {
     if (taken && threadIdx.x >= 64) {
       /* the other warps, while the event's hits are on their way: its records, window rows and seed parameters -> L2 */

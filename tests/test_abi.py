@@ -34,7 +34,7 @@ def test_struct_sizes_match_binding(lib):
     from paper_2402_14670_b200 import binding
     for i, st in enumerate(binding._STRUCTS):
         assert lib.lf_sizeof(i) == ctypes.sizeof(st)
-    assert lib.lf_sizeof(99) == 0 and lib.lf_abi_version() == 6
+    assert lib.lf_sizeof(99) == 0 and lib.lf_abi_version() == 7
 
 
 def test_argument_validation_needs_no_gpu(lib, geometry, params):

@@ -616,3 +616,48 @@ def test_stream_compaction_lookback_stress(lfmod, oracle, geometry, params):
     lf.run_host(lfmod.HostBatch(tiny), ht)
     assert_tracks_equal(ht.to_numpy(), ref, "tiny events through lf_run_host")
     lf.close()
+
+
+def test_host_submit_collect_pipeline(lfmod, oracle, geometry, params):
+    """lf_host_submit / lf_host_collect (include/lf.h): a stream of different batches, two in flight, gives for every batch
+    exactly what lf_run_host gives (= the oracle's tracks); misuse is refused before anything is enqueued."""
+    import torch
+    whole = dg.generate_config(1, n_events=900)
+    cuts = [0, 260, 300, 610, 611, 900]  # batches of different sizes, one of them a single event
+    batches = [whole.slice_events(a, b) for a, b in zip(cuts[:-1], cuts[1:])] + [dg.generate(dg.GenConfig("e", 0, 1))]
+    refs = [oracle.run(geometry, params, b, threads=NTHREADS) for b in batches]
+    lf = lfmod.LookingForward(geometry, params, max(b.n_events for b in batches), max(b.n_seeds for b in batches),
+                              max(b.n_hits for b in batches))
+    lf.set_host_chunk_events(64)
+    hbs = [lfmod.HostBatch(b) for b in batches]
+    hts = [lfmod.HostTracks(max(b.n_seeds, 1), b.n_events) for b in batches]
+    st = torch.cuda.Stream()
+    for rep in range(2):
+        for t in hts:
+            t.hit_idx.fill_(-7)
+            t.n_tracks.zero_()
+        lf.host_submit(hbs[0], hts[0], 0, st)
+        for i in range(1, len(batches)):
+            lf.host_submit(hbs[i], hts[i], i % 2, st)
+            lf.host_collect((i - 1) % 2)
+            assert_tracks_equal(hts[i - 1].to_numpy(), refs[i - 1], f"pipelined batch {i - 1}")
+        lf.host_collect((len(batches) - 1) % 2)
+        assert_tracks_equal(hts[-1].to_numpy(), refs[-1], "pipelined last batch")
+    # the one-call path still works afterwards and agrees
+    lf.run_host(hbs[2], hts[2], st)
+    assert_tracks_equal(hts[2].to_numpy(), refs[2], "lf_run_host after the pipeline")
+    # misuse
+    lf.host_submit(hbs[0], hts[0], 0, st)
+    with pytest.raises(lfmod.LfError):
+        lf.host_submit(hbs[1], hts[1], 0, st)                      # slot not collected
+    with pytest.raises(lfmod.LfError):
+        lf.host_submit(hbs[1], hts[1], 1, torch.cuda.Stream())     # another stream while a batch is in flight
+    with pytest.raises(lfmod.LfError):
+        lf.run_host(hbs[1], hts[1], st)                            # one-call path while a batch is in flight
+    with pytest.raises(lfmod.LfError):
+        lf.host_collect(1)                                         # nothing submitted there
+    with pytest.raises(lfmod.LfError):
+        lf.host_submit(hbs[1], hts[1], 2, st)                      # no such slot
+    lf.host_collect(0)
+    assert_tracks_equal(hts[0].to_numpy(), refs[0], "batch collected after refused calls")
+    lf.close()
