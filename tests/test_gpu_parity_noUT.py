@@ -167,6 +167,30 @@ def test_noUT_run_host_and_determinism(lfmod, oracle, geometry, nparams):
     assert np.array_equal(a.quality.view(np.uint32), c.quality.view(np.uint32))
 
 
+def test_noUT_stream_of_batches(lfmod, oracle, geometry, nparams):
+    """lf_host_submit / lf_host_collect in the no-UT tuning (two rows per seed, seeds without q/p): a stream of unequal
+    batches, two in flight, against the oracle."""
+    import torch
+    whole = dg.generate_config(1, n_events=240)
+    cuts = [0, 100, 101, 170, 240]
+    batches = [whole.slice_events(a, b) for a, b in zip(cuts[:-1], cuts[1:])]
+    refs = [oracle.run(geometry, nparams, b, threads=NTHREADS) for b in batches]
+    lf = lfmod.LookingForward(geometry, nparams, max(b.n_events for b in batches), max(b.n_seeds for b in batches),
+                              max(b.n_hits for b in batches))
+    lf.set_host_chunk_events(16)
+    hbs = [lfmod.HostBatch(b) for b in batches]
+    hts = [lfmod.HostTracks(b.n_seeds, b.n_events) for b in batches]
+    st = torch.cuda.Stream()
+    lf.host_submit(hbs[0], hts[0], 0, st)
+    for i in range(1, len(batches)):
+        lf.host_submit(hbs[i], hts[i], i % 2, st)
+        lf.host_collect((i - 1) % 2)
+        assert_tracks_equal(hts[i - 1].to_numpy(), refs[i - 1], f"no-UT stream, batch {i - 1}")
+    lf.host_collect((len(batches) - 1) % 2)
+    assert_tracks_equal(hts[-1].to_numpy(), refs[-1], "no-UT stream, last batch")
+    lf.close()
+
+
 def test_full_eq9_table_both_tunings(lfmod, oracle, geometry, params, nparams):
     """geometry.qop_mode = 1: q/p from the 2-D polynomial table, in a non-uniform toy field,
     narrow kernels (with UT) and wide kernels (no-UT); also the mirrored event (negated stereo angles, polarity)."""
