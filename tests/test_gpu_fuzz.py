@@ -2,7 +2,8 @@
 
 Seeded draws of the tunables (window cap 2..64, triplet cap 1..32, hit-count rule, tolerances, window overlap incl. a
 negative one, polarity, dRatio, Eq. 9 table on/off) on small dense and sparse batches.  Everything must equal the oracle:
-windows, kept triplets, extension hit lists, candidate Q, tracks."""
+windows, kept triplets, extension hit lists, candidate Q, tracks; every third set also through the release build of the
+kernels, every fifth through the host path as a stream of two batches."""
 import os
 
 import numpy as np
@@ -76,13 +77,26 @@ def test_random_parameter_sets(lfmod, oracle, geometry):
         torch.cuda.synchronize()
         got = out.to_numpy()
         got.debug = {k: v.cpu().numpy() for k, v in vars(out.debug_tensors).items()}
-        lf.close()
         what = f"fuzz {it}: mode {P['mode']}, n_window {P['n_window']}, n_triplets {P['n_triplets']}, min_hits {P['min_hits']}"
         try:
             assert_debug_equal(got.debug, ref.debug)
             assert_tracks_equal(got, ref, what)
+            if it % 3 == 0:  # the release build of the kernels
+                out2 = lf.run(lfmod.DeviceBatch(b))
+                torch.cuda.synchronize()
+                assert_tracks_equal(out2.to_numpy(), ref, what + " (release kernels)")
+            if it % 5 == 0:  # the host path as a stream: the same batch in both slots, small chunks
+                lf.set_host_chunk_events(int(rng.integers(1, 9)))
+                hb = lfmod.HostBatch(b)
+                hts = [lfmod.HostTracks(max(b.n_seeds, 1), b.n_events) for _ in range(2)]
+                lf.host_submit(hb, hts[0], 0)
+                lf.host_submit(hb, hts[1], 1)
+                for slot in range(2):
+                    lf.host_collect(slot)
+                    assert_tracks_equal(hts[slot].to_numpy(), ref, what + f" (stream, slot {slot})")
         except AssertionError as e:
             raise AssertionError(f"{what}: {e}\nparams: {P}") from e
+        lf.close()
         n_wide += int(P["mode"] == 1 or P["n_window"] > 32 or P["n_triplets"] > 16)
         n_tracks += ref.n_tracks
     assert 20 <= n_wide <= 58 and n_tracks > 3000
