@@ -572,6 +572,17 @@ lf_status lf_create(const lf_geometry* geometry, const lf_params* params, size_t
 
 lf_status lf_destroy(lf_handle* h) {
   if (!h) return LF_OK;
+  { /* a batch still in flight through the host path: let its copies and kernels finish before their memory goes */
+    bool in_flight = false;
+    for (const HostSlot& b : h->hb.slot) in_flight = in_flight || b.pending;
+    if (in_flight) {
+      for (const HostSlot& b : h->hb.slot)
+        if (b.pending) cudaStreamSynchronize(b.st);
+      if (h->hb.s_h2d) cudaStreamSynchronize(h->hb.s_h2d);
+      if (h->hb.s_cnt) cudaStreamSynchronize(h->hb.s_cnt);
+      if (h->hb.s_d2h) cudaStreamSynchronize(h->hb.s_d2h);
+    }
+  }
   cudaFree(h->hx16); cudaFree(h->origin16); cudaFree(h->hx_scratch);
   cudaFree(h->win); cudaFree(h->trip_code); cudaFree(h->n_trip);
   cudaFree(h->ws_rec); cudaFree(h->ws_nh); cudaFree(h->ws_rank);
@@ -677,6 +688,8 @@ lf_status lf_run(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_
                  void* cuda_stream) {
   const lf_status st = check_run_args(h, seeds, hits, n_events, out);
   if (st != LF_OK) return st;
+  for (const HostSlot& b : h->hb.slot) /* the workspace is in use */
+    if (b.pending) return fail(h, LF_ERR_INVALID_ARG, "lf_run: a batch submitted with lf_host_submit has not been collected");
   h->err.clear();
   return launch<false>(h, seeds, hits, n_events, out, nullptr, (cudaStream_t)cuda_stream);
 }
@@ -686,6 +699,8 @@ lf_status lf_run_debug(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits,
   const lf_status st = check_run_args(h, seeds, hits, n_events, out);
   if (st != LF_OK) return st;
   if (!debug) return fail(h, LF_ERR_INVALID_ARG, "lf_run_debug: NULL debug");
+  for (const HostSlot& b : h->hb.slot)
+    if (b.pending) return fail(h, LF_ERR_INVALID_ARG, "lf_run_debug: a batch submitted with lf_host_submit has not been collected");
   h->err.clear();
   return launch<true>(h, seeds, hits, n_events, out, debug, (cudaStream_t)cuda_stream);
 }

@@ -655,9 +655,13 @@ def test_host_submit_collect_pipeline(lfmod, oracle, geometry, params):
     with pytest.raises(lfmod.LfError):
         lf.run_host(hbs[1], hts[1], st)                            # one-call path while a batch is in flight
     with pytest.raises(lfmod.LfError):
+        lf.run(lfmod.DeviceBatch(batches[1]))                      # device path while a batch is in flight
+    with pytest.raises(lfmod.LfError):
         lf.host_collect(1)                                         # nothing submitted there
     with pytest.raises(lfmod.LfError):
         lf.host_submit(hbs[1], hts[1], 2, st)                      # no such slot
     lf.host_collect(0)
     assert_tracks_equal(hts[0].to_numpy(), refs[0], "batch collected after refused calls")
-    lf.close()
+    lf.host_submit(hbs[0], hts[0], 1, st)
+    lf.close()  # lf_destroy with a batch in flight waits for it
+    torch.cuda.synchronize()
