@@ -293,6 +293,48 @@ lf_status lf_kernel_times(lf_handle* h, float ms[LF_N_KERNELS]);
 #define LF_N_COUNTERS 8
 lf_status lf_run_counters(lf_handle* h, uint64_t counters[LF_N_COUNTERS]);
 
+/* Search windows (a1 + a2, no-UT: Eq. 7/8) without any allocation and without a handle.
+ *
+ * Who this is for.  Everything else in this header goes through lf_create, which calls cudaMalloc.  Some hosts cannot
+ * afford or are not allowed that call: a trigger application whose framework grabs the whole GPU at start-up and hands
+ * out slices itself (a later cudaMalloc then simply fails for lack of memory), an event loop with a latency budget
+ * (cudaMalloc and cudaFree stall the whole device and take unbounded time), a plug-in that lives inside somebody else's
+ * memory pool, or code that runs where the CUDA allocator must not be entered at all.  Such a caller can still ask this
+ * one function which hits each seed would look at: it brings its own input and output buffers, and the kernel's scratch
+ * memory is a fixed array compiled into the library (`static __device__`, LF_STATIC_SCRATCH_BYTES = 1 097 984 bytes).
+ * The price: every GPU whose context loads this library holds that array from load time until the process exits, whether
+ * or not this function is ever called, and the batch size is bounded:
+ *     n_events <= LF_STATIC_MAX_EVENTS, followed tracks = seeds->n_seeds * (params->mode == 1 ? 2 : 1) <= LF_STATIC_MAX_ROWS;
+ * anything larger is refused with LF_ERR_CAPACITY (split the batch, or use lf_create + lf_run_debug).
+ *
+ * Arguments: `geometry`, `params` HOST structs as for lf_create (validated the same way; params->hit_storage must be 0,
+ * LF_ERR_UNSUPPORTED otherwise); `seeds`, `hits` HOST structs holding DEVICE pointers as for lf_run; `win_first`,
+ * `win_count` DEVICE arrays of (followed tracks) * 12 int32, caller-owned, with the meaning and row order of
+ * lf_debug.win_first / win_count (global index of the window's first hit -- undefined where the count is 0 -- and the
+ * number of hits, <= params->n_window).  The result is what lf_run_debug writes into those two tables, bit for bit.
+ * Asynchronous on `cuda_stream` (one 4-byte memset + one kernel); results are valid once the stream has been synchronised.
+ * The function calls no cudaMalloc, cudaMallocAsync, cudaFree or other routine that allocates device memory.
+ *
+ * First call on a device: looks up, once per device and with that device current, where the array lives there
+ * (cudaGetSymbolAddress), reads two device attributes and makes sure the window kernel may use the 33 KB of shared
+ * memory it is launched with (a function attribute; an lf_create for small events may have set it lower).  The lookup can
+ * make the CUDA runtime load the library's code onto the device, so make the first call per device early, during
+ * set-up, and before any stream capture begins.
+ *
+ * Sharing: all calls on a device use the same array, and the array keeps whatever the previous call left in it.  The
+ * function clears the one word that has to start at zero (the event counter its thread blocks draw from) at the head of
+ * its own work on `cuda_stream`; everything else is overwritten before it is read.  Two calls whose GPU work overlaps in
+ * time (different streams, or different host threads on different streams) race on the array and give garbage: keep
+ * calls on one device in stream order, or order them with events.  lf_create handles do not touch the array.
+ * Errors: status code; the message is lf_last_error(NULL) in the calling thread.  Size and argument errors are found
+ * before the first CUDA call. */
+#define LF_STATIC_MAX_EVENTS 4096
+#define LF_STATIC_MAX_ROWS 16384
+#define LF_STATIC_SCRATCH_BYTES (LF_STATIC_MAX_ROWS * 64 + LF_STATIC_MAX_EVENTS * 12 + 256)
+lf_status lf_windows_static(const lf_geometry* geometry, const lf_params* params, const lf_seeds* seeds,
+                            const lf_hits* hits, size_t n_events, int32_t* win_first, int32_t* win_count,
+                            void* cuda_stream);
+
 /* ABI self-description for bindings: version and struct sizes
  * (which: 0 geometry, 1 params, 2 seeds, 3 hits, 4 tracks, 5 debug, 6 info). */
 uint32_t lf_abi_version(void);

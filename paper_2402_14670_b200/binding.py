@@ -136,6 +136,9 @@ def load_library() -> C.CDLL:
     lib.lf_set_profiling.argtypes = [C.c_void_p, C.c_int]
     lib.lf_kernel_times.restype = C.c_int
     lib.lf_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_float * len(KERNEL_NAMES))]
+    lib.lf_windows_static.restype = C.c_int
+    lib.lf_windows_static.argtypes = [C.POINTER(lf_geometry), C.POINTER(lf_params), C.POINTER(lf_seeds), C.POINTER(lf_hits),
+                                      C.c_size_t, C.c_void_p, C.c_void_p, C.c_void_p]
     if lib.lf_abi_version() != 7:
         raise ImportError("liblf_b200.so: ABI version mismatch")
     for i, st in enumerate(_STRUCTS):
@@ -155,6 +158,33 @@ def _fill(struct, values: Dict[str, object]):
         else:
             setattr(struct, name, v)
     return struct
+
+
+STATIC_MAX_EVENTS, STATIC_MAX_ROWS = 4096, 16384  # LF_STATIC_MAX_EVENTS / LF_STATIC_MAX_ROWS of include/lf.h
+
+
+def windows_static(geometry: Dict[str, object], params: Dict[str, object], db: "DeviceBatch", win_first, win_count,
+                   stream=None) -> None:
+    """``lf_windows_static``: the search windows of every seed of ``db``, written into the caller's two int32 CUDA
+    tensors of shape (followed tracks, 12), with no handle and no device allocation anywhere in the call.
+
+    This is the entry point for hosts that cannot call ``cudaMalloc`` once they are running (a framework that owns all of
+    the GPU's memory, a latency-bound event loop): the kernel's scratch is a fixed array inside the library, so batches
+    are limited to ``STATIC_MAX_EVENTS`` events and ``STATIC_MAX_ROWS`` followed tracks (``LfError`` with
+    LF_ERR_CAPACITY beyond that), calls on one device must not overlap on the GPU, and the first call per device should
+    be made during set-up.  The binding allocates nothing either: both outputs are the caller's.  Asynchronous on
+    ``stream`` (default: torch's current stream)."""
+    lib = load_library()
+    g = _fill(lf_geometry(), geometry)
+    p = _fill(lf_params(), params)
+    seeds = lf_seeds(db.seed_x.data_ptr(), db.seed_y.data_ptr(), db.seed_tx.data_ptr(), db.seed_ty.data_ptr(),
+                     db.seed_qop.data_ptr(), db.seed_offsets.data_ptr(), db.n_seeds)
+    hits = db.c_hits()
+    st = lib.lf_windows_static(C.byref(g), C.byref(p), C.byref(seeds), C.byref(hits), db.n_events,
+                               win_first.data_ptr() if win_first is not None else None,
+                               win_count.data_ptr() if win_count is not None else None, LookingForward._stream_ptr(stream))
+    if st != LF_OK:
+        raise LfError(st, lib.lf_last_error(None).decode())
 
 
 class DeviceBatch:

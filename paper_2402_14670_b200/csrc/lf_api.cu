@@ -983,3 +983,122 @@ static lf_status host_collect(lf_handle* h, int slot) {
 }
 
 } /* extern "C" */
+
+/* ============================================================================================
+ * lf_windows_static (include/lf.h): the search-window stage (a1 + a2) for callers that cannot allocate.
+ *
+ * The window kernel needs global memory besides the caller's inputs and outputs: its 64-byte window rows, the events'
+ * equal-neighbour flags and look-back words, and the event ticket its persistent CTAs draw from.  lf_run takes that from
+ * the workspace lf_create allocated.  Here it lives in the array below, which is part of the library's image: the driver
+ * reserves it on every GPU that loads the library and keeps it until the process exits, so this entry point never
+ * calls cudaMalloc / cudaFree (nor anything else that allocates device memory) and needs no handle.
+ *
+ * `lf_static_scratch` as written in HOST code is only the host-side shadow of the symbol, not an address the GPU can
+ * use: the device address comes from cudaGetSymbolAddress, asked once per device with that device current (below).
+ * ============================================================================================ */
+namespace {
+constexpr size_t STATIC_WIN_BYTES = (size_t)LF_STATIC_MAX_ROWS * lf::WIN_ROW * sizeof(uint32_t);  /* window rows */
+constexpr size_t STATIC_STATE_BYTES = (size_t)LF_STATIC_MAX_EVENTS * sizeof(unsigned long long);  /* look-back words */
+constexpr size_t STATIC_DUP_BYTES = (size_t)LF_STATIC_MAX_EVENTS * sizeof(uint32_t);              /* equal-neighbour flags */
+constexpr size_t STATIC_TICKET_BYTES = 256;                                                        /* the event ticket */
+constexpr size_t STATIC_SCRATCH_BYTES = STATIC_WIN_BYTES + STATIC_STATE_BYTES + STATIC_DUP_BYTES + STATIC_TICKET_BYTES;
+static_assert(STATIC_SCRATCH_BYTES == LF_STATIC_SCRATCH_BYTES, "include/lf.h states the size of the static scratch");
+constexpr int STATIC_STAGE_CAP = 8192; /* floats of shared memory for one event's hits: header + 32 KB stays under the 48 KB a
+                                          kernel may use without raising an attribute; larger events read global memory */
+struct StaticDevice {
+  unsigned char* scratch = nullptr; /* device address of lf_static_scratch on this device */
+  int sm_count = 0;
+  bool ready = false;
+};
+StaticDevice g_static_dev[MAX_DEVICES];
+std::mutex g_static_mutex;
+} // namespace
+
+static __device__ __align__(256) unsigned char lf_static_scratch[LF_STATIC_SCRATCH_BYTES];
+
+extern "C" lf_status lf_windows_static(const lf_geometry* geometry, const lf_params* params, const lf_seeds* seeds,
+                                       const lf_hits* hits, size_t n_events, int32_t* win_first, int32_t* win_count,
+                                       void* cuda_stream) {
+  /* ---- argument checks: all of them before the first CUDA call */
+  if (!geometry || !params || !seeds || !hits)
+    return fail(nullptr, LF_ERR_INVALID_ARG, "lf_windows_static: NULL geometry/params/seeds/hits");
+  if (const char* why = validate(*geometry, *params)) return fail(nullptr, LF_ERR_INVALID_ARG, std::string("lf_windows_static: ") + why);
+  if (params->hit_storage != 0)
+    return fail(nullptr, LF_ERR_UNSUPPORTED, "lf_windows_static: fp32 hits only (hit_storage = 1 needs a scratch image of the hits)");
+  const size_t sides = params->mode == 1 ? 2 : 1;
+  if (n_events > (size_t)LF_STATIC_MAX_EVENTS || seeds->n_seeds > (size_t)LF_STATIC_MAX_ROWS / sides) {
+    char msg[256];
+    std::snprintf(msg, sizeof(msg),
+                  "lf_windows_static: %zu events / %zu followed tracks exceed the static scratch (LF_STATIC_MAX_EVENTS = %d, "
+                  "LF_STATIC_MAX_ROWS = %d): split the batch, or use lf_create + lf_run_debug",
+                  n_events, seeds->n_seeds * sides, LF_STATIC_MAX_EVENTS, LF_STATIC_MAX_ROWS);
+    return fail(nullptr, LF_ERR_CAPACITY, msg);
+  }
+  if (hits->n_hits >= (size_t)0x7fffffff) return fail(nullptr, LF_ERR_CAPACITY, "lf_windows_static: hit indices must fit int32");
+  if (n_events == 0) {
+    if (seeds->n_seeds != 0 || hits->n_hits != 0)
+      return fail(nullptr, LF_ERR_INVALID_ARG, "lf_windows_static: n_events == 0 with non-empty seeds or hits");
+    return LF_OK; /* nothing to write */
+  }
+  if (!seeds->event_offsets || !hits->seg_offsets) return fail(nullptr, LF_ERR_INVALID_ARG, "lf_windows_static: NULL offset table");
+  if (seeds->n_seeds > 0 && (!seeds->x || !seeds->y || !seeds->tx || !seeds->ty || (!seeds->qop && params->mode == 0)))
+    return fail(nullptr, LF_ERR_INVALID_ARG, "lf_windows_static: NULL seed array");
+  if (hits->n_hits > 0 && !hits->x) return fail(nullptr, LF_ERR_INVALID_ARG, "lf_windows_static: NULL hit array");
+  if (seeds->n_seeds > 0 && (!win_first || !win_count)) return fail(nullptr, LF_ERR_INVALID_ARG, "lf_windows_static: NULL output array");
+
+  /* ---- once per device, with that device current: where the static array lives on it */
+  int device = 0;
+  LF_CUDA(nullptr, cudaGetDevice(&device));
+  if (device < 0 || device >= MAX_DEVICES) return fail(nullptr, LF_ERR_UNSUPPORTED, "lf_windows_static: device index beyond the library's table");
+  StaticDevice sd;
+  {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice& slot = g_static_dev[device];
+    if (!slot.ready) {
+      int major = 0;
+      LF_CUDA(nullptr, cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device));
+      if (major < 10) return fail(nullptr, LF_ERR_UNSUPPORTED, "lf_windows_static: this library is built for sm_100a (Blackwell) only");
+      LF_CUDA(nullptr, cudaDeviceGetAttribute(&slot.sm_count, cudaDevAttrMultiProcessorCount, device));
+      unsigned char* ptr = nullptr;
+      LF_CUDA(nullptr, cudaGetSymbolAddress((void**)&ptr, lf_static_scratch));
+      if (!ptr) return fail(nullptr, LF_ERR_CUDA, "lf_windows_static: cudaGetSymbolAddress returned no address");
+      /* The shared-memory limit of a kernel is a property of the kernel, and an lf_create with a small stage may have set
+       * it below what this entry point launches with: raise it through the library's raise-only table (no later
+       * lf_create can lower it again).  Sets a function attribute; allocates nothing. */
+      const int smem_bytes = lf::HDR_BYTES + STATIC_STAGE_CAP * (int)sizeof(float);
+      LF_CUDA(nullptr, raise_dynamic_smem((const void*)lf::lf_window_kernel<true, false>, 0, 0, 1, device, smem_bytes));
+      LF_CUDA(nullptr, raise_dynamic_smem((const void*)lf::lf_window_kernel<true, true>, 1, 0, 1, device, smem_bytes));
+      slot.scratch = ptr;
+      slot.ready = true;
+    }
+    sd = slot;
+  }
+
+  lf::Consts consts;
+  make_consts(*geometry, *params, consts);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  uint32_t* ticket = reinterpret_cast<uint32_t*>(sd.scratch + STATIC_WIN_BYTES + STATIC_STATE_BYTES + STATIC_DUP_BYTES);
+  lf::EventArgs A;
+  std::memset(&A, 0, sizeof(A));
+  A.sx = seeds->x; A.sy = seeds->y; A.stx = seeds->tx; A.sty = seeds->ty; A.sqop = seeds->qop;
+  A.seed_off = seeds->event_offsets;
+  A.hx = hits->x; A.seg_off = hits->seg_offsets;
+  A.n_events = (uint32_t)n_events;
+  A.stage_cap = STATIC_STAGE_CAP;
+  A.stage_cap_x = STATIC_STAGE_CAP;
+  A.win = reinterpret_cast<uint32_t*>(sd.scratch);
+  A.ev_state = reinterpret_cast<unsigned long long*>(sd.scratch + STATIC_WIN_BYTES);
+  A.ev_dup = reinterpret_cast<uint32_t*>(sd.scratch + STATIC_WIN_BYTES + STATIC_STATE_BYTES);
+  A.ticket = ticket;
+  A.dbg.win_first = win_first;
+  A.dbg.win_count = win_count;
+  /* The array keeps what the previous call left.  Only the ticket must start at zero (the CTAs count events up from
+   * it); window rows, flags and look-back words are written by the kernel before anybody reads them. */
+  LF_CUDA(nullptr, cudaMemsetAsync(ticket, 0, sizeof(uint32_t), st));
+  const int grid = (int)std::min<size_t>((size_t)sd.sm_count * 4, n_events);
+  const size_t smem = (size_t)lf::HDR_BYTES + (size_t)STATIC_STAGE_CAP * sizeof(float);
+  if (use_wide(*params)) lf::lf_window_kernel<true, true><<<grid, lf::WIN_THREADS, smem, st>>>(consts, A);
+  else lf::lf_window_kernel<true, false><<<grid, lf::WIN_THREADS, smem, st>>>(consts, A);
+  LF_CUDA(nullptr, cudaGetLastError());
+  return LF_OK;
+}
