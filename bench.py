@@ -126,22 +126,94 @@ def source_sha256() -> str:
     return h.hexdigest()
 
 
-# Algorithmic work model ("Algorithmic lane-operations"): lane-operations (one fp32 / int32 ALU
-# operation on one lane) the interval-search formulation of the method needs per work item, at 100 % lane use.
-LANE_OPS = {
-    "per_row": 70,              # a1: extrapolation, 12 layer centres and y positions
-    "per_row_layer_fixed": 10,  # a2: window edges and cap
-    "per_search_step": 2,       # compare + index update of one binary-search step
-    "per_h0_hit": 10,           # a3: bounds of the h2 interval of one h0 hit (+ two searches over <= n_window hits)
-    "per_doublet": 16,          # a3: both filters + x1_expected (+ one closest-hit search in the h1 window)
-    "closest_fixed": 6,         # neighbour compare of a closest-hit search
-    "per_triplet_passing": 12,  # a3: key + insertion into the n smallest
-    "per_triplet_kept": 15,     # a4: parabola through the triplet (+ 9 predictions and closest-hit searches)
-    "per_prediction": 6,        # a4/a5: expected coordinate on one layer
-    "per_accepted": 331,        # a6: residuals, both least-squares fits, chi2 sums, Q
-    "per_track": 60,            # a6/a7: Eq. (9), state, 20-word record moved once
-    "per_seed": 2,              # a7: flag + scan
+# Algorithmic work model ("Algorithmic lane-operations"): lane-operations (one fp32 / int32 add,
+# multiply, divide, abs, min / max, compare or select on one lane) that the canonical arithmetic of DESIGN.md section 3 needs
+# per work item in the interval-search formulation of the method, at 100 % lane use.  Every coefficient is the sum of the
+# terms below, one per expression of section 3; DESIGN.md carries the same table and tests/test_bench_contract.py pins the
+# two to each other.  Loads, address arithmetic, packing of the library's tables and the work of mapping items to lanes
+# are not counted: they belong to an implementation, not to the method.
+LANE_OPS_TERMS = {
+    "per_row": {                        # a1, once per followed track
+        "aq = max(|qop|, 1e-6); p = 1/aq": 3,
+        "x_mag = x + tx*(z_mag - z_seed)": 2,
+        "txp = tx + kick*qop": 2,
+        "xc_l = x_mag + txp*dzm_l on 12 layers": 24,
+        "y_l = y + ty*dzs_l on the 6 u/v layers": 12,
+        "yt_l = y_l*tan(alpha_l) on the 6 u/v layers": 6,
+        "zone = (ty >= 0)": 1,
+        "x_tol = xtol_base + xtol_inv_p*aq": 2,
+        "a_left, a_right from sign(q) = polarity": 3,
+    },
+    "per_row_layer_fixed": {            # a2, once per (followed track, layer), besides the searches
+        "lo = (xc - x_tol) - a_left; hi = (xc + x_tol) + a_right": 4,
+        "mid = (lo + hi)*0.5": 2,
+        "last - first > n_window": 2,
+        "first = max(first, c - n/2); last = min(last, c + n/2)": 4,
+    },
+    "per_search_step": {                # every binary search
+        "compare the probed hit": 1,
+        "select the new position": 1,
+    },
+    "per_h0_hit": {                     # a3, once per hit of the first layer's window: the h2 interval filter 2 allows
+        "d = x_mag - x0": 1,
+        "largest |t| a doublet of this h0 can have": 2,
+        "tol = min(mag_tol_max, c_seed + mag_tol_tx*|t|)": 3,
+        "lo2 = x0 + (d - tol)*inv_r": 3,
+        "hi2 = x0 + (d + tol)*inv_r": 3,
+    },
+    "per_doublet": {                    # a3, once per doublet that passes both filters
+        "t = (x2 - x0)*inv_dz": 2,
+        "filter 1: (t - tx)*(kick*qop) > 0": 3,
+        "filter 2: |x0 + t*zmag_a - x_mag|": 4,
+        "filter 2: < min(mag_tol_max, c_seed + mag_tol_tx*|t|)": 5,
+        "x1e = z_b*t + (x0 - t*z_a)*K": 5,
+        "(x1 - x1e)^2 < T_triplet": 3,
+    },
+    "closest_fixed": {                  # every closest-hit search, after its binary search
+        "pred - x_left; x_right - pred": 2,
+        "compare (ties -> lower index)": 1,
+        "select hit and distance": 2,
+        "index of the hit": 1,
+    },
+    "per_triplet_passing": {            # a3, once per triplet below the chi2 cut
+        "key (chi2, set, h0, h2)": 4,
+        "position among the n smallest: ceil(log2(12 + 1)) = 4 steps": 8,
+    },
+    "per_triplet_kept": {               # a4, once per triplet extended
+        "X10 = x1 - x0; X20 = x2 - x0": 2,
+        "c0 = (X20*D10 - X10*D20)*inv_det": 4,
+        "t0 = (X10 - c0*W10)*inv_D10": 3,
+        "a0 = (x0 - t0*d_a) - c0*w_a": 4,
+    },
+    "per_prediction": {                 # a4 / a5, once per (candidate, other layer)
+        "pred = (a0 + t0*d_l) + c0*w_l": 4,
+        "+ yt_l (u/v layers)": 1,
+        "dist^2 < T_x or T_uv": 2,
+    },
+    "per_accepted": {                   # a6, once per candidate that passed the hit-count rule (12 hits, 6 of them u/v)
+        "r_l = (s_l - yt_l) - ((a0 + t0*d_l) + c0*w_l): 6 u/v x 6 + 6 x x 5": 66,
+        "Sr, Sdr, Swr over 12 hits (the geometry sums come from the per-mask table)": 60,
+        "da, dt, dc = ((C.0*Sr + C.1*Sdr) + C.2*Swr)*inv_det": 18,
+        "e_l = r_l - ((da + dt*d_l) + dc*w_l) on 12 hits": 60,
+        "Q_x += e_l^2 * (1/T) on 12 hits": 36,
+        "rho_l = e_l*inv_tan_l on 6 u/v hits": 6,
+        "S_rho, S_d_rho over 6 u/v hits": 18,
+        "dy0, dty from the 2x2 system": 8,
+        "|dty*0.001| < T_ty": 3,
+        "Q_y += (rho - (dy0 + dty*d))^2 * (1/T_y) on 6 u/v hits": 36,
+        "Q = (Q_x/(n - 3) + Q_y/(n_uv - 2))*C(n); Q < T_Q; lowest Q of the seed": 12,
+    },
+    "per_track": {                      # a6 / a7, once per output track
+        "dSlope = t*0.001 - tx; q/p = dSlope / F(dSlope), F of degree 4 by Horner": 11,
+        "state x, tx, y, ty at z_state": 13,
+        "20-word record moved to its dense position": 20,
+    },
+    "per_seed": {                       # a7
+        "has-track flag": 1,
+        "scan": 1,
+    },
 }
+LANE_OPS = {k: sum(v.values()) for k, v in LANE_OPS_TERMS.items()}
 
 
 def algorithmic_lane_ops(counters: dict, batch, n_window: int, sides: int) -> dict:
@@ -331,6 +403,7 @@ def run_ours(args):
         local_ms = e0.elapsed_time(e1)
     ktimes = dict(zip(binding.KERNEL_NAMES, lf.kernel_times()))
     lf.set_profiling(False)
+    kernels_per_run = lf.info().kernels_per_run  # what the last timed lf_run enqueued: 4, or 5 when the library packed the fp16 copy
     total_ms, (tot_events, tot_seeds, tot_tracks) = sharding.reduce_job(
         local_ms, [batch.n_events, batch.n_seeds, n_tracks], dev)
     ms_per_step = total_ms / args.steps
@@ -392,15 +465,24 @@ def run_ours(args):
     sides = 2 if no_ut else 1
     kb = kernel_bytes(batch, n_tracks, int(P["n_triplets"]), n_acc, sides=sides, wide=wide)
     dom = max(binding.EVENT_KERNELS, key=lambda k: ktimes[k])
-    achieved = kb[dom] / (ktimes[dom] * 1e-3) / 1e9
+    # achieved = ALGORITHMIC bytes (inputs read once + tracks written once: ~34.9 KB per event) of the
+    # units one launch processes (the whole batch: every kernel is launched once per step on all of it) over the dominant
+    # kernel's live duration.  The library's own tables (window rows, triplet codes, candidate records) are not algorithmic
+    # bytes; the figure that counts them for the one kernel sits beside it as kernel_table_* (all keys flat).
     path_bytes = algorithmic_bytes(batch, n_tracks)
-    path_gbs = path_bytes / (local_ms / args.steps * 1e-3) / 1e9
+    achieved = path_bytes / (ktimes[dom] * 1e-3) / 1e9
+    step_gbs = path_bytes / (local_ms / args.steps * 1e-3) / 1e9
+    table_gbs = kb[dom] / (ktimes[dom] * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": None, "kernel": f"lf_{dom}_kernel", "kernel_ms": ktimes[dom],
-                "algorithmic_bytes_per_launch": kb[dom], "peak_source": peak_src,
-                "whole_path": {"algorithmic_bytes_per_step": path_bytes, "achieved_gbs": path_gbs, "frac_of_measured": path_gbs / peak,
-                               "frac_of_nominal_8TBs": path_gbs / NOMINAL_HBM_GBS},
-                "note": "the path is not HBM-bound (DESIGN.md section 7); this is the fraction BASELINE.json's metric asks for"}
+                "algorithmic_bytes_per_launch": path_bytes, "algorithmic_bytes_per_event": path_bytes / max(batch.n_events, 1),
+                "peak_source": peak_src,
+                # the same bytes over the whole step (all four kernels): what the driver-timed ms_per_step implies
+                "step_achieved": step_gbs, "step_frac": step_gbs / peak, "step_frac_of_nominal_8TBs": step_gbs / NOMINAL_HBM_GBS,
+                # bytes the dominant kernel itself has to touch, its tables included
+                "kernel_table_bytes": kb[dom], "kernel_table_achieved": table_gbs, "kernel_table_frac": table_gbs / peak,
+                "note": "the path is not HBM-bound (DESIGN.md section 7); frac = SURVEY 8(d) algorithmic bytes of the batch / dominant "
+                        "kernel time / measured peak; step_frac = the same bytes / ms_per_step"}
     sm_mhz = float(clocks.get("sm_max_mhz") or 1965.0)
     lane_peak = 148 * 128 * sm_mhz * 1e6
     model = algorithmic_lane_ops(counters, batch, int(P["n_window"]), sides)
@@ -471,8 +553,7 @@ def run_ours(args):
                    "sharding": "events, no data-path collective"},
         "seeds_per_s": tot_seeds / (ms_per_step * 1e-3),
         "tracks_per_s": tot_tracks / (ms_per_step * 1e-3),
-        # kernels_per_run counts the library's own packing kernel of hit_storage = 1; it does not run when the caller packs
-        "e2e": e2e, "gpu_launches": (info.kernels_per_run - (1 if fp16_mode in ("caller", "only") else 0)) * args.steps,
+        "e2e": e2e, "gpu_launches": kernels_per_run * args.steps,
         "clocks": clocks, "roofline": roofline,
         "alu_algorithmic_frac": alu_frac, "issue_utilisation": issue_util, "alu_model": alu_model, "issue_detail": issue_detail,
         "cpu_baseline": cpu,
@@ -502,8 +583,9 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--tuning", choices=["with-ut", "no-ut"], default="with-ut",
                     help="with-ut: BASELINE.json's headline (default); no-ut: the no-UT tuning of PAPER.md:285-325 on the same events")
-    ap.add_argument("--seed-arith", choices=["half2", "fp32"], default="half2",
-                    help="config 2 (fp16 hit storage) only: half2 = pairs of doublets in __half2 (PAPER.md:366), fp32 = one doublet per lane")
+    ap.add_argument("--seed-arith", choices=["half2", "fp32"], default="fp32",
+                    help="config 2 (fp16 hit storage) only: fp32 = one doublet per lane on the decoded fp16 hits (default, the faster "
+                         "one), half2 = pairs of doublets in __half2 (PAPER.md:366; the measured comparison)")
     ap.add_argument("--fp16-input", choices=["library", "caller", "only"], default="library",
                     help="config 2 only: library = lf_run packs the fp32 hits itself (default); caller = the caller hands the packed "
                          "copy next to the fp32 hits; only = the packed copy alone (every stage on fp16: lossy, outside configs[2]'s rule)")
@@ -512,7 +594,37 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
-    return run_reference(args) if args.impl == "reference" else run_ours(args)
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
+    if args.impl == "reference":
+        return run_reference(args)  # the oracle on the host cores: rank 0 alone works, whatever N is
+    if "WORLD_SIZE" in os.environ:   # launched by torchrun: its world size is the number of GPUs
+        if int(os.environ["WORLD_SIZE"]) != args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} under a launcher with WORLD_SIZE={os.environ['WORLD_SIZE']}")
+        return run_ours(args)
+    if args.gpus > 1:
+        return launch_ranks(args.gpus)
+    return run_ours(args)
+
+
+def launch_ranks(n: int) -> int:
+    """`python bench.py --gpus N` without a launcher: start N ranks (one per GPU) of this same command under
+    torch.distributed.run on 127.0.0.1; rank 0 prints the one JSON line with n_gpus = N (each GPU
+    its own events, no data-path collective).  Refuses when fewer than N devices are visible instead of timing fewer GPUs
+    than the line would claim."""
+    import socket
+    import subprocess
+    import torch
+    have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+    if have < n:
+        raise SystemExit(f"bench.py --gpus {n}: only {have} CUDA device(s) visible; one rank per GPU is needed "
+                         "(there is no CPU fallback and no oversubscription)")
+    with socket.socket(socket.AF_INET, socket.SOCK_STREAM) as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.run(cmd).returncode
 
 
 if __name__ == "__main__":

@@ -109,8 +109,11 @@ typedef struct {
   float xtol_poly[8];            /* c0..c7 of Eq. (7), Table 5 */
   float x_overlap;               /* overlap of the LEFT and RIGHT windows of Eq. (8): 5 mm */
   /* read only when hit_storage == 1 */
-  int32_t seed_arith;            /* 0 = the seeding kernel evaluates PAIRS of doublets in __half2 ("two combinations at a time",
-                                    PAPER.md:366); 1 = one doublet per lane in fp32 on the decoded fp16 hits (for comparison) */
+  int32_t seed_arith;            /* 1 = one doublet per lane in fp32 on the decoded fp16 hits: the recommended setting and what the
+                                    repository's parameter sets (datagen.default_params, bench.py) use, because it is the faster of
+                                    the two on B200; 0 = the seeding kernel evaluates PAIRS of doublets in
+                                    __half2 ("two combinations at a time"), kept as the measured comparison.  Both
+                                    pass configs[2]'s rule */
 } lf_params;
 
 /* Input seeds: upstream track states at z_seed, SoA, all events back to back. */
@@ -171,7 +174,9 @@ typedef struct {
 #define LF_N_EVENT_KERNELS 4
 #define LF_N_KERNELS 4 /* kernels one lf_run enqueues = entries of lf_kernel_times */
 typedef struct {
-  int32_t kernels_per_run;       /* kernel launches one lf_run enqueues (4; 5 with hit_storage = 1 when the library packs the hits) */
+  int32_t kernels_per_run;       /* kernel launches the most recent lf_run / lf_run_debug on the handle enqueued (lf_run_host: its
+                                    last chunk): 4; 5 with hit_storage = 1 when the library packed the hits itself (no x16 / origin16
+                                    from the caller); 0 for an empty batch.  Before the first run: the upper bound, 4 + hit_storage */
   int32_t regs[LF_N_EVENT_KERNELS], block[LF_N_EVENT_KERNELS], grid[LF_N_EVENT_KERNELS], ctas_per_sm[LF_N_EVENT_KERNELS];
   int32_t smem_bytes[LF_N_EVENT_KERNELS]; /* dynamic shared memory per CTA */
   int32_t staged_hits_per_event; /* events with more hits than this read hits from global memory */
@@ -230,7 +235,10 @@ lf_status lf_run_host(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
  * work already queued on `cuda_stream`.  The host arrays of `seeds`, `hits` and `out` must stay valid and untouched until the
  * batch has been collected (the structs themselves are copied).  Batches in flight share the handle's workspace, so they must
  * all use the same `cuda_stream` (LF_ERR_INVALID_ARG otherwise); a slot takes a new batch only after its previous one has been
- * collected; lf_run and lf_run_host must not be called while a batch is in flight. */
+ * collected; lf_run and lf_run_host must not be called while a batch is in flight.  An LF_ERR_CUDA from lf_host_submit or
+ * any error from lf_host_collect ABORTS EVERY BATCH IN FLIGHT on the handle: the library waits for its own copy streams and
+ * for the stream each pending batch was submitted on, marks all slots idle (their batches can no longer be collected; the
+ * host output arrays hold unspecified data) and leaves the handle ready for the next lf_run / lf_host_submit. */
 #define LF_HOST_SLOTS 2
 lf_status lf_host_submit(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events,
                          lf_tracks* out, void* cuda_stream, int slot);
@@ -255,7 +263,10 @@ lf_status lf_pack_hits(lf_handle* h, const lf_hits* hits, size_t n_events, uint1
 /* Checks, on the device, the input preconditions lf_run relies on but does not check (see "Conventions"): segment
  * offsets monotone, starting at 0 and ending at n_hits; stored coordinates finite and ascending inside every
  * segment; seed offsets monotone, starting at 0 and ending at n_seeds; seed states finite (q/p only when params.mode
- * == 0).  Arguments as for lf_run (HOST structs holding DEVICE pointers); `out` is not needed.  SYNCHRONOUS: waits
+ * == 0).  With the fp16 copy as the only hit input (hits->x == NULL, hit_storage = 1, x16 + origin16 given) the decoded
+ * coordinates are checked instead: finite, and ascending inside every block of 8 hits (across blocks the encoding may
+ * overlap by a rounding error, which that lossy mode accepts).
+ * Arguments as for lf_run (HOST structs holding DEVICE pointers); `out` is not needed.  SYNCHRONOUS: waits
  * for `cuda_stream`.  Returns LF_OK, or LF_ERR_INVALID_ARG with lf_last_error naming the kind of violation and the
  * index of one offending segment / hit / event / seed.  A debugging aid: not part of the hot path. */
 lf_status lf_validate_inputs(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, size_t n_events, void* cuda_stream);

@@ -93,6 +93,7 @@ struct lf_handle {
   HostBufs hb;
   size_t host_chunk_events = HOST_CHUNK_EVENTS;
   size_t last_events = 0; /* n_events of the most recent launch (lf_run_counters) */
+  int last_kernels = -1;  /* kernels the most recent launch enqueued (lf_get_info); -1 = nothing launched yet */
   bool profiling = false;
   size_t prof_runs = 0;                 /* runs recorded since profiling was enabled */
   cudaEvent_t (*prof_ev)[N_PROF_EV] = nullptr;  /* ring of PROF_RING event sets */
@@ -321,6 +322,7 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
   h->counters_valid = DEBUG;
   h->last_events = n_events;
   const bool work = n_events > 0;
+  int n_kernels = work ? LF_N_KERNELS : 0; /* what this call enqueues (lf_get_info) */
   auto grid_of = [&](int k) { return (int)std::min<size_t>((size_t)h->grid[k], n_events); };
   const bool half_hits = h->P.hit_storage == 1;
   const __half* use16 = nullptr;
@@ -334,6 +336,7 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
         const int pg = (int)std::min<size_t>((size_t)h->sm_count * 8, n_events);
         lf::lf_pack_hits_kernel<<<pg, 256, 0, st>>>(hits->x, hits->seg_offsets, (uint32_t)n_events, (uint32_t)event_base, h->hx16,
                                                     h->origin16);
+        ++n_kernels;
       }
       use16 = h->hx16;
       use_origin = h->origin16;
@@ -385,6 +388,7 @@ lf_status launch_impl(lf_handle* h, const lf_seeds* seeds, const lf_hits* hits, 
   }
   LF_CUDA(h, cudaGetLastError());
   h->tickets_dirty = false;
+  h->last_kernels = n_kernels;
   return LF_OK;
 }
 
@@ -618,7 +622,7 @@ lf_status lf_destroy(lf_handle* h) {
 
 lf_status lf_get_info(const lf_handle* h, lf_info* out) {
   if (!h || !out) return LF_ERR_INVALID_ARG;
-  out->kernels_per_run = LF_N_KERNELS + (h->P.hit_storage == 1 ? 1 : 0);
+  out->kernels_per_run = h->last_kernels >= 0 ? h->last_kernels : LF_N_KERNELS + (h->P.hit_storage == 1 ? 1 : 0);
   const int threads[4] = {h->win_threads, lf::SEED_THREADS, lf::FIT_THREADS, lf::FIT_THREADS};
   for (int k = 0; k < 4; ++k) {
     out->regs[k] = h->regs[k];
@@ -711,7 +715,9 @@ lf_status lf_validate_inputs(lf_handle* h, const lf_seeds* seeds, const lf_hits*
     return fail(h, LF_ERR_INVALID_ARG, "lf_validate_inputs: NULL seeds/hits or offset table");
   if (seeds->n_seeds > 0 && (!seeds->x || !seeds->y || !seeds->tx || !seeds->ty || (!seeds->qop && h->P.mode == 0)))
     return fail(h, LF_ERR_INVALID_ARG, "lf_validate_inputs: NULL seed array");
-  if (hits->n_hits > 0 && !hits->x) return fail(h, LF_ERR_INVALID_ARG, "lf_validate_inputs: NULL hit array");
+  const bool only16 = !hits->x && h->P.hit_storage == 1 && hits->x16 && hits->origin16; /* the fp16 copy is the only input */
+  if (hits->n_hits > 0 && !hits->x && !only16)
+    return fail(h, LF_ERR_INVALID_ARG, "lf_validate_inputs: NULL hit array (x may be NULL only with hit_storage = 1 and x16 + origin16 given)");
   if (n_events > h->max_events || seeds->n_seeds > h->max_seeds || hits->n_hits > h->max_hits)
     return fail(h, LF_ERR_CAPACITY, "lf_validate_inputs: batch exceeds the maxima given to lf_create");
   h->err.clear();
@@ -720,7 +726,8 @@ lf_status lf_validate_inputs(lf_handle* h, const lf_seeds* seeds, const lf_hits*
   LF_CUDA(h, cudaMemsetAsync(res, 0, sizeof(uint32_t), st));
   LF_CUDA(h, cudaMemsetAsync(res + 1, 0xFF, 3 * sizeof(uint32_t), st));
   const int blocks = std::max(1, std::min<int>(h->sm_count * 8, (int)((n_events * lf::NSEG + 7) / 8) + 1));
-  lf::lf_validate_kernel<<<blocks, 256, 0, st>>>(hits->x, hits->seg_offsets, (uint32_t)n_events, (uint32_t)hits->n_hits,
+  lf::lf_validate_kernel<<<blocks, 256, 0, st>>>(hits->x, only16 ? reinterpret_cast<const __half*>(hits->x16) : nullptr,
+                                               only16 ? hits->origin16 : nullptr, hits->seg_offsets, (uint32_t)n_events, (uint32_t)hits->n_hits,
                                                seeds->event_offsets, (uint32_t)seeds->n_seeds, seeds->x, seeds->y, seeds->tx,
                                                seeds->ty, h->P.mode == 0 ? seeds->qop : nullptr, res);
   LF_CUDA(h, cudaGetLastError());
@@ -771,7 +778,12 @@ static void host_drain(lf_handle* h, void* cuda_stream) {
   if (hb.s_h2d) cudaStreamSynchronize(hb.s_h2d);
   if (hb.s_cnt) cudaStreamSynchronize(hb.s_cnt);
   if (hb.s_d2h) cudaStreamSynchronize(hb.s_d2h);
-  cudaStreamSynchronize((cudaStream_t)cuda_stream);
+  /* An error aborts EVERY batch in flight on the handle (include/lf.h): the kernels of each of them run on the stream it
+   * was submitted on, which need not be `cuda_stream` (lf_host_collect has none to pass), so wait for those streams
+   * before the slots are marked idle and the workspace is handed to the next lf_run. */
+  for (HostSlot& b : hb.slot)
+    if (b.pending) cudaStreamSynchronize(b.st);
+  if (cuda_stream) cudaStreamSynchronize((cudaStream_t)cuda_stream);
   for (HostSlot& b : hb.slot) b.pending = false;
 }
 
@@ -832,37 +844,43 @@ static lf_status host_submit(lf_handle* h, int slot, const lf_seeds* seeds, cons
   b.pending = true;
   if (n_events == 0) return LF_OK;
   const bool packed = h->P.hit_storage == 1 && hits->x16 && hits->origin16; /* the caller ships the fp16 copy */
-  if (!hb.s_h2d) {
-    LF_CUDA(h, cudaStreamCreateWithFlags(&hb.s_h2d, cudaStreamNonBlocking));
-    LF_CUDA(h, cudaStreamCreateWithFlags(&hb.s_cnt, cudaStreamNonBlocking));
-    LF_CUDA(h, cudaStreamCreateWithFlags(&hb.s_d2h, cudaStreamNonBlocking));
-  }
+  if (!hb.s_h2d) LF_CUDA(h, cudaStreamCreateWithFlags(&hb.s_h2d, cudaStreamNonBlocking));
+  if (!hb.s_cnt) LF_CUDA(h, cudaStreamCreateWithFlags(&hb.s_cnt, cudaStreamNonBlocking));
+  if (!hb.s_d2h) LF_CUDA(h, cudaStreamCreateWithFlags(&hb.s_d2h, cudaStreamNonBlocking));
   if (!b.ready) {
+    /* First use of the slot.  Every member is allocated only while it is still null, so that a submit that ran out of
+     * memory part-way leaks nothing: the next one completes the set (and lf_destroy frees whatever exists). */
     const size_t ns = std::max<size_t>(h->max_seeds, 1), ne = std::max<size_t>(h->max_events, 1);
     const size_t nh = std::max<size_t>(h->max_hits, 1);
-    LF_CUDA(h, cudaMalloc(&b.seeds, 5 * ns * sizeof(float)));
-    LF_CUDA(h, cudaMalloc(&b.seed_off, (ne + 1) * sizeof(uint32_t)));
-    LF_CUDA(h, cudaMalloc(&b.hits, nh * sizeof(float)));
+#define LF_SLOT_ALLOC(member, bytes) \
+    do { if (!(member)) LF_CUDA(h, cudaMalloc(&(member), (bytes))); } while (0)
+#define LF_SLOT_EVENT(member) \
+    do { if (!(member)) LF_CUDA(h, cudaEventCreateWithFlags(&(member), cudaEventDisableTiming)); } while (0)
+    LF_SLOT_ALLOC(b.seeds, 5 * ns * sizeof(float));
+    LF_SLOT_ALLOC(b.seed_off, (ne + 1) * sizeof(uint32_t));
+    LF_SLOT_ALLOC(b.hits, nh * sizeof(float));
     if (h->P.hit_storage == 1) {
-      LF_CUDA(h, cudaMalloc(&b.hits16, nh * sizeof(uint16_t)));
-      LF_CUDA(h, cudaMalloc(&b.origin16, lf_origin_slots(ne, nh) * sizeof(float)));
+      LF_SLOT_ALLOC(b.hits16, nh * sizeof(uint16_t));
+      LF_SLOT_ALLOC(b.origin16, lf_origin_slots(ne, nh) * sizeof(float));
     }
-    LF_CUDA(h, cudaMalloc(&b.seg_off, (ne * lf::NSEG + 1) * sizeof(uint32_t)));
-    LF_CUDA(h, cudaMalloc(&b.hit_idx, ns * lf::NL * sizeof(int32_t)));
-    LF_CUDA(h, cudaMalloc(&b.seed_idx, ns * sizeof(int32_t)));
-    LF_CUDA(h, cudaMalloc(&b.n_hits, ns * sizeof(int32_t)));
-    LF_CUDA(h, cudaMalloc(&b.state, ns * 5 * sizeof(float)));
-    LF_CUDA(h, cudaMalloc(&b.quality, ns * sizeof(float)));
-    LF_CUDA(h, cudaMalloc(&b.ev_off, (ne + HOST_MAX_CHUNKS + 1) * sizeof(uint32_t)));
-    LF_CUDA(h, cudaMalloc(&b.n_tracks, HOST_MAX_CHUNKS * sizeof(uint32_t)));
-    LF_CUDA(h, cudaMallocHost(&b.pinned_count, (ne + 2 * HOST_MAX_CHUNKS + 1) * sizeof(uint32_t)));
-    LF_CUDA(h, cudaEventCreateWithFlags(&b.ev_start, cudaEventDisableTiming));
-    LF_CUDA(h, cudaEventCreateWithFlags(&b.ev_done, cudaEventDisableTiming));
+    LF_SLOT_ALLOC(b.seg_off, (ne * lf::NSEG + 1) * sizeof(uint32_t));
+    LF_SLOT_ALLOC(b.hit_idx, ns * lf::NL * sizeof(int32_t));
+    LF_SLOT_ALLOC(b.seed_idx, ns * sizeof(int32_t));
+    LF_SLOT_ALLOC(b.n_hits, ns * sizeof(int32_t));
+    LF_SLOT_ALLOC(b.state, ns * 5 * sizeof(float));
+    LF_SLOT_ALLOC(b.quality, ns * sizeof(float));
+    LF_SLOT_ALLOC(b.ev_off, (ne + HOST_MAX_CHUNKS + 1) * sizeof(uint32_t));
+    LF_SLOT_ALLOC(b.n_tracks, HOST_MAX_CHUNKS * sizeof(uint32_t));
+    if (!b.pinned_count) LF_CUDA(h, cudaMallocHost(&b.pinned_count, (ne + 2 * HOST_MAX_CHUNKS + 1) * sizeof(uint32_t)));
+    LF_SLOT_EVENT(b.ev_start);
+    LF_SLOT_EVENT(b.ev_done);
     for (int c = 0; c < HOST_MAX_CHUNKS; ++c) {
-      LF_CUDA(h, cudaEventCreateWithFlags(&b.ev_h2d[c], cudaEventDisableTiming));
-      LF_CUDA(h, cudaEventCreateWithFlags(&b.ev_comp[c], cudaEventDisableTiming));
-      LF_CUDA(h, cudaEventCreateWithFlags(&b.ev_cnt[c], cudaEventDisableTiming));
+      LF_SLOT_EVENT(b.ev_h2d[c]);
+      LF_SLOT_EVENT(b.ev_comp[c]);
+      LF_SLOT_EVENT(b.ev_cnt[c]);
     }
+#undef LF_SLOT_ALLOC
+#undef LF_SLOT_EVENT
     b.ready = true;
   }
   const size_t stride = std::max<size_t>(h->max_seeds, 1);

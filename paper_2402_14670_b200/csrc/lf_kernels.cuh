@@ -2207,7 +2207,8 @@ __global__ void __launch_bounds__(256) lf_pack_hits_kernel(const float* __restri
  * (event, layer, zone) segment, grid-stride; result[0] = OR of the violation bits, result[1..3] = smallest index of
  * a violation of each kind (segment / hit / event-or-seed), preset to 0xFFFFFFFF by the caller. */
 constexpr uint32_t BAD_SEG_OFFSETS = 1u, BAD_HIT_ORDER = 2u, BAD_SEED_OFFSETS = 4u, BAD_SEED_VALUE = 8u, BAD_HIT_VALUE = 16u;
-__global__ void __launch_bounds__(256) lf_validate_kernel(const float* __restrict__ hx, const uint32_t* __restrict__ seg_off,
+__global__ void __launch_bounds__(256) lf_validate_kernel(const float* __restrict__ hx, const __half* __restrict__ hx16,
+                                                          const float* __restrict__ origin16, const uint32_t* __restrict__ seg_off,
                                                           uint32_t n_events, uint32_t n_hits, const uint32_t* __restrict__ seed_off,
                                                           uint32_t n_seeds, const float* __restrict__ sx, const float* __restrict__ sy,
                                                           const float* __restrict__ stx, const float* __restrict__ sty,
@@ -2221,10 +2222,27 @@ __global__ void __launch_bounds__(256) lf_validate_kernel(const float* __restric
       if (lane == 0) { atomicOr(result, BAD_SEG_OFFSETS); atomicMin(result + 1, sg); }
       continue;
     }
-    for (uint32_t i = a + lane; i < e; i += 32u) {
-      const float v = hx[i];
-      if (!isfinite(v)) { atomicOr(result, BAD_HIT_VALUE); atomicMin(result + 2, i); }
-      if (i + 1 < e && !(v <= hx[i + 1])) { atomicOr(result, BAD_HIT_ORDER); atomicMin(result + 2, i); }
+    if (hx != nullptr) {
+      for (uint32_t i = a + lane; i < e; i += 32u) {
+        const float v = hx[i];
+        if (!isfinite(v)) { atomicOr(result, BAD_HIT_VALUE); atomicMin(result + 2, i); }
+        if (i + 1 < e && !(v <= hx[i + 1])) { atomicOr(result, BAD_HIT_ORDER); atomicMin(result + 2, i); }
+      }
+    } else {
+      /* fp16-only input (lf_hits.x == NULL): the hits as the kernels decode them, origin of the block of 8 + half offset.
+       * Rounding is monotone under one origin, so ascending fp32 hits stay ascending inside a block; neighbouring blocks
+       * have different origins and may overlap by a rounding error, which the lossy mode accepts: the order is checked
+       * inside blocks only. */
+      const uint32_t slot0 = (a >> H16_SHIFT) + sg;
+      for (uint32_t i = a + lane; i < e; i += 32u) {
+        const uint32_t k = i - a;
+        const float v = origin16[slot0 + (k >> H16_SHIFT)] + __half2float(hx16[i]);
+        if (!isfinite(v)) { atomicOr(result, BAD_HIT_VALUE); atomicMin(result + 2, i); }
+        if (i + 1 < e && ((k + 1u) >> H16_SHIFT) == (k >> H16_SHIFT) && !(__half2float(hx16[i]) <= __half2float(hx16[i + 1]))) {
+          atomicOr(result, BAD_HIT_ORDER);
+          atomicMin(result + 2, i);
+        }
+      }
     }
   }
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, n_thr = gridDim.x * blockDim.x;

@@ -109,7 +109,8 @@ def default_params() -> Dict[str, object]:
         "mode": 0, "velo_p_min": 5.0, "velo_pt_min": 1.0,
         "xtol_poly": [4824.3, 426.3, 7071.1, 12080.4, 14077.8, 13909.3, 9315.3, 3209.5],  # Table 5
         "x_overlap": 5.0,
-        "seed_arith": 0,  # hit_storage = 1 only: 0 = pairs of doublets in __half2, 1 = fp32 per doublet
+        "seed_arith": 1,  # hit_storage = 1 only: 1 = fp32 per doublet on the decoded fp16 hits (default: the faster one, DESIGN.md
+                          # section 7b), 0 = pairs of doublets in __half2 (kept as the comparison)
     }
 
 

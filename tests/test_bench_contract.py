@@ -48,6 +48,20 @@ def test_gpu_arm_line(tuning):
     # "traffic" and "issue_utilisation" must be null, never a stale number
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and 0 < r["frac"] < 1 and r["achieved"] > 0 and r["peak"] > 0
     assert r["traffic"] is None and r["algorithmic_bytes_per_launch"] > 0 and d["issue_utilisation"] is None
+    # frac is SURVEY.md section 8(d)'s fraction, reproducible by hand from flat keys of the line: the batch's algorithmic bytes
+    # (inputs once + 80 bytes per track + offsets) over the dominant kernel's live time; step_frac = the same bytes over
+    # ms_per_step; the figure that also counts the library's tables is kept apart as kernel_table_*
+    cfg = d["config"]
+    by_hand = (4 * cfg["hits_per_gpu"] + 20 * cfg["seeds_per_gpu"] + 80 * cfg["tracks_per_step_per_gpu"]
+               + 4 * (cfg["events_per_gpu"] * 24 + 1) + 4 * (cfg["events_per_gpu"] + 1) + 4 * (cfg["events_per_gpu"] + 1) + 4)
+    assert r["algorithmic_bytes_per_launch"] == by_hand
+    dom_ms = d["kernels"]["ms"][r["kernel"][3:-7]]
+    assert dom_ms == max(d["kernels"]["ms"].values()) == r["kernel_ms"]
+    assert abs(r["achieved"] - by_hand / (dom_ms * 1e-3) / 1e9) < 1e-6 * r["achieved"]
+    assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
+    assert abs(r["step_frac"] - by_hand / (d["ms_per_step"] * 1e-3) / 1e9 / r["peak"]) < 1e-6 * r["step_frac"]
+    assert r["step_frac"] < r["frac"] and r["kernel_table_bytes"] > 0 and r["kernel_table_frac"] > 0
+    assert not any(isinstance(v, dict) for v in r.values()), "the driver keeps flat roofline keys only"
     # the algorithmic ALU fraction comes from the committed model evaluated on this batch's own work counters
     assert 0 < d["alu_algorithmic_frac"] < 1
     c = d["alu_model"]["counters"]
@@ -86,3 +100,57 @@ def test_gpu_arm_under_torchrun():
     # whole-job aggregate: the units all ranks processed over the max-over-ranks time
     assert abs(d["value"] - n * 600 / (d["ms_per_step"] * 1e-3)) / d["value"] < 1e-6
     assert d["e2e"]["value"] > 0 and d["gpu_launches"] == 4 * 3
+
+
+def test_lane_ops_table_matches_design():
+    """The coefficients of the algorithmic work model (alu_algorithmic_frac) are derived, expression by expression, in
+    DESIGN.md section 7.2; bench.LANE_OPS_TERMS must hold exactly that table, and LANE_OPS its row sums."""
+    import re
+    sys.path.insert(0, ROOT)
+    import bench
+    text = open(os.path.join(ROOT, "DESIGN.md")).read()
+    body = text[text.index("<!-- LANE_OPS derivation begin -->"):text.index("<!-- LANE_OPS derivation end -->")]
+    terms, totals = {}, {}
+    for line in body.splitlines():
+        m = re.match(r"^\| `(\w+)` \| (.*) \| \**(\d+)\** \|$", line)
+        if not m:
+            continue
+        key, what, n = m.group(1), m.group(2).replace("\\|", "|"), int(m.group(3))
+        if what.startswith("**total per"):
+            totals[key] = n
+        else:
+            assert what not in terms.setdefault(key, {}), f"duplicate row {what!r}"
+            terms[key][what] = n
+    assert terms == bench.LANE_OPS_TERMS
+    assert totals == bench.LANE_OPS == {k: sum(v.values()) for k, v in terms.items()}
+    # the model uses every coefficient, and only these
+    src = open(os.path.join(ROOT, "bench.py")).read()
+    used = set(re.findall(r'L\["(\w+)"\]', src))
+    assert used == set(bench.LANE_OPS)
+
+
+def test_gpus_n_without_a_launcher_needs_n_devices():
+    """`python bench.py --gpus N` starts its own N ranks (torch.distributed.run); with fewer than N visible devices it
+    refuses loudly instead of timing one GPU and printing n_gpus: 1.  The reference arm needs no GPU at any N."""
+    import torch
+    have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+    n = have + 1 if have >= 1 else 2
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", str(n), "--steps", "1", "--warmup", "3"],
+                         capture_output=True, text=True, timeout=300, cwd=ROOT)
+    assert res.returncode != 0 and not res.stdout.strip()
+    assert f"--gpus {n}: only {have} CUDA device(s) visible" in res.stderr
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "3"],
+                         capture_output=True, text=True, timeout=300, cwd=ROOT, env=dict(os.environ, WORLD_SIZE="3", RANK="0"))
+    assert res.returncode != 0 and "WORLD_SIZE=3" in res.stderr
+    d = _run(["--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0", "--events", "60"])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0
+
+
+@pytest.mark.gpu
+def test_gpus_n_self_launch():
+    """With two devices visible `python bench.py --gpus 2` (no torchrun around it) prints one line with n_gpus: 2."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("one GPU on this box: the refusal is covered by test_gpus_n_without_a_launcher_needs_n_devices")
+    d = _run(["--gpus", "2", "--steps", "3", "--warmup", "3", "--events", "600", "--no-cpu-baseline"])
+    assert d["n_gpus"] == 2 and d["config"]["events_per_gpu"] == 600 and d["value"] > 0

@@ -440,6 +440,7 @@ def test_config2_packed_input_and_fp16_only(lfmod, oracle, geometry, params):
     a = lf.run(db)
     torch.cuda.synchronize()
     a = a.to_numpy()
+    assert lf.info().kernels_per_run == 5       # the library packed the fp16 copy itself: one more kernel
     lf.pack_hits(db)
     # the packed copy follows the documented encoding: hit = origin(block) + half; the error is half an fp16 ulp of the
     # offset to the block origin (<= 0.125 mm for offsets below 512 mm, <= 0.25 mm below 1024 mm)
@@ -453,9 +454,26 @@ def test_config2_packed_input_and_fp16_only(lfmod, oracle, geometry, params):
     c = lf.run(db)          # x and x16 given: windows + seeding on the caller's copy, extension + fit on fp32
     torch.cuda.synchronize()
     c = c.to_numpy()
+    assert lf.info().kernels_per_run == 4       # the caller's copy: nothing to pack (lf_get_info reports the last launch)
     assert c.n_tracks == a.n_tracks and np.array_equal(c.hit_idx, a.hit_idx) and np.array_equal(c.state.view(np.uint32), a.state.view(np.uint32))
     _rule_config2(b, c, ref, "fp16 windows+seeding, fp32 extension+fit")
     db.drop_fp32()          # fp16 only
+    # lf_validate_inputs checks the fp16-only input as the kernels decode it: finite, ascending inside every block of 8
+    lf.validate_inputs(db)
+    s0 = int(b.seg_offsets[7])
+    assert int(b.seg_offsets[8]) - s0 >= 8
+    keep16, keep_org = db.hit_x16.clone(), db.origin16.clone()
+    db.hit_x16[s0 + 1], db.hit_x16[s0 + 2] = keep16[s0 + 2] + 1.0, keep16[s0 + 1]
+    with pytest.raises(lfmod.LfError) as ei:
+        lf.validate_inputs(db)
+    assert "not ascending" in str(ei.value) and f"hit {s0 + 1})" in str(ei.value), str(ei.value)
+    db.hit_x16.copy_(keep16)
+    db.origin16[(s0 >> 3) + 7] = float("inf")
+    with pytest.raises(lfmod.LfError) as ei:
+        lf.validate_inputs(db)
+    assert "non-finite hit" in str(ei.value), str(ei.value)
+    db.origin16.copy_(keep_org)
+    lf.validate_inputs(db)
     d = lf.run(db)
     torch.cuda.synchronize()
     d = d.to_numpy()

@@ -81,9 +81,12 @@ def test_noUT_config1_stage_boundaries_subset(lfmod, oracle, geometry, nparams):
     _both(lfmod, oracle, geometry, nparams, dg.generate_config(1, n_events=100), "no-UT config 1 subset")
 
 
-def test_noUT_config4_subset(lfmod, oracle, geometry, nparams):
-    """High occupancy (about 500 hits per segment): the 64-hit cap binds often."""
-    b = dg.generate_config(4, n_events=600)
+def test_noUT_config4_full_size(lfmod, oracle, geometry, nparams):
+    """High occupancy (about 500 hits per segment): the 64-hit cap binds often.  All 5 000 events of BASELINE.json
+    configs[4] in one lf_run, element by element: the workload whose no-UT time DESIGN.md section 7.1 quotes; the stage
+    boundaries on a 40-event subset."""
+    b = dg.generate_config(4)
+    assert b.n_events == 5000
     info, ref = _both(lfmod, oracle, geometry, nparams, b, "no-UT config 4", debug=False)
     b2 = dg.generate_config(4, n_events=40)
     info2, ref2 = _both(lfmod, oracle, geometry, nparams, b2, "no-UT config 4 subset")
